@@ -1,0 +1,157 @@
+/*
+ * gbe.h - C ABI of the B200-native graph-based electronic-structure hot path
+ *         (arXiv:1603.00937, "Graph-based linear scaling electronic structure theory").
+ *
+ * What the library computes (citations: P:Lnn = line nn of the paper text; A-n = reading n in DESIGN.md 3):
+ *
+ *   P_tau(H): the thresholded matrix polynomial of Eq.(4), evaluated by the partitioned
+ *   subgraph expansion of Eq.(6) P:L58-63.  For every community p (obs. (vi) P:L65) the core vertices and
+ *   all halo vertices directly connected to them in the data-dependency graph S_tau (Eq.(2) P:L38-40,
+ *   Fig.1) induce a dense principal submatrix x[s_p].  The polynomial is the recursive
+ *   second-order zero-temperature Fermi-operator expansion ("SP2"):
+ *   X <- X^2 or 2X - X^2, the SAME sequence for every subgraph ("the same for each subgraph expansion",
+ *   P:L90), chosen on the device from the trace summed over all core diagonals.  The core columns are
+ *   collected into the sparse, non-symmetric density matrix D = P_tau(H) (obs. (i) P:L65).
+ *
+ * Conventions
+ *   - All functions return 0 (GBE_OK) or a negative gbe_status.  No exceptions, no aborts, no stdout.
+ *   - "device" pointers are CUDA device memory of the current device; "host" pointers are ordinary host
+ *     memory.  Inputs are borrowed for the duration of the call (device inputs: until the work enqueued on
+ *     `cuda_stream` has finished); the library never frees caller memory.  Outputs and the workspace are
+ *     caller-allocated; the only library allocation is the graph handle (freed by gbe_free_graph).
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - gbe_build_graph synchronises the stream (it sizes its outputs).  gbe_density and the three phase calls
+ *     only enqueue work: no host round trip between SP2 iterations; they return before completion.
+ *   - CSR: row_ptr int64 [n+1], col_idx int32 [nnz] ascending within a row, val double [nnz]; 0-based.
+ */
+#ifndef GBE_H
+#define GBE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  GBE_OK = 0,
+  GBE_EINVAL = -1,      /* null pointer, n <= 0, tau < 0 or NaN, n_occ outside [0,n], iters outside [0,GBE_MAX_ITERS],
+                           partition id out of range, power outside [1,GBE_MAX_POWER], n above the supported size */
+  GBE_ENOTSYM = -2,     /* H is not symmetric (pattern or values); only tested when opts.check_symmetry != 0 */
+  GBE_EDEGENERATE = -3, /* eps_max == eps_min: the spectrum cannot be mapped to [0,1] (A-12) */
+  GBE_EMISMATCH = -4,   /* H.n differs from the graph's n */
+  GBE_ENOMEM = -5,      /* workspace too small (required size: gbe_graph_info.workspace_bytes) or allocation failed */
+  GBE_ECUDA = -6        /* a CUDA call failed; text via gbe_strerror / gbe_last_cuda_error */
+} gbe_status;
+
+#define GBE_MAX_ITERS 1024
+#define GBE_MAX_POWER 8
+
+/* Sparse symmetric matrix in CSR (the Hamiltonian H).  DEVICE pointers, borrowed. */
+typedef struct {
+  int64_t n;
+  int64_t nnz;
+  const int64_t* row_ptr; /* n+1 */
+  const int32_t* col_idx; /* nnz, ascending within a row */
+  const double* val;      /* nnz */
+} gbe_csr_view;
+
+/* Opaque, library-owned, immutable after gbe_build_graph: S_tau, the communities, their core+halo index
+ * lists, the padded batched dense layout, the pattern of D and the scatter map, the tile work list. */
+typedef struct gbe_graph gbe_graph;
+
+typedef struct {
+  double tau;             /* threshold of Eq.(2), applied to magnitudes (A-3), on the normalised X0 (A-1) */
+  int32_t power;          /* highest thresholded power T^(n) entering S_tau (A-1); 0 -> default 2 */
+  int32_t check_symmetry; /* != 0: verify H == H^T (pattern and values) and fail with GBE_ENOTSYM otherwise */
+} gbe_graph_opts;
+
+typedef struct {
+  int64_t n;          /* vertices = orbitals = rows of H */
+  int64_t nnz_S;      /* edges of S_tau incl. self loops (directed count) */
+  int64_t n_part;     /* communities */
+  int64_t sum_m;      /* sum over communities of m_p = core + halo size */
+  int64_t max_m;      /* largest m_p */
+  int64_t nnz_D;      /* stored entries of D = sum_p m_p * ncore_p */
+  int64_t dense_elems;/* doubles in ONE batched dense buffer = sum_p m_p * ld_p (ld_p = m_p rounded up to 16) */
+  int64_t n_tiles;    /* X^2 work items per SP2 iteration (upper-triangle tiles over all communities) */
+  double sp2_flops_per_iter; /* sum_p 2 m_p^3: algorithmic flops of one SP2 iteration (unpadded, no symmetry) */
+  double eps_min, eps_max;   /* Gershgorin bounds of the H given to gbe_build_graph (A-5) */
+  int32_t contiguous_cores;  /* 1: every core is a contiguous index range (fast scatter); 0: per-entry map */
+  int32_t tile;              /* edge of the square X^2 tile chosen for this graph */
+  size_t workspace_bytes;    /* device workspace gbe_density needs (two dense buffers + state + partials) */
+} gbe_graph_info;
+
+/* SP2 log (host memory, caller-allocated; valid after the stream has been synchronised).
+ * t1[k] = sum_p sum_{i<ncore_p} (X_k)_ii, t2[k] = same for X_k^2, k = 0..iters_done;
+ * branch[k] = 0 (X <- X^2) or 1 (X <- 2X - X^2), k = 0..iters_done-1 (A-6). */
+typedef struct {
+  int32_t iters_done;
+  uint8_t* branch; /* >= iters entries */
+  double* t1;      /* >= iters + 1 entries */
+  double* t2;      /* >= iters + 1 entries */
+} gbe_sp2_log;
+
+/* Steps 0-2 of the path: Gershgorin bounds of H, the graph
+ *     S_tau = I u pat(A) u pat(floor(A A)_tau) [u ... up to `power`], A = floor((eps_max I - H)/(eps_max-eps_min))_tau,
+ * symmetrised (reading A-1 of Eq.(2) P:L38-40 / Eq.(8)), then for every community p its subgraph
+ *     s_p = C_p u { k : (k,i) in S_tau, i in C_p }            (local order: core ascending, halo ascending)
+ * and the pattern S' of D (A-9).
+ *   H     device CSR, symmetric.
+ *   part  device int32[n], vertex -> community id in [0, n_part); every vertex lies in exactly one core;
+ *         empty communities are allowed.  NULL: contiguous blocks of ceil(n / n_part) rows.
+ *         (The paper's partitioner, METIS P:L78, is outside the library.)
+ *   out   receives the handle.  Synchronises `cuda_stream`. */
+int gbe_build_graph(const gbe_csr_view* H, const gbe_graph_opts* opts, const int32_t* part, int32_t n_part,
+                    void* cuda_stream, gbe_graph** out);
+
+int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* out);
+
+/* Copies the graph to caller-allocated DEVICE buffers (any may be NULL to skip), sizes from gbe_graph_info:
+ * S_row_ptr[n+1], S_col[nnz_S], sub_ptr[n_part+1], sub_idx[sum_m], ncore[n_part], D_row_ptr[n+1], D_col[nnz_D]. */
+int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, int32_t* S_col, int64_t* sub_ptr,
+                     int32_t* sub_idx, int32_t* ncore, int64_t* D_row_ptr, int32_t* D_col);
+
+/* Steps 0 and 3-6: D = P_tau(H) on the pattern fixed by the graph (Eq.(6)).
+ *   H         device CSR; values AND pattern may differ from the H the graph was built from (MD use):
+ *             H values are looked up at gather time, entries outside a subgraph are simply not gathered.
+ *             The Gershgorin bounds are recomputed from this H.
+ *   n_occ     target occupation (number of occupied orbitals), 0 <= n_occ <= n.
+ *   iters     SP2 iterations (fixed count when idem_tol < 0).
+ *   idem_tol  >= 0: stop before iteration k >= 1 once |t1[k] - t2[k]| <= idem_tol (A-7); < 0: never stop early.
+ *   workspace device memory, >= info.workspace_bytes, 256-byte aligned; contents are scratch.
+ *   D_val     device double[nnz_D], CSR order of (D_row_ptr, D_col); entry (k,i) is taken from the expansion of
+ *             the community that owns column i.  NOT symmetric (obs. (i) P:L65); not symmetrised.
+ *   log       optional host log; filled by an asynchronous copy (synchronise the stream before reading). */
+int gbe_density(const gbe_csr_view* H, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
+                void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val, gbe_sp2_log* log);
+
+/* The three phases of gbe_density as separate calls (same arguments, same kernels, same stream semantics);
+ * gbe_density == gbe_gather; gbe_sp2; gbe_scatter.  They exist so that a caller can time the phases. */
+int gbe_gather(const gbe_csr_view* H, const gbe_graph* g, void* workspace, size_t workspace_bytes,
+               void* cuda_stream);   /* steps 0, 3: bounds, pack x[s_p] = X0[s_p,s_p], traces of X_0 */
+int gbe_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_tol, void* workspace,
+            size_t workspace_bytes, void* cuda_stream);   /* steps 4-5, `iters` times */
+int gbe_scatter(const gbe_graph* g, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                double* D_val);       /* step 6 */
+int gbe_read_log(const gbe_graph* g, const void* workspace, size_t workspace_bytes, void* cuda_stream,
+                 gbe_sp2_log* log);   /* enqueue the device->host copy of the log of the last gbe_sp2 */
+
+/* Same as gbe_density with HOST buffers: H (row_ptr, col_idx, val) and D_val are host pointers; the call
+ * copies H to the device, runs the path, copies D back and synchronises the stream before returning.
+ * `workspace` stays a device buffer of info.workspace_bytes. */
+int gbe_density_host(const gbe_csr_view* H_host, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val_host,
+                     gbe_sp2_log* log);
+
+void gbe_free_graph(gbe_graph* g);
+
+const char* gbe_strerror(int status);
+const char* gbe_last_cuda_error(void); /* text of the most recent failing CUDA call in this thread ("" if none) */
+const char* gbe_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GBE_H */

@@ -1,0 +1,27 @@
+"""B200-native graph-based SP2 density-matrix path (arXiv:1603.00937) behind the C ABI of include/gbe.h.
+
+    from paper_1603_00937_b200 import DeviceCSR, gbe_build_graph, gbe_density
+    H = DeviceCSR.from_host(system.H)
+    g = gbe_build_graph(H, tau=1e-5, part=None, n_part=512)
+    D_val, log = gbe_density(H, g, n_occ, iters=40)
+
+The CUDA library (libgbe.so, sm_100a) is built in-tree by `python -m paper_1603_00937_b200.build`; the
+binding loads it lazily and fails loudly if it is missing - there is no CPU fallback.
+"""
+from .binding import (  # noqa: F401
+    DeviceCSR,
+    Graph,
+    GbeError,
+    Sp2Log,
+    EXPORTS,
+    LIB_PATH,
+    lib,
+    gbe_build_graph,
+    gbe_graph_export,
+    gbe_density,
+    gbe_density_host,
+    gbe_gather,
+    gbe_sp2,
+    gbe_scatter,
+    gbe_read_log,
+)

@@ -1,0 +1,251 @@
+"""Thin Python binding of the C ABI in include/gbe.h (same names, argument marshalling only).
+
+PyTorch is used for device memory and streams; every step of the path runs inside libgbe.so.
+There is no CPU fallback: a missing library or a failing call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgbe.so")
+
+GBE_MAX_ITERS = 1024
+EXPORTS = [
+    "gbe_build_graph", "gbe_graph_get_info", "gbe_graph_export", "gbe_density", "gbe_gather", "gbe_sp2",
+    "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
+    "gbe_version",
+]
+
+
+class GbeError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__(f"gbe status {status}: {text}")
+        self.status = status
+
+
+class _CsrView(C.Structure):
+    _fields_ = [("n", C.c_int64), ("nnz", C.c_int64), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p),
+                ("val", C.c_void_p)]
+
+
+class _GraphOpts(C.Structure):
+    _fields_ = [("tau", C.c_double), ("power", C.c_int32), ("check_symmetry", C.c_int32)]
+
+
+class _GraphInfo(C.Structure):
+    _fields_ = [("n", C.c_int64), ("nnz_S", C.c_int64), ("n_part", C.c_int64), ("sum_m", C.c_int64),
+                ("max_m", C.c_int64), ("nnz_D", C.c_int64), ("dense_elems", C.c_int64), ("n_tiles", C.c_int64),
+                ("sp2_flops_per_iter", C.c_double), ("eps_min", C.c_double), ("eps_max", C.c_double),
+                ("contiguous_cores", C.c_int32), ("tile", C.c_int32), ("workspace_bytes", C.c_size_t)]
+
+
+class _Sp2Log(C.Structure):
+    _fields_ = [("iters_done", C.c_int32), ("branch", C.c_void_p), ("t1", C.c_void_p), ("t2", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads libgbe.so (built in-tree by `python -m paper_1603_00937_b200.build`). Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1603_00937_b200.build` "
+                              "(there is no CPU fallback)")
+        l = C.CDLL(LIB_PATH)
+        for name in ("gbe_strerror", "gbe_last_cuda_error", "gbe_version"):
+            getattr(l, name).restype = C.c_char_p
+        l.gbe_free_graph.restype = None
+        l.gbe_free_graph.argtypes = [C.c_void_p]
+        l.gbe_build_graph.argtypes = [C.POINTER(_CsrView), C.POINTER(_GraphOpts), C.c_void_p, C.c_int32, C.c_void_p,
+                                      C.POINTER(C.c_void_p)]
+        l.gbe_graph_get_info.argtypes = [C.c_void_p, C.POINTER(_GraphInfo)]
+        l.gbe_graph_export.argtypes = [C.c_void_p] * 9
+        l.gbe_density.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_double, C.c_int32, C.c_double, C.c_void_p,
+                                  C.c_size_t, C.c_void_p, C.c_void_p, C.POINTER(_Sp2Log)]
+        l.gbe_density_host.argtypes = l.gbe_density.argtypes
+        l.gbe_gather.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        l.gbe_sp2.argtypes = [C.c_void_p, C.c_double, C.c_int32, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
+        l.gbe_scatter.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p]
+        l.gbe_read_log.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(_Sp2Log)]
+        _lib = l
+    return _lib
+
+
+def _check(status: int) -> None:
+    if status != 0:
+        raise GbeError(status, lib().gbe_strerror(status).decode())
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _ptr(t) -> int | None:
+    return None if t is None else int(t.data_ptr())
+
+
+@dataclass
+class DeviceCSR:
+    """CSR on the device, dtypes of gbe_csr_view."""
+    n: int
+    row_ptr: torch.Tensor  # int64
+    col_idx: torch.Tensor  # int32
+    val: torch.Tensor  # float64
+
+    @staticmethod
+    def from_host(h, device="cuda") -> "DeviceCSR":
+        return DeviceCSR(int(h.n), torch.from_numpy(np.ascontiguousarray(h.row_ptr, dtype=np.int64)).to(device),
+                         torch.from_numpy(np.ascontiguousarray(h.col_idx, dtype=np.int32)).to(device),
+                         torch.from_numpy(np.ascontiguousarray(h.val, dtype=np.float64)).to(device))
+
+    def view(self) -> _CsrView:
+        assert self.row_ptr.dtype == torch.int64 and self.col_idx.dtype == torch.int32 and self.val.dtype == torch.float64
+        assert self.row_ptr.is_cuda and self.row_ptr.is_contiguous() and self.col_idx.is_contiguous() and self.val.is_contiguous()
+        return _CsrView(self.n, int(self.col_idx.numel()), _ptr(self.row_ptr), _ptr(self.col_idx), _ptr(self.val))
+
+
+@dataclass
+class Sp2Log:
+    iters_done: int
+    branch: np.ndarray
+    t1: np.ndarray
+    t2: np.ndarray
+
+
+class Graph:
+    """Owner of an opaque gbe_graph handle."""
+
+    def __init__(self, handle: int):
+        self._h = C.c_void_p(handle)
+        info = _GraphInfo()
+        _check(lib().gbe_graph_get_info(self._h, C.byref(info)))
+        self.info = {k: getattr(info, k) for k, _ in _GraphInfo._fields_}
+
+    @property
+    def handle(self):
+        if not self._h:
+            raise ValueError("graph already freed")
+        return self._h
+
+    def free(self):
+        if self._h:
+            lib().gbe_free_graph(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+    def new_workspace(self, device="cuda") -> torch.Tensor:
+        return torch.empty(self.info["workspace_bytes"], dtype=torch.uint8, device=device)
+
+    def export(self, stream=None) -> dict:
+        return gbe_graph_export(self, stream)
+
+
+def gbe_build_graph(H: DeviceCSR, tau: float, part: torch.Tensor | None, n_part: int, power: int = 2,
+                    check_symmetry: bool = False, stream=None) -> Graph:
+    opts = _GraphOpts(float(tau), int(power), int(bool(check_symmetry)))
+    if part is not None:
+        assert part.dtype == torch.int32 and part.is_cuda and part.is_contiguous() and part.numel() == H.n
+    out = C.c_void_p()
+    v = H.view()
+    _check(lib().gbe_build_graph(C.byref(v), C.byref(opts), _ptr(part), int(n_part), _stream(stream), C.byref(out)))
+    return Graph(out.value)
+
+
+def gbe_graph_export(g: Graph, stream=None) -> dict:
+    i = g.info
+    dev = "cuda"
+    out = dict(
+        S_row_ptr=torch.empty(i["n"] + 1, dtype=torch.int64, device=dev),
+        S_col=torch.empty(i["nnz_S"], dtype=torch.int32, device=dev),
+        sub_ptr=torch.empty(i["n_part"] + 1, dtype=torch.int64, device=dev),
+        sub_idx=torch.empty(i["sum_m"], dtype=torch.int32, device=dev),
+        ncore=torch.empty(i["n_part"], dtype=torch.int32, device=dev),
+        D_row_ptr=torch.empty(i["n"] + 1, dtype=torch.int64, device=dev),
+        D_col=torch.empty(i["nnz_D"], dtype=torch.int32, device=dev),
+    )
+    _check(lib().gbe_graph_export(g.handle, _stream(stream), *[_ptr(out[k]) for k in
+                                  ("S_row_ptr", "S_col", "sub_ptr", "sub_idx", "ncore", "D_row_ptr", "D_col")]))
+    return out
+
+
+def _new_log(iters: int):
+    br = np.zeros(max(iters, 1), dtype=np.uint8)
+    t1 = np.zeros(iters + 1, dtype=np.float64)
+    t2 = np.zeros(iters + 1, dtype=np.float64)
+    return _Sp2Log(0, br.ctypes.data, t1.ctypes.data, t2.ctypes.data), (br, t1, t2)
+
+
+def _finish_log(clog, arrs) -> Sp2Log:
+    k = int(clog.iters_done)
+    br, t1, t2 = arrs
+    return Sp2Log(k, br[:k].copy(), t1[:k + 1].copy(), t2[:k + 1].copy())
+
+
+def gbe_density(H: DeviceCSR, g: Graph, n_occ: float, iters: int, idem_tol: float = -1.0,
+                workspace: torch.Tensor | None = None, D_val: torch.Tensor | None = None, want_log: bool = True,
+                stream=None):
+    """Returns (D_val, Sp2Log | None).  With want_log the call synchronises the stream to read the log."""
+    if workspace is None:
+        workspace = g.new_workspace()
+    if D_val is None:
+        D_val = torch.empty(g.info["nnz_D"], dtype=torch.float64, device="cuda")
+    v = H.view()
+    clog, arrs = _new_log(iters) if want_log else (None, None)
+    _check(lib().gbe_density(C.byref(v), g.handle, float(n_occ), int(iters), float(idem_tol), _ptr(workspace),
+                             workspace.numel(), _stream(stream), _ptr(D_val), C.byref(clog) if want_log else None))
+    return D_val, (_finish_log(clog, arrs) if want_log else None)
+
+
+def gbe_gather(H: DeviceCSR, g: Graph, workspace: torch.Tensor, stream=None) -> None:
+    v = H.view()
+    _check(lib().gbe_gather(C.byref(v), g.handle, _ptr(workspace), workspace.numel(), _stream(stream)))
+
+
+def gbe_sp2(g: Graph, n_occ: float, iters: int, idem_tol: float, workspace: torch.Tensor, stream=None) -> None:
+    _check(lib().gbe_sp2(g.handle, float(n_occ), int(iters), float(idem_tol), _ptr(workspace), workspace.numel(),
+                         _stream(stream)))
+
+
+def gbe_scatter(g: Graph, workspace: torch.Tensor, D_val: torch.Tensor, stream=None) -> None:
+    _check(lib().gbe_scatter(g.handle, _ptr(workspace), workspace.numel(), _stream(stream), _ptr(D_val)))
+
+
+def gbe_read_log(g: Graph, workspace: torch.Tensor, iters: int = GBE_MAX_ITERS, stream=None) -> Sp2Log:
+    clog, arrs = _new_log(iters)
+    _check(lib().gbe_read_log(g.handle, _ptr(workspace), workspace.numel(), _stream(stream), C.byref(clog)))
+    return _finish_log(clog, arrs)
+
+
+def gbe_density_host(H_host, g: Graph, n_occ: float, iters: int, idem_tol: float = -1.0,
+                     workspace: torch.Tensor | None = None, D_val_host: np.ndarray | None = None,
+                     want_log: bool = False, stream=None):
+    """H_host: object with numpy fields n, row_ptr (int64), col_idx (int32), val (float64) - HOST memory
+    (pinned or pageable).  Copies in, runs, copies D back, synchronises."""
+    if workspace is None:
+        workspace = g.new_workspace()
+    if D_val_host is None:
+        D_val_host = np.empty(g.info["nnz_D"], dtype=np.float64)
+    rp = np.ascontiguousarray(H_host.row_ptr, dtype=np.int64)
+    ci = np.ascontiguousarray(H_host.col_idx, dtype=np.int32)
+    va = np.ascontiguousarray(H_host.val, dtype=np.float64)
+    v = _CsrView(int(H_host.n), int(ci.size), rp.ctypes.data, ci.ctypes.data, va.ctypes.data)
+    clog, arrs = _new_log(iters) if want_log else (None, None)
+    _check(lib().gbe_density_host(C.byref(v), g.handle, float(n_occ), int(iters), float(idem_tol), _ptr(workspace),
+                                  workspace.numel(), _stream(stream), D_val_host.ctypes.data,
+                                  C.byref(clog) if want_log else None))
+    return D_val_host, (_finish_log(clog, arrs) if want_log else None)

@@ -1,0 +1,260 @@
+// The C ABI of include/gbe.h: argument checks, the graph handle, workspace carving and the launch sequence.
+// Every step of the path runs in the kernels of gbe_{bounds,graph,halo,gather,x2,trace,scatter}.cu.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "gbe_internal.cuh"
+
+namespace {
+thread_local char g_cuda_err[512] = "";
+
+__global__ void k_init_state(gbe_state* st, double n_occ, double idem_tol, int iters) {
+  st->n_occ = n_occ;
+  st->idem_tol = idem_tol;
+  st->iters = iters;
+  st->iter = 0;
+  st->branch = 0;
+  st->stop = 0;
+  st->iters_done = 0;
+}
+
+struct WS {
+  gbe_state* st;
+  double *blo, *bhi, *partials, *X0, *X1;
+};
+int carve(const gbe_graph* g, void* workspace, size_t bytes, WS* w) {
+  if (!workspace) return GBE_EINVAL;
+  if (bytes < g->ws_bytes) return GBE_ENOMEM;
+  if (reinterpret_cast<uintptr_t>(workspace) % 256) return GBE_EINVAL;
+  unsigned char* b = static_cast<unsigned char*>(workspace);
+  w->st = reinterpret_cast<gbe_state*>(b);
+  w->blo = reinterpret_cast<double*>(b + g->ws_bounds);
+  w->bhi = w->blo + 1024;
+  w->partials = reinterpret_cast<double*>(b + g->ws_partials);
+  w->X0 = reinterpret_cast<double*>(b + g->ws_x0);
+  w->X1 = reinterpret_cast<double*>(b + g->ws_x1);
+  return GBE_OK;
+}
+int check_csr(const gbe_csr_view* H) {
+  if (!H || !H->row_ptr || H->n <= 0 || H->nnz < 0 || H->n > INT32_MAX) return GBE_EINVAL;
+  if (H->nnz > 0 && (!H->col_idx || !H->val)) return GBE_EINVAL;
+  return GBE_OK;
+}
+}  // namespace
+
+void gbe_set_cuda_error(cudaError_t e, const char* what, int line) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "%s (%s) at %s, line %d", cudaGetErrorString(e), cudaGetErrorName(e), what,
+           line);
+}
+
+extern "C" {
+
+const char* gbe_last_cuda_error(void) { return g_cuda_err; }
+const char* gbe_version(void) { return "gbe 0.1 (sm_100a)"; }
+
+const char* gbe_strerror(int status) {
+  switch (status) {
+    case GBE_OK: return "ok";
+    case GBE_EINVAL: return "invalid argument";
+    case GBE_ENOTSYM: return "H is not symmetric";
+    case GBE_EDEGENERATE: return "degenerate spectral bounds (eps_max == eps_min)";
+    case GBE_EMISMATCH: return "H does not match the graph";
+    case GBE_ENOMEM: return "workspace too small or allocation failed";
+    case GBE_ECUDA: return g_cuda_err[0] ? g_cuda_err : "CUDA error";
+    default: return "unknown status";
+  }
+}
+
+void gbe_free_graph(gbe_graph* g) {
+  if (!g) return;
+  void* ptrs[] = {g->S_row_ptr, g->S_col,     g->sub_ptr,  g->sub_idx,  g->ncore,    g->msize, g->dense_off, g->D_row_ptr,
+                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->gitems};
+  for (void* p : ptrs)
+    if (p) cudaFree(p);
+  delete g;
+}
+
+int gbe_build_graph(const gbe_csr_view* H, const gbe_graph_opts* opts, const int32_t* part, int32_t n_part,
+                    void* cuda_stream, gbe_graph** out) {
+  if (!out) return GBE_EINVAL;
+  *out = nullptr;
+  GBE_TRY(check_csr(H));
+  if (!opts || !(opts->tau >= 0.0) || std::isnan(opts->tau)) return GBE_EINVAL;
+  const int power = opts->power == 0 ? 2 : opts->power;
+  if (power < 1 || power > GBE_MAX_POWER) return GBE_EINVAL;
+  if (n_part < 1 || n_part > H->n) return GBE_EINVAL;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+
+  gbe_graph* g = new (std::nothrow) gbe_graph();
+  if (!g) return GBE_ENOMEM;
+  g->n = H->n;
+  g->n_part = n_part;
+  g->tau = opts->tau;
+  g->power = power;
+  g->tile = 128;
+  struct Guard {
+    gbe_graph* g;
+    ~Guard() { if (g) gbe_free_graph(g); }
+  } guard{g};
+
+  // step 0: bounds of the H given here
+  DevBuf st, bl;
+  GBE_TRY(st.alloc(sizeof(gbe_state)));
+  GBE_TRY(bl.alloc(2 * 1024 * sizeof(double)));
+  GBE_TRY(gbe_launch_bounds(*H, bl.as<double>(), bl.as<double>() + 1024, 1024, st.as<gbe_state>(), s));
+  struct { double lo, hi; } b;
+  GBE_CUDA(cudaMemcpyAsync(&b, st.p, sizeof(b), cudaMemcpyDeviceToHost, s));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  if (!(b.hi > b.lo) || !std::isfinite(b.lo) || !std::isfinite(b.hi)) return GBE_EDEGENERATE;
+  g->eps_min = b.lo;
+  g->eps_max = b.hi;
+
+  // step 1: S_tau
+  GBE_TRY(gbe_build_pattern(*H, st.as<gbe_state>(), g->tau, power, opts->check_symmetry, s, &g->S_row_ptr, &g->S_col,
+                            &g->nnz_S));
+  // step 2: subgraphs, layout, pattern of D, work lists
+  GBE_TRY(gbe_build_subgraphs(g, part, s));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  guard.g = nullptr;
+  *out = g;
+  return GBE_OK;
+}
+
+int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
+  if (!g || !o) return GBE_EINVAL;
+  memset(o, 0, sizeof(*o));
+  o->n = g->n;
+  o->nnz_S = g->nnz_S;
+  o->n_part = g->n_part;
+  o->sum_m = g->sum_m;
+  o->max_m = g->max_m;
+  o->nnz_D = g->nnz_D;
+  o->dense_elems = g->dense_elems;
+  o->n_tiles = g->n_items;
+  o->sp2_flops_per_iter = g->flops_per_iter;
+  o->eps_min = g->eps_min;
+  o->eps_max = g->eps_max;
+  o->contiguous_cores = g->contiguous;
+  o->tile = g->tile;
+  o->workspace_bytes = g->ws_bytes;
+  return GBE_OK;
+}
+
+int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, int32_t* S_col, int64_t* sub_ptr,
+                     int32_t* sub_idx, int32_t* ncore, int64_t* D_row_ptr, int32_t* D_col) {
+  if (!g) return GBE_EINVAL;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  auto cp = [&](void* dst, const void* src, size_t bytes) -> int {
+    if (dst && bytes) GBE_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, s));
+    return GBE_OK;
+  };
+  GBE_TRY(cp(S_row_ptr, g->S_row_ptr, (size_t)(g->n + 1) * 8));
+  GBE_TRY(cp(S_col, g->S_col, (size_t)g->nnz_S * 4));
+  GBE_TRY(cp(sub_ptr, g->sub_ptr, (size_t)(g->n_part + 1) * 8));
+  GBE_TRY(cp(sub_idx, g->sub_idx, (size_t)g->sum_m * 4));
+  GBE_TRY(cp(ncore, g->ncore, (size_t)g->n_part * 4));
+  GBE_TRY(cp(D_row_ptr, g->D_row_ptr, (size_t)(g->n + 1) * 8));
+  GBE_TRY(cp(D_col, g->D_col, (size_t)g->nnz_D * 4));
+  return GBE_OK;
+}
+
+int gbe_gather(const gbe_csr_view* H, const gbe_graph* g, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!g) return GBE_EINVAL;
+  GBE_TRY(check_csr(H));
+  if (H->n != g->n) return GBE_EMISMATCH;
+  WS w;
+  GBE_TRY(carve(g, workspace, workspace_bytes, &w));
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  GBE_TRY(gbe_launch_bounds(*H, w.blo, w.bhi, 1024, w.st, s));
+  GBE_TRY(gbe_launch_gather(*H, g, w.st, w.X0, w.partials, s));
+  return GBE_OK;
+}
+
+int gbe_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_tol, void* workspace, size_t workspace_bytes,
+            void* cuda_stream) {
+  if (!g) return GBE_EINVAL;
+  if (!(n_occ >= 0.0) || n_occ > (double)g->n || iters < 0 || iters > GBE_MAX_ITERS || std::isnan(idem_tol))
+    return GBE_EINVAL;
+  WS w;
+  GBE_TRY(carve(g, workspace, workspace_bytes, &w));
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters);
+  GBE_CUDA(cudaGetLastError());
+  // traces of X_0 (partials written by the gather), branch of iteration 0
+  GBE_TRY(gbe_launch_trace_branch(w.st, w.partials, g->n_gitems, s));
+  for (int it = 0; it < iters; ++it) {
+    const double* in = (it & 1) ? w.X1 : w.X0;
+    double* outp = (it & 1) ? w.X0 : w.X1;
+    GBE_TRY(gbe_launch_x2(g, w.st, in, outp, w.partials, it, s));
+    GBE_TRY(gbe_launch_trace_branch(w.st, w.partials, g->n_items, s));
+  }
+  return GBE_OK;
+}
+
+int gbe_scatter(const gbe_graph* g, void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val) {
+  if (!g || (!D_val && g->nnz_D > 0)) return GBE_EINVAL;
+  WS w;
+  GBE_TRY(carve(g, workspace, workspace_bytes, &w));
+  return gbe_launch_scatter(g, w.st, w.X0, w.X1, D_val, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int gbe_read_log(const gbe_graph* g, const void* workspace, size_t workspace_bytes, void* cuda_stream, gbe_sp2_log* log) {
+  if (!g || !log) return GBE_EINVAL;
+  WS w;
+  GBE_TRY(carve(g, const_cast<void*>(workspace), workspace_bytes, &w));
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  gbe_state hs_small;  // only the header is needed first
+  GBE_CUDA(cudaMemcpyAsync(&hs_small, w.st, offsetof(gbe_state, t1), cudaMemcpyDeviceToHost, s));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  if (hs_small.degenerate) return GBE_EDEGENERATE;
+  const int k = hs_small.iters_done;
+  log->iters_done = k;
+  if (log->t1) GBE_CUDA(cudaMemcpyAsync(log->t1, w.st->t1, (size_t)(k + 1) * 8, cudaMemcpyDeviceToHost, s));
+  if (log->t2) GBE_CUDA(cudaMemcpyAsync(log->t2, w.st->t2, (size_t)(k + 1) * 8, cudaMemcpyDeviceToHost, s));
+  if (log->branch && k > 0) GBE_CUDA(cudaMemcpyAsync(log->branch, w.st->br, (size_t)k, cudaMemcpyDeviceToHost, s));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  return GBE_OK;
+}
+
+int gbe_density(const gbe_csr_view* H, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
+                void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val, gbe_sp2_log* log) {
+  if (!g || (!D_val && g->nnz_D > 0)) return GBE_EINVAL;
+  if (!(n_occ >= 0.0) || n_occ > (double)g->n || iters < 0 || iters > GBE_MAX_ITERS || std::isnan(idem_tol))
+    return GBE_EINVAL;
+  GBE_TRY(gbe_gather(H, g, workspace, workspace_bytes, cuda_stream));
+  GBE_TRY(gbe_sp2(g, n_occ, iters, idem_tol, workspace, workspace_bytes, cuda_stream));
+  GBE_TRY(gbe_scatter(g, workspace, workspace_bytes, cuda_stream, D_val));
+  if (log) GBE_TRY(gbe_read_log(g, workspace, workspace_bytes, cuda_stream, log));
+  return GBE_OK;
+}
+
+int gbe_density_host(const gbe_csr_view* Hh, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val_host, gbe_sp2_log* log) {
+  if (!g || (!D_val_host && g->nnz_D > 0)) return GBE_EINVAL;
+  GBE_TRY(check_csr(Hh));
+  if (Hh->n != g->n) return GBE_EMISMATCH;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  DevBuf rp, ci, va, dv;
+  GBE_TRY(rp.alloc((size_t)(Hh->n + 1) * 8));
+  GBE_TRY(ci.alloc((size_t)Hh->nnz * 4));
+  GBE_TRY(va.alloc((size_t)Hh->nnz * 8));
+  GBE_TRY(dv.alloc((size_t)g->nnz_D * 8));
+  GBE_CUDA(cudaMemcpyAsync(rp.p, Hh->row_ptr, (size_t)(Hh->n + 1) * 8, cudaMemcpyHostToDevice, s));
+  if (Hh->nnz) {
+    GBE_CUDA(cudaMemcpyAsync(ci.p, Hh->col_idx, (size_t)Hh->nnz * 4, cudaMemcpyHostToDevice, s));
+    GBE_CUDA(cudaMemcpyAsync(va.p, Hh->val, (size_t)Hh->nnz * 8, cudaMemcpyHostToDevice, s));
+  }
+  gbe_csr_view Hd{Hh->n, Hh->nnz, rp.as<int64_t>(), ci.as<int32_t>(), va.as<double>()};
+  int rc = gbe_density(&Hd, g, n_occ, iters, idem_tol, workspace, workspace_bytes, cuda_stream, dv.as<double>(), log);
+  if (rc == GBE_OK && g->nnz_D) {
+    cudaError_t e = cudaMemcpyAsync(D_val_host, dv.p, (size_t)g->nnz_D * 8, cudaMemcpyDeviceToHost, s);
+    if (e != cudaSuccess) { gbe_set_cuda_error(e, "cudaMemcpyAsync D", __LINE__); rc = GBE_ECUDA; }
+  }
+  cudaError_t e = cudaStreamSynchronize(s);  // also keeps the staging buffers alive until the work is done
+  if (rc == GBE_OK && e != cudaSuccess) { gbe_set_cuda_error(e, "cudaStreamSynchronize", __LINE__); rc = GBE_ECUDA; }
+  return rc;
+}
+
+}  // extern "C"

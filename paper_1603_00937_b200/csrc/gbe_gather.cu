@@ -1,0 +1,143 @@
+// Step 3 - gather / pack (row 3).
+//
+//     x_p = X0[s_p, s_p],  X0 = (eps_max I - H)/(eps_max - eps_min)                         (A-2)
+// the FULL principal submatrix: every stored H entry with both indices in s_p; zero elsewhere; the diagonal
+// gets (eps_max - H_kk)/delta even when H_kk is not stored (A-12).  Output: row-major FP64 blocks,
+// ld_p = m_p rounded up to 16 doubles (rows are 128-byte aligned), pad columns zero.
+//
+// One CTA handles `gather_rows` consecutive rows of one community.  The global -> local index translation is a
+// pair of bitmaps (core, halo) over the n vertices with popcount-prefix ranks in shared memory: O(1) per
+// stored entry, no search.  Each warp builds one output row in shared memory (zero fill + scattered entries)
+// and streams it out with 128-bit stores, so every output byte is written exactly once, fully coalesced.
+// The epilogue accumulates the traces of X_0 and X_0^2 over the core rows (t1, t2 of iteration 0):
+// (X^2)_ii = sum_c X_ic^2 for symmetric X.
+// Bound: HBM - writes 8 m_p^2 B per community, reads 12 B per stored entry of every gathered H row.
+#include "gbe_internal.cuh"
+
+namespace {
+
+__global__ void __launch_bounds__(256) k_gather(int W, int ldmax, int rows_per_cta, const int2* __restrict__ gitems,
+                                                const int64_t* __restrict__ H_rp, const int32_t* __restrict__ H_col,
+                                                const double* __restrict__ H_val, int64_t n,
+                                                const int64_t* __restrict__ sub_ptr, const int32_t* __restrict__ sub_idx,
+                                                const int32_t* __restrict__ ncore_arr,
+                                                const int64_t* __restrict__ dense_off, const gbe_state* __restrict__ st,
+                                                double* __restrict__ X, double* __restrict__ partials) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint32_t* coreb = reinterpret_cast<uint32_t*>(smem_raw);
+  uint32_t* halob = coreb + W;
+  uint32_t* corerk = halob + W;
+  uint32_t* halork = corerk + W;
+  int* scratch = reinterpret_cast<int*>(halork + W);                      // 2 * 257 ints
+  double* red = reinterpret_cast<double*>(scratch + 516);                  // 16 doubles (8-byte aligned: 4W*4 + 2064)
+  double* rowbuf = red + 16;                                               // nwarps * ldmax doubles
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5, nw = blockDim.x >> 5;
+  const int2 it = gitems[blockIdx.x];
+  const int p = it.x, r0 = it.y;
+  const int64_t sb = sub_ptr[p];
+  const int m = (int)(sub_ptr[p + 1] - sb);
+  const int nc = ncore_arr[p];
+  const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+  const double eps_max = st->eps_max, delta = st->eps_max - st->eps_min;
+
+  // bitmaps of the community's core and halo vertices
+  for (int w = t; w < 2 * W; w += blockDim.x) coreb[w] = 0u;
+  __syncthreads();
+  for (int r = t; r < m; r += blockDim.x) {
+    const int v = sub_idx[sb + r];
+    atomicOr(r < nc ? &coreb[v >> 5] : &halob[v >> 5], 1u << (v & 31));
+  }
+  __syncthreads();
+  // ranks: exclusive popcount prefix per word (both bitmaps at once)
+  {
+    const int nt = blockDim.x, chunk = (W + nt - 1) / nt;
+    const int b = min(W, t * chunk), e = min(W, b + chunk);
+    int c0 = 0, c1 = 0;
+    for (int w = b; w < e; ++w) { c0 += __popc(coreb[w]); c1 += __popc(halob[w]); }
+    scratch[t] = c0;
+    scratch[258 + t] = c1;
+    __syncthreads();
+    if (t < 2) {
+      int* sc = scratch + 258 * t;
+      int run = 0;
+      for (int k = 0; k < nt; ++k) { const int v = sc[k]; sc[k] = run; run += v; }
+    }
+    __syncthreads();
+    c0 = scratch[t];
+    c1 = scratch[258 + t];
+    for (int w = b; w < e; ++w) {
+      corerk[w] = c0; c0 += __popc(coreb[w]);
+      halork[w] = c1; c1 += __popc(halob[w]);
+    }
+  }
+  __syncthreads();
+
+  double* buf = rowbuf + (size_t)wid * ldmax;
+  double* Xp = X + dense_off[p];
+  double s1 = 0.0, s2 = 0.0;
+  const int rend = min(m, r0 + rows_per_cta);
+  for (int r = r0 + wid; r < rend; r += nw) {
+    for (int c = lane * 2; c < ld; c += 64) *reinterpret_cast<double2*>(buf + c) = make_double2(0.0, 0.0);
+    __syncwarp();
+    const int k = sub_idx[sb + r];
+    if (lane == 0) buf[r] = (eps_max - 0.0) / delta;  // a stored diagonal overwrites this below
+    __syncwarp();
+    const int64_t a = H_rp[k], b = H_rp[k + 1];
+    for (int64_t e = a + lane; e < b; e += 32) {
+      const int j = H_col[e];
+      if ((unsigned)j >= (uint64_t)n) continue;
+      const uint32_t bit = 1u << (j & 31), wj = j >> 5;
+      int c = -1;
+      const uint32_t cw = coreb[wj];
+      if (cw & bit) {
+        c = corerk[wj] + __popc(cw & (bit - 1u));
+      } else {
+        const uint32_t hw = halob[wj];
+        if (hw & bit) c = nc + halork[wj] + __popc(hw & (bit - 1u));
+      }
+      if (c >= 0) buf[c] = ((j == k ? eps_max : 0.0) - H_val[e]) / delta;
+    }
+    __syncwarp();
+    double* out = Xp + (size_t)r * ld;
+    double q = 0.0;
+    for (int c = lane * 2; c < ld; c += 64) {
+      const double2 v = *reinterpret_cast<const double2*>(buf + c);
+      *reinterpret_cast<double2*>(out + c) = v;
+      q += v.x * v.x + v.y * v.y;
+    }
+    if (r < nc) {  // warp-uniform
+      s2 += q;
+      if (lane == 0) s1 += buf[r];
+    }
+    __syncwarp();
+  }
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  if (lane == 0) { red[wid] = s1; red[8 + wid] = s2; }
+  __syncthreads();
+  if (t == 0) {
+    double a1 = 0.0, a2 = 0.0;
+    for (int w = 0; w < nw; ++w) { a1 += red[w]; a2 += red[8 + w]; }
+    partials[2 * (size_t)blockIdx.x] = a1;
+    partials[2 * (size_t)blockIdx.x + 1] = a2;
+  }
+}
+
+}  // namespace
+
+int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state* st, double* X, double* partials,
+                      cudaStream_t s) {
+  if (g->n_gitems == 0) return GBE_OK;
+  const int W = (int)((g->n + 31) / 32);
+  const int ldmax = (g->max_m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+  const size_t fixed = (size_t)4 * W * 4 + 516 * 4 + 16 * 8;
+  const size_t budget = 220 * 1024;
+  if (fixed + (size_t)ldmax * 8 > budget) return GBE_EINVAL;
+  int nw = (int)std::min<size_t>(8, (budget - fixed) / ((size_t)ldmax * 8));
+  const size_t smem = fixed + (size_t)nw * ldmax * 8;
+  GBE_CUDA(cudaFuncSetAttribute(k_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_gather<<<g->n_gitems, nw * 32, smem, s>>>(W, ldmax, g->gather_rows, g->gitems, H.row_ptr, H.col_idx, H.val, g->n,
+                                              g->sub_ptr, g->sub_idx, g->ncore, g->dense_off, st, X, partials);
+  GBE_CUDA(cudaGetLastError());
+  return GBE_OK;
+}

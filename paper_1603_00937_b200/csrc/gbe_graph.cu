@@ -1,0 +1,430 @@
+// Step 1 - the data-dependency graph S_tau (row 1).
+//
+// Reading A-1 of Eq.(2) P:L38-40 (in the spirit of Eq.(8)):
+//     A = floor(X0)_tau,  X0 = (eps_max I - H)/(eps_max - eps_min)       (|value| >= tau kept, A-3)
+//     T^(1) = A,  T^(n) = floor(A T^(n-1))_tau,  n = 2..power
+//     S = I u pat(T^(1)) u ... u pat(T^(power)),  then S u S^T          (self loops: T^(0) = I, A-4)
+//
+// Every kernel is warp-per-row CSR work with a per-warp bitmap over the n columns in shared memory:
+//   - the thresholded product is a row-wise (Gustavson, ref. 18 P:L132) accumulation: pass 1 marks the candidate
+//     columns in the bitmap, a popcount prefix turns the bitmap into a compact slot index, pass 2 accumulates
+//     a_ik * t_kj into the compact accumulator with k ASCENDING and a separate multiply and add, so the value of
+//     every entry does not depend on scheduling (and A A is bitwise symmetric when H is);
+//   - walking the bitmap emits the columns in ascending order, so no sort is ever needed.
+// Bound: L2/shared-memory latency (integer + a few FP64 operations per candidate); it runs once per graph.
+#include "gbe_internal.cuh"
+
+namespace {
+
+
+__device__ __forceinline__ double x0_entry(double h, bool diag, double eps_max, double delta) {
+  return ((diag ? eps_max : 0.0) - h) / delta;
+}
+
+// ---------------------------------------------------------------- A = floor(X0)_tau with an explicit diagonal
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_materialise_A(int64_t n, const int64_t* __restrict__ rp,
+                                                       const int32_t* __restrict__ col, const double* __restrict__ val,
+                                                       const gbe_state* __restrict__ st, double tau,
+                                                       int32_t* __restrict__ cnt, const int64_t* __restrict__ out_rp,
+                                                       int32_t* __restrict__ out_col, double* __restrict__ out_val) {
+  const int lane = threadIdx.x & 31;
+  const int64_t i = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (i >= n) return;
+  const double eps_max = st->eps_max, delta = st->eps_max - st->eps_min;
+  const int64_t a = rp[i], b = rp[i + 1];
+  // does the row store its diagonal?  (A-12: a missing diagonal means H_ii = 0, X0_ii = eps_max/delta)
+  int has = 0;
+  for (int64_t e = a + lane; e < b; e += 32) has |= (col[e] == i);
+  has = __any_sync(0xffffffffu, has);
+  const double dmiss = x0_entry(0.0, true, eps_max, delta);
+  const bool ins = !has && fabs(dmiss) >= tau;
+  int kept = 0, less = 0;  // kept entries so far; kept entries with column < i
+  const int64_t ob = FILL ? out_rp[i] : 0;
+  for (int64_t e0 = a; e0 < b; e0 += 32) {
+    const int64_t e = e0 + lane;
+    int c = -1;
+    double x = 0.0;
+    bool keep = false;
+    if (e < b) {
+      c = col[e];
+      x = x0_entry(val[e], c == i, eps_max, delta);
+      keep = fabs(x) >= tau;
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, keep);
+    const unsigned ml = __ballot_sync(0xffffffffu, keep && c < i);
+    if (FILL && keep) {
+      const int pos = kept + __popc(m & ((1u << lane) - 1)) + ((ins && c > i) ? 1 : 0);
+      out_col[ob + pos] = c;
+      out_val[ob + pos] = x;
+    }
+    kept += __popc(m);
+    less += __popc(ml);
+  }
+  if (lane == 0) {
+    if (FILL) {
+      if (ins) { out_col[ob + less] = (int32_t)i; out_val[ob + less] = dmiss; }
+    } else {
+      cnt[i] = kept + (ins ? 1 : 0);
+    }
+  }
+}
+
+// ---------------------------------------------------------------- T_next = floor(A T)_tau
+// MODE 0: distinct candidate columns per row (sizes the accumulator); 1: count kept entries; 2: fill.
+template <int MODE>
+__global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __restrict__ A_rp,
+                                   const int32_t* __restrict__ A_col, const double* __restrict__ A_val,
+                                   const int64_t* __restrict__ T_rp, const int32_t* __restrict__ T_col,
+                                   const double* __restrict__ T_val, double tau, int32_t* __restrict__ cnt,
+                                   const int64_t* __restrict__ out_rp, int32_t* __restrict__ out_col,
+                                   double* __restrict__ out_val) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, w_in_blk = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const size_t per_warp = (size_t)W * 8 + (MODE == 0 ? 0 : (size_t)cap * 8);
+  unsigned char* base = smem_raw + per_warp * w_in_blk;
+  double* acc = reinterpret_cast<double*>(base);  // cap doubles (first: keeps 8-byte alignment)
+  uint32_t* bm = reinterpret_cast<uint32_t*>(base + (MODE == 0 ? 0 : (size_t)cap * 8));
+  uint32_t* rk = bm + W;
+
+  for (int64_t i = (int64_t)blockIdx.x * nw + w_in_blk; i < n; i += (int64_t)gridDim.x * nw) {
+    for (int w = lane; w < W; w += 32) bm[w] = 0u;
+    __syncwarp();
+    const int64_t a = A_rp[i], b = A_rp[i + 1];
+    // pass 1: mark candidate columns
+    for (int64_t e0 = a; e0 < b; e0 += 32) {
+      const int64_t e = e0 + lane;
+      const int kk = e < b ? A_col[e] : 0;
+      const int nk = (int)min((int64_t)32, b - e0);
+      for (int q = 0; q < nk; ++q) {
+        const int k = __shfl_sync(0xffffffffu, kk, q);
+        const int64_t tb = T_rp[k], te = T_rp[k + 1];
+        for (int64_t f = tb + lane; f < te; f += 32) {
+          const int j = T_col[f];
+          atomicOr(&bm[j >> 5], 1u << (j & 31));
+        }
+      }
+    }
+    __syncwarp();
+    // compact slot index: rk[w] = number of candidates in words < w
+    int running = 0;
+    for (int w0 = 0; w0 < W; w0 += 32) {
+      const int w = w0 + lane;
+      const int c = w < W ? __popc(bm[w]) : 0;
+      int tot;
+      const int ex = warp_excl_scan_i(c, lane, &tot);
+      if (w < W) rk[w] = running + ex;
+      running += tot;
+    }
+    if constexpr (MODE == 0) {
+      if (lane == 0) cnt[i] = running;
+      __syncwarp();
+      continue;
+    }
+    for (int s = lane; s < running; s += 32) acc[s] = 0.0;
+    __syncwarp();
+    // pass 2: accumulate, k ascending, multiply and add separately rounded
+    for (int64_t e0 = a; e0 < b; e0 += 32) {
+      const int64_t e = e0 + lane;
+      const int kk = e < b ? A_col[e] : 0;
+      const double av = e < b ? A_val[e] : 0.0;
+      const int nk = (int)min((int64_t)32, b - e0);
+      for (int q = 0; q < nk; ++q) {
+        const int k = __shfl_sync(0xffffffffu, kk, q);
+        const double aik = __shfl_sync(0xffffffffu, av, q);
+        const int64_t tb = T_rp[k], te = T_rp[k + 1];
+        for (int64_t f = tb + lane; f < te; f += 32) {
+          const int j = T_col[f];
+          const uint32_t word = bm[j >> 5];
+          const int slot = rk[j >> 5] + __popc(word & ((1u << (j & 31)) - 1u));
+          acc[slot] = __dadd_rn(acc[slot], __dmul_rn(aik, T_val[f]));
+        }
+        __syncwarp();  // the next k may hit the same slots
+      }
+    }
+    // emit kept entries in ascending column order
+    int kept = 0;
+    const int64_t ob = MODE == 2 ? out_rp[i] : 0;
+    for (int w0 = 0; w0 < W; w0 += 32) {
+      const int w = w0 + lane;
+      uint32_t bits = w < W ? bm[w] : 0u;
+      const int s0 = w < W ? (int)rk[w] : 0;
+      int mine = 0;
+      {
+        uint32_t t = bits;
+        int idx = 0;
+        while (t) {
+          t &= t - 1;
+          if (fabs(acc[s0 + idx]) >= tau) ++mine;
+          ++idx;
+        }
+      }
+      int tot;
+      const int ex = warp_excl_scan_i(mine, lane, &tot);
+      if (MODE == 2) {
+        int pos = kept + ex, idx = 0;
+        while (bits) {
+          const int bpos = __ffs(bits) - 1;
+          bits &= bits - 1;
+          const double v = acc[s0 + idx];
+          ++idx;
+          if (fabs(v) >= tau) {
+            out_col[ob + pos] = w * 32 + bpos;
+            out_val[ob + pos] = v;
+            ++pos;
+          }
+        }
+      }
+      kept += tot;
+    }
+    if (MODE == 1 && lane == 0) cnt[i] = kept;
+    __syncwarp();
+  }
+}
+
+// ---------------------------------------------------------------- row-wise union of two patterns (+ self loops)
+template <bool FILL>
+__global__ void k_union_rows(int64_t n, int W, const int64_t* __restrict__ P_rp, const int32_t* __restrict__ P_col,
+                             const int64_t* __restrict__ Q_rp, const int32_t* __restrict__ Q_col, int add_diag,
+                             int32_t* __restrict__ cnt, const int64_t* __restrict__ out_rp,
+                             int32_t* __restrict__ out_col) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, w_in_blk = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  uint32_t* bm = reinterpret_cast<uint32_t*>(smem_raw) + (size_t)W * w_in_blk;
+  for (int64_t i = (int64_t)blockIdx.x * nw + w_in_blk; i < n; i += (int64_t)gridDim.x * nw) {
+    for (int w = lane; w < W; w += 32) bm[w] = 0u;
+    __syncwarp();
+    for (int64_t e = P_rp[i] + lane; e < P_rp[i + 1]; e += 32) { const int j = P_col[e]; atomicOr(&bm[j >> 5], 1u << (j & 31)); }
+    if (Q_rp)
+      for (int64_t e = Q_rp[i] + lane; e < Q_rp[i + 1]; e += 32) { const int j = Q_col[e]; atomicOr(&bm[j >> 5], 1u << (j & 31)); }
+    if (add_diag && lane == 0) atomicOr(&bm[i >> 5], 1u << (i & 31));
+    __syncwarp();
+    int total = 0;
+    const int64_t ob = FILL ? out_rp[i] : 0;
+    for (int w0 = 0; w0 < W; w0 += 32) {
+      const int w = w0 + lane;
+      uint32_t bits = w < W ? bm[w] : 0u;
+      int tot;
+      const int ex = warp_excl_scan_i(__popc(bits), lane, &tot);
+      if (FILL) {
+        int pos = total + ex;
+        while (bits) {
+          const int bpos = __ffs(bits) - 1;
+          bits &= bits - 1;
+          out_col[ob + pos++] = w * 32 + bpos;
+        }
+      }
+      total += tot;
+    }
+    if (!FILL && lane == 0) cnt[i] = total;
+    __syncwarp();
+  }
+}
+
+// ---------------------------------------------------------------- transpose of a pattern (rows left unsorted)
+__global__ void k_transpose_count(int64_t n, const int64_t* __restrict__ rp, const int32_t* __restrict__ col,
+                                  int32_t* __restrict__ cnt) {
+  const int lane = threadIdx.x & 31;
+  const int64_t i = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (i >= n) return;
+  for (int64_t e = rp[i] + lane; e < rp[i + 1]; e += 32) atomicAdd(&cnt[col[e]], 1);
+}
+__global__ void k_transpose_fill(int64_t n, const int64_t* __restrict__ rp, const int32_t* __restrict__ col,
+                                 const int64_t* __restrict__ t_rp, int32_t* __restrict__ cursor,
+                                 int32_t* __restrict__ t_col) {
+  const int lane = threadIdx.x & 31;
+  const int64_t i = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (i >= n) return;
+  for (int64_t e = rp[i] + lane; e < rp[i + 1]; e += 32) {
+    const int j = col[e];
+    const int pos = atomicAdd(&cursor[j], 1);
+    t_col[t_rp[j] + pos] = (int32_t)i;
+  }
+}
+
+// ---------------------------------------------------------------- optional symmetry check of H
+__global__ void k_check_symmetric(int64_t n, const int64_t* __restrict__ rp, const int32_t* __restrict__ col,
+                                  const double* __restrict__ val, int32_t* __restrict__ flag) {
+  const int lane = threadIdx.x & 31;
+  const int64_t i = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (i >= n) return;
+  for (int64_t e = rp[i] + lane; e < rp[i + 1]; e += 32) {
+    const int j = col[e];
+    const double v = val[e];
+    if (j < 0 || j >= n) { atomicOr(flag, 2); continue; }
+    int64_t lo = rp[j], hi = rp[j + 1];
+    while (lo < hi) {
+      const int64_t mid = (lo + hi) >> 1;
+      if (col[mid] < i) lo = mid + 1; else hi = mid;
+    }
+    bool ok = lo < rp[j + 1] && col[lo] == i;
+    if (ok) {
+      const double u = val[lo];
+      ok = fabs(u - v) <= 1e-12 * fmax(fabs(u), fabs(v));
+    } else {
+      ok = (v == 0.0);  // an explicitly stored zero needs no partner
+    }
+    if (!ok) atomicOr(flag, 1);
+  }
+}
+
+int pick_warps(size_t per_warp, int max_warps) {
+  const size_t budget = 200 * 1024;
+  int nw = (int)(budget / (per_warp ? per_warp : 1));
+  if (nw > max_warps) nw = max_warps;
+  return nw;
+}
+
+struct Pattern {  // device CSR (pattern, optionally with values) owned by DevBufs
+  DevBuf rp, col, val;
+  int64_t nnz = 0;
+};
+
+int count_to_rowptr(DevBuf& cnt, int64_t n, DevBuf& rp, int64_t* nnz, cudaStream_t s) {
+  GBE_TRY(rp.alloc((size_t)(n + 1) * 8));
+  GBE_TRY(gbe_exclusive_scan_i32_to_i64(cnt.as<int32_t>(), rp.as<int64_t>(), n, s));
+  GBE_CUDA(cudaMemcpyAsync(nnz, rp.as<int64_t>() + n, 8, cudaMemcpyDeviceToHost, s));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  return GBE_OK;
+}
+
+}  // namespace
+
+int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, int power, int check_sym,
+                      cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S) {
+  const int64_t n = H.n;
+  const int W = (int)((n + 31) / 32);
+  const int rows_grid = (int)((n + 7) / 8);
+  int sm_count = 148;
+  cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, 0);
+
+  if (check_sym) {
+    DevBuf flag;
+    GBE_TRY(flag.alloc(4));
+    GBE_CUDA(cudaMemsetAsync(flag.p, 0, 4, s));
+    k_check_symmetric<<<rows_grid, 256, 0, s>>>(n, H.row_ptr, H.col_idx, H.val, flag.as<int32_t>());
+    GBE_CUDA(cudaGetLastError());
+    int32_t f = 0;
+    GBE_CUDA(cudaMemcpyAsync(&f, flag.p, 4, cudaMemcpyDeviceToHost, s));
+    GBE_CUDA(cudaStreamSynchronize(s));
+    if (f & 2) return GBE_EINVAL;
+    if (f) return GBE_ENOTSYM;
+  }
+
+  DevBuf cnt;
+  GBE_TRY(cnt.alloc((size_t)n * 4));
+
+  // A = floor(X0)_tau, explicit diagonal
+  Pattern A;
+  k_materialise_A<false><<<rows_grid, 256, 0, s>>>(n, H.row_ptr, H.col_idx, H.val, st, tau, cnt.as<int32_t>(), nullptr,
+                                                   nullptr, nullptr);
+  GBE_CUDA(cudaGetLastError());
+  GBE_TRY(count_to_rowptr(cnt, n, A.rp, &A.nnz, s));
+  GBE_TRY(A.col.alloc((size_t)A.nnz * 4));
+  GBE_TRY(A.val.alloc((size_t)A.nnz * 8));
+  k_materialise_A<true><<<rows_grid, 256, 0, s>>>(n, H.row_ptr, H.col_idx, H.val, st, tau, nullptr, A.rp.as<int64_t>(),
+                                                  A.col.as<int32_t>(), A.val.as<double>());
+  GBE_CUDA(cudaGetLastError());
+
+  // pattern accumulator P = I u pat(A)
+  const size_t bm_bytes = (size_t)W * 4;
+  const int uw = pick_warps(bm_bytes, 8);
+  if (uw < 1) return GBE_EINVAL;  // n too large for a shared-memory bitmap
+  GBE_CUDA(cudaFuncSetAttribute(k_union_rows<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bm_bytes * uw)));
+  GBE_CUDA(cudaFuncSetAttribute(k_union_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bm_bytes * uw)));
+  const int ugrid = (int)std::min<int64_t>((n + uw - 1) / uw, (int64_t)sm_count * 8);
+
+  auto do_union = [&](const int64_t* p_rp, const int32_t* p_col, const int64_t* q_rp, const int32_t* q_col, int diag,
+                      Pattern& out) -> int {
+    k_union_rows<false><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, q_rp, q_col, diag, cnt.as<int32_t>(),
+                                                              nullptr, nullptr);
+    GBE_CUDA(cudaGetLastError());
+    GBE_TRY(count_to_rowptr(cnt, n, out.rp, &out.nnz, s));
+    GBE_TRY(out.col.alloc((size_t)out.nnz * 4));
+    k_union_rows<true><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, q_rp, q_col, diag, nullptr,
+                                                             out.rp.as<int64_t>(), out.col.as<int32_t>());
+    GBE_CUDA(cudaGetLastError());
+    return GBE_OK;
+  };
+
+  Pattern P;
+  GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), nullptr, nullptr, 1, P));
+
+  // thresholded powers
+  Pattern Tprev;  // T^(k-1) with values; T^(1) aliases A
+  const int64_t* T_rp = A.rp.as<int64_t>();
+  const int32_t* T_col = A.col.as<int32_t>();
+  const double* T_val = A.val.as<double>();
+  for (int k = 2; k <= power; ++k) {
+    // symbolic: accumulator capacity
+    {
+      const size_t per_warp = (size_t)W * 8;
+      const int nw = pick_warps(per_warp, 8);
+      if (nw < 1) return GBE_EINVAL;
+      GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
+      const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
+      k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, A.rp.as<int64_t>(), A.col.as<int32_t>(),
+                                                                 A.val.as<double>(), T_rp, T_col, T_val, tau,
+                                                                 cnt.as<int32_t>(), nullptr, nullptr, nullptr);
+      GBE_CUDA(cudaGetLastError());
+    }
+    std::vector<int32_t> h_cnt((size_t)n);
+    GBE_CUDA(cudaMemcpyAsync(h_cnt.data(), cnt.p, (size_t)n * 4, cudaMemcpyDeviceToHost, s));
+    GBE_CUDA(cudaStreamSynchronize(s));
+    int cap = 1;
+    for (int64_t i = 0; i < n; ++i) cap = std::max(cap, h_cnt[(size_t)i]);
+    cap = (cap + 1) & ~1;
+    const size_t per_warp = (size_t)W * 8 + (size_t)cap * 8;
+    const int nw = pick_warps(per_warp, 8);
+    if (nw < 1) return GBE_EINVAL;
+    GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
+    GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
+    const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
+    Pattern Tn;
+    k_spgemm_threshold<1><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, A.rp.as<int64_t>(), A.col.as<int32_t>(),
+                                                               A.val.as<double>(), T_rp, T_col, T_val, tau,
+                                                               cnt.as<int32_t>(), nullptr, nullptr, nullptr);
+    GBE_CUDA(cudaGetLastError());
+    GBE_TRY(count_to_rowptr(cnt, n, Tn.rp, &Tn.nnz, s));
+    GBE_TRY(Tn.col.alloc((size_t)Tn.nnz * 4));
+    GBE_TRY(Tn.val.alloc((size_t)Tn.nnz * 8));
+    k_spgemm_threshold<2><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, A.rp.as<int64_t>(), A.col.as<int32_t>(),
+                                                               A.val.as<double>(), T_rp, T_col, T_val, tau, nullptr,
+                                                               Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(),
+                                                               Tn.val.as<double>());
+    GBE_CUDA(cudaGetLastError());
+    Pattern Pn;
+    GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(), 0, Pn));
+    GBE_CUDA(cudaStreamSynchronize(s));
+    std::swap(P.rp.p, Pn.rp.p);
+    std::swap(P.col.p, Pn.col.p);
+    P.nnz = Pn.nnz;
+    std::swap(Tprev.rp.p, Tn.rp.p);
+    std::swap(Tprev.col.p, Tn.col.p);
+    std::swap(Tprev.val.p, Tn.val.p);
+    Tprev.nnz = Tn.nnz;
+    T_rp = Tprev.rp.as<int64_t>();
+    T_col = Tprev.col.as<int32_t>();
+    T_val = Tprev.val.as<double>();
+    // Tn (now holding the previous T) and Pn are released here, after the sync above
+  }
+
+  // S = P u P^T
+  Pattern PT;
+  GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
+  k_transpose_count<<<rows_grid, 256, 0, s>>>(n, P.rp.as<int64_t>(), P.col.as<int32_t>(), cnt.as<int32_t>());
+  GBE_CUDA(cudaGetLastError());
+  GBE_TRY(count_to_rowptr(cnt, n, PT.rp, &PT.nnz, s));
+  GBE_TRY(PT.col.alloc((size_t)PT.nnz * 4));
+  GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
+  k_transpose_fill<<<rows_grid, 256, 0, s>>>(n, P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(),
+                                             cnt.as<int32_t>(), PT.col.as<int32_t>());
+  GBE_CUDA(cudaGetLastError());
+  Pattern S;
+  GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(), PT.col.as<int32_t>(), 0, S));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  *nnz_S = S.nnz;
+  *S_row_ptr = reinterpret_cast<int64_t*>(S.rp.release());
+  *S_col = reinterpret_cast<int32_t*>(S.col.release());
+  return GBE_OK;
+}

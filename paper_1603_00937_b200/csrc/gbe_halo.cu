@@ -1,0 +1,371 @@
+// Step 2 - halo discovery (row 2).
+//
+// For community p with core C_p = {i : part[i] = p} (obs. (vi) P:L65):
+//     s_p = C_p u { k : (k, i) in S_tau, i in C_p }                       (Fig.1)
+// local order: core vertices ascending, then halo vertices ascending.  Also built here, once per graph:
+//   - the padded batched dense layout (ld_p = m_p rounded up to 16 doubles, element offsets),
+//   - the pattern S' of D (A-9): row k holds the core vertices of every community whose subgraph contains k,
+//   - the scatter map: for dense row (p, r) the offset in D.val of the run of its ncore_p core columns
+//     (contiguous when every core is an index range; otherwise a per-entry map),
+//   - the X^2 tile work list (largest communities first) and the gather work list.
+// All set work uses a bitmap over the n vertices in shared memory; walking it emits ascending indices.
+// Bound: integer/latency; runs once per graph.
+#include <algorithm>
+#include <numeric>
+
+#include "gbe_internal.cuh"
+
+namespace {
+
+
+__device__ __forceinline__ int part_of(const int32_t* part, int64_t i, int64_t blk) {
+  return part ? part[i] : (int)(i / blk);
+}
+
+__global__ void k_core_count(int64_t n, const int32_t* __restrict__ part, int64_t blk, int n_part,
+                             int32_t* __restrict__ cnt, int32_t* __restrict__ flag) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int p = part_of(part, i, blk);
+  if (p < 0 || p >= n_part) { atomicOr(flag, 1); return; }
+  atomicAdd(&cnt[p], 1);
+}
+__global__ void k_core_fill(int64_t n, const int32_t* __restrict__ part, int64_t blk, const int64_t* __restrict__ core_ptr,
+                            int32_t* __restrict__ cursor, int32_t* __restrict__ core_tmp) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int p = part_of(part, i, blk);
+  const int pos = atomicAdd(&cursor[p], 1);
+  core_tmp[core_ptr[p] + pos] = (int32_t)i;  // order fixed later by the bitmap walk
+}
+
+// block-wide: emit the set bits of (bm[w] for w < W) in ascending order to out[], returns the count
+__device__ int block_emit_bits(const uint32_t* bm, int W, int32_t* out, int* scratch /* blockDim.x + 1 */) {
+  const int t = threadIdx.x, nt = blockDim.x;
+  const int chunk = (W + nt - 1) / nt;
+  const int b = min(W, t * chunk), e = min(W, b + chunk);
+  int c = 0;
+  for (int w = b; w < e; ++w) c += __popc(bm[w]);
+  scratch[t] = c;
+  __syncthreads();
+  if (t == 0) {
+    int run = 0;
+    for (int k = 0; k < nt; ++k) { const int v = scratch[k]; scratch[k] = run; run += v; }
+    scratch[nt] = run;
+  }
+  __syncthreads();
+  if (out) {
+    int pos = scratch[t];
+    for (int w = b; w < e; ++w) {
+      uint32_t bits = bm[w];
+      while (bits) {
+        const int bp = __ffs(bits) - 1;
+        bits &= bits - 1;
+        out[pos++] = w * 32 + bp;
+      }
+    }
+  }
+  const int total = scratch[nt];
+  __syncthreads();
+  return total;
+}
+
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_halo(int W, const int64_t* __restrict__ core_ptr,
+                                              const int32_t* __restrict__ core_tmp, const int64_t* __restrict__ S_rp,
+                                              const int32_t* __restrict__ S_col, int32_t* __restrict__ msize,
+                                              int32_t* __restrict__ ncore, const int64_t* __restrict__ sub_ptr,
+                                              int32_t* __restrict__ sub_idx, int32_t* __restrict__ row_part) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint32_t* coreb = reinterpret_cast<uint32_t*>(smem_raw);
+  uint32_t* allb = coreb + W;
+  int* scratch = reinterpret_cast<int*>(allb + W);
+  const int p = blockIdx.x, t = threadIdx.x, lane = t & 31, wid = t >> 5;
+  for (int w = t; w < 2 * W; w += 256) coreb[w] = 0u;
+  __syncthreads();
+  const int64_t cb = core_ptr[p], ce = core_ptr[p + 1];
+  for (int64_t c = cb + wid; c < ce; c += 8) {  // warp per core vertex, lanes along its S row
+    const int i = core_tmp[c];
+    if (lane == 0) atomicOr(&coreb[i >> 5], 1u << (i & 31));
+    for (int64_t e = S_rp[i] + lane; e < S_rp[i + 1]; e += 32) {
+      const int k = S_col[e];
+      atomicOr(&allb[k >> 5], 1u << (k & 31));
+    }
+  }
+  __syncthreads();
+  for (int w = t; w < W; w += 256) allb[w] &= ~coreb[w];  // halo = neighbours that are not core
+  __syncthreads();
+  const int64_t ob = FILL ? sub_ptr[p] : 0;
+  const int nc = block_emit_bits(coreb, W, FILL ? sub_idx + ob : nullptr, scratch);
+  const int nh = block_emit_bits(allb, W, FILL ? sub_idx + ob + nc : nullptr, scratch);
+  if (FILL) {
+    for (int r = t; r < nc + nh; r += 256) row_part[ob + r] = p;
+  } else if (t == 0) {
+    msize[p] = nc + nh;
+    ncore[p] = nc;
+  }
+}
+
+// counts for the pattern of D and the membership lists
+__global__ void k_member_count(int64_t sum_m, const int32_t* __restrict__ sub_idx, const int32_t* __restrict__ row_part,
+                               const int32_t* __restrict__ ncore, int32_t* __restrict__ cntD, int32_t* __restrict__ mcnt) {
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= sum_m) return;
+  const int k = sub_idx[q];
+  atomicAdd(&cntD[k], ncore[row_part[q]]);
+  atomicAdd(&mcnt[k], 1);
+}
+__global__ void k_member_fill(int64_t sum_m, const int32_t* __restrict__ sub_idx, const int64_t* __restrict__ memb_ptr,
+                              int32_t* __restrict__ cursor, int64_t* __restrict__ memb) {
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= sum_m) return;
+  const int k = sub_idx[q];
+  const int pos = atomicAdd(&cursor[k], 1);
+  memb[memb_ptr[k] + pos] = q;
+}
+__global__ void k_row_ncore(int64_t sum_m, const int32_t* __restrict__ row_part, const int32_t* __restrict__ ncore,
+                            int32_t* __restrict__ out) {
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q < sum_m) out[q] = ncore[row_part[q]];
+}
+
+// warp per row k of D: columns = union of the cores of the communities containing k, ascending; scatter offsets.
+// MODE 0: D_col + scat_base + contiguity flag; MODE 1: per-entry scat_pos.
+template <int MODE>
+__global__ void k_d_pattern(int64_t n, int W, const int64_t* __restrict__ memb_ptr, const int64_t* __restrict__ memb,
+                            const int32_t* __restrict__ row_part, const int64_t* __restrict__ sub_ptr,
+                            const int32_t* __restrict__ sub_idx, const int32_t* __restrict__ ncore,
+                            const int64_t* __restrict__ D_rp, int32_t* __restrict__ D_col,
+                            int64_t* __restrict__ scat_base, int32_t* __restrict__ noncontig,
+                            const int64_t* __restrict__ scat_ofs, int64_t* __restrict__ scat_pos) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, w_in_blk = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  uint32_t* bm = reinterpret_cast<uint32_t*>(smem_raw) + (size_t)2 * W * w_in_blk;
+  uint32_t* rk = bm + W;
+  for (int64_t k = (int64_t)blockIdx.x * nw + w_in_blk; k < n; k += (int64_t)gridDim.x * nw) {
+    for (int w = lane; w < W; w += 32) bm[w] = 0u;
+    __syncwarp();
+    const int64_t mb = memb_ptr[k], me = memb_ptr[k + 1];
+    for (int64_t x = mb; x < me; ++x) {
+      const int p = row_part[memb[x]];
+      const int64_t sb = sub_ptr[p];
+      const int nc = ncore[p];
+      for (int c = lane; c < nc; c += 32) { const int i = sub_idx[sb + c]; atomicOr(&bm[i >> 5], 1u << (i & 31)); }
+    }
+    __syncwarp();
+    int running = 0;
+    const int64_t ob = D_rp[k];
+    for (int w0 = 0; w0 < W; w0 += 32) {
+      const int w = w0 + lane;
+      uint32_t bits = w < W ? bm[w] : 0u;
+      int tot;
+      const int ex = warp_excl_scan_i(__popc(bits), lane, &tot);
+      if (w < W) rk[w] = running + ex;
+      if (MODE == 0) {
+        int pos = running + ex;
+        while (bits) {
+          const int bp = __ffs(bits) - 1;
+          bits &= bits - 1;
+          D_col[ob + pos++] = w * 32 + bp;
+        }
+      }
+      running += tot;
+    }
+    __syncwarp();
+    for (int64_t x = mb; x < me; ++x) {
+      const int64_t q = memb[x];
+      const int p = row_part[q];
+      const int64_t sb = sub_ptr[p];
+      const int nc = ncore[p];
+      const int first = sub_idx[sb];
+      const int pos0 = rk[first >> 5] + __popc(bm[first >> 5] & ((1u << (first & 31)) - 1u));
+      if (MODE == 0 && lane == 0) scat_base[q] = ob + pos0;
+      for (int c = lane; c < nc; c += 32) {
+        const int i = sub_idx[sb + c];
+        const int pos = rk[i >> 5] + __popc(bm[i >> 5] & ((1u << (i & 31)) - 1u));
+        if (MODE == 0) {
+          if (pos != pos0 + c) atomicOr(noncontig, 1);
+        } else {
+          scat_pos[scat_ofs[q] + c] = ob + pos;
+        }
+      }
+    }
+    __syncwarp();
+  }
+}
+
+template <typename T>
+int upload(const std::vector<T>& h, T** d, cudaStream_t s) {
+  cudaError_t e = cudaMalloc((void**)d, std::max<size_t>(16, h.size() * sizeof(T)));
+  if (e != cudaSuccess) { gbe_set_cuda_error(e, "cudaMalloc", __LINE__); return GBE_ENOMEM; }
+  if (!h.empty()) GBE_CUDA(cudaMemcpyAsync(*d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, s));
+  return GBE_OK;
+}
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
+  const int64_t n = g->n;
+  const int n_part = g->n_part;
+  const int W = (int)((n + 31) / 32);
+  const int64_t blk = (n + n_part - 1) / n_part;
+  int sm_count = 148;
+  cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, 0);
+  const int tgrid = (int)((n + 255) / 256);
+
+  // ---- cores
+  DevBuf cnt, flag, core_tmp, cursor;
+  GBE_TRY(cnt.alloc((size_t)std::max<int64_t>(n_part, n) * 4));
+  GBE_TRY(flag.alloc(4));
+  GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n_part * 4, s));
+  GBE_CUDA(cudaMemsetAsync(flag.p, 0, 4, s));
+  k_core_count<<<tgrid, 256, 0, s>>>(n, part, blk, n_part, cnt.as<int32_t>(), flag.as<int32_t>());
+  GBE_CUDA(cudaGetLastError());
+  int32_t hflag = 0;
+  GBE_CUDA(cudaMemcpyAsync(&hflag, flag.p, 4, cudaMemcpyDeviceToHost, s));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  if (hflag) return GBE_EINVAL;  // partition id out of range
+  DevBuf core_ptr;
+  GBE_TRY(core_ptr.alloc((size_t)(n_part + 1) * 8));
+  GBE_TRY(gbe_exclusive_scan_i32_to_i64(cnt.as<int32_t>(), core_ptr.as<int64_t>(), n_part, s));
+  GBE_TRY(core_tmp.alloc((size_t)n * 4));
+  GBE_TRY(cursor.alloc((size_t)std::max<int64_t>(n_part, n) * 4));
+  GBE_CUDA(cudaMemsetAsync(cursor.p, 0, (size_t)n_part * 4, s));
+  k_core_fill<<<tgrid, 256, 0, s>>>(n, part, blk, core_ptr.as<int64_t>(), cursor.as<int32_t>(), core_tmp.as<int32_t>());
+  GBE_CUDA(cudaGetLastError());
+
+  // ---- halo: count, then fill
+  const size_t halo_smem = (size_t)2 * W * 4 + 257 * 4;
+  if (halo_smem > 220 * 1024) return GBE_EINVAL;  // n too large for the shared-memory bitmaps
+  GBE_CUDA(cudaFuncSetAttribute(k_halo<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)halo_smem));
+  GBE_CUDA(cudaFuncSetAttribute(k_halo<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)halo_smem));
+  GBE_CUDA(cudaMalloc((void**)&g->msize, (size_t)n_part * 4));
+  GBE_CUDA(cudaMalloc((void**)&g->ncore, (size_t)n_part * 4));
+  k_halo<false><<<n_part, 256, halo_smem, s>>>(W, core_ptr.as<int64_t>(), core_tmp.as<int32_t>(), g->S_row_ptr, g->S_col,
+                                               g->msize, g->ncore, nullptr, nullptr, nullptr);
+  GBE_CUDA(cudaGetLastError());
+  g->h_m.resize(n_part);
+  g->h_ncore.resize(n_part);
+  GBE_CUDA(cudaMemcpyAsync(g->h_m.data(), g->msize, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
+  GBE_CUDA(cudaMemcpyAsync(g->h_ncore.data(), g->ncore, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
+  GBE_CUDA(cudaStreamSynchronize(s));
+
+  // ---- host: layout, work lists
+  std::vector<int64_t> h_sub_ptr(n_part + 1, 0);
+  g->h_dense_off.assign(n_part + 1, 0);
+  g->max_m = 0;
+  g->max_ncore = 0;
+  g->nnz_D = 0;
+  g->flops_per_iter = 0;
+  for (int p = 0; p < n_part; ++p) {
+    const int64_t m = g->h_m[p];
+    const int64_t ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+    h_sub_ptr[p + 1] = h_sub_ptr[p] + m;
+    g->h_dense_off[p + 1] = g->h_dense_off[p] + m * ld;
+    g->max_m = std::max<int32_t>(g->max_m, (int32_t)m);
+    g->max_ncore = std::max<int32_t>(g->max_ncore, g->h_ncore[p]);
+    g->nnz_D += m * g->h_ncore[p];
+    g->flops_per_iter += 2.0 * (double)m * (double)m * (double)m;
+  }
+  g->sum_m = h_sub_ptr[n_part];
+  g->dense_elems = g->h_dense_off[n_part];
+  GBE_TRY(upload(h_sub_ptr, &g->sub_ptr, s));
+  GBE_TRY(upload(g->h_dense_off, &g->dense_off, s));
+
+  // X^2 tile list: communities by decreasing m (longest work first), the tiles of one community adjacent
+  // so that its panels are reused from L2 by the CTAs that run together.
+  {
+    std::vector<int32_t> order(n_part);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return g->h_m[a] > g->h_m[b]; });
+    std::vector<gbe_tile_item> items;
+    const int tile = g->tile;
+    for (int p : order) {
+      const int T = (g->h_m[p] + tile - 1) / tile;
+      for (int ti = 0; ti < T; ++ti)
+        for (int tj = ti; tj < T; ++tj) items.push_back({p, ti, tj, 0});
+    }
+    g->n_items = (int32_t)items.size();
+    GBE_TRY(upload(items, &g->items, s));
+  }
+  {
+    g->gather_rows = 64;
+    std::vector<int2> gi;
+    for (int p = 0; p < n_part; ++p)
+      for (int r0 = 0; r0 < g->h_m[p]; r0 += g->gather_rows) gi.push_back(make_int2(p, r0));
+    g->n_gitems = (int32_t)gi.size();
+    GBE_TRY(upload(gi, &g->gitems, s));
+  }
+  g->n_partials = std::max(g->n_items, g->n_gitems);
+
+  // workspace layout
+  size_t off = align_up(sizeof(gbe_state), 256);
+  g->ws_bounds = off;
+  off += align_up(2 * 1024 * sizeof(double), 256);
+  g->ws_partials = off;
+  off += align_up((size_t)std::max(1, g->n_partials) * 2 * sizeof(double), 256);
+  g->ws_x0 = off;
+  off += align_up((size_t)g->dense_elems * 8, 256);
+  g->ws_x1 = off;
+  off += align_up((size_t)g->dense_elems * 8, 256);
+  g->ws_bytes = off;
+
+  // ---- fill sub_idx / row_part
+  GBE_CUDA(cudaMalloc((void**)&g->sub_idx, std::max<size_t>(16, (size_t)g->sum_m * 4)));
+  GBE_CUDA(cudaMalloc((void**)&g->row_part, std::max<size_t>(16, (size_t)g->sum_m * 4)));
+  k_halo<true><<<n_part, 256, halo_smem, s>>>(W, core_ptr.as<int64_t>(), core_tmp.as<int32_t>(), g->S_row_ptr, g->S_col,
+                                              nullptr, nullptr, g->sub_ptr, g->sub_idx, g->row_part);
+  GBE_CUDA(cudaGetLastError());
+
+  // ---- pattern of D and scatter map
+  const int64_t sum_m = g->sum_m;
+  const int qgrid = (int)std::max<int64_t>(1, (sum_m + 255) / 256);
+  DevBuf mcnt, memb_ptr, memb;
+  GBE_TRY(mcnt.alloc((size_t)n * 4));
+  GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
+  GBE_CUDA(cudaMemsetAsync(mcnt.p, 0, (size_t)n * 4, s));
+  k_member_count<<<qgrid, 256, 0, s>>>(sum_m, g->sub_idx, g->row_part, g->ncore, cnt.as<int32_t>(), mcnt.as<int32_t>());
+  GBE_CUDA(cudaGetLastError());
+  GBE_CUDA(cudaMalloc((void**)&g->D_row_ptr, (size_t)(n + 1) * 8));
+  GBE_TRY(gbe_exclusive_scan_i32_to_i64(cnt.as<int32_t>(), g->D_row_ptr, n, s));
+  GBE_TRY(memb_ptr.alloc((size_t)(n + 1) * 8));
+  GBE_TRY(gbe_exclusive_scan_i32_to_i64(mcnt.as<int32_t>(), memb_ptr.as<int64_t>(), n, s));
+  GBE_TRY(memb.alloc(std::max<size_t>(16, (size_t)sum_m * 8)));
+  GBE_CUDA(cudaMemsetAsync(cursor.p, 0, (size_t)n * 4, s));
+  k_member_fill<<<qgrid, 256, 0, s>>>(sum_m, g->sub_idx, memb_ptr.as<int64_t>(), cursor.as<int32_t>(), memb.as<int64_t>());
+  GBE_CUDA(cudaGetLastError());
+  GBE_CUDA(cudaMalloc((void**)&g->D_col, std::max<size_t>(16, (size_t)g->nnz_D * 4)));
+  GBE_CUDA(cudaMalloc((void**)&g->scat_base, std::max<size_t>(16, (size_t)sum_m * 8)));
+  const size_t per_warp = (size_t)2 * W * 4;
+  int nw = (int)std::min<size_t>(8, (200 * 1024) / per_warp);
+  if (nw < 1) return GBE_EINVAL;
+  GBE_CUDA(cudaFuncSetAttribute(k_d_pattern<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
+  GBE_CUDA(cudaFuncSetAttribute(k_d_pattern<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
+  const int dgrid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
+  GBE_CUDA(cudaMemsetAsync(flag.p, 0, 4, s));
+  k_d_pattern<0><<<dgrid, nw * 32, per_warp * nw, s>>>(n, W, memb_ptr.as<int64_t>(), memb.as<int64_t>(), g->row_part,
+                                                       g->sub_ptr, g->sub_idx, g->ncore, g->D_row_ptr, g->D_col,
+                                                       g->scat_base, flag.as<int32_t>(), nullptr, nullptr);
+  GBE_CUDA(cudaGetLastError());
+  GBE_CUDA(cudaMemcpyAsync(&hflag, flag.p, 4, cudaMemcpyDeviceToHost, s));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  g->contiguous = hflag ? 0 : 1;
+  if (!g->contiguous) {
+    DevBuf rn, scat_ofs;
+    GBE_TRY(rn.alloc(std::max<size_t>(16, (size_t)sum_m * 4)));
+    k_row_ncore<<<qgrid, 256, 0, s>>>(sum_m, g->row_part, g->ncore, rn.as<int32_t>());
+    GBE_CUDA(cudaGetLastError());
+    GBE_TRY(scat_ofs.alloc((size_t)(sum_m + 1) * 8));
+    GBE_TRY(gbe_exclusive_scan_i32_to_i64(rn.as<int32_t>(), scat_ofs.as<int64_t>(), sum_m, s));
+    GBE_CUDA(cudaMalloc((void**)&g->scat_pos, std::max<size_t>(16, (size_t)g->nnz_D * 8)));
+    k_d_pattern<1><<<dgrid, nw * 32, per_warp * nw, s>>>(n, W, memb_ptr.as<int64_t>(), memb.as<int64_t>(), g->row_part,
+                                                         g->sub_ptr, g->sub_idx, g->ncore, g->D_row_ptr, nullptr, nullptr,
+                                                         nullptr, scat_ofs.as<int64_t>(), g->scat_pos);
+    GBE_CUDA(cudaGetLastError());
+    GBE_CUDA(cudaStreamSynchronize(s));
+    g->scat_ofs = reinterpret_cast<int64_t*>(scat_ofs.release());
+  }
+  GBE_CUDA(cudaStreamSynchronize(s));
+  return GBE_OK;
+}

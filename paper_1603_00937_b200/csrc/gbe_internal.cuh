@@ -1,0 +1,156 @@
+// Internal declarations shared by the kernels of the hot path (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "gbe.h"
+
+// ----------------------------------------------------------------------------------------------
+// error plumbing
+// ----------------------------------------------------------------------------------------------
+void gbe_set_cuda_error(cudaError_t e, const char* what, int line);
+#define GBE_CUDA(call)                                   \
+  do {                                                   \
+    cudaError_t e__ = (call);                            \
+    if (e__ != cudaSuccess) {                            \
+      gbe_set_cuda_error(e__, #call, __LINE__);          \
+      return GBE_ECUDA;                                  \
+    }                                                    \
+  } while (0)
+#define GBE_TRY(call)          \
+  do {                         \
+    int s__ = (call);          \
+    if (s__ != GBE_OK) return s__; \
+  } while (0)
+
+// scoped device allocation for build-time temporaries
+struct DevBuf {
+  void* p = nullptr;
+  DevBuf() = default;
+  DevBuf(const DevBuf&) = delete;
+  DevBuf& operator=(const DevBuf&) = delete;
+  ~DevBuf() { if (p) cudaFree(p); }
+  template <typename T> T* as() { return reinterpret_cast<T*>(p); }
+  int alloc(size_t bytes) {
+    if (p) { cudaFree(p); p = nullptr; }
+    cudaError_t e = cudaMalloc(&p, bytes ? bytes : 16);
+    if (e != cudaSuccess) { gbe_set_cuda_error(e, "cudaMalloc", __LINE__); p = nullptr; return GBE_ENOMEM; }
+    return GBE_OK;
+  }
+  void* release() { void* q = p; p = nullptr; return q; }
+};
+
+// ----------------------------------------------------------------------------------------------
+// layout constants
+// ----------------------------------------------------------------------------------------------
+constexpr int GBE_LD_ALIGN = 16;  // leading dimension of a dense block: m rounded up to 16 doubles (128 B rows)
+constexpr int GBE_KC = 16;        // K chunk of the X^2 pipeline (one 128-byte line per row)
+
+// Device-resident state of one gbe_density run: lives at the start of the workspace.
+struct gbe_state {
+  double eps_min, eps_max;  // Gershgorin bounds of the current H (step 0)
+  double n_occ, idem_tol;
+  int32_t iters;       // requested iterations
+  int32_t iter;        // index n of the X_n the partials currently describe
+  int32_t branch;      // branch chosen for iteration `iter` (0: X^2, 1: 2X - X^2)
+  int32_t stop;        // 1 once the idempotency stop fired (A-7) or `iters` iterations are done
+  int32_t iters_done;  // number of updates applied; the final X lives in buffer iters_done & 1
+  int32_t degenerate;  // eps_max == eps_min
+  int32_t pad_[2];
+  double t1[GBE_MAX_ITERS + 1];
+  double t2[GBE_MAX_ITERS + 1];
+  uint8_t br[GBE_MAX_ITERS];
+};
+
+struct gbe_tile_item {  // one X^2 work item: tile (ti, tj), ti <= tj, of community p
+  int32_t p, ti, tj, pad;
+};
+
+// ----------------------------------------------------------------------------------------------
+// the graph handle
+// ----------------------------------------------------------------------------------------------
+struct gbe_graph {
+  int64_t n = 0, nnz_S = 0, sum_m = 0, nnz_D = 0, dense_elems = 0;
+  int32_t n_part = 0, max_m = 0, max_ncore = 0, tile = 128;
+  double eps_min = 0, eps_max = 0, tau = 0, flops_per_iter = 0;
+  int32_t power = 2, contiguous = 1;
+  // device arrays (owned)
+  int64_t* S_row_ptr = nullptr;  // n+1
+  int32_t* S_col = nullptr;      // nnz_S
+  int64_t* sub_ptr = nullptr;    // n_part+1
+  int32_t* sub_idx = nullptr;    // sum_m: core ascending then halo ascending
+  int32_t* ncore = nullptr;      // n_part
+  int32_t* msize = nullptr;      // n_part: m_p
+  int64_t* dense_off = nullptr;  // n_part+1, element offset of X_p in a dense buffer
+  int64_t* D_row_ptr = nullptr;  // n+1
+  int32_t* D_col = nullptr;      // nnz_D
+  int64_t* scat_base = nullptr;  // sum_m: D.val offset of the run (p, r), contiguous-core case
+  int64_t* scat_pos = nullptr;   // nnz_D: D.val offset of (p, r, c), general case (else null)
+  int64_t* scat_ofs = nullptr;   // sum_m+1: offset of dense row q in scat_pos (general case)
+  int32_t* row_part = nullptr;   // sum_m: community of dense row q
+  gbe_tile_item* items = nullptr;
+  int32_t n_items = 0;
+  int2* gitems = nullptr;  // gather work items (p, first row)
+  int32_t n_gitems = 0, gather_rows = 0;
+  // workspace layout (byte offsets)
+  size_t ws_partials = 0, ws_bounds = 0, ws_x0 = 0, ws_x1 = 0, ws_bytes = 0;
+  int32_t n_partials = 0;
+  // host mirrors
+  std::vector<int32_t> h_m, h_ncore;
+  std::vector<int64_t> h_dense_off;
+};
+
+// ----------------------------------------------------------------------------------------------
+// kernel launchers (each file holds one step of DESIGN.md section 1)
+// ----------------------------------------------------------------------------------------------
+// step 0
+int gbe_launch_bounds(const gbe_csr_view& H, double* block_lo, double* block_hi, int max_blocks, gbe_state* st,
+                      cudaStream_t s);
+// step 1
+int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st_dev, double tau, int power, int check_sym,
+                      cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S);
+// step 2
+int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s);
+// step 3
+int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state* st, double* X, double* partials,
+                      cudaStream_t s);
+// step 4
+int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
+                  cudaStream_t s);
+// step 5
+int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s);
+// step 6
+int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0, const double* X1, double* D_val,
+                       cudaStream_t s);
+
+// small device utilities (gbe_util.cu)
+int gbe_exclusive_scan_i64(const int64_t* in, int64_t* out, int64_t n, cudaStream_t s);  // out has n+1 entries
+int gbe_exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s);
+
+// ----------------------------------------------------------------------------------------------
+// device helpers
+// ----------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ int warp_sum_i(int v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ int warp_excl_scan_i(int v, int lane, int* total) {
+  int x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int y = __shfl_up_sync(0xffffffffu, x, o);
+    if (lane >= o) x += y;
+  }
+  *total = __shfl_sync(0xffffffffu, x, 31);
+  return x - v;
+}
+#endif

@@ -1,0 +1,55 @@
+// Step 6 - core-column scatter (row 6).
+//
+//     D[s_p[r], s_p[c]] = (X_p)[r, c],  r < m_p, c < ncore_p                                (A-9, A-10)
+// Column i of P_tau(H) is column j of P(x[s]) (Eq.(6)); P(x[s]) is symmetric, so the kernel reads ROW
+// segments instead (contiguous): for dense row (p, r) the ncore_p leading entries go to one contiguous run of
+// D.val when every core is an index range, else through a per-entry position map.  D is NOT symmetrised
+// (obs. (i) P:L65).  The final X lives in buffer (iters_done & 1), read from the device state.
+// Bound: HBM - 8 B read + 8 B written per stored entry of D (+ 8 B map in the general case).
+#include "gbe_internal.cuh"
+
+namespace {
+template <bool CONTIG>
+__global__ void __launch_bounds__(256) k_scatter(int64_t sum_m, const int32_t* __restrict__ row_part,
+                                                 const int64_t* __restrict__ sub_ptr, const int32_t* __restrict__ ncore,
+                                                 const int64_t* __restrict__ dense_off,
+                                                 const int64_t* __restrict__ scat_base,
+                                                 const int64_t* __restrict__ scat_ofs,
+                                                 const int64_t* __restrict__ scat_pos, const gbe_state* __restrict__ st,
+                                                 const double* __restrict__ X0, const double* __restrict__ X1,
+                                                 double* __restrict__ D_val) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warp = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5), nwarps = (int64_t)gridDim.x * 8;
+  const double* __restrict__ X = (st->iters_done & 1) ? X1 : X0;
+  for (int64_t q = warp; q < sum_m; q += nwarps) {
+    const int p = row_part[q];
+    const int64_t sb = sub_ptr[p];
+    const int m = (int)(sub_ptr[p + 1] - sb);
+    const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+    const int nc = ncore[p];
+    const double* src = X + dense_off[p] + (size_t)(q - sb) * ld;
+    if (CONTIG) {
+      double* dst = D_val + scat_base[q];
+      for (int c = lane; c < nc; c += 32) dst[c] = src[c];
+    } else {
+      const int64_t* pos = scat_pos + scat_ofs[q];
+      for (int c = lane; c < nc; c += 32) D_val[pos[c]] = src[c];
+    }
+  }
+}
+}  // namespace
+
+int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0, const double* X1, double* D_val,
+                       cudaStream_t s) {
+  if (g->sum_m == 0) return GBE_OK;
+  const int64_t want = (g->sum_m + 7) / 8;
+  const int grid = (int)std::min<int64_t>(want, 148 * 64);
+  if (g->contiguous)
+    k_scatter<true><<<grid, 256, 0, s>>>(g->sum_m, g->row_part, g->sub_ptr, g->ncore, g->dense_off, g->scat_base, nullptr,
+                                         nullptr, st, X0, X1, D_val);
+  else
+    k_scatter<false><<<grid, 256, 0, s>>>(g->sum_m, g->row_part, g->sub_ptr, g->ncore, g->dense_off, nullptr, g->scat_ofs,
+                                          g->scat_pos, st, X0, X1, D_val);
+  GBE_CUDA(cudaGetLastError());
+  return GBE_OK;
+}

@@ -1,0 +1,54 @@
+// Step 5 - global trace and SP2 branch choice (row 5).
+//
+//     t1 = sum_p sum_{i<ncore_p} (X_n)_ii,   t2 = sum_p sum_{i<ncore_p} (X_n^2)_ii      (fixed-order reduction)
+//     [idem_tol >= 0 and n >= 1 and |t1 - t2| <= idem_tol: stop]                          (A-7)
+//     branch_n = X^2 if |t2 - n_occ| < |2 t1 - t2 - n_occ| else 2X - X^2 (tie -> 2X - X^2)  (A-6)
+// One polynomial for every subgraph (Eq.(4); "the same for each subgraph expansion ... for the correct
+// total occupation").  The paper pre-sets the sequence from a gap estimate (ref. 41); north_star
+// asks for the choice from the global trace, taken on the device with no host round trip.
+// A single CTA sums the per-work-item partials in a fixed order (no floating-point atomics): reproducible.
+// Bound: latency (16 B per partial).
+#include "gbe_internal.cuh"
+
+namespace {
+constexpr int TB = 1024;
+
+__global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double* __restrict__ partials, int n) {
+  __shared__ double s1[TB], s2[TB];
+  const int t = threadIdx.x;
+  if (st->stop) return;
+  double a1 = 0.0, a2 = 0.0;
+  for (int i = t; i < n; i += TB) {
+    a1 += partials[2 * (size_t)i];
+    a2 += partials[2 * (size_t)i + 1];
+  }
+  s1[t] = a1;
+  s2[t] = a2;
+  __syncthreads();
+  for (int o = TB / 2; o > 0; o >>= 1) {
+    if (t < o) { s1[t] += s1[t + o]; s2[t] += s2[t + o]; }
+    __syncthreads();
+  }
+  if (t == 0) {
+    const double t1 = s1[0], t2 = s2[0], n_occ = st->n_occ;
+    const int k = st->iter;  // the partials describe X_k
+    st->t1[k] = t1;
+    st->t2[k] = t2;
+    st->iters_done = k;
+    if (k >= st->iters || (st->idem_tol >= 0.0 && k >= 1 && fabs(t1 - t2) <= st->idem_tol)) {
+      st->stop = 1;
+    } else {
+      const int b = (fabs(t2 - n_occ) < fabs(2.0 * t1 - t2 - n_occ)) ? 0 : 1;
+      st->branch = b;
+      st->br[k] = (uint8_t)b;
+      st->iter = k + 1;
+    }
+  }
+}
+}  // namespace
+
+int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s) {
+  k_trace_branch<<<1, TB, 0, s>>>(st, partials, n_partials);
+  GBE_CUDA(cudaGetLastError());
+  return GBE_OK;
+}

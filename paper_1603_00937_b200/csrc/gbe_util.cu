@@ -1,0 +1,42 @@
+// Small device utilities: exclusive scans used while sizing CSR outputs (not on the per-iteration path).
+#include "gbe_internal.cuh"
+
+namespace {
+template <typename TI>
+__global__ void __launch_bounds__(1024) k_scan_single_block(const TI* __restrict__ in, int64_t* __restrict__ out,
+                                                            int64_t n) {
+  __shared__ int64_t part[1024];
+  const int t = threadIdx.x;
+  const int64_t chunk = (n + 1023) / 1024;
+  const int64_t b = (int64_t)t * chunk, e = min(n, b + chunk);
+  int64_t s = 0;
+  for (int64_t i = b; i < e; ++i) s += (int64_t)in[i];
+  part[t] = s;
+  __syncthreads();
+  // Hillis-Steele inclusive scan over the 1024 chunk sums
+  for (int o = 1; o < 1024; o <<= 1) {
+    int64_t v = (t >= o) ? part[t - o] : 0;
+    __syncthreads();
+    part[t] += v;
+    __syncthreads();
+  }
+  int64_t run = part[t] - s;
+  for (int64_t i = b; i < e; ++i) {
+    int64_t v = (int64_t)in[i];
+    out[i] = run;
+    run += v;
+  }
+  if (t == 1023) out[n] = part[1023];
+}
+}  // namespace
+
+int gbe_exclusive_scan_i64(const int64_t* in, int64_t* out, int64_t n, cudaStream_t s) {
+  k_scan_single_block<int64_t><<<1, 1024, 0, s>>>(in, out, n);
+  GBE_CUDA(cudaGetLastError());
+  return GBE_OK;
+}
+int gbe_exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s) {
+  k_scan_single_block<int32_t><<<1, 1024, 0, s>>>(in, out, n);
+  GBE_CUDA(cudaGetLastError());
+  return GBE_OK;
+}

@@ -1,0 +1,256 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): integer/index work bit-exact; max|D_gpu - D_oracle| <= 1e-10;
+|Tr D_gpu - Tr D_oracle| <= 1e-8.  The oracle builds its OWN graph from the same H; the two graphs are
+compared first (set equality - an edge whose value sits within rounding of tau may differ, reading A-8;
+on these seeded inputs none does) and no oracle input comes from the CUDA path.
+"""
+import numpy as np
+import pytest
+import scipy.sparse as sp
+
+import gbe_inputs as gi
+import oracle as o
+
+pytestmark = pytest.mark.gpu
+
+TOL_D = 1e-10
+TOL_TR = 1e-8
+
+
+@pytest.fixture(scope="module")
+def gbe():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1603_00937_b200 import build
+    build.build()
+    import paper_1603_00937_b200 as pkg
+    pkg.lib()  # fails loudly if the CUDA library is missing
+    return pkg
+
+
+def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None):
+    import torch
+    Hd = gbe.DeviceCSR.from_host(s.H if H is None else H)
+    part_t = None if part is None else torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
+    g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part, power=power)
+    D, log = gbe.gbe_density(Hd, g, s.n_occ, s.iters if iters is None else iters, idem_tol)
+    torch.cuda.synchronize()
+    ex = {k: v.cpu().numpy() for k, v in g.export().items()}
+    return g, ex, D.cpu().numpy(), log
+
+
+def run_oracle(s, iters=None, idem_tol=-1.0, power=2, H=None):
+    H = s.H if H is None else H
+    rp, ci = o.build_graph(H, s.tau, power=power)
+    return (rp, ci), o.o_sub(H, rp, ci, s.part, s.n_part, s.n_occ, s.iters if iters is None else iters, idem_tol)
+
+
+def check_structure(ex, graph, r, info):
+    rp, ci = graph
+    assert np.array_equal(ex["S_row_ptr"], rp) and np.array_equal(ex["S_col"], ci)
+    sub_ptr = np.concatenate([[0], np.cumsum([len(i) for i, _ in r.subs])])
+    assert np.array_equal(ex["sub_ptr"], sub_ptr)
+    assert np.array_equal(ex["sub_idx"], np.concatenate([i for i, _ in r.subs]) if len(r.subs) else [])
+    assert np.array_equal(ex["ncore"], [nc for _, nc in r.subs])
+    assert np.array_equal(ex["D_row_ptr"], r.D_row_ptr) and np.array_equal(ex["D_col"], r.D_col)
+    assert info["nnz_D"] == r.D_val.size and info["sum_m"] == sub_ptr[-1]
+    assert info["max_m"] == max(len(i) for i, _ in r.subs)
+    assert abs(info["eps_min"] - r.eps_min) <= 1e-13 * abs(r.eps_min)
+    assert abs(info["eps_max"] - r.eps_max) <= 1e-13 * abs(r.eps_max)
+    assert abs(info["sp2_flops_per_iter"] - sum(2.0 * len(i) ** 3 for i, _ in r.subs)) < 1e-6 * info["sp2_flops_per_iter"]
+
+
+def check_density(Dg, log, r, compare_all_branches=True):
+    assert log.iters_done == r.iters_done
+    live = np.abs(r.t1[:-1] - r.t2[:-1]) > 1e-9  # A-8: once idempotent either branch is a no-op
+    assert np.array_equal(log.branch[live[:log.iters_done]], r.branch[live[:r.iters_done]])
+    if compare_all_branches:
+        assert np.array_equal(log.branch, r.branch)
+    assert np.abs(log.t1 - r.t1).max() <= TOL_TR and np.abs(log.t2 - r.t2).max() <= TOL_TR
+    assert np.abs(Dg - r.D_val).max() <= TOL_D
+    assert abs(Dg.sum() * 0 + log.t1[-1] - r.t1[-1]) <= TOL_TR
+
+
+# ------------------------------------------------------------------------------- main configurations
+def test_config1_chain(gbe):
+    s = gi.config(1)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+    assert g.info["contiguous_cores"] == 1
+    # trace of the assembled D equals the logged core trace
+    D = sp.csr_matrix((Dg, ex["D_col"], ex["D_row_ptr"]), shape=(s.n, s.n))
+    assert abs(D.diagonal().sum() - log.t1[-1]) < 1e-9
+
+
+def test_config1_default_partition_is_contiguous_blocks(gbe):
+    s = gi.config(1)
+    g, ex, Dg, log = run_gpu(gbe, s, part=None)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+
+
+@pytest.mark.parametrize("seed", [0, 1])
+def test_shuffled_communities_general_scatter(gbe, seed):
+    s = gi.random_banded(200, half_bw=5, n_part=7, seed=seed, tau=1e-4, iters=30, shuffle=True)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+    assert g.info["contiguous_cores"] == 0
+
+
+def test_config2_water_1024(gbe):
+    s = gi.config(2)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r, compare_all_branches=False)
+    m = np.diff(ex["sub_ptr"])
+    assert m.min() > 128 and m.max() > 512  # several tiles and a ragged tail per community
+
+
+# ------------------------------------------------------------------------------- pieces
+def test_iters_zero_returns_gathered_x0(gbe):
+    """gather + scatter alone: D = core columns of X0[s,s]; exact up to the rounding of the two bounds."""
+    s = gi.random_banded(150, half_bw=4, n_part=5, seed=3, tau=1e-3)
+    g, ex, Dg, log = run_gpu(gbe, s, iters=0)
+    graph, r = run_oracle(s, iters=0)
+    check_structure(ex, graph, r, g.info)
+    assert log.iters_done == 0 and log.t1.size == 1
+    assert np.abs(Dg - r.D_val).max() <= 4e-16
+    assert abs(log.t1[0] - r.t1[0]) < 1e-12 and abs(log.t2[0] - r.t2[0]) < 1e-12
+
+
+@pytest.mark.parametrize("power", [1, 3])
+def test_graph_power(gbe, power):
+    s = gi.random_banded(120, half_bw=3, n_part=4, seed=5, tau=1e-3, iters=25)
+    g, ex, Dg, log = run_gpu(gbe, s, power=power)
+    graph, r = run_oracle(s, power=power)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+
+
+@pytest.mark.parametrize("tau", [1e-1, 1e-3, 1e-7, 0.0, 1.5])
+def test_tau_sweep_chain(gbe, tau):
+    s = gi.chain(256, 8, tau=tau, iters=30)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+    if tau > 1:
+        assert g.info["nnz_S"] == s.n  # self loops only (A-12)
+
+
+def test_idem_tol_stops_on_device(gbe):
+    s = gi.config(1)
+    g, ex, Dg, log = run_gpu(gbe, s, iters=60, idem_tol=1e-9)
+    graph, r = run_oracle(s, iters=60, idem_tol=1e-9)
+    assert 15 < log.iters_done < 40
+    check_density(Dg, log, r)
+
+
+# ------------------------------------------------------------------------------- degenerate shapes
+def test_one_partition_equals_exact_projector(gbe):
+    s = gi.config(1)
+    s.part = np.zeros(s.n, np.int32)
+    s.n_part = 1
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r, compare_all_branches=False)
+    D = sp.csr_matrix((Dg, ex["D_col"], ex["D_row_ptr"]), shape=(s.n, s.n)).toarray()
+    assert abs(D - o.o_diag(s.H, 256)).max() < 1e-10
+    assert abs(log.t1[-1] - s.n_occ) <= 1e-8  # north_star trace bar, attainable here (A-11)
+
+
+def test_single_vertex_cores_and_empty_partitions(gbe):
+    s = gi.chain(96, 96, tau=1e-3, iters=25)  # one vertex per core
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+    s2 = gi.random_banded(90, n_part=9, seed=11, tau=1e-3, iters=25)
+    s2.part = (s2.part // 2 * 2).astype(np.int32)  # odd communities are empty
+    g, ex, Dg, log = run_gpu(gbe, s2)
+    graph, r = run_oracle(s2)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+    assert (ex["ncore"][1::2] == 0).all()
+
+
+def test_missing_diagonal_entries(gbe):
+    s = gi.random_banded(64, half_bw=3, n_part=4, seed=8, tau=1e-3, iters=25)
+    a = s.H.to_dense()
+    a[np.arange(0, 64, 3), np.arange(0, 64, 3)] = 0.0  # not stored -> H_kk = 0 (A-12)
+    H = gi.CSR.from_dense(a)
+    assert H.nnz < s.H.nnz
+    g, ex, Dg, log = run_gpu(gbe, s, H=H)
+    graph, r = run_oracle(s, H=H)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+
+
+def test_h_may_change_between_build_and_density(gbe):
+    """MD use: the graph fixes S, the communities and D's pattern; H values are read at gather time."""
+    import torch
+    s = gi.chain(256, 8, seed=0, tau=1e-4, iters=30)
+    s_new = gi.chain(256, 8, seed=7, tau=1e-4, iters=30)
+    Hd0, Hd1 = gbe.DeviceCSR.from_host(s.H), gbe.DeviceCSR.from_host(s_new.H)
+    g = gbe.gbe_build_graph(Hd0, s.tau, None, s.n_part)
+    Dg, log = gbe.gbe_density(Hd1, g, s.n_occ, s.iters)
+    torch.cuda.synchronize()
+    rp, ci = o.build_graph(s.H, s.tau)
+    r = o.o_sub(s_new.H, rp, ci, s.part, s.n_part, s.n_occ, s.iters)
+    check_density(Dg.cpu().numpy(), log, r)
+
+
+def test_density_host_and_phase_calls(gbe):
+    import torch
+    s = gi.chain(256, 8, tau=1e-4, iters=30)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    ws = g.new_workspace()
+    D1, log1 = gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws)
+    Dh, logh = gbe.gbe_density_host(s.H, g, s.n_occ, s.iters, workspace=ws, want_log=True)
+    D3 = torch.empty_like(D1)
+    gbe.gbe_gather(Hd, g, ws)
+    gbe.gbe_sp2(g, s.n_occ, s.iters, -1.0, ws)
+    gbe.gbe_scatter(g, ws, D3)
+    log3 = gbe.gbe_read_log(g, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(D1.cpu().numpy(), Dh) and np.array_equal(D1.cpu().numpy(), D3.cpu().numpy())  # reproducible
+    assert np.array_equal(log1.branch, logh.branch) and np.array_equal(log1.t1, log3.t1)
+
+
+def test_errors(gbe):
+    import torch
+    s = gi.chain(64, 4)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_build_graph(Hd, -1.0, None, 4)
+    assert e.value.status == -1
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_build_graph(Hd, 1e-5, torch.full((64,), 9, dtype=torch.int32).cuda(), 4)
+    assert e.value.status == -1  # partition id out of range
+    a = s.H.to_dense()
+    a[0, 1] += 0.5
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_build_graph(gbe.DeviceCSR.from_host(gi.CSR.from_dense(a)), 1e-5, None, 4, check_symmetry=True)
+    assert e.value.status == -2
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_build_graph(gbe.DeviceCSR.from_host(gi.CSR.from_dense(np.zeros((4, 4)), keep_zeros=True)), 1e-5, None, 2)
+    assert e.value.status == -3  # eps_max == eps_min
+    g = gbe.gbe_build_graph(Hd, 1e-5, None, 4, check_symmetry=True)
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_density(Hd, g, 32.0, 10, workspace=torch.empty(256, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == -5
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_density(Hd, g, 65.0, 10)
+    assert e.value.status == -1
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_density(gbe.DeviceCSR.from_host(gi.chain(32, 4).H), g, 16.0, 10)
+    assert e.value.status == -4
