@@ -1,0 +1,365 @@
+"""bench.py - throughput of the graph-based SP2 density-matrix path (arXiv:1603.00937) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload water4096] [--impl ours|reference]
+
+One STEP = one pass of the whole hot path over one synthetic system (rows 0-6):
+gbe_build_graph (bounds, S_tau, halos, D pattern) + gbe_density (gather, 40 SP2 iterations with the on-device
+branch choice, core-column scatter).  Metric: density-matrix orbitals/s = orbitals / step time.
+
+* `value`   : inputs resident in HBM, step timed with CUDA events on the launching stream.
+* `e2e`     : the same step through the C ABI's HOST entry points (gbe_build_graph_host + gbe_density_host):
+              H comes from pinned host memory and D goes back to pinned host memory inside the timed region.
+* `roofline`: the dominant kernel (k_x2, FP64 tensor pipe), per-launch time from CUDA events recorded around every
+              launch by gbe_density_timed in the same process.
+* `cpu_baseline` / `--impl reference`: the CPU oracle as it stands, on a bounded sample of the same workload.
+
+N > 1 (torchrun): the path does not shard across GPUs in this build (north_star: one GPU, no collectives) - every rank
+runs an independent replica on its own seeded system ("replicas only"); value = all orbitals / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "density_matrix_orbitals_per_s"
+UNIT = "orbitals/s"
+# FP64 tensor peak: MEASURED_PEAKS.json has no FP64 entry.  Rule of the profiling guide: another dtype's
+# measured peak x the nominal ratio.  Nominal B200 dense: bf16 2250 TF, FP64 tensor 40 TF (128 flop/clk/SM x 148 SMs
+# x 1.965 GHz = 37.2 TF is the issue-rate ceiling; a register-resident DMMA.8x8x4 loop measured 37.07 TF, cuBLAS DGEMM
+# 8192^3 35.3 TF on this pool - profiles/r01_fp64_peak_probe.md).
+FP64_NOMINAL_TF, BF16_NOMINAL_TF = 40.0, 2250.0
+DMMA_PROBE_TF = 37.07
+
+WORKLOADS = {
+    # name: (molecules, communities) - BASELINE.json configs[1], configs[2] (SURVEY numbering: config 2, config 3)
+    "water1024": (1024, 128),
+    "water4096": (4096, 512),
+}
+
+
+def make_system(workload: str, seed: int):
+    import gbe_inputs as gi
+    n_mol, n_part = WORKLOADS[workload]
+    return gi.water_box(n_mol, n_part, seed=seed)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), bf16_tf=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
+                    source="MEASURED_PEAKS.json (of measured)")
+    return dict(hbm_gbs=6650.0, bf16_tf=1400.0, source="B200_PROFILING.md fallback (of fallback)")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md, clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows, self.proc, self.idx = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.rows:
+            if not (t0 <= ts <= t1 + 0.2):
+                continue
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); pw.append(float(f[3]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, f[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# the CPU oracle, timed as it stands (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------------
+def oracle_step(s) -> float:
+    """One pass of the whole path by the oracle (graph, halos, gather, SP2, scatter); returns seconds."""
+    import oracle as o
+    t0 = time.perf_counter()
+    rp, ci = o.build_graph(s.H, s.tau)
+    r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, s.iters)
+    dt = time.perf_counter() - t0
+    assert r.iters_done == s.iters
+    return dt
+
+
+def cpu_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def sample_description(s) -> str:
+    return (f"{s.meta['n_mol']}-molecule water box ({s.n} orbitals, {s.n_part} communities): same construction, density, "
+            f"tau={s.tau:g} and {s.iters} SP2 iterations as the workload; the path is linear scaling, so cost per orbital "
+            "does not depend on the box size")
+
+
+def run_reference(args) -> None:
+    """--impl reference: the oracle on the host cores, each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    total = args.steps + args.warmup
+    n_mol = 1024 if total <= 4 else (512 if total <= 12 else 256)
+    import gbe_inputs as gi
+    s = gi.water_box(n_mol, n_mol // 8, seed=0)
+    for _ in range(args.warmup):
+        oracle_step(s)
+    times = [oracle_step(s) for _ in range(args.steps)]
+    dt = float(np.mean(times))
+    v = s.n / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "note": "CPU oracle (numpy/scipy, host BLAS), bounded sample per step"},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle", "sample": sample_description(s)},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------------
+def pinned_host_csr(H):
+    """The CSR arrays of H in pinned host memory (numpy views of pinned torch tensors)."""
+    import torch
+    import gbe_inputs as gi
+    keep = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (H.row_ptr, H.col_idx, H.val)]
+    h = gi.CSR(H.n, keep[0].numpy(), keep[1].numpy(), keep[2].numpy())
+    h._keep = keep
+    return h
+
+
+def run_ours(args) -> None:
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_1603_00937_b200 import build as gbe_build
+    if rank == 0:
+        gbe_build.build()
+    if world > 1:
+        dist.barrier()
+    import paper_1603_00937_b200 as gbe
+    gbe.lib()
+
+    s = make_system(args.workload, seed=rank)  # replicas: one independent seeded box per rank
+    stream = torch.cuda.current_stream()
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    Hh = pinned_host_csr(s.H)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+    # sizes are fixed by the graph: build once to allocate outputs/workspace outside the timed region
+    g0 = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    info = dict(g0.info)
+    ws = g0.new_workspace()
+    D_val = torch.empty(info["nnz_D"], dtype=torch.float64, device="cuda")
+    D_host = torch.empty(info["nnz_D"], dtype=torch.float64).pin_memory()
+    g0.free()
+
+    def step_device():
+        g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part, stream=stream)
+        gbe.gbe_density(Hd, g, s.n_occ, s.iters, -1.0, workspace=ws, D_val=D_val, want_log=False, stream=stream)
+        return g
+
+    def step_host():
+        g = gbe.gbe_build_graph_host(Hh, s.tau, None, s.n_part, stream=stream)
+        gbe.gbe_density_host(Hh, g, s.n_occ, s.iters, -1.0, workspace=ws, D_val_host=D_host.numpy(), stream=stream)
+        return g
+
+    def timed_region(step, steps):
+        """K steps, each bracketed by CUDA events on the launching stream, L2 flushed (untimed) between steps."""
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        graphs = []
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        n0 = gbe.gbe_launch_count()
+        for e0, e1 in ev:
+            flush.zero_()
+            e0.record(stream)
+            graphs.append(step())
+            e1.record(stream)
+        torch.cuda.synchronize()
+        launches = gbe.gbe_launch_count() - n0
+        if world > 1:
+            dist.barrier()
+        ms = [e0.elapsed_time(e1) for e0, e1 in ev]
+        for g in graphs:
+            g.free()
+        return float(np.sum(ms)), int(launches)
+
+    for _ in range(max(args.warmup, 3)):
+        step_device().free()
+    torch.cuda.synchronize()
+
+    clocks = ClockSampler(local)
+    clocks.start()
+    time.sleep(0.3)
+    t_wall0 = time.time()
+    total_ms, launches = timed_region(step_device, args.steps)
+    t_wall1 = time.time()
+    clk = clocks.stop(t_wall0, t_wall1)
+
+    # end to end: HOST buffers through the C ABI, copies inside the timed region
+    step_host().free()
+    e2e_ms, _ = timed_region(step_host, args.steps)
+
+    # per-kernel device times, same process, same inputs (CUDA events around every launch of gbe_density)
+    g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    ph = None
+    for _ in range(2):
+        flush.zero_()
+        _, ph = gbe.gbe_density_timed(Hd, g, s.n_occ, s.iters, -1.0, workspace=ws, D_val=D_val)
+    # graph build alone
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    gbe.gbe_build_graph(Hd, s.tau, None, s.n_part).free()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    graph_ms = e0.elapsed_time(e1)
+
+    def allmax(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def allsum(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    total_ms_max, e2e_ms_max = allmax(total_ms), allmax(e2e_ms)
+    orbitals_all = allsum(float(s.n))
+    value = orbitals_all * args.steps / (total_ms_max * 1e-3)
+    e2e_value = orbitals_all * args.steps / (e2e_ms_max * 1e-3)
+
+    if rank == 0:
+        peaks = load_peaks()
+        peak_tf = peaks["bf16_tf"] * FP64_NOMINAL_TF / BF16_NOMINAL_TF
+        x2_ms = ph["x2_ms"] / max(1, ph["x2_launches"])
+        alg_tf = info["sp2_flops_per_iter"] / (x2_ms * 1e-3) * 1e-12
+        exec_tf = info["sp2_exec_flops_per_iter"] / (x2_ms * 1e-3) * 1e-12
+        nnzH = int(s.H.nnz)
+        gather_bytes = info["dense_elems"] * 8 + 12.0 * nnzH * info["sum_m"] / info["n"]
+        scatter_bytes = 16.0 * info["nnz_D"]
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {
+                "workload": f"{args.workload}: periodic water box, {s.meta['n_mol']} molecules, {s.n} orbitals, "
+                            f"n_occ={s.n_occ:g}, tau={s.tau:g}, {s.n_part} communities, {s.iters} SP2 iterations, FP64",
+                "step": "gbe_build_graph + gbe_density (rows 0-6)", "parallelism": "replicas only" if world > 1 else "1 GPU",
+                "l2": "256 MiB buffer written between timed steps; dense batch (2 x %.2f GB) exceeds L2" % (info["dense_elems"] * 8e-9),
+                "m_mean": info["sum_m"] / info["n_part"], "m_max": info["max_m"], "nnz_H": nnzH, "nnz_D": info["nnz_D"],
+            },
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max / args.steps,
+                    "h2d_bytes_per_step": int(2 * (s.H.row_ptr.nbytes + s.H.col_idx.nbytes + s.H.val.nbytes)),
+                    "d2h_bytes_per_step": int(info["nnz_D"] * 8)},
+            "gpu_launches": launches,
+            "clocks": clk,
+            "roofline": {
+                "kernel": "k_x2 (Y = X X^T on DMMA.8x8x4, fused branch/trace epilogue)", "bound": "tensor",
+                "achieved": alg_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": alg_tf / peak_tf, "traffic": None,
+                "basis": "algorithmic 2 m^3 flop per community per iteration (unpadded, symmetry not counted) / mean "
+                         "CUDA-event time of the %d launches" % ph["x2_launches"],
+                "peak_source": "FP64: %s bf16 sustained %.1f TF x nominal 40/2250" % (peaks["source"], peaks["bf16_tf"]),
+                "executed_tflops": exec_tf, "executed_frac_of_dmma_probe": exec_tf / DMMA_PROBE_TF,
+                "dmma_probe_peak": DMMA_PROBE_TF, "ms_per_launch": x2_ms,
+            },
+            "phases_ms": {"graph_build": graph_ms, "bounds": ph["bounds_ms"], "gather": ph["gather_ms"], "x2": ph["x2_ms"],
+                          "trace_branch": ph["trace_ms"], "scatter": ph["scatter_ms"], "density_total": ph["total_ms"]},
+            "sp2_solves_per_s": info["n_part"] / ((ph["x2_ms"] + ph["trace_ms"]) * 1e-3),
+            "hbm": {"peak_gbs": peaks["hbm_gbs"],
+                    "gather_gbs": gather_bytes / (ph["gather_ms"] * 1e-3) * 1e-9,
+                    "gather_frac": gather_bytes / (ph["gather_ms"] * 1e-3) * 1e-9 / peaks["hbm_gbs"],
+                    "scatter_gbs": scatter_bytes / (ph["scatter_ms"] * 1e-3) * 1e-9,
+                    "scatter_frac": scatter_bytes / (ph["scatter_ms"] * 1e-3) * 1e-9 / peaks["hbm_gbs"]},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            import gbe_inputs as gi
+            cs = gi.water_box(1024, 128, seed=0)
+            dt = oracle_step(cs)
+            line["cpu_baseline"] = {"value": cs.n / dt, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle",
+                                    "seconds": dt, "sample": sample_description(cs)}
+        print(json.dumps(line), flush=True)
+    g.free()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="water4096", choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

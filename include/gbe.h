@@ -77,6 +77,8 @@ typedef struct {
   int64_t dense_elems;/* doubles in ONE batched dense buffer = sum_p m_p * ld_p (ld_p = m_p rounded up to 16) */
   int64_t n_tiles;    /* X^2 work items per SP2 iteration (upper-triangle tiles over all communities) */
   double sp2_flops_per_iter; /* sum_p 2 m_p^3: algorithmic flops of one SP2 iteration (unpadded, no symmetry) */
+  double sp2_exec_flops_per_iter; /* flops the X^2 kernel issues to the FP64 tensor pipe per iteration: upper-triangle
+                                     tiles only (X is symmetric), tile and K padding included */
   double eps_min, eps_max;   /* Gershgorin bounds of the H given to gbe_build_graph (A-5) */
   int32_t contiguous_cores;  /* 1: every core is a contiguous index range (fast scatter); 0: per-entry map */
   int32_t tile;              /* edge of the square X^2 tile chosen for this graph */
@@ -144,6 +146,31 @@ int gbe_read_log(const gbe_graph* g, const void* workspace, size_t workspace_byt
 int gbe_density_host(const gbe_csr_view* H_host, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
                      void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val_host,
                      gbe_sp2_log* log);
+
+/* gbe_build_graph with HOST buffers: H (row_ptr, col_idx, val) and part (may be NULL) are host pointers; the call
+ * copies them to the device, builds the graph and frees the staging copies before it returns. */
+int gbe_build_graph_host(const gbe_csr_view* H_host, const gbe_graph_opts* opts, const int32_t* part_host,
+                         int32_t n_part, void* cuda_stream, gbe_graph** out);
+
+/* Device time of the kernels of one gbe_density run, measured with CUDA events recorded on `cuda_stream` around
+ * every launch (milliseconds; *_launches = kernel launches summed into the field before it). */
+typedef struct {
+  float bounds_ms;  int32_t bounds_launches;   /* step 0 */
+  float gather_ms;  int32_t gather_launches;   /* step 3 */
+  float x2_ms;      int32_t x2_launches;       /* step 4: the X^2 / 2X - X^2 kernel, one launch per SP2 iteration */
+  float trace_ms;   int32_t trace_launches;    /* step 5 (+ the state initialisation kernel) */
+  float scatter_ms; int32_t scatter_launches;  /* step 6 */
+  float total_ms;                              /* first launch to last launch, on the stream */
+} gbe_phase_times;
+
+/* gbe_density with the same kernels and the same launch sequence, plus one event pair per launch; synchronises
+ * the stream before returning.  For measurement only: the events serialise nothing but cost a few us each. */
+int gbe_density_timed(const gbe_csr_view* H, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
+                      void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val, gbe_sp2_log* log,
+                      gbe_phase_times* times);
+
+/* Number of CUDA kernels this library has launched in this process so far (all threads). */
+uint64_t gbe_launch_count(void);
 
 void gbe_free_graph(gbe_graph* g);
 

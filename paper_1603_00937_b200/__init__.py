@@ -17,6 +17,9 @@ from .binding import (  # noqa: F401
     LIB_PATH,
     lib,
     gbe_build_graph,
+    gbe_build_graph_host,
+    gbe_density_timed,
+    gbe_launch_count,
     gbe_graph_export,
     gbe_density,
     gbe_density_host,

@@ -19,7 +19,7 @@ GBE_MAX_ITERS = 1024
 EXPORTS = [
     "gbe_build_graph", "gbe_graph_get_info", "gbe_graph_export", "gbe_density", "gbe_gather", "gbe_sp2",
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
-    "gbe_version",
+    "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count",
 ]
 
 
@@ -41,12 +41,20 @@ class _GraphOpts(C.Structure):
 class _GraphInfo(C.Structure):
     _fields_ = [("n", C.c_int64), ("nnz_S", C.c_int64), ("n_part", C.c_int64), ("sum_m", C.c_int64),
                 ("max_m", C.c_int64), ("nnz_D", C.c_int64), ("dense_elems", C.c_int64), ("n_tiles", C.c_int64),
-                ("sp2_flops_per_iter", C.c_double), ("eps_min", C.c_double), ("eps_max", C.c_double),
+                ("sp2_flops_per_iter", C.c_double), ("sp2_exec_flops_per_iter", C.c_double),
+                ("eps_min", C.c_double), ("eps_max", C.c_double),
                 ("contiguous_cores", C.c_int32), ("tile", C.c_int32), ("workspace_bytes", C.c_size_t)]
 
 
 class _Sp2Log(C.Structure):
     _fields_ = [("iters_done", C.c_int32), ("branch", C.c_void_p), ("t1", C.c_void_p), ("t2", C.c_void_p)]
+
+
+class _PhaseTimes(C.Structure):
+    _fields_ = [("bounds_ms", C.c_float), ("bounds_launches", C.c_int32), ("gather_ms", C.c_float),
+                ("gather_launches", C.c_int32), ("x2_ms", C.c_float), ("x2_launches", C.c_int32),
+                ("trace_ms", C.c_float), ("trace_launches", C.c_int32), ("scatter_ms", C.c_float),
+                ("scatter_launches", C.c_int32), ("total_ms", C.c_float)]
 
 
 _lib = None
@@ -71,6 +79,10 @@ def lib() -> C.CDLL:
         l.gbe_density.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_double, C.c_int32, C.c_double, C.c_void_p,
                                   C.c_size_t, C.c_void_p, C.c_void_p, C.POINTER(_Sp2Log)]
         l.gbe_density_host.argtypes = l.gbe_density.argtypes
+        l.gbe_density_timed.argtypes = l.gbe_density.argtypes + [C.POINTER(_PhaseTimes)]
+        l.gbe_build_graph_host.argtypes = l.gbe_build_graph.argtypes
+        l.gbe_launch_count.restype = C.c_uint64
+        l.gbe_launch_count.argtypes = []
         l.gbe_gather.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         l.gbe_sp2.argtypes = [C.c_void_p, C.c_double, C.c_int32, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
         l.gbe_scatter.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p]
@@ -166,6 +178,25 @@ def gbe_build_graph(H: DeviceCSR, tau: float, part: torch.Tensor | None, n_part:
     return Graph(out.value)
 
 
+def gbe_build_graph_host(H_host, tau: float, part_host: np.ndarray | None, n_part: int, power: int = 2,
+                         check_symmetry: bool = False, stream=None) -> Graph:
+    """H_host: numpy fields n, row_ptr (int64), col_idx (int32), val (float64); part_host: int32[n] or None. HOST memory."""
+    opts = _GraphOpts(float(tau), int(power), int(bool(check_symmetry)))
+    rp = np.ascontiguousarray(H_host.row_ptr, dtype=np.int64)
+    ci = np.ascontiguousarray(H_host.col_idx, dtype=np.int32)
+    va = np.ascontiguousarray(H_host.val, dtype=np.float64)
+    pt = None if part_host is None else np.ascontiguousarray(part_host, dtype=np.int32)
+    v = _CsrView(int(H_host.n), int(ci.size), rp.ctypes.data, ci.ctypes.data, va.ctypes.data)
+    out = C.c_void_p()
+    _check(lib().gbe_build_graph_host(C.byref(v), C.byref(opts), None if pt is None else pt.ctypes.data, int(n_part),
+                                      _stream(stream), C.byref(out)))
+    return Graph(out.value)
+
+
+def gbe_launch_count() -> int:
+    return int(lib().gbe_launch_count())
+
+
 def gbe_graph_export(g: Graph, stream=None) -> dict:
     i = g.info
     dev = "cuda"
@@ -209,6 +240,20 @@ def gbe_density(H: DeviceCSR, g: Graph, n_occ: float, iters: int, idem_tol: floa
     _check(lib().gbe_density(C.byref(v), g.handle, float(n_occ), int(iters), float(idem_tol), _ptr(workspace),
                              workspace.numel(), _stream(stream), _ptr(D_val), C.byref(clog) if want_log else None))
     return D_val, (_finish_log(clog, arrs) if want_log else None)
+
+
+def gbe_density_timed(H: DeviceCSR, g: Graph, n_occ: float, iters: int, idem_tol: float = -1.0,
+                      workspace: torch.Tensor | None = None, D_val: torch.Tensor | None = None, stream=None):
+    """gbe_density with one CUDA-event pair per launch; synchronises.  Returns (D_val, dict of gbe_phase_times)."""
+    if workspace is None:
+        workspace = g.new_workspace()
+    if D_val is None:
+        D_val = torch.empty(g.info["nnz_D"], dtype=torch.float64, device="cuda")
+    v = H.view()
+    pt = _PhaseTimes()
+    _check(lib().gbe_density_timed(C.byref(v), g.handle, float(n_occ), int(iters), float(idem_tol), _ptr(workspace),
+                                   workspace.numel(), _stream(stream), _ptr(D_val), None, C.byref(pt)))
+    return D_val, {k: getattr(pt, k) for k, _ in _PhaseTimes._fields_}
 
 
 def gbe_gather(H: DeviceCSR, g: Graph, workspace: torch.Tensor, stream=None) -> None:

@@ -7,8 +7,32 @@
 
 #include "gbe_internal.cuh"
 
+std::atomic<uint64_t> g_gbe_launches{0};
+
 namespace {
 thread_local char g_cuda_err[512] = "";
+
+// Optional per-launch timing (gbe_density_timed): one event pair around every launcher call.
+enum Phase { PH_BOUNDS = 0, PH_GATHER, PH_X2, PH_TRACE, PH_SCATTER, PH_COUNT };
+struct Timer {
+  struct Rec { int phase, launches; cudaEvent_t e0, e1; };
+  std::vector<Rec> recs;
+  cudaStream_t s;
+  explicit Timer(cudaStream_t st) : s(st) {}
+  ~Timer() { for (auto& r : recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); } }
+};
+template <typename F>
+int timed(Timer* tm, int phase, int launches, F&& fn) {
+  if (!tm) return fn();
+  Timer::Rec r{phase, launches, nullptr, nullptr};
+  GBE_CUDA(cudaEventCreate(&r.e0));
+  GBE_CUDA(cudaEventCreate(&r.e1));
+  tm->recs.push_back(r);
+  GBE_CUDA(cudaEventRecord(r.e0, tm->s));
+  const int rc = fn();
+  GBE_CUDA(cudaEventRecord(r.e1, tm->s));
+  return rc;
+}
 
 __global__ void k_init_state(gbe_state* st, double n_occ, double idem_tol, int iters) {
   st->n_occ = n_occ;
@@ -134,6 +158,7 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   o->dense_elems = g->dense_elems;
   o->n_tiles = g->n_items;
   o->sp2_flops_per_iter = g->flops_per_iter;
+  o->sp2_exec_flops_per_iter = g->exec_flops_per_iter;
   o->eps_min = g->eps_min;
   o->eps_max = g->eps_max;
   o->contiguous_cores = g->contiguous;
@@ -160,44 +185,61 @@ int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, 
   return GBE_OK;
 }
 
-int gbe_gather(const gbe_csr_view* H, const gbe_graph* g, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+static int do_gather(const gbe_csr_view* H, const gbe_graph* g, void* workspace, size_t workspace_bytes,
+                     void* cuda_stream, Timer* tm) {
   if (!g) return GBE_EINVAL;
   GBE_TRY(check_csr(H));
   if (H->n != g->n) return GBE_EMISMATCH;
   WS w;
   GBE_TRY(carve(g, workspace, workspace_bytes, &w));
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  GBE_TRY(gbe_launch_bounds(*H, w.blo, w.bhi, 1024, w.st, s));
-  GBE_TRY(gbe_launch_gather(*H, g, w.st, w.X0, w.partials, s));
+  GBE_TRY(timed(tm, PH_BOUNDS, 2, [&] { return gbe_launch_bounds(*H, w.blo, w.bhi, 1024, w.st, s); }));
+  GBE_TRY(timed(tm, PH_GATHER, g->n_gitems ? 1 : 0,
+                [&] { return gbe_launch_gather(*H, g, w.st, w.X0, w.partials, s); }));
   return GBE_OK;
 }
+int gbe_gather(const gbe_csr_view* H, const gbe_graph* g, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  return do_gather(H, g, workspace, workspace_bytes, cuda_stream, nullptr);
+}
 
-int gbe_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_tol, void* workspace, size_t workspace_bytes,
-            void* cuda_stream) {
+static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_tol, void* workspace,
+                  size_t workspace_bytes, void* cuda_stream, Timer* tm) {
   if (!g) return GBE_EINVAL;
   if (!(n_occ >= 0.0) || n_occ > (double)g->n || iters < 0 || iters > GBE_MAX_ITERS || std::isnan(idem_tol))
     return GBE_EINVAL;
   WS w;
   GBE_TRY(carve(g, workspace, workspace_bytes, &w));
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters);
-  GBE_CUDA(cudaGetLastError());
   // traces of X_0 (partials written by the gather), branch of iteration 0
-  GBE_TRY(gbe_launch_trace_branch(w.st, w.partials, g->n_gitems, s));
+  GBE_TRY(timed(tm, PH_TRACE, 2, [&]() -> int {
+    k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters);
+    GBE_LAUNCHED();
+    return gbe_launch_trace_branch(w.st, w.partials, g->n_gitems, s);
+  }));
   for (int it = 0; it < iters; ++it) {
     const double* in = (it & 1) ? w.X1 : w.X0;
     double* outp = (it & 1) ? w.X0 : w.X1;
-    GBE_TRY(gbe_launch_x2(g, w.st, in, outp, w.partials, it, s));
-    GBE_TRY(gbe_launch_trace_branch(w.st, w.partials, g->n_items, s));
+    GBE_TRY(timed(tm, PH_X2, g->n_items ? 1 : 0, [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, s); }));
+    GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, g->n_items, s); }));
   }
   return GBE_OK;
 }
+int gbe_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_tol, void* workspace, size_t workspace_bytes,
+            void* cuda_stream) {
+  return do_sp2(g, n_occ, iters, idem_tol, workspace, workspace_bytes, cuda_stream, nullptr);
+}
 
-int gbe_scatter(const gbe_graph* g, void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val) {
+static int do_scatter(const gbe_graph* g, void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val,
+                      Timer* tm) {
   if (!g || (!D_val && g->nnz_D > 0)) return GBE_EINVAL;
   WS w;
   GBE_TRY(carve(g, workspace, workspace_bytes, &w));
-  return gbe_launch_scatter(g, w.st, w.X0, w.X1, D_val, static_cast<cudaStream_t>(cuda_stream));
+  return timed(tm, PH_SCATTER, g->sum_m ? 1 : 0, [&] {
+    return gbe_launch_scatter(g, w.st, w.X0, w.X1, D_val, static_cast<cudaStream_t>(cuda_stream));
+  });
+}
+int gbe_scatter(const gbe_graph* g, void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val) {
+  return do_scatter(g, workspace, workspace_bytes, cuda_stream, D_val, nullptr);
 }
 
 int gbe_read_log(const gbe_graph* g, const void* workspace, size_t workspace_bytes, void* cuda_stream, gbe_sp2_log* log) {
@@ -218,16 +260,70 @@ int gbe_read_log(const gbe_graph* g, const void* workspace, size_t workspace_byt
   return GBE_OK;
 }
 
-int gbe_density(const gbe_csr_view* H, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
-                void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val, gbe_sp2_log* log) {
+static int do_density(const gbe_csr_view* H, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
+                      void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val, gbe_sp2_log* log,
+                      Timer* tm) {
   if (!g || (!D_val && g->nnz_D > 0)) return GBE_EINVAL;
   if (!(n_occ >= 0.0) || n_occ > (double)g->n || iters < 0 || iters > GBE_MAX_ITERS || std::isnan(idem_tol))
     return GBE_EINVAL;
-  GBE_TRY(gbe_gather(H, g, workspace, workspace_bytes, cuda_stream));
-  GBE_TRY(gbe_sp2(g, n_occ, iters, idem_tol, workspace, workspace_bytes, cuda_stream));
-  GBE_TRY(gbe_scatter(g, workspace, workspace_bytes, cuda_stream, D_val));
+  GBE_TRY(do_gather(H, g, workspace, workspace_bytes, cuda_stream, tm));
+  GBE_TRY(do_sp2(g, n_occ, iters, idem_tol, workspace, workspace_bytes, cuda_stream, tm));
+  GBE_TRY(do_scatter(g, workspace, workspace_bytes, cuda_stream, D_val, tm));
   if (log) GBE_TRY(gbe_read_log(g, workspace, workspace_bytes, cuda_stream, log));
   return GBE_OK;
+}
+int gbe_density(const gbe_csr_view* H, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
+                void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val, gbe_sp2_log* log) {
+  return do_density(H, g, n_occ, iters, idem_tol, workspace, workspace_bytes, cuda_stream, D_val, log, nullptr);
+}
+
+int gbe_density_timed(const gbe_csr_view* H, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
+                      void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val, gbe_sp2_log* log,
+                      gbe_phase_times* times) {
+  if (!times) return GBE_EINVAL;
+  memset(times, 0, sizeof(*times));
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  Timer tm(s);
+  GBE_TRY(do_density(H, g, n_occ, iters, idem_tol, workspace, workspace_bytes, cuda_stream, D_val, log, &tm));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  float* ms[PH_COUNT] = {&times->bounds_ms, &times->gather_ms, &times->x2_ms, &times->trace_ms, &times->scatter_ms};
+  int32_t* nl[PH_COUNT] = {&times->bounds_launches, &times->gather_launches, &times->x2_launches,
+                           &times->trace_launches, &times->scatter_launches};
+  for (auto& r : tm.recs) {
+    float t = 0.f;
+    GBE_CUDA(cudaEventElapsedTime(&t, r.e0, r.e1));
+    *ms[r.phase] += t;
+    *nl[r.phase] += r.launches;
+  }
+  if (!tm.recs.empty()) GBE_CUDA(cudaEventElapsedTime(&times->total_ms, tm.recs.front().e0, tm.recs.back().e1));
+  return GBE_OK;
+}
+
+uint64_t gbe_launch_count(void) { return g_gbe_launches.load(std::memory_order_relaxed); }
+
+int gbe_build_graph_host(const gbe_csr_view* Hh, const gbe_graph_opts* opts, const int32_t* part_host, int32_t n_part,
+                         void* cuda_stream, gbe_graph** out) {
+  if (!out) return GBE_EINVAL;
+  *out = nullptr;
+  GBE_TRY(check_csr(Hh));
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  DevBuf rp, ci, va, pt;
+  GBE_TRY(rp.alloc((size_t)(Hh->n + 1) * 8));
+  GBE_TRY(ci.alloc((size_t)Hh->nnz * 4));
+  GBE_TRY(va.alloc((size_t)Hh->nnz * 8));
+  GBE_CUDA(cudaMemcpyAsync(rp.p, Hh->row_ptr, (size_t)(Hh->n + 1) * 8, cudaMemcpyHostToDevice, s));
+  if (Hh->nnz) {
+    GBE_CUDA(cudaMemcpyAsync(ci.p, Hh->col_idx, (size_t)Hh->nnz * 4, cudaMemcpyHostToDevice, s));
+    GBE_CUDA(cudaMemcpyAsync(va.p, Hh->val, (size_t)Hh->nnz * 8, cudaMemcpyHostToDevice, s));
+  }
+  if (part_host) {
+    GBE_TRY(pt.alloc((size_t)Hh->n * 4));
+    GBE_CUDA(cudaMemcpyAsync(pt.p, part_host, (size_t)Hh->n * 4, cudaMemcpyHostToDevice, s));
+  }
+  gbe_csr_view Hd{Hh->n, Hh->nnz, rp.as<int64_t>(), ci.as<int32_t>(), va.as<double>()};
+  const int rc = gbe_build_graph(&Hd, opts, part_host ? pt.as<int32_t>() : nullptr, n_part, cuda_stream, out);
+  cudaStreamSynchronize(s);  // the staging buffers are freed on return
+  return rc;
 }
 
 int gbe_density_host(const gbe_csr_view* Hh, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,

@@ -62,8 +62,8 @@ int gbe_launch_bounds(const gbe_csr_view& H, double* block_lo, double* block_hi,
   int nb = (int)(want < max_blocks ? want : max_blocks);
   if (nb < 1) nb = 1;
   k_row_bounds<<<nb, BLK, 0, s>>>(H.n, H.row_ptr, H.col_idx, H.val, block_lo, block_hi);
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   k_bounds_final<<<1, 32, 0, s>>>(block_lo, block_hi, nb, st);
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   return GBE_OK;
 }

@@ -138,6 +138,6 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
   GBE_CUDA(cudaFuncSetAttribute(k_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   k_gather<<<g->n_gitems, nw * 32, smem, s>>>(W, ldmax, g->gather_rows, g->gitems, H.row_ptr, H.col_idx, H.val, g->n,
                                               g->sub_ptr, g->sub_idx, g->ncore, g->dense_off, st, X, partials);
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   return GBE_OK;
 }

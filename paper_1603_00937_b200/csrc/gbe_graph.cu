@@ -303,7 +303,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     GBE_TRY(flag.alloc(4));
     GBE_CUDA(cudaMemsetAsync(flag.p, 0, 4, s));
     k_check_symmetric<<<rows_grid, 256, 0, s>>>(n, H.row_ptr, H.col_idx, H.val, flag.as<int32_t>());
-    GBE_CUDA(cudaGetLastError());
+    GBE_LAUNCHED();
     int32_t f = 0;
     GBE_CUDA(cudaMemcpyAsync(&f, flag.p, 4, cudaMemcpyDeviceToHost, s));
     GBE_CUDA(cudaStreamSynchronize(s));
@@ -318,13 +318,13 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   Pattern A;
   k_materialise_A<false><<<rows_grid, 256, 0, s>>>(n, H.row_ptr, H.col_idx, H.val, st, tau, cnt.as<int32_t>(), nullptr,
                                                    nullptr, nullptr);
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   GBE_TRY(count_to_rowptr(cnt, n, A.rp, &A.nnz, s));
   GBE_TRY(A.col.alloc((size_t)A.nnz * 4));
   GBE_TRY(A.val.alloc((size_t)A.nnz * 8));
   k_materialise_A<true><<<rows_grid, 256, 0, s>>>(n, H.row_ptr, H.col_idx, H.val, st, tau, nullptr, A.rp.as<int64_t>(),
                                                   A.col.as<int32_t>(), A.val.as<double>());
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
 
   // pattern accumulator P = I u pat(A)
   const size_t bm_bytes = (size_t)W * 4;
@@ -338,12 +338,12 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                       Pattern& out) -> int {
     k_union_rows<false><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, q_rp, q_col, diag, cnt.as<int32_t>(),
                                                               nullptr, nullptr);
-    GBE_CUDA(cudaGetLastError());
+    GBE_LAUNCHED();
     GBE_TRY(count_to_rowptr(cnt, n, out.rp, &out.nnz, s));
     GBE_TRY(out.col.alloc((size_t)out.nnz * 4));
     k_union_rows<true><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, q_rp, q_col, diag, nullptr,
                                                              out.rp.as<int64_t>(), out.col.as<int32_t>());
-    GBE_CUDA(cudaGetLastError());
+    GBE_LAUNCHED();
     return GBE_OK;
   };
 
@@ -366,7 +366,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
       k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, A.rp.as<int64_t>(), A.col.as<int32_t>(),
                                                                  A.val.as<double>(), T_rp, T_col, T_val, tau,
                                                                  cnt.as<int32_t>(), nullptr, nullptr, nullptr);
-      GBE_CUDA(cudaGetLastError());
+      GBE_LAUNCHED();
     }
     std::vector<int32_t> h_cnt((size_t)n);
     GBE_CUDA(cudaMemcpyAsync(h_cnt.data(), cnt.p, (size_t)n * 4, cudaMemcpyDeviceToHost, s));
@@ -384,7 +384,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     k_spgemm_threshold<1><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, A.rp.as<int64_t>(), A.col.as<int32_t>(),
                                                                A.val.as<double>(), T_rp, T_col, T_val, tau,
                                                                cnt.as<int32_t>(), nullptr, nullptr, nullptr);
-    GBE_CUDA(cudaGetLastError());
+    GBE_LAUNCHED();
     GBE_TRY(count_to_rowptr(cnt, n, Tn.rp, &Tn.nnz, s));
     GBE_TRY(Tn.col.alloc((size_t)Tn.nnz * 4));
     GBE_TRY(Tn.val.alloc((size_t)Tn.nnz * 8));
@@ -392,7 +392,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                                A.val.as<double>(), T_rp, T_col, T_val, tau, nullptr,
                                                                Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(),
                                                                Tn.val.as<double>());
-    GBE_CUDA(cudaGetLastError());
+    GBE_LAUNCHED();
     Pattern Pn;
     GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(), 0, Pn));
     GBE_CUDA(cudaStreamSynchronize(s));
@@ -413,13 +413,13 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   Pattern PT;
   GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
   k_transpose_count<<<rows_grid, 256, 0, s>>>(n, P.rp.as<int64_t>(), P.col.as<int32_t>(), cnt.as<int32_t>());
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   GBE_TRY(count_to_rowptr(cnt, n, PT.rp, &PT.nnz, s));
   GBE_TRY(PT.col.alloc((size_t)PT.nnz * 4));
   GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
   k_transpose_fill<<<rows_grid, 256, 0, s>>>(n, P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(),
                                              cnt.as<int32_t>(), PT.col.as<int32_t>());
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   Pattern S;
   GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(), PT.col.as<int32_t>(), 0, S));
   GBE_CUDA(cudaStreamSynchronize(s));

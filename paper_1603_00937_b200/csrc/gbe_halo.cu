@@ -221,7 +221,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n_part * 4, s));
   GBE_CUDA(cudaMemsetAsync(flag.p, 0, 4, s));
   k_core_count<<<tgrid, 256, 0, s>>>(n, part, blk, n_part, cnt.as<int32_t>(), flag.as<int32_t>());
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   int32_t hflag = 0;
   GBE_CUDA(cudaMemcpyAsync(&hflag, flag.p, 4, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaStreamSynchronize(s));
@@ -233,7 +233,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_TRY(cursor.alloc((size_t)std::max<int64_t>(n_part, n) * 4));
   GBE_CUDA(cudaMemsetAsync(cursor.p, 0, (size_t)n_part * 4, s));
   k_core_fill<<<tgrid, 256, 0, s>>>(n, part, blk, core_ptr.as<int64_t>(), cursor.as<int32_t>(), core_tmp.as<int32_t>());
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
 
   // ---- halo: count, then fill
   const size_t halo_smem = (size_t)2 * W * 4 + 257 * 4;
@@ -244,7 +244,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_CUDA(cudaMalloc((void**)&g->ncore, (size_t)n_part * 4));
   k_halo<false><<<n_part, 256, halo_smem, s>>>(W, core_ptr.as<int64_t>(), core_tmp.as<int32_t>(), g->S_row_ptr, g->S_col,
                                                g->msize, g->ncore, nullptr, nullptr, nullptr);
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   g->h_m.resize(n_part);
   g->h_ncore.resize(n_part);
   GBE_CUDA(cudaMemcpyAsync(g->h_m.data(), g->msize, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
@@ -281,10 +281,13 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return g->h_m[a] > g->h_m[b]; });
     std::vector<gbe_tile_item> items;
     const int tile = g->tile;
+    g->exec_flops_per_iter = 0;
     for (int p : order) {
       const int T = (g->h_m[p] + tile - 1) / tile;
+      const int64_t ld = (g->h_m[p] + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
       for (int ti = 0; ti < T; ++ti)
         for (int tj = ti; tj < T; ++tj) items.push_back({p, ti, tj, 0});
+      g->exec_flops_per_iter += (double)T * (T + 1) / 2 * 2.0 * tile * tile * (double)ld;
     }
     g->n_items = (int32_t)items.size();
     GBE_TRY(upload(items, &g->items, s));
@@ -316,7 +319,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_CUDA(cudaMalloc((void**)&g->row_part, std::max<size_t>(16, (size_t)g->sum_m * 4)));
   k_halo<true><<<n_part, 256, halo_smem, s>>>(W, core_ptr.as<int64_t>(), core_tmp.as<int32_t>(), g->S_row_ptr, g->S_col,
                                               nullptr, nullptr, g->sub_ptr, g->sub_idx, g->row_part);
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
 
   // ---- pattern of D and scatter map
   const int64_t sum_m = g->sum_m;
@@ -326,7 +329,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
   GBE_CUDA(cudaMemsetAsync(mcnt.p, 0, (size_t)n * 4, s));
   k_member_count<<<qgrid, 256, 0, s>>>(sum_m, g->sub_idx, g->row_part, g->ncore, cnt.as<int32_t>(), mcnt.as<int32_t>());
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   GBE_CUDA(cudaMalloc((void**)&g->D_row_ptr, (size_t)(n + 1) * 8));
   GBE_TRY(gbe_exclusive_scan_i32_to_i64(cnt.as<int32_t>(), g->D_row_ptr, n, s));
   GBE_TRY(memb_ptr.alloc((size_t)(n + 1) * 8));
@@ -334,7 +337,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_TRY(memb.alloc(std::max<size_t>(16, (size_t)sum_m * 8)));
   GBE_CUDA(cudaMemsetAsync(cursor.p, 0, (size_t)n * 4, s));
   k_member_fill<<<qgrid, 256, 0, s>>>(sum_m, g->sub_idx, memb_ptr.as<int64_t>(), cursor.as<int32_t>(), memb.as<int64_t>());
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   GBE_CUDA(cudaMalloc((void**)&g->D_col, std::max<size_t>(16, (size_t)g->nnz_D * 4)));
   GBE_CUDA(cudaMalloc((void**)&g->scat_base, std::max<size_t>(16, (size_t)sum_m * 8)));
   const size_t per_warp = (size_t)2 * W * 4;
@@ -347,7 +350,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   k_d_pattern<0><<<dgrid, nw * 32, per_warp * nw, s>>>(n, W, memb_ptr.as<int64_t>(), memb.as<int64_t>(), g->row_part,
                                                        g->sub_ptr, g->sub_idx, g->ncore, g->D_row_ptr, g->D_col,
                                                        g->scat_base, flag.as<int32_t>(), nullptr, nullptr);
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   GBE_CUDA(cudaMemcpyAsync(&hflag, flag.p, 4, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaStreamSynchronize(s));
   g->contiguous = hflag ? 0 : 1;
@@ -355,14 +358,14 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     DevBuf rn, scat_ofs;
     GBE_TRY(rn.alloc(std::max<size_t>(16, (size_t)sum_m * 4)));
     k_row_ncore<<<qgrid, 256, 0, s>>>(sum_m, g->row_part, g->ncore, rn.as<int32_t>());
-    GBE_CUDA(cudaGetLastError());
+    GBE_LAUNCHED();
     GBE_TRY(scat_ofs.alloc((size_t)(sum_m + 1) * 8));
     GBE_TRY(gbe_exclusive_scan_i32_to_i64(rn.as<int32_t>(), scat_ofs.as<int64_t>(), sum_m, s));
     GBE_CUDA(cudaMalloc((void**)&g->scat_pos, std::max<size_t>(16, (size_t)g->nnz_D * 8)));
     k_d_pattern<1><<<dgrid, nw * 32, per_warp * nw, s>>>(n, W, memb_ptr.as<int64_t>(), memb.as<int64_t>(), g->row_part,
                                                          g->sub_ptr, g->sub_idx, g->ncore, g->D_row_ptr, nullptr, nullptr,
                                                          nullptr, scat_ofs.as<int64_t>(), g->scat_pos);
-    GBE_CUDA(cudaGetLastError());
+    GBE_LAUNCHED();
     GBE_CUDA(cudaStreamSynchronize(s));
     g->scat_ofs = reinterpret_cast<int64_t*>(scat_ofs.release());
   }

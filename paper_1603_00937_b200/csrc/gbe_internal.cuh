@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <vector>
 
 #include "gbe.h"
@@ -18,6 +19,13 @@ void gbe_set_cuda_error(cudaError_t e, const char* what, int line);
       gbe_set_cuda_error(e__, #call, __LINE__);          \
       return GBE_ECUDA;                                  \
     }                                                    \
+  } while (0)
+// after every kernel launch: count it (gbe_launch_count) and surface launch errors
+extern std::atomic<uint64_t> g_gbe_launches;
+#define GBE_LAUNCHED()                                   \
+  do {                                                   \
+    g_gbe_launches.fetch_add(1, std::memory_order_relaxed); \
+    GBE_CUDA(cudaGetLastError());                        \
   } while (0)
 #define GBE_TRY(call)          \
   do {                         \
@@ -74,7 +82,7 @@ struct gbe_tile_item {  // one X^2 work item: tile (ti, tj), ti <= tj, of commun
 struct gbe_graph {
   int64_t n = 0, nnz_S = 0, sum_m = 0, nnz_D = 0, dense_elems = 0;
   int32_t n_part = 0, max_m = 0, max_ncore = 0, tile = 128;
-  double eps_min = 0, eps_max = 0, tau = 0, flops_per_iter = 0;
+  double eps_min = 0, eps_max = 0, tau = 0, flops_per_iter = 0, exec_flops_per_iter = 0;
   int32_t power = 2, contiguous = 1;
   // device arrays (owned)
   int64_t* S_row_ptr = nullptr;  // n+1

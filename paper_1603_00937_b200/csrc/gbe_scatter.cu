@@ -50,6 +50,6 @@ int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0
   else
     k_scatter<false><<<grid, 256, 0, s>>>(g->sum_m, g->row_part, g->sub_ptr, g->ncore, g->dense_off, nullptr, g->scat_ofs,
                                           g->scat_pos, st, X0, X1, D_val);
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   return GBE_OK;
 }

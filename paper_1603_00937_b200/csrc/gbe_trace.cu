@@ -49,6 +49,6 @@ __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double
 
 int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s) {
   k_trace_branch<<<1, TB, 0, s>>>(st, partials, n_partials);
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   return GBE_OK;
 }

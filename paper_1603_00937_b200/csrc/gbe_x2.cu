@@ -193,6 +193,6 @@ int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* 
     configured = true;
   }
   kern<<<g->n_items, WMN * WNN * 32, smem, s>>>(g->items, g->sub_ptr, g->ncore, g->dense_off, st, Xin, Xout, partials);
-  GBE_CUDA(cudaGetLastError());
+  GBE_LAUNCHED();
   return GBE_OK;
 }

@@ -61,15 +61,15 @@ def check_structure(ex, graph, r, info):
     assert abs(info["sp2_flops_per_iter"] - sum(2.0 * len(i) ** 3 for i, _ in r.subs)) < 1e-6 * info["sp2_flops_per_iter"]
 
 
-def check_density(Dg, log, r, compare_all_branches=True):
+def check_density(Dg, log, r):
+    """Branch bits are compared while the expansion is still moving (|t1 - t2| > 1e-9); once every X_p is
+    idempotent to roundoff either branch is a no-op and the bit is decided by rounding order (reading A-8)."""
     assert log.iters_done == r.iters_done
-    live = np.abs(r.t1[:-1] - r.t2[:-1]) > 1e-9  # A-8: once idempotent either branch is a no-op
+    live = np.abs(r.t1[:-1] - r.t2[:-1]) > 1e-9
     assert np.array_equal(log.branch[live[:log.iters_done]], r.branch[live[:r.iters_done]])
-    if compare_all_branches:
-        assert np.array_equal(log.branch, r.branch)
     assert np.abs(log.t1 - r.t1).max() <= TOL_TR and np.abs(log.t2 - r.t2).max() <= TOL_TR
     assert np.abs(Dg - r.D_val).max() <= TOL_D
-    assert abs(Dg.sum() * 0 + log.t1[-1] - r.t1[-1]) <= TOL_TR
+    assert abs(log.t1[-1] - r.t1[-1]) <= TOL_TR  # |Tr D_gpu - Tr D_oracle| (reading A-11)
 
 
 # ------------------------------------------------------------------------------- main configurations
@@ -108,7 +108,7 @@ def test_config2_water_1024(gbe):
     g, ex, Dg, log = run_gpu(gbe, s)
     graph, r = run_oracle(s)
     check_structure(ex, graph, r, g.info)
-    check_density(Dg, log, r, compare_all_branches=False)
+    check_density(Dg, log, r)
     m = np.diff(ex["sub_ptr"])
     assert m.min() > 128 and m.max() > 512  # several tiles and a ragged tail per community
 
@@ -161,7 +161,7 @@ def test_one_partition_equals_exact_projector(gbe):
     g, ex, Dg, log = run_gpu(gbe, s)
     graph, r = run_oracle(s)
     check_structure(ex, graph, r, g.info)
-    check_density(Dg, log, r, compare_all_branches=False)
+    check_density(Dg, log, r)
     D = sp.csr_matrix((Dg, ex["D_col"], ex["D_row_ptr"]), shape=(s.n, s.n)).toarray()
     assert abs(D - o.o_diag(s.H, 256)).max() < 1e-10
     assert abs(log.t1[-1] - s.n_occ) <= 1e-8  # north_star trace bar, attainable here (A-11)
