@@ -117,7 +117,7 @@ int gbe_build_graph(const gbe_csr_view* H, const gbe_graph_opts* opts, const int
   g->n_part = n_part;
   g->tau = opts->tau;
   g->power = power;
-  g->tile = 128;
+  g->tile = 64;
   struct Guard {
     gbe_graph* g;
     ~Guard() { if (g) gbe_free_graph(g); }

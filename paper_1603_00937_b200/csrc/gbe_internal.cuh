@@ -81,7 +81,7 @@ struct gbe_tile_item {  // one X^2 work item: tile (ti, tj), ti <= tj, of commun
 // ----------------------------------------------------------------------------------------------
 struct gbe_graph {
   int64_t n = 0, nnz_S = 0, sum_m = 0, nnz_D = 0, dense_elems = 0;
-  int32_t n_part = 0, max_m = 0, max_ncore = 0, tile = 128;
+  int32_t n_part = 0, max_m = 0, max_ncore = 0, tile = 64;
   double eps_min = 0, eps_max = 0, tau = 0, flops_per_iter = 0, exec_flops_per_iter = 0;
   int32_t power = 2, contiguous = 1;
   // device arrays (owned)
