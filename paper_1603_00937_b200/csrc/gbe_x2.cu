@@ -8,15 +8,22 @@
 // FP64 tensor cores: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4 - tcgen05 has no f64 kind).  The DMMA pipe is the
 // bound (37 TFLOP/s measured, one DMMA per 16 cycles per SM sub-partition), so the design spends everything else
 // to keep that pipe on USEFUL flops:
-//   - 64x64 CTA tiles, 4 warps of 32x32 (16 accumulator pairs), 3 CTAs per SM: the epilogue of one CTA (stores,
-//     mirrored stores, the X read of the 2X - X^2 branch) overlaps the main loops of the other two;
+//   - 64x64 CTA tiles, 4 warps with 16 accumulator pairs each, 4 CTAs per SM: the epilogue of one CTA (stores,
+//     mirrored stores, the X read of the 2X - X^2 branch) overlaps the main loops of the other three;
 //   - work skipped at 8x8 granularity with warp-uniform masks: sub-tiles strictly below the diagonal (their values
 //     arrive by the mirrored store) and sub-tiles beyond the ragged edge m_p.  Executed flops ~ 0.52 x 2 m^3;
-//   - in a diagonal CTA the warp whose 32x32 block lies below the diagonal is idle; the warp -> block map rotates
-//     with the CTA index so that the idle warp does not always sit on the same SM sub-partition;
-//   - panels staged by a 3-stage cp.async pipeline in 128-byte rows (K chunk = 16 doubles), read with conflict-free
-//     64-bit loads (row stride 20 doubles).  Loads of rows >= m_p are zero-filled, stores predicated; pad columns
-//     [m_p, ld_p) stay zero by construction.
+//   - a CTA runs in lockstep (one barrier per K chunk), so its four warps - one per SM sub-partition, each with its
+//     own DMMA pipe - must carry equal work or the lighter sub-partitions idle: warp w owns the 8-row blocks
+//     {w, 7 - w} x all eight 8-column blocks, which gives every warp 9 of the 36 upper-triangle sub-tiles of a
+//     diagonal tile and an equal share of a ragged right edge; the map rotates with the CTA index;
+//   - measured on B200 (profiles/r01_fp64_peak_probe.md): every non-DMMA ALU instruction a warp issues costs ~1.4
+//     cycles of its sub-partition's DMMA pipe (shared-memory loads cost almost nothing), so the main loop is pared
+//     down to 64 DMMA + 32 LDS.64 + 8 LDGSTS per K chunk: per-thread copy pointers live in registers, rows beyond
+//     the ragged edge are clamped to row m_p - 1 instead of predicated (their products are never stored), stage
+//     and K offsets are immediates of a loop unrolled over the two stages, and the sub-tile masks are compile-time
+//     patterns (full / upper triangle) with a predicated fallback for edge tiles only;
+//   - panels staged by a 2-stage cp.async pipeline in 128-byte rows (K chunk = 16 doubles), read with conflict-free
+//     64-bit loads (row stride 20 doubles).  Stores are predicated; pad columns [m_p, ld_p) are written as zeros.
 //
 // Fused epilogue (warp-shuffle partials, north_star item 3): while X_{n+1} is written, accumulate over the core
 // rows  t1 = sum_i X_ii  and  t2 = sum_i sum_c X_ic^2 (= Tr_core(X^2) for symmetric X), one fixed-order partial
@@ -26,35 +33,71 @@
 
 namespace {
 
-constexpr int X2_STRIDE = GBE_KC + 4;  // doubles per shared-memory row: 20 -> 8*row mod 32 banks, conflict-free
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(c0), "+d"(c1)
                : "d"(a), "d"(b));
 }
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, bool pred) {
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
   const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
-  const int sz = pred ? 16 : 0;  // src-size 0: the 16 bytes are zero-filled
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(sz));
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc));
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
 
 constexpr int X2_BT = 64;       // CTA tile edge
-constexpr int X2_WT = 32;       // warp tile edge (2 x 2 warps)
 constexpr int X2_THREADS = 128;
+constexpr int X2_KC = GBE_KC;                    // K chunk: 16 doubles = one 128-byte line per row
+constexpr int X2_STRIDE = X2_KC + 4;             // doubles per shared-memory row: 8 banks mod 32 -> conflict-free LDS.64
+constexpr int X2_PANEL = X2_BT * X2_STRIDE;      // doubles per panel per stage
+constexpr int X2_STAGE = 2 * X2_PANEL;           // A panel + B panel
+constexpr unsigned X2_FULL = 0xFFFFu;
 
-template <int STAGES>
-__global__ void __launch_bounds__(X2_THREADS, 3)
+// Sub-tile masks, bit (i * 8 + j): the warp with role w owns the 8-row blocks {w, 7 - w} (i = 0, 1) and all eight
+// 8-column blocks j of the 64 x 64 tile.  In a diagonal tile row block b needs the columns j >= b only, so every
+// warp has exactly 9 of the 36 upper-triangle sub-tiles: the four warps (one per SM sub-partition) stay balanced.
+__host__ __device__ constexpr unsigned x2_diag_mask(int w) {
+  return ((0xFFu << w) & 0xFFu) | (((0xFFu << (7 - w)) & 0xFFu) << 8);
+}
+
+// one K chunk of the warp's 2 x 8 sub-tiles: 4 k-steps of 10 LDS.64 + (up to) 16 DMMA; MASK is a compile-time
+// pattern, MASK == 0 means "use the run-time mask"
+template <unsigned MASK>
+__device__ __forceinline__ void x2_chunk(double (&acc)[2][8][2], const double* __restrict__ pa0,
+                                         const double* __restrict__ pa1, const double* __restrict__ pb,
+                                         unsigned rt_mask) {
+#pragma unroll
+  for (int ks = 0; ks < X2_KC / 4; ++ks) {
+    double a[2], b[8];
+    a[0] = pa0[ks * 4];
+    a[1] = pa1[ks * 4];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const bool need = MASK == 0 || ((MASK | (MASK >> 8)) & (1u << j));
+      if (need) b[j] = pb[j * 8 * X2_STRIDE + ks * 4];
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        if (MASK != 0) {
+          if (MASK & (1u << (i * 8 + j))) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        } else {
+          if (rt_mask & (1u << (i * 8 + j))) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+      }
+  }
+}
+
+template <int MINB>
+__global__ void __launch_bounds__(X2_THREADS, MINB)
     k_x2(const gbe_tile_item* __restrict__ items, const int64_t* __restrict__ sub_ptr,
          const int32_t* __restrict__ ncore_arr, const int64_t* __restrict__ dense_off,
          const gbe_state* __restrict__ st, const double* __restrict__ Xin, double* __restrict__ Xout,
          double* __restrict__ partials) {
-  constexpr int SUB = X2_WT / 8;  // 4 x 4 sub-tiles of 8 x 8 per warp
-  constexpr int STAGE_ELEMS = 2 * X2_BT * X2_STRIDE;
-  extern __shared__ __align__(16) double smem[];
+  extern __shared__ __align__(16) double smem[];  // 2 stages x (A panel, B panel)
   __shared__ double red[8];
 
   if (st->stop) return;  // idempotency stop already fired (A-7): X is final
@@ -69,115 +112,101 @@ __global__ void __launch_bounds__(X2_THREADS, 3)
   double* __restrict__ Y = Xout + dense_off[p];
   const bool diag = (ti == tj);
   const int row0 = ti * X2_BT, col0 = tj * X2_BT;
-  const int nchunks = ld / GBE_KC;
+  const int nchunks = ld / X2_KC;
 
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
-  const int role = (wid + blockIdx.x) & 3;  // rotate: the idle warp of a diagonal CTA changes sub-partition
-  const int wm = role >> 1, wn = role & 1;
+  const int role = (wid + blockIdx.x) & 3;  // rotate the warp -> row-block map over the SM sub-partitions
   const int g = lane >> 2, q = lane & 3;
-  const int wr0 = row0 + wm * X2_WT, wc0 = col0 + wn * X2_WT;  // first row / column of the warp tile
+  const int rblk[2] = {role, 7 - role};
 
-  // warp-uniform masks over the 4 x 4 sub-tiles: bit (i * 4 + j)
-  //   active: rows < m, columns < ld, and not strictly below the diagonal;  mirrored: strictly above the diagonal
+  // warp-uniform masks over the 2 x 8 sub-tiles, bit (i * 8 + j):
+  //   active: rows < m, columns < ld, not strictly below the diagonal;  mirror: strictly above the diagonal
   unsigned active = 0, mirror = 0;
 #pragma unroll
-  for (int i = 0; i < SUB; ++i)
+  for (int i = 0; i < 2; ++i)
 #pragma unroll
-    for (int j = 0; j < SUB; ++j) {
-      const int r8 = wr0 + 8 * i, c8 = wc0 + 8 * j;
+    for (int j = 0; j < 8; ++j) {
+      const int r8 = row0 + 8 * rblk[i], c8 = col0 + 8 * j;
       if (r8 < m && c8 < ld && r8 <= c8) {
-        active |= 1u << (i * 4 + j);
-        if (r8 < c8) mirror |= 1u << (i * 4 + j);
+        active |= 1u << (i * 8 + j);
+        if (r8 < c8) mirror |= 1u << (i * 8 + j);
       }
     }
 
-  auto load_stage = [&](int stage, int kc) {
-    double* sA = smem + (size_t)stage * STAGE_ELEMS;
-    double* sB = sA + X2_BT * X2_STRIDE;
-    const int k0 = kc * GBE_KC;
+  // copy slots of this thread: rows (t >> 3) + 16 u, u = 0..3, 16-byte chunk (t & 7) of each K chunk.
+  // Rows beyond the edge are clamped to row m - 1: finite data whose products are never stored.
+  const double* gA[4];
+  const double* gB[4];
 #pragma unroll
-    for (int c = t; c < X2_BT * 8; c += X2_THREADS) {
-      const int r = c >> 3, ch = c & 7;
-      const int gr = row0 + r;
-      const bool ok = gr < m;
-      cp_async16(sA + r * X2_STRIDE + ch * 2, X + (size_t)(ok ? gr : 0) * ld + k0 + ch * 2, ok);
-    }
+  for (int u = 0; u < 4; ++u) {
+    const int r = (t >> 3) + 16 * u;
+    gA[u] = X + (size_t)min(row0 + r, m - 1) * ld + (t & 7) * 2;
+    gB[u] = X + (size_t)min(col0 + r, m - 1) * ld + (t & 7) * 2;
+  }
+  double* const sdst = smem + (t >> 3) * X2_STRIDE + (t & 7) * 2;  // slot 0 of the A panel of stage 0
+
+  auto issue = [&](int stage, int kofs) {  // both arguments are compile-time constants after unrolling
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      cp_async16(sdst + stage * X2_STAGE + u * 16 * X2_STRIDE, gA[u] + kofs);
     if (!diag) {
 #pragma unroll
-      for (int c = t; c < X2_BT * 8; c += X2_THREADS) {
-        const int r = c >> 3, ch = c & 7;
-        const int gr = col0 + r;
-        const bool ok = gr < m;
-        cp_async16(sB + r * X2_STRIDE + ch * 2, X + (size_t)(ok ? gr : 0) * ld + k0 + ch * 2, ok);
-      }
+      for (int u = 0; u < 4; ++u)
+        cp_async16(sdst + stage * X2_STAGE + X2_PANEL + u * 16 * X2_STRIDE, gB[u] + kofs);
+    }
+    cp_async_commit();
+  };
+
+  double acc[2][8][2];
+#pragma unroll
+  for (int i = 0; i < 2; ++i)
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+  const double* const pa0 = smem + (rblk[0] * 8 + g) * X2_STRIDE + q;
+  const double* const pa1 = smem + (rblk[1] * 8 + g) * X2_STRIDE + q;
+  const double* const pb0 = smem + (diag ? 0 : X2_PANEL) + g * X2_STRIDE + q;
+  // warp-uniform code path: 0 full, 1..4 the diagonal pattern of role 0..3, 5 run-time mask (ragged edge), 6 idle
+  const int pattern = active == X2_FULL ? 0 : (active == x2_diag_mask(role) ? 1 + role : (active ? 5 : 6));
+  auto compute = [&](int stage) {
+    const double* a0 = pa0 + stage * X2_STAGE;
+    const double* a1 = pa1 + stage * X2_STAGE;
+    const double* pb = pb0 + stage * X2_STAGE;
+    switch (pattern) {
+      case 0: x2_chunk<X2_FULL>(acc, a0, a1, pb, 0); break;
+      case 1: x2_chunk<x2_diag_mask(0)>(acc, a0, a1, pb, 0); break;
+      case 2: x2_chunk<x2_diag_mask(1)>(acc, a0, a1, pb, 0); break;
+      case 3: x2_chunk<x2_diag_mask(2)>(acc, a0, a1, pb, 0); break;
+      case 4: x2_chunk<x2_diag_mask(3)>(acc, a0, a1, pb, 0); break;
+      case 5: x2_chunk<0>(acc, a0, a1, pb, active); break;
+      default: break;
     }
   };
 
-  double acc[SUB][SUB][2];
-#pragma unroll
-  for (int i = 0; i < SUB; ++i)
-#pragma unroll
-    for (int j = 0; j < SUB; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-#pragma unroll
-  for (int s = 0; s < STAGES - 1; ++s) {
-    if (s < nchunks) load_stage(s, s);
-    cp_async_commit();
-  }
-
-  for (int kc = 0; kc < nchunks; ++kc) {
-    cp_async_wait<STAGES - 2>();
+  issue(0, 0);
+  for (int kc = 0; kc < nchunks; kc += 2) {
+    cp_async_wait<0>();
+    __syncthreads();  // chunk kc has landed for every thread; every warp is done with the other stage
+    if (kc + 1 < nchunks) issue(1, X2_KC);
+    compute(0);
+    if (kc + 1 >= nchunks) break;
+    cp_async_wait<0>();
     __syncthreads();
-    {
-      const int nk = kc + STAGES - 1;
-      if (nk < nchunks) load_stage(nk % STAGES, nk);
-      cp_async_commit();
-    }
-    if (active == 0) continue;  // warp-uniform: this warp's block lies below the diagonal or beyond the edge
-    const double* sA = smem + (size_t)(kc % STAGES) * STAGE_ELEMS;
-    const double* sB = diag ? sA : sA + X2_BT * X2_STRIDE;
-    const double* pa = sA + (wm * X2_WT + g) * X2_STRIDE + q;
-    const double* pb = sB + (wn * X2_WT + g) * X2_STRIDE + q;
-    if (active == 0xFFFFu) {
+    if (kc + 2 < nchunks) issue(0, 2 * X2_KC);
+    compute(1);
 #pragma unroll
-      for (int ks = 0; ks < GBE_KC / 4; ++ks) {
-        double a[SUB], b[SUB];
-#pragma unroll
-        for (int i = 0; i < SUB; ++i) a[i] = pa[i * 8 * X2_STRIDE + ks * 4];
-#pragma unroll
-        for (int j = 0; j < SUB; ++j) b[j] = pb[j * 8 * X2_STRIDE + ks * 4];
-#pragma unroll
-        for (int i = 0; i < SUB; ++i)
-#pragma unroll
-          for (int j = 0; j < SUB; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-      }
-    } else {
-#pragma unroll
-      for (int ks = 0; ks < GBE_KC / 4; ++ks) {
-        double a[SUB], b[SUB];
-#pragma unroll
-        for (int i = 0; i < SUB; ++i) a[i] = pa[i * 8 * X2_STRIDE + ks * 4];
-#pragma unroll
-        for (int j = 0; j < SUB; ++j) b[j] = pb[j * 8 * X2_STRIDE + ks * 4];
-#pragma unroll
-        for (int i = 0; i < SUB; ++i)
-#pragma unroll
-          for (int j = 0; j < SUB; ++j)
-            if (active & (1u << (i * 4 + j))) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-      }
-    }
+    for (int u = 0; u < 4; ++u) { gA[u] += 2 * X2_KC; gB[u] += 2 * X2_KC; }
   }
-  cp_async_wait<0>();
 
   // epilogue: X_{n+1} = Y or 2 X_n - Y, direct + mirrored store, core-row trace partials
   double s1 = 0.0, s2 = 0.0;
 #pragma unroll
-  for (int i = 0; i < SUB; ++i) {
-    const int r = wr0 + i * 8 + g;
+  for (int i = 0; i < 2; ++i) {
+    const int r = row0 + rblk[i] * 8 + g;
 #pragma unroll
-    for (int j = 0; j < SUB; ++j) {
-      if (!(active & (1u << (i * 4 + j)))) continue;
-      const int c = wc0 + j * 8 + 2 * q;
+    for (int j = 0; j < 8; ++j) {
+      if (!(active & (1u << (i * 8 + j)))) continue;
+      const int c = col0 + j * 8 + 2 * q;
       if (r < m) {  // c < ld holds for every active sub-tile
         double v0 = acc[i][j][0], v1 = acc[i][j][1];
         if (branch) {
@@ -185,13 +214,15 @@ __global__ void __launch_bounds__(X2_THREADS, 3)
           v0 = 2.0 * x.x - v0;
           v1 = 2.0 * x.y - v1;
         }
+        if (c >= m) v0 = 0.0;  // pad columns [m, ld) stay zero (the clamped rows above put finite junk here)
+        if (c + 1 >= m) v1 = 0.0;
         *reinterpret_cast<double2*>(Y + (size_t)r * ld + c) = make_double2(v0, v1);
         if (r < nc) {
           s2 += v0 * v0 + v1 * v1;
           if (r == c) s1 += v0;
           if (r == c + 1) s1 += v1;
         }
-        if (mirror & (1u << (i * 4 + j))) {
+        if (mirror & (1u << (i * 8 + j))) {
           if (c < m) {
             Y[(size_t)c * ld + r] = v0;
             if (c < nc) s2 += v0 * v0;
@@ -214,15 +245,10 @@ __global__ void __launch_bounds__(X2_THREADS, 3)
   }
 }
 
-}  // namespace
-
-int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                  cudaStream_t s) {
-  (void)iter;
-  if (g->n_items == 0) return GBE_OK;
-  constexpr int STAGES = 3;
-  auto kern = k_x2<STAGES>;
-  const size_t smem = (size_t)STAGES * 2 * X2_BT * X2_STRIDE * sizeof(double);
+template <int MINB>
+int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, cudaStream_t s) {
+  auto kern = k_x2<MINB>;
+  const size_t smem = (size_t)2 * X2_STAGE * sizeof(double);
   static bool configured = false;
   if (!configured) {
     GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -232,4 +258,12 @@ int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* 
   kern<<<g->n_items, X2_THREADS, smem, s>>>(g->items, g->sub_ptr, g->ncore, g->dense_off, st, Xin, Xout, partials);
   GBE_LAUNCHED();
   return GBE_OK;
+}
+}  // namespace
+
+int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
+                  cudaStream_t s) {
+  (void)iter;
+  if (g->n_items == 0) return GBE_OK;
+  return launch_x2<4>(g, st, Xin, Xout, partials, s);
 }
