@@ -163,6 +163,25 @@ def run_reference(args) -> None:
 
 
 # ------------------------------------------------------------------------------------------------
+# N > 1: replicas only - the single cross-rank step is the reduction of the timings
+# ------------------------------------------------------------------------------------------------
+def over_ranks(x: float, op: str, device: str) -> float:
+    """max / sum of a per-rank scalar over all ranks (identity when torch.distributed is not initialised)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def job_throughput(units_all_ranks: float, steps: int, ms_max_over_ranks: float) -> float:
+    """Whole-job throughput: units processed by ALL ranks per step x steps / the slowest rank's time."""
+    return units_all_ranks * steps / (ms_max_over_ranks * 1e-3)
+
+
+# ------------------------------------------------------------------------------------------------
 # the CUDA path
 # ------------------------------------------------------------------------------------------------
 def pinned_host_csr(H):
@@ -272,24 +291,10 @@ def run_ours(args) -> None:
     torch.cuda.synchronize()
     graph_ms = e0.elapsed_time(e1)
 
-    def allmax(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
-    def allsum(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
-
-    total_ms_max, e2e_ms_max = allmax(total_ms), allmax(e2e_ms)
-    orbitals_all = allsum(float(s.n))
-    value = orbitals_all * args.steps / (total_ms_max * 1e-3)
-    e2e_value = orbitals_all * args.steps / (e2e_ms_max * 1e-3)
+    total_ms_max, e2e_ms_max = over_ranks(total_ms, "max", "cuda"), over_ranks(e2e_ms, "max", "cuda")
+    orbitals_all = over_ranks(float(s.n), "sum", "cuda")
+    value = job_throughput(orbitals_all, args.steps, total_ms_max)
+    e2e_value = job_throughput(orbitals_all, args.steps, e2e_ms_max)
 
     if rank == 0:
         peaks = load_peaks()
