@@ -71,7 +71,9 @@ __global__ void __launch_bounds__(256) k_materialise_A(int64_t n, const int64_t*
 }
 
 // ---------------------------------------------------------------- T_next = floor(A T)_tau
-// MODE 0: distinct candidate columns per row (sizes the accumulator); 1: count kept entries; 2: fill.
+// MODE 0: distinct candidate columns per row (sizes the accumulator); 1: count kept entries; 2: fill (columns + values);
+// 3: one pass for the LAST power, whose values are not needed: kept columns go to a scratch row of candidate capacity
+//    (offsets out_rp from MODE 0's counts) and cnt[i] = number kept.
 template <int MODE>
 __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __restrict__ A_rp,
                                    const int32_t* __restrict__ A_col, const double* __restrict__ A_val,
@@ -144,7 +146,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
     }
     // emit kept entries in ascending column order
     int kept = 0;
-    const int64_t ob = MODE == 2 ? out_rp[i] : 0;
+    const int64_t ob = (MODE == 2 || MODE == 3) ? out_rp[i] : 0;
     for (int w0 = 0; w0 < W; w0 += 32) {
       const int w = w0 + lane;
       uint32_t bits = w < W ? bm[w] : 0u;
@@ -161,7 +163,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
       }
       int tot;
       const int ex = warp_excl_scan_i(mine, lane, &tot);
-      if (MODE == 2) {
+      if (MODE == 2 || MODE == 3) {
         int pos = kept + ex, idx = 0;
         while (bits) {
           const int bpos = __ffs(bits) - 1;
@@ -170,14 +172,14 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
           ++idx;
           if (fabs(v) >= tau) {
             out_col[ob + pos] = w * 32 + bpos;
-            out_val[ob + pos] = v;
+            if (MODE == 2) out_val[ob + pos] = v;
             ++pos;
           }
         }
       }
       kept += tot;
     }
-    if (MODE == 1 && lane == 0) cnt[i] = kept;
+    if ((MODE == 1 || MODE == 3) && lane == 0) cnt[i] = kept;
     __syncwarp();
   }
 }
@@ -185,7 +187,8 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
 // ---------------------------------------------------------------- row-wise union of two patterns (+ self loops)
 template <bool FILL>
 __global__ void k_union_rows(int64_t n, int W, const int64_t* __restrict__ P_rp, const int32_t* __restrict__ P_col,
-                             const int64_t* __restrict__ Q_rp, const int32_t* __restrict__ Q_col, int add_diag,
+                             const int64_t* __restrict__ Q_rp, const int32_t* __restrict__ Q_col,
+                             const int32_t* __restrict__ Q_len /* null: compact CSR */, int add_diag,
                              int32_t* __restrict__ cnt, const int64_t* __restrict__ out_rp,
                              int32_t* __restrict__ out_col) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -195,8 +198,10 @@ __global__ void k_union_rows(int64_t n, int W, const int64_t* __restrict__ P_rp,
     for (int w = lane; w < W; w += 32) bm[w] = 0u;
     __syncwarp();
     for (int64_t e = P_rp[i] + lane; e < P_rp[i + 1]; e += 32) { const int j = P_col[e]; atomicOr(&bm[j >> 5], 1u << (j & 31)); }
-    if (Q_rp)
-      for (int64_t e = Q_rp[i] + lane; e < Q_rp[i + 1]; e += 32) { const int j = Q_col[e]; atomicOr(&bm[j >> 5], 1u << (j & 31)); }
+    if (Q_rp) {
+      const int64_t qb = Q_rp[i], qe = Q_len ? qb + Q_len[i] : Q_rp[i + 1];
+      for (int64_t e = qb + lane; e < qe; e += 32) { const int j = Q_col[e]; atomicOr(&bm[j >> 5], 1u << (j & 31)); }
+    }
     if (add_diag && lane == 0) atomicOr(&bm[i >> 5], 1u << (i & 31));
     __syncwarp();
     int total = 0;
@@ -334,21 +339,23 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   GBE_CUDA(cudaFuncSetAttribute(k_union_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bm_bytes * uw)));
   const int ugrid = (int)std::min<int64_t>((n + uw - 1) / uw, (int64_t)sm_count * 8);
 
-  auto do_union = [&](const int64_t* p_rp, const int32_t* p_col, const int64_t* q_rp, const int32_t* q_col, int diag,
-                      Pattern& out) -> int {
-    k_union_rows<false><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, q_rp, q_col, diag, cnt.as<int32_t>(),
-                                                              nullptr, nullptr);
+  DevBuf ucnt;  // row counts of the union being sized (cnt may hold the Q_len of a scratch pattern)
+  GBE_TRY(ucnt.alloc((size_t)n * 4));
+  auto do_union = [&](const int64_t* p_rp, const int32_t* p_col, const int64_t* q_rp, const int32_t* q_col,
+                      const int32_t* q_len, int diag, Pattern& out) -> int {
+    k_union_rows<false><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, q_rp, q_col, q_len, diag,
+                                                              ucnt.as<int32_t>(), nullptr, nullptr);
     GBE_LAUNCHED();
-    GBE_TRY(count_to_rowptr(cnt, n, out.rp, &out.nnz, s));
+    GBE_TRY(count_to_rowptr(ucnt, n, out.rp, &out.nnz, s));
     GBE_TRY(out.col.alloc((size_t)out.nnz * 4));
-    k_union_rows<true><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, q_rp, q_col, diag, nullptr,
+    k_union_rows<true><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, q_rp, q_col, q_len, diag, nullptr,
                                                              out.rp.as<int64_t>(), out.col.as<int32_t>());
     GBE_LAUNCHED();
     return GBE_OK;
   };
 
   Pattern P;
-  GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), nullptr, nullptr, 1, P));
+  GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), nullptr, nullptr, nullptr, 1, P));
 
   // thresholded powers
   Pattern Tprev;  // T^(k-1) with values; T^(1) aliases A
@@ -380,6 +387,27 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
     GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
     const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
+    if (k == power) {
+      // last power: only its pattern enters S - one numeric pass into scratch rows of candidate capacity
+      GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
+      Pattern Tc;  // scratch: rp = offsets by candidate count, col = kept columns, cnt = kept per row
+      int64_t total_cand = 0;
+      GBE_TRY(count_to_rowptr(cnt, n, Tc.rp, &total_cand, s));
+      GBE_TRY(Tc.col.alloc((size_t)total_cand * 4));
+      k_spgemm_threshold<3><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, A.rp.as<int64_t>(), A.col.as<int32_t>(),
+                                                                 A.val.as<double>(), T_rp, T_col, T_val, tau,
+                                                                 cnt.as<int32_t>(), Tc.rp.as<int64_t>(),
+                                                                 Tc.col.as<int32_t>(), nullptr);
+      GBE_LAUNCHED();
+      Pattern Pn;
+      GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tc.rp.as<int64_t>(), Tc.col.as<int32_t>(),
+                       cnt.as<int32_t>(), 0, Pn));
+      GBE_CUDA(cudaStreamSynchronize(s));
+      std::swap(P.rp.p, Pn.rp.p);
+      std::swap(P.col.p, Pn.col.p);
+      P.nnz = Pn.nnz;
+      break;
+    }
     Pattern Tn;
     k_spgemm_threshold<1><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, A.rp.as<int64_t>(), A.col.as<int32_t>(),
                                                                A.val.as<double>(), T_rp, T_col, T_val, tau,
@@ -394,7 +422,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                                Tn.val.as<double>());
     GBE_LAUNCHED();
     Pattern Pn;
-    GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(), 0, Pn));
+    GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(), nullptr, 0, Pn));
     GBE_CUDA(cudaStreamSynchronize(s));
     std::swap(P.rp.p, Pn.rp.p);
     std::swap(P.col.p, Pn.col.p);
@@ -421,7 +449,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                              cnt.as<int32_t>(), PT.col.as<int32_t>());
   GBE_LAUNCHED();
   Pattern S;
-  GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(), PT.col.as<int32_t>(), 0, S));
+  GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(), PT.col.as<int32_t>(), nullptr, 0, S));
   GBE_CUDA(cudaStreamSynchronize(s));
   *nnz_S = S.nnz;
   *S_row_ptr = reinterpret_cast<int64_t*>(S.rp.release());

@@ -29,6 +29,8 @@
 // rows  t1 = sum_i X_ii  and  t2 = sum_i sum_c X_ic^2 (= Tr_core(X^2) for symmetric X), one fixed-order partial
 // per work item, so that the branch of the NEXT iteration is known before its GEMM starts.
 // Bound: FP64 tensor pipe - 2 m^3 algorithmic flop per community per iteration (~m^3 executed thanks to symmetry).
+#include <type_traits>
+
 #include "gbe_internal.cuh"
 
 namespace {
@@ -198,42 +200,58 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
     for (int u = 0; u < 4; ++u) { gA[u] += 2 * X2_KC; gB[u] += 2 * X2_KC; }
   }
 
-  // epilogue: X_{n+1} = Y or 2 X_n - Y, direct + mirrored store, core-row trace partials
+  // epilogue: X_{n+1} = Y or 2 X_n - Y, direct + mirrored store, core-row trace partials.
+  // Interior tiles (no ragged edge, no core row or column: most of them) take the path without any predicate.
   double s1 = 0.0, s2 = 0.0;
+  auto epilogue = [&](auto edge_c, auto trace_c) {
+    constexpr bool EDGE = decltype(edge_c)::value, TRACE = decltype(trace_c)::value;
 #pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    const int r = row0 + rblk[i] * 8 + g;
+    for (int i = 0; i < 2; ++i) {
+      const int r = row0 + rblk[i] * 8 + g;
+      if (EDGE && r >= m) continue;
+      const double* __restrict__ xr = X + (size_t)r * ld + col0 + 2 * q;
+      double* __restrict__ yr = Y + (size_t)r * ld + col0 + 2 * q;
+      double* __restrict__ ym = Y + (size_t)(col0 + 2 * q) * ld + r;  // mirrored position of column block 0
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      if (!(active & (1u << (i * 8 + j)))) continue;
-      const int c = col0 + j * 8 + 2 * q;
-      if (r < m) {  // c < ld holds for every active sub-tile
+      for (int j = 0; j < 8; ++j) {
+        if (!(active & (1u << (i * 8 + j)))) continue;  // c < ld holds for every active sub-tile
+        const int c = col0 + j * 8 + 2 * q;
         double v0 = acc[i][j][0], v1 = acc[i][j][1];
         if (branch) {
-          const double2 x = *reinterpret_cast<const double2*>(X + (size_t)r * ld + c);
+          const double2 x = *reinterpret_cast<const double2*>(xr + j * 8);
           v0 = 2.0 * x.x - v0;
           v1 = 2.0 * x.y - v1;
         }
-        if (c >= m) v0 = 0.0;  // pad columns [m, ld) stay zero (the clamped rows above put finite junk here)
-        if (c + 1 >= m) v1 = 0.0;
-        *reinterpret_cast<double2*>(Y + (size_t)r * ld + c) = make_double2(v0, v1);
-        if (r < nc) {
+        if (EDGE) {  // pad columns [m, ld) stay zero (the clamped rows above put finite junk here)
+          if (c >= m) v0 = 0.0;
+          if (c + 1 >= m) v1 = 0.0;
+        }
+        *reinterpret_cast<double2*>(yr + j * 8) = make_double2(v0, v1);
+        if (TRACE && r < nc) {
           s2 += v0 * v0 + v1 * v1;
           if (r == c) s1 += v0;
           if (r == c + 1) s1 += v1;
         }
         if (mirror & (1u << (i * 8 + j))) {
-          if (c < m) {
-            Y[(size_t)c * ld + r] = v0;
-            if (c < nc) s2 += v0 * v0;
+          if (!EDGE || c < m) {
+            ym[(size_t)(j * 8) * ld] = v0;
+            if (TRACE && c < nc) s2 += v0 * v0;
           }
-          if (c + 1 < m) {
-            Y[(size_t)(c + 1) * ld + r] = v1;
-            if (c + 1 < nc) s2 += v1 * v1;
+          if (!EDGE || c + 1 < m) {
+            ym[(size_t)(j * 8 + 1) * ld] = v1;
+            if (TRACE && c + 1 < nc) s2 += v1 * v1;
           }
         }
       }
     }
+  };
+  const bool edge = col0 + X2_BT > m;             // row0 <= col0: the row edge implies the column edge
+  const bool trace = row0 < nc || col0 < nc;      // a core row, directly or through the mirror
+  if (edge || trace) {
+    if (edge) epilogue(std::true_type{}, std::true_type{});
+    else epilogue(std::false_type{}, std::true_type{});
+  } else {
+    epilogue(std::false_type{}, std::false_type{});
   }
   s1 = warp_sum(s1);
   s2 = warp_sum(s2);
