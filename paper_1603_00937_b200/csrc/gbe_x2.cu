@@ -64,6 +64,10 @@ __host__ __device__ constexpr unsigned x2_diag_mask(int w) {
   return ((0xFFu << w) & 0xFFu) | (((0xFFu << (7 - w)) & 0xFFu) << 8);
 }
 
+__host__ __device__ constexpr unsigned x2_cols_mask(int nb) {  // the first nb column blocks of both row blocks
+  return ((1u << nb) - 1u) | (((1u << nb) - 1u) << 8);
+}
+
 // one K chunk of the warp's 2 x 8 sub-tiles: 4 k-steps of 10 LDS.64 + (up to) 16 DMMA; MASK is a compile-time
 // pattern, MASK == 0 means "use the run-time mask"
 template <unsigned MASK>
@@ -168,8 +172,16 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   const double* const pa0 = smem + (rblk[0] * 8 + g) * X2_STRIDE + q;
   const double* const pa1 = smem + (rblk[1] * 8 + g) * X2_STRIDE + q;
   const double* const pb0 = smem + (diag ? 0 : X2_PANEL) + g * X2_STRIDE + q;
-  // warp-uniform code path: 0 full, 1..4 the diagonal pattern of role 0..3, 5 run-time mask (ragged edge), 6 idle
-  const int pattern = active == X2_FULL ? 0 : (active == x2_diag_mask(role) ? 1 + role : (active ? 5 : 6));
+  // warp-uniform code path: 0 full, 1..4 the diagonal pattern of role 0..3, 5..11 the first 1..7 column blocks of
+  // both row blocks (ragged right edge), 12 run-time mask (the last diagonal tile), 13 idle
+  int pattern = active ? 12 : 13;
+  if (active == X2_FULL) pattern = 0;
+  else if (active == x2_diag_mask(role)) pattern = 1 + role;
+  else {
+#pragma unroll
+    for (int nb = 1; nb < 8; ++nb)
+      if (active == x2_cols_mask(nb)) pattern = 4 + nb;
+  }
   auto compute = [&](int stage) {
     const double* a0 = pa0 + stage * X2_STAGE;
     const double* a1 = pa1 + stage * X2_STAGE;
@@ -180,7 +192,14 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
       case 2: x2_chunk<x2_diag_mask(1)>(acc, a0, a1, pb, 0); break;
       case 3: x2_chunk<x2_diag_mask(2)>(acc, a0, a1, pb, 0); break;
       case 4: x2_chunk<x2_diag_mask(3)>(acc, a0, a1, pb, 0); break;
-      case 5: x2_chunk<0>(acc, a0, a1, pb, active); break;
+      case 5: x2_chunk<x2_cols_mask(1)>(acc, a0, a1, pb, 0); break;
+      case 6: x2_chunk<x2_cols_mask(2)>(acc, a0, a1, pb, 0); break;
+      case 7: x2_chunk<x2_cols_mask(3)>(acc, a0, a1, pb, 0); break;
+      case 8: x2_chunk<x2_cols_mask(4)>(acc, a0, a1, pb, 0); break;
+      case 9: x2_chunk<x2_cols_mask(5)>(acc, a0, a1, pb, 0); break;
+      case 10: x2_chunk<x2_cols_mask(6)>(acc, a0, a1, pb, 0); break;
+      case 11: x2_chunk<x2_cols_mask(7)>(acc, a0, a1, pb, 0); break;
+      case 12: x2_chunk<0>(acc, a0, a1, pb, active); break;
       default: break;
     }
   };
