@@ -316,6 +316,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     if (f) return GBE_ENOTSYM;
   }
 
+  gbe_trace("start pattern");
   DevBuf cnt;
   GBE_TRY(cnt.alloc((size_t)n * 4));
 
@@ -331,6 +332,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                   A.col.as<int32_t>(), A.val.as<double>());
   GBE_LAUNCHED();
 
+  gbe_trace("materialise A");
   // pattern accumulator P = I u pat(A)
   const size_t bm_bytes = (size_t)W * 4;
   const int uw = pick_warps(bm_bytes, 8);
@@ -357,6 +359,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   Pattern P;
   GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), nullptr, nullptr, nullptr, 1, P));
 
+  gbe_trace("union I+A");
   // thresholded powers
   Pattern Tprev;  // T^(k-1) with values; T^(1) aliases A
   const int64_t* T_rp = A.rp.as<int64_t>();
@@ -375,6 +378,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                                  cnt.as<int32_t>(), nullptr, nullptr, nullptr);
       GBE_LAUNCHED();
     }
+    gbe_trace("spgemm symbolic");
     std::vector<int32_t> h_cnt((size_t)n);
     GBE_CUDA(cudaMemcpyAsync(h_cnt.data(), cnt.p, (size_t)n * 4, cudaMemcpyDeviceToHost, s));
     GBE_CUDA(cudaStreamSynchronize(s));
@@ -399,6 +403,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                                  cnt.as<int32_t>(), Tc.rp.as<int64_t>(),
                                                                  Tc.col.as<int32_t>(), nullptr);
       GBE_LAUNCHED();
+      gbe_trace("spgemm numeric");
       Pattern Pn;
       GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tc.rp.as<int64_t>(), Tc.col.as<int32_t>(),
                        cnt.as<int32_t>(), 0, Pn));
@@ -437,6 +442,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     // Tn (now holding the previous T) and Pn are released here, after the sync above
   }
 
+  gbe_trace("union P+T");
   // S = P u P^T
   Pattern PT;
   GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
@@ -451,6 +457,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   Pattern S;
   GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(), PT.col.as<int32_t>(), nullptr, 0, S));
   GBE_CUDA(cudaStreamSynchronize(s));
+  gbe_trace("transpose+union");
   *nnz_S = S.nnz;
   *S_row_ptr = reinterpret_cast<int64_t*>(S.rp.release());
   *S_col = reinterpret_cast<int32_t*>(S.col.release());

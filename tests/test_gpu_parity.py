@@ -113,6 +113,72 @@ def test_config2_water_1024(gbe):
     assert m.min() > 128 and m.max() > 512  # several tiles and a ragged tail per community
 
 
+def test_config3_water_4096_full_size(gbe):
+    """BASELINE.json configs[2], the workload bench.py times (24,576 orbitals, 512 communities, 40 iterations):
+    every stored entry of D against the oracle's full expansion (the oracle needs about half a minute here)."""
+    s = gi.config(3)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+    assert g.info["n"] == 24576 and g.info["n_part"] == 512 and log.iters_done == 40
+
+
+def test_config4_reduced_peptide_heterogeneous_sizes(gbe):
+    """BASELINE.json configs[3] at a size the oracle finishes in about a minute: the same construction
+    (random-coil solute + water, reading A-16) with 150 residues in a 30 A cube - 10,626 orbitals, 216 communities
+    given by an explicit partition vector, core+halo sizes 200 ... 1,530 (many tiles, ragged tails, two core sizes)."""
+    s = gi.peptide_water(150, box=30.0, seed=1)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+    m = np.diff(ex["sub_ptr"])
+    assert m.min() < 256 and m.max() > 1400
+
+
+def check_any_size_properties(s, g, ex, Dg, log):
+    """Properties of the path that hold at any size (used where the oracle is too slow to run in full)."""
+    t1, t2, br = log.t1, log.t2, log.branch
+    assert log.iters_done == s.iters and np.isfinite(Dg).all()
+    # spectrum of every X_p stays in [0,1]: 0 <= Tr_core X^2 <= Tr_core X (up to roundoff of a sum of ~n terms)
+    assert (t2 >= -1e-9).all() and (t2 <= t1 + 1e-9 * s.n).all()
+    # the logged branch is the rule of reading A-6 applied to the logged traces
+    for k in range(log.iters_done):
+        if abs(t1[k] - t2[k]) > 1e-9:
+            assert br[k] == (0 if abs(t2[k] - s.n_occ) < abs(2 * t1[k] - t2[k] - s.n_occ) else 1)
+    # the update really was X <- X^2 or 2X - X^2 for EVERY community: the next core trace follows exactly
+    nxt = np.where(br == 0, t2[:-1], 2 * t1[:-1] - t2[:-1])
+    assert np.abs(t1[1:] - nxt).max() <= 1e-9 * max(1.0, s.n_occ)
+    D = sp.csr_matrix((Dg, ex["D_col"], ex["D_row_ptr"]), shape=(s.n, s.n))
+    assert abs(D.diagonal().sum() - t1[-1]) <= 1e-9 * s.n          # scatter: Tr D = last core trace
+    # X_p is symmetric, so D restricted to core x core of one community is symmetric (sampled communities)
+    rng = np.random.default_rng(0)
+    for p in rng.choice(s.n_part, size=min(8, s.n_part), replace=False):
+        idx = ex["sub_idx"][ex["sub_ptr"][p]:ex["sub_ptr"][p] + ex["ncore"][p]]
+        blk = D[idx][:, idx].toarray()
+        assert np.abs(blk - blk.T).max() <= 1e-11
+    # D is zero outside S' by construction: every stored row index of column i lies in the subgraph of i's community
+    assert D.nnz <= g.info["nnz_D"]
+
+
+@pytest.mark.slow
+def test_config4_full_size_properties(gbe):
+    """BASELINE.json configs[3] at full size (2,000 residues, ~1.2e5 orbitals, 2 x 27 GB dense batch).  The oracle would
+    need ~1e15 flop here, so the full-size run is checked through properties that hold at any size; element-by-element
+    parity of the same construction is test_config4_reduced_peptide_heterogeneous_sizes."""
+    s = gi.config(4)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    assert g.info["n"] == s.n and g.info["max_m"] > 1500
+    check_any_size_properties(s, g, ex, Dg, log)
+
+
+def test_any_size_properties_hold_where_parity_is_known(gbe):
+    s = gi.config(2)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    check_any_size_properties(s, g, ex, Dg, log)
+
+
 # ------------------------------------------------------------------------------- pieces
 def test_iters_zero_returns_gathered_x0(gbe):
     """gather + scatter alone: D = core columns of X0[s,s]; exact up to the rounding of the two bounds."""
