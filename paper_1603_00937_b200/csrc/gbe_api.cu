@@ -110,6 +110,7 @@ int gbe_build_graph(const gbe_csr_view* H, const gbe_graph_opts* opts, const int
   if (power < 1 || power > GBE_MAX_POWER) return GBE_EINVAL;
   if (n_part < 1 || n_part > H->n) return GBE_EINVAL;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  gbe_set_alloc_stream(s);
 
   gbe_graph* g = new (std::nothrow) gbe_graph();
   if (!g) return GBE_ENOMEM;
@@ -307,6 +308,7 @@ int gbe_build_graph_host(const gbe_csr_view* Hh, const gbe_graph_opts* opts, con
   *out = nullptr;
   GBE_TRY(check_csr(Hh));
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  gbe_set_alloc_stream(s);
   DevBuf rp, ci, va, pt;
   GBE_TRY(rp.alloc((size_t)(Hh->n + 1) * 8));
   GBE_TRY(ci.alloc((size_t)Hh->nnz * 4));
@@ -332,6 +334,7 @@ int gbe_density_host(const gbe_csr_view* Hh, const gbe_graph* g, double n_occ, i
   GBE_TRY(check_csr(Hh));
   if (Hh->n != g->n) return GBE_EMISMATCH;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  gbe_set_alloc_stream(s);
   DevBuf rp, ci, va, dv;
   GBE_TRY(rp.alloc((size_t)(Hh->n + 1) * 8));
   GBE_TRY(ci.alloc((size_t)Hh->nnz * 4));

@@ -196,8 +196,7 @@ __global__ void k_d_pattern(int64_t n, int W, const int64_t* __restrict__ memb_p
 
 template <typename T>
 int upload(const std::vector<T>& h, T** d, cudaStream_t s) {
-  cudaError_t e = cudaMalloc((void**)d, std::max<size_t>(16, h.size() * sizeof(T)));
-  if (e != cudaSuccess) { gbe_set_cuda_error(e, "cudaMalloc", __LINE__); return GBE_ENOMEM; }
+  GBE_TRY(gbe_dev_alloc((void**)d, std::max<size_t>(16, h.size() * sizeof(T))));
   if (!h.empty()) GBE_CUDA(cudaMemcpyAsync(*d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, s));
   return GBE_OK;
 }
@@ -241,8 +240,8 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   if (halo_smem > 220 * 1024) return GBE_EINVAL;  // n too large for the shared-memory bitmaps
   GBE_CUDA(cudaFuncSetAttribute(k_halo<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)halo_smem));
   GBE_CUDA(cudaFuncSetAttribute(k_halo<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)halo_smem));
-  GBE_CUDA(cudaMalloc((void**)&g->msize, (size_t)n_part * 4));
-  GBE_CUDA(cudaMalloc((void**)&g->ncore, (size_t)n_part * 4));
+  GBE_TRY(gbe_dev_alloc((void**)&g->msize, (size_t)n_part * 4));
+  GBE_TRY(gbe_dev_alloc((void**)&g->ncore, (size_t)n_part * 4));
   k_halo<false><<<n_part, 256, halo_smem, s>>>(W, core_ptr.as<int64_t>(), core_tmp.as<int32_t>(), g->S_row_ptr, g->S_col,
                                                g->msize, g->ncore, nullptr, nullptr, nullptr);
   GBE_LAUNCHED();
@@ -320,8 +319,8 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
 
   gbe_trace("host layout+lists");
   // ---- fill sub_idx / row_part
-  GBE_CUDA(cudaMalloc((void**)&g->sub_idx, std::max<size_t>(16, (size_t)g->sum_m * 4)));
-  GBE_CUDA(cudaMalloc((void**)&g->row_part, std::max<size_t>(16, (size_t)g->sum_m * 4)));
+  GBE_TRY(gbe_dev_alloc((void**)&g->sub_idx, std::max<size_t>(16, (size_t)g->sum_m * 4)));
+  GBE_TRY(gbe_dev_alloc((void**)&g->row_part, std::max<size_t>(16, (size_t)g->sum_m * 4)));
   k_halo<true><<<n_part, 256, halo_smem, s>>>(W, core_ptr.as<int64_t>(), core_tmp.as<int32_t>(), g->S_row_ptr, g->S_col,
                                               nullptr, nullptr, g->sub_ptr, g->sub_idx, g->row_part);
   GBE_LAUNCHED();
@@ -336,7 +335,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_CUDA(cudaMemsetAsync(mcnt.p, 0, (size_t)n * 4, s));
   k_member_count<<<qgrid, 256, 0, s>>>(sum_m, g->sub_idx, g->row_part, g->ncore, cnt.as<int32_t>(), mcnt.as<int32_t>());
   GBE_LAUNCHED();
-  GBE_CUDA(cudaMalloc((void**)&g->D_row_ptr, (size_t)(n + 1) * 8));
+  GBE_TRY(gbe_dev_alloc((void**)&g->D_row_ptr, (size_t)(n + 1) * 8));
   GBE_TRY(gbe_exclusive_scan_i32_to_i64(cnt.as<int32_t>(), g->D_row_ptr, n, s));
   GBE_TRY(memb_ptr.alloc((size_t)(n + 1) * 8));
   GBE_TRY(gbe_exclusive_scan_i32_to_i64(mcnt.as<int32_t>(), memb_ptr.as<int64_t>(), n, s));
@@ -344,8 +343,8 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_CUDA(cudaMemsetAsync(cursor.p, 0, (size_t)n * 4, s));
   k_member_fill<<<qgrid, 256, 0, s>>>(sum_m, g->sub_idx, memb_ptr.as<int64_t>(), cursor.as<int32_t>(), memb.as<int64_t>());
   GBE_LAUNCHED();
-  GBE_CUDA(cudaMalloc((void**)&g->D_col, std::max<size_t>(16, (size_t)g->nnz_D * 4)));
-  GBE_CUDA(cudaMalloc((void**)&g->scat_base, std::max<size_t>(16, (size_t)sum_m * 8)));
+  GBE_TRY(gbe_dev_alloc((void**)&g->D_col, std::max<size_t>(16, (size_t)g->nnz_D * 4)));
+  GBE_TRY(gbe_dev_alloc((void**)&g->scat_base, std::max<size_t>(16, (size_t)sum_m * 8)));
   const size_t per_warp = (size_t)2 * W * 4;
   int nw = (int)std::min<size_t>(8, (200 * 1024) / per_warp);
   if (nw < 1) return GBE_EINVAL;
@@ -367,7 +366,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     GBE_LAUNCHED();
     GBE_TRY(scat_ofs.alloc((size_t)(sum_m + 1) * 8));
     GBE_TRY(gbe_exclusive_scan_i32_to_i64(rn.as<int32_t>(), scat_ofs.as<int64_t>(), sum_m, s));
-    GBE_CUDA(cudaMalloc((void**)&g->scat_pos, std::max<size_t>(16, (size_t)g->nnz_D * 8)));
+    GBE_TRY(gbe_dev_alloc((void**)&g->scat_pos, std::max<size_t>(16, (size_t)g->nnz_D * 8)));
     k_d_pattern<1><<<dgrid, nw * 32, per_warp * nw, s>>>(n, W, memb_ptr.as<int64_t>(), memb.as<int64_t>(), g->row_part,
                                                          g->sub_ptr, g->sub_idx, g->ncore, g->D_row_ptr, nullptr, nullptr,
                                                          nullptr, scat_ofs.as<int64_t>(), g->scat_pos);

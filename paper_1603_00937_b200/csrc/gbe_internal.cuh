@@ -46,19 +46,25 @@ inline void gbe_trace(const char* label) {
   fprintf(stderr, "[trace] %-28s %8.3f ms\n", label, std::chrono::duration<double, std::milli>(now - last).count());
   last = std::chrono::steady_clock::now();
 }
+// Device allocations of the library come from the device's default stream-ordered memory pool (cudaMallocAsync) with
+// the release threshold lifted, so that the dozens of build-time temporaries cost microseconds instead of a
+// cudaMalloc / cudaFree (device synchronisation) each.  The stream is the one of the current API call.
+void gbe_set_alloc_stream(cudaStream_t s);
+cudaStream_t gbe_alloc_stream();
+int gbe_dev_alloc(void** p, size_t bytes);  // on gbe_alloc_stream(); GBE_ENOMEM on failure
+void gbe_dev_free(void* p);                 // stream-ordered free on gbe_alloc_stream()
+
 // scoped device allocation for build-time temporaries
 struct DevBuf {
   void* p = nullptr;
   DevBuf() = default;
   DevBuf(const DevBuf&) = delete;
   DevBuf& operator=(const DevBuf&) = delete;
-  ~DevBuf() { if (p) cudaFree(p); }
+  ~DevBuf() { if (p) gbe_dev_free(p); }
   template <typename T> T* as() { return reinterpret_cast<T*>(p); }
   int alloc(size_t bytes) {
-    if (p) { cudaFree(p); p = nullptr; }
-    cudaError_t e = cudaMalloc(&p, bytes ? bytes : 16);
-    if (e != cudaSuccess) { gbe_set_cuda_error(e, "cudaMalloc", __LINE__); p = nullptr; return GBE_ENOMEM; }
-    return GBE_OK;
+    if (p) { gbe_dev_free(p); p = nullptr; }
+    return gbe_dev_alloc(&p, bytes ? bytes : 16);
   }
   void* release() { void* q = p; p = nullptr; return q; }
 };

@@ -1,6 +1,38 @@
 // Small device utilities: exclusive scans used while sizing CSR outputs (not on the per-iteration path).
 #include "gbe_internal.cuh"
 
+// ---------------------------------------------------------------------------------------------- allocator
+namespace {
+thread_local cudaStream_t t_alloc_stream = nullptr;
+}
+void gbe_set_alloc_stream(cudaStream_t s) {
+  static bool pool_ready = false;  // benign race: setting the attribute twice is harmless
+  if (!pool_ready) {
+    int dev = 0;
+    cudaMemPool_t pool;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+      uint64_t keep = UINT64_MAX;  // keep freed blocks in the pool across synchronisations
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    cudaGetLastError();
+    pool_ready = true;
+  }
+  t_alloc_stream = s;
+}
+cudaStream_t gbe_alloc_stream() { return t_alloc_stream; }
+int gbe_dev_alloc(void** p, size_t bytes) {
+  cudaError_t e = cudaMallocAsync(p, bytes ? bytes : 16, t_alloc_stream);
+  if (e != cudaSuccess) {
+    gbe_set_cuda_error(e, "cudaMallocAsync", __LINE__);
+    *p = nullptr;
+    return GBE_ENOMEM;
+  }
+  return GBE_OK;
+}
+void gbe_dev_free(void* p) {
+  if (p) cudaFreeAsync(p, t_alloc_stream);
+}
+
 namespace {
 template <typename TI>
 __global__ void __launch_bounds__(1024) k_scan_single_block(const TI* __restrict__ in, int64_t* __restrict__ out,
