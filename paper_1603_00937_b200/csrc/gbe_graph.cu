@@ -71,6 +71,69 @@ __global__ void __launch_bounds__(256) k_materialise_A(int64_t n, const int64_t*
 }
 
 // ---------------------------------------------------------------- T_next = floor(A T)_tau
+// Walks every product a_ik * t_kj of row i (k ascending; the entries of one T row spread over the lanes) and calls
+// fn(aik, j, t_kj).  The kernels around it are latency bound (a few warps per SM, dependent loads), so the walk is
+// software pipelined: the row pointers of 32 neighbours k are fetched by the 32 lanes at once, and the up to 128
+// entries of the NEXT chunk (same k or the next one) are in flight while the current chunk is processed.
+// ORDERED: a __syncwarp separates consecutive k, because the next k may hit the accumulator slots of this one.
+template <bool NEED_VAL, bool ORDERED, typename F>
+__device__ __forceinline__ void walk_products(int lane, int64_t a, int64_t b, const int32_t* __restrict__ A_col,
+                                              const double* __restrict__ A_val, const int64_t* __restrict__ T_rp,
+                                              const int32_t* __restrict__ T_col, const double* __restrict__ T_val,
+                                              F&& fn) {
+  constexpr unsigned FULL = 0xffffffffu;
+  for (int64_t e0 = a; e0 < b; e0 += 32) {
+    const int64_t e = e0 + lane;
+    const int nk = (int)min((int64_t)32, b - e0);
+    const int kk = e < b ? A_col[e] : 0;
+    const double av = (NEED_VAL && e < b) ? A_val[e] : 0.0;
+    const int64_t tb_l = e < b ? T_rp[kk] : 0;
+    const int64_t te_l = e < b ? T_rp[kk + 1] : 0;
+    int cj[4], nj[4];
+    double cv[4], nv[4];
+    auto fetch = [&](int64_t base, int64_t end, int (&j)[4], double (&v)[4]) {
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const int64_t f = base + lane + 32 * r;
+        j[r] = f < end ? T_col[f] : -1;
+        if (NEED_VAL) v[r] = f < end ? T_val[f] : 0.0;
+      }
+    };
+    // first non-empty chunk
+    int q = 0;
+    int64_t base = 0, end = 0;
+    while (q < nk) {
+      base = __shfl_sync(FULL, tb_l, q);
+      end = __shfl_sync(FULL, te_l, q);
+      if (base < end) break;
+      ++q;
+    }
+    if (q < nk) fetch(base, end, cj, cv);
+    while (q < nk) {
+      // locate and prefetch the next chunk
+      int nq = q;
+      int64_t nbase = base + 128, nend = end;
+      while (nbase >= nend) {
+        if (++nq >= nk) break;
+        nbase = __shfl_sync(FULL, tb_l, nq);
+        nend = __shfl_sync(FULL, te_l, nq);
+      }
+      if (nq < nk) fetch(nbase, nend, nj, nv);
+      const double aik = NEED_VAL ? __shfl_sync(FULL, av, q) : 0.0;
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+        if (cj[r] >= 0) fn(aik, cj[r], cv[r]);
+      if (ORDERED && nq != q) __syncwarp();
+#pragma unroll
+      for (int r = 0; r < 4; ++r) { cj[r] = nj[r]; if (NEED_VAL) cv[r] = nv[r]; }
+      q = nq;
+      base = nbase;
+      end = nend;
+    }
+    if (ORDERED) __syncwarp();
+  }
+}
+
 // MODE 0: distinct candidate columns per row (sizes the accumulator); 1: count kept entries; 2: fill (columns + values);
 // 3: one pass for the LAST power, whose values are not needed: kept columns go to a scratch row of candidate capacity
 //    (offsets out_rp from MODE 0's counts) and cnt[i] = number kept.
@@ -94,19 +157,8 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
     __syncwarp();
     const int64_t a = A_rp[i], b = A_rp[i + 1];
     // pass 1: mark candidate columns
-    for (int64_t e0 = a; e0 < b; e0 += 32) {
-      const int64_t e = e0 + lane;
-      const int kk = e < b ? A_col[e] : 0;
-      const int nk = (int)min((int64_t)32, b - e0);
-      for (int q = 0; q < nk; ++q) {
-        const int k = __shfl_sync(0xffffffffu, kk, q);
-        const int64_t tb = T_rp[k], te = T_rp[k + 1];
-        for (int64_t f = tb + lane; f < te; f += 32) {
-          const int j = T_col[f];
-          atomicOr(&bm[j >> 5], 1u << (j & 31));
-        }
-      }
-    }
+    walk_products<false, false>(lane, a, b, A_col, A_val, T_rp, T_col, T_val,
+                                [&](double, int j, double) { atomicOr(&bm[j >> 5], 1u << (j & 31)); });
     __syncwarp();
     // compact slot index: rk[w] = number of candidates in words < w
     int running = 0;
@@ -126,24 +178,11 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
     for (int s = lane; s < running; s += 32) acc[s] = 0.0;
     __syncwarp();
     // pass 2: accumulate, k ascending, multiply and add separately rounded
-    for (int64_t e0 = a; e0 < b; e0 += 32) {
-      const int64_t e = e0 + lane;
-      const int kk = e < b ? A_col[e] : 0;
-      const double av = e < b ? A_val[e] : 0.0;
-      const int nk = (int)min((int64_t)32, b - e0);
-      for (int q = 0; q < nk; ++q) {
-        const int k = __shfl_sync(0xffffffffu, kk, q);
-        const double aik = __shfl_sync(0xffffffffu, av, q);
-        const int64_t tb = T_rp[k], te = T_rp[k + 1];
-        for (int64_t f = tb + lane; f < te; f += 32) {
-          const int j = T_col[f];
-          const uint32_t word = bm[j >> 5];
-          const int slot = rk[j >> 5] + __popc(word & ((1u << (j & 31)) - 1u));
-          acc[slot] = __dadd_rn(acc[slot], __dmul_rn(aik, T_val[f]));
-        }
-        __syncwarp();  // the next k may hit the same slots
-      }
-    }
+    walk_products<true, true>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, [&](double aik, int j, double t) {
+      const uint32_t word = bm[j >> 5];
+      const int slot = rk[j >> 5] + __popc(word & ((1u << (j & 31)) - 1u));
+      acc[slot] = __dadd_rn(acc[slot], __dmul_rn(aik, t));
+    });
     // emit kept entries in ascending column order
     int kept = 0;
     const int64_t ob = (MODE == 2 || MODE == 3) ? out_rp[i] : 0;
@@ -315,8 +354,6 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     if (f & 2) return GBE_EINVAL;
     if (f) return GBE_ENOTSYM;
   }
-
-  gbe_trace("start pattern");
   DevBuf cnt;
   GBE_TRY(cnt.alloc((size_t)n * 4));
 
@@ -331,8 +368,6 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   k_materialise_A<true><<<rows_grid, 256, 0, s>>>(n, H.row_ptr, H.col_idx, H.val, st, tau, nullptr, A.rp.as<int64_t>(),
                                                   A.col.as<int32_t>(), A.val.as<double>());
   GBE_LAUNCHED();
-
-  gbe_trace("materialise A");
   // pattern accumulator P = I u pat(A)
   const size_t bm_bytes = (size_t)W * 4;
   const int uw = pick_warps(bm_bytes, 8);
@@ -358,8 +393,6 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
 
   Pattern P;
   GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), nullptr, nullptr, nullptr, 1, P));
-
-  gbe_trace("union I+A");
   // thresholded powers
   Pattern Tprev;  // T^(k-1) with values; T^(1) aliases A
   const int64_t* T_rp = A.rp.as<int64_t>();
@@ -369,7 +402,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     // symbolic: accumulator capacity
     {
       const size_t per_warp = (size_t)W * 8;
-      const int nw = pick_warps(per_warp, 8);
+      const int nw = pick_warps(per_warp, 16);
       if (nw < 1) return GBE_EINVAL;
       GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
       const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
@@ -378,7 +411,6 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                                  cnt.as<int32_t>(), nullptr, nullptr, nullptr);
       GBE_LAUNCHED();
     }
-    gbe_trace("spgemm symbolic");
     std::vector<int32_t> h_cnt((size_t)n);
     GBE_CUDA(cudaMemcpyAsync(h_cnt.data(), cnt.p, (size_t)n * 4, cudaMemcpyDeviceToHost, s));
     GBE_CUDA(cudaStreamSynchronize(s));
@@ -386,7 +418,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     for (int64_t i = 0; i < n; ++i) cap = std::max(cap, h_cnt[(size_t)i]);
     cap = (cap + 1) & ~1;
     const size_t per_warp = (size_t)W * 8 + (size_t)cap * 8;
-    const int nw = pick_warps(per_warp, 8);
+    const int nw = pick_warps(per_warp, 16);
     if (nw < 1) return GBE_EINVAL;
     GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
     GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
@@ -403,7 +435,6 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                                  cnt.as<int32_t>(), Tc.rp.as<int64_t>(),
                                                                  Tc.col.as<int32_t>(), nullptr);
       GBE_LAUNCHED();
-      gbe_trace("spgemm numeric");
       Pattern Pn;
       GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tc.rp.as<int64_t>(), Tc.col.as<int32_t>(),
                        cnt.as<int32_t>(), 0, Pn));
@@ -441,8 +472,6 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     T_val = Tprev.val.as<double>();
     // Tn (now holding the previous T) and Pn are released here, after the sync above
   }
-
-  gbe_trace("union P+T");
   // S = P u P^T
   Pattern PT;
   GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
@@ -457,7 +486,6 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   Pattern S;
   GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(), PT.col.as<int32_t>(), nullptr, 0, S));
   GBE_CUDA(cudaStreamSynchronize(s));
-  gbe_trace("transpose+union");
   *nnz_S = S.nnz;
   *S_row_ptr = reinterpret_cast<int64_t*>(S.rp.release());
   *S_col = reinterpret_cast<int32_t*>(S.col.release());

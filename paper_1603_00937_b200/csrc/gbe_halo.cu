@@ -233,8 +233,6 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_CUDA(cudaMemsetAsync(cursor.p, 0, (size_t)n_part * 4, s));
   k_core_fill<<<tgrid, 256, 0, s>>>(n, part, blk, core_ptr.as<int64_t>(), cursor.as<int32_t>(), core_tmp.as<int32_t>());
   GBE_LAUNCHED();
-
-  gbe_trace("cores");
   // ---- halo: count, then fill
   const size_t halo_smem = (size_t)2 * W * 4 + 257 * 4;
   if (halo_smem > 220 * 1024) return GBE_EINVAL;  // n too large for the shared-memory bitmaps
@@ -250,8 +248,6 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_CUDA(cudaMemcpyAsync(g->h_m.data(), g->msize, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaMemcpyAsync(g->h_ncore.data(), g->ncore, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaStreamSynchronize(s));
-
-  gbe_trace("halo count");
   // ---- host: layout, work lists
   std::vector<int64_t> h_sub_ptr(n_part + 1, 0);
   g->h_dense_off.assign(n_part + 1, 0);
@@ -316,16 +312,12 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   g->ws_x1 = off;
   off += align_up((size_t)g->dense_elems * 8, 256);
   g->ws_bytes = off;
-
-  gbe_trace("host layout+lists");
   // ---- fill sub_idx / row_part
   GBE_TRY(gbe_dev_alloc((void**)&g->sub_idx, std::max<size_t>(16, (size_t)g->sum_m * 4)));
   GBE_TRY(gbe_dev_alloc((void**)&g->row_part, std::max<size_t>(16, (size_t)g->sum_m * 4)));
   k_halo<true><<<n_part, 256, halo_smem, s>>>(W, core_ptr.as<int64_t>(), core_tmp.as<int32_t>(), g->S_row_ptr, g->S_col,
                                               nullptr, nullptr, g->sub_ptr, g->sub_idx, g->row_part);
   GBE_LAUNCHED();
-
-  gbe_trace("halo fill");
   // ---- pattern of D and scatter map
   const int64_t sum_m = g->sum_m;
   const int qgrid = (int)std::max<int64_t>(1, (sum_m + 255) / 256);
@@ -375,6 +367,5 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     g->scat_ofs = reinterpret_cast<int64_t*>(scat_ofs.release());
   }
   GBE_CUDA(cudaStreamSynchronize(s));
-  gbe_trace("D pattern");
   return GBE_OK;
 }

@@ -33,19 +33,6 @@ extern std::atomic<uint64_t> g_gbe_launches;
     if (s__ != GBE_OK) return s__; \
   } while (0)
 
-// TEMP tracing
-#include <chrono>
-#include <cstdio>
-#include <cstdlib>
-inline void gbe_trace(const char* label) {
-  static const bool on = getenv("GBE_TRACE") != nullptr;
-  static auto last = std::chrono::steady_clock::now();
-  if (!on) return;
-  cudaDeviceSynchronize();
-  auto now = std::chrono::steady_clock::now();
-  fprintf(stderr, "[trace] %-28s %8.3f ms\n", label, std::chrono::duration<double, std::milli>(now - last).count());
-  last = std::chrono::steady_clock::now();
-}
 // Device allocations of the library come from the device's default stream-ordered memory pool (cudaMallocAsync) with
 // the release threshold lifted, so that the dozens of build-time temporaries cost microseconds instead of a
 // cudaMalloc / cudaFree (device synchronisation) each.  The stream is the one of the current API call.
