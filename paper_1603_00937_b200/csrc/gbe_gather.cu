@@ -76,17 +76,23 @@ __global__ void __launch_bounds__(256) k_gather(int W, int ldmax, int rows_per_c
   double* Xp = X + dense_off[p];
   double s1 = 0.0, s2 = 0.0;
   const int rend = min(m, r0 + rows_per_cta);
-  for (int r = r0 + wid; r < rend; r += nw) {
-    for (int c = lane * 2; c < ld; c += 64) *reinterpret_cast<double2*>(buf + c) = make_double2(0.0, 0.0);
-    __syncwarp();
-    const int k = sub_idx[sb + r];
-    if (lane == 0) buf[r] = (eps_max - 0.0) / delta;  // a stored diagonal overwrites this below
-    __syncwarp();
-    const int64_t a = H_rp[k], b = H_rp[k + 1];
-    for (int64_t e = a + lane; e < b; e += 32) {
-      const int j = H_col[e];
-      if ((unsigned)j >= (uint64_t)n) continue;
-      const uint32_t bit = 1u << (j & 31), wj = j >> 5;
+  // The row loop is latency bound (sub_idx -> H row pointers -> H entries are dependent loads), so it is software
+  // pipelined: the vertex of the row after next, the row pointers of the next row and the first 128 entries of the
+  // next row are in flight while the current row is scattered into shared memory and streamed out.
+  auto fetch = [&](int64_t base, int64_t end, int (&j)[4], double (&v)[4]) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int64_t e = base + lane + 32 * u;
+      j[u] = e < end ? H_col[e] : -1;
+      v[u] = e < end ? H_val[e] : 0.0;
+    }
+  };
+  auto place = [&](int k, const int (&j)[4], const double (&v)[4]) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int col = j[u];
+      if (col < 0 || (int64_t)col >= n) continue;
+      const uint32_t bit = 1u << (col & 31), wj = col >> 5;
       int c = -1;
       const uint32_t cw = coreb[wj];
       if (cw & bit) {
@@ -95,8 +101,39 @@ __global__ void __launch_bounds__(256) k_gather(int W, int ldmax, int rows_per_c
         const uint32_t hw = halob[wj];
         if (hw & bit) c = nc + halork[wj] + __popc(hw & (bit - 1u));
       }
-      if (c >= 0) buf[c] = ((j == k ? eps_max : 0.0) - H_val[e]) / delta;
+      if (c >= 0) buf[c] = ((col == k ? eps_max : 0.0) - v[u]) / delta;
     }
+  };
+  int r = r0 + wid;
+  int k0 = r < rend ? sub_idx[sb + r] : 0;
+  int k1 = r + nw < rend ? sub_idx[sb + r + nw] : 0;
+  int64_t a0 = 0, b0 = 0, a1 = 0, b1 = 0;
+  int cj[4], nj[4];
+  double cv[4], nv[4];
+  if (r < rend) {
+    a0 = H_rp[k0];
+    b0 = H_rp[k0 + 1];
+    fetch(a0, b0, cj, cv);
+  }
+  for (; r < rend; r += nw) {
+    const bool has1 = r + nw < rend;
+    const int k2 = r + 2 * nw < rend ? sub_idx[sb + r + 2 * nw] : 0;
+    if (has1) {
+      a1 = H_rp[k1];
+      b1 = H_rp[k1 + 1];
+    }
+    for (int c = lane * 2; c < ld; c += 64) *reinterpret_cast<double2*>(buf + c) = make_double2(0.0, 0.0);
+    __syncwarp();
+    if (lane == 0) buf[r] = (eps_max - 0.0) / delta;  // a stored diagonal overwrites this below
+    __syncwarp();
+    for (int64_t base = a0; base < b0; base += 128) {
+      if (base + 128 < b0) fetch(base + 128, b0, nj, nv);        // rest of a long row
+      else if (has1) fetch(a1, b1, nj, nv);                      // first entries of the next row
+      place(k0, cj, cv);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { cj[u] = nj[u]; cv[u] = nv[u]; }
+    }
+    if (a0 >= b0 && has1) fetch(a1, b1, cj, cv);                 // empty row: nothing was prefetched above
     __syncwarp();
     double* out = Xp + (size_t)r * ld;
     double q = 0.0;
@@ -110,6 +147,7 @@ __global__ void __launch_bounds__(256) k_gather(int W, int ldmax, int rows_per_c
       if (lane == 0) s1 += buf[r];
     }
     __syncwarp();
+    k0 = k1; k1 = k2; a0 = a1; b0 = b1;
   }
   s1 = warp_sum(s1);
   s2 = warp_sum(s2);

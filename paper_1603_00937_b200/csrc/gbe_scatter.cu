@@ -21,19 +21,50 @@ __global__ void __launch_bounds__(256) k_scatter(int64_t sum_m, const int32_t* _
   const int lane = threadIdx.x & 31;
   const int64_t warp = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5), nwarps = (int64_t)gridDim.x * 8;
   const double* __restrict__ X = (st->iters_done & 1) ? X1 : X0;
-  for (int64_t q = warp; q < sum_m; q += nwarps) {
-    const int p = row_part[q];
-    const int64_t sb = sub_ptr[p];
-    const int m = (int)(sub_ptr[p + 1] - sb);
-    const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
-    const int nc = ncore[p];
-    const double* src = X + dense_off[p] + (size_t)(q - sb) * ld;
-    if (CONTIG) {
-      double* dst = D_val + scat_base[q];
-      for (int c = lane; c < nc; c += 32) dst[c] = src[c];
-    } else {
-      const int64_t* pos = scat_pos + scat_ofs[q];
-      for (int c = lane; c < nc; c += 32) D_val[pos[c]] = src[c];
+  constexpr int R = 8;  // dense rows per warp iteration: their metadata is fetched by 8 lanes at once and the loads
+                        // of all 8 rows are issued before the first store (the kernel is latency bound otherwise)
+  for (int64_t q0 = warp * R; q0 < sum_m; q0 += nwarps * R) {
+    int nc_l = 0;
+    int64_t src_l = 0, dst_l = 0;
+    if (lane < R && q0 + lane < sum_m) {
+      const int64_t q = q0 + lane;
+      const int p = row_part[q];
+      const int64_t sb = sub_ptr[p];
+      const int m = (int)(sub_ptr[p + 1] - sb);
+      const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+      nc_l = ncore[p];
+      src_l = dense_off[p] + (q - sb) * ld;
+      dst_l = CONTIG ? scat_base[q] : scat_ofs[q];
+    }
+    double v[R][2];
+    int ncs[R];
+    int64_t dsts[R], srcs[R];
+#pragma unroll
+    for (int l = 0; l < R; ++l) {
+      ncs[l] = __shfl_sync(0xffffffffu, nc_l, l);
+      srcs[l] = __shfl_sync(0xffffffffu, src_l, l);
+      dsts[l] = __shfl_sync(0xffffffffu, dst_l, l);
+    }
+#pragma unroll
+    for (int l = 0; l < R; ++l) {
+      const double* src = X + srcs[l];
+      v[l][0] = lane < ncs[l] ? src[lane] : 0.0;
+      v[l][1] = lane + 32 < ncs[l] ? src[lane + 32] : 0.0;
+    }
+#pragma unroll
+    for (int l = 0; l < R; ++l) {
+      const int nc = ncs[l];
+      if (CONTIG) {
+        double* dst = D_val + dsts[l];
+        if (lane < nc) dst[lane] = v[l][0];
+        if (lane + 32 < nc) dst[lane + 32] = v[l][1];
+        for (int c = lane + 64; c < nc; c += 32) dst[c] = X[srcs[l] + c];
+      } else {
+        const int64_t* pos = scat_pos + dsts[l];
+        if (lane < nc) D_val[pos[lane]] = v[l][0];
+        if (lane + 32 < nc) D_val[pos[lane + 32]] = v[l][1];
+        for (int c = lane + 64; c < nc; c += 32) D_val[pos[c]] = X[srcs[l] + c];
+      }
     }
   }
 }
@@ -42,7 +73,7 @@ __global__ void __launch_bounds__(256) k_scatter(int64_t sum_m, const int32_t* _
 int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0, const double* X1, double* D_val,
                        cudaStream_t s) {
   if (g->sum_m == 0) return GBE_OK;
-  const int64_t want = (g->sum_m + 7) / 8;
+  const int64_t want = (g->sum_m + 63) / 64;  // 8 warps x 8 rows per CTA iteration
   const int grid = (int)std::min<int64_t>(want, 148 * 64);
   if (g->contiguous)
     k_scatter<true><<<grid, 256, 0, s>>>(g->sum_m, g->row_part, g->sub_ptr, g->ncore, g->dense_off, g->scat_base, nullptr,
