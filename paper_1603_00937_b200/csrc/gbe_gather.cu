@@ -16,7 +16,7 @@
 
 namespace {
 
-__global__ void __launch_bounds__(256) k_gather(int W, int ldmax, int rows_per_cta, const int2* __restrict__ gitems,
+__global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_per_cta, const int2* __restrict__ gitems,
                                                 const int64_t* __restrict__ H_rp, const int32_t* __restrict__ H_col,
                                                 const double* __restrict__ H_val, int64_t n,
                                                 const int64_t* __restrict__ sub_ptr, const int32_t* __restrict__ sub_idx,
@@ -39,6 +39,13 @@ __global__ void __launch_bounds__(256) k_gather(int W, int ldmax, int rows_per_c
   const int nc = ncore_arr[p];
   const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
   const double eps_max = st->eps_max, delta = st->eps_max - st->eps_min;
+  const double inv_delta = 1.0 / delta;
+  // x / delta as a reciprocal multiply plus one residual correction: the correctly rounded quotient except in rare
+  // half-ulp cases, at a tenth of the instructions of the IEEE division sequence (the row loop is issue bound)
+  auto div_delta = [&](double x) {
+    const double q = x * inv_delta;
+    return fma(fma(-q, delta, x), inv_delta, q);
+  };
 
   // bitmaps of the community's core and halo vertices
   for (int w = t; w < 2 * W; w += blockDim.x) coreb[w] = 0u;
@@ -57,10 +64,16 @@ __global__ void __launch_bounds__(256) k_gather(int W, int ldmax, int rows_per_c
     scratch[t] = c0;
     scratch[258 + t] = c1;
     __syncthreads();
-    if (t < 2) {
-      int* sc = scratch + 258 * t;
+    for (int which = wid; which < 2; which += nw) {  // one warp each scans the per-thread counts of the core and the halo bitmap
+      int* sc = scratch + 258 * which;
       int run = 0;
-      for (int k = 0; k < nt; ++k) { const int v = sc[k]; sc[k] = run; run += v; }
+      for (int k0 = 0; k0 < nt; k0 += 32) {
+        const int v = k0 + lane < nt ? sc[k0 + lane] : 0;
+        int tot;
+        const int ex = warp_excl_scan_i(v, lane, &tot);
+        if (k0 + lane < nt) sc[k0 + lane] = run + ex;
+        run += tot;
+      }
     }
     __syncthreads();
     c0 = scratch[t];
@@ -101,7 +114,7 @@ __global__ void __launch_bounds__(256) k_gather(int W, int ldmax, int rows_per_c
         const uint32_t hw = halob[wj];
         if (hw & bit) c = nc + halork[wj] + __popc(hw & (bit - 1u));
       }
-      if (c >= 0) buf[c] = ((col == k ? eps_max : 0.0) - v[u]) / delta;
+      if (c >= 0) buf[c] = div_delta((col == k ? eps_max : 0.0) - v[u]);
     }
   };
   int r = r0 + wid;
@@ -124,7 +137,7 @@ __global__ void __launch_bounds__(256) k_gather(int W, int ldmax, int rows_per_c
     }
     for (int c = lane * 2; c < ld; c += 64) *reinterpret_cast<double2*>(buf + c) = make_double2(0.0, 0.0);
     __syncwarp();
-    if (lane == 0) buf[r] = (eps_max - 0.0) / delta;  // a stored diagonal overwrites this below
+    if (lane == 0) buf[r] = div_delta(eps_max - 0.0);  // a stored diagonal overwrites this below
     __syncwarp();
     for (int64_t base = a0; base < b0; base += 128) {
       if (base + 128 < b0) fetch(base + 128, b0, nj, nv);        // rest of a long row
@@ -174,6 +187,7 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
   int nw = (int)std::min<size_t>(8, (budget - fixed) / ((size_t)ldmax * 8));
   const size_t smem = fixed + (size_t)nw * ldmax * 8;
   GBE_CUDA(cudaFuncSetAttribute(k_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  GBE_CUDA(cudaFuncSetAttribute(k_gather, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
   k_gather<<<g->n_gitems, nw * 32, smem, s>>>(W, ldmax, g->gather_rows, g->gitems, H.row_ptr, H.col_idx, H.val, g->n,
                                               g->sub_ptr, g->sub_idx, g->ncore, g->dense_off, st, X, partials);
   GBE_LAUNCHED();

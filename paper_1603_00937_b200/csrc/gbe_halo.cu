@@ -123,6 +123,19 @@ __global__ void k_member_fill(int64_t sum_m, const int32_t* __restrict__ sub_idx
   const int pos = atomicAdd(&cursor[k], 1);
   memb[memb_ptr[k] + pos] = q;
 }
+// per dense row q: where it starts in a dense buffer and how many core columns it carries (read by the scatter)
+__global__ void k_row_meta(int64_t sum_m, const int32_t* __restrict__ row_part, const int64_t* __restrict__ sub_ptr,
+                           const int32_t* __restrict__ ncore, const int64_t* __restrict__ dense_off,
+                           int64_t* __restrict__ row_src, int32_t* __restrict__ row_nc) {
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= sum_m) return;
+  const int p = row_part[q];
+  const int64_t sb = sub_ptr[p];
+  const int64_t m = sub_ptr[p + 1] - sb;
+  const int64_t ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+  row_src[q] = dense_off[p] + (q - sb) * ld;
+  row_nc[q] = ncore[p];
+}
 __global__ void k_row_ncore(int64_t sum_m, const int32_t* __restrict__ row_part, const int32_t* __restrict__ ncore,
                             int32_t* __restrict__ out) {
   const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -321,6 +334,10 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   // ---- pattern of D and scatter map
   const int64_t sum_m = g->sum_m;
   const int qgrid = (int)std::max<int64_t>(1, (sum_m + 255) / 256);
+  GBE_TRY(gbe_dev_alloc((void**)&g->row_src, std::max<size_t>(16, (size_t)sum_m * 8)));
+  GBE_TRY(gbe_dev_alloc((void**)&g->row_nc, std::max<size_t>(16, (size_t)sum_m * 4)));
+  k_row_meta<<<qgrid, 256, 0, s>>>(sum_m, g->row_part, g->sub_ptr, g->ncore, g->dense_off, g->row_src, g->row_nc);
+  GBE_LAUNCHED();
   DevBuf mcnt, memb_ptr, memb;
   GBE_TRY(mcnt.alloc((size_t)n * 4));
   GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));

@@ -104,6 +104,8 @@ struct gbe_graph {
   int64_t* scat_pos = nullptr;   // nnz_D: D.val offset of (p, r, c), general case (else null)
   int64_t* scat_ofs = nullptr;   // sum_m+1: offset of dense row q in scat_pos (general case)
   int32_t* row_part = nullptr;   // sum_m: community of dense row q
+  int64_t* row_src = nullptr;    // sum_m: element offset of dense row q in a dense buffer
+  int32_t* row_nc = nullptr;     // sum_m: ncore of the community of dense row q
   gbe_tile_item* items = nullptr;
   int32_t n_items = 0;
   int2* gitems = nullptr;  // gather work items (p, first row)

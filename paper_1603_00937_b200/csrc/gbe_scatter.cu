@@ -10,9 +10,8 @@
 
 namespace {
 template <bool CONTIG>
-__global__ void __launch_bounds__(256) k_scatter(int64_t sum_m, const int32_t* __restrict__ row_part,
-                                                 const int64_t* __restrict__ sub_ptr, const int32_t* __restrict__ ncore,
-                                                 const int64_t* __restrict__ dense_off,
+__global__ void __launch_bounds__(256, 4) k_scatter(int64_t sum_m, const int64_t* __restrict__ row_src,
+                                                 const int32_t* __restrict__ row_nc,
                                                  const int64_t* __restrict__ scat_base,
                                                  const int64_t* __restrict__ scat_ofs,
                                                  const int64_t* __restrict__ scat_pos, const gbe_state* __restrict__ st,
@@ -28,42 +27,53 @@ __global__ void __launch_bounds__(256) k_scatter(int64_t sum_m, const int32_t* _
     int64_t src_l = 0, dst_l = 0;
     if (lane < R && q0 + lane < sum_m) {
       const int64_t q = q0 + lane;
-      const int p = row_part[q];
-      const int64_t sb = sub_ptr[p];
-      const int m = (int)(sub_ptr[p + 1] - sb);
-      const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
-      nc_l = ncore[p];
-      src_l = dense_off[p] + (q - sb) * ld;
+      nc_l = row_nc[q];
+      src_l = row_src[q];
       dst_l = CONTIG ? scat_base[q] : scat_ofs[q];
     }
-    double v[R][2];
-    int ncs[R];
-    int64_t dsts[R], srcs[R];
+    // phase 1: all loads of the 8 rows; 16-byte loads when the row can be moved as aligned pairs
+    double2 v[R];
+    bool vec[R];
 #pragma unroll
     for (int l = 0; l < R; ++l) {
-      ncs[l] = __shfl_sync(0xffffffffu, nc_l, l);
-      srcs[l] = __shfl_sync(0xffffffffu, src_l, l);
-      dsts[l] = __shfl_sync(0xffffffffu, dst_l, l);
-    }
-#pragma unroll
-    for (int l = 0; l < R; ++l) {
-      const double* src = X + srcs[l];
-      v[l][0] = lane < ncs[l] ? src[lane] : 0.0;
-      v[l][1] = lane + 32 < ncs[l] ? src[lane + 32] : 0.0;
-    }
-#pragma unroll
-    for (int l = 0; l < R; ++l) {
-      const int nc = ncs[l];
-      if (CONTIG) {
-        double* dst = D_val + dsts[l];
-        if (lane < nc) dst[lane] = v[l][0];
-        if (lane + 32 < nc) dst[lane + 32] = v[l][1];
-        for (int c = lane + 64; c < nc; c += 32) dst[c] = X[srcs[l] + c];
+      const int nc = __shfl_sync(0xffffffffu, nc_l, l);
+      const int64_t so = __shfl_sync(0xffffffffu, src_l, l);
+      const int64_t dofs = __shfl_sync(0xffffffffu, dst_l, l);
+      const double* src = X + so;  // 128-byte aligned: rows of a dense block start on a line
+      vec[l] = CONTIG && nc <= 64 && !(nc & 1) && !((reinterpret_cast<uintptr_t>(D_val + dofs)) & 15);
+      v[l] = make_double2(0.0, 0.0);
+      if (vec[l]) {
+        if (2 * lane < nc) v[l] = *reinterpret_cast<const double2*>(src + 2 * lane);
       } else {
-        const int64_t* pos = scat_pos + dsts[l];
-        if (lane < nc) D_val[pos[lane]] = v[l][0];
-        if (lane + 32 < nc) D_val[pos[lane + 32]] = v[l][1];
-        for (int c = lane + 64; c < nc; c += 32) D_val[pos[c]] = X[srcs[l] + c];
+        if (lane < nc) v[l].x = src[lane];
+        if (lane + 32 < nc) v[l].y = src[lane + 32];
+      }
+    }
+    // phase 2: all stores
+#pragma unroll
+    for (int l = 0; l < R; ++l) {
+      const int nc = __shfl_sync(0xffffffffu, nc_l, l);
+      const int64_t dofs = __shfl_sync(0xffffffffu, dst_l, l);
+      if (CONTIG) {
+        double* dst = D_val + dofs;
+        if (vec[l]) {
+          if (2 * lane < nc) *reinterpret_cast<double2*>(dst + 2 * lane) = v[l];
+        } else {
+          if (lane < nc) dst[lane] = v[l].x;
+          if (lane + 32 < nc) dst[lane + 32] = v[l].y;
+          if (nc > 64) {
+            const double* src = X + __shfl_sync(0xffffffffu, src_l, l);
+            for (int c = lane + 64; c < nc; c += 32) dst[c] = src[c];
+          }
+        }
+      } else {
+        const int64_t* pos = scat_pos + dofs;
+        if (lane < nc) D_val[pos[lane]] = v[l].x;
+        if (lane + 32 < nc) D_val[pos[lane + 32]] = v[l].y;
+        if (nc > 64) {
+          const double* src = X + __shfl_sync(0xffffffffu, src_l, l);
+          for (int c = lane + 64; c < nc; c += 32) D_val[pos[c]] = src[c];
+        }
       }
     }
   }
@@ -76,10 +86,10 @@ int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0
   const int64_t want = (g->sum_m + 63) / 64;  // 8 warps x 8 rows per CTA iteration
   const int grid = (int)std::min<int64_t>(want, 148 * 64);
   if (g->contiguous)
-    k_scatter<true><<<grid, 256, 0, s>>>(g->sum_m, g->row_part, g->sub_ptr, g->ncore, g->dense_off, g->scat_base, nullptr,
+    k_scatter<true><<<grid, 256, 0, s>>>(g->sum_m, g->row_src, g->row_nc, g->scat_base, nullptr,
                                          nullptr, st, X0, X1, D_val);
   else
-    k_scatter<false><<<grid, 256, 0, s>>>(g->sum_m, g->row_part, g->sub_ptr, g->ncore, g->dense_off, nullptr, g->scat_ofs,
+    k_scatter<false><<<grid, 256, 0, s>>>(g->sum_m, g->row_src, g->row_nc, nullptr, g->scat_ofs,
                                           g->scat_pos, st, X0, X1, D_val);
   GBE_LAUNCHED();
   return GBE_OK;
