@@ -238,6 +238,8 @@ def run_ours(args) -> None:
         gbe.gbe_density_host(Hh, g, s.n_occ, s.iters, -1.0, workspace=ws, D_val_host=D_host.numpy(), stream=stream)
         return g
 
+    step_ms_log = []
+
     def timed_region(step, steps):
         """K steps, each bracketed by CUDA events on the launching stream, L2 flushed (untimed) between steps."""
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
@@ -258,6 +260,7 @@ def run_ours(args) -> None:
         ms = [e0.elapsed_time(e1) for e0, e1 in ev]
         for g in graphs:
             g.free()
+        step_ms_log.append([round(x, 3) for x in ms])
         return float(np.sum(ms)), int(launches)
 
     for _ in range(max(args.warmup, 3)):
@@ -320,6 +323,7 @@ def run_ours(args) -> None:
                     "h2d_bytes_per_step": int(2 * (s.H.row_ptr.nbytes + s.H.col_idx.nbytes + s.H.val.nbytes)),
                     "d2h_bytes_per_step": int(info["nnz_D"] * 8)},
             "gpu_launches": launches,
+            "ms_steps": {"device": step_ms_log[0], "e2e": step_ms_log[-1]},
             "clocks": clk,
             "roofline": {
                 "kernel": "k_x2 (Y = X X^T on DMMA.8x8x4, fused branch/trace epilogue)", "bound": "tensor",
@@ -351,6 +355,86 @@ def run_ours(args) -> None:
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------
+# BASELINE.json configs[4]: threshold x partition sweep on the 24,576-orbital water box
+# ------------------------------------------------------------------------------------------------
+def run_sweep(args) -> None:
+    """tau in {1e-3..1e-7} x communities in {128,256,512,1024} on one geometry: halo size distribution, cost
+    (sum 2 m^3, the paper's cost law P:L78), throughput, and the error against the exact zero-temperature projector.
+    The exact projector comes from torch.linalg.eigh on the GPU (a library call, used for this report only).
+    One JSON line per point; `--sweep-out FILE` also writes a markdown table."""
+    import torch
+    import gbe_inputs as gi
+    from paper_1603_00937_b200 import build as gbe_build
+    gbe_build.build()
+    import paper_1603_00937_b200 as gbe
+
+    n_mol = WORKLOADS[args.workload][0]
+    taus = [1e-3, 1e-4, 1e-5, 1e-6, 1e-7]
+    parts = [n_mol // 32, n_mol // 16, n_mol // 8, n_mol // 4]
+    base = gi.water_box(n_mol, parts[2], seed=0)
+    Hd = gbe.DeviceCSR.from_host(base.H)
+    n, n_occ = base.n, base.n_occ
+    Dex = None
+    if not args.no_exact:
+        t0 = time.time()
+        Hdense = torch.from_numpy(base.H.to_dense()).cuda()
+        w, V = torch.linalg.eigh(Hdense)
+        del Hdense
+        k = int(round(n_occ))
+        gap = float(w[k] - w[k - 1])
+        Dex = V[:, :k] @ V[:, :k].T
+        del V
+        torch.cuda.synchronize()
+        sys.stderr.write(f"exact projector: {time.time() - t0:.1f} s, HOMO-LUMO gap {gap:.3e} eV\n")
+    rows = []
+    for tau in taus:
+        for n_part in parts:
+            torch.cuda.synchronize()
+            e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            gbe.gbe_build_graph(Hd, tau, None, n_part).free()  # warm-up of the allocator for this size
+            e0.record()
+            g = gbe.gbe_build_graph(Hd, tau, None, n_part)
+            e1.record()
+            info = g.info
+            ws = g.new_workspace()
+            D_val = torch.empty(info["nnz_D"], dtype=torch.float64, device="cuda")
+            gbe.gbe_density(Hd, g, n_occ, base.iters, -1.0, workspace=ws, D_val=D_val, want_log=False)  # warm-up
+            torch.cuda.synchronize()
+            e1.record()
+            _, log = gbe.gbe_density(Hd, g, n_occ, base.iters, -1.0, workspace=ws, D_val=D_val, want_log=True)
+            e2.record()
+            torch.cuda.synchronize()
+            ex = g.export()
+            m = (ex["sub_ptr"][1:] - ex["sub_ptr"][:-1]).double()
+            rec = {"sweep": args.workload, "tau": tau, "n_part": n_part, "m_min": int(m.min()), "m_mean": float(m.mean()),
+                   "m_max": int(m.max()), "sum_2m3": info["sp2_flops_per_iter"], "nnz_S": info["nnz_S"],
+                   "nnz_D": info["nnz_D"], "density_ms": e1.elapsed_time(e2),
+                   "orbitals_per_s": n / (e1.elapsed_time(e2) * 1e-3),
+                   "sp2_tflops_alg": info["sp2_flops_per_iter"] * base.iters / (e1.elapsed_time(e2) * 1e-3) * 1e-12,
+                   "trace_minus_nocc": float(log.t1[-1] - n_occ), "idempotency_residual": float(log.t1[-1] - log.t2[-1])}
+            if Dex is not None:
+                rp = ex["D_row_ptr"]
+                r_idx = torch.repeat_interleave(torch.arange(n, device="cuda"), rp[1:] - rp[:-1])
+                diff = D_val - Dex[r_idx, ex["D_col"].long()]
+                rec["max_abs_err_vs_exact"] = float(diff.abs().max())
+                rec["frobenius_err_per_orbital"] = float(torch.sqrt((diff * diff).sum()) / n)
+                del r_idx, diff
+            rows.append(rec)
+            print(json.dumps(rec), flush=True)
+            g.free()
+            del ws, D_val, ex
+    if args.sweep_out:
+        with open(args.sweep_out, "w") as f:
+            f.write("| tau | communities | m min/mean/max | sum 2m^3 per iteration | density ms | orbitals/s | TFLOP/s (2m^3) | "
+                    "max abs err vs exact | Frobenius err / orbital | Tr D - n_occ |\n|---|---|---|---|---|---|---|---|---|---|\n")
+            for r in rows:
+                f.write(f"| {r['tau']:g} | {r['n_part']} | {r['m_min']}/{r['m_mean']:.0f}/{r['m_max']} | {r['sum_2m3']:.3g} | "
+                        f"{r['density_ms']:.1f} | {r['orbitals_per_s']:.3g} | {r['sp2_tflops_alg']:.1f} | "
+                        f"{r.get('max_abs_err_vs_exact', float('nan')):.3g} | {r.get('frobenius_err_per_orbital', float('nan')):.3g} | "
+                        f"{r['trace_minus_nocc']:.3g} |\n")
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -359,8 +443,13 @@ def main() -> None:
     ap.add_argument("--workload", default="water4096", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="tau x partition sweep (BASELINE.json configs[4]) instead of the bench line")
+    ap.add_argument("--sweep-out", default="", help="markdown table of the sweep")
+    ap.add_argument("--no-exact", action="store_true", help="sweep without the exact projector (no error columns)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
