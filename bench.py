@@ -40,6 +40,8 @@ UNIT = "orbitals/s"
 # 8192^3 35.3 TF on this pool - profiles/r01_fp64_peak_probe.md).
 FP64_NOMINAL_TF, BF16_NOMINAL_TF = 40.0, 2250.0
 DMMA_PROBE_TF = 37.07
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_x2 launch, from the committed ncu capture of this bench command
+X2_DRAM_BYTES_PER_LAUNCH = {"water4096": 2.01e9}
 
 WORKLOADS = {
     # name: (molecules, communities) - BASELINE.json configs[1], configs[2] (SURVEY numbering: config 2, config 3)
@@ -327,7 +329,8 @@ def run_ours(args) -> None:
             "clocks": clk,
             "roofline": {
                 "kernel": "k_x2 (Y = X X^T on DMMA.8x8x4, fused branch/trace epilogue)", "bound": "tensor",
-                "achieved": alg_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": alg_tf / peak_tf, "traffic": None,
+                "achieved": alg_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": alg_tf / peak_tf,
+                "traffic": X2_DRAM_BYTES_PER_LAUNCH.get(args.workload), "traffic_unit": "B per launch (dram read + write, ncu --set full, profiles/r01_x2_v4_ncu.md); algorithmic bytes per launch = %.3g" % (16.0 * info["dense_elems"]),
                 "basis": "algorithmic 2 m^3 flop per community per iteration (unpadded, symmetry not counted) / mean "
                          "CUDA-event time of the %d launches" % ph["x2_launches"],
                 "peak_source": "FP64: %s bf16 sustained %.1f TF x nominal 40/2250" % (peaks["source"], peaks["bf16_tf"]),

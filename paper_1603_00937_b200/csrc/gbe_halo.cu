@@ -296,7 +296,8 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
       const int T = (g->h_m[p] + tile - 1) / tile;
       const int64_t ld = (g->h_m[p] + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
       for (int ti = 0; ti < T; ++ti)
-        for (int tj = ti; tj < T; ++tj) items.push_back({p, ti, tj, 0});
+        for (int tj = ti; tj < T; ++tj)
+          items.push_back({p, ti, tj, g->h_m[p], g->h_ncore[p], (int32_t)ld, g->h_dense_off[p]});
       // executed DMMA work: 8x8 sub-tiles (bi <= bj) with rows < m, columns < ld, each 2*8*8*ld flop
       const double R = (double)((g->h_m[p] + 7) / 8), C = (double)(ld / 8);
       g->exec_flops_per_iter += (R * C - R * (R - 1) / 2) * 128.0 * (double)ld;

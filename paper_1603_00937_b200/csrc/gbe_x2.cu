@@ -99,9 +99,7 @@ __device__ __forceinline__ void x2_chunk(double (&acc)[2][8][2], const double* _
 
 template <int MINB>
 __global__ void __launch_bounds__(X2_THREADS, MINB)
-    k_x2(const gbe_tile_item* __restrict__ items, const int64_t* __restrict__ sub_ptr,
-         const int32_t* __restrict__ ncore_arr, const int64_t* __restrict__ dense_off,
-         const gbe_state* __restrict__ st, const double* __restrict__ Xin, double* __restrict__ Xout,
+    k_x2(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin, double* __restrict__ Xout,
          double* __restrict__ partials) {
   extern __shared__ __align__(16) double smem[];  // 2 stages x (A panel, B panel)
   __shared__ double red[8];
@@ -109,13 +107,12 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   if (st->stop) return;  // idempotency stop already fired (A-7): X is final
   const int branch = st->branch;
 
-  const gbe_tile_item it = items[blockIdx.x];
-  const int p = it.p, ti = it.ti, tj = it.tj;
-  const int m = (int)(sub_ptr[p + 1] - sub_ptr[p]);
-  const int nc = ncore_arr[p];
-  const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
-  const double* __restrict__ X = Xin + dense_off[p];
-  double* __restrict__ Y = Xout + dense_off[p];
+  const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // p, ti, tj, m
+  const int4 it1 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x + 1];  // nc, ld, dense_off
+  const int ti = it0.y, tj = it0.z, m = it0.w, nc = it1.x, ld = it1.y;
+  const int64_t doff = ((int64_t)(uint32_t)it1.z) | ((int64_t)it1.w << 32);
+  const double* __restrict__ X = Xin + doff;
+  double* __restrict__ Y = Xout + doff;
   const bool diag = (ti == tj);
   const int row0 = ti * X2_BT, col0 = tj * X2_BT;
   const int nchunks = ld / X2_KC;
@@ -127,17 +124,14 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
 
   // warp-uniform masks over the 2 x 8 sub-tiles, bit (i * 8 + j):
   //   active: rows < m, columns < ld, not strictly below the diagonal;  mirror: strictly above the diagonal
-  unsigned active = 0, mirror = 0;
-#pragma unroll
-  for (int i = 0; i < 2; ++i)
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      const int r8 = row0 + 8 * rblk[i], c8 = col0 + 8 * j;
-      if (r8 < m && c8 < ld && r8 <= c8) {
-        active |= 1u << (i * 8 + j);
-        if (r8 < c8) mirror |= 1u << (i * 8 + j);
-      }
-    }
+  unsigned active, mirror;
+  {  // lane L < 16 evaluates bit L = (i, j); two ballots build the masks
+    const int i = (lane >> 3) & 1, j = lane & 7;
+    const int r8 = row0 + 8 * (i ? 7 - role : role), c8 = col0 + 8 * j;
+    const bool on = lane < 16 && r8 < m && c8 < ld && r8 <= c8;
+    active = __ballot_sync(0xffffffffu, on);
+    mirror = __ballot_sync(0xffffffffu, on && r8 < c8);
+  }
 
   // copy slots of this thread: rows (t >> 3) + 16 u, u = 0..3, 16-byte chunk (t & 7) of each K chunk.
   // Rows beyond the edge are clamped to row m - 1: finite data whose products are never stored.
@@ -222,8 +216,9 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   // epilogue: X_{n+1} = Y or 2 X_n - Y, direct + mirrored store, core-row trace partials.
   // Interior tiles (no ragged edge, no core row or column: most of them) take the path without any predicate.
   double s1 = 0.0, s2 = 0.0;
-  auto epilogue = [&](auto edge_c, auto trace_c) {
+  auto epilogue = [&](auto edge_c, auto trace_c, auto full_c) {
     constexpr bool EDGE = decltype(edge_c)::value, TRACE = decltype(trace_c)::value;
+    constexpr bool FULL = decltype(full_c)::value;  // every sub-tile active and strictly above the diagonal
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
       const int r = row0 + rblk[i] * 8 + g;
@@ -233,7 +228,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
       double* __restrict__ ym = Y + (size_t)(col0 + 2 * q) * ld + r;  // mirrored position of column block 0
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
-        if (!(active & (1u << (i * 8 + j)))) continue;  // c < ld holds for every active sub-tile
+        if (!FULL && !(active & (1u << (i * 8 + j)))) continue;  // c < ld holds for every active sub-tile
         const int c = col0 + j * 8 + 2 * q;
         double v0 = acc[i][j][0], v1 = acc[i][j][1];
         if (branch) {
@@ -251,7 +246,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
           if (r == c) s1 += v0;
           if (r == c + 1) s1 += v1;
         }
-        if (mirror & (1u << (i * 8 + j))) {
+        if (FULL || (mirror & (1u << (i * 8 + j)))) {
           if (!EDGE || c < m) {
             ym[(size_t)(j * 8) * ld] = v0;
             if (TRACE && c < nc) s2 += v0 * v0;
@@ -267,10 +262,12 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   const bool edge = col0 + X2_BT > m;             // row0 <= col0: the row edge implies the column edge
   const bool trace = row0 < nc || col0 < nc;      // a core row, directly or through the mirror
   if (edge || trace) {
-    if (edge) epilogue(std::true_type{}, std::true_type{});
-    else epilogue(std::false_type{}, std::true_type{});
+    if (edge) epilogue(std::true_type{}, std::true_type{}, std::false_type{});
+    else epilogue(std::false_type{}, std::true_type{}, std::false_type{});
+  } else if (active == X2_FULL && mirror == X2_FULL) {
+    epilogue(std::false_type{}, std::false_type{}, std::true_type{});
   } else {
-    epilogue(std::false_type{}, std::false_type{});
+    epilogue(std::false_type{}, std::false_type{}, std::false_type{});
   }
   s1 = warp_sum(s1);
   s2 = warp_sum(s2);
@@ -292,7 +289,7 @@ int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout
     GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     configured = true;
   }
-  kern<<<g->n_items, X2_THREADS, smem, s>>>(g->items, g->sub_ptr, g->ncore, g->dense_off, st, Xin, Xout, partials);
+  kern<<<g->n_items, X2_THREADS, smem, s>>>(g->items, st, Xin, Xout, partials);
   GBE_LAUNCHED();
   return GBE_OK;
 }
