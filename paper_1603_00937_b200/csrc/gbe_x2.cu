@@ -225,10 +225,16 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
       if (EDGE && r >= m) continue;
       const double* __restrict__ xr = X + (size_t)r * ld + col0 + 2 * q;
       double* __restrict__ yr = Y + (size_t)r * ld + col0 + 2 * q;
-      double* __restrict__ ym = Y + (size_t)(col0 + 2 * q) * ld + r;  // mirrored position of column block 0
+      double* __restrict__ ym0 = Y + (size_t)(col0 + 2 * q) * ld + r;  // mirrored position (c, r) of column block 0
+      double* __restrict__ ym1 = ym0 + ld;                            // and (c + 1, r); both advance by 8 rows per j
+      const size_t mstep = (size_t)8 * ld;
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
-        if (!FULL && !(active & (1u << (i * 8 + j)))) continue;  // c < ld holds for every active sub-tile
+        if (!FULL && !(active & (1u << (i * 8 + j)))) {  // c < ld holds for every active sub-tile
+          ym0 += mstep;
+          ym1 += mstep;
+          continue;
+        }
         const int c = col0 + j * 8 + 2 * q;
         double v0 = acc[i][j][0], v1 = acc[i][j][1];
         if (branch) {
@@ -248,14 +254,16 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
         }
         if (FULL || (mirror & (1u << (i * 8 + j)))) {
           if (!EDGE || c < m) {
-            ym[(size_t)(j * 8) * ld] = v0;
+            *ym0 = v0;
             if (TRACE && c < nc) s2 += v0 * v0;
           }
           if (!EDGE || c + 1 < m) {
-            ym[(size_t)(j * 8 + 1) * ld] = v1;
+            *ym1 = v1;
             if (TRACE && c + 1 < nc) s2 += v1 * v1;
           }
         }
+        ym0 += mstep;
+        ym1 += mstep;
       }
     }
   };
