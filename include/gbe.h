@@ -169,6 +169,25 @@ int gbe_density_timed(const gbe_csr_view* H, const gbe_graph* g, double n_occ, i
                       void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val, gbe_sp2_log* log,
                       gbe_phase_times* times);
 
+/* gbe_density with a PRE-DETERMINED SP2 sequence ("the complete SP2 sequence (the same for each subgraph
+ * expansion) ... determined beforehand", e.g. from the previous MD step): iteration k applies X <- X^2 if branch[k] == 0,
+ * X <- 2X - X^2 if branch[k] == 1, for every community.  No decision is taken on the device.
+ *   branch   HOST array of `iters` bytes, each 0 or 1 (read before the call returns).
+ *   trace_every_iteration != 0: the global traces t1[k], t2[k] are still reduced and logged every iteration;
+ *                         == 0: no per-iteration reduction kernel at all ("without exchange of information during or
+ *                               between the matrix multiplications"); the log then holds only t1, t2 of the
+ *                               final X at index `iters` (earlier entries are unspecified) and the given branches.
+ * Other arguments, stream semantics and D_val as gbe_density. */
+int gbe_density_preset(const gbe_csr_view* H, const gbe_graph* g, const uint8_t* branch, int32_t iters,
+                       int32_t trace_every_iteration, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                       double* D_val, gbe_sp2_log* log);
+
+/* Expectation value <A> = Tr[D A] = sum_{k,i} D_ki A_ik; with A = H the band energy E_band = Tr[DH].
+ *   D_val  device double[nnz_D]: the values gbe_density wrote, on the pattern of `g`.
+ *   A      device CSR of dimension n, ascending columns (need not be symmetric, need not share D's pattern).
+ *   out    HOST double; the call synchronises the stream.  The reduction order is fixed: reproducible bit for bit. */
+int gbe_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view* A, void* cuda_stream, double* out);
+
 /* Number of CUDA kernels this library has launched in this process so far (all threads). */
 uint64_t gbe_launch_count(void);
 

@@ -13,6 +13,7 @@ line numbers of the paper text; `A-n` are the readings listed in DESIGN.md secti
     subgraphs, density_pattern     step 2   P:L58, Fig.1, obs. (vi) P:L65 (A-9)
     o_sub                          steps 3-6: Eq.(6) P:L60-63 with SP2   <- parity target
     o_diag                         exact zero-temperature projector theta(mu I - H)
+    expectation                    <A> = Tr[D A], E_band = Tr[D H]
     o_eq5_exact, o_eq5_nested      Eq.(4)-(5) P:L47-56 literally on the full matrix (tiny inputs)
 
 Pins (tests/test_oracle_*.py): closed forms (2x2 projector, periodic-chain projector),
@@ -30,6 +31,7 @@ from .gbe_oracle import (  # noqa: F401
     sp2_polynomial_coeffs,
     o_sub,
     o_diag,
+    expectation,
     o_eq5_exact,
     o_eq5_nested,
     SubResult,

@@ -236,6 +236,22 @@ def o_sub(H, S_row_ptr, S_col, part, n_part: int, n_occ: float, iters: int, idem
 
 
 # ----------------------------------------------------------------------------------------
+# observables
+# ----------------------------------------------------------------------------------------
+def expectation(D_row_ptr, D_col, D_val, A, n: int | None = None) -> float:
+    """<A> = Tr[D A] = sum_{k,i} D_ki A_ik (P:L72 'expectation values ... Tr[DA]'; E_band = Tr[DH]).
+    D given as CSR arrays (the assembled, non-symmetric P_tau), A a duck-typed CSR object or a dense array."""
+    if hasattr(A, "row_ptr"):
+        n = A.n
+        Ad = sp.csr_matrix((A.val, A.col_idx, A.row_ptr), shape=(n, n))
+    else:
+        Ad = sp.csr_matrix(np.asarray(A))
+        n = Ad.shape[0]
+    D = sp.csr_matrix((D_val, D_col, D_row_ptr), shape=(n, n))
+    return float(D.multiply(Ad.T).sum())
+
+
+# ----------------------------------------------------------------------------------------
 # exact projector
 # ----------------------------------------------------------------------------------------
 def o_diag(H, n_occ: int) -> np.ndarray:

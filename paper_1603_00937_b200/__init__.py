@@ -19,6 +19,8 @@ from .binding import (  # noqa: F401
     gbe_build_graph,
     gbe_build_graph_host,
     gbe_density_timed,
+    gbe_density_preset,
+    gbe_expectation,
     gbe_launch_count,
     gbe_graph_export,
     gbe_density,

@@ -19,7 +19,7 @@ GBE_MAX_ITERS = 1024
 EXPORTS = [
     "gbe_build_graph", "gbe_graph_get_info", "gbe_graph_export", "gbe_density", "gbe_gather", "gbe_sp2",
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
-    "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count",
+    "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation",
 ]
 
 
@@ -81,6 +81,9 @@ def lib() -> C.CDLL:
         l.gbe_density_host.argtypes = l.gbe_density.argtypes
         l.gbe_density_timed.argtypes = l.gbe_density.argtypes + [C.POINTER(_PhaseTimes)]
         l.gbe_build_graph_host.argtypes = l.gbe_build_graph.argtypes
+        l.gbe_density_preset.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p,
+                                         C.c_size_t, C.c_void_p, C.c_void_p, C.POINTER(_Sp2Log)]
+        l.gbe_expectation.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CsrView), C.c_void_p, C.POINTER(C.c_double)]
         l.gbe_launch_count.restype = C.c_uint64
         l.gbe_launch_count.argtypes = []
         l.gbe_gather.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -254,6 +257,33 @@ def gbe_density_timed(H: DeviceCSR, g: Graph, n_occ: float, iters: int, idem_tol
     _check(lib().gbe_density_timed(C.byref(v), g.handle, float(n_occ), int(iters), float(idem_tol), _ptr(workspace),
                                    workspace.numel(), _stream(stream), _ptr(D_val), None, C.byref(pt)))
     return D_val, {k: getattr(pt, k) for k, _ in _PhaseTimes._fields_}
+
+
+def gbe_density_preset(H: DeviceCSR, g: Graph, branch, trace_every_iteration: bool = True,
+                       workspace: torch.Tensor | None = None, D_val: torch.Tensor | None = None, want_log: bool = True,
+                       stream=None):
+    """gbe_density with a pre-determined SP2 sequence: branch[k] in {0, 1}, host array.  Returns (D_val, log)."""
+    if workspace is None:
+        workspace = g.new_workspace()
+    if D_val is None:
+        D_val = torch.empty(g.info["nnz_D"], dtype=torch.float64, device="cuda")
+    br = np.ascontiguousarray(branch, dtype=np.uint8)
+    iters = int(br.size)
+    v = H.view()
+    clog, arrs = _new_log(iters) if want_log else (None, None)
+    _check(lib().gbe_density_preset(C.byref(v), g.handle, br.ctypes.data if iters else None, iters,
+                                    int(bool(trace_every_iteration)), _ptr(workspace), workspace.numel(), _stream(stream),
+                                    _ptr(D_val), C.byref(clog) if want_log else None))
+    return D_val, (_finish_log(clog, arrs) if want_log else None)
+
+
+def gbe_expectation(g: Graph, D_val: torch.Tensor, A: DeviceCSR, stream=None) -> float:
+    """<A> = Tr[D A]; A = H gives the band energy.  Synchronises."""
+    assert D_val.dtype == torch.float64 and D_val.is_cuda and D_val.numel() == g.info["nnz_D"]
+    v = A.view()
+    out = C.c_double(0.0)
+    _check(lib().gbe_expectation(g.handle, _ptr(D_val), C.byref(v), _stream(stream), C.byref(out)))
+    return float(out.value)
 
 
 def gbe_gather(H: DeviceCSR, g: Graph, workspace: torch.Tensor, stream=None) -> None:

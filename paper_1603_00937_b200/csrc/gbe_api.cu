@@ -34,14 +34,17 @@ int timed(Timer* tm, int phase, int launches, F&& fn) {
   return rc;
 }
 
-__global__ void k_init_state(gbe_state* st, double n_occ, double idem_tol, int iters) {
+// mode 0: branch chosen on the device every iteration; 1: preset sequence, traces logged every iteration;
+// 2: preset sequence, no per-iteration trace kernel (the final X is in buffer iters & 1)
+__global__ void k_init_state(gbe_state* st, double n_occ, double idem_tol, int iters, int mode) {
   st->n_occ = n_occ;
   st->idem_tol = idem_tol;
   st->iters = iters;
-  st->iter = 0;
+  st->iter = mode == 2 ? iters : 0;
   st->branch = 0;
   st->stop = 0;
-  st->iters_done = 0;
+  st->iters_done = mode == 2 ? iters : 0;
+  st->preset = mode != 0;
 }
 
 struct WS {
@@ -204,7 +207,8 @@ int gbe_gather(const gbe_csr_view* H, const gbe_graph* g, void* workspace, size_
 }
 
 static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_tol, void* workspace,
-                  size_t workspace_bytes, void* cuda_stream, Timer* tm) {
+                  size_t workspace_bytes, void* cuda_stream, Timer* tm, const uint8_t* preset = nullptr,
+                  bool trace_each = true) {
   if (!g) return GBE_EINVAL;
   if (!(n_occ >= 0.0) || n_occ > (double)g->n || iters < 0 || iters > GBE_MAX_ITERS || std::isnan(idem_tol))
     return GBE_EINVAL;
@@ -212,17 +216,26 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
   GBE_TRY(carve(g, workspace, workspace_bytes, &w));
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   // traces of X_0 (partials written by the gather), branch of iteration 0
-  GBE_TRY(timed(tm, PH_TRACE, 2, [&]() -> int {
-    k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters);
+  const int mode = !preset ? 0 : (trace_each ? 1 : 2);
+  GBE_TRY(timed(tm, PH_TRACE, mode == 2 ? 1 : 2, [&]() -> int {
+    k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode);
     GBE_LAUNCHED();
+    if (preset && iters > 0)
+      GBE_CUDA(cudaMemcpyAsync(w.st->br, preset, (size_t)iters, cudaMemcpyHostToDevice, s));
+    if (mode == 2) return GBE_OK;
     return gbe_launch_trace_branch(w.st, w.partials, g->n_gitems, s);
   }));
   for (int it = 0; it < iters; ++it) {
     const double* in = (it & 1) ? w.X1 : w.X0;
     double* outp = (it & 1) ? w.X0 : w.X1;
     GBE_TRY(timed(tm, PH_X2, g->n_items ? 1 : 0, [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, s); }));
-    GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, g->n_items, s); }));
+    if (mode != 2)
+      GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, g->n_items, s); }));
   }
+  if (mode == 2)  // one trace kernel at the end: t1, t2 of the final X for the log (written at index iters)
+    GBE_TRY(timed(tm, PH_TRACE, 1, [&] {
+      return gbe_launch_trace_branch(w.st, w.partials, iters > 0 ? g->n_items : g->n_gitems, s);
+    }));
   return GBE_OK;
 }
 int gbe_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_tol, void* workspace, size_t workspace_bytes,
@@ -297,6 +310,37 @@ int gbe_density_timed(const gbe_csr_view* H, const gbe_graph* g, double n_occ, i
     *nl[r.phase] += r.launches;
   }
   if (!tm.recs.empty()) GBE_CUDA(cudaEventElapsedTime(&times->total_ms, tm.recs.front().e0, tm.recs.back().e1));
+  return GBE_OK;
+}
+
+int gbe_density_preset(const gbe_csr_view* H, const gbe_graph* g, const uint8_t* branch, int32_t iters,
+                       int32_t trace_every_iteration, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                       double* D_val, gbe_sp2_log* log) {
+  if (!g || (!D_val && g->nnz_D > 0)) return GBE_EINVAL;
+  if (iters < 0 || iters > GBE_MAX_ITERS || (iters > 0 && !branch)) return GBE_EINVAL;
+  for (int k = 0; k < iters; ++k)
+    if (branch[k] > 1) return GBE_EINVAL;
+  static const uint8_t none = 0;
+  GBE_TRY(do_gather(H, g, workspace, workspace_bytes, cuda_stream, nullptr));
+  GBE_TRY(do_sp2(g, 0.0, iters, -1.0, workspace, workspace_bytes, cuda_stream, nullptr, iters > 0 ? branch : &none,
+                 trace_every_iteration != 0));
+  GBE_TRY(do_scatter(g, workspace, workspace_bytes, cuda_stream, D_val, nullptr));
+  if (log) GBE_TRY(gbe_read_log(g, workspace, workspace_bytes, cuda_stream, log));
+  return GBE_OK;
+}
+
+int gbe_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view* A, void* cuda_stream, double* out) {
+  if (!g || !out || (!D_val && g->nnz_D > 0)) return GBE_EINVAL;
+  GBE_TRY(check_csr(A));
+  if (A->n != g->n) return GBE_EMISMATCH;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  gbe_set_alloc_stream(s);
+  DevBuf rows, res;
+  GBE_TRY(rows.alloc((size_t)g->n * 8));
+  GBE_TRY(res.alloc(8));
+  GBE_TRY(gbe_launch_expectation(g, D_val, *A, rows.as<double>(), res.as<double>(), s));
+  GBE_CUDA(cudaMemcpyAsync(out, res.p, 8, cudaMemcpyDeviceToHost, s));
+  GBE_CUDA(cudaStreamSynchronize(s));
   return GBE_OK;
 }
 

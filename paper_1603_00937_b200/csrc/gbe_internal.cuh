@@ -72,7 +72,8 @@ struct gbe_state {
   int32_t stop;        // 1 once the idempotency stop fired (A-7) or `iters` iterations are done
   int32_t iters_done;  // number of updates applied; the final X lives in buffer iters_done & 1
   int32_t degenerate;  // eps_max == eps_min
-  int32_t pad_[2];
+  int32_t preset;      // 1: the branch sequence br[] was given by the caller (gbe_density_preset)
+  int32_t pad_;
   double t1[GBE_MAX_ITERS + 1];
   double t2[GBE_MAX_ITERS + 1];
   uint8_t br[GBE_MAX_ITERS];
@@ -135,6 +136,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s);
 int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state* st, double* X, double* partials,
                       cudaStream_t s);
 // step 4
+// iter: index n of the update X_n -> X_{n+1} (selects br[n] when the sequence is preset)
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
                   cudaStream_t s);
 // step 5
@@ -142,6 +144,10 @@ int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partial
 // step 6
 int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0, const double* X1, double* D_val,
                        cudaStream_t s);
+
+// observables (gbe_observe.cu)
+int gbe_launch_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view& A, double* row_sum, double* out,
+                           cudaStream_t s);
 
 // small device utilities (gbe_util.cu)
 int gbe_exclusive_scan_i64(const int64_t* in, int64_t* out, int64_t n, cudaStream_t s);  // out has n+1 entries

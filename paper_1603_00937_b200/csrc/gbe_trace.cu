@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double
     if (k >= st->iters || (st->idem_tol >= 0.0 && k >= 1 && fabs(t1 - t2) <= st->idem_tol)) {
       st->stop = 1;
     } else {
-      const int b = (fabs(t2 - n_occ) < fabs(2.0 * t1 - t2 - n_occ)) ? 0 : 1;
+      const int b = st->preset ? (int)st->br[k] : ((fabs(t2 - n_occ) < fabs(2.0 * t1 - t2 - n_occ)) ? 0 : 1);
       st->branch = b;
       st->br[k] = (uint8_t)b;
       st->iter = k + 1;

@@ -100,12 +100,12 @@ __device__ __forceinline__ void x2_chunk(double (&acc)[2][8][2], const double* _
 template <int MINB>
 __global__ void __launch_bounds__(X2_THREADS, MINB)
     k_x2(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin, double* __restrict__ Xout,
-         double* __restrict__ partials) {
+         double* __restrict__ partials, int iter) {
   extern __shared__ __align__(16) double smem[];  // 2 stages x (A panel, B panel)
   __shared__ double red[8];
 
   if (st->stop) return;  // idempotency stop already fired (A-7): X is final
-  const int branch = st->branch;
+  const int branch = st->preset ? (int)st->br[iter] : st->branch;  // preset sequence or the on-device choice
 
   const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // p, ti, tj, m
   const int4 it1 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x + 1];  // nc, ld, dense_off
@@ -288,7 +288,8 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
 }
 
 template <int MINB>
-int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, cudaStream_t s) {
+int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
+              cudaStream_t s) {
   auto kern = k_x2<MINB>;
   const size_t smem = (size_t)2 * X2_STAGE * sizeof(double);
   static bool configured = false;
@@ -297,7 +298,7 @@ int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout
     GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     configured = true;
   }
-  kern<<<g->n_items, X2_THREADS, smem, s>>>(g->items, st, Xin, Xout, partials);
+  kern<<<g->n_items, X2_THREADS, smem, s>>>(g->items, st, Xin, Xout, partials, iter);
   GBE_LAUNCHED();
   return GBE_OK;
 }
@@ -305,7 +306,6 @@ int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout
 
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
                   cudaStream_t s) {
-  (void)iter;
   if (g->n_items == 0) return GBE_OK;
-  return launch_x2<4>(g, st, Xin, Xout, partials, s);
+  return launch_x2<4>(g, st, Xin, Xout, partials, iter, s);
 }

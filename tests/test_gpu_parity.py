@@ -219,6 +219,74 @@ def test_idem_tol_stops_on_device(gbe):
     check_density(Dg, log, r)
 
 
+# ------------------------------------------------------------------------------- pre-determined SP2 sequence
+@pytest.mark.parametrize("trace", [True, False])
+def test_preset_sequence_from_the_previous_md_step(gbe, trace):
+    """'the complete SP2 sequence (the same for each subgraph expansion) ... can be determined beforehand' (P:L90):
+    the sequence is the one the oracle chooses for the Hamiltonian of the previous step (another noise draw), applied
+    to the current H; the oracle replays the same sequence."""
+    import torch
+    prev = gi.chain(512, 16, seed=3)
+    s = gi.chain(512, 16, seed=0)
+    rp, ci = o.build_graph(prev.H, prev.tau)
+    seq = o.o_sub(prev.H, rp, ci, prev.part, prev.n_part, prev.n_occ, prev.iters).branch
+    rp, ci = o.build_graph(s.H, s.tau)
+    r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, s.iters, replay=(seq, len(seq)))
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    Dg, log = gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=trace)
+    torch.cuda.synchronize()
+    assert log.iters_done == len(seq) and np.array_equal(log.branch, seq)
+    assert np.abs(Dg.cpu().numpy() - r.D_val).max() <= TOL_D
+    assert abs(log.t1[-1] - r.t1[-1]) <= TOL_TR and abs(log.t2[-1] - r.t2[-1]) <= TOL_TR
+    if trace:
+        assert np.abs(log.t1 - r.t1).max() <= TOL_TR and np.abs(log.t2 - r.t2).max() <= TOL_TR
+
+
+def test_preset_arbitrary_sequence_on_water(gbe):
+    """Any 0/1 sequence is a polynomial (Eq.(1)): a fixed alternating sequence on the 6,144-orbital box, with no
+    reduction kernel between the products; compared with the oracle's replay of the same sequence."""
+    import torch
+    s = gi.config(2)
+    seq = np.array([1, 0] * 6, dtype=np.uint8)
+    rp, ci = o.build_graph(s.H, s.tau)
+    r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, len(seq), replay=(seq, len(seq)))
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    n0 = gbe.gbe_launch_count()
+    Dg, log = gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False)
+    torch.cuda.synchronize()
+    assert gbe.gbe_launch_count() - n0 == 2 + 1 + 1 + len(seq) + 1 + 1  # bounds(2) gather init x2... final trace scatter
+    assert np.abs(Dg.cpu().numpy() - r.D_val).max() <= TOL_D
+    assert abs(log.t1[-1] - r.t1[-1]) <= TOL_TR
+    with pytest.raises(gbe.GbeError):
+        gbe.gbe_density_preset(Hd, g, np.array([0, 2], dtype=np.uint8))
+
+
+# ------------------------------------------------------------------------------- observables (P:L72, P:L76)
+def test_band_energy_and_expectation_values(gbe):
+    import torch
+    s = gi.config(2)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    Dt = torch.from_numpy(Dg).cuda()
+    e_gpu = gbe.gbe_expectation(g, Dt, Hd)
+    e_ref = o.expectation(ex["D_row_ptr"], ex["D_col"], Dg, s.H)
+    assert abs(e_gpu - e_ref) <= 1e-9 * abs(e_ref)
+    assert gbe.gbe_expectation(g, Dt, Hd) == e_gpu  # fixed reduction order: reproducible
+    # Tr[D I] is the trace the SP2 log reports; a non-symmetric operand exercises the transposed lookup
+    eye = gi.CSR.from_scipy(sp.identity(s.n, format="csr"))
+    assert abs(gbe.gbe_expectation(g, Dt, gbe.DeviceCSR.from_host(eye)) - log.t1[-1]) <= 1e-8
+    rng = np.random.default_rng(1)
+    A = sp.random(s.n, s.n, density=2e-3, random_state=rng, format="csr") + sp.triu(s.H.to_scipy(), k=1)
+    Ac = gi.CSR.from_scipy(A)
+    a_ref = o.expectation(ex["D_row_ptr"], ex["D_col"], Dg, Ac)
+    assert abs(gbe.gbe_expectation(g, Dt, gbe.DeviceCSR.from_host(Ac)) - a_ref) <= 1e-9 * max(1.0, abs(a_ref))
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_expectation(g, Dt, gbe.DeviceCSR.from_host(gi.chain(32, 4).H))
+    assert e.value.status == -4
+
+
 # ------------------------------------------------------------------------------- degenerate shapes
 def test_one_partition_equals_exact_projector(gbe):
     s = gi.config(1)

@@ -381,3 +381,29 @@ def test_error_falls_with_tau_and_is_insensitive_to_partition_count():
         e.append(abs(dense_D(r, s.n) - D)[pattern_mask(r, s.n)].max())
     assert max(e) / min(e) < 5  # 'fairly insensitive to the number of graph partitions'
     assert abs(errs[3] - 3.04e-4) < 2e-5  # survey probe value for config 1
+
+
+# ------------------------------------------------------------------------------- observables
+def test_expectation_band_energy_is_the_sum_of_occupied_eigenvalues():
+    """Closed form: for the exact projector Tr[D H] = sum of the n_occ lowest eigenvalues; Tr[D I] = n_occ."""
+    s = gi.random_banded(60, half_bw=4, n_part=4, seed=2)
+    Hd = s.H.to_dense()
+    D = o.o_diag(s.H, 30)
+    Dc = gi.CSR.from_dense(D, keep_zeros=True)
+    e = o.expectation(Dc.row_ptr, Dc.col_idx, Dc.val, s.H)
+    assert abs(e - np.linalg.eigvalsh(Hd)[:30].sum()) < 1e-10
+    assert abs(o.expectation(Dc.row_ptr, Dc.col_idx, Dc.val, np.eye(60)) - 30.0) < 1e-10
+
+
+def test_expectation_uses_the_transpose_of_a_nonsymmetric_operand():
+    """Tr[D A] = sum_ki D_ki A_ik, by explicit loops on a non-symmetric D (the assembled P_tau, obs. (i)) and a
+    non-symmetric A - a transposed operand or a dropped off-pattern term would change the value."""
+    rng = np.random.default_rng(5)
+    n = 9
+    D = rng.normal(size=(n, n)) * (rng.uniform(size=(n, n)) < 0.5)
+    A = rng.normal(size=(n, n)) * (rng.uniform(size=(n, n)) < 0.6)
+    want = sum(D[k, i] * A[i, k] for k in range(n) for i in range(n))
+    Dc, Ac = gi.CSR.from_dense(D), gi.CSR.from_dense(A)
+    assert abs(o.expectation(Dc.row_ptr, Dc.col_idx, Dc.val, Ac) - want) < 1e-13
+    assert abs(want - np.trace(D @ A)) < 1e-13
+    assert abs(o.expectation(Dc.row_ptr, Dc.col_idx, Dc.val, Ac) - np.trace(D @ A.T)) > 1e-3
