@@ -108,6 +108,17 @@ typedef struct {
 int gbe_build_graph(const gbe_csr_view* H, const gbe_graph_opts* opts, const int32_t* part, int32_t n_part,
                     void* cuda_stream, gbe_graph** out);
 
+/* The graph for the NEXT molecular-dynamics step, Eq.(8) P:L84-88:
+ *     S_tau(t) <- floor( ( floor(D(t - dt))_tau + H(t) )^2 )_eps
+ * in the symbolic form the paper uses (eps = 0): M = I u pat(|D_ij| >= tau) u pat(H(t)), S = pattern of M M ("paths of
+ * length two"), symmetrised.  Steps 0 and 2 (bounds of H(t), halos, pattern of the new D) as gbe_build_graph.
+ *   prev    the graph D_prev was computed on (gives D's CSR pattern); not modified, still to be freed by the caller.
+ *   D_prev  device double[prev nnz_D]: D(t - dt) as written by gbe_density.
+ *   H       device CSR of H(t); opts->tau is the threshold applied to D (the paper uses 1e-4); opts->power is ignored.
+ *   part / n_part as gbe_build_graph (may differ from prev's).  Synchronises `cuda_stream`. */
+int gbe_update_graph(const gbe_graph* prev, const double* D_prev, const gbe_csr_view* H, const gbe_graph_opts* opts,
+                     const int32_t* part, int32_t n_part, void* cuda_stream, gbe_graph** out);
+
 int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* out);
 
 /* Copies the graph to caller-allocated DEVICE buffers (any may be NULL to skip), sizes from gbe_graph_info:

@@ -10,6 +10,7 @@ line numbers of the paper text; `A-n` are the readings listed in DESIGN.md secti
 
     gershgorin, normalised_x0      step 0   (readings A-5, A-12)
     build_graph                    step 1   Eq.(2), Eq.(8) P:L86 (reading A-1, A-3, A-4)
+    update_graph                   Eq.(8), symbolic form (graph of the next MD step from D(t-dt) and H(t))
     subgraphs, density_pattern     step 2   P:L58, Fig.1, obs. (vi) P:L65 (A-9)
     o_sub                          steps 3-6: Eq.(6) P:L60-63 with SP2   <- parity target
     o_diag                         exact zero-temperature projector theta(mu I - H)
@@ -25,6 +26,7 @@ from .gbe_oracle import (  # noqa: F401
     gershgorin,
     normalised_x0,
     build_graph,
+    update_graph,
     subgraphs,
     density_pattern,
     dense_block,

@@ -95,6 +95,26 @@ def build_graph(H, tau: float, power: int = 2, bounds: tuple[float, float] | Non
     return pat.indptr.astype(np.int64), pat.indices.astype(np.int32)
 
 
+def update_graph(D_row_ptr, D_col, D_val, H, tau: float):
+    """Eq.(8) P:L84-88 in the symbolic form the paper uses (eps = 0):
+        S_tau(t) <- floor( ( floor(D(t - dt))_tau + H(t) )^2 )_eps
+    'the non-zero pattern of the thresholded density matrix ... combined with the non-zero pattern of H(t), and instead
+    of the matrix square we use paths of length two'.  M = I u pat(|D_ij| >= tau) u pat(H); S = pat(M M); then S u S^T
+    (D is not symmetric, obs. (i) P:L65; self loops as in build_graph, A-4).  Returns (row_ptr int64, col int32)."""
+    n = H.n
+    D = sp.csr_matrix((D_val, D_col, D_row_ptr), shape=(n, n)).tocoo()
+    keep = np.abs(D.data) >= tau
+    M = sp.csr_matrix((np.ones(int(keep.sum()), dtype=np.int64), (D.row[keep], D.col[keep])), shape=(n, n))
+    Hp = sp.csr_matrix((np.ones(len(H.col_idx), dtype=np.int64), H.col_idx, H.row_ptr), shape=(n, n))
+    M = M + Hp + sp.identity(n, dtype=np.int64, format="csr")
+    M.data[:] = 1
+    S = sp.csr_matrix(M @ M)          # entry (i, j) > 0 iff a path i - k - j of length two exists in M
+    S.data[:] = 1
+    S = sp.csr_matrix(S + S.T)
+    S.sort_indices()
+    return S.indptr.astype(np.int64), S.indices.astype(np.int32)
+
+
 # ----------------------------------------------------------------------------------------
 # step 2 - subgraphs (core + halo) and the pattern of the assembled result
 # ----------------------------------------------------------------------------------------

@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     lib,
     gbe_build_graph,
     gbe_build_graph_host,
+    gbe_update_graph,
     gbe_density_timed,
     gbe_density_preset,
     gbe_expectation,

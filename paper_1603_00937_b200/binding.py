@@ -19,7 +19,7 @@ GBE_MAX_ITERS = 1024
 EXPORTS = [
     "gbe_build_graph", "gbe_graph_get_info", "gbe_graph_export", "gbe_density", "gbe_gather", "gbe_sp2",
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
-    "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation",
+    "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation", "gbe_update_graph",
 ]
 
 
@@ -74,6 +74,8 @@ def lib() -> C.CDLL:
         l.gbe_free_graph.argtypes = [C.c_void_p]
         l.gbe_build_graph.argtypes = [C.POINTER(_CsrView), C.POINTER(_GraphOpts), C.c_void_p, C.c_int32, C.c_void_p,
                                       C.POINTER(C.c_void_p)]
+        l.gbe_update_graph.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CsrView), C.POINTER(_GraphOpts), C.c_void_p,
+                                       C.c_int32, C.c_void_p, C.POINTER(C.c_void_p)]
         l.gbe_graph_get_info.argtypes = [C.c_void_p, C.POINTER(_GraphInfo)]
         l.gbe_graph_export.argtypes = [C.c_void_p] * 9
         l.gbe_density.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_double, C.c_int32, C.c_double, C.c_void_p,
@@ -193,6 +195,20 @@ def gbe_build_graph_host(H_host, tau: float, part_host: np.ndarray | None, n_par
     out = C.c_void_p()
     _check(lib().gbe_build_graph_host(C.byref(v), C.byref(opts), None if pt is None else pt.ctypes.data, int(n_part),
                                       _stream(stream), C.byref(out)))
+    return Graph(out.value)
+
+
+def gbe_update_graph(prev: Graph, D_prev: torch.Tensor, H: DeviceCSR, tau: float, part: torch.Tensor | None, n_part: int,
+                     stream=None) -> Graph:
+    """Eq.(8): the graph of the next MD step from D(t - dt) (on prev's pattern) and H(t), symbolic square."""
+    assert D_prev.dtype == torch.float64 and D_prev.is_cuda and D_prev.numel() == prev.info["nnz_D"]
+    opts = _GraphOpts(float(tau), 0, 0)
+    if part is not None:
+        assert part.dtype == torch.int32 and part.is_cuda and part.is_contiguous() and part.numel() == H.n
+    out = C.c_void_p()
+    v = H.view()
+    _check(lib().gbe_update_graph(prev.handle, _ptr(D_prev), C.byref(v), C.byref(opts), _ptr(part), int(n_part),
+                                  _stream(stream), C.byref(out)))
     return Graph(out.value)
 
 

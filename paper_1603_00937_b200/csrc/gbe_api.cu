@@ -103,8 +103,8 @@ void gbe_free_graph(gbe_graph* g) {
   delete g;
 }
 
-int gbe_build_graph(const gbe_csr_view* H, const gbe_graph_opts* opts, const int32_t* part, int32_t n_part,
-                    void* cuda_stream, gbe_graph** out) {
+static int build_graph_impl(const gbe_csr_view* H, const gbe_graph_opts* opts, const int32_t* part, int32_t n_part,
+                            void* cuda_stream, gbe_graph** out, const gbe_graph* prev, const double* D_prev) {
   if (!out) return GBE_EINVAL;
   *out = nullptr;
   GBE_TRY(check_csr(H));
@@ -139,15 +139,30 @@ int gbe_build_graph(const gbe_csr_view* H, const gbe_graph_opts* opts, const int
   g->eps_min = b.lo;
   g->eps_max = b.hi;
 
-  // step 1: S_tau
-  GBE_TRY(gbe_build_pattern(*H, st.as<gbe_state>(), g->tau, power, opts->check_symmetry, s, &g->S_row_ptr, &g->S_col,
-                            &g->nnz_S));
+  // step 1: S_tau - from H and its thresholded powers (A-1), or by Eq.(8) from the previous D and this H
+  if (prev)
+    GBE_TRY(gbe_build_pattern_eq8(*H, prev->D_row_ptr, prev->D_col, D_prev, g->tau, s, &g->S_row_ptr, &g->S_col, &g->nnz_S));
+  else
+    GBE_TRY(gbe_build_pattern(*H, st.as<gbe_state>(), g->tau, power, opts->check_symmetry, s, &g->S_row_ptr, &g->S_col,
+                              &g->nnz_S));
   // step 2: subgraphs, layout, pattern of D, work lists
   GBE_TRY(gbe_build_subgraphs(g, part, s));
   GBE_CUDA(cudaStreamSynchronize(s));
   guard.g = nullptr;
   *out = g;
   return GBE_OK;
+}
+
+int gbe_build_graph(const gbe_csr_view* H, const gbe_graph_opts* opts, const int32_t* part, int32_t n_part,
+                    void* cuda_stream, gbe_graph** out) {
+  return build_graph_impl(H, opts, part, n_part, cuda_stream, out, nullptr, nullptr);
+}
+
+int gbe_update_graph(const gbe_graph* prev, const double* D_prev, const gbe_csr_view* H, const gbe_graph_opts* opts,
+                     const int32_t* part, int32_t n_part, void* cuda_stream, gbe_graph** out) {
+  if (!prev || (!D_prev && prev->nnz_D > 0)) return GBE_EINVAL;
+  if (H && H->n != prev->n) return GBE_EMISMATCH;
+  return build_graph_impl(H, opts, part, n_part, cuda_stream, out, prev, D_prev);
 }
 
 int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {

@@ -137,6 +137,7 @@ __device__ __forceinline__ void walk_products(int lane, int64_t a, int64_t b, co
 // MODE 0: distinct candidate columns per row (sizes the accumulator); 1: count kept entries; 2: fill (columns + values);
 // 3: one pass for the LAST power, whose values are not needed: kept columns go to a scratch row of candidate capacity
 //    (offsets out_rp from MODE 0's counts) and cnt[i] = number kept.
+// 4: symbolic product (Eq.(8) with eps = 0: "paths of length two"): emits every candidate column at out_rp.
 template <int MODE>
 __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __restrict__ A_rp,
                                    const int32_t* __restrict__ A_col, const double* __restrict__ A_val,
@@ -146,10 +147,10 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
                                    double* __restrict__ out_val) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, w_in_blk = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  const size_t per_warp = (size_t)W * 8 + (MODE == 0 ? 0 : (size_t)cap * 8);
+  const size_t per_warp = (size_t)W * 8 + ((MODE == 0 || MODE == 4) ? 0 : (size_t)cap * 8);
   unsigned char* base = smem_raw + per_warp * w_in_blk;
   double* acc = reinterpret_cast<double*>(base);  // cap doubles (first: keeps 8-byte alignment)
-  uint32_t* bm = reinterpret_cast<uint32_t*>(base + (MODE == 0 ? 0 : (size_t)cap * 8));
+  uint32_t* bm = reinterpret_cast<uint32_t*>(base + ((MODE == 0 || MODE == 4) ? 0 : (size_t)cap * 8));
   uint32_t* rk = bm + W;
 
   for (int64_t i = (int64_t)blockIdx.x * nw + w_in_blk; i < n; i += (int64_t)gridDim.x * nw) {
@@ -172,6 +173,20 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
     }
     if constexpr (MODE == 0) {
       if (lane == 0) cnt[i] = running;
+      __syncwarp();
+      continue;
+    }
+    if constexpr (MODE == 4) {
+      const int64_t ob4 = out_rp[i];
+      for (int w = lane; w < W; w += 32) {
+        uint32_t bits = bm[w];
+        int pos = (int)rk[w];
+        while (bits) {
+          const int bpos = __ffs(bits) - 1;
+          bits &= bits - 1;
+          out_col[ob4 + pos++] = w * 32 + bpos;
+        }
+      }
       __syncwarp();
       continue;
     }
@@ -226,6 +241,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
 // ---------------------------------------------------------------- row-wise union of two patterns (+ self loops)
 template <bool FILL>
 __global__ void k_union_rows(int64_t n, int W, const int64_t* __restrict__ P_rp, const int32_t* __restrict__ P_col,
+                             const double* __restrict__ P_val /* null: pattern only */, double p_tau,
                              const int64_t* __restrict__ Q_rp, const int32_t* __restrict__ Q_col,
                              const int32_t* __restrict__ Q_len /* null: compact CSR */, int add_diag,
                              int32_t* __restrict__ cnt, const int64_t* __restrict__ out_rp,
@@ -236,10 +252,16 @@ __global__ void k_union_rows(int64_t n, int W, const int64_t* __restrict__ P_rp,
   for (int64_t i = (int64_t)blockIdx.x * nw + w_in_blk; i < n; i += (int64_t)gridDim.x * nw) {
     for (int w = lane; w < W; w += 32) bm[w] = 0u;
     __syncwarp();
-    for (int64_t e = P_rp[i] + lane; e < P_rp[i + 1]; e += 32) { const int j = P_col[e]; atomicOr(&bm[j >> 5], 1u << (j & 31)); }
+    for (int64_t e = P_rp[i] + lane; e < P_rp[i + 1]; e += 32) {
+      const int j = P_col[e];
+      if ((unsigned)j < (uint64_t)n && (!P_val || fabs(P_val[e]) >= p_tau)) atomicOr(&bm[j >> 5], 1u << (j & 31));
+    }
     if (Q_rp) {
       const int64_t qb = Q_rp[i], qe = Q_len ? qb + Q_len[i] : Q_rp[i + 1];
-      for (int64_t e = qb + lane; e < qe; e += 32) { const int j = Q_col[e]; atomicOr(&bm[j >> 5], 1u << (j & 31)); }
+      for (int64_t e = qb + lane; e < qe; e += 32) {
+        const int j = Q_col[e];
+        if ((unsigned)j < (uint64_t)n) atomicOr(&bm[j >> 5], 1u << (j & 31));
+      }
     }
     if (add_diag && lane == 0) atomicOr(&bm[i >> 5], 1u << (i & 31));
     __syncwarp();
@@ -324,6 +346,64 @@ struct Pattern {  // device CSR (pattern, optionally with values) owned by DevBu
   int64_t nnz = 0;
 };
 
+int count_to_rowptr(DevBuf& cnt, int64_t n, DevBuf& rp, int64_t* nnz, cudaStream_t s);
+
+// row-wise unions on the device: out = [I u] filter(P) u Q
+struct Unioner {
+  int64_t n = 0;
+  int W = 0, uw = 0, ugrid = 0;
+  size_t bm_bytes = 0;
+  cudaStream_t s = nullptr;
+  DevBuf ucnt;  // row counts of the union being sized
+  int init(int64_t n_, cudaStream_t s_) {
+    n = n_;
+    s = s_;
+    W = (int)((n + 31) / 32);
+    bm_bytes = (size_t)W * 4;
+    int sm_count = 148;
+    cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, 0);
+    uw = pick_warps(bm_bytes, 8);
+    if (uw < 1) return GBE_EINVAL;  // n too large for a shared-memory bitmap
+    GBE_CUDA(cudaFuncSetAttribute(k_union_rows<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bm_bytes * uw)));
+    GBE_CUDA(cudaFuncSetAttribute(k_union_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bm_bytes * uw)));
+    ugrid = (int)std::min<int64_t>((n + uw - 1) / uw, (int64_t)sm_count * 8);
+    return ucnt.alloc((size_t)n * 4);
+  }
+  int run(const int64_t* p_rp, const int32_t* p_col, const double* p_val, double p_tau, const int64_t* q_rp,
+          const int32_t* q_col, const int32_t* q_len, int diag, Pattern& out) {
+    k_union_rows<false><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, p_val, p_tau, q_rp, q_col, q_len, diag,
+                                                              ucnt.as<int32_t>(), nullptr, nullptr);
+    GBE_LAUNCHED();
+    GBE_TRY(count_to_rowptr(ucnt, n, out.rp, &out.nnz, s));
+    GBE_TRY(out.col.alloc((size_t)out.nnz * 4));
+    k_union_rows<true><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, p_val, p_tau, q_rp, q_col, q_len, diag,
+                                                             nullptr, out.rp.as<int64_t>(), out.col.as<int32_t>());
+    GBE_LAUNCHED();
+    return GBE_OK;
+  }
+};
+
+// S = P u P^T (P's rows need not be sorted on input; S's are ascending)
+int symmetrise(Pattern& P, Unioner& U, DevBuf& cnt, Pattern& S) {
+  const int64_t n = U.n;
+  cudaStream_t s = U.s;
+  const int rows_grid = (int)((n + 7) / 8);
+  Pattern PT;
+  GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
+  k_transpose_count<<<rows_grid, 256, 0, s>>>(n, P.rp.as<int64_t>(), P.col.as<int32_t>(), cnt.as<int32_t>());
+  GBE_LAUNCHED();
+  GBE_TRY(count_to_rowptr(cnt, n, PT.rp, &PT.nnz, s));
+  GBE_TRY(PT.col.alloc((size_t)PT.nnz * 4));
+  GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
+  k_transpose_fill<<<rows_grid, 256, 0, s>>>(n, P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(),
+                                             cnt.as<int32_t>(), PT.col.as<int32_t>());
+  GBE_LAUNCHED();
+  GBE_TRY(U.run(P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr, 0.0, PT.rp.as<int64_t>(), PT.col.as<int32_t>(), nullptr,
+                0, S));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  return GBE_OK;
+}
+
 int count_to_rowptr(DevBuf& cnt, int64_t n, DevBuf& rp, int64_t* nnz, cudaStream_t s) {
   GBE_TRY(rp.alloc((size_t)(n + 1) * 8));
   GBE_TRY(gbe_exclusive_scan_i32_to_i64(cnt.as<int32_t>(), rp.as<int64_t>(), n, s));
@@ -369,26 +449,13 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                   A.col.as<int32_t>(), A.val.as<double>());
   GBE_LAUNCHED();
   // pattern accumulator P = I u pat(A)
-  const size_t bm_bytes = (size_t)W * 4;
-  const int uw = pick_warps(bm_bytes, 8);
-  if (uw < 1) return GBE_EINVAL;  // n too large for a shared-memory bitmap
-  GBE_CUDA(cudaFuncSetAttribute(k_union_rows<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bm_bytes * uw)));
-  GBE_CUDA(cudaFuncSetAttribute(k_union_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bm_bytes * uw)));
-  const int ugrid = (int)std::min<int64_t>((n + uw - 1) / uw, (int64_t)sm_count * 8);
-
-  DevBuf ucnt;  // row counts of the union being sized (cnt may hold the Q_len of a scratch pattern)
-  GBE_TRY(ucnt.alloc((size_t)n * 4));
+  Unioner U;
+  GBE_TRY(U.init(n, s));
+  DevBuf& ucnt = U.ucnt;
+  (void)ucnt;
   auto do_union = [&](const int64_t* p_rp, const int32_t* p_col, const int64_t* q_rp, const int32_t* q_col,
                       const int32_t* q_len, int diag, Pattern& out) -> int {
-    k_union_rows<false><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, q_rp, q_col, q_len, diag,
-                                                              ucnt.as<int32_t>(), nullptr, nullptr);
-    GBE_LAUNCHED();
-    GBE_TRY(count_to_rowptr(ucnt, n, out.rp, &out.nnz, s));
-    GBE_TRY(out.col.alloc((size_t)out.nnz * 4));
-    k_union_rows<true><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, q_rp, q_col, q_len, diag, nullptr,
-                                                             out.rp.as<int64_t>(), out.col.as<int32_t>());
-    GBE_LAUNCHED();
-    return GBE_OK;
+    return U.run(p_rp, p_col, nullptr, 0.0, q_rp, q_col, q_len, diag, out);
   };
 
   Pattern P;
@@ -473,19 +540,50 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     // Tn (now holding the previous T) and Pn are released here, after the sync above
   }
   // S = P u P^T
-  Pattern PT;
-  GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
-  k_transpose_count<<<rows_grid, 256, 0, s>>>(n, P.rp.as<int64_t>(), P.col.as<int32_t>(), cnt.as<int32_t>());
+  Pattern S;
+  GBE_TRY(symmetrise(P, U, cnt, S));
+  *nnz_S = S.nnz;
+  *S_row_ptr = reinterpret_cast<int64_t*>(S.rp.release());
+  *S_col = reinterpret_cast<int32_t*>(S.col.release());
+  return GBE_OK;
+}
+
+// ---------------------------------------------------------------- Eq.(8): graph for the next MD step
+//     S_tau(t) <- floor( ( floor(D(t - dt))_tau + H(t) )^2 )_eps,  used symbolically with eps = 0:
+//     M = I u pat(|D_ij| >= tau) u pat(H(t)),   S = pat(M M) ("paths of length two"),  then S u S^T.
+// D is the assembled, non-symmetric P_tau of the previous step on the pattern (D_rp, D_col).
+int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int32_t* D_col, const double* D_val, double tau,
+                          cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S) {
+  const int64_t n = H.n;
+  const int W = (int)((n + 31) / 32);
+  int sm_count = 148;
+  cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, 0);
+  Unioner U;
+  GBE_TRY(U.init(n, s));
+  DevBuf cnt;
+  GBE_TRY(cnt.alloc((size_t)n * 4));
+  Pattern M;
+  GBE_TRY(U.run(D_rp, D_col, D_val, tau, H.row_ptr, H.col_idx, nullptr, 1, M));
+  // symbolic square: count the candidates of every row, then emit them
+  const size_t per_warp = (size_t)W * 8;
+  const int nw = pick_warps(per_warp, 16);
+  if (nw < 1) return GBE_EINVAL;
+  GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
+  GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
+  const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
+  k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr,
+                                                             M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr, 0.0,
+                                                             cnt.as<int32_t>(), nullptr, nullptr, nullptr);
   GBE_LAUNCHED();
-  GBE_TRY(count_to_rowptr(cnt, n, PT.rp, &PT.nnz, s));
-  GBE_TRY(PT.col.alloc((size_t)PT.nnz * 4));
-  GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
-  k_transpose_fill<<<rows_grid, 256, 0, s>>>(n, P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(),
-                                             cnt.as<int32_t>(), PT.col.as<int32_t>());
+  Pattern P;
+  GBE_TRY(count_to_rowptr(cnt, n, P.rp, &P.nnz, s));
+  GBE_TRY(P.col.alloc((size_t)P.nnz * 4));
+  k_spgemm_threshold<4><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr,
+                                                             M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr, 0.0, nullptr,
+                                                             P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr);
   GBE_LAUNCHED();
   Pattern S;
-  GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(), PT.col.as<int32_t>(), nullptr, 0, S));
-  GBE_CUDA(cudaStreamSynchronize(s));
+  GBE_TRY(symmetrise(P, U, cnt, S));
   *nnz_S = S.nnz;
   *S_row_ptr = reinterpret_cast<int64_t*>(S.rp.release());
   *S_col = reinterpret_cast<int32_t*>(S.col.release());

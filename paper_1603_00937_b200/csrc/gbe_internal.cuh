@@ -130,6 +130,9 @@ int gbe_launch_bounds(const gbe_csr_view& H, double* block_lo, double* block_hi,
 // step 1
 int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st_dev, double tau, int power, int check_sym,
                       cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S);
+// Eq.(8): S for the next MD step from the previous D and the new H
+int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int32_t* D_col, const double* D_val, double tau,
+                          cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S);
 // step 2
 int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s);
 // step 3

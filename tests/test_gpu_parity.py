@@ -263,6 +263,35 @@ def test_preset_arbitrary_sequence_on_water(gbe):
         gbe.gbe_density_preset(Hd, g, np.array([0, 2], dtype=np.uint8))
 
 
+# ------------------------------------------------------------------------------- Eq.(8): graph of the next MD step
+@pytest.mark.parametrize("which", ["chain", "water"])
+def test_update_graph_eq8_md_step(gbe, which):
+    """One MD step: D(t - dt) on S(t - dt), then S(t) from Eq.(8) with the moved Hamiltonian H(t), then D(t) on
+    S(t).  Graph, halos and the new D against the oracle, which does the same from its own D(t - dt)."""
+    import torch
+    if which == "chain":
+        s0, s1, tau_d = gi.chain(512, 16, seed=0), gi.chain(512, 16, seed=1), 1e-4
+    else:
+        s0, s1, tau_d = gi.water_box(256, 32, seed=0, iters=20), gi.water_box(256, 32, seed=0, iters=20), 1e-4
+        # H(t): the same box with every element moved by up to 0.1 %, kept symmetric
+        Hs = s1.H.to_scipy()
+        Hs.data = Hs.data * (1.0 + 1e-3 * np.cos(np.arange(Hs.nnz) * 0.37))
+        s1.H = gi.CSR.from_scipy((Hs + Hs.T) * 0.5)
+    g0, ex0, D0, log0 = run_gpu(gbe, s0)
+    H1 = gbe.DeviceCSR.from_host(s1.H)
+    g1 = gbe.gbe_update_graph(g0, torch.from_numpy(D0).cuda(), H1, tau_d, None, s1.n_part)
+    D1, log1 = gbe.gbe_density(H1, g1, s1.n_occ, s1.iters)
+    torch.cuda.synchronize()
+    ex1 = {k: v.cpu().numpy() for k, v in g1.export().items()}
+    # oracle: its own previous step, its own Eq.(8)
+    (rp0, ci0), r0 = run_oracle(s0)
+    rp1, ci1 = o.update_graph(r0.D_row_ptr, r0.D_col, r0.D_val, s1.H, tau_d)
+    r1 = o.o_sub(s1.H, rp1, ci1, s1.part, s1.n_part, s1.n_occ, s1.iters)
+    check_structure(ex1, (rp1, ci1), r1, g1.info)
+    check_density(D1.cpu().numpy(), log1, r1)
+    assert g1.info["nnz_S"] >= ex0["S_col"].size or which == "water"
+
+
 # ------------------------------------------------------------------------------- observables (P:L72, P:L76)
 def test_band_energy_and_expectation_values(gbe):
     import torch

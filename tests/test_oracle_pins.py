@@ -407,3 +407,58 @@ def test_expectation_uses_the_transpose_of_a_nonsymmetric_operand():
     assert abs(o.expectation(Dc.row_ptr, Dc.col_idx, Dc.val, Ac) - want) < 1e-13
     assert abs(want - np.trace(D @ A)) < 1e-13
     assert abs(o.expectation(Dc.row_ptr, Dc.col_idx, Dc.val, Ac) - np.trace(D @ A.T)) > 1e-3
+
+
+# ------------------------------------------------------------------------------- Eq.(8): graph of the next MD step
+def test_update_graph_is_paths_of_length_two_by_brute_force():
+    """S = every (i, j) joined by a path of length <= 2 in M = I u pat(|D| >= tau) u pat(H), symmetrised - explicit loops."""
+    rng = np.random.default_rng(3)
+    n = 14
+    Hd = np.zeros((n, n))
+    for i in range(n - 1):
+        Hd[i, i + 1] = Hd[i + 1, i] = -1.0
+    Hd[np.arange(n), np.arange(n)] = rng.normal(size=n)
+    D = rng.normal(size=(n, n)) * (rng.uniform(size=(n, n)) < 0.15)      # not symmetric, some entries below tau
+    D[np.abs(D) < 0.05] *= 1e-3
+    tau = 1e-2
+    H, Dc = gi.CSR.from_dense(Hd), gi.CSR.from_dense(D)
+    rp, ci = o.update_graph(Dc.row_ptr, Dc.col_idx, Dc.val, H, tau)
+    M = (np.abs(D) >= tau) | (Hd != 0) | np.eye(n, dtype=bool)
+    want = np.zeros((n, n), dtype=bool)
+    for i in range(n):
+        for k in range(n):
+            if M[i, k]:
+                for j in range(n):
+                    if M[k, j]:
+                        want[i, j] = True
+    want |= want.T
+    got = np.zeros((n, n), dtype=bool)
+    for i in range(n):
+        got[i, ci[rp[i]:rp[i + 1]]] = True
+    assert np.array_equal(got, want)
+    assert (got & M).sum() == M.sum()          # S contains M (self loops make every edge a path of length two)
+    assert np.all(np.diff(ci[rp[3]:rp[4]]) > 0)
+
+
+def test_update_graph_follows_the_previous_density_matrix():
+    """S(t) 'cannot increase by more than paths of length two between two MD steps' - with H unchanged and the
+    previous D on the previous graph, every new edge is a path of length two of old edges and H edges; and a density
+    matrix computed on the updated graph is at least as accurate as on the old one (extra edges are harmless, obs. (iii))."""
+    s = gi.chain(128, 8, tau=1e-3, iters=30)
+    rp, ci = o.build_graph(s.H, s.tau)
+    r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, s.iters)
+    rp2, ci2 = o.update_graph(r.D_row_ptr, r.D_col, r.D_val, s.H, 1e-4)
+    n = s.n
+    old = sp.csr_matrix((np.ones(ci.size), ci, rp), shape=(n, n)).toarray() > 0
+    Dpat = sp.csr_matrix((np.ones(r.D_col.size), r.D_col, r.D_row_ptr), shape=(n, n)).toarray() > 0
+    new = sp.csr_matrix((np.ones(ci2.size), ci2, rp2), shape=(n, n)).toarray() > 0
+    reach = (Dpat | (s.H.to_dense() != 0) | np.eye(n, dtype=bool)).astype(int)
+    two = (reach @ reach) > 0
+    assert not (new & ~(two | two.T)).any()
+    r2 = o.o_sub(s.H, rp2, ci2, s.part, s.n_part, s.n_occ, s.iters)
+    exact = o.o_diag(s.H, int(s.n_occ))
+    def err(res):
+        D = sp.csr_matrix((res.D_val, res.D_col, res.D_row_ptr), shape=(n, n)).toarray()
+        mask = sp.csr_matrix((np.ones(res.D_col.size), res.D_col, res.D_row_ptr), shape=(n, n)).toarray() > 0
+        return np.abs((D - exact)[mask]).max()
+    assert err(r2) <= err(r) * 1.01
