@@ -137,6 +137,17 @@ def test_config4_reduced_peptide_heterogeneous_sizes(gbe):
     assert m.min() < 256 and m.max() > 1400
 
 
+@pytest.mark.parametrize("tau,n_part", [(1e-3, 256), (1e-3, 32), (1e-6, 128), (1e-7, 64)])
+def test_config5_sweep_points(gbe, tau, n_part):
+    """BASELINE.json configs[4] (tau x partition sweep), at the 1,024-molecule box the oracle finishes quickly: the
+    corners of the grid give core+halo sizes from ~35 (less than one tile) to ~1,600 (25 x 25 tiles)."""
+    s = gi.water_box(1024, n_part, seed=0, tau=tau, iters=16)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+
+
 def check_any_size_properties(s, g, ex, Dg, log):
     """Properties of the path that hold at any size (used where the oracle is too slow to run in full)."""
     t1, t2, br = log.t1, log.t2, log.branch
