@@ -153,13 +153,16 @@ int gbe_read_log(const gbe_graph* g, const void* workspace, size_t workspace_byt
 
 /* Same as gbe_density with HOST buffers: H (row_ptr, col_idx, val) and D_val are host pointers; the call
  * copies H to the device, runs the path, copies D back and synchronises the stream before returning.
+ * H_host == NULL: use the device copy of H that gbe_build_graph_host left with the graph (one upload for
+ * build + density of the same H); GBE_EINVAL if the graph was built from device pointers.
  * `workspace` stays a device buffer of info.workspace_bytes. */
 int gbe_density_host(const gbe_csr_view* H_host, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
                      void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val_host,
                      gbe_sp2_log* log);
 
 /* gbe_build_graph with HOST buffers: H (row_ptr, col_idx, val) and part (may be NULL) are host pointers; the call
- * copies them to the device, builds the graph and frees the staging copies before it returns. */
+ * copies them to the device and builds the graph.  The device copy of H stays with the graph (freed by
+ * gbe_free_graph) so that gbe_density_host(H_host = NULL) can reuse it. */
 int gbe_build_graph_host(const gbe_csr_view* H_host, const gbe_graph_opts* opts, const int32_t* part_host,
                          int32_t n_part, void* cuda_stream, gbe_graph** out);
 

@@ -326,17 +326,19 @@ def gbe_density_host(H_host, g: Graph, n_occ: float, iters: int, idem_tol: float
                      workspace: torch.Tensor | None = None, D_val_host: np.ndarray | None = None,
                      want_log: bool = False, stream=None):
     """H_host: object with numpy fields n, row_ptr (int64), col_idx (int32), val (float64) - HOST memory
-    (pinned or pageable).  Copies in, runs, copies D back, synchronises."""
+    (pinned or pageable).  Copies in, runs, copies D back, synchronises.  H_host=None reuses the device copy of H that
+    gbe_build_graph_host left with the graph."""
     if workspace is None:
         workspace = g.new_workspace()
     if D_val_host is None:
         D_val_host = np.empty(g.info["nnz_D"], dtype=np.float64)
-    rp = np.ascontiguousarray(H_host.row_ptr, dtype=np.int64)
-    ci = np.ascontiguousarray(H_host.col_idx, dtype=np.int32)
-    va = np.ascontiguousarray(H_host.val, dtype=np.float64)
-    v = _CsrView(int(H_host.n), int(ci.size), rp.ctypes.data, ci.ctypes.data, va.ctypes.data)
+    if H_host is not None:
+        rp = np.ascontiguousarray(H_host.row_ptr, dtype=np.int64)
+        ci = np.ascontiguousarray(H_host.col_idx, dtype=np.int32)
+        va = np.ascontiguousarray(H_host.val, dtype=np.float64)
+        v = _CsrView(int(H_host.n), int(ci.size), rp.ctypes.data, ci.ctypes.data, va.ctypes.data)
     clog, arrs = _new_log(iters) if want_log else (None, None)
-    _check(lib().gbe_density_host(C.byref(v), g.handle, float(n_occ), int(iters), float(idem_tol), _ptr(workspace),
+    _check(lib().gbe_density_host(C.byref(v) if H_host is not None else None, g.handle, float(n_occ), int(iters), float(idem_tol), _ptr(workspace),
                                   workspace.numel(), _stream(stream), D_val_host.ctypes.data,
                                   C.byref(clog) if want_log else None))
     return D_val_host, (_finish_log(clog, arrs) if want_log else None)

@@ -97,7 +97,7 @@ const char* gbe_strerror(int status) {
 void gbe_free_graph(gbe_graph* g) {
   if (!g) return;
   void* ptrs[] = {g->S_row_ptr, g->S_col,     g->sub_ptr,  g->sub_idx,  g->ncore,    g->msize, g->dense_off, g->D_row_ptr,
-                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->gitems, g->row_src, g->row_nc};
+                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   delete g;
@@ -384,27 +384,39 @@ int gbe_build_graph_host(const gbe_csr_view* Hh, const gbe_graph_opts* opts, con
   gbe_csr_view Hd{Hh->n, Hh->nnz, rp.as<int64_t>(), ci.as<int32_t>(), va.as<double>()};
   const int rc = gbe_build_graph(&Hd, opts, part_host ? pt.as<int32_t>() : nullptr, n_part, cuda_stream, out);
   cudaStreamSynchronize(s);  // the staging buffers are freed on return
+  if (rc == GBE_OK) {  // the device copy of H stays with the graph: gbe_density_host(H_host = NULL) reuses it
+    (*out)->H_n = Hh->n;
+    (*out)->H_nnz = Hh->nnz;
+    (*out)->H_rp = reinterpret_cast<int64_t*>(rp.release());
+    (*out)->H_ci = reinterpret_cast<int32_t*>(ci.release());
+    (*out)->H_va = reinterpret_cast<double*>(va.release());
+  }
   return rc;
 }
 
 int gbe_density_host(const gbe_csr_view* Hh, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
                      void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val_host, gbe_sp2_log* log) {
   if (!g || (!D_val_host && g->nnz_D > 0)) return GBE_EINVAL;
-  GBE_TRY(check_csr(Hh));
-  if (Hh->n != g->n) return GBE_EMISMATCH;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   gbe_set_alloc_stream(s);
   DevBuf rp, ci, va, dv;
-  GBE_TRY(rp.alloc((size_t)(Hh->n + 1) * 8));
-  GBE_TRY(ci.alloc((size_t)Hh->nnz * 4));
-  GBE_TRY(va.alloc((size_t)Hh->nnz * 8));
   GBE_TRY(dv.alloc((size_t)g->nnz_D * 8));
-  GBE_CUDA(cudaMemcpyAsync(rp.p, Hh->row_ptr, (size_t)(Hh->n + 1) * 8, cudaMemcpyHostToDevice, s));
-  if (Hh->nnz) {
-    GBE_CUDA(cudaMemcpyAsync(ci.p, Hh->col_idx, (size_t)Hh->nnz * 4, cudaMemcpyHostToDevice, s));
-    GBE_CUDA(cudaMemcpyAsync(va.p, Hh->val, (size_t)Hh->nnz * 8, cudaMemcpyHostToDevice, s));
+  gbe_csr_view Hd{g->H_n, g->H_nnz, g->H_rp, g->H_ci, g->H_va};
+  if (Hh) {
+    GBE_TRY(check_csr(Hh));
+    if (Hh->n != g->n) return GBE_EMISMATCH;
+    GBE_TRY(rp.alloc((size_t)(Hh->n + 1) * 8));
+    GBE_TRY(ci.alloc((size_t)Hh->nnz * 4));
+    GBE_TRY(va.alloc((size_t)Hh->nnz * 8));
+    GBE_CUDA(cudaMemcpyAsync(rp.p, Hh->row_ptr, (size_t)(Hh->n + 1) * 8, cudaMemcpyHostToDevice, s));
+    if (Hh->nnz) {
+      GBE_CUDA(cudaMemcpyAsync(ci.p, Hh->col_idx, (size_t)Hh->nnz * 4, cudaMemcpyHostToDevice, s));
+      GBE_CUDA(cudaMemcpyAsync(va.p, Hh->val, (size_t)Hh->nnz * 8, cudaMemcpyHostToDevice, s));
+    }
+    Hd = gbe_csr_view{Hh->n, Hh->nnz, rp.as<int64_t>(), ci.as<int32_t>(), va.as<double>()};
+  } else if (!g->H_rp) {
+    return GBE_EINVAL;  // no H given and the graph was not built by gbe_build_graph_host
   }
-  gbe_csr_view Hd{Hh->n, Hh->nnz, rp.as<int64_t>(), ci.as<int32_t>(), va.as<double>()};
   int rc = gbe_density(&Hd, g, n_occ, iters, idem_tol, workspace, workspace_bytes, cuda_stream, dv.as<double>(), log);
   if (rc == GBE_OK && g->nnz_D) {
     cudaError_t e = cudaMemcpyAsync(D_val_host, dv.p, (size_t)g->nnz_D * 8, cudaMemcpyDeviceToHost, s);

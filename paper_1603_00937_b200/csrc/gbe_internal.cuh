@@ -113,6 +113,11 @@ struct gbe_graph {
   int32_t n_items = 0;
   int2* gitems = nullptr;  // gather work items (p, first row)
   int32_t n_gitems = 0, gather_rows = 0;
+  // device copy of the H uploaded by gbe_build_graph_host (owned; null for graphs built from device pointers)
+  int64_t H_n = 0, H_nnz = 0;
+  int64_t* H_rp = nullptr;
+  int32_t* H_ci = nullptr;
+  double* H_va = nullptr;
   // workspace layout (byte offsets)
   size_t ws_partials = 0, ws_bounds = 0, ws_x0 = 0, ws_x1 = 0, ws_bytes = 0;
   int32_t n_partials = 0;

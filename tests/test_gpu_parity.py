@@ -390,6 +390,11 @@ def test_density_host_and_phase_calls(gbe):
     ws = g.new_workspace()
     D1, log1 = gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws)
     Dh, logh = gbe.gbe_density_host(s.H, g, s.n_occ, s.iters, workspace=ws, want_log=True)
+    with pytest.raises(gbe.GbeError):
+        gbe.gbe_density_host(None, g, s.n_occ, s.iters, workspace=ws)  # no H was left with a device-built graph
+    gh = gbe.gbe_build_graph_host(s.H, s.tau, None, s.n_part)
+    Dh2, _ = gbe.gbe_density_host(None, gh, s.n_occ, s.iters)           # one upload for build + density
+    assert np.array_equal(Dh, Dh2)
     D3 = torch.empty_like(D1)
     gbe.gbe_gather(Hd, g, ws)
     gbe.gbe_sp2(g, s.n_occ, s.iters, -1.0, ws)
