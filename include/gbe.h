@@ -83,6 +83,7 @@ typedef struct {
   int32_t contiguous_cores;  /* 1: every core is a contiguous index range (fast scatter); 0: per-entry map */
   int32_t tile;              /* edge of the square X^2 tile chosen for this graph */
   size_t workspace_bytes;    /* device workspace gbe_density needs (two dense buffers + state + partials) */
+  size_t workspace_bytes_fermi; /* device workspace gbe_density_fermi needs (four dense buffers + state + partials) */
 } gbe_graph_info;
 
 /* SP2 log (host memory, caller-allocated; valid after the stream has been synchronised).
@@ -195,6 +196,19 @@ int gbe_density_timed(const gbe_csr_view* H, const gbe_graph* g, double n_occ, i
 int gbe_density_preset(const gbe_csr_view* H, const gbe_graph* g, const uint8_t* branch, int32_t iters,
                        int32_t trace_every_iteration, void* workspace, size_t workspace_bytes, void* cuda_stream,
                        double* D_val, gbe_sp2_log* log);
+
+/* Finite-temperature density matrix by the Chebyshev Fermi-operator expansion, Eq.(7) P:L67-72:
+ *     D = [e^{beta (H - mu)} + 1]^{-1}  ~  sum_{n=0}^{order} c_n T_n((H - b)/a)
+ * evaluated per community on x[s_p] (Eq.(6)) with the three-term recurrence T_{n+1} = 2 Ht T_n - T_{n-1}
+ * (Eq.(5)), one dense product per term; a, b from the Gershgorin bounds of H, c_n by Chebyshev-Gauss
+ * quadrature of the Fermi function (2048 nodes), all on the device.  Gather and scatter as gbe_density.
+ *   mu, beta   chemical potential and inverse temperature, in the units of H (beta > 0).
+ *   order      highest Chebyshev order, 1 <= order <= GBE_MAX_ITERS.
+ *   workspace  >= info.workspace_bytes_fermi.
+ *   n_elec     optional HOST double: sum over all core diagonals of D (the occupation); if given, the call
+ *              synchronises the stream, otherwise it only enqueues. */
+int gbe_density_fermi(const gbe_csr_view* H, const gbe_graph* g, double mu, double beta, int32_t order, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream, double* D_val, double* n_elec);
 
 /* Expectation value <A> = Tr[D A] = sum_{k,i} D_ki A_ik; with A = H the band energy E_band = Tr[DH].
  *   D_val  device double[nnz_D]: the values gbe_density wrote, on the pattern of `g`.

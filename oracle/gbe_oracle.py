@@ -256,6 +256,69 @@ def o_sub(H, S_row_ptr, S_col, part, n_part: int, n_occ: float, iters: int, idem
 
 
 # ----------------------------------------------------------------------------------------
+# finite-temperature expansion, Eq.(7)
+# ----------------------------------------------------------------------------------------
+def fermi_chebyshev_coeffs(mu: float, beta: float, order: int, eps_min: float, eps_max: float, nq: int = 2048) -> np.ndarray:
+    """c_0..c_order of f(x) = 1/(1 + exp(beta (a x + b - mu))) on x in [-1, 1], a = (eps_max - eps_min)/2,
+    b = (eps_max + eps_min)/2, by Chebyshev-Gauss quadrature with nq nodes:
+        c_n = (2 - delta_n0)/nq * sum_k f(cos th_k) cos(n th_k),  th_k = pi (k + 1/2)/nq.
+    (Eq.(7) P:L67-72: 'the Fermi-operator expansion ... Chebyshev'.)"""
+    a, b = 0.5 * (eps_max - eps_min), 0.5 * (eps_max + eps_min)
+    th = np.pi * (np.arange(nq) + 0.5) / nq
+    arg = beta * (a * np.cos(th) + b - mu)
+    f = np.where(arg > 0, np.exp(-np.abs(arg)) / (1.0 + np.exp(-np.abs(arg))), 1.0 / (1.0 + np.exp(-np.abs(arg))))
+    n = np.arange(order + 1)
+    c = (np.cos(np.outer(n, th)) @ f) * (2.0 / nq)
+    c[0] *= 0.5
+    return c
+
+
+@dataclass
+class FermiResult:
+    D_row_ptr: np.ndarray
+    D_col: np.ndarray
+    D_val: np.ndarray
+    n_elec: float      # sum over all core diagonals
+    coeffs: np.ndarray
+    eps_min: float
+    eps_max: float
+    subs: list
+
+
+def o_fermi(H, S_row_ptr, S_col, part, n_part: int, mu: float, beta: float, order: int,
+            bounds: tuple[float, float] | None = None) -> FermiResult:
+    """The partitioned subgraph expansion (Eq.(6)) of the finite-temperature Fermi operator (Eq.(7)):
+      1. Gershgorin bounds of the global H (A-5); Ht = (H - b)/a with spectrum in [-1, 1]
+      2. per community: xt = Ht[s_p, s_p] (full principal submatrix, A-2); T_0 = I, T_1 = xt,
+         T_{n+1} = 2 xt T_n - T_{n-1} (Eq.(5) P:L51-56 with the Chebyshev alpha_n);  D_p = sum_{n<=order} c_n T_n
+      3. core columns of D_p assembled as in o_sub."""
+    lo, hi = bounds if bounds is not None else gershgorin(H)
+    a, b = 0.5 * (hi - lo), 0.5 * (hi + lo)
+    c = fermi_chebyshev_coeffs(mu, beta, order, lo, hi)
+    subs = subgraphs(S_row_ptr, S_col, part, n_part)
+    Hs = sp.csr_matrix((H.val, H.col_idx, H.row_ptr), shape=(H.n, H.n))
+    blocks, n_elec = [], 0.0
+    for idx, nc in subs:
+        m = len(idx)
+        xt = (Hs[idx][:, idx].toarray() - b * np.eye(m)) / a
+        Tm, Tn = np.eye(m), xt.copy()
+        D = c[0] * Tm + c[1] * Tn
+        for n in range(1, order):
+            Tm, Tn = Tn, 2.0 * (xt @ Tn) - Tm
+            D = D + c[n + 1] * Tn
+        blocks.append(D)
+        n_elec += float(np.diagonal(D)[:nc].sum())
+    rp, ci = density_pattern(subs, H.n)
+    rows = np.concatenate([np.repeat(idx, nc) for idx, nc in subs]) if subs else np.zeros(0, int)
+    cols = np.concatenate([np.tile(idx[:nc], idx.size) for idx, nc in subs]) if subs else np.zeros(0, int)
+    vals = np.concatenate([x[:, :nc].reshape(-1) for x, (idx, nc) in zip(blocks, subs)]) if subs else np.zeros(0)
+    Dm = sp.csr_matrix((np.arange(1, rows.size + 1, dtype=np.float64), (rows, cols)), shape=(H.n, H.n))
+    Dm.sort_indices()
+    order_ = Dm.data.astype(np.int64) - 1
+    return FermiResult(rp, ci, vals[order_], n_elec, c, lo, hi, subs)
+
+
+# ----------------------------------------------------------------------------------------
 # observables
 # ----------------------------------------------------------------------------------------
 def expectation(D_row_ptr, D_col, D_val, A, n: int | None = None) -> float:

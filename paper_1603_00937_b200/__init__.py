@@ -21,6 +21,7 @@ from .binding import (  # noqa: F401
     gbe_update_graph,
     gbe_density_timed,
     gbe_density_preset,
+    gbe_density_fermi,
     gbe_expectation,
     gbe_launch_count,
     gbe_graph_export,

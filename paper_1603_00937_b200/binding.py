@@ -19,7 +19,7 @@ GBE_MAX_ITERS = 1024
 EXPORTS = [
     "gbe_build_graph", "gbe_graph_get_info", "gbe_graph_export", "gbe_density", "gbe_gather", "gbe_sp2",
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
-    "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation", "gbe_update_graph",
+    "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation", "gbe_update_graph", "gbe_density_fermi",
 ]
 
 
@@ -43,7 +43,8 @@ class _GraphInfo(C.Structure):
                 ("max_m", C.c_int64), ("nnz_D", C.c_int64), ("dense_elems", C.c_int64), ("n_tiles", C.c_int64),
                 ("sp2_flops_per_iter", C.c_double), ("sp2_exec_flops_per_iter", C.c_double),
                 ("eps_min", C.c_double), ("eps_max", C.c_double),
-                ("contiguous_cores", C.c_int32), ("tile", C.c_int32), ("workspace_bytes", C.c_size_t)]
+                ("contiguous_cores", C.c_int32), ("tile", C.c_int32), ("workspace_bytes", C.c_size_t),
+                ("workspace_bytes_fermi", C.c_size_t)]
 
 
 class _Sp2Log(C.Structure):
@@ -85,6 +86,8 @@ def lib() -> C.CDLL:
         l.gbe_build_graph_host.argtypes = l.gbe_build_graph.argtypes
         l.gbe_density_preset.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p,
                                          C.c_size_t, C.c_void_p, C.c_void_p, C.POINTER(_Sp2Log)]
+        l.gbe_density_fermi.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_double, C.c_double, C.c_int32, C.c_void_p,
+                                        C.c_size_t, C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]
         l.gbe_expectation.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CsrView), C.c_void_p, C.POINTER(C.c_double)]
         l.gbe_launch_count.restype = C.c_uint64
         l.gbe_launch_count.argtypes = []
@@ -291,6 +294,20 @@ def gbe_density_preset(H: DeviceCSR, g: Graph, branch, trace_every_iteration: bo
                                     int(bool(trace_every_iteration)), _ptr(workspace), workspace.numel(), _stream(stream),
                                     _ptr(D_val), C.byref(clog) if want_log else None))
     return D_val, (_finish_log(clog, arrs) if want_log else None)
+
+
+def gbe_density_fermi(H: DeviceCSR, g: Graph, mu: float, beta: float, order: int, workspace: torch.Tensor | None = None,
+                      D_val: torch.Tensor | None = None, want_n_elec: bool = True, stream=None):
+    """Finite-temperature D by the Chebyshev Fermi-operator expansion (Eq.(7)).  Returns (D_val, n_elec | None)."""
+    if workspace is None:
+        workspace = torch.empty(g.info["workspace_bytes_fermi"], dtype=torch.uint8, device="cuda")
+    if D_val is None:
+        D_val = torch.empty(g.info["nnz_D"], dtype=torch.float64, device="cuda")
+    v = H.view()
+    ne = C.c_double(0.0)
+    _check(lib().gbe_density_fermi(C.byref(v), g.handle, float(mu), float(beta), int(order), _ptr(workspace),
+                                   workspace.numel(), _stream(stream), _ptr(D_val), C.byref(ne) if want_n_elec else None))
+    return D_val, (float(ne.value) if want_n_elec else None)
 
 
 def gbe_expectation(g: Graph, D_val: torch.Tensor, A: DeviceCSR, stream=None) -> float:

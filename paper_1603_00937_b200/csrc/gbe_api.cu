@@ -183,6 +183,7 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   o->contiguous_cores = g->contiguous;
   o->tile = g->tile;
   o->workspace_bytes = g->ws_bytes;
+  o->workspace_bytes_fermi = g->ws_bytes_fermi;
   return GBE_OK;
 }
 
@@ -341,6 +342,36 @@ int gbe_density_preset(const gbe_csr_view* H, const gbe_graph* g, const uint8_t*
                  trace_every_iteration != 0));
   GBE_TRY(do_scatter(g, workspace, workspace_bytes, cuda_stream, D_val, nullptr));
   if (log) GBE_TRY(gbe_read_log(g, workspace, workspace_bytes, cuda_stream, log));
+  return GBE_OK;
+}
+
+int gbe_density_fermi(const gbe_csr_view* H, const gbe_graph* g, double mu, double beta, int32_t order, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream, double* D_val, double* n_elec) {
+  if (!g || (!D_val && g->nnz_D > 0)) return GBE_EINVAL;
+  if (!(beta > 0.0) || std::isnan(mu) || order < 1 || order > GBE_MAX_ITERS) return GBE_EINVAL;
+  if (workspace_bytes < g->ws_bytes_fermi) return GBE_ENOMEM;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  GBE_TRY(do_gather(H, g, workspace, workspace_bytes, cuda_stream, nullptr));  // bounds + X0 into the first buffer
+  WS w;
+  GBE_TRY(carve(g, workspace, workspace_bytes, &w));
+  unsigned char* base = static_cast<unsigned char*>(workspace);
+  double* BX = w.X0;
+  double* Ta = w.X1;                                             // T_0, then T_2, T_4, ...
+  double* Tb = reinterpret_cast<double*>(base + g->ws_x2);       // T_1, then T_3, ...
+  double* BD = reinterpret_cast<double*>(base + g->ws_x3);
+  GBE_TRY(gbe_launch_cheb_coef(w.st, mu, beta, order, s));
+  GBE_TRY(gbe_launch_cheb_init(g, w.st, BX, Ta, Tb, BD, s));
+  for (int n = 1; n < order; ++n) {  // T_{n+1} from T_n (B operand) and T_{n-1} (overwritten), coefficient c_{n+1}
+    const double* Tn = (n & 1) ? Tb : Ta;
+    double* Tio = (n & 1) ? Ta : Tb;
+    GBE_TRY(gbe_launch_cheb_step(g, w.st, BX, Tn, Tio, BD, w.st->t1, n + 1, w.partials, s));
+  }
+  GBE_TRY(gbe_launch_core_trace(g, BD, w.st, s));
+  GBE_TRY(gbe_launch_scatter(g, w.st, BD, BD, D_val, s));
+  if (n_elec) {
+    GBE_CUDA(cudaMemcpyAsync(n_elec, &w.st->t2[0], 8, cudaMemcpyDeviceToHost, s));
+    GBE_CUDA(cudaStreamSynchronize(s));
+  }
   return GBE_OK;
 }
 

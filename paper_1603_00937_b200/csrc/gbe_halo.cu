@@ -326,6 +326,11 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   g->ws_x1 = off;
   off += align_up((size_t)g->dense_elems * 8, 256);
   g->ws_bytes = off;
+  g->ws_x2 = off;
+  off += align_up((size_t)g->dense_elems * 8, 256);
+  g->ws_x3 = off;
+  off += align_up((size_t)g->dense_elems * 8, 256);
+  g->ws_bytes_fermi = off;
   // ---- fill sub_idx / row_part
   GBE_TRY(gbe_dev_alloc((void**)&g->sub_idx, std::max<size_t>(16, (size_t)g->sum_m * 4)));
   GBE_TRY(gbe_dev_alloc((void**)&g->row_part, std::max<size_t>(16, (size_t)g->sum_m * 4)));

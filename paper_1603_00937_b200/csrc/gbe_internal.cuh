@@ -120,6 +120,7 @@ struct gbe_graph {
   double* H_va = nullptr;
   // workspace layout (byte offsets)
   size_t ws_partials = 0, ws_bounds = 0, ws_x0 = 0, ws_x1 = 0, ws_bytes = 0;
+  size_t ws_x2 = 0, ws_x3 = 0, ws_bytes_fermi = 0;  // two more dense buffers for the Chebyshev recurrence
   int32_t n_partials = 0;
   // host mirrors
   std::vector<int32_t> h_m, h_ncore;
@@ -153,6 +154,13 @@ int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partial
 int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0, const double* X1, double* D_val,
                        cudaStream_t s);
 
+// finite-temperature Chebyshev expansion (gbe_fermi.cu; the product of every term is gbe_x2.cu in its second mode)
+int gbe_launch_cheb_coef(gbe_state* st, double mu, double beta, int order, cudaStream_t s);
+int gbe_launch_cheb_init(const gbe_graph* g, const gbe_state* st, double* BX, double* B0, double* B1, double* BD,
+                         cudaStream_t s);
+int gbe_launch_cheb_step(const gbe_graph* g, gbe_state* st, const double* Xt, const double* Tn, double* Tio, double* Dacc,
+                         const double* coef, int iter, double* partials, cudaStream_t s);
+int gbe_launch_core_trace(const gbe_graph* g, const double* BD, gbe_state* st, cudaStream_t s);
 // observables (gbe_observe.cu)
 int gbe_launch_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view& A, double* row_sum, double* out,
                            cudaStream_t s);

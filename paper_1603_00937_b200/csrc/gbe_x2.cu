@@ -97,15 +97,24 @@ __device__ __forceinline__ void x2_chunk(double (&acc)[2][8][2], const double* _
   }
 }
 
-template <int MINB>
+// OP 0: one SP2 iteration, Y = X X^T then X' = Y or 2X - Y (Xin -> Xout).
+// OP 1: one step of the Chebyshev recurrence of the finite-temperature expansion (Eq.(7); Eq.(5) P:L51-56 with
+//       its alpha_n): T_{n+1} = 2 Xt T_n - T_{n-1}, D += c_{n+1} T_{n+1}.  Xin = Xt (A operand), Xb = T_n (B operand),
+//       Xout holds T_{n-1} on entry and T_{n+1} on exit (every element is read and written by the same thread), Dacc
+//       the running sum, coef[iter] = c_{n+1}.  Xt and T_n are symmetric and commute, so the product is symmetric and
+//       the same upper-triangle / mirrored-store scheme applies; only the B panel now comes from another matrix.
+template <int MINB, int OP>
 __global__ void __launch_bounds__(X2_THREADS, MINB)
-    k_x2(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin, double* __restrict__ Xout,
-         double* __restrict__ partials, int iter) {
+    k_x2(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin,
+         double* __restrict__ Xout, double* __restrict__ partials, int iter, const double* __restrict__ Xb,
+         double* __restrict__ Dacc, const double* __restrict__ coef) {
   extern __shared__ __align__(16) double smem[];  // 2 stages x (A panel, B panel)
   __shared__ double red[8];
 
-  if (st->stop) return;  // idempotency stop already fired (A-7): X is final
-  const int branch = st->preset ? (int)st->br[iter] : st->branch;  // preset sequence or the on-device choice
+  if (OP == 0 && st->stop) return;  // idempotency stop already fired (A-7): X is final
+  // preset sequence or the on-device choice
+  const int branch = OP == 0 ? (st->preset ? (int)st->br[iter] : st->branch) : 0;
+  const double cn = OP == 1 ? coef[iter] : 0.0;
 
   const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // p, ti, tj, m
   const int4 it1 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x + 1];  // nc, ld, dense_off
@@ -113,7 +122,10 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   const int64_t doff = ((int64_t)(uint32_t)it1.z) | ((int64_t)it1.w << 32);
   const double* __restrict__ X = Xin + doff;
   double* __restrict__ Y = Xout + doff;
+  const double* __restrict__ XB = OP == 1 ? Xb + doff : X;  // rows of the B operand
+  double* __restrict__ DA = OP == 1 ? Dacc + doff : nullptr;
   const bool diag = (ti == tj);
+  const bool share = diag && OP == 0;  // X X^T on a diagonal tile: the B panel is the A panel
   const int row0 = ti * X2_BT, col0 = tj * X2_BT;
   const int nchunks = ld / X2_KC;
 
@@ -141,7 +153,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   for (int u = 0; u < 4; ++u) {
     const int r = (t >> 3) + 16 * u;
     gA[u] = X + (size_t)min(row0 + r, m - 1) * ld + (t & 7) * 2;
-    gB[u] = X + (size_t)min(col0 + r, m - 1) * ld + (t & 7) * 2;
+    gB[u] = XB + (size_t)min(col0 + r, m - 1) * ld + (t & 7) * 2;
   }
   double* const sdst = smem + (t >> 3) * X2_STRIDE + (t & 7) * 2;  // slot 0 of the A panel of stage 0
 
@@ -149,7 +161,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
 #pragma unroll
     for (int u = 0; u < 4; ++u)
       cp_async16(sdst + stage * X2_STAGE + u * 16 * X2_STRIDE, gA[u] + kofs);
-    if (!diag) {
+    if (!share) {
 #pragma unroll
       for (int u = 0; u < 4; ++u)
         cp_async16(sdst + stage * X2_STAGE + X2_PANEL + u * 16 * X2_STRIDE, gB[u] + kofs);
@@ -165,7 +177,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
 
   const double* const pa0 = smem + (rblk[0] * 8 + g) * X2_STRIDE + q;
   const double* const pa1 = smem + (rblk[1] * 8 + g) * X2_STRIDE + q;
-  const double* const pb0 = smem + (diag ? 0 : X2_PANEL) + g * X2_STRIDE + q;
+  const double* const pb0 = smem + (share ? 0 : X2_PANEL) + g * X2_STRIDE + q;
   // warp-uniform code path: 0 full, 1..4 the diagonal pattern of role 0..3, 5..11 the first 1..7 column blocks of
   // both row blocks (ragged right edge), 12 run-time mask (the last diagonal tile), 13 idle
   int pattern = active ? 12 : 13;
@@ -228,16 +240,24 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
       double* __restrict__ ym0 = Y + (size_t)(col0 + 2 * q) * ld + r;  // mirrored position (c, r) of column block 0
       double* __restrict__ ym1 = ym0 + ld;                            // and (c + 1, r); both advance by 8 rows per j
       const size_t mstep = (size_t)8 * ld;
+      double* __restrict__ dr = OP == 1 ? DA + (size_t)r * ld + col0 + 2 * q : nullptr;
+      double* __restrict__ dm0 = OP == 1 ? DA + (size_t)(col0 + 2 * q) * ld + r : nullptr;
+      double* __restrict__ dm1 = dm0 + ld;
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         if (!FULL && !(active & (1u << (i * 8 + j)))) {  // c < ld holds for every active sub-tile
           ym0 += mstep;
           ym1 += mstep;
+          if (OP == 1) { dm0 += mstep; dm1 += mstep; }
           continue;
         }
         const int c = col0 + j * 8 + 2 * q;
         double v0 = acc[i][j][0], v1 = acc[i][j][1];
-        if (branch) {
+        if (OP == 1) {  // T_{n+1} = 2 (Xt T_n) - T_{n-1}; T_{n-1} sits where T_{n+1} goes
+          const double2 told = *reinterpret_cast<const double2*>(yr + j * 8);
+          v0 = 2.0 * v0 - told.x;
+          v1 = 2.0 * v1 - told.y;
+        } else if (branch) {
           const double2 x = *reinterpret_cast<const double2*>(xr + j * 8);
           v0 = 2.0 * x.x - v0;
           v1 = 2.0 * x.y - v1;
@@ -247,6 +267,12 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
           if (c + 1 >= m) v1 = 0.0;
         }
         *reinterpret_cast<double2*>(yr + j * 8) = make_double2(v0, v1);
+        if (OP == 1) {  // D += c_{n+1} T_{n+1}
+          double2 d = *reinterpret_cast<const double2*>(dr + j * 8);
+          d.x = fma(cn, v0, d.x);
+          d.y = fma(cn, v1, d.y);
+          *reinterpret_cast<double2*>(dr + j * 8) = d;
+        }
         if (TRACE && r < nc) {
           s2 += v0 * v0 + v1 * v1;
           if (r == c) s1 += v0;
@@ -255,20 +281,23 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
         if (FULL || (mirror & (1u << (i * 8 + j)))) {
           if (!EDGE || c < m) {
             *ym0 = v0;
+            if (OP == 1) *dm0 = fma(cn, v0, *dm0);
             if (TRACE && c < nc) s2 += v0 * v0;
           }
           if (!EDGE || c + 1 < m) {
             *ym1 = v1;
+            if (OP == 1) *dm1 = fma(cn, v1, *dm1);
             if (TRACE && c + 1 < nc) s2 += v1 * v1;
           }
         }
         ym0 += mstep;
         ym1 += mstep;
+        if (OP == 1) { dm0 += mstep; dm1 += mstep; }
       }
     }
   };
   const bool edge = col0 + X2_BT > m;             // row0 <= col0: the row edge implies the column edge
-  const bool trace = row0 < nc || col0 < nc;      // a core row, directly or through the mirror
+  const bool trace = OP == 0 && (row0 < nc || col0 < nc);  // a core row, directly or through the mirror
   if (edge || trace) {
     if (edge) epilogue(std::true_type{}, std::true_type{}, std::false_type{});
     else epilogue(std::false_type{}, std::true_type{}, std::false_type{});
@@ -287,10 +316,10 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   }
 }
 
-template <int MINB>
+template <int MINB, int OP>
 int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-              cudaStream_t s) {
-  auto kern = k_x2<MINB>;
+              const double* Xb, double* Dacc, const double* coef, cudaStream_t s) {
+  auto kern = k_x2<MINB, OP>;
   const size_t smem = (size_t)2 * X2_STAGE * sizeof(double);
   static bool configured = false;
   if (!configured) {
@@ -298,7 +327,7 @@ int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout
     GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     configured = true;
   }
-  kern<<<g->n_items, X2_THREADS, smem, s>>>(g->items, st, Xin, Xout, partials, iter);
+  kern<<<g->n_items, X2_THREADS, smem, s>>>(g->items, st, Xin, Xout, partials, iter, Xb, Dacc, coef);
   GBE_LAUNCHED();
   return GBE_OK;
 }
@@ -307,5 +336,11 @@ int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
                   cudaStream_t s) {
   if (g->n_items == 0) return GBE_OK;
-  return launch_x2<4>(g, st, Xin, Xout, partials, iter, s);
+  return launch_x2<4, 0>(g, st, Xin, Xout, partials, iter, nullptr, nullptr, nullptr, s);
+}
+
+int gbe_launch_cheb_step(const gbe_graph* g, gbe_state* st, const double* Xt, const double* Tn, double* Tio, double* Dacc,
+                         const double* coef, int iter, double* partials, cudaStream_t s) {
+  if (g->n_items == 0) return GBE_OK;
+  return launch_x2<4, 1>(g, st, Xt, Tio, partials, iter, Tn, Dacc, coef, s);
 }

@@ -303,6 +303,45 @@ def test_update_graph_eq8_md_step(gbe, which):
     assert g1.info["nnz_S"] >= ex0["S_col"].size or which == "water"
 
 
+# ------------------------------------------------------------------------------- Eq.(7): finite-temperature expansion
+def run_fermi(gbe, s, mu, beta, order):
+    import torch
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    part_t = torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
+    g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
+    D, ne = gbe.gbe_density_fermi(Hd, g, mu, beta, order)
+    torch.cuda.synchronize()
+    ex = {k: v.cpu().numpy() for k, v in g.export().items()}
+    rp, ci = o.build_graph(s.H, s.tau)
+    r = o.o_fermi(s.H, rp, ci, s.part, s.n_part, mu, beta, order)
+    assert np.array_equal(ex["D_row_ptr"], r.D_row_ptr) and np.array_equal(ex["D_col"], r.D_col)
+    return g, D.cpu().numpy(), ne, r
+
+
+@pytest.mark.parametrize("order", [1, 2, 7, 64])
+def test_fermi_chebyshev_chain(gbe, order):
+    """Eq.(7) P:L67-72 on config 1's chain (16 communities of 40-48 orbitals, less than one tile each), odd and even
+    orders (the recurrence ping-pongs two buffers) and the shortest series."""
+    s = gi.config(1)
+    g, Dg, ne, r = run_fermi(gbe, s, 0.3, 2.0, order)
+    assert np.abs(Dg - r.D_val).max() <= TOL_D
+    assert abs(ne - r.n_elec) <= TOL_TR
+
+
+def test_fermi_chebyshev_water_and_shuffled(gbe):
+    """Several tiles with ragged tails (6,144-orbital water box, order 60) and non-contiguous communities."""
+    s = gi.config(2)
+    w_mid = -11.0  # inside the O-p / H-s manifold of the synthetic water model
+    g, Dg, ne, r = run_fermi(gbe, s, w_mid, 0.8, 60)
+    assert np.abs(Dg - r.D_val).max() <= TOL_D
+    assert abs(ne - r.n_elec) <= 1e-7
+    s2 = gi.random_banded(200, half_bw=5, n_part=7, seed=1, tau=1e-4, shuffle=True)
+    g, Dg, ne, r = run_fermi(gbe, s2, 0.0, 1.5, 33)
+    assert np.abs(Dg - r.D_val).max() <= TOL_D and abs(ne - r.n_elec) <= TOL_TR
+    with pytest.raises(gbe.GbeError):
+        gbe.gbe_density_fermi(gbe.DeviceCSR.from_host(s2.H), g, 0.0, -1.0, 10)
+
+
 # ------------------------------------------------------------------------------- observables (P:L72, P:L76)
 def test_band_energy_and_expectation_values(gbe):
     import torch

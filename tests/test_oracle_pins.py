@@ -462,3 +462,47 @@ def test_update_graph_follows_the_previous_density_matrix():
         mask = sp.csr_matrix((np.ones(res.D_col.size), res.D_col, res.D_row_ptr), shape=(n, n)).toarray() > 0
         return np.abs((D - exact)[mask]).max()
     assert err(r2) <= err(r) * 1.01
+
+
+# ------------------------------------------------------------------------------- Eq.(7): finite-temperature expansion
+def test_fermi_coefficients_reproduce_the_fermi_function():
+    """Closed form: sum_n c_n T_n(x) -> f(x) pointwise; the coefficients of a smooth f decay geometrically, so with
+    order 400 at beta*a = 20 the series equals the Fermi function to 1e-12 on a grid of x (numpy's chebval)."""
+    lo, hi, mu, beta = -3.0, 5.0, 0.4, 5.0
+    c = o.fermi_chebyshev_coeffs(mu, beta, 400, lo, hi)
+    x = np.linspace(-1, 1, 201)
+    a, b = 0.5 * (hi - lo), 0.5 * (hi + lo)
+    f = 1.0 / (1.0 + np.exp(beta * (a * x + b - mu)))
+    assert np.abs(np.polynomial.chebyshev.chebval(x, c) - f).max() < 1e-12
+    assert abs(c[0] - np.mean(1.0 / (1.0 + np.exp(beta * (a * np.cos(np.pi * (np.arange(4096) + 0.5) / 4096) + b - mu))))) < 1e-13
+
+
+def test_o_fermi_one_partition_equals_the_fermi_function_of_the_eigenvalues():
+    """Library special case: one partition => D = V f(eps) V^T from the dense eigendecomposition, to within the
+    truncation bound sum_{n > order} |c_n| of the Chebyshev series (plus roundoff)."""
+    s = gi.random_banded(72, half_bw=5, n_part=1, seed=4)
+    mu, beta, order = 0.1, 3.0, 120
+    rp, ci = o.build_graph(s.H, 0.0)
+    r = o.o_fermi(s.H, rp, ci, s.part, 1, mu, beta, order)
+    w, v = np.linalg.eigh(s.H.to_dense())
+    exact = (v * (1.0 / (1.0 + np.exp(beta * (w - mu))))) @ v.T
+    D = sp.csr_matrix((r.D_val, r.D_col, r.D_row_ptr), shape=(s.n, s.n)).toarray()
+    tail = np.abs(o.fermi_chebyshev_coeffs(mu, beta, 600, r.eps_min, r.eps_max)[order + 1:]).sum()
+    assert tail < 1e-6
+    assert np.linalg.norm(D - exact, 2) <= tail + 1e-12
+    assert abs(r.n_elec - (1.0 / (1.0 + np.exp(beta * (w - mu)))).sum()) <= s.n * (tail + 1e-12)
+    assert np.abs(D - D.T).max() < 1e-13
+
+
+def test_o_fermi_reaches_the_zero_temperature_projector_and_respects_the_graph():
+    """beta -> large with mu in the gap: the Fermi operator tends to theta(mu - H), so the partitioned
+    finite-temperature result approaches the partitioned SP2 result; and P_tau is zero outside S' (obs. (iv))."""
+    s = gi.chain(96, 6, tau=1e-3, iters=30)
+    rp, ci = o.build_graph(s.H, s.tau)
+    rs = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, s.iters)
+    w = np.linalg.eigvalsh(s.H.to_dense())
+    mu = 0.5 * (w[47] + w[48])
+    rf = o.o_fermi(s.H, rp, ci, s.part, s.n_part, mu, 40.0, 600)
+    assert np.array_equal(rf.D_row_ptr, rs.D_row_ptr) and np.array_equal(rf.D_col, rs.D_col)
+    assert np.abs(rf.D_val - rs.D_val).max() < 1e-6
+    assert abs(rf.n_elec - rs.t1[-1]) < 1e-5
