@@ -439,6 +439,34 @@ def run_sweep(args) -> None:
                         f"{r['trace_minus_nocc']:.3g} |\n")
 
 
+def run_fermi(args) -> None:
+    """the finite-temperature Chebyshev expansion (Eq.(7)) on the bench workload, one JSON line."""
+    import torch
+    from paper_1603_00937_b200 import build as gbe_build
+    gbe_build.build()
+    import paper_1603_00937_b200 as gbe
+    s = make_system(args.workload, 0)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    info = g.info
+    ws = torch.empty(info["workspace_bytes_fermi"], dtype=torch.uint8, device="cuda")
+    D_val = torch.empty(info["nnz_D"], dtype=torch.float64, device="cuda")
+    order, mu, beta = args.fermi_order, -11.0, 0.8
+    gbe.gbe_density_fermi(Hd, g, mu, beta, order, workspace=ws, D_val=D_val)
+    ms = []
+    for _ in range(max(1, args.steps)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _, ne = gbe.gbe_density_fermi(Hd, g, mu, beta, order, workspace=ws, D_val=D_val, want_n_elec=False)
+        e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    t = float(np.median(ms))
+    print(json.dumps({"fermi": args.workload, "order": order, "mu": mu, "beta": beta, "ms": t,
+                      "ms_per_term": t / (order - 1), "orbitals_per_s": s.n / (t * 1e-3),
+                      "tflops_alg": info["sp2_flops_per_iter"] * (order - 1) / (t * 1e-3) * 1e-12}), flush=True)
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -449,10 +477,14 @@ def main() -> None:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="tau x partition sweep (BASELINE.json configs[4]) instead of the bench line")
     ap.add_argument("--sweep-out", default="", help="markdown table of the sweep")
+    ap.add_argument("--fermi", action="store_true", help="time the finite-temperature Chebyshev expansion (Eq.(7)) instead")
+    ap.add_argument("--fermi-order", type=int, default=60)
     ap.add_argument("--no-exact", action="store_true", help="sweep without the exact projector (no error columns)")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
+    elif args.fermi:
+        run_fermi(args)
     elif args.impl == "reference":
         run_reference(args)
     else:
