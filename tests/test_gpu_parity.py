@@ -366,6 +366,28 @@ def test_band_energy_and_expectation_values(gbe):
     assert e.value.status == -4
 
 
+# ------------------------------------------------------------------------------- seeded random shapes
+@pytest.mark.parametrize("case", range(24))
+def test_random_shapes_and_partitions(gbe, case):
+    """Seeded random banded Hamiltonians with random sizes (5 .. 330 orbitals: below one 8 x 8 sub-tile up to several
+    64 x 64 tiles with ragged tails), bandwidths, thresholds, graph powers, and arbitrary partition vectors (unequal,
+    non-contiguous, some communities empty).  Graph, halos, D pattern bit-exact; D within 1e-10."""
+    rng = np.random.default_rng(1000 + case)
+    n = int(rng.integers(5, 330))
+    n_part = int(rng.integers(1, max(2, n // 3)))
+    s = gi.random_banded(n, half_bw=int(rng.integers(1, 9)), n_part=n_part, seed=case, gap=float(rng.uniform(0.5, 3.0)),
+                         tau=float(rng.choice([0.0, 1e-6, 1e-4, 1e-2, 0.3])), iters=int(rng.integers(3, 26)),
+                         shuffle=bool(rng.integers(0, 2)))
+    if case % 3 == 0:  # an arbitrary partition vector: unequal communities, possibly empty ones
+        s.part = rng.integers(0, n_part, size=n).astype(np.int32)
+    s.n_occ = float(rng.integers(0, n + 1)) if case % 5 == 0 else s.n_occ
+    power = int(rng.integers(1, 4))
+    g, ex, Dg, log = run_gpu(gbe, s, power=power)
+    graph, r = run_oracle(s, power=power)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+
+
 # ------------------------------------------------------------------------------- degenerate shapes
 def test_one_partition_equals_exact_projector(gbe):
     s = gi.config(1)
