@@ -166,7 +166,6 @@ int gbe_launch_expectation(const gbe_graph* g, const double* D_val, const gbe_cs
                            cudaStream_t s);
 
 // small device utilities (gbe_util.cu)
-int gbe_exclusive_scan_i64(const int64_t* in, int64_t* out, int64_t n, cudaStream_t s);  // out has n+1 entries
 int gbe_exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s);
 
 // ----------------------------------------------------------------------------------------------

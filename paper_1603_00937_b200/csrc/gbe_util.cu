@@ -62,11 +62,6 @@ __global__ void __launch_bounds__(1024) k_scan_single_block(const TI* __restrict
 }
 }  // namespace
 
-int gbe_exclusive_scan_i64(const int64_t* in, int64_t* out, int64_t n, cudaStream_t s) {
-  k_scan_single_block<int64_t><<<1, 1024, 0, s>>>(in, out, n);
-  GBE_LAUNCHED();
-  return GBE_OK;
-}
 int gbe_exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s) {
   k_scan_single_block<int32_t><<<1, 1024, 0, s>>>(in, out, n);
   GBE_LAUNCHED();
