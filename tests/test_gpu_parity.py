@@ -466,6 +466,46 @@ def test_density_host_and_phase_calls(gbe):
     assert np.array_equal(log1.branch, logh.branch) and np.array_equal(log1.t1, log3.t1)
 
 
+def test_side_stream_and_two_graphs_in_flight(gbe):
+    """Everything is enqueued on the caller's stream: two systems on two non-default streams at once, results equal to
+    the ones computed alone on the default stream."""
+    import torch
+    sa, sb = gi.chain(256, 8, seed=1, tau=1e-4, iters=30), gi.random_banded(180, n_part=6, seed=2, tau=1e-3, iters=25)
+    ref = []
+    for s in (sa, sb):
+        g, ex, Dg, log = run_gpu(gbe, s, part=None)
+        ref.append(Dg)
+    st = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs, keep = [], []
+    for s, stream in zip((sa, sb), st):
+        with torch.cuda.stream(stream):
+            Hd = gbe.DeviceCSR.from_host(s.H)
+            g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part, stream=stream)
+            ws = g.new_workspace()
+            D = torch.empty(g.info["nnz_D"], dtype=torch.float64, device="cuda")
+            keep.append((Hd, g, ws))
+            outs.append(D)
+    for _ in range(3):  # interleave enqueues on the two streams, no synchronisation in between
+        for (Hd, g, ws), D, s, stream in zip(keep, outs, (sa, sb), st):
+            gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws, D_val=D, want_log=False, stream=stream)
+    torch.cuda.synchronize()
+    for D, r in zip(outs, ref):
+        assert np.array_equal(D.cpu().numpy(), r)  # same kernels, same reduction order: bit-identical
+
+
+@pytest.mark.parametrize("n", [2, 3, 9])
+def test_tiny_matrices(gbe, n):
+    s = gi.random_banded(n, half_bw=1, n_part=min(2, n), seed=n, tau=1e-3, iters=12)
+    if n == 2:
+        # Gershgorin bounds of a 2 x 2 matrix are symmetric about the mean eigenvalue, so at half filling the two
+        # candidate traces tie EXACTLY in every iteration and rounding picks the branch (reading A-8): use another filling
+        s.n_occ = 0.75
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+
+
 def test_errors(gbe):
     import torch
     s = gi.chain(64, 4)
