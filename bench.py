@@ -94,6 +94,11 @@ class ClockSampler:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.15)
         self.proc.terminate()
+        try:  # nvidia-smi's exit briefly stalls the driver: be sure it is gone before anything else is timed
+            self.proc.wait(timeout=10)
+        except Exception:
+            self.proc.kill()
+        time.sleep(0.5)
         sm, smax, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for ts, line in self.rows:
@@ -233,20 +238,19 @@ def run_ours(args) -> None:
     def step_device():
         g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part, stream=stream)
         gbe.gbe_density(Hd, g, s.n_occ, s.iters, -1.0, workspace=ws, D_val=D_val, want_log=False, stream=stream)
-        return g
+        g.free()  # inside the step: the graph of a step is released when its D is done (returns its arrays to the pool)
 
     def step_host():
         g = gbe.gbe_build_graph_host(Hh, s.tau, None, s.n_part, stream=stream)
         # H_host=None: the device copy uploaded by gbe_build_graph_host is reused (one upload per step)
         gbe.gbe_density_host(None, g, s.n_occ, s.iters, -1.0, workspace=ws, D_val_host=D_host.numpy(), stream=stream)
-        return g
+        g.free()
 
     step_ms_log = []
 
     def timed_region(step, steps):
         """K steps, each bracketed by CUDA events on the launching stream, L2 flushed (untimed) between steps."""
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-        graphs = []
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
@@ -254,20 +258,18 @@ def run_ours(args) -> None:
         for e0, e1 in ev:
             flush.zero_()
             e0.record(stream)
-            graphs.append(step())
+            step()
             e1.record(stream)
         torch.cuda.synchronize()
         launches = gbe.gbe_launch_count() - n0
         if world > 1:
             dist.barrier()
         ms = [e0.elapsed_time(e1) for e0, e1 in ev]
-        for g in graphs:
-            g.free()
         step_ms_log.append([round(x, 3) for x in ms])
         return float(np.sum(ms)), int(launches)
 
     for _ in range(max(args.warmup, 3)):
-        step_device().free()
+        step_device()
     torch.cuda.synchronize()
 
     clocks = ClockSampler(local)
@@ -279,7 +281,8 @@ def run_ours(args) -> None:
     clk = clocks.stop(t_wall0, t_wall1)
 
     # end to end: HOST buffers through the C ABI, copies inside the timed region
-    step_host().free()
+    for _ in range(max(args.warmup, 3)):
+        step_host()
     e2e_ms, _ = timed_region(step_host, args.steps)
 
     # per-kernel device times, same process, same inputs (CUDA events around every launch of gbe_density)

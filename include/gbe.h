@@ -101,7 +101,9 @@ typedef struct {
  * symmetrised (reading A-1 of Eq.(2) P:L38-40 / Eq.(8)), then for every community p its subgraph
  *     s_p = C_p u { k : (k,i) in S_tau, i in C_p }            (local order: core ascending, halo ascending)
  * and the pattern S' of D (A-9).
- *   H     device CSR, symmetric.
+ *   H     device CSR, SYMMETRIC.  With the default power 2 the library forms only the upper triangle of the
+ *         thresholded product A A (bit for bit symmetric when A is) and symmetrises the pattern; a non-symmetric H
+ *         gives the graph of that upper triangle.  opts.check_symmetry verifies the premise.
  *   part  device int32[n], vertex -> community id in [0, n_part); every vertex lies in exactly one core;
  *         empty communities are allowed.  NULL: contiguous blocks of ceil(n / n_part) rows.
  *         (The paper's partitioner, METIS P:L78, is outside the library.)

@@ -139,7 +139,7 @@ __device__ __forceinline__ void walk_products(int lane, int64_t a, int64_t b, co
 //    (offsets out_rp from MODE 0's counts) and cnt[i] = number kept.
 // 4: symbolic product (Eq.(8) with eps = 0: "paths of length two"): emits every candidate column at out_rp.
 template <int MODE>
-__global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __restrict__ A_rp,
+__global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, const int64_t* __restrict__ A_rp,
                                    const int32_t* __restrict__ A_col, const double* __restrict__ A_val,
                                    const int64_t* __restrict__ T_rp, const int32_t* __restrict__ T_col,
                                    const double* __restrict__ T_val, double tau, int32_t* __restrict__ cnt,
@@ -158,8 +158,12 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
     __syncwarp();
     const int64_t a = A_rp[i], b = A_rp[i + 1];
     // pass 1: mark candidate columns
-    walk_products<false, false>(lane, a, b, A_col, A_val, T_rp, T_col, T_val,
-                                [&](double, int j, double) { atomicOr(&bm[j >> 5], 1u << (j & 31)); });
+    // upper_only: the product is A A with A symmetric, so (A A)_ij == (A A)_ji bit for bit (k ascending, the two
+    // factors of every product commute) and only the columns j >= i are formed; S u S^T restores the rest
+    const int jmin = upper_only ? (int)i : 0;
+    walk_products<false, false>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, [&](double, int j, double) {
+      if (j >= jmin) atomicOr(&bm[j >> 5], 1u << (j & 31));
+    });
     __syncwarp();
     // compact slot index: rk[w] = number of candidates in words < w
     int running = 0;
@@ -194,6 +198,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, const int64_t* __r
     __syncwarp();
     // pass 2: accumulate, k ascending, multiply and add separately rounded
     walk_products<true, true>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, [&](double aik, int j, double t) {
+      if (j < jmin) return;
       const uint32_t word = bm[j >> 5];
       const int slot = rk[j >> 5] + __popc(word & ((1u << (j & 31)) - 1u));
       acc[slot] = __dadd_rn(acc[slot], __dmul_rn(aik, t));
@@ -466,6 +471,8 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   const int32_t* T_col = A.col.as<int32_t>();
   const double* T_val = A.val.as<double>();
   for (int k = 2; k <= power; ++k) {
+    // A A with symmetric A is symmetric bit for bit: when it is the LAST power only its upper triangle is formed
+    const int upper_only = (k == 2 && power == 2) ? 1 : 0;
     // symbolic: accumulator capacity
     {
       const size_t per_warp = (size_t)W * 8;
@@ -473,8 +480,8 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
       if (nw < 1) return GBE_EINVAL;
       GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
       const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
-      k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, A.rp.as<int64_t>(), A.col.as<int32_t>(),
-                                                                 A.val.as<double>(), T_rp, T_col, T_val, tau,
+      k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, upper_only, A.rp.as<int64_t>(),
+                                                                 A.col.as<int32_t>(), A.val.as<double>(), T_rp, T_col, T_val, tau,
                                                                  cnt.as<int32_t>(), nullptr, nullptr, nullptr);
       GBE_LAUNCHED();
     }
@@ -497,8 +504,8 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
       int64_t total_cand = 0;
       GBE_TRY(count_to_rowptr(cnt, n, Tc.rp, &total_cand, s));
       GBE_TRY(Tc.col.alloc((size_t)total_cand * 4));
-      k_spgemm_threshold<3><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, A.rp.as<int64_t>(), A.col.as<int32_t>(),
-                                                                 A.val.as<double>(), T_rp, T_col, T_val, tau,
+      k_spgemm_threshold<3><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, upper_only, A.rp.as<int64_t>(),
+                                                                 A.col.as<int32_t>(), A.val.as<double>(), T_rp, T_col, T_val, tau,
                                                                  cnt.as<int32_t>(), Tc.rp.as<int64_t>(),
                                                                  Tc.col.as<int32_t>(), nullptr);
       GBE_LAUNCHED();
@@ -512,14 +519,14 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
       break;
     }
     Pattern Tn;
-    k_spgemm_threshold<1><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, A.rp.as<int64_t>(), A.col.as<int32_t>(),
+    k_spgemm_threshold<1><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, 0, A.rp.as<int64_t>(), A.col.as<int32_t>(),
                                                                A.val.as<double>(), T_rp, T_col, T_val, tau,
                                                                cnt.as<int32_t>(), nullptr, nullptr, nullptr);
     GBE_LAUNCHED();
     GBE_TRY(count_to_rowptr(cnt, n, Tn.rp, &Tn.nnz, s));
     GBE_TRY(Tn.col.alloc((size_t)Tn.nnz * 4));
     GBE_TRY(Tn.val.alloc((size_t)Tn.nnz * 8));
-    k_spgemm_threshold<2><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, A.rp.as<int64_t>(), A.col.as<int32_t>(),
+    k_spgemm_threshold<2><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, 0, A.rp.as<int64_t>(), A.col.as<int32_t>(),
                                                                A.val.as<double>(), T_rp, T_col, T_val, tau, nullptr,
                                                                Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(),
                                                                Tn.val.as<double>());
@@ -571,14 +578,14 @@ int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int3
   GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
   GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
   const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
-  k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr,
+  k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, 0, M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr,
                                                              M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr, 0.0,
                                                              cnt.as<int32_t>(), nullptr, nullptr, nullptr);
   GBE_LAUNCHED();
   Pattern P;
   GBE_TRY(count_to_rowptr(cnt, n, P.rp, &P.nnz, s));
   GBE_TRY(P.col.alloc((size_t)P.nnz * 4));
-  k_spgemm_threshold<4><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr,
+  k_spgemm_threshold<4><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, 0, M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr,
                                                              M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr, 0.0, nullptr,
                                                              P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr);
   GBE_LAUNCHED();
