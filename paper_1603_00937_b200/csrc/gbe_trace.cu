@@ -17,10 +17,21 @@ __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double
   __shared__ double s1[TB], s2[TB];
   const int t = threadIdx.x;
   if (st->stop) return;
+  // the kernel is one CTA and latency bound: 8 independent 16-byte loads in flight per thread, summed in a fixed order
   double a1 = 0.0, a2 = 0.0;
-  for (int i = t; i < n; i += TB) {
-    a1 += partials[2 * (size_t)i];
-    a2 += partials[2 * (size_t)i + 1];
+  const double2* __restrict__ p2 = reinterpret_cast<const double2*>(partials);
+  int i = t;
+  for (; i + 7 * TB < n; i += 8 * TB) {
+    double2 v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = p2[i + u * TB];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { a1 += v[u].x; a2 += v[u].y; }
+  }
+  for (; i < n; i += TB) {
+    const double2 v = p2[i];
+    a1 += v.x;
+    a2 += v.y;
   }
   s1[t] = a1;
   s2[t] = a2;
