@@ -148,6 +148,19 @@ def test_config5_sweep_points(gbe, tau, n_part):
     check_density(Dg, log, r)
 
 
+@pytest.mark.slow
+def test_config5_largest_point_at_full_size(gbe):
+    """BASELINE.json configs[4] on the full 24,576-orbital box at the corner with the largest subgraphs (tau = 1e-7, 128
+    communities: core+halo 1,493 .. 2,295, up to 36 x 36 tiles per community, 3.4 GB per dense buffer).  Four SP2
+    iterations keep the oracle at about a minute; every stored entry of D is compared."""
+    s = gi.water_box(4096, 128, seed=0, tau=1e-7, iters=4)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+    assert g.info["max_m"] > 2000
+
+
 def check_any_size_properties(s, g, ex, Dg, log):
     """Properties of the path that hold at any size (used where the oracle is too slow to run in full)."""
     t1, t2, br = log.t1, log.t2, log.branch
