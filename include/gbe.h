@@ -37,7 +37,9 @@ extern "C" {
 typedef enum {
   GBE_OK = 0,
   GBE_EINVAL = -1,      /* null pointer, n <= 0, tau < 0 or NaN, n_occ outside [0,n], iters outside [0,GBE_MAX_ITERS],
-                           partition id out of range, power outside [1,GBE_MAX_POWER], n above the supported size */
+                           partition id out of range, power outside [1,GBE_MAX_POWER], n above the supported size
+                           (the index maps of steps 1-3 are bitmaps over the n vertices in shared memory: about
+                           4e5 orbitals with core+halo sizes up to a few thousand) */
   GBE_ENOTSYM = -2,     /* H is not symmetric (pattern or values); only tested when opts.check_symmetry != 0 */
   GBE_EDEGENERATE = -3, /* eps_max == eps_min: the spectrum cannot be mapped to [0,1] (A-12) */
   GBE_EMISMATCH = -4,   /* H.n differs from the graph's n */
