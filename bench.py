@@ -47,11 +47,15 @@ WORKLOADS = {
     # name: (molecules, communities) - BASELINE.json configs[1], configs[2] (SURVEY numbering: config 2, config 3)
     "water1024": (1024, 128),
     "water4096": (4096, 512),
+    # BASELINE.json configs[3]: 2,000-residue random coil in water, ~1.2e5 orbitals, heterogeneous core+halo sizes
+    "peptide2000": (None, None),
 }
 
 
 def make_system(workload: str, seed: int):
     import gbe_inputs as gi
+    if workload == "peptide2000":
+        return gi.peptide_water(2000, seed=seed)
     n_mol, n_part = WORKLOADS[workload]
     return gi.water_box(n_mol, n_part, seed=seed)
 
@@ -228,7 +232,9 @@ def run_ours(args) -> None:
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
 
     # sizes are fixed by the graph: build once to allocate outputs/workspace outside the timed region
-    g0 = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    part_t = None if s.meta.get("kind") == "water" else torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
+    part_h = None if part_t is None else np.asarray(s.part, dtype=np.int32)
+    g0 = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
     info = dict(g0.info)
     ws = g0.new_workspace()
     D_val = torch.empty(info["nnz_D"], dtype=torch.float64, device="cuda")
@@ -236,12 +242,12 @@ def run_ours(args) -> None:
     g0.free()
 
     def step_device():
-        g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part, stream=stream)
+        g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part, stream=stream)
         gbe.gbe_density(Hd, g, s.n_occ, s.iters, -1.0, workspace=ws, D_val=D_val, want_log=False, stream=stream)
         g.free()  # inside the step: the graph of a step is released when its D is done (returns its arrays to the pool)
 
     def step_host():
-        g = gbe.gbe_build_graph_host(Hh, s.tau, None, s.n_part, stream=stream)
+        g = gbe.gbe_build_graph_host(Hh, s.tau, part_h, s.n_part, stream=stream)
         # H_host=None: the device copy uploaded by gbe_build_graph_host is reused (one upload per step)
         gbe.gbe_density_host(None, g, s.n_occ, s.iters, -1.0, workspace=ws, D_val_host=D_host.numpy(), stream=stream)
         g.free()
@@ -286,7 +292,7 @@ def run_ours(args) -> None:
     e2e_ms, _ = timed_region(step_host, args.steps)
 
     # per-kernel device times, same process, same inputs (CUDA events around every launch of gbe_density)
-    g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
     ph = None
     for _ in range(2):
         flush.zero_()
@@ -295,7 +301,7 @@ def run_ours(args) -> None:
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
-    gbe.gbe_build_graph(Hd, s.tau, None, s.n_part).free()
+    gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part).free()
     e1.record(stream)
     torch.cuda.synchronize()
     graph_ms = e0.elapsed_time(e1)
@@ -319,7 +325,7 @@ def run_ours(args) -> None:
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {
-                "workload": f"{args.workload}: periodic water box, {s.meta['n_mol']} molecules, {s.n} orbitals, "
+                "workload": f"{args.workload}: {s.meta['kind']}, {s.n} orbitals, "
                             f"n_occ={s.n_occ:g}, tau={s.tau:g}, {s.n_part} communities, {s.iters} SP2 iterations, FP64",
                 "step": "gbe_build_graph + gbe_density (rows 0-6)", "parallelism": "replicas only" if world > 1 else "1 GPU",
                 "l2": "256 MiB buffer written between timed steps; dense batch (2 x %.2f GB) exceeds L2" % (info["dense_elems"] * 8e-9),
