@@ -506,6 +506,37 @@ def test_side_stream_and_two_graphs_in_flight(gbe):
         assert np.array_equal(D.cpu().numpy(), r)  # same kernels, same reduction order: bit-identical
 
 
+def test_density_is_capturable_in_a_cuda_graph(gbe):
+    """gbe_density without a log only enqueues kernels on the caller's stream (no allocation, no synchronisation, the
+    branch decision stays on the device), so the whole SP2 loop can be captured once and replayed - the way to run
+    launch-bound small systems (config 1: 82 launches of a few microseconds each)."""
+    import torch
+    s = gi.config(1)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    ws = g.new_workspace()
+    D_eager = torch.empty(g.info["nnz_D"], dtype=torch.float64, device="cuda")
+    gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws, D_val=D_eager, want_log=False)
+    torch.cuda.synchronize()
+    D_graph = torch.zeros_like(D_eager)
+    side = torch.cuda.Stream()
+    cg = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(cg, stream=side):
+            gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws, D_val=D_graph, want_log=False, stream=side)
+    for _ in range(3):
+        D_graph.zero_()
+        cg.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(D_graph, D_eager)
+    # H may change between replays (values are read at gather time): replay after perturbing H in place
+    Hd.val.mul_(1.0 + 1e-3)
+    gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws, D_val=D_eager, want_log=False)
+    cg.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(D_graph, D_eager)
+
+
 @pytest.mark.parametrize("n", [2, 3, 9])
 def test_tiny_matrices(gbe, n):
     s = gi.random_banded(n, half_bw=1, n_part=min(2, n), seed=n, tau=1e-3, iters=12)
