@@ -79,8 +79,8 @@ typedef struct {
   int64_t dense_elems;/* doubles in ONE batched dense buffer = sum_p m_p * ld_p (ld_p = m_p rounded up to 16) */
   int64_t n_tiles;    /* X^2 work items per SP2 iteration (upper-triangle tiles over all communities) */
   double sp2_flops_per_iter; /* sum_p 2 m_p^3: algorithmic flops of one SP2 iteration (unpadded, no symmetry) */
-  double sp2_exec_flops_per_iter; /* flops the X^2 kernel issues to the FP64 tensor pipe per iteration: upper-triangle
-                                     tiles only (X is symmetric), tile and K padding included */
+  double sp2_exec_flops_per_iter; /* flops the X^2 kernel issues to the FP64 tensor pipe per iteration: the 8 x 8
+                                     sub-tiles on or above the diagonal only (X is symmetric), K padded to ld_p */
   double eps_min, eps_max;   /* Gershgorin bounds of the H given to gbe_build_graph (A-5) */
   int32_t contiguous_cores;  /* 1: every core is a contiguous index range (fast scatter); 0: per-entry map */
   int32_t tile;              /* edge of the square X^2 tile chosen for this graph */
