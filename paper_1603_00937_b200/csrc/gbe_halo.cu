@@ -306,7 +306,9 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     GBE_TRY(upload(items, &g->items, s));
   }
   {
-    g->gather_rows = 64;
+    // rows per gather CTA: every CTA first builds the community's index bitmaps over the n vertices (O(n / 32) words), so
+    // large systems amortise that over more rows
+    g->gather_rows = n <= 32768 ? 64 : (n <= 131072 ? 256 : 512);
     std::vector<int2> gi;
     for (int p = 0; p < n_part; ++p)
       for (int r0 = 0; r0 < g->h_m[p]; r0 += g->gather_rows) gi.push_back(make_int2(p, r0));
