@@ -178,9 +178,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
     if constexpr (MODE == 0) {
       if (lane == 0) cnt[i] = running;
       __syncwarp();
-      continue;
-    }
-    if constexpr (MODE == 4) {
+    } else if constexpr (MODE == 4) {
       const int64_t ob4 = out_rp[i];
       for (int w = lane; w < W; w += 32) {
         uint32_t bits = bm[w];
@@ -192,8 +190,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
         }
       }
       __syncwarp();
-      continue;
-    }
+    } else {
     for (int s = lane; s < running; s += 32) acc[s] = 0.0;
     __syncwarp();
     // pass 2: accumulate, k ascending, multiply and add separately rounded
@@ -240,6 +237,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
     }
     if ((MODE == 1 || MODE == 3) && lane == 0) cnt[i] = kept;
     __syncwarp();
+    }  // numeric modes
   }
 }
 
