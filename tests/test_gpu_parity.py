@@ -357,13 +357,18 @@ def test_fermi_chebyshev_water_and_shuffled(gbe):
 
 # ------------------------------------------------------------------------------- observables
 def test_band_energy_and_expectation_values(gbe):
+    """The whole chain on both sides: the GPU takes the expectation of ITS density matrix, the oracle of its own (no
+    oracle input comes from the CUDA path); |D_gpu - D_oracle| <= 1e-10 bounds the difference by 1e-10 * sum|A|."""
     import torch
     s = gi.config(2)
     g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
     Hd = gbe.DeviceCSR.from_host(s.H)
     Dt = torch.from_numpy(Dg).cuda()
     e_gpu = gbe.gbe_expectation(g, Dt, Hd)
-    e_ref = o.expectation(ex["D_row_ptr"], ex["D_col"], Dg, s.H)
+    e_ref = o.expectation(r.D_row_ptr, r.D_col, r.D_val, s.H)
+    assert abs(e_gpu - e_ref) <= 1e-10 * np.abs(s.H.val).sum()
     assert abs(e_gpu - e_ref) <= 1e-9 * abs(e_ref)
     assert gbe.gbe_expectation(g, Dt, Hd) == e_gpu  # fixed reduction order: reproducible
     # Tr[D I] is the trace the SP2 log reports; a non-symmetric operand exercises the transposed lookup
@@ -372,8 +377,8 @@ def test_band_energy_and_expectation_values(gbe):
     rng = np.random.default_rng(1)
     A = sp.random(s.n, s.n, density=2e-3, random_state=rng, format="csr") + sp.triu(s.H.to_scipy(), k=1)
     Ac = gi.CSR.from_scipy(A)
-    a_ref = o.expectation(ex["D_row_ptr"], ex["D_col"], Dg, Ac)
-    assert abs(gbe.gbe_expectation(g, Dt, gbe.DeviceCSR.from_host(Ac)) - a_ref) <= 1e-9 * max(1.0, abs(a_ref))
+    a_ref = o.expectation(r.D_row_ptr, r.D_col, r.D_val, Ac)
+    assert abs(gbe.gbe_expectation(g, Dt, gbe.DeviceCSR.from_host(Ac)) - a_ref) <= 1e-10 * np.abs(Ac.val).sum()
     with pytest.raises(gbe.GbeError) as e:
         gbe.gbe_expectation(g, Dt, gbe.DeviceCSR.from_host(gi.chain(32, 4).H))
     assert e.value.status == -4
