@@ -81,6 +81,10 @@ typedef struct {
   double sp2_flops_per_iter; /* sum_p 2 m_p^3: algorithmic flops of one SP2 iteration (unpadded, no symmetry) */
   double sp2_exec_flops_per_iter; /* flops the X^2 kernel issues to the FP64 tensor pipe per iteration: the 8 x 8
                                      sub-tiles on or above the diagonal only (X is symmetric), K padded to ld_p */
+  int64_t n_tiles_last;      /* work items of the LAST SP2 iteration: the tiles with a core row only (the trace and
+                                the scatter read nothing else of the final X_p, Eq.(6)) */
+  double sp2_flops_last_iter;      /* sum_p 2 m_p^2 ncore_p: algorithmic flops of the last iteration (core columns) */
+  double sp2_exec_flops_last_iter; /* flops issued to the FP64 tensor pipe by the last iteration */
   double eps_min, eps_max;   /* Gershgorin bounds of the H given to gbe_build_graph (A-5) */
   int32_t contiguous_cores;  /* 1: every core is a contiguous index range (fast scatter); 0: per-entry map */
   int32_t tile;              /* edge of the square X^2 tile chosen for this graph */
@@ -136,7 +140,9 @@ int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, 
  *             H values are looked up at gather time, entries outside a subgraph are simply not gathered.
  *             The Gershgorin bounds are recomputed from this H.
  *   n_occ     target occupation (number of occupied orbitals), 0 <= n_occ <= n.
- *   iters     SP2 iterations (fixed count when idem_tol < 0).
+ *   iters     SP2 iterations (fixed count when idem_tol < 0).  Iteration iters - 1 computes only the tiles of X_p that
+ *             hold a core row or core column: nothing else of the final X_p is read (Eq.(6) P:L58-63 keeps the core
+ *             columns), so after the call the rest of the dense buffers in the workspace is stale scratch.
  *   idem_tol  >= 0: stop before iteration k >= 1 once |t1[k] - t2[k]| <= idem_tol (A-7); < 0: never stop early.
  *   workspace device memory, >= info.workspace_bytes, 256-byte aligned; contents are scratch.
  *   D_val     device double[nnz_D], CSR order of (D_row_ptr, D_col); entry (k,i) is taken from the expansion of
@@ -176,10 +182,12 @@ int gbe_build_graph_host(const gbe_csr_view* H_host, const gbe_graph_opts* opts,
 typedef struct {
   float bounds_ms;  int32_t bounds_launches;   /* step 0 */
   float gather_ms;  int32_t gather_launches;   /* step 3 */
-  float x2_ms;      int32_t x2_launches;       /* step 4: the X^2 / 2X - X^2 kernel, one launch per SP2 iteration */
+  float x2_ms;      int32_t x2_launches;       /* step 4: the X^2 / 2X - X^2 kernel, one launch per SP2 iteration
+                                                  (all but the last iteration) */
   float trace_ms;   int32_t trace_launches;    /* step 5 (+ the state initialisation kernel) */
   float scatter_ms; int32_t scatter_launches;  /* step 6 */
   float total_ms;                              /* first launch to last launch, on the stream */
+  float x2_last_ms; int32_t x2_last_launches;  /* step 4, last iteration: the tiles with a core row only */
 } gbe_phase_times;
 
 /* gbe_density with the same kernels and the same launch sequence, plus one event pair per launch; synchronises

@@ -42,6 +42,8 @@ class _GraphInfo(C.Structure):
     _fields_ = [("n", C.c_int64), ("nnz_S", C.c_int64), ("n_part", C.c_int64), ("sum_m", C.c_int64),
                 ("max_m", C.c_int64), ("nnz_D", C.c_int64), ("dense_elems", C.c_int64), ("n_tiles", C.c_int64),
                 ("sp2_flops_per_iter", C.c_double), ("sp2_exec_flops_per_iter", C.c_double),
+                ("n_tiles_last", C.c_int64), ("sp2_flops_last_iter", C.c_double),
+                ("sp2_exec_flops_last_iter", C.c_double),
                 ("eps_min", C.c_double), ("eps_max", C.c_double),
                 ("contiguous_cores", C.c_int32), ("tile", C.c_int32), ("workspace_bytes", C.c_size_t),
                 ("workspace_bytes_fermi", C.c_size_t)]
@@ -55,7 +57,8 @@ class _PhaseTimes(C.Structure):
     _fields_ = [("bounds_ms", C.c_float), ("bounds_launches", C.c_int32), ("gather_ms", C.c_float),
                 ("gather_launches", C.c_int32), ("x2_ms", C.c_float), ("x2_launches", C.c_int32),
                 ("trace_ms", C.c_float), ("trace_launches", C.c_int32), ("scatter_ms", C.c_float),
-                ("scatter_launches", C.c_int32), ("total_ms", C.c_float)]
+                ("scatter_launches", C.c_int32), ("total_ms", C.c_float), ("x2_last_ms", C.c_float),
+                ("x2_last_launches", C.c_int32)]
 
 
 _lib = None

@@ -13,7 +13,7 @@ namespace {
 thread_local char g_cuda_err[512] = "";
 
 // Optional per-launch timing (gbe_density_timed): one event pair around every launcher call.
-enum Phase { PH_BOUNDS = 0, PH_GATHER, PH_X2, PH_TRACE, PH_SCATTER, PH_COUNT };
+enum Phase { PH_BOUNDS = 0, PH_GATHER, PH_X2, PH_TRACE, PH_SCATTER, PH_X2_LAST, PH_COUNT };
 struct Timer {
   struct Rec { int phase, launches; cudaEvent_t e0, e1; };
   std::vector<Rec> recs;
@@ -97,7 +97,7 @@ const char* gbe_strerror(int status) {
 void gbe_free_graph(gbe_graph* g) {
   if (!g) return;
   void* ptrs[] = {g->S_row_ptr, g->S_col,     g->sub_ptr,  g->sub_idx,  g->ncore,    g->msize, g->dense_off, g->D_row_ptr,
-                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va};
+                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   delete g;
@@ -178,6 +178,9 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   o->n_tiles = g->n_items;
   o->sp2_flops_per_iter = g->flops_per_iter;
   o->sp2_exec_flops_per_iter = g->exec_flops_per_iter;
+  o->n_tiles_last = g->n_items_last;
+  o->sp2_flops_last_iter = g->flops_last_iter;
+  o->sp2_exec_flops_last_iter = g->exec_flops_last_iter;
   o->eps_min = g->eps_min;
   o->eps_max = g->eps_max;
   o->contiguous_cores = g->contiguous;
@@ -244,13 +247,18 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
   for (int it = 0; it < iters; ++it) {
     const double* in = (it & 1) ? w.X1 : w.X0;
     double* outp = (it & 1) ? w.X0 : w.X1;
-    GBE_TRY(timed(tm, PH_X2, g->n_items ? 1 : 0, [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, s); }));
+    // Iteration iters - 1 is the last one whether or not the idempotency stop fires before it (then it is a no-op):
+    // only the core rows and columns of its result are read again (trace, scatter), so it runs the core tiles only.
+    const bool last = it == iters - 1;
+    const int n_part_it = last ? g->n_items_last : g->n_items;
+    GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, g->n_items ? 1 : 0,
+                  [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, s); }));
     if (mode != 2)
-      GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, g->n_items, s); }));
+      GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, n_part_it, s); }));
   }
   if (mode == 2)  // one trace kernel at the end: t1, t2 of the final X for the log (written at index iters)
     GBE_TRY(timed(tm, PH_TRACE, 1, [&] {
-      return gbe_launch_trace_branch(w.st, w.partials, iters > 0 ? g->n_items : g->n_gitems, s);
+      return gbe_launch_trace_branch(w.st, w.partials, iters > 0 ? g->n_items_last : g->n_gitems, s);
     }));
   return GBE_OK;
 }
@@ -316,9 +324,10 @@ int gbe_density_timed(const gbe_csr_view* H, const gbe_graph* g, double n_occ, i
   Timer tm(s);
   GBE_TRY(do_density(H, g, n_occ, iters, idem_tol, workspace, workspace_bytes, cuda_stream, D_val, log, &tm));
   GBE_CUDA(cudaStreamSynchronize(s));
-  float* ms[PH_COUNT] = {&times->bounds_ms, &times->gather_ms, &times->x2_ms, &times->trace_ms, &times->scatter_ms};
-  int32_t* nl[PH_COUNT] = {&times->bounds_launches, &times->gather_launches, &times->x2_launches,
-                           &times->trace_launches, &times->scatter_launches};
+  float* ms[PH_COUNT] = {&times->bounds_ms, &times->gather_ms,  &times->x2_ms,
+                         &times->trace_ms,  &times->scatter_ms, &times->x2_last_ms};
+  int32_t* nl[PH_COUNT] = {&times->bounds_launches, &times->gather_launches,  &times->x2_launches,
+                           &times->trace_launches,  &times->scatter_launches, &times->x2_last_launches};
   for (auto& r : tm.recs) {
     float t = 0.f;
     GBE_CUDA(cudaEventElapsedTime(&t, r.e0, r.e1));

@@ -289,21 +289,30 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     std::vector<int32_t> order(n_part);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return g->h_m[a] > g->h_m[b]; });
-    std::vector<gbe_tile_item> items;
+    std::vector<gbe_tile_item> items, last;
     const int tile = g->tile;
-    g->exec_flops_per_iter = 0;
+    g->exec_flops_per_iter = g->exec_flops_last_iter = g->flops_last_iter = 0;
     for (int p : order) {
       const int T = (g->h_m[p] + tile - 1) / tile;
       const int64_t ld = (g->h_m[p] + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
       for (int ti = 0; ti < T; ++ti)
-        for (int tj = ti; tj < T; ++tj)
+        for (int tj = ti; tj < T; ++tj) {
           items.push_back({p, ti, tj, g->h_m[p], g->h_ncore[p], (int32_t)ld, g->h_dense_off[p]});
+          if (ti * tile < g->h_ncore[p]) last.push_back(items.back());
+        }
       // executed DMMA work: 8x8 sub-tiles (bi <= bj) with rows < m, columns < ld, each 2*8*8*ld flop
       const double R = (double)((g->h_m[p] + 7) / 8), C = (double)(ld / 8);
       g->exec_flops_per_iter += (R * C - R * (R - 1) / 2) * 128.0 * (double)ld;
+      // last iteration: the same count restricted to the row blocks of the tiles with a core row
+      const int Tc = std::min(T, (g->h_ncore[p] + tile - 1) / tile);
+      const double Rc = std::min(R, (double)(Tc * (tile / 8)));
+      g->exec_flops_last_iter += (Rc * C - Rc * (Rc - 1) / 2) * 128.0 * (double)ld;
+      g->flops_last_iter += 2.0 * (double)g->h_m[p] * (double)g->h_m[p] * (double)g->h_ncore[p];
     }
     g->n_items = (int32_t)items.size();
+    g->n_items_last = (int32_t)last.size();
     GBE_TRY(upload(items, &g->items, s));
+    GBE_TRY(upload(last, &g->items_last, s));
   }
   {
     // rows per gather CTA: every CTA first builds the community's index bitmaps over the n vertices (O(n / 32) words), so

@@ -92,6 +92,7 @@ struct gbe_graph {
   int64_t n = 0, nnz_S = 0, sum_m = 0, nnz_D = 0, dense_elems = 0;
   int32_t n_part = 0, max_m = 0, max_ncore = 0, tile = 64;
   double eps_min = 0, eps_max = 0, tau = 0, flops_per_iter = 0, exec_flops_per_iter = 0;
+  double flops_last_iter = 0, exec_flops_last_iter = 0;  // the core-tiles-only last iteration
   int32_t power = 2, contiguous = 1;
   // device arrays (owned)
   int64_t* S_row_ptr = nullptr;  // n+1
@@ -111,6 +112,10 @@ struct gbe_graph {
   int32_t* row_nc = nullptr;     // sum_m: ncore of the community of dense row q
   gbe_tile_item* items = nullptr;
   int32_t n_items = 0;
+  // the tiles of the LAST SP2 iteration: only those with a core row (row0 < ncore_p); they hold, directly or through
+  // the mirrored store, every core row and core column of X_p - all that the trace and the scatter read (Eq.(6))
+  gbe_tile_item* items_last = nullptr;
+  int32_t n_items_last = 0;
   int2* gitems = nullptr;  // gather work items (p, first row)
   int32_t n_gitems = 0, gather_rows = 0;
   // device copy of the H uploaded by gbe_build_graph_host (owned; null for graphs built from device pointers)
@@ -147,7 +152,7 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
 // step 4
 // iter: index n of the update X_n -> X_{n+1} (selects br[n] when the sequence is preset)
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                  cudaStream_t s);
+                  bool last, cudaStream_t s);
 // step 5
 int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s);
 // step 6

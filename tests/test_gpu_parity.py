@@ -59,6 +59,12 @@ def check_structure(ex, graph, r, info):
     assert abs(info["eps_min"] - r.eps_min) <= 1e-13 * abs(r.eps_min)
     assert abs(info["eps_max"] - r.eps_max) <= 1e-13 * abs(r.eps_max)
     assert abs(info["sp2_flops_per_iter"] - sum(2.0 * len(i) ** 3 for i, _ in r.subs)) < 1e-6 * info["sp2_flops_per_iter"]
+    # the last SP2 iteration runs the tiles with a core row only (Eq.(6) P:L58-63 keeps the core columns)
+    assert abs(info["sp2_flops_last_iter"] - sum(2.0 * len(i) ** 2 * nc for i, nc in r.subs)) <= 1e-6 * info["sp2_flops_per_iter"]
+    tl = info["tile"]
+    tiles = [(-(-len(i) // tl), min(-(-len(i) // tl), -(-nc // tl))) for i, nc in r.subs]
+    assert info["n_tiles"] == sum(T * (T + 1) // 2 for T, _ in tiles)
+    assert info["n_tiles_last"] == sum(sum(T - ti for ti in range(Tc)) for T, Tc in tiles)
 
 
 def check_density(Dg, log, r):
