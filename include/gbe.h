@@ -90,6 +90,8 @@ typedef struct {
   int32_t tile;              /* edge of the square X^2 tile chosen for this graph */
   size_t workspace_bytes;    /* device workspace gbe_density needs (two dense buffers + state + partials) */
   size_t workspace_bytes_fermi; /* device workspace gbe_density_fermi needs (four dense buffers + state + partials) */
+  int32_t resident_sp2;      /* 1: gbe_density will run the SP2 loop of this graph in the shared-memory-resident kernel */
+  int32_t resident_fits;     /* 1: the largest community fits that kernel (max_m <= 160); see gbe_graph_set_sp2_path */
 } gbe_graph_info;
 
 /* SP2 log (host memory, caller-allocated; valid after the stream has been synchronised).
@@ -134,6 +136,19 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* out);
  * S_row_ptr[n+1], S_col[nnz_S], sub_ptr[n_part+1], sub_idx[sum_m], ncore[n_part], D_row_ptr[n+1], D_col[nnz_D]. */
 int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, int32_t* S_col, int64_t* sub_ptr,
                      int32_t* sub_idx, int32_t* ncore, int64_t* D_row_ptr, int32_t* D_col);
+
+/* Which kernels run the SP2 loop (steps 4-5) of this graph.  Two implementations compute the same updates:
+ *   tiled    (any size)  one X^2 launch + one trace/branch launch per iteration over the batched dense layout in HBM;
+ *   resident (max_m <= 160) ONE launch for the whole loop, X_p held in shared memory by one CTA per community; the
+ *            global trace (one sequence for all subgraphs) is exchanged through a grid barrier, which needs all
+ *            communities co-resident (cooperative launch) - unless the sequence is preset and no trace is logged
+ *            (gbe_density_preset with trace_every_iteration = 0), where the CTAs never communicate.
+ * path = 0 (default): resident when it applies and all communities fit the device at once, else tiled;
+ *        1: always tiled;  2: resident whenever it can run (GBE_EINVAL if max_m is too large; calls for which the
+ *        communities are not co-resident still take the tiled kernels).
+ * Results of the two paths agree to rounding (different summation order of the global trace), each is bitwise
+ * reproducible.  Not thread safe against concurrent calls on the same graph. */
+int gbe_graph_set_sp2_path(gbe_graph* g, int32_t path);
 
 /* Steps 0 and 3-6: D = P_tau(H) on the pattern fixed by the graph (Eq.(6)).
  *   H         device CSR; values AND pattern may differ from the H the graph was built from (MD use):

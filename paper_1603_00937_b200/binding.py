@@ -20,6 +20,7 @@ EXPORTS = [
     "gbe_build_graph", "gbe_graph_get_info", "gbe_graph_export", "gbe_density", "gbe_gather", "gbe_sp2",
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
     "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation", "gbe_update_graph", "gbe_density_fermi",
+    "gbe_graph_set_sp2_path",
 ]
 
 
@@ -46,7 +47,7 @@ class _GraphInfo(C.Structure):
                 ("sp2_exec_flops_last_iter", C.c_double),
                 ("eps_min", C.c_double), ("eps_max", C.c_double),
                 ("contiguous_cores", C.c_int32), ("tile", C.c_int32), ("workspace_bytes", C.c_size_t),
-                ("workspace_bytes_fermi", C.c_size_t)]
+                ("workspace_bytes_fermi", C.c_size_t), ("resident_sp2", C.c_int32), ("resident_fits", C.c_int32)]
 
 
 class _Sp2Log(C.Structure):
@@ -92,6 +93,7 @@ def lib() -> C.CDLL:
         l.gbe_density_fermi.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_double, C.c_double, C.c_int32, C.c_void_p,
                                         C.c_size_t, C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]
         l.gbe_expectation.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CsrView), C.c_void_p, C.POINTER(C.c_double)]
+        l.gbe_graph_set_sp2_path.argtypes = [C.c_void_p, C.c_int32]
         l.gbe_launch_count.restype = C.c_uint64
         l.gbe_launch_count.argtypes = []
         l.gbe_gather.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -216,6 +218,14 @@ def gbe_update_graph(prev: Graph, D_prev: torch.Tensor, H: DeviceCSR, tau: float
     _check(lib().gbe_update_graph(prev.handle, _ptr(D_prev), C.byref(v), C.byref(opts), _ptr(part), int(n_part),
                                   _stream(stream), C.byref(out)))
     return Graph(out.value)
+
+
+def gbe_graph_set_sp2_path(g: "Graph", path: int) -> None:
+    """0 auto, 1 tiled kernels, 2 shared-memory-resident kernel (include/gbe.h)."""
+    _check(lib().gbe_graph_set_sp2_path(g._h, int(path)))
+    info = _GraphInfo()
+    _check(lib().gbe_graph_get_info(g._h, C.byref(info)))
+    g.info = {k: getattr(info, k) for k, _ in _GraphInfo._fields_}
 
 
 def gbe_launch_count() -> int:

@@ -45,6 +45,7 @@ __global__ void k_init_state(gbe_state* st, double n_occ, double idem_tol, int i
   st->stop = 0;
   st->iters_done = mode == 2 ? iters : 0;
   st->preset = mode != 0;
+  st->bar = 0;
 }
 
 struct WS {
@@ -165,6 +166,8 @@ int gbe_update_graph(const gbe_graph* prev, const double* D_prev, const gbe_csr_
   return build_graph_impl(H, opts, part, n_part, cuda_stream, out, prev, D_prev);
 }
 
+static bool use_resident(const gbe_graph* g, int mode);
+
 int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   if (!g || !o) return GBE_EINVAL;
   memset(o, 0, sizeof(*o));
@@ -187,6 +190,8 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   o->tile = g->tile;
   o->workspace_bytes = g->ws_bytes;
   o->workspace_bytes_fermi = g->ws_bytes_fermi;
+  o->resident_sp2 = use_resident(g, 0) ? 1 : 0;
+  o->resident_fits = g->resident_fits;
   return GBE_OK;
 }
 
@@ -225,6 +230,22 @@ int gbe_gather(const gbe_csr_view* H, const gbe_graph* g, void* workspace, size_
   return do_gather(H, g, workspace, workspace_bytes, cuda_stream, nullptr);
 }
 
+// The resident kernel runs when the largest community fits in shared memory and, unless the sequence is preset and no
+// trace is logged (no exchange between CTAs), when all communities are co-resident (cooperative launch).
+static bool use_resident(const gbe_graph* g, int mode) {
+  if (g->sp2_path == 1 || !g->resident_fits || g->n_items == 0) return false;
+  const bool can = mode == 2 || g->n_part <= g->resident_coresident;
+  if (g->sp2_path == 2) return can;
+  return can && g->n_part <= g->resident_coresident;  // auto: one wave of CTAs
+}
+
+int gbe_graph_set_sp2_path(gbe_graph* g, int32_t path) {
+  if (!g || path < 0 || path > 2) return GBE_EINVAL;
+  if (path == 2 && !g->resident_fits) return GBE_EINVAL;
+  g->sp2_path = path;
+  return GBE_OK;
+}
+
 static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_tol, void* workspace,
                   size_t workspace_bytes, void* cuda_stream, Timer* tm, const uint8_t* preset = nullptr,
                   bool trace_each = true) {
@@ -234,8 +255,22 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
   WS w;
   GBE_TRY(carve(g, workspace, workspace_bytes, &w));
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  // traces of X_0 (partials written by the gather), branch of iteration 0
   const int mode = !preset ? 0 : (trace_each ? 1 : 2);
+  if (use_resident(g, mode)) {
+    // small communities: the whole loop in one kernel, X_p resident in shared memory (gbe_resident.cu)
+    GBE_TRY(timed(tm, PH_TRACE, 1, [&]() -> int {
+      k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode);
+      GBE_LAUNCHED();
+      if (preset && iters > 0)
+        GBE_CUDA(cudaMemcpyAsync(w.st->br, preset, (size_t)iters, cudaMemcpyHostToDevice, s));
+      return GBE_OK;
+    }));
+    GBE_TRY(timed(tm, PH_X2, 1, [&] { return gbe_launch_sp2_resident(g, w.st, w.X0, w.X1, w.partials, mode, s); }));
+    if (mode == 2)
+      GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, g->n_part, s); }));
+    return GBE_OK;
+  }
+  // traces of X_0 (partials written by the gather), branch of iteration 0
   GBE_TRY(timed(tm, PH_TRACE, mode == 2 ? 1 : 2, [&]() -> int {
     k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode);
     GBE_LAUNCHED();

@@ -324,7 +324,8 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     g->n_gitems = (int32_t)gi.size();
     GBE_TRY(upload(gi, &g->gitems, s));
   }
-  g->n_partials = std::max(g->n_items, g->n_gitems);
+  g->n_partials = std::max(std::max(g->n_items, g->n_gitems), 2 * n_part);  // the resident kernel double-buffers n_part pairs
+  GBE_TRY(gbe_resident_capacity(g, &g->resident_fits, &g->resident_coresident));
 
   // workspace layout
   size_t off = align_up(sizeof(gbe_state), 256);

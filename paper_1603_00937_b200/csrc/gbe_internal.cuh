@@ -73,7 +73,7 @@ struct gbe_state {
   int32_t iters_done;  // number of updates applied; the final X lives in buffer iters_done & 1
   int32_t degenerate;  // eps_max == eps_min
   int32_t preset;      // 1: the branch sequence br[] was given by the caller (gbe_density_preset)
-  int32_t pad_;
+  uint32_t bar;        // arrival counter of the resident kernel's grid barrier (reset by k_init_state)
   double t1[GBE_MAX_ITERS + 1];
   double t2[GBE_MAX_ITERS + 1];
   uint8_t br[GBE_MAX_ITERS];
@@ -110,6 +110,9 @@ struct gbe_graph {
   int32_t* row_part = nullptr;   // sum_m: community of dense row q
   int64_t* row_src = nullptr;    // sum_m: element offset of dense row q in a dense buffer
   int32_t* row_nc = nullptr;     // sum_m: ncore of the community of dense row q
+  // SP2 path: 0 auto, 1 tiled kernels (gbe_x2.cu), 2 resident kernel (gbe_resident.cu); set by gbe_graph_set_sp2_path
+  int32_t sp2_path = 0;
+  int32_t resident_fits = 0, resident_coresident = 0;  // gbe_resident_capacity at build time
   gbe_tile_item* items = nullptr;
   int32_t n_items = 0;
   // the tiles of the LAST SP2 iteration: only those with a core row (row0 < ncore_p); they hold, directly or through
@@ -153,6 +156,10 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
 // iter: index n of the update X_n -> X_{n+1} (selects br[n] when the sequence is preset)
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
                   bool last, cudaStream_t s);
+// steps 4 + 5 in one kernel for small communities (gbe_resident.cu); mode as in k_init_state
+int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident);
+int gbe_launch_sp2_resident(const gbe_graph* g, gbe_state* st, double* X0, double* X1, double* partials, int mode,
+                            cudaStream_t s);
 // step 5
 int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s);
 // step 6

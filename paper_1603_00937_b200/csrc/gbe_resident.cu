@@ -1,0 +1,296 @@
+// Steps 4 + 5 for SMALL subgraphs: the whole SP2 loop in one kernel, X_p resident in shared memory.
+//
+//     for n = 0 .. iters - 1:  t1, t2 (global, over core diagonals);  branch_n;  X_p <- X_p^2  or  2 X_p - X_p^2
+// (one sequence for every subgraph).  A system of a few dozen small communities (config 1: 16 blocks
+// of 48 x 48) is launch bound on the tiled path: 2 launches of a few microseconds per iteration, each iteration streaming
+// 18 KB per matrix through L2.  Here one CTA owns one community for all iterations:
+//   - X_p (m_p <= 160) sits in shared memory, row stride ld_p + 4 doubles (conflict-free 64-bit fragment loads);
+//   - Y = X X^T on FP64 tensor cores (mma.sync.m8n8k4.f64): a work unit is one 8-row block x up to four 8-column blocks
+//     on or above the diagonal, the units are dealt round robin to the 16 warps (at most 4 each), accumulators stay in
+//     registers until every warp has finished reading X, then X is overwritten in place (direct + mirrored store).
+//     Rows and columns beyond m_p are zero in shared memory and stay zero under both updates: no predicates;
+//   - the global traces need one grid-wide exchange per iteration (P:L90 pre-sets the sequence to avoid it; north_star
+//     takes the decision from the trace): every CTA publishes (t1_p, t2_p), a grid barrier (cooperative launch: all CTAs
+//     are co-resident), then EVERY CTA sums all partials in the same fixed order and takes the same decision - no
+//     broadcast, no floating-point atomics, reproducible.  Partials are double buffered by iteration parity;
+//   - with a pre-determined sequence and no per-iteration trace log (gbe_density_preset, trace_every_iteration = 0)
+//     the CTAs never communicate: a plain launch, any number of communities.
+// Bound: latency (the grid barrier, ~2 us per iteration) - the FP64 work of config 1 is under 1 us per iteration.
+#include "gbe_internal.cuh"
+
+namespace {
+
+constexpr int RS_WARPS = 16;
+constexpr int RS_THREADS = RS_WARPS * 32;
+constexpr int RS_MAXU = 4;    // work units per warp
+constexpr int RS_UCOLS = 4;   // 8-column blocks per unit
+constexpr int RS_MAX_UNITS = RS_WARPS * RS_MAXU;
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
+// All CTAs of the (cooperative) grid arrive; `target` = arrivals expected since the counter was reset by k_init_state.
+__device__ __forceinline__ void grid_barrier(unsigned* bar, unsigned target) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(bar, 1u);
+    while (ld_acquire(bar) < target) {}
+    __threadfence();
+  }
+  __syncthreads();
+}
+
+// upper-triangle work units of an R x R grid of 8 x 8 blocks
+__host__ __device__ inline int rs_units(int R) {
+  int n = 0;
+  for (int bi = 0; bi < R; ++bi) n += (R - bi + RS_UCOLS - 1) / RS_UCOLS;
+  return n;
+}
+
+template <int NB>
+__device__ __forceinline__ void rs_unit_mma(double (&acc)[RS_UCOLS][2], const double* __restrict__ pa,
+                                            const double* __restrict__ pb, int ld, int stride) {
+#pragma unroll 4
+  for (int k0 = 0; k0 < ld; k0 += 4) {
+    const double a = pa[k0];
+    double b[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) b[j] = pb[j * 8 * stride + k0];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) dmma884(acc[j][0], acc[j][1], a, b[j]);
+  }
+}
+
+// mode 0: branch from the global trace; 1: preset sequence, traces logged every iteration (both: cooperative launch);
+// mode 2: preset sequence, no exchange; the final partials go to partials[p] for one k_trace_branch launch afterwards.
+__global__ void __launch_bounds__(RS_THREADS, 1)
+    k_sp2_resident(const int32_t* __restrict__ msize, const int32_t* __restrict__ ncore,
+                   const int64_t* __restrict__ dense_off, gbe_state* st, double* X0, double* X1, double* partials,
+                   int n_part, int mode) {
+  extern __shared__ __align__(16) double xs[];  // R8 rows x stride
+  __shared__ double red[2 * RS_WARPS];
+  __shared__ double tot[2];
+  __shared__ short2 units[RS_MAX_UNITS];
+  __shared__ int n_units_s;
+
+  const int p = blockIdx.x;
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5, g = lane >> 2, q = lane & 3;
+  const int m = msize[p], nc = ncore[p];
+  const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN, stride = ld + 4;
+  const int R = (m + 7) >> 3;
+  const int64_t doff = dense_off[p];
+  const int iters = st->iters;
+  const double n_occ = st->n_occ, idem_tol = st->idem_tol;
+
+  // ---- load X_0 (written by the gather), zero the rows [m, 8R)
+  {
+    const double2* __restrict__ src = reinterpret_cast<const double2*>(X0 + doff);
+    const int h = ld >> 1;
+    for (int i = t; i < m * h; i += RS_THREADS) {
+      const int r = i / h, c2 = i - r * h;
+      *reinterpret_cast<double2*>(xs + (size_t)r * stride + 2 * c2) = src[i];
+    }
+    for (int i = m * stride + t; i < 8 * R * stride; i += RS_THREADS) xs[i] = 0.0;
+    if (t == 0) {
+      int n = 0;
+      for (int bi = 0; bi < R; ++bi)
+        for (int bj = bi; bj < R; bj += RS_UCOLS) units[n++] = make_short2((short)bi, (short)bj);
+      n_units_s = n;
+    }
+  }
+  __syncthreads();
+  const int n_units = n_units_s;
+
+  // (t1_p, t2_p) of the X in shared memory: core diagonal and squared core rows (Tr_core X^2 for symmetric X)
+  auto core_traces = [&](double& o1, double& o2) {
+    double s1 = 0.0, s2 = 0.0;
+    for (int i = wid; i < nc; i += RS_WARPS) {
+      const double* __restrict__ row = xs + (size_t)i * stride;
+      for (int c = lane; c < ld; c += 32) {
+        const double x = row[c];
+        s2 += x * x;
+        if (c == i) s1 += x;
+      }
+    }
+    s1 = warp_sum(s1);
+    s2 = warp_sum(s2);
+    if (lane == 0) { red[wid] = s1; red[RS_WARPS + wid] = s2; }
+    __syncthreads();
+    if (t == 0) {
+      double a = 0.0, b = 0.0;
+      for (int w = 0; w < RS_WARPS; ++w) { a += red[w]; b += red[RS_WARPS + w]; }
+      o1 = a;
+      o2 = b;
+    }
+  };
+
+  // one update X <- X^2 (b = 0) or 2X - X^2 (b = 1), in place
+  auto update = [&](int b) {
+    double acc[RS_MAXU][RS_UCOLS][2];
+#pragma unroll
+    for (int u = 0; u < RS_MAXU; ++u)
+#pragma unroll
+      for (int j = 0; j < RS_UCOLS; ++j) acc[u][j][0] = acc[u][j][1] = 0.0;
+#pragma unroll
+    for (int u = 0; u < RS_MAXU; ++u) {
+      const int ui = wid + u * RS_WARPS;
+      if (ui < n_units) {
+        const short2 un = units[ui];
+        const int nb = min(RS_UCOLS, R - un.y);
+        const double* pa = xs + (size_t)(un.x * 8 + g) * stride + q;
+        const double* pb = xs + (size_t)(un.y * 8 + g) * stride + q;
+        switch (nb) {
+          case 4: rs_unit_mma<4>(acc[u], pa, pb, ld, stride); break;
+          case 3: rs_unit_mma<3>(acc[u], pa, pb, ld, stride); break;
+          case 2: rs_unit_mma<2>(acc[u], pa, pb, ld, stride); break;
+          default: rs_unit_mma<1>(acc[u], pa, pb, ld, stride); break;
+        }
+      }
+    }
+    __syncthreads();  // every warp has read what it needs of X_n
+#pragma unroll
+    for (int u = 0; u < RS_MAXU; ++u) {
+      const int ui = wid + u * RS_WARPS;
+      if (ui < n_units) {
+        const short2 un = units[ui];
+        const int nb = min(RS_UCOLS, R - un.y);
+        const int r = un.x * 8 + g;
+#pragma unroll
+        for (int j = 0; j < RS_UCOLS; ++j) {
+          if (j < nb) {
+            const int c = (un.y + j) * 8 + 2 * q;
+            double* xr = xs + (size_t)r * stride + c;
+            double v0 = acc[u][j][0], v1 = acc[u][j][1];
+            if (b) {  // only this lane touches (r, c), (r, c + 1) and their mirror images
+              const double2 x = *reinterpret_cast<const double2*>(xr);
+              v0 = 2.0 * x.x - v0;
+              v1 = 2.0 * x.y - v1;
+            }
+            *reinterpret_cast<double2*>(xr) = make_double2(v0, v1);
+            if (un.y + j != un.x) {  // off-diagonal block: mirror (the diagonal block is computed whole)
+              xs[(size_t)c * stride + r] = v0;
+              xs[(size_t)(c + 1) * stride + r] = v1;
+            }
+          }
+        }
+      }
+    }
+    __syncthreads();
+  };
+
+  double* const pbuf[2] = {partials, partials + 2 * (size_t)n_part};
+  int k = 0;
+  if (mode == 2) {  // pre-determined sequence, no exchange
+    for (; k < iters; ++k) update((int)st->br[k]);
+    double a = 0.0, b = 0.0;
+    core_traces(a, b);
+    if (t == 0) { partials[2 * (size_t)p] = a; partials[2 * (size_t)p + 1] = b; }
+  } else {
+    unsigned arrivals = 0;
+    for (;;) {
+      double a = 0.0, b = 0.0;
+      core_traces(a, b);
+      double* pb = pbuf[k & 1];
+      if (t == 0) { pb[2 * (size_t)p] = a; pb[2 * (size_t)p + 1] = b; }
+      arrivals += gridDim.x;
+      grid_barrier(&st->bar, arrivals);
+      if (wid == 0) {  // every CTA: the same fixed-order sum of all partials, read from L2
+        double s1 = 0.0, s2 = 0.0;
+        const double2* __restrict__ p2 = reinterpret_cast<const double2*>(pb);
+        for (int i = lane; i < n_part; i += 32) {
+          const double2 v = __ldcg(p2 + i);
+          s1 += v.x;
+          s2 += v.y;
+        }
+        s1 = warp_sum(s1);
+        s2 = warp_sum(s2);
+        if (lane == 0) { tot[0] = s1; tot[1] = s2; }
+      }
+      __syncthreads();
+      const double t1 = tot[0], t2 = tot[1];
+      const bool stop = k >= iters || (idem_tol >= 0.0 && k >= 1 && fabs(t1 - t2) <= idem_tol);
+      int br = 0;
+      if (!stop) br = mode == 1 ? (int)st->br[k] : ((fabs(t2 - n_occ) < fabs(2.0 * t1 - t2 - n_occ)) ? 0 : 1);
+      if (p == 0 && t == 0) {  // the log, exactly as k_trace_branch keeps it
+        st->t1[k] = t1;
+        st->t2[k] = t2;
+        st->iters_done = k;
+        if (stop) {
+          st->stop = 1;
+        } else {
+          st->branch = br;
+          st->br[k] = (uint8_t)br;
+          st->iter = k + 1;
+        }
+      }
+      if (stop) break;
+      update(br);
+      ++k;
+    }
+  }
+
+  // ---- the final X goes to buffer (updates applied) & 1, where the scatter looks for it
+  {
+    double2* __restrict__ dst = reinterpret_cast<double2*>(((k & 1) ? X1 : X0) + doff);
+    const int h = ld >> 1;
+    for (int i = t; i < m * h; i += RS_THREADS) {
+      const int r = i / h, c2 = i - r * h;
+      dst[i] = *reinterpret_cast<const double2*>(xs + (size_t)r * stride + 2 * c2);
+    }
+  }
+}
+
+size_t rs_smem_bytes(int max_m) {
+  const int ld = (max_m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+  const int R = (max_m + 7) / 8;
+  return (size_t)std::max(1, 8 * R) * (ld + 4) * sizeof(double);
+}
+}  // namespace
+
+// Can the resident kernel hold the largest community of this graph, and how many CTAs are co-resident on the device?
+int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident) {
+  *fits = 0;
+  *coresident = 0;
+  if (g->n_part <= 0 || g->max_m <= 0) return GBE_OK;
+  if (rs_units((g->max_m + 7) / 8) > RS_MAX_UNITS) return GBE_OK;
+  int dev = 0, smem_max = 0, sms = 0;
+  GBE_CUDA(cudaGetDevice(&dev));
+  GBE_CUDA(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  GBE_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const size_t smem = rs_smem_bytes(g->max_m);
+  if (smem + 1024 > (size_t)smem_max) return GBE_OK;
+  GBE_CUDA(cudaFuncSetAttribute(k_sp2_resident, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int per_sm = 0;
+  GBE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sp2_resident, RS_THREADS, smem));
+  *fits = per_sm > 0;
+  *coresident = per_sm * sms;
+  return GBE_OK;
+}
+
+int gbe_launch_sp2_resident(const gbe_graph* g, gbe_state* st, double* X0, double* X1, double* partials, int mode,
+                            cudaStream_t s) {
+  const size_t smem = rs_smem_bytes(g->max_m);
+  GBE_CUDA(cudaFuncSetAttribute(k_sp2_resident, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int32_t* msize = g->msize;
+  const int32_t* ncore = g->ncore;
+  const int64_t* doff = g->dense_off;
+  int n_part = g->n_part;
+  if (mode == 2) {
+    k_sp2_resident<<<n_part, RS_THREADS, smem, s>>>(msize, ncore, doff, st, X0, X1, partials, n_part, mode);
+  } else {
+    void* args[] = {&msize, &ncore, &doff, &st, &X0, &X1, &partials, &n_part, &mode};
+    GBE_CUDA(cudaLaunchCooperativeKernel((const void*)k_sp2_resident, dim3(n_part), dim3(RS_THREADS), args, smem, s));
+  }
+  GBE_LAUNCHED();
+  return GBE_OK;
+}

@@ -29,11 +29,15 @@ def gbe():
     return pkg
 
 
-def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None):
+def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None, sp2_path=0):
+    """sp2_path: 0 = the library's choice, 1 = tiled kernels, 2 = shared-memory-resident kernel (include/gbe.h)."""
     import torch
     Hd = gbe.DeviceCSR.from_host(s.H if H is None else H)
     part_t = None if part is None else torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
     g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part, power=power)
+    if sp2_path:
+        gbe.gbe_graph_set_sp2_path(g, sp2_path)
+        assert g.info["resident_sp2"] == (1 if sp2_path == 2 else 0)
     D, log = gbe.gbe_density(Hd, g, s.n_occ, s.iters if iters is None else iters, idem_tol)
     torch.cuda.synchronize()
     ex = {k: v.cpu().numpy() for k, v in g.export().items()}
@@ -79,9 +83,10 @@ def check_density(Dg, log, r):
 
 
 # ------------------------------------------------------------------------------- main configurations
-def test_config1_chain(gbe):
+@pytest.mark.parametrize("sp2_path", [1, 2])
+def test_config1_chain(gbe, sp2_path):
     s = gi.config(1)
-    g, ex, Dg, log = run_gpu(gbe, s)
+    g, ex, Dg, log = run_gpu(gbe, s, sp2_path=sp2_path)
     graph, r = run_oracle(s)
     check_structure(ex, graph, r, g.info)
     check_density(Dg, log, r)
@@ -210,10 +215,11 @@ def test_any_size_properties_hold_where_parity_is_known(gbe):
 
 
 # ------------------------------------------------------------------------------- pieces
-def test_iters_zero_returns_gathered_x0(gbe):
+@pytest.mark.parametrize("sp2_path", [1, 2])
+def test_iters_zero_returns_gathered_x0(gbe, sp2_path):
     """gather + scatter alone: D = core columns of X0[s,s]; exact up to the rounding of the two bounds."""
     s = gi.random_banded(150, half_bw=4, n_part=5, seed=3, tau=1e-3)
-    g, ex, Dg, log = run_gpu(gbe, s, iters=0)
+    g, ex, Dg, log = run_gpu(gbe, s, iters=0, sp2_path=sp2_path)
     graph, r = run_oracle(s, iters=0)
     check_structure(ex, graph, r, g.info)
     assert log.iters_done == 0 and log.t1.size == 1
@@ -241,17 +247,19 @@ def test_tau_sweep_chain(gbe, tau):
         assert g.info["nnz_S"] == s.n  # self loops only (A-12)
 
 
-def test_idem_tol_stops_on_device(gbe):
+@pytest.mark.parametrize("sp2_path", [1, 2])
+def test_idem_tol_stops_on_device(gbe, sp2_path):
     s = gi.config(1)
-    g, ex, Dg, log = run_gpu(gbe, s, iters=60, idem_tol=1e-9)
+    g, ex, Dg, log = run_gpu(gbe, s, iters=60, idem_tol=1e-9, sp2_path=sp2_path)
     graph, r = run_oracle(s, iters=60, idem_tol=1e-9)
     assert 15 < log.iters_done < 40
     check_density(Dg, log, r)
 
 
 # ------------------------------------------------------------------------------- pre-determined SP2 sequence
+@pytest.mark.parametrize("sp2_path", [1, 2])
 @pytest.mark.parametrize("trace", [True, False])
-def test_preset_sequence_from_the_previous_md_step(gbe, trace):
+def test_preset_sequence_from_the_previous_md_step(gbe, trace, sp2_path):
     """'the complete SP2 sequence (the same for each subgraph expansion) ... can be determined beforehand' (P:L90):
     the sequence is the one the oracle chooses for the Hamiltonian of the previous step (another noise draw), applied
     to the current H; the oracle replays the same sequence."""
@@ -264,6 +272,7 @@ def test_preset_sequence_from_the_previous_md_step(gbe, trace):
     r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, s.iters, replay=(seq, len(seq)))
     Hd = gbe.DeviceCSR.from_host(s.H)
     g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    gbe.gbe_graph_set_sp2_path(g, sp2_path)
     Dg, log = gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=trace)
     torch.cuda.synchronize()
     assert log.iters_done == len(seq) and np.array_equal(log.branch, seq)
@@ -406,10 +415,16 @@ def test_random_shapes_and_partitions(gbe, case):
         s.part = rng.integers(0, n_part, size=n).astype(np.int32)
     s.n_occ = float(rng.integers(0, n + 1)) if case % 5 == 0 else s.n_occ
     power = int(rng.integers(1, 4))
-    g, ex, Dg, log = run_gpu(gbe, s, power=power)
     graph, r = run_oracle(s, power=power)
-    check_structure(ex, graph, r, g.info)
-    check_density(Dg, log, r)
+    fits = None
+    for sp2_path in (1, 2):  # the tiled kernels, then the shared-memory-resident kernel where the communities fit it
+        if sp2_path == 2 and not fits:
+            continue
+        g, ex, Dg, log = run_gpu(gbe, s, power=power, sp2_path=sp2_path)
+        fits = g.info["resident_fits"]
+        assert fits == (1 if 0 < g.info["max_m"] <= 160 else 0)
+        check_structure(ex, graph, r, g.info)
+        check_density(Dg, log, r)
 
 
 # ------------------------------------------------------------------------------- degenerate shapes
@@ -548,6 +563,69 @@ def test_density_is_capturable_in_a_cuda_graph(gbe):
     assert torch.equal(D_graph, D_eager)
 
 
+def test_resident_kernel_launches_and_choice(gbe):
+    """The shared-memory-resident SP2 kernel (one launch for the whole loop) is what the library picks for config 1;
+    both paths give the same D to rounding and each is bitwise reproducible."""
+    import torch
+    s = gi.config(1)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    assert g.info["resident_fits"] == 1 and g.info["resident_sp2"] == 1
+    n0 = gbe.gbe_launch_count()
+    D_res, log_res = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
+    torch.cuda.synchronize()
+    assert gbe.gbe_launch_count() - n0 == 2 + 1 + 1 + 1 + 1  # bounds(2), gather, state init, SP2 loop, scatter
+    D_res2, _ = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
+    assert torch.equal(D_res, D_res2)
+    gbe.gbe_graph_set_sp2_path(g, 1)
+    n0 = gbe.gbe_launch_count()
+    D_til, log_til = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
+    torch.cuda.synchronize()
+    assert gbe.gbe_launch_count() - n0 == 2 + 1 + 2 + 2 * s.iters + 1
+    assert float((D_res - D_til).abs().max()) <= 1e-12
+    live = np.abs(log_til.t1[:-1] - log_til.t2[:-1]) > 1e-9
+    assert np.array_equal(log_res.branch[live], log_til.branch[live])
+    # a water-box graph does not fit: the request is refused, the choice stays with the tiled kernels
+    w = gi.water_box(64, 8)
+    gw = gbe.gbe_build_graph(gbe.DeviceCSR.from_host(w.H), w.tau, None, w.n_part)
+    assert gw.info["max_m"] > 160 and gw.info["resident_fits"] == 0 and gw.info["resident_sp2"] == 0
+    with pytest.raises(gbe.GbeError):
+        gbe.gbe_graph_set_sp2_path(gw, 2)
+
+
+def test_resident_kernel_more_communities_than_sms(gbe):
+    """600 communities of 8 sites: more CTAs than can be co-resident, so the trace-driven loop stays on the tiled kernels
+    (the grid barrier needs every community on the device at once) while a pre-determined sequence without trace
+    logging (no exchange between the subgraph expansions) runs the resident kernel as a plain launch."""
+    import torch
+    s = gi.chain(4800, 600, seed=5)
+    rp, ci = o.build_graph(s.H, s.tau)
+    r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, s.iters)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    assert g.info["resident_fits"] == 1 and g.info["resident_sp2"] == 0
+    Dg, log = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
+    torch.cuda.synchronize()
+    check_density(Dg.cpu().numpy(), log, r)
+    gbe.gbe_graph_set_sp2_path(g, 2)
+    n0 = gbe.gbe_launch_count()
+    Dp, logp = gbe.gbe_density_preset(Hd, g, r.branch, trace_every_iteration=False)
+    torch.cuda.synchronize()
+    assert gbe.gbe_launch_count() - n0 == 2 + 1 + 1 + 1 + 1 + 1  # bounds(2), gather, init, SP2 loop, final trace, scatter
+    assert np.abs(Dp.cpu().numpy() - r.D_val).max() <= TOL_D
+    assert abs(logp.t1[-1] - r.t1[-1]) <= TOL_TR and abs(logp.t2[-1] - r.t2[-1]) <= TOL_TR
+
+
+def test_resident_kernel_largest_community(gbe):
+    """Communities at the capacity of the resident kernel (m up to 160: 64 work units, 210 KB of shared memory)."""
+    s = gi.random_banded(1450, half_bw=6, n_part=10, seed=11, tau=1e-4, iters=25)
+    graph, r = run_oracle(s)
+    g, ex, Dg, log = run_gpu(gbe, s, sp2_path=2)
+    assert g.info["max_m"] == 160
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+
+
 @pytest.mark.parametrize("n", [2, 3, 9])
 def test_tiny_matrices(gbe, n):
     s = gi.random_banded(n, half_bw=1, n_part=min(2, n), seed=n, tau=1e-3, iters=12)
@@ -555,10 +633,11 @@ def test_tiny_matrices(gbe, n):
         # Gershgorin bounds of a 2 x 2 matrix are symmetric about the mean eigenvalue, so at half filling the two
         # candidate traces tie EXACTLY in every iteration and rounding picks the branch (reading A-8): use another filling
         s.n_occ = 0.75
-    g, ex, Dg, log = run_gpu(gbe, s)
     graph, r = run_oracle(s)
-    check_structure(ex, graph, r, g.info)
-    check_density(Dg, log, r)
+    for sp2_path in (1, 2):
+        g, ex, Dg, log = run_gpu(gbe, s, sp2_path=sp2_path)
+        check_structure(ex, graph, r, g.info)
+        check_density(Dg, log, r)
 
 
 def test_errors(gbe):
