@@ -236,7 +236,9 @@ static bool use_resident(const gbe_graph* g, int mode) {
   if (g->sp2_path == 1 || !g->resident_fits || g->n_items == 0) return false;
   const bool can = mode == 2 || g->n_part <= g->resident_coresident;
   if (g->sp2_path == 2) return can;
-  return can && g->n_part <= g->resident_coresident;  // auto: one wave of CTAs
+  // auto: one wave of CTAs, and communities small enough that one SM per community beats the tiled kernels
+  // (measured: 1.3 - 2.5x faster for m <= 128, 1.4x slower at m = 160)
+  return can && g->n_part <= g->resident_coresident && g->max_m <= 128;
 }
 
 int gbe_graph_set_sp2_path(gbe_graph* g, int32_t path) {
