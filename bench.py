@@ -492,6 +492,68 @@ def run_fermi(args) -> None:
                       "tflops_alg": info["sp2_flops_per_iter"] * (order - 1) / (t * 1e-3) * 1e-12}), flush=True)
 
 
+def run_small(args) -> None:
+    """Small systems (BASELINE.json configs[0] and relatives): the tiled kernels against the shared-memory-resident SP2
+    kernel, one JSON line per (system, path): gbe_density eagerly, as a CUDA-graph replay, and gbe_density_preset
+    without trace logging.  Times are CUDA-event means over 20 calls after 3 warm-ups, graph reused (as in MD)."""
+    import torch
+    from paper_1603_00937_b200 import build as gbe_build
+    gbe_build.build()
+    import gbe_inputs as gi
+    import paper_1603_00937_b200 as gbe
+
+    def mean_ms(fn, n=20):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    cases = [("config 1: chain, 512 orbitals, 16 communities", gi.config(1)),
+             ("chain, 4736 orbitals, 148 communities", gi.chain(4736, 148, seed=1)),
+             ("water box, 1536 orbitals, tau=1e-3, 128 communities", gi.water_box(256, 128, tau=1e-3)),
+             ("banded, 14504 orbitals, 148 communities", gi.random_banded(14504, half_bw=6, n_part=148, seed=11, tau=1e-4, iters=40)),
+             ("banded, 16872 orbitals, 148 communities", gi.random_banded(16872, half_bw=6, n_part=148, seed=11, tau=1e-4, iters=40)),
+             ("banded, 1450 orbitals, 10 communities", gi.random_banded(1450, half_bw=6, n_part=10, seed=11, tau=1e-4, iters=40))]
+    for name, s in cases:
+        Hd = gbe.DeviceCSR.from_host(s.H)
+        g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+        ws = g.new_workspace()
+        D = torch.empty(g.info["nnz_D"], dtype=torch.float64, device="cuda")
+        auto = "resident" if g.info["resident_sp2"] else "tiled"
+        seq = np.array([i & 1 for i in range(s.iters)], dtype=np.uint8)
+        for path, pname in ((1, "tiled"), (2, "resident")):
+            if path == 2 and not g.info["resident_fits"]:
+                continue
+            gbe.gbe_graph_set_sp2_path(g, path)
+            n0 = gbe.gbe_launch_count()
+            gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws, D_val=D, want_log=False)
+            launches = gbe.gbe_launch_count() - n0
+            eager = mean_ms(lambda: gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws, D_val=D, want_log=False))
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                torch.cuda.synchronize()
+                cg = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(cg, stream=st):
+                    gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws, D_val=D, want_log=False, stream=st)
+            replay = mean_ms(cg.replay)
+            preset = mean_ms(lambda: gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False, workspace=ws,
+                                                            D_val=D, want_log=False))
+            _, ph = gbe.gbe_density_timed(Hd, g, s.n_occ, s.iters, -1.0, workspace=ws, D_val=D)
+            print(json.dumps({"small": name, "n": s.n, "n_part": s.n_part, "m_max": g.info["max_m"], "iters": s.iters,
+                              "path": pname, "library_choice": auto, "launches_per_call": int(launches),
+                              "density_eager_us": eager * 1e3, "density_graph_replay_us": replay * 1e3,
+                              "preset_no_trace_eager_us": preset * 1e3,
+                              "sp2_loop_us": (ph["x2_ms"] + ph["x2_last_ms"] + ph["trace_ms"]) * 1e3,
+                              "orbitals_per_s_eager": s.n / (eager * 1e-3)}), flush=True)
+        g.free()
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -504,11 +566,14 @@ def main() -> None:
     ap.add_argument("--sweep-out", default="", help="markdown table of the sweep")
     ap.add_argument("--fermi", action="store_true", help="time the finite-temperature Chebyshev expansion (Eq.(7)) instead")
     ap.add_argument("--fermi-order", type=int, default=60)
+    ap.add_argument("--small", action="store_true", help="small systems: tiled kernels against the shared-memory-resident SP2 kernel")
     ap.add_argument("--gapped", action="store_true", help="sweep on the gapped variant of the water model, run to idempotency")
     ap.add_argument("--no-exact", action="store_true", help="sweep without the exact projector (no error columns)")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
+    elif args.small:
+        run_small(args)
     elif args.fermi:
         run_fermi(args)
     elif args.impl == "reference":
