@@ -16,6 +16,7 @@ line numbers of the paper text; `A-n` are the readings listed in DESIGN.md secti
     o_diag                         exact zero-temperature projector theta(mu I - H)
     o_fermi, fermi_chebyshev_coeffs  finite-temperature Chebyshev Fermi-operator expansion on the subgraphs, Eq.(7)
     expectation                    <A> = Tr[D A], E_band = Tr[D H]
+    error_norms                    max and Frobenius error of the sparse D against a dense reference (Fig.2)
     o_eq5_exact, o_eq5_nested      Eq.(4)-(5) P:L47-56 literally on the full matrix (tiny inputs)
 
 Pins (tests/test_oracle_*.py): closed forms (2x2 projector, periodic-chain projector),
@@ -38,6 +39,7 @@ from .gbe_oracle import (  # noqa: F401
     fermi_chebyshev_coeffs,
     FermiResult,
     expectation,
+    error_norms,
     o_eq5_exact,
     o_eq5_nested,
     SubResult,

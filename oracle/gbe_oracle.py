@@ -334,6 +334,26 @@ def expectation(D_row_ptr, D_col, D_val, A, n: int | None = None) -> float:
     return float(D.multiply(Ad.T).sum())
 
 
+def error_norms(D_row_ptr, D_col, D_val, D_ref) -> tuple[float, float, float]:
+    """Error of the assembled sparse D against a dense reference (Fig.2: "the error in the calculated density
+    matrix ... as measured by the Frobenius norm (normalized per atom)"; obs. (ii) P:L65: the error is set by tau).
+    Returns (max |D - D_ref| over the stored entries of D,
+             sum (D - D_ref)^2 over the stored entries,
+             ||D - D_ref||_F^2 over the full matrix: where D stores nothing it is zero, obs. (iv) P:L65)."""
+    D_ref = np.asarray(D_ref, dtype=np.float64)
+    n = D_ref.shape[0]
+    D = np.zeros((n, n))
+    stored = np.zeros((n, n), dtype=bool)
+    for k in range(n):
+        cols = np.asarray(D_col[D_row_ptr[k]:D_row_ptr[k + 1]])
+        D[k, cols] = D_val[D_row_ptr[k]:D_row_ptr[k + 1]]
+        stored[k, cols] = True
+    diff = D - D_ref
+    inside = diff[stored]
+    return (float(np.abs(inside).max()) if inside.size else 0.0, float((inside * inside).sum()),
+            float((diff * diff).sum()))
+
+
 # ----------------------------------------------------------------------------------------
 # exact projector
 # ----------------------------------------------------------------------------------------

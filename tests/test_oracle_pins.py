@@ -409,6 +409,35 @@ def test_expectation_uses_the_transpose_of_a_nonsymmetric_operand():
     assert abs(o.expectation(Dc.row_ptr, Dc.col_idx, Dc.val, Ac) - np.trace(D @ A.T)) > 1e-3
 
 
+def test_error_norms_on_a_hand_worked_example():
+    """Fig.2: Frobenius norm of the density-matrix error.  3 x 3 example worked by hand: D stores (0,0)=1, (0,2)=2,
+    (1,1)=-1, (2,0)=0 (a stored zero counts as stored); the reference is [[1.5,0.25,2],[0,-1,0.5],[3,0,0.125]]."""
+    rp, col, val = np.array([0, 2, 3, 4]), np.array([0, 2, 1, 0]), np.array([1.0, 2.0, -1.0, 0.0])
+    ref = np.array([[1.5, 0.25, 2.0], [0.0, -1.0, 0.5], [3.0, 0.0, 0.125]])
+    mx, f_in, f_all = o.error_norms(rp, col, val, ref)
+    assert mx == 3.0                                   # entry (2,0): |0 - 3|
+    assert f_in == 0.25 + 0.0 + 0.0 + 9.0               # stored entries: (0,0), (0,2), (1,1), (2,0)
+    assert f_all == 9.25 + 0.0625 + 0.25 + 0.015625     # + what the reference holds where D stores nothing
+    # a transposed pattern or a transposed reference changes all three
+    assert o.error_norms(rp, col, val, ref.T) != (mx, f_in, f_all)
+
+
+def test_error_norms_full_norm_is_the_dense_frobenius_norm_and_falls_with_tau():
+    """Against numpy's norm of the dense difference, on the chain: obs. (ii) P:L65, the error falls as tau falls."""
+    s = gi.chain(128, 8)
+    Dx = o.o_diag(s.H, 64)
+    prev = None
+    for tau in (1e-2, 1e-4, 1e-6):
+        rp, ci = o.build_graph(s.H, tau)
+        r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, 40)
+        mx, f_in, f_all = o.error_norms(r.D_row_ptr, r.D_col, r.D_val, Dx)
+        Dd = sp.csr_matrix((r.D_val, r.D_col, r.D_row_ptr), shape=(s.n, s.n)).toarray()
+        assert abs(f_all - np.linalg.norm(Dd - Dx, "fro") ** 2) <= 1e-12 * max(1.0, f_all)
+        assert f_in <= f_all and mx ** 2 <= f_in * (1 + 1e-12)
+        assert prev is None or f_all < prev
+        prev = f_all
+
+
 # ------------------------------------------------------------------------------- Eq.(8): graph of the next MD step
 def test_update_graph_is_paths_of_length_two_by_brute_force():
     """S = every (i, j) joined by a path of length <= 2 in M = I u pat(|D| >= tau) u pat(H), symmetrised - explicit loops."""
