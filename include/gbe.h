@@ -243,6 +243,18 @@ int gbe_density_fermi(const gbe_csr_view* H, const gbe_graph* g, double mu, doub
  *   out    HOST double; the call synchronises the stream.  The reduction order is fixed: reproducible bit for bit. */
 int gbe_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view* A, void* cuda_stream, double* out);
 
+/* Error of D against a dense reference matrix, e.g. the exact projector (Fig.2: "the error in the calculated
+ * density matrix ... as measured by the Frobenius norm (normalized per atom)"; obs. (ii) P:L65: the error is set by tau).
+ *   D_val   device double[nnz_D] on the pattern of `g`.
+ *   D_ref   device double, n rows of ld_ref >= n doubles, row-major (entry (k,i) at D_ref[k * ld_ref + i]).
+ *   out     HOST double[3]; the call synchronises the stream:
+ *           out[0] = max |D_ki - D_ref_ki| over the stored entries of D,
+ *           out[1] = sum (D_ki - D_ref_ki)^2 over the stored entries,
+ *           out[2] = ||D - D_ref||_F^2 over the full matrix: where D stores nothing it is zero (obs. (iv) P:L65).
+ *           Frobenius error per atom = sqrt(out[2]) / n_atoms.  Fixed reduction order: reproducible bit for bit. */
+int gbe_error_norms(const gbe_graph* g, const double* D_val, const double* D_ref, int64_t ld_ref, void* cuda_stream,
+                    double* out);
+
 /* Number of CUDA kernels this library has launched in this process so far (all threads). */
 uint64_t gbe_launch_count(void);
 

@@ -20,7 +20,7 @@ EXPORTS = [
     "gbe_build_graph", "gbe_graph_get_info", "gbe_graph_export", "gbe_density", "gbe_gather", "gbe_sp2",
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
     "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation", "gbe_update_graph", "gbe_density_fermi",
-    "gbe_graph_set_sp2_path",
+    "gbe_graph_set_sp2_path", "gbe_error_norms",
 ]
 
 
@@ -93,6 +93,7 @@ def lib() -> C.CDLL:
         l.gbe_density_fermi.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_double, C.c_double, C.c_int32, C.c_void_p,
                                         C.c_size_t, C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]
         l.gbe_expectation.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CsrView), C.c_void_p, C.POINTER(C.c_double)]
+        l.gbe_error_norms.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.POINTER(C.c_double)]
         l.gbe_graph_set_sp2_path.argtypes = [C.c_void_p, C.c_int32]
         l.gbe_launch_count.restype = C.c_uint64
         l.gbe_launch_count.argtypes = []
@@ -330,6 +331,18 @@ def gbe_expectation(g: Graph, D_val: torch.Tensor, A: DeviceCSR, stream=None) ->
     out = C.c_double(0.0)
     _check(lib().gbe_expectation(g.handle, _ptr(D_val), C.byref(v), _stream(stream), C.byref(out)))
     return float(out.value)
+
+
+def gbe_error_norms(g: Graph, D_val: torch.Tensor, D_ref: torch.Tensor, stream=None) -> tuple[float, float, float]:
+    """(max error over the stored entries, sum of squared errors over them, ||D - D_ref||_F^2 over the full matrix)
+    against a dense n x n reference on the device (Fig.2).  Synchronises."""
+    n = g.info["n"]
+    assert D_val.dtype == torch.float64 and D_val.is_cuda and D_val.numel() == g.info["nnz_D"]
+    assert D_ref.dtype == torch.float64 and D_ref.is_cuda and D_ref.dim() == 2 and D_ref.shape[0] == n
+    assert D_ref.stride(1) == 1 and D_ref.stride(0) >= n and D_ref.shape[1] == n
+    out = (C.c_double * 3)()
+    _check(lib().gbe_error_norms(g.handle, _ptr(D_val), _ptr(D_ref), int(D_ref.stride(0)), _stream(stream), out))
+    return float(out[0]), float(out[1]), float(out[2])
 
 
 def gbe_gather(H: DeviceCSR, g: Graph, workspace: torch.Tensor, stream=None) -> None:

@@ -436,6 +436,20 @@ int gbe_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view*
   return GBE_OK;
 }
 
+int gbe_error_norms(const gbe_graph* g, const double* D_val, const double* D_ref, int64_t ld_ref, void* cuda_stream,
+                    double* out) {
+  if (!g || !out || !D_ref || ld_ref < g->n || (!D_val && g->nnz_D > 0)) return GBE_EINVAL;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  gbe_set_alloc_stream(s);
+  DevBuf rows, res;
+  GBE_TRY(rows.alloc((size_t)g->n * 3 * 8));
+  GBE_TRY(res.alloc(3 * 8));
+  GBE_TRY(gbe_launch_error_norms(g, D_val, D_ref, ld_ref, rows.as<double>(), res.as<double>(), s));
+  GBE_CUDA(cudaMemcpyAsync(out, res.p, 3 * 8, cudaMemcpyDeviceToHost, s));
+  GBE_CUDA(cudaStreamSynchronize(s));
+  return GBE_OK;
+}
+
 uint64_t gbe_launch_count(void) { return g_gbe_launches.load(std::memory_order_relaxed); }
 
 int gbe_build_graph_host(const gbe_csr_view* Hh, const gbe_graph_opts* opts, const int32_t* part_host, int32_t n_part,

@@ -177,6 +177,9 @@ int gbe_launch_core_trace(const gbe_graph* g, const double* BD, gbe_state* st, c
 int gbe_launch_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view& A, double* row_sum, double* out,
                            cudaStream_t s);
 
+int gbe_launch_error_norms(const gbe_graph* g, const double* D_val, const double* D_ref, int64_t ld_ref, double* row_out,
+                           double* out, cudaStream_t s);
+
 // small device utilities (gbe_util.cu)
 int gbe_exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s);
 

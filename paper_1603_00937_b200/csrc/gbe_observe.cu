@@ -56,3 +56,86 @@ int gbe_launch_expectation(const gbe_graph* g, const double* D_val, const gbe_cs
   GBE_LAUNCHED();
   return GBE_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// Error of the assembled D against a dense reference (Fig.2: "the error in the calculated density matrix ... as
+// measured by the Frobenius norm (normalized per atom)"):
+//     out[0] = max |D_ki - R_ki| over the stored entries of D,   out[1] = sum (D_ki - R_ki)^2 over the stored entries,
+//     out[2] = ||D - R||_F^2 over the full matrix (D is zero where it stores nothing, obs. (iv) P:L65).
+// Warp per row: the stored entries lane-strided, then the gaps between consecutive stored columns summed directly
+// (no ||R||^2 - sum cancellation).  Fixed-order reductions: reproducible.  Bound: HBM (one pass over the n x n reference).
+namespace {
+__global__ void __launch_bounds__(256) k_error_rows(int64_t n, const int64_t* __restrict__ D_rp,
+                                                    const int32_t* __restrict__ D_col, const double* __restrict__ D_val,
+                                                    const double* __restrict__ R, int64_t ld,
+                                                    double* __restrict__ row_out /* 3 n */) {
+  const int lane = threadIdx.x & 31;
+  const int64_t k = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (k >= n) return;
+  const double* __restrict__ r = R + k * ld;
+  const int64_t e0 = D_rp[k], e1 = D_rp[k + 1];
+  double mx = 0.0, in2 = 0.0, out2 = 0.0;
+  for (int64_t e = e0 + lane; e < e1; e += 32) {
+    const double d = D_val[e] - r[D_col[e]];
+    mx = fmax(mx, fabs(d));
+    in2 += d * d;
+  }
+  int prev = -1;  // last stored column seen (n < 2^31: columns are int32)
+  for (int64_t b = e0; b <= e1; b += 32) {  // 32 stored columns at a time; the sentinel n closes the last gap
+    const int64_t e = b + lane;
+    const int mine = e < e1 ? D_col[e] : (int)n;
+    const int cnt = (int)min((int64_t)32, e1 - b + 1);
+    for (int u = 0; u < cnt; ++u) {
+      const int next = __shfl_sync(0xffffffffu, mine, u);
+      for (int c = prev + 1 + lane; c < next; c += 32) {
+        const double x = r[c];
+        out2 += x * x;
+      }
+      prev = next;
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  in2 = warp_sum(in2);
+  out2 = warp_sum(out2);
+  if (lane == 0) {
+    row_out[k] = mx;
+    row_out[n + k] = in2;
+    row_out[2 * n + k] = in2 + out2;
+  }
+}
+
+__global__ void __launch_bounds__(1024) k_error_final(int64_t n, const double* __restrict__ row_out,
+                                                      double* __restrict__ out) {
+  __shared__ double sh[3][1024];
+  const int t = threadIdx.x;
+  double mx = 0.0, a = 0.0, b = 0.0;
+  for (int64_t i = t; i < n; i += 1024) {
+    mx = fmax(mx, row_out[i]);
+    a += row_out[n + i];
+    b += row_out[2 * n + i];
+  }
+  sh[0][t] = mx;
+  sh[1][t] = a;
+  sh[2][t] = b;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if (t < o) {
+      sh[0][t] = fmax(sh[0][t], sh[0][t + o]);
+      sh[1][t] += sh[1][t + o];
+      sh[2][t] += sh[2][t + o];
+    }
+    __syncthreads();
+  }
+  if (t == 0) { out[0] = sh[0][0]; out[1] = sh[1][0]; out[2] = sh[2][0]; }
+}
+}  // namespace
+
+int gbe_launch_error_norms(const gbe_graph* g, const double* D_val, const double* D_ref, int64_t ld_ref, double* row_out,
+                           double* out, cudaStream_t s) {
+  const int64_t n = g->n;
+  k_error_rows<<<(unsigned)((n + 7) / 8), 256, 0, s>>>(n, g->D_row_ptr, g->D_col, D_val, D_ref, ld_ref, row_out);
+  GBE_LAUNCHED();
+  k_error_final<<<1, 1024, 0, s>>>(n, row_out, out);
+  GBE_LAUNCHED();
+  return GBE_OK;
+}

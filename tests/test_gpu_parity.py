@@ -399,6 +399,42 @@ def test_band_energy_and_expectation_values(gbe):
     assert e.value.status == -4
 
 
+def test_error_norms_against_the_exact_projector(gbe):
+    """Fig.2: max and Frobenius error of D against the exact projector, on the device; the oracle measures its own
+    D against the same reference.  A random non-symmetric reference with a padded leading dimension catches a
+    transposed or mis-strided lookup."""
+    import torch
+    s = gi.config(1)
+    g, ex, Dg, log = run_gpu(gbe, s)
+    graph, r = run_oracle(s)
+    Dx = o.o_diag(s.H, int(s.n_occ))
+    Dt = torch.from_numpy(Dg).cuda()
+    got = gbe.gbe_error_norms(g, Dt, torch.from_numpy(Dx).cuda())
+    want = o.error_norms(r.D_row_ptr, r.D_col, r.D_val, Dx)
+    tol = 4e-10 * np.sqrt(r.D_val.size * want[1]) + 1e-15
+    assert abs(got[0] - want[0]) <= TOL_D and abs(got[1] - want[1]) <= tol and abs(got[2] - want[2]) <= tol
+    assert abs(want[0] - 3.04e-4) < 2e-5  # the survey's probe value for config 1
+    assert gbe.gbe_error_norms(g, Dt, torch.from_numpy(Dx).cuda()) == got  # reproducible
+    rng = np.random.default_rng(3)
+    R = rng.normal(size=(s.n, s.n))
+    Rpad = torch.zeros(s.n, s.n + 24, dtype=torch.float64, device="cuda")
+    Rpad[:, :s.n] = torch.from_numpy(R).cuda()
+    got = gbe.gbe_error_norms(g, Dt, Rpad[:, :s.n])
+    want = o.error_norms(r.D_row_ptr, r.D_col, r.D_val, R)
+    assert abs(got[0] - want[0]) <= 1e-9 and abs(got[1] - want[1]) <= 1e-9 * want[1] and abs(got[2] - want[2]) <= 1e-9 * want[2]
+    # shuffled communities: rows of D with many short runs of stored columns
+    s2 = gi.random_banded(300, half_bw=5, n_part=11, seed=4, tau=1e-3, shuffle=True)
+    g2, ex2, Dg2, _ = run_gpu(gbe, s2)
+    _, r2 = run_oracle(s2)
+    R2 = rng.normal(size=(s2.n, s2.n))
+    got = gbe.gbe_error_norms(g2, torch.from_numpy(Dg2).cuda(), torch.from_numpy(R2).cuda())
+    want = o.error_norms(r2.D_row_ptr, r2.D_col, r2.D_val, R2)
+    assert abs(got[0] - want[0]) <= 1e-9 and abs(got[1] - want[1]) <= 1e-9 * want[1] and abs(got[2] - want[2]) <= 1e-9 * want[2]
+    import ctypes as C
+    out = (C.c_double * 3)()
+    assert gbe.lib().gbe_error_norms(g.handle, Dt.data_ptr(), Rpad.data_ptr(), s.n - 1, None, out) == -1  # ld_ref < n
+
+
 # ------------------------------------------------------------------------------- seeded random shapes
 @pytest.mark.parametrize("case", range(24))
 def test_random_shapes_and_partitions(gbe, case):
