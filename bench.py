@@ -545,7 +545,7 @@ def run_small(args) -> None:
                                                             D_val=D, want_log=False))
             _, ph = gbe.gbe_density_timed(Hd, g, s.n_occ, s.iters, -1.0, workspace=ws, D_val=D)
             print(json.dumps({"small": name, "n": s.n, "n_part": s.n_part, "m_max": g.info["max_m"], "iters": s.iters,
-                              "path": pname, "library_choice": auto, "launches_per_call": int(launches),
+                              "path": pname, "library_choice": auto, "cluster_exchange": int(g.info["resident_cluster"]) if path == 2 else 0, "launches_per_call": int(launches),
                               "density_eager_us": eager * 1e3, "density_graph_replay_us": replay * 1e3,
                               "preset_no_trace_eager_us": preset * 1e3,
                               "sp2_loop_us": (ph["x2_ms"] + ph["x2_last_ms"] + ph["trace_ms"]) * 1e3,

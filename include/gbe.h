@@ -92,6 +92,9 @@ typedef struct {
   size_t workspace_bytes_fermi; /* device workspace gbe_density_fermi needs (four dense buffers + state + partials) */
   int32_t resident_sp2;      /* 1: gbe_density will run the SP2 loop of this graph in the shared-memory-resident kernel */
   int32_t resident_fits;     /* 1: the largest community fits that kernel (max_m <= 160); see gbe_graph_set_sp2_path */
+  int32_t resident_cluster;  /* 1: all communities fit ONE thread-block cluster (n_part <= 16): the resident kernel then
+                                exchanges the traces through distributed shared memory and the cluster barrier */
+  int32_t reserved_;
 } gbe_graph_info;
 
 /* SP2 log (host memory, caller-allocated; valid after the stream has been synchronised).
@@ -141,7 +144,8 @@ int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, 
  *   tiled    (any size)  one X^2 launch + one trace/branch launch per iteration over the batched dense layout in HBM;
  *   resident (max_m <= 160) ONE launch for the whole loop, X_p held in shared memory by one CTA per community; the
  *            global trace (one sequence for all subgraphs) is exchanged through a grid barrier, which needs all
- *            communities co-resident (cooperative launch) - unless the sequence is preset and no trace is logged
+ *            communities co-resident (cooperative launch; one thread-block cluster with the exchange in distributed
+ *            shared memory when there are at most 16 communities) - unless the sequence is preset and no trace is logged
  *            (gbe_density_preset with trace_every_iteration = 0), where the CTAs never communicate.
  * path = 0 (default): resident when it applies and all communities fit the device at once, else tiled;
  *        1: always tiled;  2: resident whenever it can run (GBE_EINVAL if max_m is too large; calls for which the

@@ -192,6 +192,7 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   o->workspace_bytes_fermi = g->ws_bytes_fermi;
   o->resident_sp2 = use_resident(g, 0) ? 1 : 0;
   o->resident_fits = g->resident_fits;
+  o->resident_cluster = g->resident_cluster;
   return GBE_OK;
 }
 

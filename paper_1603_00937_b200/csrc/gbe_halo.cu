@@ -325,7 +325,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     GBE_TRY(upload(gi, &g->gitems, s));
   }
   g->n_partials = std::max(std::max(g->n_items, g->n_gitems), 2 * n_part);  // the resident kernel double-buffers n_part pairs
-  GBE_TRY(gbe_resident_capacity(g, &g->resident_fits, &g->resident_coresident));
+  GBE_TRY(gbe_resident_capacity(g, &g->resident_fits, &g->resident_coresident, &g->resident_cluster));
 
   // workspace layout
   size_t off = align_up(sizeof(gbe_state), 256);

@@ -113,6 +113,7 @@ struct gbe_graph {
   // SP2 path: 0 auto, 1 tiled kernels (gbe_x2.cu), 2 resident kernel (gbe_resident.cu); set by gbe_graph_set_sp2_path
   int32_t sp2_path = 0;
   int32_t resident_fits = 0, resident_coresident = 0;  // gbe_resident_capacity at build time
+  int32_t resident_cluster = 0;  // 1: all communities fit ONE thread-block cluster (<= 16): exchange through DSMEM
   gbe_tile_item* items = nullptr;
   int32_t n_items = 0;
   // the tiles of the LAST SP2 iteration: only those with a core row (row0 < ncore_p); they hold, directly or through
@@ -157,7 +158,7 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
                   bool last, cudaStream_t s);
 // steps 4 + 5 in one kernel for small communities (gbe_resident.cu); mode as in k_init_state
-int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident);
+int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident, int* cluster);
 int gbe_launch_sp2_resident(const gbe_graph* g, gbe_state* st, double* X0, double* X1, double* partials, int mode,
                             cudaStream_t s);
 // step 5

@@ -16,15 +16,19 @@
 //   - with a pre-determined sequence and no per-iteration trace log (gbe_density_preset, trace_every_iteration = 0)
 //     the CTAs never communicate: a plain launch, any number of communities.
 // Bound: latency (the grid barrier, ~2 us per iteration) - the FP64 work of config 1 is under 1 us per iteration.
+#include <cooperative_groups.h>
+
 #include "gbe_internal.cuh"
 
 namespace {
+namespace cg = cooperative_groups;
 
 constexpr int RS_WARPS = 16;
 constexpr int RS_THREADS = RS_WARPS * 32;
 constexpr int RS_MAXU = 4;    // work units per warp
 constexpr int RS_UCOLS = 4;   // 8-column blocks per unit
 constexpr int RS_MAX_UNITS = RS_WARPS * RS_MAXU;
+constexpr int RS_CLUSTER_MAX = 16;  // largest thread-block cluster (non-portable size)
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -76,12 +80,13 @@ __device__ __forceinline__ void rs_unit_mma(double (&acc)[RS_UCOLS][2], const do
 __global__ void __launch_bounds__(RS_THREADS, 1)
     k_sp2_resident(const int32_t* __restrict__ msize, const int32_t* __restrict__ ncore,
                    const int64_t* __restrict__ dense_off, gbe_state* st, double* X0, double* X1, double* partials,
-                   int n_part, int mode) {
+                   int n_part, int mode, int cl) {
   extern __shared__ __align__(16) double xs[];  // R8 rows x stride
   __shared__ double red[2 * RS_WARPS];
   __shared__ double tot[2];
   __shared__ short2 units[RS_MAX_UNITS];
   __shared__ int n_units_s;
+  __shared__ double cl_slots[2][RS_CLUSTER_MAX][2];  // [iteration parity][community] = (t1, t2), written by the peers
 
   const int p = blockIdx.x;
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5, g = lane >> 2, q = lane & 3;
@@ -110,8 +115,11 @@ __global__ void __launch_bounds__(RS_THREADS, 1)
   }
   __syncthreads();
   const int n_units = n_units_s;
+  // distributed shared memory may only be touched once every CTA of the cluster has started executing
+  if (cl) cg::this_cluster().sync();
 
-  // (t1_p, t2_p) of the X in shared memory: core diagonal and squared core rows (Tr_core X^2 for symmetric X)
+  // (t1_p, t2_p) of the X in shared memory: core diagonal and squared core rows (Tr_core X^2 for symmetric X);
+  // the result is valid in every lane of warp 0
   auto core_traces = [&](double& o1, double& o2) {
     double s1 = 0.0, s2 = 0.0;
     for (int i = wid; i < nc; i += RS_WARPS) {
@@ -126,11 +134,9 @@ __global__ void __launch_bounds__(RS_THREADS, 1)
     s2 = warp_sum(s2);
     if (lane == 0) { red[wid] = s1; red[RS_WARPS + wid] = s2; }
     __syncthreads();
-    if (t == 0) {
-      double a = 0.0, b = 0.0;
-      for (int w = 0; w < RS_WARPS; ++w) { a += red[w]; b += red[RS_WARPS + w]; }
-      o1 = a;
-      o2 = b;
+    if (wid == 0) {  // every lane of warp 0 ends up with both sums (fixed butterfly order)
+      o1 = warp_sum(lane < RS_WARPS ? red[lane] : 0.0);
+      o2 = warp_sum(lane < RS_WARPS ? red[RS_WARPS + lane] : 0.0);
     }
   };
 
@@ -205,32 +211,52 @@ __global__ void __launch_bounds__(RS_THREADS, 1)
   } else {
     unsigned arrivals = 0;
     for (;;) {
-      double a = 0.0, b = 0.0;
+      double a = 0.0, b = 0.0, t1, t2;
       core_traces(a, b);
-      double* pb = pbuf[k & 1];
-      arrivals += gridDim.x;
-      if (t == 0) {
-        pb[2 * (size_t)p] = a;
-        pb[2 * (size_t)p + 1] = b;
-        grid_arrive(&st->bar);
-      }
-      if (k < iters) square();  // Y = X_k X_k^T, whichever branch is taken (unused if the idempotency stop fires)
-      if (t == 0) grid_wait(&st->bar, arrivals);
-      __syncthreads();  // all partials are visible; every warp is done reading X_k
-      if (wid == 0) {  // every CTA: the same fixed-order sum of all partials, read from L2
-        double s1 = 0.0, s2 = 0.0;
-        const double2* __restrict__ p2 = reinterpret_cast<const double2*>(pb);
-        for (int i = lane; i < n_part; i += 32) {
-          const double2 v = __ldcg(p2 + i);
-          s1 += v.x;
-          s2 += v.y;
+      if (cl) {
+        // <= 16 communities: the grid is ONE thread-block cluster; the sums travel through distributed shared memory and
+        // the hardware cluster barrier (arrive.release / wait.acquire) replaces the round trips through L2
+        cg::cluster_group cluster = cg::this_cluster();
+        if (t < n_part) {  // lanes of warp 0: lane t delivers this community's pair to peer t
+          double* dst = cluster.map_shared_rank(&cl_slots[k & 1][p][0], t);
+          dst[0] = a;
+          dst[1] = b;
         }
-        s1 = warp_sum(s1);
-        s2 = warp_sum(s2);
-        if (lane == 0) { tot[0] = s1; tot[1] = s2; }
+        __syncwarp();  // the cluster barrier is .aligned: warp 0 must be converged again
+        cluster.barrier_arrive();
+        if (k < iters) square();
+        cluster.barrier_wait();  // every peer's pair has landed here
+        __syncthreads();         // every warp is done reading X_k (the arrivals were counted BEFORE the squaring)
+        // every warp sums the pairs itself, in the same butterfly order: no broadcast, no further barrier
+        t1 = warp_sum(lane < n_part ? cl_slots[k & 1][lane][0] : 0.0);
+        t2 = warp_sum(lane < n_part ? cl_slots[k & 1][lane][1] : 0.0);
+      } else {
+        double* pb = pbuf[k & 1];
+        arrivals += gridDim.x;
+        if (t == 0) {
+          pb[2 * (size_t)p] = a;
+          pb[2 * (size_t)p + 1] = b;
+          grid_arrive(&st->bar);
+        }
+        if (k < iters) square();  // Y = X_k X_k^T, whichever branch is taken (unused if the idempotency stop fires)
+        if (t == 0) grid_wait(&st->bar, arrivals);
+        __syncthreads();  // all partials are visible; every warp is done reading X_k
+        if (wid == 0) {  // the same fixed-order sum of all partials in every CTA, read from L2 by one warp
+          double s1 = 0.0, s2 = 0.0;
+          const double2* __restrict__ p2 = reinterpret_cast<const double2*>(pb);
+          for (int i = lane; i < n_part; i += 32) {
+            const double2 v = __ldcg(p2 + i);
+            s1 += v.x;
+            s2 += v.y;
+          }
+          s1 = warp_sum(s1);
+          s2 = warp_sum(s2);
+          if (lane == 0) { tot[0] = s1; tot[1] = s2; }
+        }
+        __syncthreads();
+        t1 = tot[0];
+        t2 = tot[1];
       }
-      __syncthreads();
-      const double t1 = tot[0], t2 = tot[1];
       const bool stop = k >= iters || (idem_tol >= 0.0 && k >= 1 && fabs(t1 - t2) <= idem_tol);
       int br = 0;
       if (!stop) br = mode == 1 ? (int)st->br[k] : ((fabs(t2 - n_occ) < fabs(2.0 * t1 - t2 - n_occ)) ? 0 : 1);
@@ -271,9 +297,10 @@ size_t rs_smem_bytes(int max_m) {
 }  // namespace
 
 // Can the resident kernel hold the largest community of this graph, and how many CTAs are co-resident on the device?
-int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident) {
+int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident, int* cluster) {
   *fits = 0;
   *coresident = 0;
+  *cluster = 0;
   if (g->n_part <= 0 || g->max_m <= 0) return GBE_OK;
   if (rs_units((g->max_m + 7) / 8) > RS_MAX_UNITS) return GBE_OK;
   int dev = 0, smem_max = 0, sms = 0;
@@ -287,6 +314,24 @@ int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident) {
   GBE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sp2_resident, RS_THREADS, smem));
   *fits = per_sm > 0;
   *coresident = per_sm * sms;
+  *cluster = 0;
+  if (*fits && g->n_part <= RS_CLUSTER_MAX) {  // can one cluster of n_part CTAs be scheduled?
+    GBE_CUDA(cudaFuncSetAttribute(k_sp2_resident, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(g->n_part);
+    cfg.blockDim = dim3(RS_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)g->n_part;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    int n_clusters = 0;
+    if (cudaOccupancyMaxActiveClusters(&n_clusters, k_sp2_resident, &cfg) == cudaSuccess) *cluster = n_clusters > 0;
+    else (void)cudaGetLastError();
+  }
   return GBE_OK;
 }
 
@@ -298,10 +343,27 @@ int gbe_launch_sp2_resident(const gbe_graph* g, gbe_state* st, double* X0, doubl
   const int32_t* ncore = g->ncore;
   const int64_t* doff = g->dense_off;
   int n_part = g->n_part;
+  int cl = 0;
   if (mode == 2) {
-    k_sp2_resident<<<n_part, RS_THREADS, smem, s>>>(msize, ncore, doff, st, X0, X1, partials, n_part, mode);
+    k_sp2_resident<<<n_part, RS_THREADS, smem, s>>>(msize, ncore, doff, st, X0, X1, partials, n_part, mode, cl);
+  } else if (g->resident_cluster) {
+    // one thread-block cluster holds every community: exchange through distributed shared memory
+    cl = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(n_part);
+    cfg.blockDim = dim3(RS_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)n_part;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    GBE_CUDA(cudaLaunchKernelEx(&cfg, k_sp2_resident, msize, ncore, doff, st, X0, X1, partials, n_part, mode, cl));
   } else {
-    void* args[] = {&msize, &ncore, &doff, &st, &X0, &X1, &partials, &n_part, &mode};
+    void* args[] = {&msize, &ncore, &doff, &st, &X0, &X1, &partials, &n_part, &mode, &cl};
     GBE_CUDA(cudaLaunchCooperativeKernel((const void*)k_sp2_resident, dim3(n_part), dim3(RS_THREADS), args, smem, s));
   }
   GBE_LAUNCHED();

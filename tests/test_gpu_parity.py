@@ -607,12 +607,14 @@ def test_resident_kernel_launches_and_choice(gbe):
     Hd = gbe.DeviceCSR.from_host(s.H)
     g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
     assert g.info["resident_fits"] == 1 and g.info["resident_sp2"] == 1
+    assert g.info["resident_cluster"] == 1  # 16 communities: one thread-block cluster, exchange through DSMEM
     n0 = gbe.gbe_launch_count()
     D_res, log_res = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
     torch.cuda.synchronize()
     assert gbe.gbe_launch_count() - n0 == 2 + 1 + 1 + 1 + 1  # bounds(2), gather, state init, SP2 loop, scatter
-    D_res2, _ = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
-    assert torch.equal(D_res, D_res2)
+    for _ in range(10):  # a race between the CTAs of the cluster or the warps of a CTA would show up as run-to-run noise
+        D_res2, log2 = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
+        assert torch.equal(D_res, D_res2) and np.array_equal(log2.t1, log_res.t1) and np.array_equal(log2.t2, log_res.t2)
     gbe.gbe_graph_set_sp2_path(g, 1)
     n0 = gbe.gbe_launch_count()
     D_til, log_til = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
@@ -639,10 +641,22 @@ def test_resident_kernel_more_communities_than_sms(gbe):
     r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, s.iters)
     Hd = gbe.DeviceCSR.from_host(s.H)
     g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
-    assert g.info["resident_fits"] == 1 and g.info["resident_sp2"] == 0
+    assert g.info["resident_fits"] == 1 and g.info["resident_sp2"] == 0 and g.info["resident_cluster"] == 0
     Dg, log = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
     torch.cuda.synchronize()
     check_density(Dg.cpu().numpy(), log, r)
+    # 148 of these communities are co-resident: the cooperative launch with the exchange through L2, run to run identical
+    s148 = gi.chain(1184, 148, seed=6)
+    H148 = gbe.DeviceCSR.from_host(s148.H)
+    g148 = gbe.gbe_build_graph(H148, s148.tau, None, s148.n_part)
+    assert g148.info["resident_sp2"] == 1 and g148.info["resident_cluster"] == 0
+    rp8, ci8 = o.build_graph(s148.H, s148.tau)
+    r148 = o.o_sub(s148.H, rp8, ci8, s148.part, s148.n_part, s148.n_occ, s148.iters)
+    D0, log0 = gbe.gbe_density(H148, g148, s148.n_occ, s148.iters)
+    check_density(D0.cpu().numpy(), log0, r148)
+    for _ in range(10):
+        D1, log1 = gbe.gbe_density(H148, g148, s148.n_occ, s148.iters)
+        assert torch.equal(D0, D1) and np.array_equal(log0.t1, log1.t1)
     gbe.gbe_graph_set_sp2_path(g, 2)
     n0 = gbe.gbe_launch_count()
     Dp, logp = gbe.gbe_density_preset(Hd, g, r.branch, trace_every_iteration=False)
