@@ -10,9 +10,12 @@
 //     registers until every warp has finished reading X, then X is overwritten in place (direct + mirrored store).
 //     Rows and columns beyond m_p are zero in shared memory and stay zero under both updates: no predicates;
 //   - the global traces need one grid-wide exchange per iteration (P:L90 pre-sets the sequence to avoid it; north_star
-//     takes the decision from the trace): every CTA publishes (t1_p, t2_p), a grid barrier (cooperative launch: all CTAs
-//     are co-resident), then EVERY CTA sums all partials in the same fixed order and takes the same decision - no
-//     broadcast, no floating-point atomics, reproducible.  Partials are double buffered by iteration parity;
+//     takes the decision from the trace).  <= 16 communities: the grid is one thread-block cluster, every CTA stores its
+//     (t1_p, t2_p) into each peer's shared memory (DSMEM) and the hardware cluster barrier orders it.  More communities
+//     (cooperative launch: all CTAs are co-resident): the pairs go to global memory, the CTAs arrive at a counter with
+//     a release reduction and acquire it.  Either way EVERY CTA sums all pairs in the same fixed order and takes the same
+//     decision - no broadcast, no floating-point atomics, reproducible.  The squaring does not depend on the branch and
+//     runs between arrive and wait;
 //   - with a pre-determined sequence and no per-iteration trace log (gbe_density_preset, trace_every_iteration = 0)
 //     the CTAs never communicate: a plain launch, any number of communities.
 // Bound: latency (the grid barrier, ~2 us per iteration) - the FP64 work of config 1 is under 1 us per iteration.
