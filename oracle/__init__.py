@@ -13,6 +13,7 @@ line numbers of the paper text; `A-n` are the readings listed in DESIGN.md secti
     update_graph                   Eq.(8), symbolic form (graph of the next MD step from D(t-dt) and H(t))
     subgraphs, density_pattern     step 2   P:L58, Fig.1, obs. (vi) P:L65 (A-9)
     o_sub                          steps 3-6: Eq.(6) P:L60-63 with SP2   <- parity target
+    OneCommunity                   steps 1-6 for one community at a time, branch sequence given (sampled outputs at full size)
     o_diag                         exact zero-temperature projector theta(mu I - H)
     o_fermi, fermi_chebyshev_coeffs  finite-temperature Chebyshev Fermi-operator expansion on the subgraphs, Eq.(7)
     expectation                    <A> = Tr[D A], E_band = Tr[D H]
@@ -43,4 +44,5 @@ from .gbe_oracle import (  # noqa: F401
     o_eq5_exact,
     o_eq5_nested,
     SubResult,
+    OneCommunity,
 )

@@ -256,6 +256,55 @@ def o_sub(H, S_row_ptr, S_col, part, n_part: int, n_occ: float, iters: int, idem
 
 
 # ----------------------------------------------------------------------------------------
+# one community at a time (full-size inputs, where the whole batch is too much work for a CPU)
+# ----------------------------------------------------------------------------------------
+class OneCommunity:
+    """The same definitions as build_graph / subgraphs / o_sub, evaluated for ONE community p at a time, so that
+    sampled outputs of a full-size system can be computed one by one:
+
+      graph rows  S_tau is I u pat(A) u pat(floor(A A)_tau), then S u S^T (reading A-1 of Eq.(2), power 2).
+                  The rows of S u S^T that belong to the core vertices C_p are the rows C_p of S together with the
+                  columns C_p of S, i.e. floor(A[C_p, :] A)_tau and floor(A A[:, C_p])_tau - two thin products.
+      subgraph    s_p = C_p u {k : (k, i) in S, i in C_p}, core ascending then halo ascending (obs. (vi) P:L65)
+      expansion   x_p = X0[s_p, s_p] (A-2), then the GIVEN branch sequence b_0 .. b_{iters-1} ('the same for
+                  each subgraph expansion' - the sequence is a global quantity, so it is an input here), and the
+                  core columns of the result (Eq.(6)).
+    The global quantities a single community cannot produce (eps_min/eps_max, A) are computed once from the whole H."""
+
+    def __init__(self, H, tau: float, part, bounds: tuple[float, float] | None = None):
+        if not (tau >= 0):
+            raise ValueError("tau must be >= 0")
+        self.H, self.tau, self.part = H, float(tau), np.asarray(part)
+        self.lo, self.hi = bounds if bounds is not None else gershgorin(H)
+        self.A = _threshold(normalised_x0(H, self.lo, self.hi), tau)
+        self.A_csc = self.A.tocsc()
+        self.Hs = sp.csr_matrix((H.val, H.col_idx, H.row_ptr), shape=(H.n, H.n))
+
+    def subgraph(self, p: int):
+        """(idx int32, ncore) of community p, from the rows and columns C_p of S."""
+        core = np.nonzero(self.part == p)[0]
+        if core.size == 0:
+            return np.zeros(0, dtype=np.int32), 0
+        A_rows = self.A[core, :]                                        # A[C_p, :]
+        A_cols = self.A_csc[:, core]                                    # A[:, C_p]
+        AA_rows = _threshold(sp.csr_matrix(A_rows @ self.A), self.tau)  # floor(A A)_tau, rows C_p
+        AA_cols = _threshold(sp.csr_matrix(self.A @ A_cols), self.tau)  # floor(A A)_tau, columns C_p
+        reached = [core, A_rows.tocoo().col, AA_rows.tocoo().col, A_cols.tocoo().row, AA_cols.tocoo().row]
+        allv = np.unique(np.concatenate(reached))
+        halo = np.setdiff1d(allv, core)
+        return np.concatenate([core, halo]).astype(np.int32), int(core.size)
+
+    def expand(self, p: int, branch, iters: int):
+        """(idx, ncore, X[:, :ncore]) after `iters` SP2 steps with the given branches (0: X^2, 1: 2X - X^2)."""
+        idx, nc = self.subgraph(p)
+        X = dense_block(self.Hs, idx, self.lo, self.hi)
+        for n in range(iters):
+            Y = X @ X
+            X = Y if int(branch[n]) == 0 else 2.0 * X - Y
+        return idx, nc, X[:, :nc]
+
+
+# ----------------------------------------------------------------------------------------
 # finite-temperature expansion, Eq.(7)
 # ----------------------------------------------------------------------------------------
 def fermi_chebyshev_coeffs(mu: float, beta: float, order: int, eps_min: float, eps_max: float, nq: int = 2048) -> np.ndarray:

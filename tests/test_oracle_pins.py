@@ -535,3 +535,48 @@ def test_o_fermi_reaches_the_zero_temperature_projector_and_respects_the_graph()
     assert np.array_equal(rf.D_row_ptr, rs.D_row_ptr) and np.array_equal(rf.D_col, rs.D_col)
     assert np.abs(rf.D_val - rs.D_val).max() < 1e-6
     assert abs(rf.n_elec - rs.t1[-1]) < 1e-5
+
+
+# ----------------------------------------------------------------------------- one community at a time
+@pytest.mark.parametrize("tau", [0.2, 1e-2, 1e-4])
+def test_one_community_brute_force(tau):
+    """OneCommunity against explicit loops: the subgraph from the brute-force edge set of A-1 (no sparse library, no
+    matmul) and the expansion of the dense principal submatrix with the given branches by triple loops."""
+    s = gi.random_banded(14, half_bw=2, n_part=4, seed=11, shuffle=True)
+    Hd = s.H.to_dense()
+    n = s.n
+    edges = brute_graph(Hd, tau, 2)
+    lo = min(Hd[i, i] - sum(abs(Hd[i, j]) for j in range(n) if j != i) for i in range(n))
+    hi = max(Hd[i, i] + sum(abs(Hd[i, j]) for j in range(n) if j != i) for i in range(n))
+    branch = [1, 0, 0, 1, 1]
+    oc = o.OneCommunity(s.H, tau, s.part)
+    for p in range(s.n_part):
+        core = [i for i in range(n) if s.part[i] == p]
+        halo = sorted({k for i in core for k in range(n) if (k, i) in edges} - set(core))
+        idx, nc, cols = oc.expand(p, branch, len(branch))
+        assert list(idx) == core + halo and nc == len(core)
+        sidx = core + halo
+        m = len(sidx)
+        X = [[((hi if a == b else 0.0) - Hd[sidx[a], sidx[b]]) / (hi - lo) for b in range(m)] for a in range(m)]
+        for b_n in branch:
+            Y = [[sum(X[a][k] * X[k][b] for k in range(m)) for b in range(m)] for a in range(m)]
+            X = Y if b_n == 0 else [[2.0 * X[a][b] - Y[a][b] for b in range(m)] for a in range(m)]
+        want = np.array(X).reshape(m, m)[:, :nc]
+        assert np.abs(cols - want).max() <= 1e-13
+
+
+@pytest.mark.parametrize("system", ["chain", "water", "shuffled"])
+def test_one_community_equals_the_whole_batch(system):
+    """Every community of a small system, one at a time with the sequence the whole batch chose, reproduces o_sub's block:
+    same subgraph (bit for bit) and the same core columns."""
+    s = {"chain": lambda: gi.config(1),
+         "water": lambda: gi.water_box(48, 6, seed=2, tau=1e-4, iters=12),
+         "shuffled": lambda: gi.random_banded(120, half_bw=4, n_part=5, seed=4, tau=1e-3, iters=10, shuffle=True)}[system]()
+    rp, ci = o.build_graph(s.H, s.tau)
+    r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, s.iters, keep_blocks=True)
+    oc = o.OneCommunity(s.H, s.tau, s.part)
+    assert (oc.lo, oc.hi) == (r.eps_min, r.eps_max)
+    for p in range(s.n_part):
+        idx, nc, cols = oc.expand(p, r.branch, r.iters_done)
+        assert np.array_equal(idx, r.subs[p][0]) and nc == r.subs[p][1]
+        assert np.abs(cols - r.blocks[p][:, :nc]).max() <= 1e-14
