@@ -197,21 +197,43 @@ def check_any_size_properties(s, g, ex, Dg, log):
     assert D.nnz <= g.info["nnz_D"]
 
 
+def check_sampled_communities(s, ex, Dg, log, n_random):
+    """Sampled outputs the oracle can compute one by one at any size: for the largest, the smallest and a few random
+    communities the oracle derives the subgraph from (H, tau) alone and expands it with the branch sequence the GPU
+    logged (the sequence is a global quantity: P:L90); subgraph indices bit for bit, every stored entry of D in the
+    community's core columns within the 1e-10 bar."""
+    oc = o.OneCommunity(s.H, s.tau, s.part)
+    m = np.diff(ex["sub_ptr"])
+    rng = np.random.default_rng(1)
+    picks = {int(np.argmax(m)), int(np.argmin(np.where(m > 0, m, m.max())))}
+    picks |= {int(p) for p in rng.choice(s.n_part, size=min(n_random, s.n_part), replace=False)}
+    D = sp.csr_matrix((Dg, ex["D_col"], ex["D_row_ptr"]), shape=(s.n, s.n))
+    for p in sorted(picks):
+        idx, nc, cols = oc.expand(p, log.branch, log.iters_done)
+        a, b = ex["sub_ptr"][p], ex["sub_ptr"][p + 1]
+        assert np.array_equal(ex["sub_idx"][a:b], idx) and ex["ncore"][p] == nc
+        got = D[idx][:, idx[:nc]].toarray()
+        assert np.abs(got - cols).max() <= TOL_D, (p, len(idx))
+
+
 @pytest.mark.slow
 def test_config4_full_size_properties(gbe):
     """BASELINE.json configs[3] at full size (2,000 residues, ~1.2e5 orbitals, 2 x 27 GB dense batch).  The oracle would
-    need ~1e15 flop here, so the full-size run is checked through properties that hold at any size; element-by-element
-    parity of the same construction is test_config4_reduced_peptide_heterogeneous_sizes."""
+    need ~1e15 flop for the whole batch, so the full-size run is checked (1) through properties that hold at any size and
+    (2) element by element on sampled communities the oracle computes one at a time; element-by-element parity of the
+    whole batch for the same construction is test_config4_reduced_peptide_heterogeneous_sizes."""
     s = gi.config(4)
     g, ex, Dg, log = run_gpu(gbe, s)
     assert g.info["n"] == s.n and g.info["max_m"] > 1500
     check_any_size_properties(s, g, ex, Dg, log)
+    check_sampled_communities(s, ex, Dg, log, n_random=4)
 
 
 def test_any_size_properties_hold_where_parity_is_known(gbe):
     s = gi.config(2)
     g, ex, Dg, log = run_gpu(gbe, s)
     check_any_size_properties(s, g, ex, Dg, log)
+    check_sampled_communities(s, ex, Dg, log, n_random=2)
 
 
 # ------------------------------------------------------------------------------- pieces
