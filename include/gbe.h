@@ -154,6 +154,15 @@ int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, 
  * reproducible.  Not thread safe against concurrent calls on the same graph. */
 int gbe_graph_set_sp2_path(gbe_graph* g, int32_t path);
 
+/* Which kernel packs the dense blocks (step 3).  Two variants compute the same x_p = X0[s_p, s_p]:
+ *   staged  each warp builds an output row in a shared-memory row buffer and streams it out once;
+ *   direct  the row is zero-filled and the stored entries are stored straight to global memory (no row buffer: for
+ *           large systems, where the index bitmaps over the n vertices and row buffers of max_m doubles would leave one
+ *           CTA per SM).
+ * path = 0 (default): staged while three CTAs with their row buffers fit an SM, else direct; 1: staged; 2: direct.
+ * The dense blocks of the two are bit-identical; the traces of X_0 are summed in a different order (agree to rounding). */
+int gbe_graph_set_gather_path(gbe_graph* g, int32_t path);
+
 /* Steps 0 and 3-6: D = P_tau(H) on the pattern fixed by the graph (Eq.(6)).
  *   H         device CSR; values AND pattern may differ from the H the graph was built from (MD use):
  *             H values are looked up at gather time, entries outside a subgraph are simply not gathered.

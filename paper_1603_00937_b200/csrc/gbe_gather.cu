@@ -11,11 +11,16 @@
 // and streams it out with 128-bit stores, so every output byte is written exactly once, fully coalesced.
 // The epilogue accumulates the traces of X_0 and X_0^2 over the core rows (t1, t2 of iteration 0):
 // (X^2)_ii = sum_c X_ic^2 for symmetric X.
+// DIRECT variant (large systems: the bitmaps of ~1e5 vertices plus row buffers of ~2,400 doubles leave one CTA per SM):
+// no row buffer - the warp zero-fills the output row in global memory with 128-bit stores and then stores the stored
+// entries straight to it (L2 merges the two before the line leaves for DRAM), so the CTA needs the bitmaps only and
+// three CTAs fit an SM.  The traces are then summed over the stored entries as they are placed.
 // Bound: HBM - writes 8 m_p^2 B per community, reads 12 B per stored entry of every gathered H row.
 #include "gbe_internal.cuh"
 
 namespace {
 
+template <bool DIRECT>
 __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_per_cta, const int2* __restrict__ gitems,
                                                 const int64_t* __restrict__ H_rp, const int32_t* __restrict__ H_col,
                                                 const double* __restrict__ H_val, int64_t n,
@@ -85,7 +90,7 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   }
   __syncthreads();
 
-  double* buf = rowbuf + (size_t)wid * ldmax;
+  double* buf = DIRECT ? nullptr : rowbuf + (size_t)wid * ldmax;
   double* Xp = X + dense_off[p];
   double s1 = 0.0, s2 = 0.0;
   const int rend = min(m, r0 + rows_per_cta);
@@ -100,6 +105,9 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
       v[u] = e < end ? H_val[e] : 0.0;
     }
   };
+  double* out = nullptr;     // DIRECT: the output row being built
+  double q = 0.0, dg = 0.0;  // DIRECT: this lane's sum of squares of the row, and the stored diagonal if it placed it
+  bool dseen = false;
   auto place = [&](int k, const int (&j)[4], const double (&v)[4]) {
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
@@ -114,7 +122,16 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
         const uint32_t hw = halob[wj];
         if (hw & bit) c = nc + halork[wj] + __popc(hw & (bit - 1u));
       }
-      if (c >= 0) buf[c] = div_delta((col == k ? eps_max : 0.0) - v[u]);
+      if (c >= 0) {
+        const double x = div_delta((col == k ? eps_max : 0.0) - v[u]);
+        if (DIRECT) {
+          out[c] = x;
+          q += x * x;
+          if (col == k) { dseen = true; dg = x; }
+        } else {
+          buf[c] = x;
+        }
+      }
     }
   };
   int r = r0 + wid;
@@ -135,10 +152,17 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
       a1 = H_rp[k1];
       b1 = H_rp[k1 + 1];
     }
-    for (int c = lane * 2; c < ld; c += 64) *reinterpret_cast<double2*>(buf + c) = make_double2(0.0, 0.0);
-    __syncwarp();
-    if (lane == 0) buf[r] = div_delta(eps_max - 0.0);  // a stored diagonal overwrites this below
-    __syncwarp();
+    double* const zrow = DIRECT ? Xp + (size_t)r * ld : buf;
+    for (int c = lane * 2; c < ld; c += 64) *reinterpret_cast<double2*>(zrow + c) = make_double2(0.0, 0.0);
+    __syncwarp();  // orders the zero fill before the entries other lanes store into the same row
+    if (DIRECT) {
+      out = zrow;
+      q = 0.0;
+      dseen = false;
+    } else {
+      if (lane == 0) buf[r] = div_delta(eps_max - 0.0);  // a stored diagonal overwrites this below
+      __syncwarp();
+    }
     for (int64_t base = a0; base < b0; base += 128) {
       if (base + 128 < b0) fetch(base + 128, b0, nj, nv);        // rest of a long row
       else if (has1) fetch(a1, b1, nj, nv);                      // first entries of the next row
@@ -147,19 +171,32 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
       for (int u = 0; u < 4; ++u) { cj[u] = nj[u]; cv[u] = nv[u]; }
     }
     if (a0 >= b0 && has1) fetch(a1, b1, cj, cv);                 // empty row: nothing was prefetched above
-    __syncwarp();
-    double* out = Xp + (size_t)r * ld;
-    double q = 0.0;
-    for (int c = lane * 2; c < ld; c += 64) {
-      const double2 v = *reinterpret_cast<const double2*>(buf + c);
-      *reinterpret_cast<double2*>(out + c) = v;
-      q += v.x * v.x + v.y * v.y;
+    if (DIRECT) {
+      if (!__any_sync(0xffffffffu, dseen) && lane == 0) {  // H_kk is not stored: it is zero (A-12)
+        dg = div_delta(eps_max - 0.0);
+        out[r] = dg;
+        q += dg * dg;
+        dseen = true;
+      }
+      if (r < nc) {  // warp-uniform
+        s2 += q;
+        if (dseen) s1 += dg;
+      }
+    } else {
+      __syncwarp();
+      double* orow = Xp + (size_t)r * ld;
+      double qq = 0.0;
+      for (int c = lane * 2; c < ld; c += 64) {
+        const double2 v = *reinterpret_cast<const double2*>(buf + c);
+        *reinterpret_cast<double2*>(orow + c) = v;
+        qq += v.x * v.x + v.y * v.y;
+      }
+      if (r < nc) {  // warp-uniform
+        s2 += qq;
+        if (lane == 0) s1 += buf[r];
+      }
+      __syncwarp();
     }
-    if (r < nc) {  // warp-uniform
-      s2 += q;
-      if (lane == 0) s1 += buf[r];
-    }
-    __syncwarp();
     k0 = k1; k1 = k2; a0 = a1; b0 = b1;
   }
   s1 = warp_sum(s1);
@@ -183,13 +220,25 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
   const int ldmax = (g->max_m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
   const size_t fixed = (size_t)4 * W * 4 + 516 * 4 + 16 * 8;
   const size_t budget = 220 * 1024;
-  if (fixed + (size_t)ldmax * 8 > budget) return GBE_EINVAL;
-  int nw = (int)std::min<size_t>(8, (budget - fixed) / ((size_t)ldmax * 8));
-  const size_t smem = fixed + (size_t)nw * ldmax * 8;
-  GBE_CUDA(cudaFuncSetAttribute(k_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  GBE_CUDA(cudaFuncSetAttribute(k_gather, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-  k_gather<<<g->n_gitems, nw * 32, smem, s>>>(W, ldmax, g->gather_rows, g->gitems, H.row_ptr, H.col_idx, H.val, g->n,
-                                              g->sub_ptr, g->sub_idx, g->ncore, g->dense_off, st, X, partials);
+  // staged: one row buffer per warp in shared memory; direct: none.  Auto: staged while three CTAs of eight warps still
+  // fit an SM with their row buffers (measured: 82 % of the copy bandwidth on the 24,576-orbital box), else direct.
+  const size_t staged8 = fixed + (size_t)8 * ldmax * 8;
+  bool direct = g->gather_path == 2 || (g->gather_path == 0 && 3 * (staged8 + 1024) > 227 * 1024);
+  if (!direct && fixed + (size_t)ldmax * 8 > budget) direct = true;  // not even one row buffer fits
+  if (fixed > budget) return GBE_EINVAL;
+  if (direct) {
+    GBE_CUDA(cudaFuncSetAttribute(k_gather<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fixed));
+    GBE_CUDA(cudaFuncSetAttribute(k_gather<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    k_gather<true><<<g->n_gitems, 256, fixed, s>>>(W, ldmax, g->gather_rows, g->gitems, H.row_ptr, H.col_idx, H.val, g->n,
+                                                   g->sub_ptr, g->sub_idx, g->ncore, g->dense_off, st, X, partials);
+  } else {
+    const int nw = (int)std::min<size_t>(8, (budget - fixed) / ((size_t)ldmax * 8));
+    const size_t smem = fixed + (size_t)nw * ldmax * 8;
+    GBE_CUDA(cudaFuncSetAttribute(k_gather<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    GBE_CUDA(cudaFuncSetAttribute(k_gather<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    k_gather<false><<<g->n_gitems, nw * 32, smem, s>>>(W, ldmax, g->gather_rows, g->gitems, H.row_ptr, H.col_idx, H.val,
+                                                       g->n, g->sub_ptr, g->sub_idx, g->ncore, g->dense_off, st, X, partials);
+  }
   GBE_LAUNCHED();
   return GBE_OK;
 }

@@ -112,6 +112,8 @@ struct gbe_graph {
   int32_t* row_nc = nullptr;     // sum_m: ncore of the community of dense row q
   // SP2 path: 0 auto, 1 tiled kernels (gbe_x2.cu), 2 resident kernel (gbe_resident.cu); set by gbe_graph_set_sp2_path
   int32_t sp2_path = 0;
+  // gather path: 0 auto, 1 staged (row buffer in shared memory), 2 direct (rows built in global memory); gbe_graph_set_gather_path
+  int32_t gather_path = 0;
   int32_t resident_fits = 0, resident_coresident = 0;  // gbe_resident_capacity at build time
   int32_t resident_cluster = 0;  // 1: all communities fit ONE thread-block cluster (<= 16): exchange through DSMEM
   gbe_tile_item* items = nullptr;

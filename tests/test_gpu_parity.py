@@ -29,8 +29,9 @@ def gbe():
     return pkg
 
 
-def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None, sp2_path=0):
-    """sp2_path: 0 = the library's choice, 1 = tiled kernels, 2 = shared-memory-resident kernel (include/gbe.h)."""
+def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None, sp2_path=0, gather_path=0):
+    """sp2_path: 0 = the library's choice, 1 = tiled kernels, 2 = shared-memory-resident kernel (include/gbe.h);
+    gather_path: 0 = the library's choice, 1 = staged through shared memory, 2 = direct to global memory."""
     import torch
     Hd = gbe.DeviceCSR.from_host(s.H if H is None else H)
     part_t = None if part is None else torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
@@ -38,6 +39,8 @@ def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None, sp
     if sp2_path:
         gbe.gbe_graph_set_sp2_path(g, sp2_path)
         assert g.info["resident_sp2"] == (1 if sp2_path == 2 else 0)
+    if gather_path:
+        gbe.gbe_graph_set_gather_path(g, gather_path)
     D, log = gbe.gbe_density(Hd, g, s.n_occ, s.iters if iters is None else iters, idem_tol)
     torch.cuda.synchronize()
     ex = {k: v.cpu().numpy() for k, v in g.export().items()}
@@ -237,6 +240,25 @@ def test_any_size_properties_hold_where_parity_is_known(gbe):
 
 
 # ------------------------------------------------------------------------------- pieces
+@pytest.mark.parametrize("which", ["chain", "water", "shuffled", "peptide"])
+def test_gather_paths_pack_identical_blocks(gbe, which):
+    """The staged and the direct gather kernel (include/gbe.h, gbe_graph_set_gather_path): with iters = 0 the result is
+    the gathered X0 itself, which must agree bit for bit; the traces of X_0 are summed in another order (rounding);
+    the full expansion through the direct kernel meets the same bar against the oracle."""
+    s = {"chain": lambda: gi.config(1),
+         "water": lambda: gi.water_box(256, 32, seed=3, tau=1e-5, iters=12),
+         "shuffled": lambda: gi.random_banded(300, half_bw=6, n_part=9, seed=5, tau=1e-4, iters=20, shuffle=True),
+         "peptide": lambda: gi.peptide_water(40, box=20.0, seed=2)}[which]()
+    _, _, D1, log1 = run_gpu(gbe, s, iters=0, gather_path=1)
+    _, _, D2, log2 = run_gpu(gbe, s, iters=0, gather_path=2)
+    assert np.array_equal(D1, D2)
+    assert abs(log1.t1[0] - log2.t1[0]) <= 1e-12 * s.n and abs(log1.t2[0] - log2.t2[0]) <= 1e-12 * s.n
+    g, ex, Dg, log = run_gpu(gbe, s, gather_path=2)
+    graph, r = run_oracle(s)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+
+
 @pytest.mark.parametrize("sp2_path", [1, 2])
 def test_iters_zero_returns_gathered_x0(gbe, sp2_path):
     """gather + scatter alone: D = core columns of X0[s,s]; exact up to the rounding of the two bounds."""
@@ -514,13 +536,14 @@ def test_single_vertex_cores_and_empty_partitions(gbe):
     assert (ex["ncore"][1::2] == 0).all()
 
 
-def test_missing_diagonal_entries(gbe):
+@pytest.mark.parametrize("gather_path", [1, 2])
+def test_missing_diagonal_entries(gbe, gather_path):
     s = gi.random_banded(64, half_bw=3, n_part=4, seed=8, tau=1e-3, iters=25)
     a = s.H.to_dense()
     a[np.arange(0, 64, 3), np.arange(0, 64, 3)] = 0.0  # not stored -> H_kk = 0 (A-12)
     H = gi.CSR.from_dense(a)
     assert H.nnz < s.H.nnz
-    g, ex, Dg, log = run_gpu(gbe, s, H=H)
+    g, ex, Dg, log = run_gpu(gbe, s, H=H, gather_path=gather_path)
     graph, r = run_oracle(s, H=H)
     check_structure(ex, graph, r, g.info)
     check_density(Dg, log, r)
