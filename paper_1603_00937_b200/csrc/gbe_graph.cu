@@ -72,65 +72,71 @@ __global__ void __launch_bounds__(256) k_materialise_A(int64_t n, const int64_t*
 
 // ---------------------------------------------------------------- T_next = floor(A T)_tau
 // Walks every product a_ik * t_kj of row i (k ascending; the entries of one T row spread over the lanes) and calls
-// fn(aik, j, t_kj).  The kernels around it are latency bound (a few warps per SM, dependent loads), so the walk is
-// software pipelined: the row pointers of 32 neighbours k are fetched by the 32 lanes at once, and the up to 128
-// entries of the NEXT chunk (same k or the next one) are in flight while the current chunk is processed.
-// ORDERED: a __syncwarp separates consecutive k, because the next k may hit the accumulator slots of this one.
+// fn(aik, j[4], t_kj[4]) once per ROUND of up to 128 entries of one T row (4 per lane; j = -1 marks an empty slot).
+// The kernels around it are bound by instruction issue and by the latency of dependent loads from L2 (ncu: the
+// integer and branch instructions around each product were ~10 times the useful ones), so the walk is written to
+// be cheap and flat: the 32 lanes fetch the row pointers of 32 neighbours k at once (and the neighbour indices of
+// the NEXT 32 while these are walked); a warp scan numbers the rounds of the 32 T rows, so that round r is located
+// with one ballot and two shuffles instead of a search loop; each round costs one 64-bit address per array and
+// predicated loads at immediate offsets with 32-bit bounds; the loads of round r + 1 are in flight while round r is
+// processed.  ORDERED: a __syncwarp follows every round, because the next k may hit the accumulator slots of this one.
 template <bool NEED_VAL, bool ORDERED, typename F>
 __device__ __forceinline__ void walk_products(int lane, int64_t a, int64_t b, const int32_t* __restrict__ A_col,
                                               const double* __restrict__ A_val, const int64_t* __restrict__ T_rp,
                                               const int32_t* __restrict__ T_col, const double* __restrict__ T_val,
                                               F&& fn) {
   constexpr unsigned FULL = 0xffffffffu;
+  struct Buf {
+    int j[4];
+    double v[4];
+    int q;
+  };
+  int kk_n = a + lane < b ? A_col[a + lane] : -1;
+  double av_n = (NEED_VAL && a + lane < b) ? A_val[a + lane] : 0.0;
   for (int64_t e0 = a; e0 < b; e0 += 32) {
-    const int64_t e = e0 + lane;
-    const int nk = (int)min((int64_t)32, b - e0);
-    const int kk = e < b ? A_col[e] : 0;
-    const double av = (NEED_VAL && e < b) ? A_val[e] : 0.0;
-    const int64_t tb_l = e < b ? T_rp[kk] : 0;
-    const int64_t te_l = e < b ? T_rp[kk + 1] : 0;
-    int cj[4], nj[4];
-    double cv[4], nv[4];
-    auto fetch = [&](int64_t base, int64_t end, int (&j)[4], double (&v)[4]) {
+    const int kk = kk_n;
+    const double av = av_n;
+    const int64_t tb_l = kk >= 0 ? T_rp[kk] : 0;
+    const int64_t te_l = kk >= 0 ? T_rp[kk + 1] : 0;
+    {  // neighbour indices of the next 32: in flight during this block
+      const int64_t en = e0 + 32 + lane;
+      kk_n = en < b ? A_col[en] : -1;
+      if (NEED_VAL) av_n = en < b ? A_val[en] : 0.0;
+    }
+    const int len_l = (int)(te_l - tb_l);
+    const int rounds_l = (len_l + 127) >> 7;
+    int R;
+    const int ex_l = warp_excl_scan_i(rounds_l, lane, &R);
+    const int cum_l = ex_l + rounds_l;
+    const int64_t tbx_l = tb_l - ((int64_t)ex_l << 7);  // round r of this k starts at tbx + 128 r ...
+    const int lenx_l = len_l + (ex_l << 7);              // ... and holds the entries below lenx - 128 r
+    auto load = [&](int r, Buf& B) {
+      const int q = __ffs(__ballot_sync(FULL, cum_l > r)) - 1;  // the first k whose rounds end beyond r owns round r
+      const int64_t first = __shfl_sync(FULL, tbx_l, q) + ((int64_t)r << 7) + lane;
+      const int left = __shfl_sync(FULL, lenx_l, q) - (r << 7) - lane;  // entries from this lane's first one on
+      B.q = q;
+      const int32_t* __restrict__ cp = T_col + first;
+      const double* __restrict__ vp = T_val + first;
 #pragma unroll
-      for (int r = 0; r < 4; ++r) {
-        const int64_t f = base + lane + 32 * r;
-        j[r] = f < end ? T_col[f] : -1;
-        if (NEED_VAL) v[r] = f < end ? T_val[f] : 0.0;
+      for (int u = 0; u < 4; ++u) {
+        B.j[u] = 32 * u < left ? cp[32 * u] : -1;
+        if (NEED_VAL) B.v[u] = 32 * u < left ? vp[32 * u] : 0.0;
       }
     };
-    // first non-empty chunk
-    int q = 0;
-    int64_t base = 0, end = 0;
-    while (q < nk) {
-      base = __shfl_sync(FULL, tb_l, q);
-      end = __shfl_sync(FULL, te_l, q);
-      if (base < end) break;
-      ++q;
+    auto process = [&](const Buf& B) {
+      const double aik = NEED_VAL ? __shfl_sync(FULL, av, B.q) : 0.0;
+      fn(aik, B.j, B.v);
+      if (ORDERED) __syncwarp();
+    };
+    Buf b0, b1;
+    if (0 < R) load(0, b0);
+    for (int r = 0; r < R; r += 2) {
+      if (r + 1 < R) load(r + 1, b1);
+      process(b0);
+      if (r + 1 >= R) break;
+      if (r + 2 < R) load(r + 2, b0);
+      process(b1);
     }
-    if (q < nk) fetch(base, end, cj, cv);
-    while (q < nk) {
-      // locate and prefetch the next chunk
-      int nq = q;
-      int64_t nbase = base + 128, nend = end;
-      while (nbase >= nend) {
-        if (++nq >= nk) break;
-        nbase = __shfl_sync(FULL, tb_l, nq);
-        nend = __shfl_sync(FULL, te_l, nq);
-      }
-      if (nq < nk) fetch(nbase, nend, nj, nv);
-      const double aik = NEED_VAL ? __shfl_sync(FULL, av, q) : 0.0;
-#pragma unroll
-      for (int r = 0; r < 4; ++r)
-        if (cj[r] >= 0) fn(aik, cj[r], cv[r]);
-      if (ORDERED && nq != q) __syncwarp();
-#pragma unroll
-      for (int r = 0; r < 4; ++r) { cj[r] = nj[r]; if (NEED_VAL) cv[r] = nv[r]; }
-      q = nq;
-      base = nbase;
-      end = nend;
-    }
-    if (ORDERED) __syncwarp();
   }
 }
 
@@ -144,7 +150,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
                                    const int64_t* __restrict__ T_rp, const int32_t* __restrict__ T_col,
                                    const double* __restrict__ T_val, double tau, int32_t* __restrict__ cnt,
                                    const int64_t* __restrict__ out_rp, int32_t* __restrict__ out_col,
-                                   double* __restrict__ out_val) {
+                                   double* __restrict__ out_val, uint32_t* __restrict__ bm_io) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, w_in_blk = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const size_t per_warp = (size_t)W * 8 + ((MODE == 0 || MODE == 4) ? 0 : (size_t)cap * 8);
@@ -154,17 +160,29 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
   uint32_t* rk = bm + W;
 
   for (int64_t i = (int64_t)blockIdx.x * nw + w_in_blk; i < n; i += (int64_t)gridDim.x * nw) {
-    for (int w = lane; w < W; w += 32) bm[w] = 0u;
-    __syncwarp();
     const int64_t a = A_rp[i], b = A_rp[i + 1];
     // pass 1: mark candidate columns
     // upper_only: the product is A A with A symmetric, so (A A)_ij == (A A)_ji bit for bit (k ascending, the two
     // factors of every product commute) and only the columns j >= i are formed; S u S^T restores the rest
     const int jmin = upper_only ? (int)i : 0;
-    walk_products<false, false>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, [&](double, int j, double) {
-      if (j >= jmin) atomicOr(&bm[j >> 5], 1u << (j & 31));
-    });
+    // bm_io: MODE 0 (the sizing pass) leaves its candidate bitmaps there and the later modes of the same product
+    // read them back (W coalesced words per row) instead of walking the products a second time
+    const bool reload = MODE != 0 && bm_io != nullptr;
+    if (reload) {
+      for (int w = lane; w < W; w += 32) bm[w] = bm_io[(size_t)i * W + w];
+    } else {
+    for (int w = lane; w < W; w += 32) bm[w] = 0u;
     __syncwarp();
+    walk_products<false, false>(lane, a, b, A_col, A_val, T_rp, T_col, T_val,
+                                [&](double, const int (&j)[4], const double (&)[4]) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (j[u] >= jmin) atomicOr(&bm[j[u] >> 5], 1u << (j[u] & 31));  // an empty slot is -1 < jmin
+    });
+    }
+    __syncwarp();
+    if (MODE == 0 && bm_io != nullptr)
+      for (int w = lane; w < W; w += 32) bm_io[(size_t)i * W + w] = bm[w];
     // compact slot index: rk[w] = number of candidates in words < w
     int running = 0;
     for (int w0 = 0; w0 < W; w0 += 32) {
@@ -194,11 +212,24 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
     for (int s = lane; s < running; s += 32) acc[s] = 0.0;
     __syncwarp();
     // pass 2: accumulate, k ascending, multiply and add separately rounded
-    walk_products<true, true>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, [&](double aik, int j, double t) {
-      if (j < jmin) return;
-      const uint32_t word = bm[j >> 5];
-      const int slot = rk[j >> 5] + __popc(word & ((1u << (j & 31)) - 1u));
-      acc[slot] = __dadd_rn(acc[slot], __dmul_rn(aik, t));
+    // branch free, the four entries of a lane as independent chains (the columns of one T row are distinct, so
+    // their slots are): entries that do not count (empty, or j < jmin) go to the spare slot cap - 1
+    walk_products<true, true>(lane, a, b, A_col, A_val, T_rp, T_col, T_val,
+                              [&](double aik, const int (&j)[4], const double (&t)[4]) {
+      int slot[4];
+      double o[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const bool ok = j[u] >= jmin;
+        const int jj = ok ? j[u] : 0;
+        const uint32_t word = bm[jj >> 5];
+        const int sl = rk[jj >> 5] + __popc(word & ((1u << (jj & 31)) - 1u));
+        slot[u] = ok ? sl : cap - 1;
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) o[u] = acc[slot[u]];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) acc[slot[u]] = __dadd_rn(o[u], __dmul_rn(aik, t[u]));
     });
     // emit kept entries in ascending column order
     int kept = 0;
@@ -468,6 +499,12 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   const int64_t* T_rp = A.rp.as<int64_t>();
   const int32_t* T_col = A.col.as<int32_t>();
   const double* T_val = A.val.as<double>();
+  // candidate bitmaps of the sizing pass, kept for the numeric passes of the same product (n * W words: only while
+  // that is a small part of the device memory - beyond it the numeric passes walk the products again)
+  DevBuf bmsave;
+  constexpr size_t BM_SAVE_MAX = (size_t)8 << 30;
+  if ((size_t)n * W * 4 <= BM_SAVE_MAX && power >= 2) GBE_TRY(bmsave.alloc((size_t)n * W * 4));
+  uint32_t* const bm_io = bmsave.as<uint32_t>();
   for (int k = 2; k <= power; ++k) {
     // A A with symmetric A is symmetric bit for bit: when it is the LAST power only its upper triangle is formed
     const int upper_only = (k == 2 && power == 2) ? 1 : 0;
@@ -480,7 +517,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
       const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
       k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, upper_only, A.rp.as<int64_t>(),
                                                                  A.col.as<int32_t>(), A.val.as<double>(), T_rp, T_col, T_val, tau,
-                                                                 cnt.as<int32_t>(), nullptr, nullptr, nullptr);
+                                                                 cnt.as<int32_t>(), nullptr, nullptr, nullptr, bm_io);
       GBE_LAUNCHED();
     }
     std::vector<int32_t> h_cnt((size_t)n);
@@ -488,7 +525,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     GBE_CUDA(cudaStreamSynchronize(s));
     int cap = 1;
     for (int64_t i = 0; i < n; ++i) cap = std::max(cap, h_cnt[(size_t)i]);
-    cap = (cap + 1) & ~1;
+    cap = ((cap + 1) & ~1) + 2;  // + the spare slot that takes the entries that do not count
     const size_t per_warp = (size_t)W * 8 + (size_t)cap * 8;
     const int nw = pick_warps(per_warp, 16);
     if (nw < 1) return GBE_EINVAL;
@@ -505,7 +542,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
       k_spgemm_threshold<3><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, upper_only, A.rp.as<int64_t>(),
                                                                  A.col.as<int32_t>(), A.val.as<double>(), T_rp, T_col, T_val, tau,
                                                                  cnt.as<int32_t>(), Tc.rp.as<int64_t>(),
-                                                                 Tc.col.as<int32_t>(), nullptr);
+                                                                 Tc.col.as<int32_t>(), nullptr, bm_io);
       GBE_LAUNCHED();
       Pattern Pn;
       GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tc.rp.as<int64_t>(), Tc.col.as<int32_t>(),
@@ -519,7 +556,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     Pattern Tn;
     k_spgemm_threshold<1><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, 0, A.rp.as<int64_t>(), A.col.as<int32_t>(),
                                                                A.val.as<double>(), T_rp, T_col, T_val, tau,
-                                                               cnt.as<int32_t>(), nullptr, nullptr, nullptr);
+                                                               cnt.as<int32_t>(), nullptr, nullptr, nullptr, bm_io);
     GBE_LAUNCHED();
     GBE_TRY(count_to_rowptr(cnt, n, Tn.rp, &Tn.nnz, s));
     GBE_TRY(Tn.col.alloc((size_t)Tn.nnz * 4));
@@ -527,7 +564,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     k_spgemm_threshold<2><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, 0, A.rp.as<int64_t>(), A.col.as<int32_t>(),
                                                                A.val.as<double>(), T_rp, T_col, T_val, tau, nullptr,
                                                                Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(),
-                                                               Tn.val.as<double>());
+                                                               Tn.val.as<double>(), bm_io);
     GBE_LAUNCHED();
     Pattern Pn;
     GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(), nullptr, 0, Pn));
@@ -576,16 +613,19 @@ int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int3
   GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
   GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
   const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
+  DevBuf bmsave;  // candidate bitmaps of the counting pass, read back by the emitting pass
+  if ((size_t)n * W * 4 <= ((size_t)8 << 30)) GBE_TRY(bmsave.alloc((size_t)n * W * 4));
+  uint32_t* const bm_io = bmsave.as<uint32_t>();
   k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, 0, M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr,
                                                              M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr, 0.0,
-                                                             cnt.as<int32_t>(), nullptr, nullptr, nullptr);
+                                                             cnt.as<int32_t>(), nullptr, nullptr, nullptr, bm_io);
   GBE_LAUNCHED();
   Pattern P;
   GBE_TRY(count_to_rowptr(cnt, n, P.rp, &P.nnz, s));
   GBE_TRY(P.col.alloc((size_t)P.nnz * 4));
   k_spgemm_threshold<4><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, 0, M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr,
                                                              M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr, 0.0, nullptr,
-                                                             P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr);
+                                                             P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr, bm_io);
   GBE_LAUNCHED();
   Pattern S;
   GBE_TRY(symmetrise(P, U, cnt, S));
