@@ -159,11 +159,23 @@ __global__ void k_d_pattern(int64_t n, int W, const int64_t* __restrict__ memb_p
     for (int w = lane; w < W; w += 32) bm[w] = 0u;
     __syncwarp();
     const int64_t mb = memb_ptr[k], me = memb_ptr[k + 1];
-    for (int64_t x = mb; x < me; ++x) {
-      const int p = row_part[memb[x]];
-      const int64_t sb = sub_ptr[p];
-      const int nc = ncore[p];
-      for (int c = lane; c < nc; c += 32) { const int i = sub_idx[sb + c]; atomicOr(&bm[i >> 5], 1u << (i & 31)); }
+    // the communities that contain row k: their metadata is fetched by the lanes side by side (one chain of
+    // dependent loads per 32 members instead of one per member) and handed round by shuffle
+    for (int64_t x0 = mb; x0 < me; x0 += 32) {
+      const int64_t xl = x0 + lane;
+      int64_t sb_l = 0;
+      int nc_l = 0;
+      if (xl < me) {
+        const int p = row_part[memb[xl]];
+        sb_l = sub_ptr[p];
+        nc_l = ncore[p];
+      }
+      const int cnt = (int)min((int64_t)32, me - x0);
+      for (int y = 0; y < cnt; ++y) {
+        const int64_t sb = __shfl_sync(0xffffffffu, sb_l, y);
+        const int nc = __shfl_sync(0xffffffffu, nc_l, y);
+        for (int c = lane; c < nc; c += 32) { const int i = sub_idx[sb + c]; atomicOr(&bm[i >> 5], 1u << (i & 31)); }
+      }
     }
     __syncwarp();
     int running = 0;
@@ -185,21 +197,35 @@ __global__ void k_d_pattern(int64_t n, int W, const int64_t* __restrict__ memb_p
       running += tot;
     }
     __syncwarp();
-    for (int64_t x = mb; x < me; ++x) {
-      const int64_t q = memb[x];
-      const int p = row_part[q];
-      const int64_t sb = sub_ptr[p];
-      const int nc = ncore[p];
-      const int first = sub_idx[sb];
-      const int pos0 = rk[first >> 5] + __popc(bm[first >> 5] & ((1u << (first & 31)) - 1u));
-      if (MODE == 0 && lane == 0) scat_base[q] = ob + pos0;
-      for (int c = lane; c < nc; c += 32) {
-        const int i = sub_idx[sb + c];
-        const int pos = rk[i >> 5] + __popc(bm[i >> 5] & ((1u << (i & 31)) - 1u));
-        if (MODE == 0) {
-          if (pos != pos0 + c) atomicOr(noncontig, 1);
-        } else {
-          scat_pos[scat_ofs[q] + c] = ob + pos;
+    for (int64_t x0 = mb; x0 < me; x0 += 32) {
+      const int64_t xl = x0 + lane;
+      int64_t q_l = 0, sb_l = 0, so_l = 0;
+      int nc_l = 0, first_l = 0;
+      if (xl < me) {
+        q_l = memb[xl];
+        const int p = row_part[q_l];
+        sb_l = sub_ptr[p];
+        nc_l = ncore[p];
+        first_l = sub_idx[sb_l];
+        if (MODE == 1) so_l = scat_ofs[q_l];
+      }
+      const int cnt = (int)min((int64_t)32, me - x0);
+      for (int y = 0; y < cnt; ++y) {
+        const int64_t q = __shfl_sync(0xffffffffu, q_l, y);
+        const int64_t sb = __shfl_sync(0xffffffffu, sb_l, y);
+        const int nc = __shfl_sync(0xffffffffu, nc_l, y);
+        const int first = __shfl_sync(0xffffffffu, first_l, y);
+        const int64_t so = MODE == 1 ? __shfl_sync(0xffffffffu, so_l, y) : 0;
+        const int pos0 = rk[first >> 5] + __popc(bm[first >> 5] & ((1u << (first & 31)) - 1u));
+        if (MODE == 0 && lane == 0) scat_base[q] = ob + pos0;
+        for (int c = lane; c < nc; c += 32) {
+          const int i = sub_idx[sb + c];
+          const int pos = rk[i >> 5] + __popc(bm[i >> 5] & ((1u << (i & 31)) - 1u));
+          if (MODE == 0) {
+            if (pos != pos0 + c) atomicOr(noncontig, 1);
+          } else {
+            scat_pos[so + c] = ob + pos;
+          }
         }
       }
     }

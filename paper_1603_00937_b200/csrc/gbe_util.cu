@@ -34,31 +34,52 @@ void gbe_dev_free(void* p) {
 }
 
 namespace {
+// One CTA walks the array in tiles of 4,096: every thread takes 4 consecutive elements (a warp reads 512 contiguous
+// bytes), warp scans by shuffle, one scan over the 32 warp sums, a running carry between tiles.
 template <typename TI>
 __global__ void __launch_bounds__(1024) k_scan_single_block(const TI* __restrict__ in, int64_t* __restrict__ out,
                                                             int64_t n) {
-  __shared__ int64_t part[1024];
-  const int t = threadIdx.x;
-  const int64_t chunk = (n + 1023) / 1024;
-  const int64_t b = (int64_t)t * chunk, e = min(n, b + chunk);
-  int64_t s = 0;
-  for (int64_t i = b; i < e; ++i) s += (int64_t)in[i];
-  part[t] = s;
-  __syncthreads();
-  // Hillis-Steele inclusive scan over the 1024 chunk sums
-  for (int o = 1; o < 1024; o <<= 1) {
-    int64_t v = (t >= o) ? part[t - o] : 0;
+  __shared__ int64_t wsum[32];
+  __shared__ int64_t tile_total;
+  const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+  int64_t carry = 0;
+  for (int64_t base = 0; base < n; base += 4096) {
+    const int64_t i0 = base + 4 * t;
+    int64_t v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = i0 + k < n ? (int64_t)in[i0 + k] : 0;
+    const int64_t s = (v[0] + v[1]) + (v[2] + v[3]);
+    int64_t x = s;  // inclusive scan over the warp
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int64_t y = __shfl_up_sync(0xffffffffu, x, o);
+      if (lane >= o) x += y;
+    }
+    if (lane == 31) wsum[w] = x;
     __syncthreads();
-    part[t] += v;
+    if (w == 0) {
+      const int64_t ws = wsum[lane];
+      int64_t z = ws;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int64_t y = __shfl_up_sync(0xffffffffu, z, o);
+        if (lane >= o) z += y;
+      }
+      wsum[lane] = z - ws;  // exclusive over the warps
+      if (lane == 31) tile_total = z;
+    }
     __syncthreads();
+    int64_t run = carry + wsum[w] + (x - s);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (i0 + k < n) {
+        out[i0 + k] = run;
+        run += v[k];
+      }
+    carry += tile_total;
+    __syncthreads();  // wsum and tile_total are rewritten by the next tile
   }
-  int64_t run = part[t] - s;
-  for (int64_t i = b; i < e; ++i) {
-    int64_t v = (int64_t)in[i];
-    out[i] = run;
-    run += v;
-  }
-  if (t == 1023) out[n] = part[1023];
+  if (t == 0) out[n] = carry;
 }
 }  // namespace
 
