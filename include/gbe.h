@@ -271,6 +271,13 @@ int gbe_error_norms(const gbe_graph* g, const double* D_val, const double* D_ref
 /* Number of CUDA kernels this library has launched in this process so far (all threads). */
 uint64_t gbe_launch_count(void);
 
+/* Scratch memory the graph builds (gbe_build_graph, gbe_update_graph) may take for the candidate bitmaps of the
+ * thresholded product (step 1): the sizing pass leaves one bitmap of n bits per row (n^2 / 8 bytes) for the numeric pass,
+ * which otherwise walks all products a_ik t_kj a second time.  Above the limit (default 8 GiB), or when the allocation
+ * fails, the second walk is taken; the graph is the same bit for bit.  bytes = 0 switches the bitmaps off.
+ * Process-wide; returns the previous limit. */
+size_t gbe_set_build_scratch_limit(size_t bytes);
+
 void gbe_free_graph(gbe_graph* g);
 
 const char* gbe_strerror(int status);

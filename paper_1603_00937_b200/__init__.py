@@ -26,6 +26,7 @@ from .binding import (  # noqa: F401
     gbe_launch_count,
     gbe_graph_set_sp2_path,
     gbe_graph_set_gather_path,
+    gbe_set_build_scratch_limit,
     gbe_error_norms,
     gbe_graph_export,
     gbe_density,

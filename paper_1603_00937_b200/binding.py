@@ -20,7 +20,7 @@ EXPORTS = [
     "gbe_build_graph", "gbe_graph_get_info", "gbe_graph_export", "gbe_density", "gbe_gather", "gbe_sp2",
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
     "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation", "gbe_update_graph", "gbe_density_fermi",
-    "gbe_graph_set_sp2_path", "gbe_error_norms", "gbe_graph_set_gather_path",
+    "gbe_graph_set_sp2_path", "gbe_error_norms", "gbe_graph_set_gather_path", "gbe_set_build_scratch_limit",
 ]
 
 
@@ -97,6 +97,8 @@ def lib() -> C.CDLL:
         l.gbe_error_norms.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.POINTER(C.c_double)]
         l.gbe_graph_set_sp2_path.argtypes = [C.c_void_p, C.c_int32]
         l.gbe_graph_set_gather_path.argtypes = [C.c_void_p, C.c_int32]
+        l.gbe_set_build_scratch_limit.restype = C.c_size_t
+        l.gbe_set_build_scratch_limit.argtypes = [C.c_size_t]
         l.gbe_launch_count.restype = C.c_uint64
         l.gbe_launch_count.argtypes = []
         l.gbe_gather.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -234,6 +236,11 @@ def gbe_graph_set_sp2_path(g: "Graph", path: int) -> None:
 def gbe_graph_set_gather_path(g: "Graph", path: int) -> None:
     """0 auto, 1 staged through a shared-memory row buffer, 2 direct to global memory (include/gbe.h)."""
     _check(lib().gbe_graph_set_gather_path(g._h, int(path)))
+
+
+def gbe_set_build_scratch_limit(nbytes: int) -> int:
+    """Scratch limit of the graph builds for the candidate bitmaps (include/gbe.h); returns the previous limit."""
+    return int(lib().gbe_set_build_scratch_limit(int(nbytes)))
 
 
 def gbe_launch_count() -> int:

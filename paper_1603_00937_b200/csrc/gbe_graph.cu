@@ -14,6 +14,13 @@
 // Bound: L2/shared-memory latency (integer + a few FP64 operations per candidate); it runs once per graph.
 #include "gbe_internal.cuh"
 
+static size_t g_bm_save_max = (size_t)8 << 30;  // gbe_set_build_scratch_limit
+size_t gbe_set_build_scratch_limit(size_t bytes) {
+  const size_t old = g_bm_save_max;
+  g_bm_save_max = bytes;
+  return old;
+}
+
 namespace {
 
 
@@ -84,7 +91,9 @@ template <bool NEED_VAL, bool ORDERED, typename F>
 __device__ __forceinline__ void walk_products(int lane, int64_t a, int64_t b, const int32_t* __restrict__ A_col,
                                               const double* __restrict__ A_val, const int64_t* __restrict__ T_rp,
                                               const int32_t* __restrict__ T_col, const double* __restrict__ T_val,
-                                              F&& fn) {
+                                              const int64_t* __restrict__ T_start, F&& fn) {
+  // T_start (may be null): per entry e = (i, k) of the A row, the offset in T of the first entry of row k that counts
+  // (k_first_upper: the first column >= i when only the upper triangle is formed); null: the whole row, from T_rp[k]
   constexpr unsigned FULL = 0xffffffffu;
   struct Buf {
     int j[4];
@@ -96,7 +105,7 @@ __device__ __forceinline__ void walk_products(int lane, int64_t a, int64_t b, co
   for (int64_t e0 = a; e0 < b; e0 += 32) {
     const int kk = kk_n;
     const double av = av_n;
-    const int64_t tb_l = kk >= 0 ? T_rp[kk] : 0;
+    const int64_t tb_l = kk >= 0 ? (T_start ? T_start[e0 + lane] : T_rp[kk]) : 0;
     const int64_t te_l = kk >= 0 ? T_rp[kk + 1] : 0;
     {  // neighbour indices of the next 32: in flight during this block
       const int64_t en = e0 + 32 + lane;
@@ -140,6 +149,25 @@ __device__ __forceinline__ void walk_products(int lane, int64_t a, int64_t b, co
   }
 }
 
+// Upper triangle only (A A with A symmetric): of row k the product for row i needs the columns j >= i.  One binary
+// search per entry (i, k) of A, all in parallel, finds where they start, so that the walks neither load nor test the
+// rest (half of all entries, and rows longer than 128 entries mostly fit one round again).
+__global__ void __launch_bounds__(256) k_first_upper(int64_t n, const int64_t* __restrict__ rp,
+                                                     const int32_t* __restrict__ col, int64_t* __restrict__ start) {
+  const int lane = threadIdx.x & 31;
+  const int64_t i = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (i >= n) return;
+  for (int64_t e = rp[i] + lane; e < rp[i + 1]; e += 32) {
+    const int k = col[e];
+    int64_t lo = rp[k], hi = rp[k + 1];
+    while (lo < hi) {
+      const int64_t mid = (lo + hi) >> 1;
+      if (col[mid] < i) lo = mid + 1; else hi = mid;
+    }
+    start[e] = lo;
+  }
+}
+
 // MODE 0: distinct candidate columns per row (sizes the accumulator); 1: count kept entries; 2: fill (columns + values);
 // 3: one pass for the LAST power, whose values are not needed: kept columns go to a scratch row of candidate capacity
 //    (offsets out_rp from MODE 0's counts) and cnt[i] = number kept.
@@ -150,7 +178,8 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
                                    const int64_t* __restrict__ T_rp, const int32_t* __restrict__ T_col,
                                    const double* __restrict__ T_val, double tau, int32_t* __restrict__ cnt,
                                    const int64_t* __restrict__ out_rp, int32_t* __restrict__ out_col,
-                                   double* __restrict__ out_val, uint32_t* __restrict__ bm_io) {
+                                   double* __restrict__ out_val, uint32_t* __restrict__ bm_io,
+                                   const int64_t* __restrict__ T_start) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, w_in_blk = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const size_t per_warp = (size_t)W * 8 + ((MODE == 0 || MODE == 4) ? 0 : (size_t)cap * 8);
@@ -173,7 +202,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
     } else {
     for (int w = lane; w < W; w += 32) bm[w] = 0u;
     __syncwarp();
-    walk_products<false, false>(lane, a, b, A_col, A_val, T_rp, T_col, T_val,
+    walk_products<false, false>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, T_start,
                                 [&](double, const int (&j)[4], const double (&)[4]) {
 #pragma unroll
       for (int u = 0; u < 4; ++u)
@@ -214,7 +243,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
     // pass 2: accumulate, k ascending, multiply and add separately rounded
     // branch free, the four entries of a lane as independent chains (the columns of one T row are distinct, so
     // their slots are): entries that do not count (empty, or j < jmin) go to the spare slot cap - 1
-    walk_products<true, true>(lane, a, b, A_col, A_val, T_rp, T_col, T_val,
+    walk_products<true, true>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, T_start,
                               [&](double aik, const int (&j)[4], const double (&t)[4]) {
       int slot[4];
       double o[4];
@@ -502,12 +531,24 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   // candidate bitmaps of the sizing pass, kept for the numeric passes of the same product (n * W words: only while
   // that is a small part of the device memory - beyond it the numeric passes walk the products again)
   DevBuf bmsave;
-  constexpr size_t BM_SAVE_MAX = (size_t)8 << 30;
-  if ((size_t)n * W * 4 <= BM_SAVE_MAX && power >= 2) GBE_TRY(bmsave.alloc((size_t)n * W * 4));
+  const size_t BM_SAVE_MAX = g_bm_save_max;
+  if ((size_t)n * W * 4 <= BM_SAVE_MAX && power >= 2 && bmsave.alloc((size_t)n * W * 4) != GBE_OK) {
+    (void)cudaGetLastError();  // no room for the bitmaps: not an error, the numeric passes walk the products again
+    bmsave.p = nullptr;
+  }
   uint32_t* const bm_io = bmsave.as<uint32_t>();
   for (int k = 2; k <= power; ++k) {
     // A A with symmetric A is symmetric bit for bit: when it is the LAST power only its upper triangle is formed
     const int upper_only = (k == 2 && power == 2) ? 1 : 0;
+    // upper triangle only: where the columns j >= i start in every row k of every entry (i, k)
+    DevBuf tstart;
+    const int64_t* t_start = nullptr;
+    if (upper_only) {
+      GBE_TRY(tstart.alloc((size_t)A.nnz * 8));
+      k_first_upper<<<rows_grid, 256, 0, s>>>(n, A.rp.as<int64_t>(), A.col.as<int32_t>(), tstart.as<int64_t>());
+      GBE_LAUNCHED();
+      t_start = tstart.as<int64_t>();
+    }
     // symbolic: accumulator capacity
     {
       const size_t per_warp = (size_t)W * 8;
@@ -517,7 +558,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
       const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
       k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, upper_only, A.rp.as<int64_t>(),
                                                                  A.col.as<int32_t>(), A.val.as<double>(), T_rp, T_col, T_val, tau,
-                                                                 cnt.as<int32_t>(), nullptr, nullptr, nullptr, bm_io);
+                                                                 cnt.as<int32_t>(), nullptr, nullptr, nullptr, bm_io, t_start);
       GBE_LAUNCHED();
     }
     std::vector<int32_t> h_cnt((size_t)n);
@@ -542,7 +583,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
       k_spgemm_threshold<3><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, upper_only, A.rp.as<int64_t>(),
                                                                  A.col.as<int32_t>(), A.val.as<double>(), T_rp, T_col, T_val, tau,
                                                                  cnt.as<int32_t>(), Tc.rp.as<int64_t>(),
-                                                                 Tc.col.as<int32_t>(), nullptr, bm_io);
+                                                                 Tc.col.as<int32_t>(), nullptr, bm_io, t_start);
       GBE_LAUNCHED();
       Pattern Pn;
       GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tc.rp.as<int64_t>(), Tc.col.as<int32_t>(),
@@ -556,7 +597,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     Pattern Tn;
     k_spgemm_threshold<1><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, 0, A.rp.as<int64_t>(), A.col.as<int32_t>(),
                                                                A.val.as<double>(), T_rp, T_col, T_val, tau,
-                                                               cnt.as<int32_t>(), nullptr, nullptr, nullptr, bm_io);
+                                                               cnt.as<int32_t>(), nullptr, nullptr, nullptr, bm_io, nullptr);
     GBE_LAUNCHED();
     GBE_TRY(count_to_rowptr(cnt, n, Tn.rp, &Tn.nnz, s));
     GBE_TRY(Tn.col.alloc((size_t)Tn.nnz * 4));
@@ -564,7 +605,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     k_spgemm_threshold<2><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, 0, A.rp.as<int64_t>(), A.col.as<int32_t>(),
                                                                A.val.as<double>(), T_rp, T_col, T_val, tau, nullptr,
                                                                Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(),
-                                                               Tn.val.as<double>(), bm_io);
+                                                               Tn.val.as<double>(), bm_io, nullptr);
     GBE_LAUNCHED();
     Pattern Pn;
     GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tn.rp.as<int64_t>(), Tn.col.as<int32_t>(), nullptr, 0, Pn));
@@ -614,18 +655,21 @@ int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int3
   GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
   const int grid = (int)std::min<int64_t>((n + nw - 1) / nw, (int64_t)sm_count * 8);
   DevBuf bmsave;  // candidate bitmaps of the counting pass, read back by the emitting pass
-  if ((size_t)n * W * 4 <= ((size_t)8 << 30)) GBE_TRY(bmsave.alloc((size_t)n * W * 4));
+  if ((size_t)n * W * 4 <= g_bm_save_max && bmsave.alloc((size_t)n * W * 4) != GBE_OK) {
+    (void)cudaGetLastError();  // no room: the emitting pass walks the products again
+    bmsave.p = nullptr;
+  }
   uint32_t* const bm_io = bmsave.as<uint32_t>();
   k_spgemm_threshold<0><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, 0, M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr,
                                                              M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr, 0.0,
-                                                             cnt.as<int32_t>(), nullptr, nullptr, nullptr, bm_io);
+                                                             cnt.as<int32_t>(), nullptr, nullptr, nullptr, bm_io, nullptr);
   GBE_LAUNCHED();
   Pattern P;
   GBE_TRY(count_to_rowptr(cnt, n, P.rp, &P.nnz, s));
   GBE_TRY(P.col.alloc((size_t)P.nnz * 4));
   k_spgemm_threshold<4><<<grid, nw * 32, per_warp * nw, s>>>(n, W, 0, 0, M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr,
                                                              M.rp.as<int64_t>(), M.col.as<int32_t>(), nullptr, 0.0, nullptr,
-                                                             P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr, bm_io);
+                                                             P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr, bm_io, nullptr);
   GBE_LAUNCHED();
   Pattern S;
   GBE_TRY(symmetrise(P, U, cnt, S));

@@ -280,6 +280,35 @@ def test_graph_power(gbe, power):
     check_density(Dg, log, r)
 
 
+@pytest.mark.parametrize("which", ["water", "banded_power3", "update"])
+def test_graph_build_with_and_without_the_kept_bitmaps(gbe, which):
+    """The numeric pass of the thresholded product either reads back the candidate bitmaps of the sizing pass or walks the
+    products again (include/gbe.h, gbe_set_build_scratch_limit): same graph bit for bit, and equal to the oracle's."""
+    import torch
+    if which == "water":
+        s, power = gi.water_box(256, 32, seed=3, iters=5), 2
+    else:
+        s, power = gi.random_banded(300, half_bw=4, n_part=6, seed=8, tau=1e-3, iters=5), 3
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    exs = []
+    for limit in (0, 8 << 30):
+        old = gbe.gbe_set_build_scratch_limit(limit)
+        try:
+            g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part, power=power)
+            if which == "update":
+                D, _ = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
+                g = gbe.gbe_update_graph(g, D, Hd, 1e-4, None, s.n_part)
+            torch.cuda.synchronize()
+        finally:
+            assert gbe.gbe_set_build_scratch_limit(old) == limit
+        exs.append({k: v.cpu().numpy() for k, v in g.export().items()})
+    for k in exs[0]:
+        assert np.array_equal(exs[0][k], exs[1][k]), k
+    if which != "update":
+        rp, ci = o.build_graph(s.H, s.tau, power=power)
+        assert np.array_equal(exs[0]["S_row_ptr"], rp) and np.array_equal(exs[0]["S_col"], ci)
+
+
 @pytest.mark.parametrize("tau", [1e-1, 1e-3, 1e-7, 0.0, 1.5])
 def test_tau_sweep_chain(gbe, tau):
     s = gi.chain(256, 8, tau=tau, iters=30)
