@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(256) k_materialise_A(int64_t n, const int64_t*
 // with one ballot and two shuffles instead of a search loop; each round costs one 64-bit address per array and
 // predicated loads at immediate offsets with 32-bit bounds; the loads of round r + 1 are in flight while round r is
 // processed.  ORDERED: a __syncwarp follows every round, because the next k may hit the accumulator slots of this one.
-template <bool NEED_VAL, bool ORDERED, typename F>
+template <bool NEED_VAL, bool ORDERED, bool CONSEC, typename F>
 __device__ __forceinline__ void walk_products(int lane, int64_t a, int64_t b, const int32_t* __restrict__ A_col,
                                               const double* __restrict__ A_val, const int64_t* __restrict__ T_rp,
                                               const int32_t* __restrict__ T_col, const double* __restrict__ T_val,
@@ -121,15 +121,17 @@ __device__ __forceinline__ void walk_products(int lane, int64_t a, int64_t b, co
     const int lenx_l = len_l + (ex_l << 7);              // ... and holds the entries below lenx - 128 r
     auto load = [&](int r, Buf& B) {
       const int q = __ffs(__ballot_sync(FULL, cum_l > r)) - 1;  // the first k whose rounds end beyond r owns round r
-      const int64_t first = __shfl_sync(FULL, tbx_l, q) + ((int64_t)r << 7) + lane;
-      const int left = __shfl_sync(FULL, lenx_l, q) - (r << 7) - lane;  // entries from this lane's first one on
+      // CONSEC: a lane takes 4 consecutive entries of the round (its columns are neighbours), else entries 32 apart
+      constexpr int LS = CONSEC ? 4 : 1, US = CONSEC ? 1 : 32;
+      const int64_t first = __shfl_sync(FULL, tbx_l, q) + ((int64_t)r << 7) + LS * lane;
+      const int left = __shfl_sync(FULL, lenx_l, q) - (r << 7) - LS * lane;  // entries from this lane's first one on
       B.q = q;
       const int32_t* __restrict__ cp = T_col + first;
       const double* __restrict__ vp = T_val + first;
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
-        B.j[u] = 32 * u < left ? cp[32 * u] : -1;
-        if (NEED_VAL) B.v[u] = 32 * u < left ? vp[32 * u] : 0.0;
+        B.j[u] = US * u < left ? cp[US * u] : -1;
+        if (NEED_VAL) B.v[u] = US * u < left ? vp[US * u] : 0.0;
       }
     };
     auto process = [&](const Buf& B) {
@@ -202,11 +204,27 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
     } else {
     for (int w = lane; w < W; w += 32) bm[w] = 0u;
     __syncwarp();
-    walk_products<false, false>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, T_start,
-                                [&](double, const int (&j)[4], const double (&)[4]) {
+    // The columns of a T row are sorted, so the entries of one round hit few bitmap words and their atomics serialise
+    // (ncu: 79 % of the shared-memory wavefronts of the sizing pass were conflicts).  Here a lane holds 4 CONSECUTIVE
+    // entries and merges those that share a word before it issues an atomic.
+    walk_products<false, false, true>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, T_start,
+                                      [&](double, const int (&j)[4], const double (&)[4]) {
+      int cw = -1;
+      unsigned cb = 0u;
 #pragma unroll
-      for (int u = 0; u < 4; ++u)
-        if (j[u] >= jmin) atomicOr(&bm[j[u] >> 5], 1u << (j[u] & 31));  // an empty slot is -1 < jmin
+      for (int u = 0; u < 4; ++u) {
+        const bool ok = j[u] >= jmin;  // an empty slot is -1 < jmin
+        const int w = ok ? (j[u] >> 5) : -1;
+        const unsigned bit = ok ? (1u << (j[u] & 31)) : 0u;
+        if (w != cw) {
+          if (cw >= 0) atomicOr(&bm[cw], cb);
+          cw = w;
+          cb = bit;
+        } else {
+          cb |= bit;
+        }
+      }
+      if (cw >= 0) atomicOr(&bm[cw], cb);
     });
     }
     __syncwarp();
@@ -243,7 +261,7 @@ __global__ void k_spgemm_threshold(int64_t n, int W, int cap, int upper_only, co
     // pass 2: accumulate, k ascending, multiply and add separately rounded
     // branch free, the four entries of a lane as independent chains (the columns of one T row are distinct, so
     // their slots are): entries that do not count (empty, or j < jmin) go to the spare slot cap - 1
-    walk_products<true, true>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, T_start,
+    walk_products<true, true, false>(lane, a, b, A_col, A_val, T_rp, T_col, T_val, T_start,
                               [&](double aik, const int (&j)[4], const double (&t)[4]) {
       int slot[4];
       double o[4];
