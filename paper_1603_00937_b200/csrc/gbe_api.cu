@@ -294,7 +294,7 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
     // Iteration iters - 1 is the last one whether or not the idempotency stop fires before it (then it is a no-op):
     // only the core rows and columns of its result are read again (trace, scatter), so it runs the core tiles only.
     const bool last = it == iters - 1;
-    const int n_part_it = last ? g->n_items_last : g->n_items;
+    const int n_part_it = g->n_items_last;  // one packed partial per tile with a core row, in every iteration
     GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, g->n_items ? 1 : 0,
                   [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, s); }));
     if (mode != 2)

@@ -323,8 +323,12 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
       const int64_t ld = (g->h_m[p] + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
       for (int ti = 0; ti < T; ++ti)
         for (int tj = ti; tj < T; ++tj) {
-          items.push_back({p, ti, tj, g->h_m[p], g->h_ncore[p], (int32_t)ld, g->h_dense_off[p]});
-          if (ti * tile < g->h_ncore[p]) last.push_back(items.back());
+          // pidx: where the tile's trace partial goes - the tiles with a core row are numbered in list order (which is
+          // their position in the list of the last iteration), the others carry no trace and get -1
+          const bool core_row = ti * tile < g->h_ncore[p];
+          items.push_back({core_row ? (int32_t)last.size() : -1, ti, tj, g->h_m[p], g->h_ncore[p], (int32_t)ld,
+                           g->h_dense_off[p]});
+          if (core_row) last.push_back(items.back());
         }
       // executed DMMA work: 8x8 sub-tiles (bi <= bj) with rows < m, columns < ld, each 2*8*8*ld flop
       const double R = (double)((g->h_m[p] + 7) / 8), C = (double)(ld / 8);

@@ -80,7 +80,7 @@ struct gbe_state {
 };
 
 struct gbe_tile_item {  // one X^2 work item: tile (ti, tj), ti <= tj, of community p, with p's layout (32 bytes)
-  int32_t p, ti, tj, m;      // m = core + halo size
+  int32_t pidx, ti, tj, m;   // pidx: index of the tile's trace partial (tiles with a core row), else -1; m = core + halo size
   int32_t nc, ld;            // core size, leading dimension (m rounded up to 16)
   int64_t dense_off;         // element offset of X_p in a dense buffer
 };

@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   const int branch = OP == 0 ? (st->preset ? (int)st->br[iter] : st->branch) : 0;
   const double cn = OP == 1 ? coef[iter] : 0.0;
 
-  const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // p, ti, tj, m
+  const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // pidx, ti, tj, m
   const int4 it1 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x + 1];  // nc, ld, dense_off
   const int ti = it0.y, tj = it0.z, m = it0.w, nc = it1.x, ld = it1.y;
   const int64_t doff = ((int64_t)(uint32_t)it1.z) | ((int64_t)it1.w << 32);
@@ -306,13 +306,17 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   } else {
     epilogue(std::false_type{}, std::false_type{}, std::false_type{});
   }
+  // only the tiles with a core row carry a trace; their partials are packed (pidx), so that step 5 reads n_tiles_last
+  // pairs instead of one per tile
+  const int pidx = it0.x;
+  if (OP != 0 || pidx < 0) return;
   s1 = warp_sum(s1);
   s2 = warp_sum(s2);
   if (lane == 0) { red[role] = s1; red[4 + role] = s2; }  // indexed by block position: order independent of the rotation
   __syncthreads();
   if (t == 0) {
-    partials[2 * (size_t)blockIdx.x] = (red[0] + red[1]) + (red[2] + red[3]);
-    partials[2 * (size_t)blockIdx.x + 1] = (red[4] + red[5]) + (red[6] + red[7]);
+    partials[2 * (size_t)pidx] = (red[0] + red[1]) + (red[2] + red[3]);
+    partials[2 * (size_t)pidx + 1] = (red[4] + red[5]) + (red[6] + red[7]);
   }
 }
 
