@@ -14,34 +14,30 @@ namespace {
 constexpr int TB = 1024;
 
 __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double* __restrict__ partials, int n) {
-  __shared__ double s1[TB], s2[TB];
+  __shared__ double s1[32], s2[32];
   const int t = threadIdx.x;
-  if (st->stop) return;
+  const int stopped = st->stop;  // read now, tested after the sums: the loads below need not wait for it
   // the kernel is one CTA and latency bound: 8 independent 16-byte loads in flight per thread, summed in a fixed order
   double a1 = 0.0, a2 = 0.0;
   const double2* __restrict__ p2 = reinterpret_cast<const double2*>(partials);
-  int i = t;
-  for (; i + 7 * TB < n; i += 8 * TB) {
+  for (int i = t; i < n; i += 8 * TB) {
     double2 v[8];
 #pragma unroll
-    for (int u = 0; u < 8; ++u) v[u] = p2[i + u * TB];
+    for (int u = 0; u < 8; ++u) v[u] = i + u * TB < n ? p2[i + u * TB] : make_double2(0.0, 0.0);
 #pragma unroll
     for (int u = 0; u < 8; ++u) { a1 += v[u].x; a2 += v[u].y; }
   }
-  for (; i < n; i += TB) {
-    const double2 v = p2[i];
-    a1 += v.x;
-    a2 += v.y;
-  }
-  s1[t] = a1;
-  s2[t] = a2;
+  // fixed-order reduction: butterfly inside each warp, then warp 0 over the 32 warp sums
+  a1 = warp_sum(a1);
+  a2 = warp_sum(a2);
+  if ((t & 31) == 0) { s1[t >> 5] = a1; s2[t >> 5] = a2; }
   __syncthreads();
-  for (int o = TB / 2; o > 0; o >>= 1) {
-    if (t < o) { s1[t] += s1[t + o]; s2[t] += s2[t + o]; }
-    __syncthreads();
+  if (t < 32) {
+    a1 = warp_sum(s1[t]);
+    a2 = warp_sum(s2[t]);
   }
-  if (t == 0) {
-    const double t1 = s1[0], t2 = s2[0], n_occ = st->n_occ;
+  if (t == 0 && !stopped) {
+    const double t1 = a1, t2 = a2, n_occ = st->n_occ;
     const int k = st->iter;  // the partials describe X_k
     st->t1[k] = t1;
     st->t2[k] = t2;
