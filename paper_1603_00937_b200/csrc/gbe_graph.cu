@@ -539,8 +539,10 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     return U.run(p_rp, p_col, nullptr, 0.0, q_rp, q_col, q_len, diag, out);
   };
 
+  // (with the default power 2 the union with the second power below takes I and pat(A) directly: one union less)
   Pattern P;
-  GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), nullptr, nullptr, nullptr, 1, P));
+  const bool P_built = power != 2;
+  if (P_built) GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), nullptr, nullptr, nullptr, 1, P));
   // thresholded powers
   Pattern Tprev;  // T^(k-1) with values; T^(1) aliases A
   const int64_t* T_rp = A.rp.as<int64_t>();
@@ -579,11 +581,16 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                                  cnt.as<int32_t>(), nullptr, nullptr, nullptr, bm_io, t_start);
       GBE_LAUNCHED();
     }
-    std::vector<int32_t> h_cnt((size_t)n);
-    GBE_CUDA(cudaMemcpyAsync(h_cnt.data(), cnt.p, (size_t)n * 4, cudaMemcpyDeviceToHost, s));
+    // one scan gives the accumulator capacity (the largest candidate count) and the scratch-row offsets of the last
+    // power (the running sum): 16 bytes come back to the host, one synchronisation
+    Pattern Tc;  // scratch: rp = offsets by candidate count, col = kept columns, cnt = kept per row
+    int64_t total_max[2] = {0, 0};
+    GBE_TRY(Tc.rp.alloc((size_t)(n + 2) * 8));
+    GBE_TRY(gbe_exclusive_scan_i32_to_i64_max(cnt.as<int32_t>(), Tc.rp.as<int64_t>(), n, s));
+    GBE_CUDA(cudaMemcpyAsync(total_max, Tc.rp.as<int64_t>() + n, 16, cudaMemcpyDeviceToHost, s));
     GBE_CUDA(cudaStreamSynchronize(s));
-    int cap = 1;
-    for (int64_t i = 0; i < n; ++i) cap = std::max(cap, h_cnt[(size_t)i]);
+    const int64_t total_cand = total_max[0];
+    int cap = std::max<int>(1, (int)total_max[1]);
     cap = ((cap + 1) & ~1) + 2;  // + the spare slot that takes the entries that do not count
     const size_t per_warp = (size_t)W * 8 + (size_t)cap * 8;
     const int nw = pick_warps(per_warp, 16);
@@ -594,9 +601,6 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     if (k == power) {
       // last power: only its pattern enters S - one numeric pass into scratch rows of candidate capacity
       GBE_CUDA(cudaFuncSetAttribute(k_spgemm_threshold<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * nw)));
-      Pattern Tc;  // scratch: rp = offsets by candidate count, col = kept columns, cnt = kept per row
-      int64_t total_cand = 0;
-      GBE_TRY(count_to_rowptr(cnt, n, Tc.rp, &total_cand, s));
       GBE_TRY(Tc.col.alloc((size_t)total_cand * 4));
       k_spgemm_threshold<3><<<grid, nw * 32, per_warp * nw, s>>>(n, W, cap, upper_only, A.rp.as<int64_t>(),
                                                                  A.col.as<int32_t>(), A.val.as<double>(), T_rp, T_col, T_val, tau,
@@ -604,9 +608,13 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                                  Tc.col.as<int32_t>(), nullptr, bm_io, t_start);
       GBE_LAUNCHED();
       Pattern Pn;
-      GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tc.rp.as<int64_t>(), Tc.col.as<int32_t>(),
-                       cnt.as<int32_t>(), 0, Pn));
-      GBE_CUDA(cudaStreamSynchronize(s));
+      if (P_built)
+        GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tc.rp.as<int64_t>(), Tc.col.as<int32_t>(),
+                         cnt.as<int32_t>(), 0, Pn));
+      else
+        GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), Tc.rp.as<int64_t>(), Tc.col.as<int32_t>(),
+                         cnt.as<int32_t>(), 1, Pn));
+      // (no synchronisation here: the scratch buffers are released in stream order)
       std::swap(P.rp.p, Pn.rp.p);
       std::swap(P.col.p, Pn.col.p);
       P.nnz = Pn.nnz;

@@ -30,11 +30,13 @@ __global__ void k_core_count(int64_t n, const int32_t* __restrict__ part, int64_
   if (p < 0 || p >= n_part) { atomicOr(flag, 1); return; }
   atomicAdd(&cnt[p], 1);
 }
-__global__ void k_core_fill(int64_t n, const int32_t* __restrict__ part, int64_t blk, const int64_t* __restrict__ core_ptr,
-                            int32_t* __restrict__ cursor, int32_t* __restrict__ core_tmp) {
+__global__ void k_core_fill(int64_t n, const int32_t* __restrict__ part, int64_t blk, int n_part,
+                            const int64_t* __restrict__ core_ptr, int32_t* __restrict__ cursor,
+                            int32_t* __restrict__ core_tmp) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int p = part_of(part, i, blk);
+  if (p < 0 || p >= n_part) return;  // flagged by k_core_count; the host looks at the flag at its next synchronisation
   const int pos = atomicAdd(&cursor[p], 1);
   core_tmp[core_ptr[p] + pos] = (int32_t)i;  // order fixed later by the bitmap walk
 }
@@ -260,17 +262,18 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_CUDA(cudaMemsetAsync(flag.p, 0, 4, s));
   k_core_count<<<tgrid, 256, 0, s>>>(n, part, blk, n_part, cnt.as<int32_t>(), flag.as<int32_t>());
   GBE_LAUNCHED();
-  int32_t hflag = 0;
-  GBE_CUDA(cudaMemcpyAsync(&hflag, flag.p, 4, cudaMemcpyDeviceToHost, s));
-  GBE_CUDA(cudaStreamSynchronize(s));
-  if (hflag) return GBE_EINVAL;  // partition id out of range
+  int32_t hflag = 0, hflag_stack = 0;
+  int32_t* const pin = gbe_pinned_words();
+  int32_t* const core_flag = pin ? pin : &hflag_stack;  // fetched now, looked at after the next synchronisation
+  *core_flag = 0;
+  GBE_CUDA(cudaMemcpyAsync(core_flag, flag.p, 4, cudaMemcpyDeviceToHost, s));
   DevBuf core_ptr;
   GBE_TRY(core_ptr.alloc((size_t)(n_part + 1) * 8));
   GBE_TRY(gbe_exclusive_scan_i32_to_i64(cnt.as<int32_t>(), core_ptr.as<int64_t>(), n_part, s));
   GBE_TRY(core_tmp.alloc((size_t)n * 4));
   GBE_TRY(cursor.alloc((size_t)std::max<int64_t>(n_part, n) * 4));
   GBE_CUDA(cudaMemsetAsync(cursor.p, 0, (size_t)n_part * 4, s));
-  k_core_fill<<<tgrid, 256, 0, s>>>(n, part, blk, core_ptr.as<int64_t>(), cursor.as<int32_t>(), core_tmp.as<int32_t>());
+  k_core_fill<<<tgrid, 256, 0, s>>>(n, part, blk, n_part, core_ptr.as<int64_t>(), cursor.as<int32_t>(), core_tmp.as<int32_t>());
   GBE_LAUNCHED();
   // ---- halo: count, then fill
   const size_t halo_smem = (size_t)2 * W * 4 + 257 * 4;
@@ -287,6 +290,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   GBE_CUDA(cudaMemcpyAsync(g->h_m.data(), g->msize, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaMemcpyAsync(g->h_ncore.data(), g->ncore, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaStreamSynchronize(s));
+  if (*core_flag) return GBE_EINVAL;  // partition id out of range (k_core_count)
   // ---- host: layout, work lists
   std::vector<int64_t> h_sub_ptr(n_part + 1, 0);
   g->h_dense_off.assign(n_part + 1, 0);

@@ -184,7 +184,9 @@ int gbe_launch_error_norms(const gbe_graph* g, const double* D_val, const double
                            double* out, cudaStream_t s);
 
 // small device utilities (gbe_util.cu)
+int32_t* gbe_pinned_words();  // 64 pinned host words per thread, or null
 int gbe_exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s);
+int gbe_exclusive_scan_i32_to_i64_max(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s);
 
 // ----------------------------------------------------------------------------------------------
 // device helpers

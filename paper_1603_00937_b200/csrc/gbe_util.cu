@@ -20,6 +20,17 @@ void gbe_set_alloc_stream(cudaStream_t s) {
   t_alloc_stream = s;
 }
 cudaStream_t gbe_alloc_stream() { return t_alloc_stream; }
+
+// A few pinned host words per thread (allocated once, kept): a device-to-host copy into them does not block the host,
+// unlike a copy into pageable memory, so a flag can be fetched now and looked at after a later synchronisation.
+int32_t* gbe_pinned_words() {
+  thread_local int32_t* w = nullptr;
+  if (!w && cudaHostAlloc((void**)&w, 64 * sizeof(int32_t), cudaHostAllocDefault) != cudaSuccess) {
+    (void)cudaGetLastError();
+    w = nullptr;
+  }
+  return w;
+}
 int gbe_dev_alloc(void** p, size_t bytes) {
   cudaError_t e = cudaMallocAsync(p, bytes ? bytes : 16, t_alloc_stream);
   if (e != cudaSuccess) {
@@ -38,17 +49,19 @@ namespace {
 // bytes), warp scans by shuffle, one scan over the 32 warp sums, a running carry between tiles.
 template <typename TI>
 __global__ void __launch_bounds__(1024) k_scan_single_block(const TI* __restrict__ in, int64_t* __restrict__ out,
-                                                            int64_t n) {
+                                                            int64_t n, int want_max) {
   __shared__ int64_t wsum[32];
   __shared__ int64_t tile_total;
   const int t = threadIdx.x, lane = t & 31, w = t >> 5;
   int64_t carry = 0;
+  int64_t vmax = 0;  // want_max: out[n + 1] = max(0, max_i in[i])
   for (int64_t base = 0; base < n; base += 4096) {
     const int64_t i0 = base + 4 * t;
     int64_t v[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) v[k] = i0 + k < n ? (int64_t)in[i0 + k] : 0;
     const int64_t s = (v[0] + v[1]) + (v[2] + v[3]);
+    vmax = max(vmax, max(max(v[0], v[1]), max(v[2], v[3])));
     int64_t x = s;  // inclusive scan over the warp
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -80,11 +93,28 @@ __global__ void __launch_bounds__(1024) k_scan_single_block(const TI* __restrict
     __syncthreads();  // wsum and tile_total are rewritten by the next tile
   }
   if (t == 0) out[n] = carry;
+  if (want_max) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) vmax = max(vmax, (int64_t)__shfl_xor_sync(0xffffffffu, vmax, o));
+    if (lane == 0) wsum[w] = vmax;
+    __syncthreads();
+    if (t == 0) {
+      int64_t m = 0;
+      for (int k = 0; k < 32; ++k) m = max(m, wsum[k]);
+      out[n + 1] = m;
+    }
+  }
 }
 }  // namespace
 
 int gbe_exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s) {
-  k_scan_single_block<int32_t><<<1, 1024, 0, s>>>(in, out, n);
+  k_scan_single_block<int32_t><<<1, 1024, 0, s>>>(in, out, n, 0);
+  GBE_LAUNCHED();
+  return GBE_OK;
+}
+// as above, and out[n + 1] = max(0, max_i in[i]) (out has n + 2 entries)
+int gbe_exclusive_scan_i32_to_i64_max(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s) {
+  k_scan_single_block<int32_t><<<1, 1024, 0, s>>>(in, out, n, 1);
   GBE_LAUNCHED();
   return GBE_OK;
 }
