@@ -6,7 +6,8 @@
 // One polynomial for every subgraph (Eq.(4); "the same for each subgraph expansion ... for the correct
 // total occupation").  The paper pre-sets the sequence from a gap estimate (ref. 41); north_star
 // asks for the choice from the global trace, taken on the device with no host round trip.
-// A single CTA sums the per-work-item partials in a fixed order (no floating-point atomics): reproducible.
+// A single CTA sums the partials (one pair per gather CTA, or per X^2 tile with a core row) in a fixed order (no
+// floating-point atomics): reproducible.
 // Bound: latency (16 B per partial).
 #include "gbe_internal.cuh"
 

@@ -27,7 +27,8 @@
 //
 // Fused epilogue (warp-shuffle partials, north_star item 3): while X_{n+1} is written, accumulate over the core
 // rows  t1 = sum_i X_ii  and  t2 = sum_i sum_c X_ic^2 (= Tr_core(X^2) for symmetric X), one fixed-order partial
-// per work item, so that the branch of the NEXT iteration is known before its GEMM starts.
+// per tile with a core row (packed: the other tiles carry no trace and write none), so that the branch of the NEXT
+// iteration is known before its GEMM starts.
 // Bound: FP64 tensor pipe - 2 m^3 algorithmic flop per community per iteration (~m^3 executed thanks to symmetry).
 #include <type_traits>
 
