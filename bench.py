@@ -340,7 +340,7 @@ def run_ours(args) -> None:
             "roofline": {
                 "kernel": "k_x2 (Y = X X^T on DMMA.8x8x4, fused branch/trace epilogue)", "bound": "tensor",
                 "achieved": alg_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": alg_tf / peak_tf,
-                "traffic": X2_DRAM_BYTES_PER_LAUNCH.get(args.workload), "traffic_unit": "B per launch (dram read + write, ncu --set full, profiles/r01_x2_v4_ncu.md); algorithmic bytes per launch = %.3g" % (16.0 * info["dense_elems"]),
+                "traffic": X2_DRAM_BYTES_PER_LAUNCH.get(args.workload), "traffic_unit": "B per launch (dram read + write, ncu --set full, profiles/r01_x2_v8_ncu.md); algorithmic bytes per launch = %.3g" % (16.0 * info["dense_elems"]),
                 "basis": "algorithmic 2 m^3 flop per community per iteration (unpadded, symmetry not counted) / mean "
                          "CUDA-event time of the %d launches" % ph["x2_launches"],
                 "peak_source": "FP64: %s bf16 sustained %.1f TF x nominal 40/2250" % (peaks["source"], peaks["bf16_tf"]),
