@@ -10,8 +10,12 @@
 //     columns in the bitmap, a popcount prefix turns the bitmap into a compact slot index, pass 2 accumulates
 //     a_ik * t_kj into the compact accumulator with k ASCENDING and a separate multiply and add, so the value of
 //     every entry does not depend on scheduling (and A A is bitwise symmetric when H is);
-//   - walking the bitmap emits the columns in ascending order, so no sort is ever needed.
-// Bound: L2/shared-memory latency (integer + a few FP64 operations per candidate); it runs once per graph.
+//   - walking the bitmap emits the columns in ascending order, so no sort is ever needed;
+//   - the candidate bitmaps of pass 1 are computed once (the sizing pass keeps them in global memory for the numeric
+//     pass, gbe_set_build_scratch_limit), and with the default power 2 only the upper triangle of A A is formed, each
+//     walk starting at the first column >= i of every T row (k_first_upper).
+// Bound: instruction issue and the latency of dependent L2 loads at 3-4 warps per scheduler (the bitmap, its ranks and
+// the accumulator of every warp live in shared memory); ncu counters in profiles/r01_spgemm_ncu.md.
 #include "gbe_internal.cuh"
 
 static size_t g_bm_save_max = (size_t)8 << 30;  // gbe_set_build_scratch_limit
