@@ -34,14 +34,17 @@ if ROOT not in sys.path:
 
 METRIC = "density_matrix_orbitals_per_s"
 UNIT = "orbitals/s"
-# FP64 tensor peak: MEASURED_PEAKS.json has no FP64 entry.  Rule of the profiling guide: another dtype's
-# measured peak x the nominal ratio.  Nominal B200 dense: bf16 2250 TF, FP64 tensor 40 TF (128 flop/clk/SM x 148 SMs
-# x 1.965 GHz = 37.2 TF is the issue-rate ceiling; a register-resident DMMA.8x8x4 loop measured 37.07 TF, cuBLAS DGEMM
-# 8192^3 35.3 TF on this pool - profiles/r01_fp64_peak_probe.md).
-FP64_NOMINAL_TF, BF16_NOMINAL_TF = 40.0, 2250.0
-DMMA_PROBE_TF = 37.07
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_x2 launch, from the committed ncu capture of this bench command
-X2_DRAM_BYTES_PER_LAUNCH = {"water4096": 2.01e9}
+# FP64 tensor ceiling.  MEASURED_PEAKS.json has no FP64 entry and the profiling guide states no nominal FP64
+# figure, so the ceiling is MEASURED IN THIS RUN, before the timed region, the way the driver measures bf16: cuBLAS DGEMM
+# (torch.matmul, float64, 8192^3), best of 10 (burst) and back to back for 4 s (sustained) -> roofline.peak.  Beside it:
+# the DMMA issue rate = 128 flop/clk/SM (one DMMA.8x8x4 = 512 flop per 16 cycles per SM sub-partition, measured in
+# profiles/r01_fp64_peak_probe.md) x SM count x the SM clock sampled during the timed region.
+DMMA_FLOP_PER_CLK_PER_SM = 128.0
+HBM_NOMINAL_GBS = 8000.0  # north_star: "about 8 TB/s"
+X2_TRAFFIC_JSON = os.path.join(ROOT, "profiles", "x2_traffic.json")
+X2_SOURCE = os.path.join(ROOT, "paper_1603_00937_b200", "csrc", "gbe_x2.cu")
+# one oracle pass over the 4,096-molecule box takes about 28 s on the box's 16 host cores (BENCH_r01)
+ORACLE_S_PER_MOLECULE_16_CORES = 28.0 / 4096
 
 WORKLOADS = {
     # name: (molecules, communities) - BASELINE.json configs[1], configs[2] (SURVEY numbering: config 2, config 3)
@@ -68,6 +71,88 @@ def load_peaks():
         return dict(hbm_gbs=float(p["hbm_gbs"]), bf16_tf=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
                     source="MEASURED_PEAKS.json (of measured)")
     return dict(hbm_gbs=6650.0, bf16_tf=1400.0, source="B200_PROFILING.md fallback (of fallback)")
+
+
+def git_blob_sha1(path: str) -> str:
+    """The git blob hash of a file's current content (what `git hash-object` prints)."""
+    import hashlib
+    data = open(path, "rb").read()
+    return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+
+
+def x2_traffic(workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one k_x2 launch from the tracked ncu record - only if that record
+    was captured on this workload AND on the gbe_x2.cu that is being run now (git blob hash); else None."""
+    try:
+        with open(X2_TRAFFIC_JSON) as f:
+            rec = json.load(f)
+    except (OSError, ValueError):
+        return None, "no profiles/x2_traffic.json"
+    if rec.get("workload") != workload:
+        return None, "profiles/x2_traffic.json was captured on workload %r" % rec.get("workload")
+    if rec.get("gbe_x2_cu_blob") != git_blob_sha1(X2_SOURCE):
+        return None, "profiles/x2_traffic.json was captured on another version of gbe_x2.cu (blob %s)" % rec.get("gbe_x2_cu_blob")
+    return float(rec["dram_bytes_per_launch"]), "B per launch, dram read + write, %s" % rec.get("source", "ncu --set full")
+
+
+def record_traffic(args) -> None:
+    """--record-traffic RAW.csv: reads an `ncu -i ... --page raw --csv` export of a `--set full` capture of k_x2 on this
+    workload and writes profiles/x2_traffic.json (mean over the captured full-size launches), stamped with the git blob
+    hash of the gbe_x2.cu in the tree."""
+    import csv
+    rows = list(csv.reader(open(args.record_traffic)))
+    hdr = rows[0]
+    k_name, k_rd, k_wr, k_grid = (hdr.index(c) for c in ("Kernel Name", "dram__bytes_read.sum", "dram__bytes_write.sum", "Grid Size"))
+    unit_rd, unit_wr = rows[1][k_rd], rows[1][k_wr]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    per = []
+    for r in rows[2:]:
+        if "k_x2" in r[k_name]:
+            per.append((int(r[k_grid].strip("()").split(",")[0]),
+                        float(r[k_rd].replace(",", "")) * scale[unit_rd] + float(r[k_wr].replace(",", "")) * scale[unit_wr]))
+    assert per, "no k_x2 launch in the capture"
+    full = max(g for g, _ in per)
+    vals = [b for g, b in per if g == full]
+    rec = {"workload": args.workload, "kernel": "k_x2<4,0>", "grid": full, "launches_averaged": len(vals),
+           "dram_bytes_per_launch": float(np.mean(vals)), "gbe_x2_cu_blob": git_blob_sha1(X2_SOURCE),
+           "source": args.traffic_source or os.path.basename(args.record_traffic)}
+    with open(X2_TRAFFIC_JSON, "w") as f:
+        json.dump(rec, f, indent=1)
+        f.write("\n")
+    print(json.dumps(rec))
+
+
+def measure_fp64_peak(torch) -> dict:
+    """cuBLAS DGEMM in this process, before the timed region (a library call, used for the roofline denominator only):
+    torch.matmul on float64 8192^3, best of 10 (burst) and back to back for ~4 s (sustained), CUDA events."""
+    n = 8192
+    a = torch.randn(n, n, dtype=torch.float64, device="cuda")
+    b = torch.randn(n, n, dtype=torch.float64, device="cuda")
+    c = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    flop = 2.0 * n ** 3
+    for _ in range(2):
+        torch.matmul(a, b, out=c)
+    torch.cuda.synchronize()
+    best = float("inf")
+    for _ in range(10):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        torch.matmul(a, b, out=c)
+        e1.record()
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    reps = max(10, int(4000.0 / best))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        torch.matmul(a, b, out=c)
+    e1.record()
+    torch.cuda.synchronize()
+    sustained = e0.elapsed_time(e1) / reps
+    del a, b, c
+    torch.cuda.empty_cache()
+    return {"burst_tflops": flop / (best * 1e-3) * 1e-12, "sustained_tflops": flop / (sustained * 1e-3) * 1e-12,
+            "reps_sustained": reps}
 
 
 class ClockSampler:
@@ -141,10 +226,24 @@ def cpu_cores() -> int:
         return os.cpu_count() or 1
 
 
-def sample_description(s) -> str:
+def sample_description(s, workload_mol: int) -> str:
+    if s.meta["n_mol"] == workload_mol:
+        return (f"the whole workload: {s.meta['n_mol']}-molecule water box ({s.n} orbitals, {s.n_part} communities), "
+                f"tau={s.tau:g}, {s.iters} SP2 iterations, one full pass of the oracle per step")
     return (f"{s.meta['n_mol']}-molecule water box ({s.n} orbitals, {s.n_part} communities): same construction, density, "
             f"tau={s.tau:g} and {s.iters} SP2 iterations as the workload; the path is linear scaling, so cost per orbital "
             "does not depend on the box size")
+
+
+def oracle_sample_molecules(workload: str, oracle_passes: int, budget_s: float) -> int:
+    """The largest box (the workload itself if it fits) whose `oracle_passes` oracle passes end within budget_s on the
+    cores this process may use; the oracle's cost is linear in the number of molecules (same density, same tau)."""
+    full = WORKLOADS[workload][0] or 4096
+    per_mol = ORACLE_S_PER_MOLECULE_16_CORES * max(1.0, 16.0 / cpu_cores())
+    n_mol = full
+    while n_mol > 256 and oracle_passes * n_mol * per_mol > budget_s:
+        n_mol //= 2
+    return n_mol
 
 
 def run_reference(args) -> None:
@@ -153,7 +252,8 @@ def run_reference(args) -> None:
     if rank != 0:
         return
     total = args.steps + args.warmup
-    n_mol = 1024 if total <= 4 else (512 if total <= 12 else 256)
+    # the real workload when all passes fit ~5 minutes (28 s per pass on 16 cores), else a smaller box of the same model
+    n_mol = oracle_sample_molecules(args.workload, total, 300.0)
     import gbe_inputs as gi
     s = gi.water_box(n_mol, n_mol // 8, seed=0)
     for _ in range(args.warmup):
@@ -165,8 +265,10 @@ def run_reference(args) -> None:
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "note": "CPU oracle (numpy/scipy, host BLAS), bounded sample per step"},
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle", "sample": sample_description(s)},
+        "config": {"workload": args.workload, "note": "CPU oracle (numpy/scipy, host BLAS), bounded sample per step",
+                   "sample_is_the_workload": s.meta["n_mol"] == (WORKLOADS[args.workload][0] or -1)},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle",
+                         "sample": sample_description(s, WORKLOADS[args.workload][0] or -1)},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -224,6 +326,9 @@ def run_ours(args) -> None:
         dist.barrier()
     import paper_1603_00937_b200 as gbe
     gbe.lib()
+
+    fp64_peak = measure_fp64_peak(torch)  # cuBLAS DGEMM, this process, before anything is timed
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
 
     s = make_system(args.workload, seed=rank)  # replicas: one independent seeded box per rank
     stream = torch.cuda.current_stream()
@@ -313,13 +418,21 @@ def run_ours(args) -> None:
 
     if rank == 0:
         peaks = load_peaks()
-        peak_tf = peaks["bf16_tf"] * FP64_NOMINAL_TF / BF16_NOMINAL_TF
         x2_ms = ph["x2_ms"] / max(1, ph["x2_launches"])
-        alg_tf = info["sp2_flops_per_iter"] / (x2_ms * 1e-3) * 1e-12
-        exec_tf = info["sp2_exec_flops_per_iter"] / (x2_ms * 1e-3) * 1e-12
+        per_s = 1.0 / (x2_ms * 1e-3) * 1e-12
+        sym_tf = info["sp2_sym_flops_per_iter"] * per_s    # what the method needs with X = X^T ("m^3 if symmetry is exploited")
+        alg_tf = info["sp2_flops_per_iter"] * per_s        # 2 m^3, symmetry not counted: an EFFECTIVE rate, never divided by a peak
+        exec_tf = info["sp2_exec_flops_per_iter"] * per_s  # issued to the FP64 tensor pipe (8x8 sub-tiles on/above the diagonal, K padded to ld)
+        peak_tf = fp64_peak["sustained_tflops"]            # the X^2 launches run back to back inside a long step
+        issue_tf = (DMMA_FLOP_PER_CLK_PER_SM * sm_count * clk["sm_mhz"] * 1e6 * 1e-12) if clk.get("sm_mhz") else None
+        traffic, traffic_note = x2_traffic(args.workload)
         nnzH = int(s.H.nnz)
-        gather_bytes = info["dense_elems"] * 8 + 12.0 * nnzH * info["sum_m"] / info["n"]
+        gather_bytes = info["dense_elems"] * 8 + 12.0 * nnzH * info["sum_m"] / info["n"]   # every H row re-read by each subgraph holding it
+        gather_dram_bytes = info["dense_elems"] * 8 + 12.0 * nnzH + 8.0 * (info["n"] + 1)  # compulsory: write X once, read H once
         scatter_bytes = 16.0 * info["nnz_D"]
+        gather_gbs = gather_bytes / (ph["gather_ms"] * 1e-3) * 1e-9
+        gather_dram_gbs = gather_dram_bytes / (ph["gather_ms"] * 1e-3) * 1e-9
+        scatter_gbs = scatter_bytes / (ph["scatter_ms"] * 1e-3) * 1e-9
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
@@ -339,13 +452,23 @@ def run_ours(args) -> None:
             "clocks": clk,
             "roofline": {
                 "kernel": "k_x2 (Y = X X^T on DMMA.8x8x4, fused branch/trace epilogue)", "bound": "tensor",
-                "achieved": alg_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": alg_tf / peak_tf,
-                "traffic": X2_DRAM_BYTES_PER_LAUNCH.get(args.workload), "traffic_unit": "B per launch (dram read + write, ncu --set full, profiles/r01_x2_v8_ncu.md); algorithmic bytes per launch = %.3g" % (16.0 * info["dense_elems"]),
-                "basis": "algorithmic 2 m^3 flop per community per iteration (unpadded, symmetry not counted) / mean "
-                         "CUDA-event time of the %d launches" % ph["x2_launches"],
-                "peak_source": "FP64: %s bf16 sustained %.1f TF x nominal 40/2250" % (peaks["source"], peaks["bf16_tf"]),
-                "executed_tflops": exec_tf, "executed_frac_of_dmma_probe": exec_tf / DMMA_PROBE_TF,
-                "dmma_probe_peak": DMMA_PROBE_TF, "ms_per_launch": x2_ms,
+                "achieved": sym_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": sym_tf / peak_tf,
+                "traffic": traffic, "traffic_note": traffic_note,
+                "algorithmic_bytes_per_launch": 16.0 * info["dense_elems"],
+                "basis": "sum_p m_p^2 (m_p + 1) flop per launch - one SP2 iteration of the whole batch with X = X^T used "
+                         "(entries on or above the diagonal of X_p^2, unpadded; gbe_graph_info.sp2_sym_flops_per_iter) - / mean "
+                         "CUDA-event time of the %d full launches" % ph["x2_launches"],
+                "flop_per_launch": info["sp2_sym_flops_per_iter"], "ms_per_launch": x2_ms,
+                "peak_source": "cuBLAS DGEMM f64 8192^3 (torch.matmul), this run, sustained over %d back-to-back calls; "
+                               "MEASURED_PEAKS.json has no FP64 entry" % fp64_peak["reps_sustained"],
+                "peak_burst": fp64_peak["burst_tflops"],
+                "issue_rate_peak": issue_tf,
+                "issue_rate_source": "%g flop/clk/SM (DMMA.8x8x4 every 16 cycles per SM sub-partition, profiles/"
+                                     "r01_fp64_peak_probe.md) x %d SMs x median SM clock sampled in the timed region"
+                                     % (DMMA_FLOP_PER_CLK_PER_SM, sm_count),
+                "frac_of_issue_rate": sym_tf / issue_tf if issue_tf else None,
+                "executed_tflops": exec_tf, "executed_frac_of_issue_rate": exec_tf / issue_tf if issue_tf else None,
+                "effective_tflops_2m3": alg_tf,
                 "last_iteration": {"note": "launch %d of %d computes the tiles with a core row only (Eq.(6): the core "
                                            "columns are kept); timed apart and not part of the mean above"
                                            % (s.iters, s.iters),
@@ -356,18 +479,26 @@ def run_ours(args) -> None:
                           "x2": ph["x2_ms"] + ph["x2_last_ms"],
                           "trace_branch": ph["trace_ms"], "scatter": ph["scatter_ms"], "density_total": ph["total_ms"]},
             "sp2_solves_per_s": info["n_part"] / ((ph["x2_ms"] + ph["x2_last_ms"] + ph["trace_ms"]) * 1e-3),
-            "hbm": {"peak_gbs": peaks["hbm_gbs"],
-                    "gather_gbs": gather_bytes / (ph["gather_ms"] * 1e-3) * 1e-9,
-                    "gather_frac": gather_bytes / (ph["gather_ms"] * 1e-3) * 1e-9 / peaks["hbm_gbs"],
-                    "scatter_gbs": scatter_bytes / (ph["scatter_ms"] * 1e-3) * 1e-9,
-                    "scatter_frac": scatter_bytes / (ph["scatter_ms"] * 1e-3) * 1e-9 / peaks["hbm_gbs"]},
+            "hbm": {"peak_gbs": peaks["hbm_gbs"], "peak_source": peaks["source"], "nominal_gbs": HBM_NOMINAL_GBS,
+                    "gather_gbs": gather_gbs, "gather_frac": gather_gbs / peaks["hbm_gbs"],
+                    "gather_frac_nominal": gather_gbs / HBM_NOMINAL_GBS,
+                    "gather_dram_gbs": gather_dram_gbs, "gather_dram_frac": gather_dram_gbs / peaks["hbm_gbs"],
+                    "gather_note": "gather_gbs counts SURVEY 8(a)'s bytes (each H row read by every subgraph that holds "
+                                   "it; those re-reads are L2 hits); gather_dram_gbs counts compulsory DRAM bytes only "
+                                   "(X written once, H read once)",
+                    "scatter_gbs": scatter_gbs, "scatter_frac": scatter_gbs / peaks["hbm_gbs"],
+                    "scatter_frac_nominal": scatter_gbs / HBM_NOMINAL_GBS},
         }
         if world == 1 and not args.no_cpu_baseline:
             import gbe_inputs as gi
-            cs = gi.water_box(1024, 128, seed=0)
+            # one pass of the oracle over the workload itself when that is ~30 s of CPU work (the 4,096-molecule box on
+            # 16 cores), else over the largest smaller box of the same model that is
+            full_mol = WORKLOADS[args.workload][0] or -1
+            n_mol = oracle_sample_molecules(args.workload, 1, 45.0)
+            cs = s if (n_mol == full_mol and s.meta.get("kind") == "water") else gi.water_box(n_mol, n_mol // 8, seed=0)
             dt = oracle_step(cs)
             line["cpu_baseline"] = {"value": cs.n / dt, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle",
-                                    "seconds": dt, "sample": sample_description(cs)}
+                                    "seconds": dt, "sample": sample_description(cs, full_mol)}
         print(json.dumps(line), flush=True)
     g.free()
     if world > 1:
@@ -568,8 +699,12 @@ def main() -> None:
     ap.add_argument("--small", action="store_true", help="small systems: tiled kernels against the shared-memory-resident SP2 kernel")
     ap.add_argument("--gapped", action="store_true", help="sweep on the gapped variant of the water model, run to idempotency")
     ap.add_argument("--no-exact", action="store_true", help="sweep without the exact projector (no error columns)")
+    ap.add_argument("--record-traffic", default="", help="ncu raw-page CSV of a --set full capture of k_x2: write profiles/x2_traffic.json")
+    ap.add_argument("--traffic-source", default="", help="the profiles/ summary that documents the capture")
     args = ap.parse_args()
-    if args.sweep:
+    if args.record_traffic:
+        record_traffic(args)
+    elif args.sweep:
         run_sweep(args)
     elif args.small:
         run_small(args)

@@ -95,6 +95,9 @@ typedef struct {
   int32_t resident_cluster;  /* 1: all communities fit ONE thread-block cluster (n_part <= 16): the resident kernel then
                                 exchanges the traces through distributed shared memory and the cluster barrier */
   int32_t reserved_;
+  double sp2_sym_flops_per_iter; /* sum_p m_p^2 (m_p + 1): the flops of one SP2 iteration the METHOD needs when the symmetry
+                                    of X_p is used (only the entries on or above the diagonal of X_p^2 are formed; obs. (x)
+                                    P:L65) - the numerator of bench.py's roofline fraction */
 } gbe_graph_info;
 
 /* SP2 log (host memory, caller-allocated; valid after the stream has been synchronised).

@@ -48,7 +48,7 @@ class _GraphInfo(C.Structure):
                 ("eps_min", C.c_double), ("eps_max", C.c_double),
                 ("contiguous_cores", C.c_int32), ("tile", C.c_int32), ("workspace_bytes", C.c_size_t),
                 ("workspace_bytes_fermi", C.c_size_t), ("resident_sp2", C.c_int32), ("resident_fits", C.c_int32),
-                ("resident_cluster", C.c_int32), ("reserved_", C.c_int32)]
+                ("resident_cluster", C.c_int32), ("reserved_", C.c_int32), ("sp2_sym_flops_per_iter", C.c_double)]
 
 
 class _Sp2Log(C.Structure):

@@ -181,6 +181,7 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   o->n_tiles = g->n_items;
   o->sp2_flops_per_iter = g->flops_per_iter;
   o->sp2_exec_flops_per_iter = g->exec_flops_per_iter;
+  o->sp2_sym_flops_per_iter = g->sym_flops_per_iter;
   o->n_tiles_last = g->n_items_last;
   o->sp2_flops_last_iter = g->flops_last_iter;
   o->sp2_exec_flops_last_iter = g->exec_flops_last_iter;

@@ -298,6 +298,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   g->max_ncore = 0;
   g->nnz_D = 0;
   g->flops_per_iter = 0;
+  g->sym_flops_per_iter = 0;
   for (int p = 0; p < n_part; ++p) {
     const int64_t m = g->h_m[p];
     const int64_t ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
@@ -307,6 +308,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     g->max_ncore = std::max<int32_t>(g->max_ncore, g->h_ncore[p]);
     g->nnz_D += m * g->h_ncore[p];
     g->flops_per_iter += 2.0 * (double)m * (double)m * (double)m;
+    g->sym_flops_per_iter += (double)m * (double)m * (double)(m + 1);  // m (m + 1) / 2 entries of 2 m flop each
   }
   g->sum_m = h_sub_ptr[n_part];
   g->dense_elems = g->h_dense_off[n_part];

@@ -93,6 +93,7 @@ struct gbe_graph {
   int32_t n_part = 0, max_m = 0, max_ncore = 0, tile = 64;
   double eps_min = 0, eps_max = 0, tau = 0, flops_per_iter = 0, exec_flops_per_iter = 0;
   double flops_last_iter = 0, exec_flops_last_iter = 0;  // the core-tiles-only last iteration
+  double sym_flops_per_iter = 0;  // sum m^2 (m + 1): upper triangle incl. diagonal of X_p^2
   int32_t power = 2, contiguous = 1;
   // device arrays (owned)
   int64_t* S_row_ptr = nullptr;  // n+1

@@ -11,6 +11,7 @@ import scipy.sparse as sp
 
 import gbe_inputs as gi
 import oracle as o
+from oracle.gbe_oracle import _branch
 
 HERE = os.path.dirname(__file__)
 
@@ -80,6 +81,55 @@ def test_graph_brute_force(tau, power):
     rp, ci = o.build_graph(s.H, tau, power=power)
     got = {(i, int(j)) for i in range(s.n) for j in ci[rp[i]:rp[i + 1]]}
     assert got == brute_graph(s.H.to_dense(), tau, power)
+
+
+def brute_graph_diag_dropped(Hd, tau, power):
+    """brute_graph with the MISTAKE the missing-diagonal branch of normalised_x0 guards against: an unstored H_kk
+    treated as 'no entry of X0' (X0_kk = 0) instead of X0_kk = eps_max / (eps_max - eps_min) (A-12)."""
+    n = Hd.shape[0]
+    lo = min(Hd[i, i] - sum(abs(Hd[i, j]) for j in range(n) if j != i) for i in range(n))
+    hi = max(Hd[i, i] + sum(abs(Hd[i, j]) for j in range(n) if j != i) for i in range(n))
+    A = [[(((hi if i == j else 0.0) - Hd[i, j]) / (hi - lo)) if Hd[i, j] != 0.0 else 0.0 for j in range(n)] for i in range(n)]
+    A = [[v if abs(v) >= tau else 0.0 for v in row] for row in A]
+    edges = {(i, i) for i in range(n)} | {(i, j) for i in range(n) for j in range(n) if A[i][j] != 0.0}
+    T = A
+    for _ in range(2, power + 1):
+        Tn = [[0.0] * n for _ in range(n)]
+        for i in range(n):
+            for j in range(n):
+                s = sum(A[i][k] * T[k][j] for k in range(n) if A[i][k] != 0.0 and T[k][j] != 0.0)
+                if abs(s) >= tau:
+                    Tn[i][j] = s
+                    edges.add((i, j))
+        T = Tn
+    return edges | {(j, i) for (i, j) in edges}
+
+
+def test_unstored_diagonal_is_a_zero_of_H_not_of_X0():
+    """A-12: a row of H without a stored diagonal has H_kk = 0, hence X0_kk = eps_max / (eps_max - eps_min) != 0.
+    Pins the missing-diagonal branch of normalised_x0 (and through it build_graph) against explicit loops over the
+    dense matrix.  The diagonal of A enters the VALUES of T^(2) = floor(A A)_tau on the pattern of A, so it decides edges
+    from power 3 on (at power 2 a term A_ii A_ij needs A_ij != 0, an edge already): the test demands that dropping the
+    diagonal WOULD change the graph, so that the branch is really exercised."""
+    sensitive = 0
+    for seed in range(6):
+        s = gi.random_banded(14, half_bw=2, seed=40 + seed)
+        Hd = s.H.to_dense()
+        Hd[np.arange(0, 14, 2), np.arange(0, 14, 2)] = 0.0  # every other diagonal entry unstored
+        H = gi.CSR.from_dense(Hd)
+        assert H.nnz == s.H.nnz - 7
+        lo, hi = o.gershgorin(H)
+        X0 = o.normalised_x0(H, lo, hi).toarray()
+        for i in range(14):
+            for j in range(14):  # (eps_max delta_ij - H_ij) / (eps_max - eps_min), written out
+                assert X0[i, j] == ((hi if i == j else 0.0) - Hd[i, j]) / (hi - lo)
+        for power in (2, 3, 4):
+            for tau in (0.05, 5e-3, 2e-3, 1e-3):
+                rp, ci = o.build_graph(H, tau, power=power)
+                got = {(i, int(j)) for i in range(14) for j in ci[rp[i]:rp[i + 1]]}
+                assert got == brute_graph(Hd, tau, power)
+                sensitive += got != brute_graph_diag_dropped(Hd, tau, power)
+    assert sensitive >= 3
 
 
 def test_graph_properties():
@@ -167,6 +217,24 @@ def test_two_level_closed_form():
     r = o.o_sub(H, rp, ci, np.zeros(2, np.int32), 1, 1.0, 40)
     ref = 0.5 * (np.eye(2) - np.array([[a, b], [b, -a]]) / np.hypot(a, b))
     np.testing.assert_allclose(dense_D(r, 2), ref, atol=1e-14)
+
+
+def test_branch_tie_takes_2x_minus_x2_hand_worked():
+    """A-6: a tie of the two next-trace errors goes to 2X - X^2.  Hand-worked, every number exact in binary:
+    H = diag(-1, 0, 1), no off-diagonals: eps_min = -1, eps_max = 1, X0 = diag(1, 1/2, 0); t1 = 3/2, t2 = 5/4.
+    n_occ = 3/2: |t2 - n_occ| = 1/4 = |2 t1 - t2 - n_occ| -> tie -> branch 1: X1 = diag(1, 3/4, 0), t1 = 7/4, t2 = 25/16.
+    (The other direction would give X1 = diag(1, 1/4, 0), t1 = 5/4.)  Then |25/16 - 3/2| = 1/16 < |7/2 - 25/16 - 3/2| = 7/16
+    -> branch 0: X2 = diag(1, 9/16, 0)."""
+    assert _branch(1.0, 0.5, 1.0) == 1  # |0.5 - 1| == |2 - 0.5 - 1|
+    assert _branch(1.5, 1.25, 1.5) == 1
+    H = gi.CSR.from_dense(np.diag([-1.0, 1e-300, 1.0]))  # the middle diagonal entry stored (value ~ 0)
+    rp, ci = o.build_graph(H, 1e-5)
+    for n_part, part in ((1, np.zeros(3, np.int32)), (3, np.arange(3, dtype=np.int32))):
+        r = o.o_sub(H, rp, ci, part, n_part, 1.5, 2)
+        assert (r.eps_min, r.eps_max) == (-1.0, 1.0)
+        assert list(r.branch) == [1, 0]
+        assert list(r.t1) == [1.5, 1.75, 1.5625] and list(r.t2[:2]) == [1.25, 1.5625]
+        np.testing.assert_array_equal(np.diag(dense_D(r, 3)), [1.0, 0.5625, 0.0])
 
 
 @pytest.mark.parametrize("system", ["chain", "banded"])
