@@ -94,10 +94,12 @@ typedef struct {
   int32_t resident_fits;     /* 1: the largest community fits that kernel (max_m <= 160); see gbe_graph_set_sp2_path */
   int32_t resident_cluster;  /* 1: all communities fit ONE thread-block cluster (n_part <= 16): the resident kernel then
                                 exchanges the traces through distributed shared memory and the cluster barrier */
-  int32_t reserved_;
+  int32_t sp2_path_chosen;   /* the kernels gbe_density will run for steps 4-5 of this graph: 1 tiled, 2 resident, 3 packed */
   double sp2_sym_flops_per_iter; /* sum_p m_p^2 (m_p + 1): the flops of one SP2 iteration the METHOD needs when the symmetry
                                     of X_p is used (only the entries on or above the diagonal of X_p^2 are formed; obs. (x)
                                     P:L65) - the numerator of bench.py's roofline fraction */
+  int64_t n_small;           /* communities with 0 < m_p <= 160: the ones the packed kernel can take */
+  int64_t n_bins;            /* CTAs of one packed launch (bins of 1..16 small communities) */
 } gbe_graph_info;
 
 /* SP2 log (host memory, caller-allocated; valid after the stream has been synchronised).
@@ -143,17 +145,24 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* out);
 int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, int32_t* S_col, int64_t* sub_ptr,
                      int32_t* sub_idx, int32_t* ncore, int64_t* D_row_ptr, int32_t* D_col);
 
-/* Which kernels run the SP2 loop (steps 4-5) of this graph.  Two implementations compute the same updates:
+/* Which kernels run the SP2 loop (steps 4-5) of this graph.  Three implementations compute the same updates:
  *   tiled    (any size)  one X^2 launch + one trace/branch launch per iteration over the batched dense layout in HBM;
+ *   packed   (communities with m_p <= 160, any number of them; the cost law P:L78 - more partitions, smaller m)
+ *            one launch per iteration: a CTA copies a bin of 1..16 whole matrices to shared memory, squares them on the
+ *            FP64 tensor cores, writes them back; the bin that finishes last reduces the traces and takes the branch
+ *            decision, so there is no separate trace/branch launch.  Larger communities of the same graph go through the
+ *            tiled kernel in the same iteration;
  *   resident (max_m <= 160) ONE launch for the whole loop, X_p held in shared memory by one CTA per community; the
  *            global trace (one sequence for all subgraphs) is exchanged through a grid barrier, which needs all
  *            communities co-resident (cooperative launch; one thread-block cluster with the exchange in distributed
  *            shared memory when there are at most 16 communities) - unless the sequence is preset and no trace is logged
  *            (gbe_density_preset with trace_every_iteration = 0), where the CTAs never communicate.
- * path = 0 (default): resident when it applies and all communities fit the device at once, else tiled;
+ * path = 0 (default): resident when it applies and all communities fit the device at once; else packed when the graph
+ *        has enough small communities to occupy the device; else tiled;
  *        1: always tiled;  2: resident whenever it can run (GBE_EINVAL if max_m is too large; calls for which the
- *        communities are not co-resident still take the tiled kernels).
- * Results of the two paths agree to rounding (different summation order of the global trace), each is bitwise
+ *        communities are not co-resident still take the tiled kernels);  3: packed whenever the graph has a community
+ *        with m_p <= 160 (else tiled).
+ * Results of the paths agree to rounding (different summation order of the global trace), each is bitwise
  * reproducible.  Not thread safe against concurrent calls on the same graph. */
 int gbe_graph_set_sp2_path(gbe_graph* g, int32_t path);
 

@@ -48,7 +48,8 @@ class _GraphInfo(C.Structure):
                 ("eps_min", C.c_double), ("eps_max", C.c_double),
                 ("contiguous_cores", C.c_int32), ("tile", C.c_int32), ("workspace_bytes", C.c_size_t),
                 ("workspace_bytes_fermi", C.c_size_t), ("resident_sp2", C.c_int32), ("resident_fits", C.c_int32),
-                ("resident_cluster", C.c_int32), ("reserved_", C.c_int32), ("sp2_sym_flops_per_iter", C.c_double)]
+                ("resident_cluster", C.c_int32), ("sp2_path_chosen", C.c_int32), ("sp2_sym_flops_per_iter", C.c_double),
+                ("n_small", C.c_int64), ("n_bins", C.c_int64)]
 
 
 class _Sp2Log(C.Structure):
@@ -226,7 +227,7 @@ def gbe_update_graph(prev: Graph, D_prev: torch.Tensor, H: DeviceCSR, tau: float
 
 
 def gbe_graph_set_sp2_path(g: "Graph", path: int) -> None:
-    """0 auto, 1 tiled kernels, 2 shared-memory-resident kernel (include/gbe.h)."""
+    """0 auto, 1 tiled kernels, 2 shared-memory-resident kernel, 3 packed kernel for the small communities (include/gbe.h)."""
     _check(lib().gbe_graph_set_sp2_path(g._h, int(path)))
     info = _GraphInfo()
     _check(lib().gbe_graph_get_info(g._h, C.byref(info)))

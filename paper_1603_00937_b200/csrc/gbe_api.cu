@@ -46,6 +46,7 @@ __global__ void k_init_state(gbe_state* st, double n_occ, double idem_tol, int i
   st->iters_done = mode == 2 ? iters : 0;
   st->preset = mode != 0;
   st->bar = 0;
+  st->ticket = 0;
 }
 
 struct WS {
@@ -98,7 +99,7 @@ const char* gbe_strerror(int status) {
 void gbe_free_graph(gbe_graph* g) {
   if (!g) return;
   void* ptrs[] = {g->S_row_ptr, g->S_col,     g->sub_ptr,  g->sub_idx,  g->ncore,    g->msize, g->dense_off, g->D_row_ptr,
-                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va};
+                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->items_h, g->items_last_h, g->pk_ctas, g->pk_slots, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   delete g;
@@ -166,7 +167,7 @@ int gbe_update_graph(const gbe_graph* prev, const double* D_prev, const gbe_csr_
   return build_graph_impl(H, opts, part, n_part, cuda_stream, out, prev, D_prev);
 }
 
-static bool use_resident(const gbe_graph* g, int mode);
+static int choose_sp2(const gbe_graph* g, int mode);
 
 int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   if (!g || !o) return GBE_EINVAL;
@@ -191,7 +192,10 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   o->tile = g->tile;
   o->workspace_bytes = g->ws_bytes;
   o->workspace_bytes_fermi = g->ws_bytes_fermi;
-  o->resident_sp2 = use_resident(g, 0) ? 1 : 0;
+  o->resident_sp2 = choose_sp2(g, 0) == 2 ? 1 : 0;
+  o->sp2_path_chosen = choose_sp2(g, 0);
+  o->n_small = g->pk_n_small;
+  o->n_bins = g->n_pk_ctas;
   o->resident_fits = g->resident_fits;
   o->resident_cluster = g->resident_cluster;
   return GBE_OK;
@@ -232,19 +236,26 @@ int gbe_gather(const gbe_csr_view* H, const gbe_graph* g, void* workspace, size_
   return do_gather(H, g, workspace, workspace_bytes, cuda_stream, nullptr);
 }
 
-// The resident kernel runs when the largest community fits in shared memory and, unless the sequence is preset and no
-// trace is logged (no exchange between CTAs), when all communities are co-resident (cooperative launch).
-static bool use_resident(const gbe_graph* g, int mode) {
-  if (g->sp2_path == 1 || !g->resident_fits || g->n_items == 0) return false;
-  const bool can = mode == 2 || g->n_part <= g->resident_coresident;
-  if (g->sp2_path == 2) return can;
-  // auto: one wave of CTAs, and communities small enough that one SM per community beats the tiled kernels
-  // (measured: 1.3 - 2.5x faster for m <= 128, 1.4x slower at m = 160)
-  return can && g->n_part <= g->resident_coresident && g->max_m <= 128;
+// Which kernels run steps 4-5 (1 tiled, 2 resident, 3 packed + tiled for the large communities); mode as in k_init_state.
+// The resident kernel needs the largest community in shared memory and, unless the sequence is preset and no trace is
+// logged (no exchange between CTAs), all communities co-resident (cooperative launch).  The packed kernel takes the
+// communities with m <= GBE_PK_MAX_M, any number of them.
+static int choose_sp2(const gbe_graph* g, int mode) {
+  if (g->n_items == 0 || g->sp2_path == 1) return 1;
+  const bool can_res = g->resident_fits && (mode == 2 || g->n_part <= g->resident_coresident);
+  const bool can_pk = g->n_pk_ctas > 0;
+  if (g->sp2_path == 2) return can_res ? 2 : 1;
+  if (g->sp2_path == 3) return can_pk ? 3 : 1;
+  // auto.  Resident: one launch for the whole loop - wins whenever the communities are small enough that one SM per
+  // community keeps up with the tiled kernels spreading the tiles over all SMs (measured).
+  if (can_res && (g->max_m <= 128 || g->n_part >= g->resident_coresident / 2)) return 2;
+  // Packed: enough small communities to occupy the device; the others of the same graph stay tiled.
+  if (can_pk && g->n_pk_ctas >= gbe_sm_count() / 2) return 3;
+  return 1;
 }
 
 int gbe_graph_set_sp2_path(gbe_graph* g, int32_t path) {
-  if (!g || path < 0 || path > 2) return GBE_EINVAL;
+  if (!g || path < 0 || path > 3) return GBE_EINVAL;
   if (path == 2 && !g->resident_fits) return GBE_EINVAL;
   g->sp2_path = path;
   return GBE_OK;
@@ -266,7 +277,8 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
   GBE_TRY(carve(g, workspace, workspace_bytes, &w));
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const int mode = !preset ? 0 : (trace_each ? 1 : 2);
-  if (use_resident(g, mode)) {
+  const int path = choose_sp2(g, mode);
+  if (path == 2) {
     // small communities: the whole loop in one kernel, X_p resident in shared memory (gbe_resident.cu)
     GBE_TRY(timed(tm, PH_TRACE, 1, [&]() -> int {
       k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode);
@@ -295,16 +307,26 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
     // Iteration iters - 1 is the last one whether or not the idempotency stop fires before it (then it is a no-op):
     // only the core rows and columns of its result are read again (trace, scatter), so it runs the core tiles only.
     const bool last = it == iters - 1;
+    if (path == 3) {
+      // small communities: bins in shared memory, one launch per iteration, step 5 taken by the bin that arrives last
+      // (gbe_small.cu); the larger communities of the same graph go through the tiled kernel first
+      const int n_pairs = g->n_items_last_h + g->n_pk_ctas;
+      GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, (g->n_items_h ? 1 : 0) + 1, [&]() -> int {
+        GBE_TRY(gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, true, s));
+        return gbe_launch_sp2_packed(g, w.st, in, outp, w.partials, g->n_items_last_h, n_pairs, it, last, mode != 2, s);
+      }));
+      continue;
+    }
     const int n_part_it = g->n_items_last;  // one packed partial per tile with a core row, in every iteration
     GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, g->n_items ? 1 : 0,
-                  [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, s); }));
+                  [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, false, s); }));
     if (mode != 2)
       GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, n_part_it, s); }));
   }
-  if (mode == 2)  // one trace kernel at the end: t1, t2 of the final X for the log (written at index iters)
-    GBE_TRY(timed(tm, PH_TRACE, 1, [&] {
-      return gbe_launch_trace_branch(w.st, w.partials, iters > 0 ? g->n_items_last : g->n_gitems, s);
-    }));
+  if (mode == 2) {  // one trace kernel at the end: t1, t2 of the final X for the log (written at index iters)
+    const int n_pairs = iters == 0 ? g->n_gitems : (path == 3 ? g->n_items_last_h + g->n_pk_ctas : g->n_items_last);
+    GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, n_pairs, s); }));
+  }
   return GBE_OK;
 }
 int gbe_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_tol, void* workspace, size_t workspace_bytes,

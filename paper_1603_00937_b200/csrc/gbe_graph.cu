@@ -445,8 +445,7 @@ struct Unioner {
     s = s_;
     W = (int)((n + 31) / 32);
     bm_bytes = (size_t)W * 4;
-    int sm_count = 148;
-    cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, 0);
+    const int sm_count = gbe_sm_count();  // of the current device
     uw = pick_warps(bm_bytes, 8);
     if (uw < 1) return GBE_EINVAL;  // n too large for a shared-memory bitmap
     GBE_CUDA(cudaFuncSetAttribute(k_union_rows<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bm_bytes * uw)));
@@ -504,8 +503,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   const int64_t n = H.n;
   const int W = (int)((n + 31) / 32);
   const int rows_grid = (int)((n + 7) / 8);
-  int sm_count = 148;
-  cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, 0);
+  const int sm_count = gbe_sm_count();  // of the current device
 
   if (check_sym) {
     DevBuf flag;
@@ -669,8 +667,7 @@ int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int3
                           cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S) {
   const int64_t n = H.n;
   const int W = (int)((n + 31) / 32);
-  int sm_count = 148;
-  cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, 0);
+  const int sm_count = gbe_sm_count();  // of the current device
   Unioner U;
   GBE_TRY(U.init(n, s));
   DevBuf cnt;

@@ -250,8 +250,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   const int n_part = g->n_part;
   const int W = (int)((n + 31) / 32);
   const int64_t blk = (n + n_part - 1) / n_part;
-  int sm_count = 148;
-  cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, 0);
+  const int sm_count = gbe_sm_count();  // of the current device
   const int tgrid = (int)((n + 255) / 256);
 
   // ---- cores
@@ -321,12 +320,13 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     std::vector<int32_t> order(n_part);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return g->h_m[a] > g->h_m[b]; });
-    std::vector<gbe_tile_item> items, last;
+    std::vector<gbe_tile_item> items, last, items_h, last_h;  // _h: the communities the packed kernel does not take
     const int tile = g->tile;
     g->exec_flops_per_iter = g->exec_flops_last_iter = g->flops_last_iter = 0;
     for (int p : order) {
       const int T = (g->h_m[p] + tile - 1) / tile;
       const int64_t ld = (g->h_m[p] + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+      const bool big = g->h_m[p] > GBE_PK_MAX_M;
       for (int ti = 0; ti < T; ++ti)
         for (int tj = ti; tj < T; ++tj) {
           // pidx: where the tile's trace partial goes - the tiles with a core row are numbered in list order (which is
@@ -335,6 +335,11 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
           items.push_back({core_row ? (int32_t)last.size() : -1, ti, tj, g->h_m[p], g->h_ncore[p], (int32_t)ld,
                            g->h_dense_off[p]});
           if (core_row) last.push_back(items.back());
+          if (big) {
+            items_h.push_back(items.back());
+            items_h.back().pidx = core_row ? (int32_t)last_h.size() : -1;
+            if (core_row) last_h.push_back(items_h.back());
+          }
         }
       // executed DMMA work: 8x8 sub-tiles (bi <= bj) with rows < m, columns < ld, each 2*8*8*ld flop
       const double R = (double)((g->h_m[p] + 7) / 8), C = (double)(ld / 8);
@@ -344,6 +349,12 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
       const double Rc = std::min(R, (double)(Tc * (tile / 8)));
       g->exec_flops_last_iter += (Rc * C - Rc * (Rc - 1) / 2) * 128.0 * (double)ld;
       g->flops_last_iter += 2.0 * (double)g->h_m[p] * (double)g->h_m[p] * (double)g->h_ncore[p];
+    }
+    g->n_items_h = (int32_t)items_h.size();
+    g->n_items_last_h = (int32_t)last_h.size();
+    if (!items_h.empty() && items_h.size() < items.size()) {  // only a mixed graph needs the second pair of lists
+      GBE_TRY(upload(items_h, &g->items_h, s));
+      GBE_TRY(upload(last_h, &g->items_last_h, s));
     }
     g->n_items = (int32_t)items.size();
     g->n_items_last = (int32_t)last.size();
@@ -360,7 +371,9 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     g->n_gitems = (int32_t)gi.size();
     GBE_TRY(upload(gi, &g->gitems, s));
   }
-  g->n_partials = std::max(std::max(g->n_items, g->n_gitems), 2 * n_part);  // the resident kernel double-buffers n_part pairs
+  GBE_TRY(gbe_build_packed(g, s));  // bins of the small communities (gbe_small.cu)
+  // the resident kernel double-buffers n_part pairs; the packed path writes one pair per bin behind the tiled kernel's
+  g->n_partials = std::max(std::max(std::max(g->n_items, g->n_gitems), 2 * n_part), g->n_items_last_h + g->n_pk_ctas);
   GBE_TRY(gbe_resident_capacity(g, &g->resident_fits, &g->resident_coresident, &g->resident_cluster));
 
   // workspace layout

@@ -74,9 +74,25 @@ struct gbe_state {
   int32_t degenerate;  // eps_max == eps_min
   int32_t preset;      // 1: the branch sequence br[] was given by the caller (gbe_density_preset)
   uint32_t bar;        // arrival counter of the resident kernel's grid barrier (reset by k_init_state)
+  uint32_t ticket;     // bins of the packed kernel that have published their partial this iteration (gbe_small.cu)
+  uint32_t pad_;
   double t1[GBE_MAX_ITERS + 1];
   double t2[GBE_MAX_ITERS + 1];
   uint8_t br[GBE_MAX_ITERS];
+};
+
+// packed small communities (gbe_small.cu): one CTA works on a bin of up to GBE_PK_MAX_SLOTS communities per launch
+constexpr int GBE_PK_MAX_M = 160;     // largest core + halo size the packed (and the resident) kernel holds in shared memory
+constexpr int GBE_PK_MAX_SLOTS = 16;  // communities per bin
+constexpr int GBE_PK_MAXU = 4;        // work units per warp (accumulator registers)
+struct gbe_pk_slot {  // one community of a bin (32 bytes)
+  int32_t p, m, nc, ld;  // community, core + halo size, core size, leading dimension
+  int32_t soff, R;       // offset of its X in the bin's shared memory (doubles), 8-row blocks
+  int64_t dense_off;     // element offset of X_p in a dense buffer
+};
+struct gbe_pk_cta {  // one bin (144 bytes)
+  int32_t first_slot, n_slots, smem_doubles, pad_;
+  uint16_t units[16][GBE_PK_MAXU];  // per warp: slot | row block | first column block | blocks (0xFFFF: none)
 };
 
 struct gbe_tile_item {  // one X^2 work item: tile (ti, tj), ti <= tj, of community p, with p's layout (32 bytes)
@@ -111,8 +127,18 @@ struct gbe_graph {
   int32_t* row_part = nullptr;   // sum_m: community of dense row q
   int64_t* row_src = nullptr;    // sum_m: element offset of dense row q in a dense buffer
   int32_t* row_nc = nullptr;     // sum_m: ncore of the community of dense row q
-  // SP2 path: 0 auto, 1 tiled kernels (gbe_x2.cu), 2 resident kernel (gbe_resident.cu); set by gbe_graph_set_sp2_path
+  // SP2 path: 0 auto, 1 tiled kernels (gbe_x2.cu), 2 resident kernel (gbe_resident.cu), 3 packed kernel for the small
+  // communities + tiled kernel for the others (gbe_small.cu); set by gbe_graph_set_sp2_path
   int32_t sp2_path = 0;
+  // packed path: bins of communities with m <= GBE_PK_MAX_M, and the tile lists of the OTHER communities
+  gbe_pk_cta* pk_ctas = nullptr;
+  gbe_pk_slot* pk_slots = nullptr;
+  int32_t n_pk_ctas = 0, pk_n_small = 0;
+  size_t pk_smem_bytes = 0;
+  double pk_dmma = 0, all_dmma = 0;  // DMMA instructions per iteration of the packed communities / of all communities
+  gbe_tile_item* items_h = nullptr;       // tiles of the communities with m > GBE_PK_MAX_M
+  gbe_tile_item* items_last_h = nullptr;  // those with a core row
+  int32_t n_items_h = 0, n_items_last_h = 0;
   // gather path: 0 auto, 1 staged (row buffer in shared memory), 2 direct (rows built in global memory); gbe_graph_set_gather_path
   int32_t gather_path = 0;
   int32_t resident_fits = 0, resident_coresident = 0;  // gbe_resident_capacity at build time
@@ -158,12 +184,17 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
                       cudaStream_t s);
 // step 4
 // iter: index n of the update X_n -> X_{n+1} (selects br[n] when the sequence is preset)
+// hybrid: only the tiles of the communities the packed kernel does not take (items_h / items_last_h)
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                  bool last, cudaStream_t s);
+                  bool last, bool hybrid, cudaStream_t s);
 // steps 4 + 5 in one kernel for small communities (gbe_resident.cu); mode as in k_init_state
 int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident, int* cluster);
 int gbe_launch_sp2_resident(const gbe_graph* g, gbe_state* st, double* X0, double* X1, double* partials, int mode,
                             cudaStream_t s);
+// steps 4 + 5, one iteration per launch, for communities with m <= GBE_PK_MAX_M (gbe_small.cu)
+int gbe_build_packed(gbe_graph* g, cudaStream_t s);
+int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials,
+                          int partial_base, int n_partials, int iter, bool last, bool fused, cudaStream_t s);
 // step 5
 int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s);
 // step 6
@@ -186,6 +217,12 @@ int gbe_launch_error_norms(const gbe_graph* g, const double* D_val, const double
 
 // small device utilities (gbe_util.cu)
 int32_t* gbe_pinned_words();  // 64 pinned host words per thread, or null
+int gbe_sm_count();           // multiprocessors of the CURRENT device (cached per device)
+// one-time set-up per DEVICE (function attributes, pool thresholds): first() is true once per device for this object
+struct gbe_device_once {
+  std::atomic<uint64_t> mask[4] = {};
+  bool first();
+};
 int gbe_exclusive_scan_i32_to_i64(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s);
 int gbe_exclusive_scan_i32_to_i64_max(const int32_t* in, int64_t* out, int64_t n, cudaStream_t s);
 
@@ -193,6 +230,24 @@ int gbe_exclusive_scan_i32_to_i64_max(const int32_t* in, int64_t* out, int64_t n
 // device helpers
 // ----------------------------------------------------------------------------------------------
 #ifdef __CUDACC__
+// Step 5's decision (A-6, A-7), taken by ONE thread from the global traces t1, t2 of X_k, k = st->iter: the log entry,
+// the idempotency stop, the branch of iteration k (preset or chosen).  Shared by k_trace_branch and by the kernels that
+// reduce the traces themselves.
+__device__ __forceinline__ void gbe_trace_decide(gbe_state* st, double t1, double t2) {
+  const double n_occ = st->n_occ;
+  const int k = st->iter;  // the partials describe X_k
+  st->t1[k] = t1;
+  st->t2[k] = t2;
+  st->iters_done = k;
+  if (k >= st->iters || (st->idem_tol >= 0.0 && k >= 1 && fabs(t1 - t2) <= st->idem_tol)) {
+    st->stop = 1;
+  } else {
+    const int b = st->preset ? (int)st->br[k] : ((fabs(t2 - n_occ) < fabs(2.0 * t1 - t2 - n_occ)) ? 0 : 1);
+    st->branch = b;
+    st->br[k] = (uint8_t)b;
+    st->iter = k + 1;
+  }
+}
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

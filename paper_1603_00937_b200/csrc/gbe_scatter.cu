@@ -84,7 +84,7 @@ int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0
                        cudaStream_t s) {
   if (g->sum_m == 0) return GBE_OK;
   const int64_t want = (g->sum_m + 63) / 64;  // 8 warps x 8 rows per CTA iteration
-  const int grid = (int)std::min<int64_t>(want, 148 * 64);
+  const int grid = (int)std::min<int64_t>(want, (int64_t)gbe_sm_count() * 64);
   if (g->contiguous)
     k_scatter<true><<<grid, 256, 0, s>>>(g->sum_m, g->row_src, g->row_nc, g->scat_base, nullptr,
                                          nullptr, st, X0, X1, D_val);

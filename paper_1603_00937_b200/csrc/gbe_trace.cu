@@ -37,21 +37,7 @@ __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double
     a1 = warp_sum(s1[t]);
     a2 = warp_sum(s2[t]);
   }
-  if (t == 0 && !stopped) {
-    const double t1 = a1, t2 = a2, n_occ = st->n_occ;
-    const int k = st->iter;  // the partials describe X_k
-    st->t1[k] = t1;
-    st->t2[k] = t2;
-    st->iters_done = k;
-    if (k >= st->iters || (st->idem_tol >= 0.0 && k >= 1 && fabs(t1 - t2) <= st->idem_tol)) {
-      st->stop = 1;
-    } else {
-      const int b = st->preset ? (int)st->br[k] : ((fabs(t2 - n_occ) < fabs(2.0 * t1 - t2 - n_occ)) ? 0 : 1);
-      st->branch = b;
-      st->br[k] = (uint8_t)b;
-      st->iter = k + 1;
-    }
-  }
+  if (t == 0 && !stopped) gbe_trace_decide(st, a1, a2);
 }
 }  // namespace
 

@@ -5,9 +5,24 @@
 namespace {
 thread_local cudaStream_t t_alloc_stream = nullptr;
 }
+bool gbe_device_once::first() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 256) return true;  // unknown device: set up every time
+  const uint64_t bit = 1ull << (dev & 63);
+  return (mask[dev >> 6].fetch_or(bit, std::memory_order_acq_rel) & bit) == 0;
+}
+int gbe_sm_count() {
+  static std::atomic<int> cached[256] = {};
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 1;
+  if (dev >= 0 && dev < 256 && (n = cached[dev].load(std::memory_order_relaxed)) > 0) return n;
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 1;
+  if (dev >= 0 && dev < 256) cached[dev].store(n, std::memory_order_relaxed);
+  return n;
+}
 void gbe_set_alloc_stream(cudaStream_t s) {
-  static bool pool_ready = false;  // benign race: setting the attribute twice is harmless
-  if (!pool_ready) {
+  static gbe_device_once pool_ready;  // per device: the release threshold belongs to the device's default pool
+  if (pool_ready.first()) {
     int dev = 0;
     cudaMemPool_t pool;
     if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
@@ -15,7 +30,6 @@ void gbe_set_alloc_stream(cudaStream_t s) {
       cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
     }
     cudaGetLastError();
-    pool_ready = true;
   }
   t_alloc_stream = s;
 }

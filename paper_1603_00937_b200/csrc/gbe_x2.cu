@@ -323,31 +323,33 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
 
 template <int MINB, int OP>
 int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-              const double* Xb, double* Dacc, const double* coef, bool last, cudaStream_t s) {
+              const double* Xb, double* Dacc, const double* coef, const gbe_tile_item* items, int n_items,
+              cudaStream_t s) {
   auto kern = k_x2<MINB, OP>;
   const size_t smem = (size_t)2 * X2_STAGE * sizeof(double);
-  static bool configured = false;
-  if (!configured) {
+  static gbe_device_once configured;  // one per template instance; function attributes are per device
+  if (configured.first()) {
     GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-    configured = true;
   }
-  // the last SP2 iteration computes the tiles with a core row only: the scatter keeps core columns (Eq.(6))
-  kern<<<last ? g->n_items_last : g->n_items, X2_THREADS, smem, s>>>(last ? g->items_last : g->items, st, Xin, Xout,
-                                                                     partials, iter, Xb, Dacc, coef);
+  kern<<<n_items, X2_THREADS, smem, s>>>(items, st, Xin, Xout, partials, iter, Xb, Dacc, coef);
   GBE_LAUNCHED();
   return GBE_OK;
 }
 }  // namespace
 
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                  bool last, cudaStream_t s) {
-  if (g->n_items == 0) return GBE_OK;
-  return launch_x2<4, 0>(g, st, Xin, Xout, partials, iter, nullptr, nullptr, nullptr, last, s);
+                  bool last, bool hybrid, cudaStream_t s) {
+  // the last SP2 iteration computes the tiles with a core row only: the scatter keeps core columns (Eq.(6));
+  // hybrid: the communities with m <= GBE_PK_MAX_M are the packed kernel's (gbe_small.cu), only the others are tiled
+  const gbe_tile_item* items = hybrid ? (last ? g->items_last_h : g->items_h) : (last ? g->items_last : g->items);
+  const int n_items = hybrid ? (last ? g->n_items_last_h : g->n_items_h) : (last ? g->n_items_last : g->n_items);
+  if (n_items == 0) return GBE_OK;
+  return launch_x2<4, 0>(g, st, Xin, Xout, partials, iter, nullptr, nullptr, nullptr, items, n_items, s);
 }
 
 int gbe_launch_cheb_step(const gbe_graph* g, gbe_state* st, const double* Xt, const double* Tn, double* Tio, double* Dacc,
                          const double* coef, int iter, double* partials, cudaStream_t s) {
   if (g->n_items == 0) return GBE_OK;
-  return launch_x2<4, 1>(g, st, Xt, Tio, partials, iter, Tn, Dacc, coef, false, s);
+  return launch_x2<4, 1>(g, st, Xt, Tio, partials, iter, Tn, Dacc, coef, g->items, g->n_items, s);
 }

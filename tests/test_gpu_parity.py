@@ -30,7 +30,8 @@ def gbe():
 
 
 def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None, sp2_path=0, gather_path=0):
-    """sp2_path: 0 = the library's choice, 1 = tiled kernels, 2 = shared-memory-resident kernel (include/gbe.h);
+    """sp2_path: 0 = the library's choice, 1 = tiled kernels, 2 = shared-memory-resident kernel, 3 = packed kernel for
+    the communities with m <= 160 + tiled kernel for the others (include/gbe.h);
     gather_path: 0 = the library's choice, 1 = staged through shared memory, 2 = direct to global memory."""
     import torch
     Hd = gbe.DeviceCSR.from_host(s.H if H is None else H)
@@ -39,6 +40,8 @@ def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None, sp
     if sp2_path:
         gbe.gbe_graph_set_sp2_path(g, sp2_path)
         assert g.info["resident_sp2"] == (1 if sp2_path == 2 else 0)
+        if sp2_path == 3:  # packed wherever the graph has a community that fits shared memory
+            assert g.info["sp2_path_chosen"] == (3 if g.info["n_small"] > 0 else 1)
     if gather_path:
         gbe.gbe_graph_set_gather_path(g, gather_path)
     D, log = gbe.gbe_density(Hd, g, s.n_occ, s.iters if iters is None else iters, idem_tol)
@@ -86,7 +89,7 @@ def check_density(Dg, log, r):
 
 
 # ------------------------------------------------------------------------------- main configurations
-@pytest.mark.parametrize("sp2_path", [1, 2])
+@pytest.mark.parametrize("sp2_path", [1, 2, 3])
 def test_config1_chain(gbe, sp2_path):
     s = gi.config(1)
     g, ex, Dg, log = run_gpu(gbe, s, sp2_path=sp2_path)
@@ -160,6 +163,31 @@ def test_config5_sweep_points(gbe, tau, n_part):
     graph, r = run_oracle(s)
     check_structure(ex, graph, r, g.info)
     check_density(Dg, log, r)
+    if (tau, n_part) == (1e-3, 256):  # 256 communities of m <= 160: more than are co-resident -> the packed kernel
+        assert g.info["sp2_path_chosen"] == 3 and g.info["n_small"] == 256
+
+
+@pytest.mark.parametrize("n_part", [256, 128, 64])
+def test_config5_small_m_regime_packed_kernel(gbe, n_part):
+    """The small-m regime of BASELINE.json configs[4] (cost law P:L78: more partitions, smaller m), tau = 1e-3 on the
+    1,024-molecule box (the same density, hence the same m, as the 24,576-orbital box with 4 x the communities):
+    256 communities m ~ 30 - 125 (all packed), 128 communities m ~ 65 - 185 (MIXED: the packed kernel takes m <= 160, the
+    tiled kernel the others, in the same iteration), 64 communities m ~ 140 - 285 (mostly tiled).  Both the library's
+    choice and the forced packed path against the oracle; the packed path is bitwise reproducible."""
+    import torch
+    s = gi.water_box(1024, n_part, seed=0, tau=1e-3, iters=20)
+    graph, r = run_oracle(s)
+    g, ex, Dg, log = run_gpu(gbe, s, sp2_path=3)
+    check_structure(ex, graph, r, g.info)
+    check_density(Dg, log, r)
+    m = np.diff(ex["sub_ptr"])
+    assert g.info["n_small"] == int(((m > 0) & (m <= 160)).sum())
+    if n_part == 128:
+        assert 0 < g.info["n_small"] < n_part  # the mixed case really is mixed
+    _, _, Dg2, log2 = run_gpu(gbe, s, sp2_path=3)
+    assert np.array_equal(Dg, Dg2) and np.array_equal(log.t1, log2.t1) and np.array_equal(log.t2, log2.t2)
+    _, _, Dt, logt = run_gpu(gbe, s, sp2_path=1)
+    assert np.abs(Dt - Dg).max() <= 1e-12
 
 
 @pytest.mark.slow
@@ -259,7 +287,7 @@ def test_gather_paths_pack_identical_blocks(gbe, which):
     check_density(Dg, log, r)
 
 
-@pytest.mark.parametrize("sp2_path", [1, 2])
+@pytest.mark.parametrize("sp2_path", [1, 2, 3])
 def test_iters_zero_returns_gathered_x0(gbe, sp2_path):
     """gather + scatter alone: D = core columns of X0[s,s]; exact up to the rounding of the two bounds."""
     s = gi.random_banded(150, half_bw=4, n_part=5, seed=3, tau=1e-3)
@@ -320,7 +348,7 @@ def test_tau_sweep_chain(gbe, tau):
         assert g.info["nnz_S"] == s.n  # self loops only (A-12)
 
 
-@pytest.mark.parametrize("sp2_path", [1, 2])
+@pytest.mark.parametrize("sp2_path", [1, 2, 3])
 def test_idem_tol_stops_on_device(gbe, sp2_path):
     s = gi.config(1)
     g, ex, Dg, log = run_gpu(gbe, s, iters=60, idem_tol=1e-9, sp2_path=sp2_path)
@@ -330,7 +358,7 @@ def test_idem_tol_stops_on_device(gbe, sp2_path):
 
 
 # ------------------------------------------------------------------------------- pre-determined SP2 sequence
-@pytest.mark.parametrize("sp2_path", [1, 2])
+@pytest.mark.parametrize("sp2_path", [1, 2, 3])
 @pytest.mark.parametrize("trace", [True, False])
 def test_preset_sequence_from_the_previous_md_step(gbe, trace, sp2_path):
     """'the complete SP2 sequence (the same for each subgraph expansion) ... can be determined beforehand' (P:L90):
@@ -526,7 +554,7 @@ def test_random_shapes_and_partitions(gbe, case):
     power = int(rng.integers(1, 4))
     graph, r = run_oracle(s, power=power)
     fits = None
-    for sp2_path in (1, 2):  # the tiled kernels, then the shared-memory-resident kernel where the communities fit it
+    for sp2_path in (1, 2, 3):  # tiled kernels; the resident kernel where every community fits it; the packed kernel
         if sp2_path == 2 and not fits:
             continue
         g, ex, Dg, log = run_gpu(gbe, s, power=power, sp2_path=sp2_path)
@@ -642,7 +670,8 @@ def test_side_stream_and_two_graphs_in_flight(gbe):
         assert np.array_equal(D.cpu().numpy(), r)  # same kernels, same reduction order: bit-identical
 
 
-def test_density_is_capturable_in_a_cuda_graph(gbe):
+@pytest.mark.parametrize("sp2_path", [0, 3])
+def test_density_is_capturable_in_a_cuda_graph(gbe, sp2_path):
     """gbe_density without a log only enqueues kernels on the caller's stream (no allocation, no synchronisation, the
     branch decision stays on the device), so the whole SP2 loop can be captured once and replayed - the way to run
     launch-bound small systems (config 1: 82 launches of a few microseconds each)."""
@@ -650,6 +679,7 @@ def test_density_is_capturable_in_a_cuda_graph(gbe):
     s = gi.config(1)
     Hd = gbe.DeviceCSR.from_host(s.H)
     g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    gbe.gbe_graph_set_sp2_path(g, sp2_path)
     ws = g.new_workspace()
     D_eager = torch.empty(g.info["nnz_D"], dtype=torch.float64, device="cuda")
     gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws, D_val=D_eager, want_log=False)
@@ -671,6 +701,35 @@ def test_density_is_capturable_in_a_cuda_graph(gbe):
     cg.replay()
     torch.cuda.synchronize()
     assert torch.equal(D_graph, D_eager)
+
+
+def test_packed_kernel_launches_and_reproducibility(gbe):
+    """The packed kernel (gbe_small.cu): ONE launch per SP2 iteration - the bin that publishes its trace partial last takes
+    step 5's decision, whichever bin that is the sums are taken in the same order - so 600 small communities (more than
+    can be co-resident, no grid barrier possible) take 40 launches for the loop instead of 80."""
+    import torch
+    s = gi.chain(4800, 600, seed=5)
+    rp, ci = o.build_graph(s.H, s.tau)
+    r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, s.iters)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
+    assert g.info["sp2_path_chosen"] == 3 and g.info["n_small"] == 600 and 0 < g.info["n_bins"] <= 600
+    n0 = gbe.gbe_launch_count()
+    D0, log0 = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
+    torch.cuda.synchronize()
+    assert gbe.gbe_launch_count() - n0 == 2 + 1 + 2 + s.iters + 1  # bounds(2), gather, init + trace of X_0, loop, scatter
+    check_density(D0.cpu().numpy(), log0, r)
+    for _ in range(10):
+        D1, log1 = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
+        assert torch.equal(D0, D1) and np.array_equal(log0.t1, log1.t1) and np.array_equal(log0.t2, log1.t2)
+    # a pre-determined sequence without trace logging on the packed path: no reduction at all between the products
+    gbe.gbe_graph_set_sp2_path(g, 3)
+    n0 = gbe.gbe_launch_count()
+    Dp, logp = gbe.gbe_density_preset(Hd, g, r.branch, trace_every_iteration=False)
+    torch.cuda.synchronize()
+    assert gbe.gbe_launch_count() - n0 == 2 + 1 + 1 + s.iters + 1 + 1  # ..., init, loop, final trace, scatter
+    assert np.abs(Dp.cpu().numpy() - r.D_val).max() <= TOL_D
+    assert abs(logp.t1[-1] - r.t1[-1]) <= TOL_TR and abs(logp.t2[-1] - r.t2[-1]) <= TOL_TR
 
 
 def test_resident_kernel_launches_and_choice(gbe):
