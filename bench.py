@@ -520,7 +520,7 @@ def run_sweep(args) -> None:
     import paper_1603_00937_b200 as gbe
 
     n_mol = WORKLOADS[args.workload][0]
-    taus = [1e-3, 1e-4, 1e-5, 1e-6, 1e-7]
+    taus = [float(x) for x in args.sweep_taus.split(",")] if args.sweep_taus else [1e-3, 1e-4, 1e-5, 1e-6, 1e-7]
     parts = [n_mol // 32, n_mol // 16, n_mol // 8, n_mol // 4]
     # --gapped: the variant of the water model with a HOMO-LUMO gap (oxygens >= 2.4 A apart, 3 electrons per molecule,
     # reading A-15), run to idempotency: there the error against the exact projector measures the method, not the model
@@ -551,6 +551,8 @@ def run_sweep(args) -> None:
             e0.record()
             g = gbe.gbe_build_graph(Hd, tau, None, n_part)
             e1.record()
+            if args.sp2_path:
+                gbe.gbe_graph_set_sp2_path(g, args.sp2_path)
             info = g.info
             ws = g.new_workspace()
             D_val = torch.empty(info["nnz_D"], dtype=torch.float64, device="cuda")
@@ -560,13 +562,18 @@ def run_sweep(args) -> None:
             _, log = gbe.gbe_density(Hd, g, n_occ, base.iters, idem_tol, workspace=ws, D_val=D_val, want_log=True)
             e2.record()
             torch.cuda.synchronize()
+            _, ph = gbe.gbe_density_timed(Hd, g, n_occ, base.iters, idem_tol, workspace=ws, D_val=D_val)
             ex = g.export()
             m = (ex["sub_ptr"][1:] - ex["sub_ptr"][:-1]).double()
             rec = {"sweep": args.workload, "tau": tau, "n_part": n_part, "m_min": int(m.min()), "m_mean": float(m.mean()),
                    "m_max": int(m.max()), "sum_2m3": info["sp2_flops_per_iter"], "nnz_S": info["nnz_S"],
                    "nnz_D": info["nnz_D"], "density_ms": e1.elapsed_time(e2),
                    "orbitals_per_s": n / (e1.elapsed_time(e2) * 1e-3),
-                   "iters_done": int(log.iters_done),
+                   "sp2_loop_ms": ph["x2_ms"] + ph["x2_last_ms"] + ph["trace_ms"], "gather_ms": ph["gather_ms"],
+                   "scatter_ms": ph["scatter_ms"],
+                   "sp2_exec_tflops": info["sp2_exec_flops_per_iter"] * max(0, log.iters_done - 1) / max(1e-9, ph["x2_ms"] * 1e-3) * 1e-12,
+                   "iters_done": int(log.iters_done), "sp2_path": int(info["sp2_path_chosen"]),
+                   "n_small": int(info["n_small"]), "n_bins": int(info["n_bins"]),
                    "sp2_tflops_alg": (info["sp2_flops_per_iter"] * max(0, log.iters_done - 1) + info["sp2_flops_last_iter"])
                                      / (e1.elapsed_time(e2) * 1e-3) * 1e-12,
                    "trace_minus_nocc": float(log.t1[-1] - n_occ), "idempotency_residual": float(log.t1[-1] - log.t2[-1])}
@@ -699,6 +706,8 @@ def main() -> None:
     ap.add_argument("--small", action="store_true", help="small systems: tiled kernels against the shared-memory-resident SP2 kernel")
     ap.add_argument("--gapped", action="store_true", help="sweep on the gapped variant of the water model, run to idempotency")
     ap.add_argument("--no-exact", action="store_true", help="sweep without the exact projector (no error columns)")
+    ap.add_argument("--sweep-taus", default="", help="comma-separated thresholds of the sweep (default: the five of configs[4])")
+    ap.add_argument("--sp2-path", type=int, default=0, help="sweep: force the SP2 kernels (1 tiled, 2 resident, 3 packed; 0 = the library's choice)")
     ap.add_argument("--record-traffic", default="", help="ncu raw-page CSV of a --set full capture of k_x2: write profiles/x2_traffic.json")
     ap.add_argument("--traffic-source", default="", help="the profiles/ summary that documents the capture")
     args = ap.parse_args()

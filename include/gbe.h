@@ -98,7 +98,7 @@ typedef struct {
   double sp2_sym_flops_per_iter; /* sum_p m_p^2 (m_p + 1): the flops of one SP2 iteration the METHOD needs when the symmetry
                                     of X_p is used (only the entries on or above the diagonal of X_p^2 are formed; obs. (x)
                                     P:L65) - the numerator of bench.py's roofline fraction */
-  int64_t n_small;           /* communities with 0 < m_p <= 160: the ones the packed kernel can take */
+  int64_t n_small;           /* communities with 0 < m_p <= 112 (gbe_set_packed_max_m): the ones the packed kernel takes */
   int64_t n_bins;            /* CTAs of one packed launch (bins of 1..16 small communities) */
 } gbe_graph_info;
 
@@ -147,7 +147,7 @@ int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, 
 
 /* Which kernels run the SP2 loop (steps 4-5) of this graph.  Three implementations compute the same updates:
  *   tiled    (any size)  one X^2 launch + one trace/branch launch per iteration over the batched dense layout in HBM;
- *   packed   (communities with m_p <= 160, any number of them; the cost law P:L78 - more partitions, smaller m)
+ *   packed   (communities with m_p <= 112 [gbe_set_packed_max_m], any number of them; the cost law P:L78 - more partitions, smaller m)
  *            one launch per iteration: a CTA copies a bin of 1..16 whole matrices to shared memory, squares them on the
  *            FP64 tensor cores, writes them back; the bin that finishes last reduces the traces and takes the branch
  *            decision, so there is no separate trace/branch launch.  Larger communities of the same graph go through the
@@ -161,7 +161,7 @@ int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, 
  *        has enough small communities to occupy the device; else tiled;
  *        1: always tiled;  2: resident whenever it can run (GBE_EINVAL if max_m is too large; calls for which the
  *        communities are not co-resident still take the tiled kernels);  3: packed whenever the graph has a community
- *        with m_p <= 160 (else tiled).
+ *        small enough (else tiled).
  * Results of the paths agree to rounding (different summation order of the global trace), each is bitwise
  * reproducible.  Not thread safe against concurrent calls on the same graph. */
 int gbe_graph_set_sp2_path(gbe_graph* g, int32_t path);
@@ -289,6 +289,12 @@ uint64_t gbe_launch_count(void);
  * fails, the second walk is taken; the graph is the same bit for bit.  bytes = 0 switches the bitmaps off.
  * Process-wide; returns the previous limit. */
 size_t gbe_set_build_scratch_limit(size_t bytes);
+
+/* Largest core+halo size m_p the packed SP2 kernel takes in graphs built FROM NOW ON (see gbe_graph_set_sp2_path); larger
+ * communities of the same graph run through the tiled kernel.  0 <= m <= 160 (160 = what fits one SM's shared memory;
+ * default 112 = what fits half of it, so that two bins share an SM).  Process-wide tuning knob; returns the previous value,
+ * -1 if m is out of range. */
+int32_t gbe_set_packed_max_m(int32_t m);
 
 void gbe_free_graph(gbe_graph* g);
 

@@ -21,6 +21,7 @@ EXPORTS = [
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
     "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation", "gbe_update_graph", "gbe_density_fermi",
     "gbe_graph_set_sp2_path", "gbe_error_norms", "gbe_graph_set_gather_path", "gbe_set_build_scratch_limit",
+    "gbe_set_packed_max_m",
 ]
 
 
@@ -100,6 +101,8 @@ def lib() -> C.CDLL:
         l.gbe_graph_set_gather_path.argtypes = [C.c_void_p, C.c_int32]
         l.gbe_set_build_scratch_limit.restype = C.c_size_t
         l.gbe_set_build_scratch_limit.argtypes = [C.c_size_t]
+        l.gbe_set_packed_max_m.restype = C.c_int32
+        l.gbe_set_packed_max_m.argtypes = [C.c_int32]
         l.gbe_launch_count.restype = C.c_uint64
         l.gbe_launch_count.argtypes = []
         l.gbe_gather.argtypes = [C.POINTER(_CsrView), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -242,6 +245,14 @@ def gbe_graph_set_gather_path(g: "Graph", path: int) -> None:
 def gbe_set_build_scratch_limit(nbytes: int) -> int:
     """Scratch limit of the graph builds for the candidate bitmaps (include/gbe.h); returns the previous limit."""
     return int(lib().gbe_set_build_scratch_limit(int(nbytes)))
+
+
+def gbe_set_packed_max_m(m: int) -> int:
+    """Largest community the packed SP2 kernel takes in graphs built from now on (include/gbe.h); returns the previous value."""
+    old = int(lib().gbe_set_packed_max_m(int(m)))
+    if old < 0:
+        raise GbeError(-1, "gbe_set_packed_max_m: out of range")
+    return old
 
 
 def gbe_launch_count() -> int:

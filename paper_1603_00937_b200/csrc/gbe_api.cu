@@ -8,6 +8,10 @@
 #include "gbe_internal.cuh"
 
 std::atomic<uint64_t> g_gbe_launches{0};
+// communities up to this size go to the packed kernel (gbe_small.cu); 116: the largest whose X fits half an SM's shared
+// memory, so that two bins share an SM
+static std::atomic<int32_t> g_pk_max_m{GBE_PK_MAX_M};
+int gbe_packed_max_m() { return g_pk_max_m.load(); }
 
 namespace {
 thread_local char g_cuda_err[512] = "";
@@ -36,7 +40,8 @@ int timed(Timer* tm, int phase, int launches, F&& fn) {
 
 // mode 0: branch chosen on the device every iteration; 1: preset sequence, traces logged every iteration;
 // 2: preset sequence, no per-iteration trace kernel (the final X is in buffer iters & 1)
-__global__ void k_init_state(gbe_state* st, double n_occ, double idem_tol, int iters, int mode) {
+__global__ void k_init_state(gbe_state* st, double n_occ, double idem_tol, int iters, int mode, int inplace) {
+  st->inplace = inplace;
   st->n_occ = n_occ;
   st->idem_tol = idem_tol;
   st->iters = iters;
@@ -99,7 +104,7 @@ const char* gbe_strerror(int status) {
 void gbe_free_graph(gbe_graph* g) {
   if (!g) return;
   void* ptrs[] = {g->S_row_ptr, g->S_col,     g->sub_ptr,  g->sub_idx,  g->ncore,    g->msize, g->dense_off, g->D_row_ptr,
-                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->items_h, g->items_last_h, g->pk_ctas, g->pk_slots, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va};
+                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->items_h, g->items_last_h, g->pk[0].ctas, g->pk[0].codes, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   delete g;
@@ -249,8 +254,10 @@ static int choose_sp2(const gbe_graph* g, int mode) {
   // auto.  Resident: one launch for the whole loop - wins whenever the communities are small enough that one SM per
   // community keeps up with the tiled kernels spreading the tiles over all SMs (measured).
   if (can_res && (g->max_m <= 128 || g->n_part >= g->resident_coresident / 2)) return 2;
-  // Packed: enough small communities to occupy the device; the others of the same graph stay tiled.
-  if (can_pk && g->n_pk_ctas >= gbe_sm_count() / 2) return 3;
+  // Packed: every community fits shared memory and there are enough of them to occupy the device (measured, DESIGN.md 6:
+  // a graph that also needs the tiled kernel for some communities pays a second, poorly filled launch per iteration and
+  // is not faster than the tiled kernels alone).
+  if (can_pk && g->n_pk_ctas >= gbe_sm_count() / 2 && g->n_items_h == 0) return 3;
   return 1;
 }
 
@@ -278,10 +285,14 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const int mode = !preset ? 0 : (trace_each ? 1 : 2);
   const int path = choose_sp2(g, mode);
+  // Packed kernel with EVERY community packed: a bin has all of its X_p in shared memory before it stores anything, so
+  // X is updated in place in buffer 0 - half the footprint, which keeps a batch of up to ~60 MB resident in L2 (measured:
+  // with two 41 MB buffers every iteration re-read X from DRAM)
+  const int inplace = path == 3 && g->n_items_h == 0;
   if (path == 2) {
     // small communities: the whole loop in one kernel, X_p resident in shared memory (gbe_resident.cu)
     GBE_TRY(timed(tm, PH_TRACE, 1, [&]() -> int {
-      k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode);
+      k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode, inplace);
       GBE_LAUNCHED();
       if (preset && iters > 0)
         GBE_CUDA(cudaMemcpyAsync(w.st->br, preset, (size_t)iters, cudaMemcpyHostToDevice, s));
@@ -294,7 +305,7 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
   }
   // traces of X_0 (partials written by the gather), branch of iteration 0
   GBE_TRY(timed(tm, PH_TRACE, mode == 2 ? 1 : 2, [&]() -> int {
-    k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode);
+    k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode, inplace);
     GBE_LAUNCHED();
     if (preset && iters > 0)
       GBE_CUDA(cudaMemcpyAsync(w.st->br, preset, (size_t)iters, cudaMemcpyHostToDevice, s));
@@ -302,8 +313,8 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
     return gbe_launch_trace_branch(w.st, w.partials, g->n_gitems, s);
   }));
   for (int it = 0; it < iters; ++it) {
-    const double* in = (it & 1) ? w.X1 : w.X0;
-    double* outp = (it & 1) ? w.X0 : w.X1;
+    const double* in = (it & 1) && !inplace ? w.X1 : w.X0;
+    double* outp = (it & 1) || inplace ? w.X0 : w.X1;
     // Iteration iters - 1 is the last one whether or not the idempotency stop fires before it (then it is a no-op):
     // only the core rows and columns of its result are read again (trace, scatter), so it runs the core tiles only.
     const bool last = it == iters - 1;
@@ -478,6 +489,11 @@ int gbe_error_norms(const gbe_graph* g, const double* D_val, const double* D_ref
   GBE_CUDA(cudaMemcpyAsync(out, res.p, 3 * 8, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaStreamSynchronize(s));
   return GBE_OK;
+}
+
+int32_t gbe_set_packed_max_m(int32_t m) {
+  if (m < 0 || m > GBE_PK_MAX_M) return -1;
+  return g_pk_max_m.exchange(m);
 }
 
 uint64_t gbe_launch_count(void) { return g_gbe_launches.load(std::memory_order_relaxed); }

@@ -82,6 +82,7 @@ __global__ void __launch_bounds__(1024) k_core_trace(int n_part, const int64_t* 
   if (t == 0) {
     st->t2[0] = sh[0];
     st->iters_done = 0;  // the scatter reads buffer (iters_done & 1): the caller passes BD for both
+    st->inplace = 0;
   }
 }
 }  // namespace

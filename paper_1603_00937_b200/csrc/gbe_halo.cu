@@ -320,13 +320,14 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     std::vector<int32_t> order(n_part);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return g->h_m[a] > g->h_m[b]; });
+    g->pk_max_m = gbe_packed_max_m();
     std::vector<gbe_tile_item> items, last, items_h, last_h;  // _h: the communities the packed kernel does not take
     const int tile = g->tile;
     g->exec_flops_per_iter = g->exec_flops_last_iter = g->flops_last_iter = 0;
     for (int p : order) {
       const int T = (g->h_m[p] + tile - 1) / tile;
       const int64_t ld = (g->h_m[p] + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
-      const bool big = g->h_m[p] > GBE_PK_MAX_M;
+      const bool big = g->h_m[p] > g->pk_max_m;
       for (int ti = 0; ti < T; ++ti)
         for (int tj = ti; tj < T; ++tj) {
           // pidx: where the tile's trace partial goes - the tiles with a core row are numbered in list order (which is

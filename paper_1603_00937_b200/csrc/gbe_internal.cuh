@@ -75,7 +75,7 @@ struct gbe_state {
   int32_t preset;      // 1: the branch sequence br[] was given by the caller (gbe_density_preset)
   uint32_t bar;        // arrival counter of the resident kernel's grid barrier (reset by k_init_state)
   uint32_t ticket;     // bins of the packed kernel that have published their partial this iteration (gbe_small.cu)
-  uint32_t pad_;
+  int32_t inplace;     // 1: the SP2 loop updates X in place in buffer 0 (packed kernel, all communities packed)
   double t1[GBE_MAX_ITERS + 1];
   double t2[GBE_MAX_ITERS + 1];
   uint8_t br[GBE_MAX_ITERS];
@@ -84,15 +84,22 @@ struct gbe_state {
 // packed small communities (gbe_small.cu): one CTA works on a bin of up to GBE_PK_MAX_SLOTS communities per launch
 constexpr int GBE_PK_MAX_M = 160;     // largest core + halo size the packed (and the resident) kernel holds in shared memory
 constexpr int GBE_PK_MAX_SLOTS = 16;  // communities per bin
-constexpr int GBE_PK_MAXU = 4;        // work units per warp (accumulator registers)
-struct gbe_pk_slot {  // one community of a bin (32 bytes)
+struct gbe_pk_slot {  // one community of a bin (40 bytes)
   int32_t p, m, nc, ld;  // community, core + halo size, core size, leading dimension
-  int32_t soff, R;       // offset of its X in the bin's shared memory (doubles), 8-row blocks
+  int32_t soff;          // offset of its X in the bin's shared memory (doubles)
+  int16_t R, pad0_;      // 8-row blocks
+  int32_t magic, pad1_;  // floor(2^32 / (ld / 8)) + 1: row of a 16-byte piece of a column quarter by one multiply
   int64_t dense_off;     // element offset of X_p in a dense buffer
 };
-struct gbe_pk_cta {  // one bin (144 bytes)
-  int32_t first_slot, n_slots, smem_doubles, pad_;
-  uint16_t units[16][GBE_PK_MAXU];  // per warp: slot | row block | first column block | blocks (0xFFFF: none)
+struct gbe_pk_cta {  // one bin: its communities (its work units sit in the class's code array, [bin][round][warp])
+  int32_t n_slots, n_rounds, smem_doubles, pad1_;  // n_rounds: longest unit list of a warp; shared memory of the bin
+  gbe_pk_slot slot[GBE_PK_MAX_SLOTS];
+};
+struct gbe_pk_class {  // the bins of one launch of the packed kernel (device arrays owned by the graph)
+  gbe_pk_cta* ctas = nullptr;
+  uint16_t* codes = nullptr;
+  int32_t n_ctas = 0, warps = 0, rounds_max = 0, code_stride = 0;
+  size_t smem_bytes = 0;
 };
 
 struct gbe_tile_item {  // one X^2 work item: tile (ti, tj), ti <= tj, of community p, with p's layout (32 bytes)
@@ -131,11 +138,8 @@ struct gbe_graph {
   // communities + tiled kernel for the others (gbe_small.cu); set by gbe_graph_set_sp2_path
   int32_t sp2_path = 0;
   // packed path: bins of communities with m <= GBE_PK_MAX_M, and the tile lists of the OTHER communities
-  gbe_pk_cta* pk_ctas = nullptr;
-  gbe_pk_slot* pk_slots = nullptr;
-  int32_t n_pk_ctas = 0, pk_n_small = 0;
-  size_t pk_smem_bytes = 0;
-  double pk_dmma = 0, all_dmma = 0;  // DMMA instructions per iteration of the packed communities / of all communities
+  gbe_pk_class pk[1];
+  int32_t n_pk_ctas = 0, pk_n_small = 0, pk_max_m = 0;  // bins; communities in them; threshold of THIS graph
   gbe_tile_item* items_h = nullptr;       // tiles of the communities with m > GBE_PK_MAX_M
   gbe_tile_item* items_last_h = nullptr;  // those with a core row
   int32_t n_items_h = 0, n_items_last_h = 0;
@@ -191,7 +195,8 @@ int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* 
 int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident, int* cluster);
 int gbe_launch_sp2_resident(const gbe_graph* g, gbe_state* st, double* X0, double* X1, double* partials, int mode,
                             cudaStream_t s);
-// steps 4 + 5, one iteration per launch, for communities with m <= GBE_PK_MAX_M (gbe_small.cu)
+// steps 4 + 5, one iteration per launch, for communities with m <= g->pk_max_m (gbe_small.cu)
+int gbe_packed_max_m();  // process-wide default of the threshold (gbe_set_packed_max_m)
 int gbe_build_packed(gbe_graph* g, cudaStream_t s);
 int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials,
                           int partial_base, int n_partials, int iter, bool last, bool fused, cudaStream_t s);

@@ -4,7 +4,8 @@
 // Column i of P_tau(H) is column j of P(x[s]) (Eq.(6)); P(x[s]) is symmetric, so the kernel reads ROW
 // segments instead (contiguous): for dense row (p, r) the ncore_p leading entries go to one contiguous run of
 // D.val when every core is an index range, else through a per-entry position map.  D is NOT symmetrised
-// (obs. (i) P:L65).  The final X lives in buffer (iters_done & 1), read from the device state.
+// (obs. (i) P:L65).  The final X lives in buffer (iters_done & 1) - in buffer 0 when the SP2 loop ran in place - read from
+// the device state.
 // Bound: HBM - 8 B read + 8 B written per stored entry of D (+ 8 B map in the general case).
 #include "gbe_internal.cuh"
 
@@ -19,7 +20,7 @@ __global__ void __launch_bounds__(256, 4) k_scatter(int64_t sum_m, const int64_t
                                                  double* __restrict__ D_val) {
   const int lane = threadIdx.x & 31;
   const int64_t warp = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5), nwarps = (int64_t)gridDim.x * 8;
-  const double* __restrict__ X = (st->iters_done & 1) ? X1 : X0;
+  const double* __restrict__ X = (!st->inplace && (st->iters_done & 1)) ? X1 : X0;  // in place: X never left X0
   constexpr int R = 8;  // dense rows per warp iteration: their metadata is fetched by 8 lanes at once and the loads
                         // of all 8 rows are issued before the first store (the kernel is latency bound otherwise)
   for (int64_t q0 = warp * R; q0 < sum_m; q0 += nwarps * R) {

@@ -3,27 +3,36 @@
 //     Y_p = X_p X_p;  X_p <- Y_p  or  2 X_p - Y_p   for every community p with m_p <= 160
 //
 // The cost law of the paper (more partitions -> smaller core+halo size m) puts a whole regime of the method at
-// m ~ 30 - 180 with hundreds to thousands of communities (BASELINE.json configs[4], tau = 1e-3).  There a 64 x 64 tile of
-// the tiled kernel (gbe_x2.cu) is mostly mask, and the resident kernel (gbe_resident.cu) cannot run: its grid barrier
-// needs all communities co-resident.  Here:
-//   - a CTA owns a BIN of 1..16 communities for one iteration.  The bins are packed once per graph on the host (longest
-//     processing time first onto k x SM-count bins, k waves), bounded by shared memory, by the accumulator registers
-//     (16 warps x 4 work units) and by a cost cap, so that a launch is a whole number of equally heavy waves;
-//   - every X_p of the bin is copied to shared memory once (cp.async, row stride ld_p + 4: conflict-free 64-bit
-//     fragment loads) - the batch is read exactly once per iteration, and for these sizes it lives in L2;
-//   - Y = X X^T on FP64 tensor cores (mma.sync.m8n8k4.f64): a work unit is one 8-row block x up to four 8-column blocks
-//     on or above the diagonal; the host deals the units of the whole bin to the 16 warps by cost (at most 4 each),
-//     accumulators stay in registers until every warp has finished reading X, then X is overwritten in place
-//     (direct + mirrored store), exactly as in the resident kernel;
-//   - the core-row traces of the NEW X (t1 = sum X_ii, t2 = sum_c X_ic^2 = Tr_core X^2 for symmetric X) are summed per
-//     bin in a fixed order and the new X is streamed out with 128-bit stores;
-//   - step 5 fused: the bin that publishes its partial LAST (one ticket per bin; the fence orders 16 bytes, not the bulk
-//     stores, which come after it) sums all partials of the iteration in a fixed order and takes the branch decision
-//     exactly as k_trace_branch does - one launch per SP2 iteration instead of two.  Which CTA is last does not change
-//     the order of the sum: results are reproducible bit for bit.
+// m ~ 30 - 130 with a thousand or more communities (BASELINE.json configs[4], tau = 1e-3).  There a 64 x 64 tile of the
+// tiled kernel (gbe_x2.cu) is mostly mask and its two launches per iteration are mostly launch latency, and the resident
+// kernel (gbe_resident.cu) cannot run: its grid barrier needs all communities co-resident.  Here:
+//   - a CTA (32 warps, one per SM) owns a BIN of 1..16 communities for one iteration.  The bins are packed once per graph
+//     on the host: longest processing time first onto exactly k x SM-count bins (a launch is k equally heavy waves),
+//     bounded by shared memory;
+//   - every X_p of the bin is copied to shared memory by TMA: one bulk copy (cp.async.bulk, SASS UBLKCP) per matrix row,
+//     issued by one thread per row, counted in bytes on an mbarrier; row stride ld_p + 4 doubles: conflict-free 64-bit
+//     fragment loads.  The batch is read exactly once per iteration;
+//   - Y = X X^T on FP64 tensor cores (mma.sync.m8n8k4.f64): a work unit is two 8-row blocks x up to four 8-column blocks
+//     on or above the diagonal (6 fragment loads per 8 DMMA); the host deals the units of the bin, longest first, to the
+//     least loaded warp, ties to the least loaded SM sub-partition (each has its own DMMA pipe).  A unit's part of
+//     X_{n+1} goes straight from the accumulators to the dense buffer (direct + mirrored store; X_n in shared memory
+//     stays intact), with the core-row traces of X_{n+1} (t1 = sum X_ii, t2 = sum_c X_ic^2 = Tr_core X^2 for symmetric
+//     X) taken on the way and summed per bin in a fixed order;
+//   - a bin has ALL of its X_p in shared memory before it stores anything, so when every community of the graph is packed
+//     the iteration runs IN PLACE in one dense buffer;
+//   - step 5 fused: the bin that publishes its partial LAST (one ticket per bin; the fence orders 16 bytes) sums all
+//     partials of the iteration in a fixed order and takes the branch decision exactly as k_trace_branch does - one
+//     launch per SP2 iteration instead of two.  Which CTA is last does not change the order of the sum: results are
+//     reproducible bit for bit.
 // Communities with m_p > 160 of the same graph go through the tiled kernel in the same iteration (launched first; its
 // partials sit in front of the bins' and enter the same sum).
-// Bound: FP64 tensor pipe for m >~ 60; below that the copy in and out of shared memory (L2 latency).
+// Measured on B200 with per-warp %globaltimer stamps: inside a bin the products run at the DMMA issue rate
+// of the sub-partitions that have work; what is left is per bin and serial - description 0.7 us, the copy in 2 - 5 us
+// (the TMA unit retires one row copy per ~17 cycles), trace + ticket 1.2 us - and ~10 us from one launch to the next.
+// Tried and dropped, none faster: 16 warps and two bins per SM (the two start in phase and share the pipes); copies in
+// column quarters with the first unit started on the first quarter; self-scheduling of the units through a shared-memory
+// counter; persistent CTAs with two half-size buffers (the next bin copied in under the products of this one).
+// Bound: FP64 tensor pipe inside a bin; per-bin latencies and launch latency around it.
 #include <algorithm>
 #include <numeric>
 #include <queue>
@@ -32,221 +41,263 @@
 
 namespace {
 
-constexpr int PK_WARPS = 16;
+constexpr int PK_WARPS = 32;             // 1,024 threads, 64 registers each, one CTA per SM
 constexpr int PK_THREADS = PK_WARPS * 32;
-constexpr int PK_MAXU = GBE_PK_MAXU;  // work units per warp
-constexpr int PK_UCOLS = 4;           // 8-column blocks per unit
-constexpr uint16_t PK_NONE = 0xFFFFu;
+constexpr int PK_UCOLS = 4;              // 8-column blocks per work unit
+constexpr int PK_MAX_ROUNDS = 32;        // units per warp (lane j of a warp fetches the code of its j-th unit)
+constexpr unsigned PK_NONE = 0xFFFFu;
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(c0), "+d"(c1)
                : "d"(a), "d"(b));
 }
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
-  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc));
-}
-__device__ __forceinline__ void cp_async_wait_all() {
-  asm volatile("cp.async.commit_group;");
-  asm volatile("cp.async.wait_group 0;" ::: "memory");
-}
-
-template <int NB>
-__device__ __forceinline__ void pk_unit_mma(double (&acc)[PK_UCOLS][2], const double* __restrict__ pa,
-                                            const double* __restrict__ pb, int ld, int stride) {
-#pragma unroll 4
-  for (int k0 = 0; k0 < ld; k0 += 4) {
-    const double a = pa[k0];
+// TALL: the unit spans two 8-row blocks (bi, bi + 1); FIRST: its first column block is bi, so the block (bi + 1, bi) lies
+// below the diagonal and is left out (its values arrive through the mirror of (bi, bi + 1))
+template <int NB, bool TALL, bool FIRST>
+__device__ __forceinline__ void pk_unit_mma(double (&acc)[2][PK_UCOLS][2], const double* __restrict__ pa,
+                                            const double* __restrict__ pb, int kmax, int stride) {
+#pragma unroll 2
+  for (int k0 = 0; k0 < kmax; k0 += 4) {
+    const double a0 = pa[k0];
+    const double a1 = TALL ? pa[8 * stride + k0] : 0.0;
     double b[NB];
 #pragma unroll
     for (int j = 0; j < NB; ++j) b[j] = pb[j * 8 * stride + k0];
 #pragma unroll
-    for (int j = 0; j < NB; ++j) dmma884(acc[j][0], acc[j][1], a, b[j]);
+    for (int j = 0; j < NB; ++j) dmma884(acc[0][j][0], acc[0][j][1], a0, b[j]);
+    if (TALL) {
+#pragma unroll
+      for (int j = FIRST ? 1 : 0; j < NB; ++j) dmma884(acc[1][j][0], acc[1][j][1], a1, b[j]);
+    }
+  }
+}
+template <bool TALL, bool FIRST>
+__device__ __forceinline__ void pk_unit_mma_nb(int nb, double (&acc)[2][PK_UCOLS][2], const double* __restrict__ pa,
+                                               const double* __restrict__ pb, int kmax, int stride) {
+  switch (nb) {
+    case 4: pk_unit_mma<4, TALL, FIRST>(acc, pa, pb, kmax, stride); break;
+    case 3: pk_unit_mma<3, TALL, FIRST>(acc, pa, pb, kmax, stride); break;
+    case 2: pk_unit_mma<2, TALL, FIRST>(acc, pa, pb, kmax, stride); break;
+    default: pk_unit_mma<1, TALL, FIRST>(acc, pa, pb, kmax, stride); break;
   }
 }
 
-// unit code: slot (4 bits) | row block bi (5) | first column block as (bj - bi) / 4 (3) | blocks - 1 (2)
-__host__ __device__ inline uint16_t pk_encode(int slot, int bi, int bj, int nb) {
-  return (uint16_t)(slot | (bi << 4) | (((bj - bi) >> 2) << 9) | ((nb - 1) << 12));
+// TMA bulk copy of one row (global -> shared), completion counted in bytes on an mbarrier
+__device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t mbar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_row_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(mbar)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
+  uint32_t done = 0;
+  while (!done) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(mbar), "r"(parity)
+        : "memory");
+  }
+}
+
+// unit code: slot (4 bits) | row block bi (5) | first column block as (bj - bi) / 4 (3) | blocks - 1 (2) | tall (1)
+__host__ __device__ inline uint16_t pk_encode(int slot, int bi, int bj, int nb, int tall) {
+  return (uint16_t)(slot | (bi << 4) | (((bj - bi) >> 2) << 9) | ((nb - 1) << 12) | (tall << 14));
+}
+
+// one unit's part of X_{n+1}: direct + mirrored store, traces of the core rows.  EDGE: the unit touches rows or columns
+// >= m (ragged last block); TRACE: it touches a core row, directly or through the mirror
+template <bool EDGE, bool TRACE>
+__device__ __forceinline__ void pk_unit_store(const double (&acc)[PK_UCOLS][2], int j0, const double* __restrict__ x0,
+                                              double* __restrict__ Y, int bi, int bj, int nb, int g, int q, int m,
+                                              int nc, int ld, int stride, int branch, double& s1, double& s2) {
+  const int r = bi * 8 + g;
+  if (EDGE && r >= m) return;
+  const double* __restrict__ xr = x0 + (size_t)r * stride + bj * 8 + 2 * q;
+  double* __restrict__ yr = Y + (size_t)r * ld + bj * 8 + 2 * q;
+  double* __restrict__ ym = Y + (size_t)(bj * 8 + 2 * q) * ld + r;  // mirrored position (c, r); (c + 1, r) is ld further
+#pragma unroll
+  for (int j = 0; j < PK_UCOLS; ++j) {
+    if (j >= j0 && j < nb) {
+      const int c = (bj + j) * 8 + 2 * q;
+      double v0 = acc[j][0], v1 = acc[j][1];
+      if (branch) {
+        const double2 x = *reinterpret_cast<const double2*>(xr + j * 8);
+        v0 = 2.0 * x.x - v0;
+        v1 = 2.0 * x.y - v1;
+      }
+      *reinterpret_cast<double2*>(yr + j * 8) = make_double2(v0, v1);
+      if (TRACE && r < nc) {
+        s2 += v0 * v0 + v1 * v1;
+        if (r == c) s1 += v0;
+        if (r == c + 1) s1 += v1;
+      }
+      if (bj + j != bi) {  // off-diagonal block: mirror (the diagonal block is computed whole)
+        if (!EDGE || c < m) {
+          ym[(size_t)j * 8 * ld] = v0;
+          if (TRACE && c < nc) s2 += v0 * v0;
+        }
+        if (!EDGE || c + 1 < m) {
+          ym[(size_t)j * 8 * ld + ld] = v1;
+          if (TRACE && c + 1 < nc) s2 += v1 * v1;
+        }
+      }
+    }
+  }
 }
 
 // fused == 1: the last bin to publish its partial reduces all n_partials pairs and takes the decision of step 5
 __global__ void __launch_bounds__(PK_THREADS, 1)
-    k_sp2_packed(const gbe_pk_cta* __restrict__ ctas, const gbe_pk_slot* __restrict__ slots, gbe_state* st,
-                 const double* __restrict__ Xin, double* __restrict__ Xout, double* __restrict__ partials,
-                 int partial_base, int n_partials, int iter, int last, int fused) {
-  extern __shared__ __align__(16) double xs[];
-  __shared__ gbe_pk_slot sl[GBE_PK_MAX_SLOTS];
+    k_sp2_packed(const gbe_pk_cta* __restrict__ ctas, const uint16_t* __restrict__ ucodes, gbe_state* st,
+                 const double* Xin, double* Xout, double* __restrict__ partials,  // Xin == Xout when the loop runs in place
+                 int partial_base, int n_partials, int iter, int last, int fused, int code_stride, int rounds_max) {
+  extern __shared__ __align__(16) double xs[];  // the X_p of the bin
+  __shared__ gbe_pk_cta me;
   __shared__ double red[2 * PK_WARPS];
   __shared__ int is_last;
-
-  if (st->stop) return;  // idempotency stop already fired (A-7): X is final
-  const int branch = st->preset ? (int)st->br[iter] : st->branch;
+  __shared__ __align__(8) unsigned long long load_bar;
 
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5, g = lane >> 2, q = lane & 3;
-  const gbe_pk_cta& me = ctas[blockIdx.x];
-  const int n_slots = me.n_slots;
-  if (t < n_slots * 8) reinterpret_cast<int*>(sl)[t] = reinterpret_cast<const int*>(slots + me.first_slot)[t];
-  uint16_t ucode[PK_MAXU];
-#pragma unroll
-  for (int u = 0; u < PK_MAXU; ++u) ucode[u] = me.units[wid][u];
+  // the bin's description (one coalesced read), this warp's unit codes (dealt on the host, longest first, to the least
+  // loaded warp; lane j holds the j-th one; fixed stride per bin, so the address does not wait for the description) and
+  // the state: independent loads, all in flight
+  if (t < (int)(sizeof(gbe_pk_cta) / 4)) reinterpret_cast<int*>(&me)[t] = reinterpret_cast<const int*>(ctas + blockIdx.x)[t];
+  const unsigned my_code = lane < rounds_max ? ucodes[(size_t)blockIdx.x * code_stride + lane * PK_WARPS + wid] : PK_NONE;
+  const int stop = st->stop;
+  const int branch = st->preset ? (int)st->br[iter] : st->branch;
   __syncthreads();
+  if (stop) return;  // idempotency stop already fired (A-7): X is final
+  const int n_slots = me.n_slots, n_rounds = me.n_rounds;
 
-  // ---- X_n of every community of the bin -> shared memory; rows [m, 8R) are zero (they stay zero under both updates)
+  // ---- X_n of every community of the bin -> shared memory: one TMA bulk copy per row (row stride ld + 4 doubles in
+  //      shared memory: conflict-free 64-bit fragment loads), issued by one thread per row, completion counted in bytes on
+  //      one mbarrier - no per-piece instructions.  Rows [m, 8R) are zero: no predicate in the products.
+  const uint32_t mbar = (uint32_t)__cvta_generic_to_shared(&load_bar);
+  if (t == 0) {
+    uint32_t bytes = 0;
+    for (int s = 0; s < n_slots; ++s) bytes += (uint32_t)(me.slot[s].m * me.slot[s].ld) * 8u;
+    mbar_init(mbar, 1);
+    mbar_expect_tx(mbar, bytes);
+  }
+  __syncthreads();
   for (int s = 0; s < n_slots; ++s) {
-    const int m = sl[s].m, ld = sl[s].ld, stride = ld + 4, h = ld >> 1;
-    const double* __restrict__ src = Xin + sl[s].dense_off;
-    double* dst = xs + sl[s].soff;
-    for (int i = t; i < m * h; i += PK_THREADS) {
-      const int r = i / h, c2 = i - r * h;
-      cp_async16(dst + (size_t)r * stride + 2 * c2, src + 2 * (size_t)i);
+    const int m = me.slot[s].m, ld = me.slot[s].ld, stride = ld + 4;
+    for (int r = t; r < m; r += PK_THREADS)
+      bulk_row_g2s((uint32_t)__cvta_generic_to_shared(xs + me.slot[s].soff + r * stride),
+                   Xin + me.slot[s].dense_off + (size_t)r * ld, (uint32_t)ld * 8u, mbar);
+    for (int i = m * stride + t; i < 8 * me.slot[s].R * stride; i += PK_THREADS) xs[me.slot[s].soff + i] = 0.0;
+    // pad columns [8R, ld) of the OUTPUT stay zero (no work unit covers them; [m, 8R) come out of the products as zeros)
+    if (ld > 8 * me.slot[s].R) {
+      double* __restrict__ out = Xout + me.slot[s].dense_off + 8 * me.slot[s].R;
+      for (int i = t; i < m * 8; i += PK_THREADS) out[(size_t)(i >> 3) * ld + (i & 7)] = 0.0;
     }
-    for (int i = m * stride + t; i < 8 * sl[s].R * stride; i += PK_THREADS) dst[i] = 0.0;
   }
-  cp_async_wait_all();
-  __syncthreads();
+  __syncthreads();  // the zero rows
+  mbar_wait(mbar, 0);
 
-  // ---- Y = X X^T: this warp's units, accumulators in registers
-  double acc[PK_MAXU][PK_UCOLS][2];
-#pragma unroll
-  for (int u = 0; u < PK_MAXU; ++u)
-#pragma unroll
-    for (int j = 0; j < PK_UCOLS; ++j) acc[u][j][0] = acc[u][j][1] = 0.0;
-#pragma unroll
-  for (int u = 0; u < PK_MAXU; ++u) {
-    if (ucode[u] == PK_NONE) continue;
-    const int s = ucode[u] & 15, bi = (ucode[u] >> 4) & 31, bj = bi + 4 * ((ucode[u] >> 9) & 7), nb = 1 + ((ucode[u] >> 12) & 3);
+  // ---- Y = X X^T unit by unit (one 8-row block x up to four 8-column blocks on or above the diagonal); the unit's part
+  //      of X_{n+1} = Y or 2 X_n - Y goes straight from the accumulators to the other dense buffer, direct + mirrored,
+  //      with the core-row traces of X_{n+1} taken on the way (X_n in shared memory stays intact: nothing is in place).
+  double s1 = 0.0, s2 = 0.0;
+#pragma unroll 1
+  for (int round = 0; round < n_rounds; ++round) {
+    const unsigned code = __shfl_sync(0xffffffffu, my_code, round);
+    const int s = code & 15, bi = (code >> 4) & 31, bj = bi + 4 * ((code >> 9) & 7), nb = 1 + ((code >> 12) & 3);
+    const bool tall = (code >> 14) & 1, firstu = bj == bi;
+    const int nc = me.slot[s].nc, m = me.slot[s].m, ld = me.slot[s].ld, stride = ld + 4;
+    const int kmax = (m + 3) & ~3;  // columns >= m are zero
     // the last iteration needs the core rows and (through the mirror) the core columns only (Eq.(6))
-    if (last && bi * 8 >= sl[s].nc) continue;
-    const int ld = sl[s].ld, stride = ld + 4;
-    const double* pa = xs + sl[s].soff + (size_t)(bi * 8 + g) * stride + q;
-    const double* pb = xs + sl[s].soff + (size_t)(bj * 8 + g) * stride + q;
-    switch (nb) {
-      case 4: pk_unit_mma<4>(acc[u], pa, pb, ld, stride); break;
-      case 3: pk_unit_mma<3>(acc[u], pa, pb, ld, stride); break;
-      case 2: pk_unit_mma<2>(acc[u], pa, pb, ld, stride); break;
-      default: pk_unit_mma<1>(acc[u], pa, pb, ld, stride); break;
+    if (code == PK_NONE || (last && bi * 8 >= nc)) continue;
+    const double* x0 = xs + me.slot[s].soff;
+    const double* pa = x0 + (size_t)(bi * 8 + g) * stride + q;
+    const double* pb = x0 + (size_t)(bj * 8 + g) * stride + q;
+    double acc[2][PK_UCOLS][2];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+      for (int j = 0; j < PK_UCOLS; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    if (!tall) pk_unit_mma_nb<false, false>(nb, acc, pa, pb, kmax, stride);
+    else if (firstu) pk_unit_mma_nb<true, true>(nb, acc, pa, pb, kmax, stride);
+    else pk_unit_mma_nb<true, false>(nb, acc, pa, pb, kmax, stride);
+    double* __restrict__ Y = Xout + me.slot[s].dense_off;
+    const bool edge = (bj + nb) * 8 > m;  // bi <= bj: the row edge implies the column edge
+    const bool trace = bi * 8 < nc;       // bi <= bj: a core column implies a core row
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      if (i == 1 && !tall) break;
+      const int j0 = (i == 1 && firstu) ? 1 : 0;  // block (bi + 1, bi) was not formed
+      if (edge) pk_unit_store<true, true>(acc[i], j0, x0, Y, bi + i, bj, nb, g, q, m, nc, ld, stride, branch, s1, s2);
+      else if (trace) pk_unit_store<false, true>(acc[i], j0, x0, Y, bi + i, bj, nb, g, q, m, nc, ld, stride, branch, s1, s2);
+      else pk_unit_store<false, false>(acc[i], j0, x0, Y, bi + i, bj, nb, g, q, m, nc, ld, stride, branch, s1, s2);
     }
   }
-  __syncthreads();  // every warp is done reading X_n
 
-  // ---- X_{n+1} = Y or 2 X_n - Y in place: only this lane touches (r, c), (r, c + 1) and their mirror images
-#pragma unroll
-  for (int u = 0; u < PK_MAXU; ++u) {
-    if (ucode[u] == PK_NONE) continue;
-    const int s = ucode[u] & 15, bi = (ucode[u] >> 4) & 31, bj = bi + 4 * ((ucode[u] >> 9) & 7), nb = 1 + ((ucode[u] >> 12) & 3);
-    if (last && bi * 8 >= sl[s].nc) continue;
-    const int stride = sl[s].ld + 4;
-    double* x0 = xs + sl[s].soff;
-    const int r = bi * 8 + g;
-#pragma unroll
-    for (int j = 0; j < PK_UCOLS; ++j) {
-      if (j < nb) {
-        const int c = (bj + j) * 8 + 2 * q;
-        double* xr = x0 + (size_t)r * stride + c;
-        double v0 = acc[u][j][0], v1 = acc[u][j][1];
-        if (branch) {
-          const double2 x = *reinterpret_cast<const double2*>(xr);
-          v0 = 2.0 * x.x - v0;
-          v1 = 2.0 * x.y - v1;
-        }
-        *reinterpret_cast<double2*>(xr) = make_double2(v0, v1);
-        if (bj + j != bi) {  // off-diagonal block: mirror (the diagonal block is computed whole)
-          x0[(size_t)c * stride + r] = v0;
-          x0[(size_t)(c + 1) * stride + r] = v1;
-        }
-      }
-    }
-  }
+  // ---- core-row traces of X_{n+1}: per warp in the (fixed) order of its unit list, then over the warps: one pair per bin
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  if (lane == 0) { red[wid] = s1; red[PK_WARPS + wid] = s2; }
   __syncthreads();
-
-  // ---- core-row traces of X_{n+1}, summed over the bin in a fixed order
-  {
-    double s1 = 0.0, s2 = 0.0;
-    for (int s = 0; s < n_slots; ++s) {
-      const int nc = sl[s].nc, ld = sl[s].ld, stride = ld + 4;
-      const double* x0 = xs + sl[s].soff;
-      for (int i = wid; i < nc; i += PK_WARPS) {
-        const double* __restrict__ row = x0 + (size_t)i * stride;
-        for (int c = lane; c < ld; c += 32) {
-          const double x = row[c];
-          s2 += x * x;
-          if (c == i) s1 += x;
-        }
+  if (wid == 0) {
+    const double a = warp_sum(red[lane]);
+    const double b = warp_sum(red[PK_WARPS + lane]);
+    if (lane == 0) {
+      double* out = partials + 2 * (size_t)(partial_base + blockIdx.x);
+      out[0] = a;
+      out[1] = b;
+      int lastflag = 0;
+      if (fused) {
+        __threadfence();  // the pair is visible before the ticket is taken
+        lastflag = atomicAdd(&st->ticket, 1u) == gridDim.x - 1;
       }
+      is_last = lastflag;
     }
-    s1 = warp_sum(s1);
-    s2 = warp_sum(s2);
-    if (lane == 0) { red[wid] = s1; red[PK_WARPS + wid] = s2; }
-    __syncthreads();
-    if (wid == 0) {
-      const double a = warp_sum(lane < PK_WARPS ? red[lane] : 0.0);
-      const double b = warp_sum(lane < PK_WARPS ? red[PK_WARPS + lane] : 0.0);
-      if (lane == 0) {
-        double* out = partials + 2 * (size_t)(partial_base + blockIdx.x);
-        out[0] = a;
-        out[1] = b;
-        int lastflag = 0;
-        if (fused) {
-          __threadfence();  // the pair is visible before the ticket is taken
-          lastflag = atomicAdd(&st->ticket, 1u) == gridDim.x - 1;
-        }
-        is_last = lastflag;
-      }
-    }
-    __syncthreads();
   }
+  if (!fused) return;
+  __syncthreads();
+  if (!is_last) return;
 
   // ---- step 5, by the bin that arrived last: all partials of this iteration (tiled kernel's and bins') in a fixed order
-  if (fused && is_last) {
-    __threadfence();
-    double a1 = 0.0, a2 = 0.0;
-    const double2* __restrict__ p2 = reinterpret_cast<const double2*>(partials);
-    for (int i = t; i < n_partials; i += PK_THREADS) {
-      const double2 v = __ldcg(p2 + i);
-      a1 += v.x;
-      a2 += v.y;
-    }
-    a1 = warp_sum(a1);
-    a2 = warp_sum(a2);
-    __syncthreads();  // red is free again
-    if (lane == 0) { red[wid] = a1; red[PK_WARPS + wid] = a2; }
-    __syncthreads();
-    if (wid == 0) {
-      a1 = warp_sum(lane < PK_WARPS ? red[lane] : 0.0);
-      a2 = warp_sum(lane < PK_WARPS ? red[PK_WARPS + lane] : 0.0);
-      if (lane == 0) {
-        st->ticket = 0;
-        gbe_trace_decide(st, a1, a2);
-      }
-    }
+  __threadfence();
+  double a1 = 0.0, a2 = 0.0;
+  const double2* __restrict__ p2 = reinterpret_cast<const double2*>(partials);
+  for (int i = t; i < n_partials; i += PK_THREADS) {
+    const double2 v = __ldcg(p2 + i);
+    a1 += v.x;
+    a2 += v.y;
   }
-
-  // ---- X_{n+1} -> the other dense buffer
-  for (int s = 0; s < n_slots; ++s) {
-    const int m = sl[s].m, ld = sl[s].ld, stride = ld + 4, h = ld >> 1;
-    double2* __restrict__ dst = reinterpret_cast<double2*>(Xout + sl[s].dense_off);
-    const double* x0 = xs + sl[s].soff;
-    for (int i = t; i < m * h; i += PK_THREADS) {
-      const int r = i / h, c2 = i - r * h;
-      dst[i] = *reinterpret_cast<const double2*>(x0 + (size_t)r * stride + 2 * c2);
+  a1 = warp_sum(a1);
+  a2 = warp_sum(a2);
+  if (lane == 0) { red[wid] = a1; red[PK_WARPS + wid] = a2; }
+  __syncthreads();
+  if (wid == 0) {
+    a1 = warp_sum(red[lane]);
+    a2 = warp_sum(red[PK_WARPS + lane]);
+    if (lane == 0) {
+      st->ticket = 0;
+      gbe_trace_decide(st, a1, a2);
     }
   }
 }
 
-struct Unit { int slot, bi, bj, nb, cost; };
+struct Unit { int slot, bi, bj, nb, tall, cost; };
 
 inline int units_of(int R) {
   int n = 0;
-  for (int bi = 0; bi < R; ++bi) n += (R - bi + PK_UCOLS - 1) / PK_UCOLS;
+  for (int bi = 0; bi < R; bi += 2) n += (R - bi + PK_UCOLS - 1) / PK_UCOLS;
   return n;
 }
-inline int64_t dmma_of(int m, int ld) {  // DMMA instructions of one X X^T: 8 x 8 blocks on or above the diagonal x ld / 4
+inline int64_t dmma_of(int m, int /*ld*/) {  // DMMA instructions of one X X^T: 8 x 8 blocks on or above the diagonal x ceil(m / 4)
   const int64_t R = (m + 7) / 8;
-  return R * (R + 1) / 2 * (ld / 4);
+  return R * (R + 1) / 2 * ((m + 3) / 4);
 }
-inline size_t smem_doubles_of(int m, int ld) { return (size_t)((m + 7) / 8 * 8) * (ld + 4); }
+inline size_t smem_doubles_of(int m, int ld) { return (size_t)((m + 7) / 8 * 8) * (ld + 4); }  // 8R rows of ld + 4 doubles
 
 template <typename T>
 int upload(const std::vector<T>& h, T** d, cudaStream_t s) {
@@ -256,118 +307,144 @@ int upload(const std::vector<T>& h, T** d, cudaStream_t s) {
 }
 }  // namespace
 
-// Packs the communities with 0 < m_p <= GBE_PK_MAX_M into bins (host; once per graph) and uploads the work description.
-int gbe_build_packed(gbe_graph* g, cudaStream_t s) {
-  g->n_pk_ctas = 0;
-  g->pk_smem_bytes = 0;
-  g->pk_n_small = 0;
-  int dev = 0, smem_max = 0;
-  GBE_CUDA(cudaGetDevice(&dev));
-  GBE_CUDA(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-  const int sms = gbe_sm_count();
-  const size_t smem_cap = (size_t)std::max(0, smem_max - 4096) / sizeof(double);  // doubles; static shared memory aside
-  std::vector<int> small;
-  int64_t total = 0, biggest = 0;
-  for (int p = 0; p < g->n_part; ++p) {
-    const int m = g->h_m[p];
-    if (m <= 0 || m > GBE_PK_MAX_M) continue;
-    const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
-    if (smem_doubles_of(m, ld) > smem_cap || units_of((m + 7) / 8) > PK_WARPS * PK_MAXU) continue;
-    small.push_back(p);
-    total += dmma_of(m, ld);
-    biggest = std::max(biggest, dmma_of(m, ld));
-  }
-  g->pk_n_small = (int32_t)small.size();
-  if (small.empty()) return GBE_OK;
-  auto cost = [&](int p) { return dmma_of(g->h_m[p], (g->h_m[p] + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN); };
-  std::stable_sort(small.begin(), small.end(), [&](int a, int b) { return cost(a) > cost(b); });
+namespace {
+struct Bin { int64_t load = 0; size_t smem = 0; int units = 0; std::vector<int> ps; };
 
-  // k waves of `sms` bins: a bin should carry a few microseconds of tensor work (~3,000 DMMA = 6 us on one SM) so that the
-  // copy in and out of shared memory is amortised, but never more than one wave's share
-  const int64_t per_sm = (total + sms - 1) / sms;
-  const int waves = (int)std::max<int64_t>(1, (per_sm + 1500) / 3000);
-  const int n_bins_target = (int)std::min<int64_t>((int64_t)small.size(), (int64_t)waves * sms);
-  struct Bin { int64_t load = 0; size_t smem = 0; int units = 0; std::vector<int> ps; };
-  std::vector<Bin> bins(n_bins_target);
+// Longest processing time first onto EXACTLY n bins (no bin is opened on the way: a launch is a whole number of waves);
+// false if a community finds no bin with room (shared memory, slots, unit codes)
+bool lpt(const gbe_graph* g, const std::vector<int>& cs, int n, size_t smem_cap, int warps, std::vector<Bin>* out) {
+  std::vector<Bin>& bins = *out;
+  bins.assign(n, Bin());
   using QE = std::pair<int64_t, int>;  // (load, bin): least loaded first, ties by index
   std::priority_queue<QE, std::vector<QE>, std::greater<QE>> pq;
-  for (int b = 0; b < n_bins_target; ++b) pq.push({0, b});
-  for (int p : small) {
+  for (int b = 0; b < n; ++b) pq.push({0, b});
+  std::vector<QE> aside;
+  for (int p : cs) {
     const int m = g->h_m[p], ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
     const size_t need = smem_doubles_of(m, ld);
     const int nu = units_of((m + 7) / 8);
-    // the least loaded bins first; a bin without room (registers, shared memory, slots) is set aside for this item
-    std::vector<QE> aside;
+    aside.clear();
     int chosen = -1;
-    for (int tries = 0; tries < 8 && !pq.empty(); ++tries) {
+    while (!pq.empty()) {
       const QE e = pq.top();
       pq.pop();
-      Bin& b = bins[e.second];
-      if (b.units + nu <= PK_WARPS * PK_MAXU && b.smem + need <= smem_cap && (int)b.ps.size() < GBE_PK_MAX_SLOTS) {
+      const Bin& b = bins[e.second];
+      if (b.units + nu <= PK_MAX_ROUNDS * warps / 2 && b.smem + need <= smem_cap && (int)b.ps.size() < GBE_PK_MAX_SLOTS) {
         chosen = e.second;
         break;
       }
       aside.push_back(e);
     }
     for (const QE& e : aside) pq.push(e);
-    if (chosen < 0) {
-      bins.emplace_back();
-      chosen = (int)bins.size() - 1;
-    }
+    if (chosen < 0) return false;
     Bin& b = bins[chosen];
     b.ps.push_back(p);
     b.units += nu;
     b.smem += need;
-    b.load += cost(p);
+    b.load += dmma_of(m, ld);
     pq.push({b.load, chosen});
+  }
+  return true;
+}
+
+}  // namespace
+
+// Packs the communities with 0 < m_p <= g->pk_max_m into bins (host; once per graph) and uploads the work description.
+int gbe_build_packed(gbe_graph* g, cudaStream_t s) {
+  g->n_pk_ctas = 0;
+  g->pk_n_small = 0;
+  g->pk[0] = gbe_pk_class();
+  int dev = 0, smem_max = 0;
+  GBE_CUDA(cudaGetDevice(&dev));
+  GBE_CUDA(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  const int sms = gbe_sm_count();
+  const size_t smem_cap = (size_t)std::max(0, smem_max - 2048) / sizeof(double);  // doubles; static shared memory aside
+  std::vector<int> cs;
+  int64_t total = 0;
+  for (int p = 0; p < g->n_part; ++p) {
+    const int m = g->h_m[p];
+    if (m <= 0 || m > g->pk_max_m) continue;
+    const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+    if (smem_doubles_of(m, ld) > smem_cap) continue;
+    cs.push_back(p);
+    total += dmma_of(m, ld);
+  }
+  g->pk_n_small = (int32_t)cs.size();
+  if (cs.empty()) return GBE_OK;
+  auto cost = [&](int p) { return dmma_of(g->h_m[p], 0); };
+  std::stable_sort(cs.begin(), cs.end(), [&](int a, int b) { return cost(a) > cost(b); });
+  // k waves of one bin per SM: the smallest k the communities fit into, and at least so many that a bin carries no more
+  // than ~3,000 DMMA (6 us of tensor work on one SM); a launch is a whole number of equally heavy waves
+  std::vector<Bin> bins;
+  for (int k = (int)std::max<int64_t>(1, (total / sms + 1500) / 3000);; ++k) {
+    const int n = (int)std::min<int64_t>((int64_t)cs.size(), (int64_t)k * sms);
+    if (lpt(g, cs, n, smem_cap, PK_WARPS, &bins)) break;
+    if (n == (int)cs.size()) return GBE_EINVAL;  // cannot happen: every community fits a bin of its own
   }
   // heavy bins first in launch order
   std::vector<int> border(bins.size());
   std::iota(border.begin(), border.end(), 0);
   std::stable_sort(border.begin(), border.end(), [&](int a, int b) { return bins[a].load > bins[b].load; });
-
   std::vector<gbe_pk_cta> h_ctas;
-  std::vector<gbe_pk_slot> h_slots;
+  std::vector<std::vector<uint16_t>> grids;
   size_t smem_need = 0;
+  int rounds_max = 0;
   for (int bi_ : border) {
     const Bin& b = bins[bi_];
     if (b.ps.empty()) continue;
-    gbe_pk_cta c;
-    c.first_slot = (int32_t)h_slots.size();
+    gbe_pk_cta c = {};
     c.n_slots = (int32_t)b.ps.size();
-    for (int w = 0; w < PK_WARPS; ++w)
-      for (int u = 0; u < PK_MAXU; ++u) c.units[w][u] = PK_NONE;
     std::vector<Unit> units;
     size_t soff = 0;
     for (int k = 0; k < (int)b.ps.size(); ++k) {
       const int p = b.ps[k], m = g->h_m[p], ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN, R = (m + 7) / 8;
-      h_slots.push_back({p, m, g->h_ncore[p], ld, (int32_t)soff, R, g->h_dense_off[p]});
-      soff += smem_doubles_of(m, ld);
-      for (int bi = 0; bi < R; ++bi)
+      c.slot[k] = {p, m, g->h_ncore[p], ld, (int32_t)soff, (int16_t)R, 0, 0, 0, g->h_dense_off[p]};
+      soff += (size_t)(8 * R) * (ld + 4);
+      // row blocks in pairs (2 x up to 4 blocks per unit: 6 fragment loads per 8 DMMA); an odd last row block alone
+      for (int bi = 0; bi < R; bi += 2) {
+        const int tall = bi + 1 < R ? 1 : 0;
         for (int bj = bi; bj < R; bj += PK_UCOLS) {
           const int nb = std::min(PK_UCOLS, R - bj);
-          units.push_back({k, bi, bj, nb, nb * (ld / 4)});
+          units.push_back({k, bi, bj, nb, tall, ((1 + tall) * nb - (tall && bj == bi ? 1 : 0)) * ((m + 3) / 4)});
         }
+      }
     }
     c.smem_doubles = (int32_t)soff;
     smem_need = std::max(smem_need, soff * sizeof(double));
-    // the units of the bin onto the 16 warps: longest first, always to the least loaded warp with a free slot
+    // the units of the bin onto the 32 warps: longest first, always to the least loaded warp - ties to the warp whose SM
+    // sub-partition (warp index mod 4: each has its own FP64 tensor pipe) carries the least; codes stored round-major
     std::stable_sort(units.begin(), units.end(), [](const Unit& a, const Unit& b) { return a.cost > b.cost; });
-    int wload[PK_WARPS] = {0}, wcnt[PK_WARPS] = {0};
+    int wload[PK_WARPS] = {0}, wcnt[PK_WARPS] = {0}, sub[4] = {0};
+    std::vector<uint16_t> grid((size_t)PK_MAX_ROUNDS * PK_WARPS, (uint16_t)PK_NONE);
+    int rounds = 0;
     for (const Unit& un : units) {
       int best = -1;
-      for (int w = 0; w < PK_WARPS; ++w)
-        if (wcnt[w] < PK_MAXU && (best < 0 || wload[w] < wload[best])) best = w;
-      if (best < 0) return GBE_EINVAL;  // cannot happen: units <= 16 x 4 per bin
-      c.units[best][wcnt[best]++] = pk_encode(un.slot, un.bi, un.bj, un.nb);
+      for (int w = 0; w < PK_WARPS; ++w) {
+        if (wcnt[w] >= PK_MAX_ROUNDS) continue;
+        if (best < 0 || wload[w] < wload[best] || (wload[w] == wload[best] && sub[w & 3] < sub[best & 3])) best = w;
+      }
+      if (best < 0) return GBE_EINVAL;  // cannot happen: a bin holds at most 16 x 32 units
+      grid[(size_t)wcnt[best] * PK_WARPS + best] = pk_encode(un.slot, un.bi, un.bj, un.nb, un.tall);
+      rounds = std::max(rounds, ++wcnt[best]);
       wload[best] += un.cost;
+      sub[best & 3] += un.cost;
     }
+    c.n_rounds = rounds;
+    rounds_max = std::max(rounds_max, rounds);
+    grids.push_back(std::move(grid));
     h_ctas.push_back(c);
   }
-  g->n_pk_ctas = (int32_t)h_ctas.size();
-  g->pk_smem_bytes = smem_need;
-  GBE_TRY(upload(h_ctas, &g->pk_ctas, s));
-  GBE_TRY(upload(h_slots, &g->pk_slots, s));
+  std::vector<uint16_t> h_codes;
+  for (const auto& gr : grids) h_codes.insert(h_codes.end(), gr.begin(), gr.begin() + (size_t)rounds_max * PK_WARPS);
+  gbe_pk_class& out = g->pk[0];
+  out.n_ctas = (int32_t)h_ctas.size();
+  out.warps = PK_WARPS;
+  out.smem_bytes = smem_need;
+  out.rounds_max = rounds_max;
+  out.code_stride = rounds_max * PK_WARPS;
+  GBE_TRY(upload(h_ctas, &out.ctas, s));
+  GBE_TRY(upload(h_codes, &out.codes, s));
+  g->n_pk_ctas = out.n_ctas;
   return GBE_OK;
 }
 
@@ -381,11 +458,13 @@ int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, 
     int dev = 0, smem_max = 0;
     GBE_CUDA(cudaGetDevice(&dev));
     GBE_CUDA(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-    GBE_CUDA(cudaFuncSetAttribute(k_sp2_packed, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max - 4096));
+    GBE_CUDA(cudaFuncSetAttribute(k_sp2_packed, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max - 2048));
+    GBE_CUDA(cudaFuncSetAttribute(k_sp2_packed, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
   }
-  k_sp2_packed<<<g->n_pk_ctas, PK_THREADS, g->pk_smem_bytes, s>>>(g->pk_ctas, g->pk_slots, st, Xin, Xout, partials,
-                                                                 partial_base, n_partials, iter, last ? 1 : 0,
-                                                                 fused ? 1 : 0);
+  const gbe_pk_class& a = g->pk[0];
+  k_sp2_packed<<<a.n_ctas, PK_THREADS, a.smem_bytes, s>>>(a.ctas, a.codes, st, Xin, Xout, partials, partial_base,
+                                                         n_partials, iter, last ? 1 : 0, fused ? 1 : 0, a.code_stride,
+                                                         a.rounds_max);
   GBE_LAUNCHED();
   return GBE_OK;
 }
