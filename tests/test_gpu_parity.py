@@ -247,6 +247,71 @@ def check_sampled_communities(s, ex, Dg, log, n_random):
         assert np.abs(got - cols).max() <= TOL_D, (p, len(idx))
 
 
+_FULL_BOX = {}
+
+
+def _full_box():
+    """The 24,576-orbital water box of BASELINE.json configs[2] and configs[4], generated once per test session."""
+    if "s" not in _FULL_BOX:
+        _FULL_BOX["s"] = gi.water_box(4096, 512, seed=0)
+    return _FULL_BOX["s"]
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("tau", [1e-3, 1e-4, 1e-5, 1e-6, 1e-7])
+def test_config5_full_grid_sampled_parity(gbe, tau):
+    """BASELINE.json configs[4] at FULL size: every (tau, communities) point of the grid on the 24,576-orbital box, 40 SP2
+    iterations, in the launch configuration bench.py --sweep times (the library's own choice of kernels).  Per tau the
+    graph S_tau is compared bit for bit with the oracle's own (it does not depend on the partition); per point the
+    any-size properties, and element by element (Eq.(6)) the largest, the smallest and two random communities
+    against the one-community oracle, which derives the subgraph from (H, tau) alone and replays the logged branch
+    sequence (the sequence is a global quantity).  The max |D_gpu - D_oracle| per point goes to
+    gpurun_out/config5_full_grid_parity.jsonl for profiles/."""
+    import json
+    import os
+    import torch
+    base = _full_box()
+    Hd = gbe.DeviceCSR.from_host(base.H)
+    rp, ci = o.build_graph(base.H, tau)
+    oc = None
+    for n_part in (128, 256, 512, 1024):
+        part = (np.arange(base.n) // -(-base.n // n_part)).astype(np.int32)  # part = NULL: contiguous blocks
+        g = gbe.gbe_build_graph(Hd, tau, None, n_part)
+        D, log = gbe.gbe_density(Hd, g, base.n_occ, base.iters)
+        torch.cuda.synchronize()
+        ex = {k: v.cpu().numpy() for k, v in g.export().items()}
+        Dg = D.cpu().numpy()
+        assert np.array_equal(ex["S_row_ptr"], rp) and np.array_equal(ex["S_col"], ci)
+
+        class _S:  # what the two checkers read
+            pass
+        sv = _S()
+        sv.H, sv.tau, sv.part, sv.n_part, sv.n, sv.n_occ, sv.iters = base.H, tau, part, n_part, base.n, base.n_occ, base.iters
+        check_any_size_properties(sv, g, ex, Dg, log)
+        if oc is None:
+            oc = o.OneCommunity(base.H, tau, part)
+        oc.part = part
+        m = np.diff(ex["sub_ptr"])
+        rng = np.random.default_rng(int(n_part))
+        picks = {int(np.argmax(m)), int(np.argmin(m))} | {int(p) for p in rng.choice(n_part, size=2, replace=False)}
+        Dm = sp.csr_matrix((Dg, ex["D_col"], ex["D_row_ptr"]), shape=(base.n, base.n))
+        worst = 0.0
+        for p in sorted(picks):
+            idx, nc, cols = oc.expand(p, log.branch, log.iters_done)
+            a, b = ex["sub_ptr"][p], ex["sub_ptr"][p + 1]
+            assert np.array_equal(ex["sub_idx"][a:b], idx) and ex["ncore"][p] == nc
+            worst = max(worst, float(np.abs(Dm[idx][:, idx[:nc]].toarray() - cols).max()))
+        assert worst <= TOL_D, (tau, n_part, worst)
+        out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+        if os.path.isdir(out):
+            with open(os.path.join(out, "config5_full_grid_parity.jsonl"), "a") as f:
+                f.write(json.dumps({"tau": tau, "n_part": n_part, "sp2_path": int(g.info["sp2_path_chosen"]),
+                                    "m_min": int(m.min()), "m_max": int(m.max()), "communities_checked": sorted(picks),
+                                    "max_abs_dD": worst, "graph_bit_exact": True, "iters": int(log.iters_done)}) + "\n")
+        g.free()
+        del D, Dg, Dm, ex
+
+
 @pytest.mark.slow
 def test_config4_full_size_properties(gbe):
     """BASELINE.json configs[3] at full size (2,000 residues, ~1.2e5 orbitals, 2 x 27 GB dense batch).  The oracle would
