@@ -23,6 +23,11 @@
  *   - gbe_build_graph synchronises the stream (it sizes its outputs).  gbe_density and the three phase calls
  *     only enqueue work: no host round trip between SP2 iterations; they return before completion.
  *   - CSR: row_ptr int64 [n+1], col_idx int32 [nnz] ascending within a row, val double [nnz]; 0-based.
+ *   - Devices and threads.  Every call works on the CURRENT device of the calling thread (cudaSetDevice); a graph, its
+ *     workspace and the buffers passed with it belong to the device that was current when the graph was built.  One-time
+ *     set-up (kernel attributes, memory-pool thresholds) is kept per device.  Calls from different host threads are safe as
+ *     long as they do not share a graph handle, a workspace or an output buffer; the process-wide knobs
+ *     (gbe_set_build_scratch_limit, gbe_set_packed_max_m) are atomic but apply to graphs built afterwards.
  */
 #ifndef GBE_H
 #define GBE_H
@@ -41,7 +46,10 @@ typedef enum {
                            (the index maps of steps 1-3 are bitmaps over the n vertices in shared memory: about
                            4e5 orbitals with core+halo sizes up to a few thousand) */
   GBE_ENOTSYM = -2,     /* H is not symmetric (pattern or values); only tested when opts.check_symmetry != 0 */
-  GBE_EDEGENERATE = -3, /* eps_max == eps_min: the spectrum cannot be mapped to [0,1] (A-12) */
+  GBE_EDEGENERATE = -3, /* eps_max == eps_min: the spectrum cannot be mapped to [0,1] (A-12).  gbe_build_graph returns it;
+                           the density calls only enqueue work, so for THEIR H it is reported by gbe_read_log (hence by a
+                           call with log != NULL) - without a log they return GBE_OK and D holds the finite values of
+                           X0 = (eps_max I - H) / 1 carried through the same updates */
   GBE_EMISMATCH = -4,   /* H.n differs from the graph's n */
   GBE_ENOMEM = -5,      /* workspace too small (required size: gbe_graph_info.workspace_bytes) or allocation failed */
   GBE_ECUDA = -6        /* a CUDA call failed; text via gbe_strerror / gbe_last_cuda_error */
@@ -187,7 +195,9 @@ int gbe_graph_set_gather_path(gbe_graph* g, int32_t path);
  *   workspace device memory, >= info.workspace_bytes, 256-byte aligned; contents are scratch.
  *   D_val     device double[nnz_D], CSR order of (D_row_ptr, D_col); entry (k,i) is taken from the expansion of
  *             the community that owns column i.  NOT symmetric (obs. (i) P:L65); not symmetrised.
- *   log       optional host log; filled by an asynchronous copy (synchronise the stream before reading). */
+ *   log       optional host log.  With log != NULL the call SYNCHRONISES the stream (twice: the header of the log sizes the
+ *             copy of its arrays) and is therefore not capturable in a CUDA graph; with log == NULL it only enqueues
+ *             (gbe_read_log fetches the log of the last run later). */
 int gbe_density(const gbe_csr_view* H, const gbe_graph* g, double n_occ, int32_t iters, double idem_tol,
                 void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val, gbe_sp2_log* log);
 

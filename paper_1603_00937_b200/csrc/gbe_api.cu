@@ -134,27 +134,29 @@ static int build_graph_impl(const gbe_csr_view* H, const gbe_graph_opts* opts, c
     ~Guard() { if (g) gbe_free_graph(g); }
   } guard{g};
 
-  // step 0: bounds of the H given here
+  // step 0: bounds of the H given here; they travel to pinned host words and are looked at after the first
+  // synchronisation of the build (a build has three: accumulator capacity of the product; subgraph sizes + nnz(S); end)
   DevBuf st, bl;
   GBE_TRY(st.alloc(sizeof(gbe_state)));
   GBE_TRY(bl.alloc(2 * 1024 * sizeof(double)));
   GBE_TRY(gbe_launch_bounds(*H, bl.as<double>(), bl.as<double>() + 1024, 1024, st.as<gbe_state>(), s));
-  struct { double lo, hi; } b;
-  GBE_CUDA(cudaMemcpyAsync(&b, st.p, sizeof(b), cudaMemcpyDeviceToHost, s));
-  GBE_CUDA(cudaStreamSynchronize(s));
-  if (!(b.hi > b.lo) || !std::isfinite(b.lo) || !std::isfinite(b.hi)) return GBE_EDEGENERATE;
-  g->eps_min = b.lo;
-  g->eps_max = b.hi;
+  double stack_b[2] = {0.0, 0.0};
+  int32_t* const pin = gbe_pinned_words();
+  double* const b = pin ? reinterpret_cast<double*>(pin + 8) : stack_b;
+  GBE_CUDA(cudaMemcpyAsync(b, st.p, 2 * sizeof(double), cudaMemcpyDeviceToHost, s));
+  if (!pin) GBE_CUDA(cudaStreamSynchronize(s));
 
   // step 1: S_tau - from H and its thresholded powers (A-1), or by Eq.(8) from the previous D and this H
   if (prev)
-    GBE_TRY(gbe_build_pattern_eq8(*H, prev->D_row_ptr, prev->D_col, D_prev, g->tau, s, &g->S_row_ptr, &g->S_col, &g->nnz_S));
+    GBE_TRY(gbe_build_pattern_eq8(*H, prev->D_row_ptr, prev->D_col, D_prev, g->tau, s, &g->S_row_ptr, &g->S_col, &g->nnz_S,
+                                  &g->S_cap, prev->nnz_D));
   else
     GBE_TRY(gbe_build_pattern(*H, st.as<gbe_state>(), g->tau, power, opts->check_symmetry, s, &g->S_row_ptr, &g->S_col,
-                              &g->nnz_S));
-  // step 2: subgraphs, layout, pattern of D, work lists
-  GBE_TRY(gbe_build_subgraphs(g, part, s));
-  GBE_CUDA(cudaStreamSynchronize(s));
+                              &g->nnz_S, &g->S_cap));
+  // step 2: subgraphs, layout, pattern of D, work lists (synchronises; checks the bounds)
+  GBE_TRY(gbe_build_subgraphs(g, part, s, b));
+  g->eps_min = b[0];
+  g->eps_max = b[1];
   guard.g = nullptr;
   *out = g;
   return GBE_OK;
@@ -284,12 +286,9 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
   GBE_TRY(carve(g, workspace, workspace_bytes, &w));
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const int mode = !preset ? 0 : (trace_each ? 1 : 2);
-  const int path = choose_sp2(g, mode);
-  // Packed kernel with EVERY community packed: a bin has all of its X_p in shared memory before it stores anything, so
-  // X is updated in place in buffer 0 - half the footprint, which keeps a batch of up to ~60 MB resident in L2 (measured:
-  // with two 41 MB buffers every iteration re-read X from DRAM)
-  const int inplace = path == 3 && g->n_items_h == 0;
+  int path = choose_sp2(g, mode);
   if (path == 2) {
+    const int inplace = 0;
     // small communities: the whole loop in one kernel, X_p resident in shared memory (gbe_resident.cu)
     GBE_TRY(timed(tm, PH_TRACE, 1, [&]() -> int {
       k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode, inplace);
@@ -298,11 +297,19 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
         GBE_CUDA(cudaMemcpyAsync(w.st->br, preset, (size_t)iters, cudaMemcpyHostToDevice, s));
       return GBE_OK;
     }));
-    GBE_TRY(timed(tm, PH_X2, 1, [&] { return gbe_launch_sp2_resident(g, w.st, w.X0, w.X1, w.partials, mode, s); }));
-    if (mode == 2)
-      GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, g->n_part, s); }));
-    return GBE_OK;
+    const int rc = timed(tm, PH_X2, 1, [&] { return gbe_launch_sp2_resident(g, w.st, w.X0, w.X1, w.partials, mode, s); });
+    if (rc != GBE_RESIDENT_UNAVAILABLE) {
+      GBE_TRY(rc);
+      if (mode == 2)
+        GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, g->n_part, s); }));
+      return GBE_OK;
+    }
+    // the grid does not fit the device at this moment (shared device): the kernels without a grid barrier take over
+    path = g->n_pk_ctas > 0 && g->n_items_h == 0 ? 3 : 1;
   }
+  // Packed kernel with EVERY community packed: a bin has all of its X_p in shared memory before it stores anything, so
+  // X is updated in place in buffer 0 (half the footprint in L2)
+  const int inplace = path == 3 && g->n_items_h == 0;
   // traces of X_0 (partials written by the gather), branch of iteration 0
   GBE_TRY(timed(tm, PH_TRACE, mode == 2 ? 1 : 2, [&]() -> int {
     k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode, inplace);

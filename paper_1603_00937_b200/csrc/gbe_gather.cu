@@ -43,7 +43,9 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   const int m = (int)(sub_ptr[p + 1] - sb);
   const int nc = ncore_arr[p];
   const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
-  const double eps_max = st->eps_max, delta = st->eps_max - st->eps_min;
+  // degenerate bounds (eps_max == eps_min, A-12: H is a multiple of I): the status travels with gbe_read_log; the values are
+  // kept finite with delta = 1 (X0 = 0) so that a call without a log still writes a defined D
+  const double eps_max = st->eps_max, delta = st->degenerate ? 1.0 : st->eps_max - st->eps_min;
   const double inv_delta = 1.0 / delta;
   // x / delta as a reciprocal multiply plus one residual correction: the correctly rounded quotient except in rare
   // half-ulp cases, at a tenth of the instructions of the IEEE division sequence (the row loop is issue bound)

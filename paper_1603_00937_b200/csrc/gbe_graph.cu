@@ -410,8 +410,9 @@ __global__ void k_check_symmetric(int64_t n, const int64_t* __restrict__ rp, con
     }
     bool ok = lo < rp[j + 1] && col[lo] == i;
     if (ok) {
-      const double u = val[lo];
-      ok = fabs(u - v) <= 1e-12 * fmax(fabs(u), fabs(v));
+      // exact equality: with the default power 2 only the upper triangle of floor(A A)_tau is formed, which is the whole
+      // product only if A is symmetric bit for bit (an entry within rounding of tau could otherwise differ from its mirror)
+      ok = val[lo] == v;
     } else {
       ok = (v == 0.0);  // an explicitly stored zero needs no partner
     }
@@ -431,7 +432,9 @@ struct Pattern {  // device CSR (pattern, optionally with values) owned by DevBu
   int64_t nnz = 0;
 };
 
-int count_to_rowptr(DevBuf& cnt, int64_t n, DevBuf& rp, int64_t* nnz, cudaStream_t s);
+// row counts -> row pointers.  ub < 0: the total comes back to the host (one synchronisation); ub >= 0: a known upper
+// bound of the total - the caller sizes its arrays with it and nothing comes back (*nnz = ub; the exact total is rp[n])
+int count_to_rowptr(DevBuf& cnt, int64_t n, DevBuf& rp, int64_t* nnz, cudaStream_t s, int64_t ub = -1);
 
 // row-wise unions on the device: out = [I u] filter(P) u Q
 struct Unioner {
@@ -454,11 +457,11 @@ struct Unioner {
     return ucnt.alloc((size_t)n * 4);
   }
   int run(const int64_t* p_rp, const int32_t* p_col, const double* p_val, double p_tau, const int64_t* q_rp,
-          const int32_t* q_col, const int32_t* q_len, int diag, Pattern& out) {
+          const int32_t* q_col, const int32_t* q_len, int diag, Pattern& out, int64_t ub = -1) {
     k_union_rows<false><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, p_val, p_tau, q_rp, q_col, q_len, diag,
                                                               ucnt.as<int32_t>(), nullptr, nullptr);
     GBE_LAUNCHED();
-    GBE_TRY(count_to_rowptr(ucnt, n, out.rp, &out.nnz, s));
+    GBE_TRY(count_to_rowptr(ucnt, n, out.rp, &out.nnz, s, ub));
     GBE_TRY(out.col.alloc((size_t)out.nnz * 4));
     k_union_rows<true><<<ugrid, uw * 32, bm_bytes * uw, s>>>(n, W, p_rp, p_col, p_val, p_tau, q_rp, q_col, q_len, diag,
                                                              nullptr, out.rp.as<int64_t>(), out.col.as<int32_t>());
@@ -467,8 +470,10 @@ struct Unioner {
   }
 };
 
-// S = P u P^T (P's rows need not be sorted on input; S's are ascending)
-int symmetrise(Pattern& P, Unioner& U, DevBuf& cnt, Pattern& S) {
+// S = P u P^T (P's rows need not be sorted on input; S's are ascending).  P.nnz may be an upper bound; with `bounded` S
+// is sized by 2 P.nnz and nothing comes back to the host (the caller fetches the exact count, S.rp[n], when it next
+// synchronises), else S is sized exactly (one synchronisation)
+int symmetrise(Pattern& P, Unioner& U, DevBuf& cnt, Pattern& S, bool bounded) {
   const int64_t n = U.n;
   cudaStream_t s = U.s;
   const int rows_grid = (int)((n + 7) / 8);
@@ -476,21 +481,24 @@ int symmetrise(Pattern& P, Unioner& U, DevBuf& cnt, Pattern& S) {
   GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
   k_transpose_count<<<rows_grid, 256, 0, s>>>(n, P.rp.as<int64_t>(), P.col.as<int32_t>(), cnt.as<int32_t>());
   GBE_LAUNCHED();
-  GBE_TRY(count_to_rowptr(cnt, n, PT.rp, &PT.nnz, s));
+  GBE_TRY(count_to_rowptr(cnt, n, PT.rp, &PT.nnz, s, P.nnz));  // a transpose has as many entries
   GBE_TRY(PT.col.alloc((size_t)PT.nnz * 4));
   GBE_CUDA(cudaMemsetAsync(cnt.p, 0, (size_t)n * 4, s));
   k_transpose_fill<<<rows_grid, 256, 0, s>>>(n, P.rp.as<int64_t>(), P.col.as<int32_t>(), PT.rp.as<int64_t>(),
                                              cnt.as<int32_t>(), PT.col.as<int32_t>());
   GBE_LAUNCHED();
   GBE_TRY(U.run(P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr, 0.0, PT.rp.as<int64_t>(), PT.col.as<int32_t>(), nullptr,
-                0, S));
-  GBE_CUDA(cudaStreamSynchronize(s));
-  return GBE_OK;
+                0, S, bounded ? 2 * P.nnz : -1));
+  return GBE_OK;  // (no synchronisation: the temporaries are released in stream order)
 }
 
-int count_to_rowptr(DevBuf& cnt, int64_t n, DevBuf& rp, int64_t* nnz, cudaStream_t s) {
+int count_to_rowptr(DevBuf& cnt, int64_t n, DevBuf& rp, int64_t* nnz, cudaStream_t s, int64_t ub) {
   GBE_TRY(rp.alloc((size_t)(n + 1) * 8));
   GBE_TRY(gbe_exclusive_scan_i32_to_i64(cnt.as<int32_t>(), rp.as<int64_t>(), n, s));
+  if (ub >= 0) {
+    *nnz = ub;
+    return GBE_OK;
+  }
   GBE_CUDA(cudaMemcpyAsync(nnz, rp.as<int64_t>() + n, 8, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaStreamSynchronize(s));
   return GBE_OK;
@@ -498,8 +506,12 @@ int count_to_rowptr(DevBuf& cnt, int64_t n, DevBuf& rp, int64_t* nnz, cudaStream
 
 }  // namespace
 
+// Outputs sized by upper bounds are kept below this many bytes; beyond it the exact sizes are fetched (more
+// synchronisations, less memory)
+static const size_t UB_BYTES_MAX = (size_t)4 << 30;
+
 int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, int power, int check_sym,
-                      cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S) {
+                      cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S, int64_t* S_cap) {
   const int64_t n = H.n;
   const int W = (int)((n + 31) / 32);
   const int rows_grid = (int)((n + 7) / 8);
@@ -525,7 +537,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   k_materialise_A<false><<<rows_grid, 256, 0, s>>>(n, H.row_ptr, H.col_idx, H.val, st, tau, cnt.as<int32_t>(), nullptr,
                                                    nullptr, nullptr);
   GBE_LAUNCHED();
-  GBE_TRY(count_to_rowptr(cnt, n, A.rp, &A.nnz, s));
+  GBE_TRY(count_to_rowptr(cnt, n, A.rp, &A.nnz, s, H.nnz + n));  // at most the stored entries + the missing diagonals
   GBE_TRY(A.col.alloc((size_t)A.nnz * 4));
   GBE_TRY(A.val.alloc((size_t)A.nnz * 8));
   k_materialise_A<true><<<rows_grid, 256, 0, s>>>(n, H.row_ptr, H.col_idx, H.val, st, tau, nullptr, A.rp.as<int64_t>(),
@@ -537,14 +549,14 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
   DevBuf& ucnt = U.ucnt;
   (void)ucnt;
   auto do_union = [&](const int64_t* p_rp, const int32_t* p_col, const int64_t* q_rp, const int32_t* q_col,
-                      const int32_t* q_len, int diag, Pattern& out) -> int {
-    return U.run(p_rp, p_col, nullptr, 0.0, q_rp, q_col, q_len, diag, out);
+                      const int32_t* q_len, int diag, Pattern& out, int64_t ub = -1) -> int {
+    return U.run(p_rp, p_col, nullptr, 0.0, q_rp, q_col, q_len, diag, out, ub);
   };
 
   // (with the default power 2 the union with the second power below takes I and pat(A) directly: one union less)
   Pattern P;
   const bool P_built = power != 2;
-  if (P_built) GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), nullptr, nullptr, nullptr, 1, P));
+  if (P_built) GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), nullptr, nullptr, nullptr, 1, P, A.nnz + n));
   // thresholded powers
   Pattern Tprev;  // T^(k-1) with values; T^(1) aliases A
   const int64_t* T_rp = A.rp.as<int64_t>();
@@ -609,13 +621,16 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
                                                                  cnt.as<int32_t>(), Tc.rp.as<int64_t>(),
                                                                  Tc.col.as<int32_t>(), nullptr, bm_io, t_start);
       GBE_LAUNCHED();
+      // P u kept(T^(k)) has at most nnz(P) + candidates entries: sized by that bound while it is small, no count comes back
       Pattern Pn;
+      const int64_t ub_base = (P_built ? P.nnz : A.nnz + n) + total_cand;
+      const int64_t ub = (size_t)ub_base * 8 <= UB_BYTES_MAX ? ub_base : -1;
       if (P_built)
         GBE_TRY(do_union(P.rp.as<int64_t>(), P.col.as<int32_t>(), Tc.rp.as<int64_t>(), Tc.col.as<int32_t>(),
-                         cnt.as<int32_t>(), 0, Pn));
+                         cnt.as<int32_t>(), 0, Pn, ub));
       else
         GBE_TRY(do_union(A.rp.as<int64_t>(), A.col.as<int32_t>(), Tc.rp.as<int64_t>(), Tc.col.as<int32_t>(),
-                         cnt.as<int32_t>(), 1, Pn));
+                         cnt.as<int32_t>(), 1, Pn, ub));
       // (no synchronisation here: the scratch buffers are released in stream order)
       std::swap(P.rp.p, Pn.rp.p);
       std::swap(P.col.p, Pn.col.p);
@@ -650,10 +665,13 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     T_val = Tprev.val.as<double>();
     // Tn (now holding the previous T) and Pn are released here, after the sync above
   }
-  // S = P u P^T
+  // S = P u P^T, sized by 2 nnz(P) while that bound is small: the exact nnz(S) = S_row_ptr[n] is then fetched by the
+  // caller with its next synchronisation (*nnz_S = -1, *S_cap = entries allocated)
   Pattern S;
-  GBE_TRY(symmetrise(P, U, cnt, S));
-  *nnz_S = S.nnz;
+  const bool bounded = (size_t)P.nnz * 8 <= UB_BYTES_MAX;
+  GBE_TRY(symmetrise(P, U, cnt, S, bounded));
+  *nnz_S = bounded ? -1 : S.nnz;
+  *S_cap = S.nnz;
   *S_row_ptr = reinterpret_cast<int64_t*>(S.rp.release());
   *S_col = reinterpret_cast<int32_t*>(S.col.release());
   return GBE_OK;
@@ -664,7 +682,8 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
 //     M = I u pat(|D_ij| >= tau) u pat(H(t)),   S = pat(M M) ("paths of length two"),  then S u S^T.
 // D is the assembled, non-symmetric P_tau of the previous step on the pattern (D_rp, D_col).
 int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int32_t* D_col, const double* D_val, double tau,
-                          cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S) {
+                          cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S, int64_t* S_cap,
+                          int64_t nnz_D) {
   const int64_t n = H.n;
   const int W = (int)((n + 31) / 32);
   const int sm_count = gbe_sm_count();  // of the current device
@@ -673,7 +692,7 @@ int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int3
   DevBuf cnt;
   GBE_TRY(cnt.alloc((size_t)n * 4));
   Pattern M;
-  GBE_TRY(U.run(D_rp, D_col, D_val, tau, H.row_ptr, H.col_idx, nullptr, 1, M));
+  GBE_TRY(U.run(D_rp, D_col, D_val, tau, H.row_ptr, H.col_idx, nullptr, 1, M, nnz_D + H.nnz + n));
   // symbolic square: count the candidates of every row, then emit them
   const size_t per_warp = (size_t)W * 8;
   const int nw = pick_warps(per_warp, 16);
@@ -699,8 +718,10 @@ int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int3
                                                              P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr, bm_io, nullptr);
   GBE_LAUNCHED();
   Pattern S;
-  GBE_TRY(symmetrise(P, U, cnt, S));
-  *nnz_S = S.nnz;
+  const bool bounded = (size_t)P.nnz * 8 <= UB_BYTES_MAX;
+  GBE_TRY(symmetrise(P, U, cnt, S, bounded));
+  *nnz_S = bounded ? -1 : S.nnz;
+  *S_cap = S.nnz;
   *S_row_ptr = reinterpret_cast<int64_t*>(S.rp.release());
   *S_col = reinterpret_cast<int32_t*>(S.col.release());
   return GBE_OK;

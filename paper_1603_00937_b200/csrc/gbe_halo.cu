@@ -13,6 +13,8 @@
 #include <algorithm>
 #include <numeric>
 
+#include <cmath>
+
 #include "gbe_internal.cuh"
 
 namespace {
@@ -245,7 +247,7 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 }  // namespace
 
-int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
+int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const double* bounds) {
   const int64_t n = g->n;
   const int n_part = g->n_part;
   const int W = (int)((n + 31) / 32);
@@ -288,8 +290,23 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
   g->h_ncore.resize(n_part);
   GBE_CUDA(cudaMemcpyAsync(g->h_m.data(), g->msize, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaMemcpyAsync(g->h_ncore.data(), g->ncore, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
+  int64_t nnz_S_stack = 0;
+  int64_t* const nnz_S_host = pin ? reinterpret_cast<int64_t*>(pin + 4) : &nnz_S_stack;
+  if (g->nnz_S < 0) GBE_CUDA(cudaMemcpyAsync(nnz_S_host, g->S_row_ptr + n, 8, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaStreamSynchronize(s));
   if (*core_flag) return GBE_EINVAL;  // partition id out of range (k_core_count)
+  if (bounds && (!(bounds[1] > bounds[0]) || !std::isfinite(bounds[0]) || !std::isfinite(bounds[1]))) return GBE_EDEGENERATE;
+  if (g->nnz_S < 0) {  // S_col was sized by an upper bound (gbe_build_pattern): the exact count is here now - trim
+    g->nnz_S = *nnz_S_host;
+    if (g->S_cap > g->nnz_S + g->nnz_S / 4 + 1024) {
+      int32_t* exact = nullptr;
+      GBE_TRY(gbe_dev_alloc((void**)&exact, std::max<size_t>(16, (size_t)g->nnz_S * 4)));
+      GBE_CUDA(cudaMemcpyAsync(exact, g->S_col, (size_t)g->nnz_S * 4, cudaMemcpyDeviceToDevice, s));
+      gbe_dev_free(g->S_col);  // stream ordered: after the copy
+      g->S_col = exact;
+      g->S_cap = g->nnz_S;
+    }
+  }
   // ---- host: layout, work lists
   std::vector<int64_t> h_sub_ptr(n_part + 1, 0);
   g->h_dense_off.assign(n_part + 1, 0);
@@ -434,7 +451,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
                                                        g->scat_base, flag.as<int32_t>(), nullptr, nullptr);
   GBE_LAUNCHED();
   GBE_CUDA(cudaMemcpyAsync(&hflag, flag.p, 4, cudaMemcpyDeviceToHost, s));
-  GBE_CUDA(cudaStreamSynchronize(s));
+  GBE_CUDA(cudaStreamSynchronize(s));  // the last synchronisation of a build (the general scatter map below needs one more)
   g->contiguous = hflag ? 0 : 1;
   if (!g->contiguous) {
     DevBuf rn, scat_ofs;
@@ -451,6 +468,5 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s) {
     GBE_CUDA(cudaStreamSynchronize(s));
     g->scat_ofs = reinterpret_cast<int64_t*>(scat_ofs.release());
   }
-  GBE_CUDA(cudaStreamSynchronize(s));
   return GBE_OK;
 }

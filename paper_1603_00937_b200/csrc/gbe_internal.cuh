@@ -113,6 +113,7 @@ struct gbe_tile_item {  // one X^2 work item: tile (ti, tj), ti <= tj, of commun
 // ----------------------------------------------------------------------------------------------
 struct gbe_graph {
   int64_t n = 0, nnz_S = 0, sum_m = 0, nnz_D = 0, dense_elems = 0;
+  int64_t S_cap = 0;  // entries S_col was allocated for (an upper bound until gbe_build_subgraphs trims it)
   int32_t n_part = 0, max_m = 0, max_ncore = 0, tile = 64;
   double eps_min = 0, eps_max = 0, tau = 0, flops_per_iter = 0, exec_flops_per_iter = 0;
   double flops_last_iter = 0, exec_flops_last_iter = 0;  // the core-tiles-only last iteration
@@ -176,13 +177,17 @@ struct gbe_graph {
 int gbe_launch_bounds(const gbe_csr_view& H, double* block_lo, double* block_hi, int max_blocks, gbe_state* st,
                       cudaStream_t s);
 // step 1
+// *nnz_S = -1: S_col was sized by an upper bound (*S_cap entries); the exact count is S_row_ptr[n] on the device and
+// gbe_build_subgraphs fetches it with its first synchronisation (and trims the array)
 int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st_dev, double tau, int power, int check_sym,
-                      cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S);
+                      cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S, int64_t* S_cap);
 // Eq.(8): S for the next MD step from the previous D and the new H
 int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int32_t* D_col, const double* D_val, double tau,
-                          cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S);
+                          cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S, int64_t* S_cap,
+                          int64_t nnz_D);
 // step 2
-int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s);
+// bounds: pinned host copy of (eps_min, eps_max) of step 0, in flight on `s`: looked at after the first synchronisation
+int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const double* bounds);
 // step 3
 int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state* st, double* X, double* partials,
                       cudaStream_t s);
@@ -193,6 +198,7 @@ int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* 
                   bool last, bool hybrid, cudaStream_t s);
 // steps 4 + 5 in one kernel for small communities (gbe_resident.cu); mode as in k_init_state
 int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident, int* cluster);
+constexpr int GBE_RESIDENT_UNAVAILABLE = 1;  // internal: the cooperative / cluster launch does not fit the device right now
 int gbe_launch_sp2_resident(const gbe_graph* g, gbe_state* st, double* X0, double* X1, double* partials, int mode,
                             cudaStream_t s);
 // steps 4 + 5, one iteration per launch, for communities with m <= g->pk_max_m (gbe_small.cu)

@@ -311,7 +311,9 @@ int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident, int* c
   GBE_CUDA(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
   GBE_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   const size_t smem = rs_smem_bytes(g->max_m);
-  if (smem + 1024 > (size_t)smem_max) return GBE_OK;
+  cudaFuncAttributes fa;
+  GBE_CUDA(cudaFuncGetAttributes(&fa, k_sp2_resident));
+  if (smem + fa.sharedSizeBytes > (size_t)smem_max) return GBE_OK;  // dynamic + the kernel's static shared memory
   GBE_CUDA(cudaFuncSetAttribute(k_sp2_resident, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0;
   GBE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sp2_resident, RS_THREADS, smem));
@@ -364,10 +366,22 @@ int gbe_launch_sp2_resident(const gbe_graph* g, gbe_state* st, double* X0, doubl
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    GBE_CUDA(cudaLaunchKernelEx(&cfg, k_sp2_resident, msize, ncore, doff, st, X0, X1, partials, n_part, mode, cl));
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, k_sp2_resident, msize, ncore, doff, st, X0, X1, partials, n_part, mode, cl);
+    if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorLaunchOutOfResources) {
+      (void)cudaGetLastError();
+      return GBE_RESIDENT_UNAVAILABLE;
+    }
+    GBE_CUDA(e);
   } else {
     void* args[] = {&msize, &ncore, &doff, &st, &X0, &X1, &partials, &n_part, &mode, &cl};
-    GBE_CUDA(cudaLaunchCooperativeKernel((const void*)k_sp2_resident, dim3(n_part), dim3(RS_THREADS), args, smem, s));
+    // the co-residency was established at build time on an otherwise idle device: if the device is shared now and the
+    // grid no longer fits, the caller falls back to the kernels that need no grid barrier
+    const cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_sp2_resident, dim3(n_part), dim3(RS_THREADS), args, smem, s);
+    if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorLaunchOutOfResources) {
+      (void)cudaGetLastError();
+      return GBE_RESIDENT_UNAVAILABLE;
+    }
+    GBE_CUDA(e);
   }
   GBE_LAUNCHED();
   return GBE_OK;

@@ -58,4 +58,26 @@ def test_sass_uses_fp64_tensor_cores_and_async_copies(libpath):
     sass = subprocess.run(["cuobjdump", "-sass", libpath], capture_output=True, text=True).stdout
     assert "DMMA.8x8x4" in sass      # mma.sync f64 -> FP64 tensor pipe
     assert "LDGSTS" in sass          # cp.async staging of the X panels
+    assert "UBLKCP" in sass          # TMA bulk copies (cp.async.bulk) of the packed small-m kernel
     assert "sm_100a" in sass
+
+
+def test_sources_take_the_current_device_not_a_literal_one():
+    """include/gbe.h: every call works on the CURRENT device.  No CUDA runtime query in the sources may name a device by a
+    literal index, none may assume the SM count of one product, and one-time set-up must not hang on a process-wide flag."""
+    import glob
+    bad = []
+    for path in sorted(glob.glob(os.path.join(ROOT, "paper_1603_00937_b200", "csrc", "*.cu*"))):
+        text = open(path).read()
+        code = re.sub(r"//[^\n]*", "", text)
+        for m in re.finditer(r"cudaDeviceGetAttribute\s*\(([^;]*?)\)\s*[;)]", code, flags=re.S):
+            last = m.group(1).split(",")[-1].strip()
+            if re.fullmatch(r"\d+", last):
+                bad.append((os.path.basename(path), "cudaDeviceGetAttribute(..., %s)" % last))
+        for m in re.finditer(r"\b148\b", code):
+            bad.append((os.path.basename(path), "literal SM count 148"))
+        for m in re.finditer(r"static\s+bool\s+\w+\s*=\s*false", code):
+            bad.append((os.path.basename(path), m.group(0)))
+        for m in re.finditer(r"cudaSetDevice\s*\(\s*\d+\s*\)|cudaDeviceGetDefaultMemPool\s*\([^,]*,\s*\d+\s*\)", code):
+            bad.append((os.path.basename(path), m.group(0)))
+    assert not bad, bad

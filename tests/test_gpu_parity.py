@@ -906,7 +906,22 @@ def test_errors(gbe):
     with pytest.raises(gbe.GbeError) as e:
         gbe.gbe_build_graph(gbe.DeviceCSR.from_host(gi.CSR.from_dense(np.zeros((4, 4)), keep_zeros=True)), 1e-5, None, 2)
     assert e.value.status == -3  # eps_max == eps_min
+    # an H that is symmetric only to rounding (one entry off by one ulp) is refused by check_symmetry: with the default
+    # power 2 only the upper triangle of floor(A A)_tau is formed, which is the whole product only for a bitwise symmetric A
+    a = s.H.to_dense()
+    a[3, 2] = np.nextafter(a[3, 2], 0.0)
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_build_graph(gbe.DeviceCSR.from_host(gi.CSR.from_dense(a)), 1e-5, None, 4, check_symmetry=True)
+    assert e.value.status == -2
     g = gbe.gbe_build_graph(Hd, 1e-5, None, 4, check_symmetry=True)
+    # a degenerate H (a multiple of I) given to gbe_density: reported through the log, D stays finite without one
+    Hdeg = gbe.DeviceCSR.from_host(gi.CSR.from_dense(np.eye(64) * 0.25))
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_density(Hdeg, g, 32.0, 5)
+    assert e.value.status == -3
+    Ddeg, _ = gbe.gbe_density(Hdeg, g, 32.0, 5, want_log=False)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(Ddeg).all())
     with pytest.raises(gbe.GbeError) as e:
         gbe.gbe_density(Hd, g, 32.0, 10, workspace=torch.empty(256, dtype=torch.uint8, device="cuda"))
     assert e.value.status == -5
