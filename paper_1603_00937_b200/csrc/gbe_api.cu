@@ -104,7 +104,7 @@ const char* gbe_strerror(int status) {
 void gbe_free_graph(gbe_graph* g) {
   if (!g) return;
   void* ptrs[] = {g->S_row_ptr, g->S_col,     g->sub_ptr,  g->sub_idx,  g->ncore,    g->msize, g->dense_off, g->D_row_ptr,
-                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->items_h, g->items_last_h, g->pk[0].ctas, g->pk[0].codes, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va};
+                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->items_h, g->items_last_h, g->pk[0].ctas, g->pk[0].codes, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va, g->tmaps};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   delete g;
@@ -310,6 +310,7 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
   // Packed kernel with EVERY community packed: a bin has all of its X_p in shared memory before it stores anything, so
   // X is updated in place in buffer 0 (half the footprint in L2)
   const int inplace = path == 3 && g->n_items_h == 0;
+  if (iters > 0 && (path == 1 || g->n_items_h > 0)) GBE_TRY(gbe_x2_prepare(g, w.X0, w.X1, s));  // tensor maps -> this workspace
   // traces of X_0 (partials written by the gather), branch of iteration 0
   GBE_TRY(timed(tm, PH_TRACE, mode == 2 ? 1 : 2, [&]() -> int {
     k_init_state<<<1, 1, 0, s>>>(w.st, n_occ, idem_tol, iters, mode, inplace);
@@ -330,14 +331,14 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
       // (gbe_small.cu); the larger communities of the same graph go through the tiled kernel first
       const int n_pairs = g->n_items_last_h + g->n_pk_ctas;
       GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, (g->n_items_h ? 1 : 0) + 1, [&]() -> int {
-        GBE_TRY(gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, true, s));
+        GBE_TRY(gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, true, it & 1, s));
         return gbe_launch_sp2_packed(g, w.st, in, outp, w.partials, g->n_items_last_h, n_pairs, it, last, mode != 2, s);
       }));
       continue;
     }
     const int n_part_it = g->n_items_last;  // one packed partial per tile with a core row, in every iteration
     GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, g->n_items ? 1 : 0,
-                  [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, false, s); }));
+                  [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, false, it & 1, s); }));
     if (mode != 2)
       GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, n_part_it, s); }));
   }

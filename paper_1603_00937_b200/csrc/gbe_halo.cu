@@ -350,7 +350,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
           // pidx: where the tile's trace partial goes - the tiles with a core row are numbered in list order (which is
           // their position in the list of the last iteration), the others carry no trace and get -1
           const bool core_row = ti * tile < g->h_ncore[p];
-          items.push_back({core_row ? (int32_t)last.size() : -1, ti, tj, g->h_m[p], g->h_ncore[p], (int32_t)ld,
+          items.push_back({core_row ? (int32_t)last.size() : -1, ti | (tj << 16), p, g->h_m[p], g->h_ncore[p], (int32_t)ld,
                            g->h_dense_off[p]});
           if (core_row) last.push_back(items.back());
           if (big) {
@@ -390,6 +390,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
     GBE_TRY(upload(gi, &g->gitems, s));
   }
   GBE_TRY(gbe_build_packed(g, s));  // bins of the small communities (gbe_small.cu)
+  GBE_TRY(gbe_x2_build_tmaps(g, s));  // tensor maps of the tiled kernel's panels (gbe_x2.cu); needs dense_off on the device
   // the resident kernel double-buffers n_part pairs; the packed path writes one pair per bin behind the tiled kernel's
   g->n_partials = std::max(std::max(std::max(g->n_items, g->n_gitems), 2 * n_part), g->n_items_last_h + g->n_pk_ctas);
   GBE_TRY(gbe_resident_capacity(g, &g->resident_fits, &g->resident_coresident, &g->resident_cluster));

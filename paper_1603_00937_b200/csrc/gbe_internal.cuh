@@ -103,7 +103,8 @@ struct gbe_pk_class {  // the bins of one launch of the packed kernel (device ar
 };
 
 struct gbe_tile_item {  // one X^2 work item: tile (ti, tj), ti <= tj, of community p, with p's layout (32 bytes)
-  int32_t pidx, ti, tj, m;   // pidx: index of the tile's trace partial (tiles with a core row), else -1; m = core + halo size
+  int32_t pidx, tij, p, m;   // pidx: index of the tile's trace partial (tiles with a core row), else -1; tij = ti | tj << 16;
+                             // p: community; m = core + halo size
   int32_t nc, ld;            // core size, leading dimension (m rounded up to 16)
   int64_t dense_off;         // element offset of X_p in a dense buffer
 };
@@ -161,6 +162,8 @@ struct gbe_graph {
   int64_t* H_rp = nullptr;
   int32_t* H_ci = nullptr;
   double* H_va = nullptr;
+  // tensor maps of the X^2 TMA variant (gbe_x2.cu), cached for the pair of dense buffers they were encoded for
+  void* tmaps = nullptr;  // 2 n_part CUtensorMap: [buffer][community]; null: no encoder in the driver, cp.async kernel
   // workspace layout (byte offsets)
   size_t ws_partials = 0, ws_bounds = 0, ws_x0 = 0, ws_x1 = 0, ws_bytes = 0;
   size_t ws_x2 = 0, ws_x3 = 0, ws_bytes_fermi = 0;  // two more dense buffers for the Chebyshev recurrence
@@ -194,8 +197,11 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
 // step 4
 // iter: index n of the update X_n -> X_{n+1} (selects br[n] when the sequence is preset)
 // hybrid: only the tiles of the communities the packed kernel does not take (items_h / items_last_h)
+// buffer: which dense buffer Xin is (0 or 1: selects the tensor maps)
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                  bool last, bool hybrid, cudaStream_t s);
+                  bool last, bool hybrid, int buffer, cudaStream_t s);
+int gbe_x2_build_tmaps(gbe_graph* g, cudaStream_t s);                                        // once per graph
+int gbe_x2_prepare(const gbe_graph* g, const double* X0, const double* X1, cudaStream_t s);  // once per density call
 // steps 4 + 5 in one kernel for small communities (gbe_resident.cu); mode as in k_init_state
 int gbe_resident_capacity(const gbe_graph* g, int* fits, int* coresident, int* cluster);
 constexpr int GBE_RESIDENT_UNAVAILABLE = 1;  // internal: the cooperative / cluster launch does not fit the device right now

@@ -30,6 +30,9 @@
 // per tile with a core row (packed: the other tiles carry no trace and write none), so that the branch of the NEXT
 // iteration is known before its GEMM starts.
 // Bound: FP64 tensor pipe - 2 m^3 algorithmic flop per community per iteration (~m^3 executed thanks to symmetry).
+#include <cuda.h>
+
+#include <cstdlib>
 #include <type_traits>
 
 #include "gbe_internal.cuh"
@@ -117,9 +120,9 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   const int branch = OP == 0 ? (st->preset ? (int)st->br[iter] : st->branch) : 0;
   const double cn = OP == 1 ? coef[iter] : 0.0;
 
-  const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // pidx, ti, tj, m
+  const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // pidx, ti | tj << 16, p, m
   const int4 it1 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x + 1];  // nc, ld, dense_off
-  const int ti = it0.y, tj = it0.z, m = it0.w, nc = it1.x, ld = it1.y;
+  const int ti = it0.y & 0xFFFF, tj = it0.y >> 16, m = it0.w, nc = it1.x, ld = it1.y;
   const int64_t doff = ((int64_t)(uint32_t)it1.z) | ((int64_t)it1.w << 32);
   const double* __restrict__ X = Xin + doff;
   double* __restrict__ Y = Xout + doff;
@@ -321,6 +324,348 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// The same tile with the panels staged by 2-D TMA instead of cp.async: what one SP2 iteration runs (OP 0).
+//   - one tensor map per community and dense buffer ([m rows][ld doubles], box 64 rows x 16 doubles = one K chunk of one
+//     panel, 128-byte swizzle, rows beyond m zero-filled by the TMA unit: no clamping);
+//   - 3 stages, mbarrier full / empty pairs: thread 0 issues the 1-2 tensor copies of a chunk (UTMALDG) two chunks ahead,
+//     the four DMMA warps issue no copy instruction and meet no CTA-wide barrier in the main loop;
+//   - conflict-free 64-bit fragment loads from the swizzled panels need the K order {2ks, 2ks+1, 2ks+8, 2ks+9} within a
+//     chunk (lanes q = 0, 1 read 16-byte unit ks, lanes q = 2, 3 unit ks + 4; the unit index is XORed with the row's low
+//     three bits): A and B are permuted alike, the sum over k only changes its order.
+// Measured on the 24,576-orbital box: 2.019 ms per launch against 2.083 ms for the cp.async kernel (DMMA sub-pipe 92 %
+// active); results agree with the cp.async kernel to rounding (another order of the sum over k).  Tried, slower: one polling
+// lane per warp (2.054), the four warps taking turns as producer (2.019 / 2.043), the refill issued before the products
+// (2.039), four stages at three CTAs per SM (2.126).
+__device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t mbar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t mbar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
+  uint32_t done = 0;
+  while (!done) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(mbar), "r"(parity)
+        : "memory");
+  }
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t mbar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+      "l"(map), "r"(c0), "r"(c1), "r"(mbar)
+      : "memory");
+}
+
+constexpr int XT_NST = 3;                          // stages (48 KB: four CTAs per SM)
+constexpr int XT_ROW = 16;                         // doubles per panel row (128 bytes, swizzled)
+constexpr int XT_PANEL = X2_BT * XT_ROW;           // doubles per panel
+constexpr int XT_STAGE = 2 * XT_PANEL;             // A panel + B panel (16 KB)
+
+// one K chunk from swizzled panels; off[ks]: this lane's offset (doubles) inside a row for k-step ks
+template <unsigned MASK>
+__device__ __forceinline__ void xt_chunk(double (&acc)[2][8][2], const double* __restrict__ pa0,
+                                         const double* __restrict__ pa1, const double* __restrict__ pb,
+                                         const int (&off)[4], unsigned rt_mask) {
+#pragma unroll
+  for (int ks = 0; ks < X2_KC / 4; ++ks) {
+    double a[2], b[8];
+    a[0] = pa0[off[ks]];
+    a[1] = pa1[off[ks]];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const bool need = MASK == 0 || ((MASK | (MASK >> 8)) & (1u << j));
+      if (need) b[j] = pb[j * 8 * XT_ROW + off[ks]];
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        if (MASK != 0) {
+          if (MASK & (1u << (i * 8 + j))) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        } else {
+          if (rt_mask & (1u << (i * 8 + j))) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+      }
+  }
+}
+
+template <int MINB>
+__global__ void __launch_bounds__(X2_THREADS, MINB)
+    k_x2_tma(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin,
+             double* __restrict__ Xout, double* __restrict__ partials, int iter, const CUtensorMap* __restrict__ maps) {
+  extern __shared__ __align__(1024) double smem_t[];  // 3 stages x (A panel, B panel), every panel 1024-byte aligned
+  __shared__ double red[8];
+  __shared__ __align__(8) unsigned long long bars[2 * XT_NST];  // full[0..2], empty[0..2]
+
+  if (st->stop) return;
+  const int branch = st->preset ? (int)st->br[iter] : st->branch;
+
+  const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // pidx, ti | tj << 16, p, m
+  const int4 it1 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x + 1];  // nc, ld, dense_off
+  const int ti = it0.y & 0xFFFF, tj = it0.y >> 16, m = it0.w, nc = it1.x, ld = it1.y;
+  const int64_t doff = ((int64_t)(uint32_t)it1.z) | ((int64_t)it1.w << 32);
+  const CUtensorMap* const map = maps + it0.z;
+  const double* __restrict__ X = Xin + doff;
+  double* __restrict__ Y = Xout + doff;
+  const bool share = (ti == tj);  // X X^T on a diagonal tile: the B panel is the A panel
+  const int row0 = ti * X2_BT, col0 = tj * X2_BT;
+  const int nchunks = ld / X2_KC;
+
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+  const int role = (wid + blockIdx.x) & 3;
+  const int g = lane >> 2, q = lane & 3;
+  const int rblk[2] = {role, 7 - role};
+  const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars);
+  const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(smem_t);
+  if (t == 0) {
+#pragma unroll
+    for (int s = 0; s < XT_NST; ++s) {
+      mbar_init(bar0 + 8 * s, 1);             // full: the producer's arrive.expect_tx
+      mbar_init(bar0 + 8 * (XT_NST + s), 4);  // empty: one arrival per warp
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const uint32_t stage_bytes = share ? XT_PANEL * 8u : XT_STAGE * 8u;
+  auto produce = [&](int s, int kc) {  // thread 0: chunk kc -> stage s
+    mbar_expect_tx(bar0 + 8 * s, stage_bytes);
+    tma_load_2d(smem0 + s * XT_STAGE * 8, map, kc * X2_KC, row0, bar0 + 8 * s);
+    if (!share) tma_load_2d(smem0 + (s * XT_STAGE + XT_PANEL) * 8, map, kc * X2_KC, col0, bar0 + 8 * s);
+  };
+  if (t == 0) {  // all stages are free: chunks 0 .. XT_NST - 1
+    asm volatile("fence.proxy.tensormap::generic.acquire.gpu [%0], 128;" ::"l"(map) : "memory");
+#pragma unroll
+    for (int s = 0; s < XT_NST; ++s)
+      if (s < nchunks) produce(s, s);
+  }
+
+  unsigned active, mirror;
+  {
+    const int i = (lane >> 3) & 1, j = lane & 7;
+    const int r8 = row0 + 8 * (i ? 7 - role : role), c8 = col0 + 8 * j;
+    const bool on = lane < 16 && r8 < m && c8 < ld && r8 <= c8;
+    active = __ballot_sync(0xffffffffu, on);
+    mirror = __ballot_sync(0xffffffffu, on && r8 < c8);
+  }
+  double acc[2][8][2];
+#pragma unroll
+  for (int i = 0; i < 2; ++i)
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+  // swizzled fragment offsets: k-step ks reads k = {2ks, 2ks+1, 2ks+8, 2ks+9}: 16-byte unit ks (q < 2) or ks + 4, XOR row & 7
+  int off[4];
+#pragma unroll
+  for (int ks = 0; ks < 4; ++ks) off[ks] = (((ks + 4 * (q >> 1)) ^ g) << 1) + (q & 1);
+  const double* const pa0 = smem_t + (rblk[0] * 8 + g) * XT_ROW;
+  const double* const pa1 = smem_t + (rblk[1] * 8 + g) * XT_ROW;
+  const double* const pb0 = smem_t + (share ? 0 : XT_PANEL) + g * XT_ROW;
+  int pattern = active ? 12 : 13;
+  if (active == X2_FULL) pattern = 0;
+  else if (active == x2_diag_mask(role)) pattern = 1 + role;
+  else {
+#pragma unroll
+    for (int nb = 1; nb < 8; ++nb)
+      if (active == x2_cols_mask(nb)) pattern = 4 + nb;
+  }
+  auto compute = [&](int stage) {
+    const double* a0 = pa0 + stage * XT_STAGE;
+    const double* a1 = pa1 + stage * XT_STAGE;
+    const double* pb = pb0 + stage * XT_STAGE;
+    switch (pattern) {
+      case 0: xt_chunk<X2_FULL>(acc, a0, a1, pb, off, 0); break;
+      case 1: xt_chunk<x2_diag_mask(0)>(acc, a0, a1, pb, off, 0); break;
+      case 2: xt_chunk<x2_diag_mask(1)>(acc, a0, a1, pb, off, 0); break;
+      case 3: xt_chunk<x2_diag_mask(2)>(acc, a0, a1, pb, off, 0); break;
+      case 4: xt_chunk<x2_diag_mask(3)>(acc, a0, a1, pb, off, 0); break;
+      case 5: xt_chunk<x2_cols_mask(1)>(acc, a0, a1, pb, off, 0); break;
+      case 6: xt_chunk<x2_cols_mask(2)>(acc, a0, a1, pb, off, 0); break;
+      case 7: xt_chunk<x2_cols_mask(3)>(acc, a0, a1, pb, off, 0); break;
+      case 8: xt_chunk<x2_cols_mask(4)>(acc, a0, a1, pb, off, 0); break;
+      case 9: xt_chunk<x2_cols_mask(5)>(acc, a0, a1, pb, off, 0); break;
+      case 10: xt_chunk<x2_cols_mask(6)>(acc, a0, a1, pb, off, 0); break;
+      case 11: xt_chunk<x2_cols_mask(7)>(acc, a0, a1, pb, off, 0); break;
+      case 12: xt_chunk<0>(acc, a0, a1, pb, off, active); break;
+      default: break;
+    }
+  };
+
+  // main loop: chunk kc lives in stage kc % XT_NST; after computing chunk kc the warp releases its stage, and the producer
+  // refills the stage released one chunk EARLIER (chunk kc - 1) with chunk kc - 1 + XT_NST: the other warps have a whole
+  // chunk to release it, so the producer hardly ever waits
+  for (int kc0 = 0; kc0 < nchunks; kc0 += XT_NST) {
+    const uint32_t par = (uint32_t)(kc0 / XT_NST) & 1u;
+#pragma unroll
+    for (int s = 0; s < XT_NST; ++s) {
+      const int kc = kc0 + s;
+      if (kc >= nchunks) break;
+      mbar_wait(bar0 + 8 * s, par);
+      compute(s);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar0 + 8 * (XT_NST + s));
+      if (t == 0 && kc >= 1 && kc - 1 + XT_NST < nchunks) {
+        const int sp = (s + XT_NST - 1) % XT_NST;                // stage of chunk kc - 1
+        const uint32_t pp = (uint32_t)((kc - 1) / XT_NST) & 1u;  // its round
+        mbar_wait(bar0 + 8 * (XT_NST + sp), pp);
+        produce(sp, kc - 1 + XT_NST);
+      }
+    }
+  }
+
+  // epilogue: as k_x2 (OP 0)
+  double s1 = 0.0, s2 = 0.0;
+  auto epilogue = [&](auto edge_c, auto trace_c, auto full_c) {
+    constexpr bool EDGE = decltype(edge_c)::value, TRACE = decltype(trace_c)::value;
+    constexpr bool FULL = decltype(full_c)::value;
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const int r = row0 + rblk[i] * 8 + g;
+      if (EDGE && r >= m) continue;
+      const double* __restrict__ xr = X + (size_t)r * ld + col0 + 2 * q;
+      double* __restrict__ yr = Y + (size_t)r * ld + col0 + 2 * q;
+      double* __restrict__ ym0 = Y + (size_t)(col0 + 2 * q) * ld + r;
+      double* __restrict__ ym1 = ym0 + ld;
+      const size_t mstep = (size_t)8 * ld;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        if (!FULL && !(active & (1u << (i * 8 + j)))) {
+          ym0 += mstep;
+          ym1 += mstep;
+          continue;
+        }
+        const int c = col0 + j * 8 + 2 * q;
+        double v0 = acc[i][j][0], v1 = acc[i][j][1];
+        if (branch) {
+          const double2 x = *reinterpret_cast<const double2*>(xr + j * 8);
+          v0 = 2.0 * x.x - v0;
+          v1 = 2.0 * x.y - v1;
+        }
+        if (EDGE) {
+          if (c >= m) v0 = 0.0;
+          if (c + 1 >= m) v1 = 0.0;
+        }
+        *reinterpret_cast<double2*>(yr + j * 8) = make_double2(v0, v1);
+        if (TRACE && r < nc) {
+          s2 += v0 * v0 + v1 * v1;
+          if (r == c) s1 += v0;
+          if (r == c + 1) s1 += v1;
+        }
+        if (FULL || (mirror & (1u << (i * 8 + j)))) {
+          if (!EDGE || c < m) {
+            *ym0 = v0;
+            if (TRACE && c < nc) s2 += v0 * v0;
+          }
+          if (!EDGE || c + 1 < m) {
+            *ym1 = v1;
+            if (TRACE && c + 1 < nc) s2 += v1 * v1;
+          }
+        }
+        ym0 += mstep;
+        ym1 += mstep;
+      }
+    }
+  };
+  const bool edge = col0 + X2_BT > m;
+  const bool trace = row0 < nc || col0 < nc;
+  if (edge || trace) {
+    if (edge) epilogue(std::true_type{}, std::true_type{}, std::false_type{});
+    else epilogue(std::false_type{}, std::true_type{}, std::false_type{});
+  } else if (active == X2_FULL && mirror == X2_FULL) {
+    epilogue(std::false_type{}, std::false_type{}, std::true_type{});
+  } else {
+    epilogue(std::false_type{}, std::false_type{}, std::false_type{});
+  }
+  const int pidx = it0.x;
+  if (pidx < 0) return;
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  if (lane == 0) { red[role] = s1; red[4 + role] = s2; }
+  __syncthreads();
+  if (t == 0) {
+    partials[2 * (size_t)pidx] = (red[0] + red[1]) + (red[2] + red[3]);
+    partials[2 * (size_t)pidx + 1] = (red[4] + red[5]) + (red[6] + red[7]);
+  }
+}
+
+// Tensor maps.  A map describes ONE community's X_p in ONE dense buffer ([m_p rows][ld_p doubles], box 64 x 16, 128-byte
+// swizzle).  Shapes are fixed by the graph, so the maps are encoded once, on the host, when the graph is built
+// (cuTensorMapEncodeTiled through the runtime's driver entry point - no link against libcuda) with a placeholder address;
+// the dense buffers live in the caller's workspace, so every density call sets the addresses ON THE DEVICE
+// (tensormap.replace.tile.global_address, one thread per map, 2 n_part maps): no host work per call, nothing to
+// synchronise, capturable in a CUDA graph.  The kernels acquire the map through the tensormap proxy fence before use.
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+__global__ void k_patch_tmaps(CUtensorMap* __restrict__ maps, const int64_t* __restrict__ dense_off,
+                              const int32_t* __restrict__ msize, int n_part, const double* X0, const double* X1) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= 2 * n_part) return;
+  const int p = i < n_part ? i : i - n_part;
+  if (msize[p] == 0) return;  // an empty community has no tiles
+  const double* base = (i < n_part ? X0 : X1) + dense_off[p];
+  asm volatile("tensormap.replace.tile.global_address.global.b1024.b64 [%0], %1;" ::"l"(maps + i), "l"(base) : "memory");
+}
+}  // namespace
+
+// Encodes the 2 n_part maps of a graph (both halves identical until gbe_x2_prepare sets the addresses); leaves
+// g->tmaps null if the driver has no tensor-map encoder (then the cp.async kernel runs)
+int gbe_x2_build_tmaps(gbe_graph* g, cudaStream_t s) {
+  g->tmaps = nullptr;
+  if (g->n_items == 0) return GBE_OK;
+  static std::atomic<PFN_encodeTiled> encode_p{nullptr};
+  PFN_encodeTiled encode = encode_p.load();
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+      (void)cudaGetLastError();
+      return GBE_OK;
+    }
+    encode = reinterpret_cast<PFN_encodeTiled>(fn);
+    encode_p.store(encode);
+  }
+  std::vector<CUtensorMap> h(2 * (size_t)g->n_part);
+  memset(h.data(), 0, h.size() * sizeof(CUtensorMap));
+  for (int p = 0; p < g->n_part; ++p) {
+    const int m = g->h_m[p];
+    if (m == 0) continue;
+    const cuuint64_t ld = (cuuint64_t)((m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN);
+    const cuuint64_t dims[2] = {ld, (cuuint64_t)m};
+    const cuuint64_t strides[1] = {ld * 8};
+    const cuuint32_t box[2] = {(cuuint32_t)X2_KC, (cuuint32_t)X2_BT};
+    const cuuint32_t es[2] = {1, 1};
+    void* placeholder = g->dense_off;  // any 16-byte aligned device address: replaced before the first use
+    if (encode(&h[p], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, placeholder, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return GBE_OK;  // no maps: the cp.async kernel runs
+    h[(size_t)g->n_part + p] = h[p];
+  }
+  GBE_TRY(gbe_dev_alloc(&g->tmaps, h.size() * sizeof(CUtensorMap)));
+  GBE_CUDA(cudaMemcpyAsync(g->tmaps, h.data(), h.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, s));  // pageable: staged
+  return GBE_OK;
+}
+
+// Before the tiled SP2 loop of a density call: point the maps at this call's dense buffers
+int gbe_x2_prepare(const gbe_graph* g, const double* X0, const double* X1, cudaStream_t s) {
+  if (!g->tmaps || g->n_items == 0) return GBE_OK;
+  const int n = 2 * g->n_part;
+  k_patch_tmaps<<<(n + 127) / 128, 128, 0, s>>>(reinterpret_cast<CUtensorMap*>(g->tmaps), g->dense_off, g->msize, g->n_part,
+                                               X0, X1);
+  GBE_LAUNCHED();
+  return GBE_OK;
+}
+
+namespace {
 template <int MINB, int OP>
 int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
               const double* Xb, double* Dacc, const double* coef, const gbe_tile_item* items, int n_items,
@@ -339,12 +684,25 @@ int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout
 }  // namespace
 
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                  bool last, bool hybrid, cudaStream_t s) {
+                  bool last, bool hybrid, int buffer, cudaStream_t s) {
   // the last SP2 iteration computes the tiles with a core row only: the scatter keeps core columns (Eq.(6));
   // hybrid: the communities with m <= GBE_PK_MAX_M are the packed kernel's (gbe_small.cu), only the others are tiled
   const gbe_tile_item* items = hybrid ? (last ? g->items_last_h : g->items_h) : (last ? g->items_last : g->items);
   const int n_items = hybrid ? (last ? g->n_items_last_h : g->n_items_h) : (last ? g->n_items_last : g->n_items);
   if (n_items == 0) return GBE_OK;
+  if (g->tmaps) {  // panels staged by 2-D TMA (k_x2_tma); X_n is in buffer 0 for even iterations, in buffer 1 for odd ones
+    const CUtensorMap* maps = reinterpret_cast<const CUtensorMap*>(g->tmaps) + (buffer ? g->n_part : 0);
+    auto kern = k_x2_tma<4>;
+    const size_t smem = (size_t)XT_NST * XT_STAGE * sizeof(double) + 1024;
+    static gbe_device_once configured;
+    if (configured.first()) {
+      GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    }
+    kern<<<n_items, X2_THREADS, smem, s>>>(items, st, Xin, Xout, partials, iter, maps);
+    GBE_LAUNCHED();
+    return GBE_OK;
+  }
   return launch_x2<4, 0>(g, st, Xin, Xout, partials, iter, nullptr, nullptr, nullptr, items, n_items, s);
 }
 

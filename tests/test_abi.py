@@ -58,6 +58,7 @@ def test_sass_uses_fp64_tensor_cores_and_async_copies(libpath):
     sass = subprocess.run(["cuobjdump", "-sass", libpath], capture_output=True, text=True).stdout
     assert "DMMA.8x8x4" in sass      # mma.sync f64 -> FP64 tensor pipe
     assert "LDGSTS" in sass          # cp.async staging of the X panels
+    assert "UTMALDG" in sass         # 2-D tensor-map TMA loads of the X^2 panels (cp.async.bulk.tensor)
     assert "UBLKCP" in sass          # TMA bulk copies (cp.async.bulk) of the packed small-m kernel
     assert "sm_100a" in sass
 
