@@ -629,6 +629,54 @@ def run_fermi(args) -> None:
                       "tflops_alg": info["sp2_flops_per_iter"] * (order - 1) / (t * 1e-3) * 1e-12}), flush=True)
 
 
+def run_waves(args) -> None:
+    """SURVEY 8(f) item 1 in a bounded workspace: gbe_density_preset without traces on the whole batch against the same call
+    in a workspace of --waves-gb GB (waves of communities: no exchange between the expansions).  One JSON line."""
+    import torch
+    from paper_1603_00937_b200 import build as gbe_build
+    gbe_build.build()
+    import paper_1603_00937_b200 as gbe
+    s = make_system(args.workload, 0)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    part_t = None if s.meta.get("kind") == "water" else torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
+    g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
+    gbe.gbe_graph_set_sp2_path(g, 1)
+    info = g.info
+    D_full = torch.empty(info["nnz_D"], dtype=torch.float64, device="cuda")
+    D_wave = torch.empty_like(D_full)
+    ws = g.new_workspace()
+    _, log = gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws, D_val=D_full)  # the sequence of this system
+    seq = log.branch
+
+    def timed(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    reps = max(1, args.steps)
+    t_full = timed(lambda: gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False, workspace=ws, D_val=D_full,
+                                                  want_log=False), reps)
+    del ws
+    torch.cuda.empty_cache()
+    nbytes = max(int(args.waves_gb * 1e9) // 256 * 256, int(info["workspace_bytes_preset_min"]))
+    wsb = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    t_wave = timed(lambda: gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False, workspace=wsb, D_val=D_wave,
+                                                  want_log=False), reps)
+    cap = (nbytes - (info["workspace_bytes"] - 2 * ((info["dense_elems"] * 8 + 255) // 256 * 256))) // 2
+    print(json.dumps({"waves": args.workload, "n": s.n, "n_part": s.n_part, "iters": int(len(seq)),
+                      "workspace_full_gb": info["workspace_bytes"] * 1e-9, "workspace_bounded_gb": nbytes * 1e-9,
+                      "workspace_min_gb": info["workspace_bytes_preset_min"] * 1e-9,
+                      "waves_estimate": int(-(-info["dense_elems"] * 8 // max(1, cap))),
+                      "ms_full": t_full, "ms_bounded": t_wave, "ratio": t_wave / t_full,
+                      "bit_identical": bool(torch.equal(D_full, D_wave))}), flush=True)
+
+
 def run_small(args) -> None:
     """Small systems (BASELINE.json configs[0] and relatives): the tiled kernels against the shared-memory-resident SP2
     kernel, one JSON line per (system, path): gbe_density eagerly, as a CUDA-graph replay, and gbe_density_preset
@@ -708,6 +756,8 @@ def main() -> None:
     ap.add_argument("--no-exact", action="store_true", help="sweep without the exact projector (no error columns)")
     ap.add_argument("--sweep-taus", default="", help="comma-separated thresholds of the sweep (default: the five of configs[4])")
     ap.add_argument("--sp2-path", type=int, default=0, help="sweep: force the SP2 kernels (1 tiled, 2 resident, 3 packed; 0 = the library's choice)")
+    ap.add_argument("--waves", action="store_true", help="gbe_density_preset on the whole batch against the same call in a bounded workspace")
+    ap.add_argument("--waves-gb", type=float, default=8.0, help="--waves: size of the bounded workspace in GB")
     ap.add_argument("--record-traffic", default="", help="ncu raw-page CSV of a --set full capture of k_x2: write profiles/x2_traffic.json")
     ap.add_argument("--traffic-source", default="", help="the profiles/ summary that documents the capture")
     args = ap.parse_args()
@@ -717,6 +767,8 @@ def main() -> None:
         run_sweep(args)
     elif args.small:
         run_small(args)
+    elif args.waves:
+        run_waves(args)
     elif args.fermi:
         run_fermi(args)
     elif args.impl == "reference":

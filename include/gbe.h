@@ -108,6 +108,8 @@ typedef struct {
                                     P:L65) - the numerator of bench.py's roofline fraction */
   int64_t n_small;           /* communities with 0 < m_p <= 112 (gbe_set_packed_max_m): the ones the packed kernel takes */
   int64_t n_bins;            /* CTAs of one packed launch (bins of 1..16 small communities) */
+  size_t workspace_bytes_preset_min; /* smallest workspace gbe_density_preset(trace_every_iteration = 0) accepts: it then
+                                        works through the communities in waves (see there) */
 } gbe_graph_info;
 
 /* SP2 log (host memory, caller-allocated; valid after the stream has been synchronised).
@@ -254,6 +256,11 @@ int gbe_density_timed(const gbe_csr_view* H, const gbe_graph* g, double n_occ, i
  *                         == 0: no per-iteration reduction kernel at all ("without exchange of information during or
  *                               between the matrix multiplications"); the log then holds only t1, t2 of the
  *                               final X at index `iters` (earlier entries are unspecified) and the given branches.
+ * Bounded workspace.  With trace_every_iteration == 0 nothing couples the communities, so the call also accepts a
+ * workspace SMALLER than info.workspace_bytes, down to info.workspace_bytes_preset_min (room for the largest community):
+ * it then gathers, expands and scatters the communities in waves that fit the workspace given - the same kernels on the
+ * same tiles, D bit for bit the same; the memory of the dense batch no longer grows with the system (config 4 of
+ * BASELINE.json: 2 x 20 GB at once, or waves in a few GB).
  * Other arguments, stream semantics and D_val as gbe_density. */
 int gbe_density_preset(const gbe_csr_view* H, const gbe_graph* g, const uint8_t* branch, int32_t iters,
                        int32_t trace_every_iteration, void* workspace, size_t workspace_bytes, void* cuda_stream,

@@ -104,7 +104,7 @@ const char* gbe_strerror(int status) {
 void gbe_free_graph(gbe_graph* g) {
   if (!g) return;
   void* ptrs[] = {g->S_row_ptr, g->S_col,     g->sub_ptr,  g->sub_idx,  g->ncore,    g->msize, g->dense_off, g->D_row_ptr,
-                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->items_h, g->items_last_h, g->pk[0].ctas, g->pk[0].codes, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va, g->tmaps};
+                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->items_h, g->items_last_h, g->pk[0].ctas, g->pk[0].codes, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va, g->tmaps, g->items_w, g->items_last_w};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   delete g;
@@ -203,6 +203,7 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   o->sp2_path_chosen = choose_sp2(g, 0);
   o->n_small = g->pk_n_small;
   o->n_bins = g->n_pk_ctas;
+  o->workspace_bytes_preset_min = g->ws_bytes_wave_min;
   o->resident_fits = g->resident_fits;
   o->resident_cluster = g->resident_cluster;
   return GBE_OK;
@@ -366,10 +367,18 @@ int gbe_scatter(const gbe_graph* g, void* workspace, size_t workspace_bytes, voi
   return do_scatter(g, workspace, workspace_bytes, cuda_stream, D_val, nullptr);
 }
 
+static int read_log_at(const gbe_graph* g, const void* workspace, void* cuda_stream, gbe_sp2_log* log);
 int gbe_read_log(const gbe_graph* g, const void* workspace, size_t workspace_bytes, void* cuda_stream, gbe_sp2_log* log) {
   if (!g || !log) return GBE_EINVAL;
   WS w;
   GBE_TRY(carve(g, const_cast<void*>(workspace), workspace_bytes, &w));
+  return read_log_at(g, workspace, cuda_stream, log);
+}
+// the state sits at the start of the workspace whatever its size
+static int read_log_at(const gbe_graph* g, const void* workspace, void* cuda_stream, gbe_sp2_log* log) {
+  (void)g;
+  WS w;
+  w.st = reinterpret_cast<gbe_state*>(const_cast<void*>(workspace));
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   gbe_state hs_small;  // only the header is needed first
   GBE_CUDA(cudaMemcpyAsync(&hs_small, w.st, offsetof(gbe_state, t1), cudaMemcpyDeviceToHost, s));
@@ -424,6 +433,44 @@ int gbe_density_timed(const gbe_csr_view* H, const gbe_graph* g, double n_occ, i
   return GBE_OK;
 }
 
+// gbe_density_preset without traces in a workspace that holds only part of the batch: waves of communities (gbe_plan_waves)
+static int density_preset_waves(const gbe_csr_view* H, const gbe_graph* g, const uint8_t* branch, int32_t iters,
+                                void* workspace, size_t workspace_bytes, void* cuda_stream, double* D_val) {
+  GBE_TRY(check_csr(H));
+  if (H->n != g->n) return GBE_EMISMATCH;
+  if (reinterpret_cast<uintptr_t>(workspace) % 256) return GBE_EINVAL;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  unsigned char* b = static_cast<unsigned char*>(workspace);
+  gbe_state* st = reinterpret_cast<gbe_state*>(b);
+  double* blo = reinterpret_cast<double*>(b + g->ws_bounds);
+  double* partials = reinterpret_cast<double*>(b + g->ws_partials);
+  const size_t cap_elems = ((workspace_bytes - g->ws_x0) / 2 / 256 * 256) / 8;  // doubles per dense buffer of a wave
+  double* const B0 = reinterpret_cast<double*>(b + g->ws_x0);
+  double* const B1 = B0 + cap_elems;
+  GBE_TRY(gbe_plan_waves(g, cap_elems, s));
+  GBE_TRY(gbe_launch_bounds(*H, blo, blo + 1024, 1024, st, s));
+  k_init_state<<<1, 1, 0, s>>>(st, 0.0, -1.0, iters, 2, 0);
+  GBE_LAUNCHED();
+  if (iters > 0) GBE_CUDA(cudaMemcpyAsync(st->br, branch, (size_t)iters, cudaMemcpyHostToDevice, s));
+  for (const gbe_wave& w : g->waves) {
+    // the wave's buffers are the full-size ones shifted by its first offset: every kernel keeps its absolute offsets
+    double* const X0 = B0 - w.base_elems;
+    double* const X1 = B1 - w.base_elems;
+    if (iters > 0) GBE_TRY(gbe_x2_prepare(g, X0, X1, s));
+    // (the traces of X_0 the gather leaves are only wanted for iters == 0: else they go behind the slots of the tiles)
+    GBE_TRY(gbe_launch_gather(*H, g, st, X0, iters > 0 ? partials + 2 * (size_t)g->n_items_last : partials, s, w.gi0, w.gi_n));
+    for (int it = 0; it < iters; ++it) {
+      const bool last = it == iters - 1;
+      GBE_TRY(gbe_launch_x2_items(g, st, (it & 1) ? X1 : X0, (it & 1) ? X0 : X1, partials, it,
+                                  (last ? g->items_last_w + w.last_first : g->items_w + w.it_first),
+                                  last ? w.last_n : w.it_n, it & 1, s));
+    }
+    GBE_TRY(gbe_launch_scatter(g, st, X0, X1, D_val, s, w.row0, w.n_rows));
+  }
+  // t1, t2 of the final X for the log (index iters): every wave left its pairs in the whole-batch slots
+  return gbe_launch_trace_branch(st, partials, iters > 0 ? g->n_items_last : g->n_gitems, s);
+}
+
 int gbe_density_preset(const gbe_csr_view* H, const gbe_graph* g, const uint8_t* branch, int32_t iters,
                        int32_t trace_every_iteration, void* workspace, size_t workspace_bytes, void* cuda_stream,
                        double* D_val, gbe_sp2_log* log) {
@@ -432,6 +479,11 @@ int gbe_density_preset(const gbe_csr_view* H, const gbe_graph* g, const uint8_t*
   for (int k = 0; k < iters; ++k)
     if (branch[k] > 1) return GBE_EINVAL;
   static const uint8_t none = 0;
+  if (!trace_every_iteration && workspace && workspace_bytes < g->ws_bytes && workspace_bytes >= g->ws_bytes_wave_min) {
+    GBE_TRY(density_preset_waves(H, g, iters > 0 ? branch : &none, iters, workspace, workspace_bytes, cuda_stream, D_val));
+    if (log) GBE_TRY(read_log_at(g, workspace, cuda_stream, log));
+    return GBE_OK;
+  }
   GBE_TRY(do_gather(H, g, workspace, workspace_bytes, cuda_stream, nullptr));
   GBE_TRY(do_sp2(g, 0.0, iters, -1.0, workspace, workspace_bytes, cuda_stream, nullptr, iters > 0 ? branch : &none,
                  trace_every_iteration != 0));

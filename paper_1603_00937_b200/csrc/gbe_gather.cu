@@ -215,9 +215,14 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
 
 }  // namespace
 
+// item0, n_it: a sub-range of the work items (one wave of communities, gbe_density_preset in a bounded workspace);
+// n_it < 0: all of them
 int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state* st, double* X, double* partials,
-                      cudaStream_t s) {
-  if (g->n_gitems == 0) return GBE_OK;
+                      cudaStream_t s, int item0, int n_it) {
+  if (n_it < 0) { item0 = 0; n_it = g->n_gitems; }
+  if (n_it == 0) return GBE_OK;
+  const int2* const gitems = g->gitems + item0;
+  partials += 2 * (size_t)item0;
   const int W = (int)((g->n + 31) / 32);
   const int ldmax = (g->max_m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
   const size_t fixed = (size_t)4 * W * 4 + 516 * 4 + 16 * 8;
@@ -231,14 +236,14 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
   if (direct) {
     GBE_CUDA(cudaFuncSetAttribute(k_gather<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fixed));
     GBE_CUDA(cudaFuncSetAttribute(k_gather<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-    k_gather<true><<<g->n_gitems, 256, fixed, s>>>(W, ldmax, g->gather_rows, g->gitems, H.row_ptr, H.col_idx, H.val, g->n,
+    k_gather<true><<<n_it, 256, fixed, s>>>(W, ldmax, g->gather_rows, gitems, H.row_ptr, H.col_idx, H.val, g->n,
                                                    g->sub_ptr, g->sub_idx, g->ncore, g->dense_off, st, X, partials);
   } else {
     const int nw = (int)std::min<size_t>(8, (budget - fixed) / ((size_t)ldmax * 8));
     const size_t smem = fixed + (size_t)nw * ldmax * 8;
     GBE_CUDA(cudaFuncSetAttribute(k_gather<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     GBE_CUDA(cudaFuncSetAttribute(k_gather<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-    k_gather<false><<<g->n_gitems, nw * 32, smem, s>>>(W, ldmax, g->gather_rows, g->gitems, H.row_ptr, H.col_idx, H.val,
+    k_gather<false><<<n_it, nw * 32, smem, s>>>(W, ldmax, g->gather_rows, gitems, H.row_ptr, H.col_idx, H.val,
                                                        g->n, g->sub_ptr, g->sub_idx, g->ncore, g->dense_off, st, X, partials);
   }
   GBE_LAUNCHED();

@@ -393,6 +393,8 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
   GBE_TRY(gbe_x2_build_tmaps(g, s));  // tensor maps of the tiled kernel's panels (gbe_x2.cu); needs dense_off on the device
   // the resident kernel double-buffers n_part pairs; the packed path writes one pair per bin behind the tiled kernel's
   g->n_partials = std::max(std::max(std::max(g->n_items, g->n_gitems), 2 * n_part), g->n_items_last_h + g->n_pk_ctas);
+  // wave mode (gbe_plan_waves): the gather of a later wave must not touch the final pairs of an earlier one
+  g->n_partials = std::max(g->n_partials, g->n_items_last + g->n_gitems);
   GBE_TRY(gbe_resident_capacity(g, &g->resident_fits, &g->resident_coresident, &g->resident_cluster));
 
   // workspace layout
@@ -406,6 +408,11 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
   g->ws_x1 = off;
   off += align_up((size_t)g->dense_elems * 8, 256);
   g->ws_bytes = off;
+  {  // smallest workspace of gbe_density_preset without traces: two buffers that hold the largest community
+    int64_t big = 0;
+    for (int p = 0; p < n_part; ++p) big = std::max<int64_t>(big, g->h_dense_off[p + 1] - g->h_dense_off[p]);
+    g->ws_bytes_wave_min = g->ws_x0 + 2 * align_up((size_t)big * 8, 256);
+  }
   g->ws_x2 = off;
   off += align_up((size_t)g->dense_elems * 8, 256);
   g->ws_x3 = off;
@@ -469,5 +476,87 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
     GBE_CUDA(cudaStreamSynchronize(s));
     g->scat_ofs = reinterpret_cast<int64_t*>(scat_ofs.release());
   }
+  return GBE_OK;
+}
+
+// ----------------------------------------------------------------------------------------------------------------------
+// Waves of communities for a pre-determined SP2 sequence in a BOUNDED workspace (with the sequence fixed beforehand
+// every expansion runs "without exchange of information during or between the matrix multiplications", so nothing couples
+// the communities and gather -> SP2 loop -> scatter can be done for a few of them at a time).  A wave is a range of
+// consecutive communities [p0, p1): contiguous in the dense layout (its buffers are the full-size ones shifted by the
+// wave's first offset), in the gather work list and in the dense rows the scatter walks; only the X^2 tile lists, which
+// are ordered by size, are re-cut per wave (same order and same trace slots as the whole-batch lists).
+// cap_elems: doubles ONE dense buffer of a wave may hold.  The plan is cached in the graph for the cap it was made for.
+int gbe_plan_waves(const gbe_graph* g, size_t cap_elems, cudaStream_t s) {
+  if (g->waves_cap == cap_elems && !g->waves.empty()) return GBE_OK;
+  const int n_part = g->n_part;
+  std::vector<gbe_wave> waves;
+  std::vector<int32_t> wave_of(n_part, 0);
+  {
+    gbe_wave w = {};
+    int64_t row = 0;
+    int gi = 0;
+    w.base_elems = 0;
+    for (int p = 0; p < n_part; ++p) {
+      const int64_t m = g->h_m[p];
+      const int64_t e = g->h_dense_off[p + 1] - g->h_dense_off[p];
+      if ((size_t)e > cap_elems) return GBE_ENOMEM;
+      if (w.p1 > w.p0 && (size_t)(w.elems + e) > cap_elems) {  // close the wave, open the next at p
+        waves.push_back(w);
+        gbe_wave nw = {};
+        nw.p0 = nw.p1 = p;
+        nw.base_elems = g->h_dense_off[p];
+        nw.row0 = row;
+        nw.gi0 = gi;
+        w = nw;
+      }
+      wave_of[p] = (int32_t)waves.size();
+      w.p1 = p + 1;
+      w.elems += e;
+      w.n_rows += m;
+      const int ng = (int)((m + g->gather_rows - 1) / g->gather_rows);
+      w.gi_n += ng;
+      row += m;
+      gi += ng;
+    }
+    waves.push_back(w);
+  }
+  // tile lists: the whole-batch order (communities by decreasing m, stable) and its trace slots, cut by wave
+  std::vector<int32_t> order(n_part);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return g->h_m[a] > g->h_m[b]; });
+  std::vector<std::vector<gbe_tile_item>> it(waves.size()), la(waves.size());
+  const int tile = g->tile;
+  int32_t slot = 0;
+  for (int p : order) {
+    const int T = (g->h_m[p] + tile - 1) / tile;
+    const int64_t ld = (g->h_m[p] + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+    const int wv = wave_of[p];
+    for (int ti = 0; ti < T; ++ti)
+      for (int tj = ti; tj < T; ++tj) {
+        const bool core_row = ti * tile < g->h_ncore[p];
+        const gbe_tile_item item = {core_row ? slot : -1, ti | (tj << 16), p, g->h_m[p], g->h_ncore[p], (int32_t)ld,
+                                    g->h_dense_off[p]};
+        it[wv].push_back(item);
+        if (core_row) { la[wv].push_back(item); ++slot; }
+      }
+  }
+  std::vector<gbe_tile_item> all_it, all_la;
+  for (size_t k = 0; k < waves.size(); ++k) {
+    waves[k].it_first = (int32_t)all_it.size();
+    waves[k].it_n = (int32_t)it[k].size();
+    waves[k].last_first = (int32_t)all_la.size();
+    waves[k].last_n = (int32_t)la[k].size();
+    all_it.insert(all_it.end(), it[k].begin(), it[k].end());
+    all_la.insert(all_la.end(), la[k].begin(), la[k].end());
+  }
+  gbe_set_alloc_stream(s);
+  if (g->items_w) gbe_dev_free(g->items_w);
+  if (g->items_last_w) gbe_dev_free(g->items_last_w);
+  g->items_w = g->items_last_w = nullptr;
+  GBE_TRY(upload(all_it, &g->items_w, s));
+  GBE_TRY(upload(all_la, &g->items_last_w, s));
+  g->waves = std::move(waves);
+  g->waves_cap = cap_elems;
   return GBE_OK;
 }

@@ -109,6 +109,15 @@ struct gbe_tile_item {  // one X^2 work item: tile (ti, tj), ti <= tj, of commun
   int64_t dense_off;         // element offset of X_p in a dense buffer
 };
 
+struct gbe_wave {  // a range of communities processed together by gbe_density_preset in a bounded workspace (gbe_plan_waves)
+  int32_t p0, p1;                  // communities [p0, p1)
+  int32_t it_first, it_n;          // its X^2 tiles in items_w
+  int32_t last_first, last_n;      // its tiles with a core row in items_last_w
+  int32_t gi0, gi_n;               // its gather work items
+  int64_t row0, n_rows;            // its dense rows (scatter)
+  int64_t base_elems, elems;       // first element and size of its part of a full dense buffer
+};
+
 // ----------------------------------------------------------------------------------------------
 // the graph handle
 // ----------------------------------------------------------------------------------------------
@@ -164,6 +173,11 @@ struct gbe_graph {
   double* H_va = nullptr;
   // tensor maps of the X^2 TMA variant (gbe_x2.cu), cached for the pair of dense buffers they were encoded for
   void* tmaps = nullptr;  // 2 n_part CUtensorMap: [buffer][community]; null: no encoder in the driver, cp.async kernel
+  // wave plan of gbe_density_preset in a bounded workspace, cached for the capacity it was made for (not thread safe)
+  mutable std::vector<gbe_wave> waves;
+  mutable size_t waves_cap = 0;
+  mutable gbe_tile_item *items_w = nullptr, *items_last_w = nullptr;
+  size_t ws_bytes_wave_min = 0;  // state + partials + two buffers of the largest community
   // workspace layout (byte offsets)
   size_t ws_partials = 0, ws_bounds = 0, ws_x0 = 0, ws_x1 = 0, ws_bytes = 0;
   size_t ws_x2 = 0, ws_x3 = 0, ws_bytes_fermi = 0;  // two more dense buffers for the Chebyshev recurrence
@@ -193,13 +207,16 @@ int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int3
 int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const double* bounds);
 // step 3
 int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state* st, double* X, double* partials,
-                      cudaStream_t s);
+                      cudaStream_t s, int item0 = 0, int n_it = -1);
 // step 4
 // iter: index n of the update X_n -> X_{n+1} (selects br[n] when the sequence is preset)
 // hybrid: only the tiles of the communities the packed kernel does not take (items_h / items_last_h)
 // buffer: which dense buffer Xin is (0 or 1: selects the tensor maps)
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
                   bool last, bool hybrid, int buffer, cudaStream_t s);
+int gbe_launch_x2_items(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
+                        const gbe_tile_item* items, int n_items, int buffer, cudaStream_t s);
+int gbe_plan_waves(const gbe_graph* g, size_t cap_elems, cudaStream_t s);  // gbe_halo.cu
 int gbe_x2_build_tmaps(gbe_graph* g, cudaStream_t s);                                        // once per graph
 int gbe_x2_prepare(const gbe_graph* g, const double* X0, const double* X1, cudaStream_t s);  // once per density call
 // steps 4 + 5 in one kernel for small communities (gbe_resident.cu); mode as in k_init_state
@@ -216,7 +233,7 @@ int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, 
 int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s);
 // step 6
 int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0, const double* X1, double* D_val,
-                       cudaStream_t s);
+                       cudaStream_t s, int64_t row0 = 0, int64_t n_rows = -1);
 
 // finite-temperature Chebyshev expansion (gbe_fermi.cu; the product of every term is gbe_x2.cu in its second mode)
 int gbe_launch_cheb_coef(gbe_state* st, double mu, double beta, int order, cudaStream_t s);

@@ -81,16 +81,18 @@ __global__ void __launch_bounds__(256, 4) k_scatter(int64_t sum_m, const int64_t
 }
 }  // namespace
 
+// row0, n_rows: a sub-range of the dense rows (one wave of communities); n_rows < 0: all of them
 int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0, const double* X1, double* D_val,
-                       cudaStream_t s) {
-  if (g->sum_m == 0) return GBE_OK;
-  const int64_t want = (g->sum_m + 63) / 64;  // 8 warps x 8 rows per CTA iteration
+                       cudaStream_t s, int64_t row0, int64_t n_rows) {
+  if (n_rows < 0) { row0 = 0; n_rows = g->sum_m; }
+  if (n_rows == 0) return GBE_OK;
+  const int64_t want = (n_rows + 63) / 64;  // 8 warps x 8 rows per CTA iteration
   const int grid = (int)std::min<int64_t>(want, (int64_t)gbe_sm_count() * 64);
   if (g->contiguous)
-    k_scatter<true><<<grid, 256, 0, s>>>(g->sum_m, g->row_src, g->row_nc, g->scat_base, nullptr,
+    k_scatter<true><<<grid, 256, 0, s>>>(n_rows, g->row_src + row0, g->row_nc + row0, g->scat_base + row0, nullptr,
                                          nullptr, st, X0, X1, D_val);
   else
-    k_scatter<false><<<grid, 256, 0, s>>>(g->sum_m, g->row_src, g->row_nc, nullptr, g->scat_ofs,
+    k_scatter<false><<<grid, 256, 0, s>>>(n_rows, g->row_src + row0, g->row_nc + row0, nullptr, g->scat_ofs + row0,
                                           g->scat_pos, st, X0, X1, D_val);
   GBE_LAUNCHED();
   return GBE_OK;

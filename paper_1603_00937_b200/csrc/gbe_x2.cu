@@ -689,6 +689,11 @@ int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* 
   // hybrid: the communities with m <= GBE_PK_MAX_M are the packed kernel's (gbe_small.cu), only the others are tiled
   const gbe_tile_item* items = hybrid ? (last ? g->items_last_h : g->items_h) : (last ? g->items_last : g->items);
   const int n_items = hybrid ? (last ? g->n_items_last_h : g->n_items_h) : (last ? g->n_items_last : g->n_items);
+  return gbe_launch_x2_items(g, st, Xin, Xout, partials, iter, items, n_items, buffer, s);
+}
+
+int gbe_launch_x2_items(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
+                        const gbe_tile_item* items, int n_items, int buffer, cudaStream_t s) {
   if (n_items == 0) return GBE_OK;
   if (g->tmaps) {  // panels staged by 2-D TMA (k_x2_tma); X_n is in buffer 0 for even iterations, in buffer 1 for odd ones
     const CUtensorMap* maps = reinterpret_cast<const CUtensorMap*>(g->tmaps) + (buffer ? g->n_part : 0);

@@ -468,6 +468,52 @@ def test_preset_arbitrary_sequence_on_water(gbe):
         gbe.gbe_density_preset(Hd, g, np.array([0, 2], dtype=np.uint8))
 
 
+@pytest.mark.parametrize("which", ["water", "shuffled", "chain"])
+def test_preset_sequence_in_a_bounded_workspace(gbe, which):
+    """with the SP2 sequence fixed beforehand the expansions run "without exchange of information during or between
+    the matrix multiplications" - nothing couples the communities, so gbe_density_preset(trace_every_iteration = 0) works
+    through them in waves when the workspace holds only part of the batch.  Same kernels on the same tiles: D must be
+    BIT FOR BIT the D of the whole-batch run, for any workspace between the minimum (the largest community) and the full
+    size; and it must meet the oracle's replay of the same sequence."""
+    import torch
+    s = {"water": lambda: gi.config(2),
+         "shuffled": lambda: gi.random_banded(700, half_bw=6, n_part=23, seed=5, tau=1e-4, iters=20, shuffle=True),
+         "chain": lambda: gi.chain(4800, 600, seed=5)}[which]()
+    seq = np.array([1, 0, 0, 1, 0, 1, 1, 0, 1, 0, 0, 1][: min(12, s.iters)], dtype=np.uint8)
+    rp, ci = o.build_graph(s.H, s.tau)
+    r = o.o_sub(s.H, rp, ci, s.part, s.n_part, s.n_occ, len(seq), replay=(seq, len(seq)))
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    part_t = torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
+    g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
+    gbe.gbe_graph_set_sp2_path(g, 1)  # the whole-batch reference on the same (tiled) kernels
+    full, small = g.info["workspace_bytes"], g.info["workspace_bytes_preset_min"]
+    assert small < full
+    D_full, log_full = gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False)
+    torch.cuda.synchronize()
+    assert np.abs(D_full.cpu().numpy() - r.D_val).max() <= TOL_D
+    for nbytes in (small, small + (full - small) // 3, full - 256):
+        ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        D_w, log_w = gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False, workspace=ws)
+        torch.cuda.synchronize()
+        assert torch.equal(D_w, D_full), nbytes
+        assert log_w.iters_done == len(seq) and abs(log_w.t1[-1] - r.t1[-1]) <= TOL_TR and abs(log_w.t2[-1] - r.t2[-1]) <= TOL_TR
+    # zero iterations: the waves return the gathered X0
+    D0f, _ = gbe.gbe_density_preset(Hd, g, seq[:0], trace_every_iteration=False)
+    D0w, l0 = gbe.gbe_density_preset(Hd, g, seq[:0], trace_every_iteration=False,
+                                     workspace=torch.empty(small, dtype=torch.uint8, device="cuda"))
+    torch.cuda.synchronize()
+    assert torch.equal(D0f, D0w) and abs(l0.t1[0] - r.t1[0]) <= TOL_TR
+    # below the minimum, or with per-iteration traces (which couple the communities), the small workspace is refused
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False,
+                               workspace=torch.empty(small - 256, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == -5
+    with pytest.raises(gbe.GbeError) as e:
+        gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=True,
+                               workspace=torch.empty(small, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == -5
+
+
 # ------------------------------------------------------------------------------- Eq.(8): graph of the next MD step
 @pytest.mark.parametrize("which", ["chain", "water"])
 def test_update_graph_eq8_md_step(gbe, which):
