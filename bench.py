@@ -113,7 +113,8 @@ def record_traffic(args) -> None:
     assert per, "no k_x2 launch in the capture"
     full = max(g for g, _ in per)
     vals = [b for g, b in per if g == full]
-    rec = {"workload": args.workload, "kernel": "k_x2<4,0>", "grid": full, "launches_averaged": len(vals),
+    kname = next(r[k_name] for r in rows[2:] if "k_x2" in r[k_name]).split("(")[0].replace("void ", "").replace("<unnamed>::", "")
+    rec = {"workload": args.workload, "kernel": kname, "grid": full, "launches_averaged": len(vals),
            "dram_bytes_per_launch": float(np.mean(vals)), "gbe_x2_cu_blob": git_blob_sha1(X2_SOURCE),
            "source": args.traffic_source or os.path.basename(args.record_traffic)}
     with open(X2_TRAFFIC_JSON, "w") as f:
@@ -451,7 +452,7 @@ def run_ours(args) -> None:
             "ms_steps": {"device": step_ms_log[0], "e2e": step_ms_log[-1]},
             "clocks": clk,
             "roofline": {
-                "kernel": "k_x2 (Y = X X^T on DMMA.8x8x4, fused branch/trace epilogue)", "bound": "tensor",
+                "kernel": "k_x2_tma (Y = X X^T on DMMA.8x8x4, panels by 2-D TMA, fused branch/trace epilogue)", "bound": "tensor",
                 "achieved": sym_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": sym_tf / peak_tf,
                 "traffic": traffic, "traffic_note": traffic_note,
                 "algorithmic_bytes_per_launch": 16.0 * info["dense_elems"],
@@ -704,18 +705,28 @@ def run_small(args) -> None:
              ("water box, 1536 orbitals, tau=1e-3, 128 communities", gi.water_box(256, 128, tau=1e-3)),
              ("banded, 14504 orbitals, 148 communities", gi.random_banded(14504, half_bw=6, n_part=148, seed=11, tau=1e-4, iters=40)),
              ("banded, 16872 orbitals, 148 communities", gi.random_banded(16872, half_bw=6, n_part=148, seed=11, tau=1e-4, iters=40)),
-             ("banded, 1450 orbitals, 10 communities", gi.random_banded(1450, half_bw=6, n_part=10, seed=11, tau=1e-4, iters=40))]
+             ("banded, 1450 orbitals, 10 communities", gi.random_banded(1450, half_bw=6, n_part=10, seed=11, tau=1e-4, iters=40)),
+             ("banded, 4608 orbitals, 32 communities", gi.random_banded(4608, half_bw=6, n_part=32, seed=11, tau=1e-4, iters=40)),
+             ("banded, 9216 orbitals, 64 communities", gi.random_banded(9216, half_bw=6, n_part=64, seed=11, tau=1e-4, iters=40)),
+             ("banded, 21312 orbitals, 148 communities", gi.random_banded(21312, half_bw=6, n_part=148, seed=11, tau=1e-4, iters=40)),
+             ("chain, 19200 orbitals, 600 communities", gi.chain(19200, 600, seed=5)),
+             ("banded, 58016 orbitals, 592 communities", gi.random_banded(58016, half_bw=6, n_part=592, seed=11, tau=1e-4, iters=40)),
+             ("water box, 6144 orbitals, tau=1e-3, 256 communities", gi.water_box(1024, 256, tau=1e-3))]
     for name, s in cases:
         Hd = gbe.DeviceCSR.from_host(s.H)
         g = gbe.gbe_build_graph(Hd, s.tau, None, s.n_part)
         ws = g.new_workspace()
         D = torch.empty(g.info["nnz_D"], dtype=torch.float64, device="cuda")
-        auto = "resident" if g.info["resident_sp2"] else "tiled"
+        auto = {1: "tiled", 2: "resident", 3: "packed"}[int(g.info["sp2_path_chosen"])]
         seq = np.array([i & 1 for i in range(s.iters)], dtype=np.uint8)
-        for path, pname in ((1, "tiled"), (2, "resident")):
+        for path, pname in ((1, "tiled"), (2, "resident"), (3, "packed")):
             if path == 2 and not g.info["resident_fits"]:
                 continue
+            if path == 3 and not g.info["n_small"]:
+                continue
             gbe.gbe_graph_set_sp2_path(g, path)
+            if int(g.info["sp2_path_chosen"]) != path:  # e.g. resident requested, communities not co-resident
+                continue
             n0 = gbe.gbe_launch_count()
             gbe.gbe_density(Hd, g, s.n_occ, s.iters, workspace=ws, D_val=D, want_log=False)
             launches = gbe.gbe_launch_count() - n0
