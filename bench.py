@@ -573,7 +573,7 @@ def run_sweep(args) -> None:
                    "sp2_loop_ms": ph["x2_ms"] + ph["x2_last_ms"] + ph["trace_ms"], "gather_ms": ph["gather_ms"],
                    "scatter_ms": ph["scatter_ms"],
                    "sp2_exec_tflops": info["sp2_exec_flops_per_iter"] * max(0, log.iters_done - 1) / max(1e-9, ph["x2_ms"] * 1e-3) * 1e-12,
-                   "iters_done": int(log.iters_done), "sp2_path": int(info["sp2_path_chosen"]),
+                   "x2_tma": int(info["x2_tma"]), "iters_done": int(log.iters_done), "sp2_path": int(info["sp2_path_chosen"]),
                    "n_small": int(info["n_small"]), "n_bins": int(info["n_bins"]),
                    "sp2_tflops_alg": (info["sp2_flops_per_iter"] * max(0, log.iters_done - 1) + info["sp2_flops_last_iter"])
                                      / (e1.elapsed_time(e2) * 1e-3) * 1e-12,

@@ -110,6 +110,9 @@ typedef struct {
   int64_t n_bins;            /* CTAs of one packed launch (bins of 1..16 small communities) */
   size_t workspace_bytes_preset_min; /* smallest workspace gbe_density_preset(trace_every_iteration = 0) accepts: it then
                                         works through the communities in waves (see there) */
+  int32_t x2_tma;            /* 1: the tiled X^2 kernel of this graph stages its panels by 2-D TMA (tensor maps; long K loops),
+                                0: by cp.async (short K loops, or no tensor-map encoder in the driver) */
+  int32_t reserved2_;
 } gbe_graph_info;
 
 /* SP2 log (host memory, caller-allocated; valid after the stream has been synchronised).

@@ -50,7 +50,8 @@ class _GraphInfo(C.Structure):
                 ("contiguous_cores", C.c_int32), ("tile", C.c_int32), ("workspace_bytes", C.c_size_t),
                 ("workspace_bytes_fermi", C.c_size_t), ("resident_sp2", C.c_int32), ("resident_fits", C.c_int32),
                 ("resident_cluster", C.c_int32), ("sp2_path_chosen", C.c_int32), ("sp2_sym_flops_per_iter", C.c_double),
-                ("n_small", C.c_int64), ("n_bins", C.c_int64), ("workspace_bytes_preset_min", C.c_size_t)]
+                ("n_small", C.c_int64), ("n_bins", C.c_int64), ("workspace_bytes_preset_min", C.c_size_t),
+                ("x2_tma", C.c_int32), ("reserved2_", C.c_int32)]
 
 
 class _Sp2Log(C.Structure):

@@ -204,6 +204,7 @@ int gbe_graph_get_info(const gbe_graph* g, gbe_graph_info* o) {
   o->n_small = g->pk_n_small;
   o->n_bins = g->n_pk_ctas;
   o->workspace_bytes_preset_min = g->ws_bytes_wave_min;
+  o->x2_tma = g->tmaps ? 1 : 0;
   o->resident_fits = g->resident_fits;
   o->resident_cluster = g->resident_cluster;
   return GBE_OK;

@@ -620,6 +620,19 @@ __global__ void k_patch_tmaps(CUtensorMap* __restrict__ maps, const int64_t* __r
 int gbe_x2_build_tmaps(gbe_graph* g, cudaStream_t s) {
   g->tmaps = nullptr;
   if (g->n_items == 0) return GBE_OK;
+  // Which kernel stages the panels.  Measured on the tau x partition grid of the 24,576-orbital box (profiles/
+  // r02_sweep_config5.md): the TMA kernel wins where the K loops are long (work-weighted mean m >~ 350: -3 % per launch at
+  // m ~ 490, -2 % at m ~ 1,800) and loses where a tile has fewer than ~20 K chunks (m ~ 170: +20 %) - its per-tile set-up
+  // (mbarrier initialisation, tensor-map fetch, three chunks requested by one thread) is longer than the cp.async kernel's.
+  {
+    double w = 0.0, wm = 0.0;
+    for (int p = 0; p < g->n_part; ++p) {
+      const double m = (double)g->h_m[p];
+      w += m * m * m;
+      wm += m * m * m * m;
+    }
+    if (w <= 0.0 || wm / w < 360.0) return GBE_OK;  // short K loops: the cp.async kernel
+  }
   static std::atomic<PFN_encodeTiled> encode_p{nullptr};
   PFN_encodeTiled encode = encode_p.load();
   if (!encode) {

@@ -461,6 +461,7 @@ def test_preset_arbitrary_sequence_on_water(gbe):
     n0 = gbe.gbe_launch_count()
     Dg, log = gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False)
     torch.cuda.synchronize()
+    assert g.info["x2_tma"] == 1  # m ~ 500: long K loops, panels by TMA (one launch sets the tensor-map addresses)
     assert gbe.gbe_launch_count() - n0 == 2 + 1 + 1 + 1 + len(seq) + 1 + 1  # bounds(2) gather tensor-maps init x2... final trace scatter
     assert np.abs(Dg.cpu().numpy() - r.D_val).max() <= TOL_D
     assert abs(log.t1[-1] - r.t1[-1]) <= TOL_TR
@@ -863,7 +864,8 @@ def test_resident_kernel_launches_and_choice(gbe):
     n0 = gbe.gbe_launch_count()
     D_til, log_til = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
     torch.cuda.synchronize()
-    assert gbe.gbe_launch_count() - n0 == 2 + 1 + 1 + 2 + 2 * s.iters + 1  # ..., tensor-map addresses, init + trace, loop, scatter
+    assert g.info["x2_tma"] == 0  # m = 48: short K loops, panels by cp.async
+    assert gbe.gbe_launch_count() - n0 == 2 + 1 + 2 + 2 * s.iters + 1
     assert float((D_res - D_til).abs().max()) <= 1e-12
     live = np.abs(log_til.t1[:-1] - log_til.t2[:-1]) > 1e-9
     assert np.array_equal(log_res.branch[live], log_til.branch[live])
