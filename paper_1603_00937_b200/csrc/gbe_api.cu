@@ -256,8 +256,9 @@ static int choose_sp2(const gbe_graph* g, int mode) {
   if (g->sp2_path == 2) return can_res ? 2 : 1;
   if (g->sp2_path == 3) return can_pk ? 3 : 1;
   // auto.  Resident: one launch for the whole loop - wins whenever the communities are small enough that one SM per
-  // community keeps up with the tiled kernels spreading the tiles over all SMs (measured).
-  if (can_res && (g->max_m <= 128 || g->n_part >= g->resident_coresident / 2)) return 2;
+  // community keeps up with the tiled kernels spreading the tiles over all SMs (measured, profiles/r02_small_systems.md:
+  // always up to m = 128; at m = 160 from about 50 communities on - 64: 1.09 against 1.24 ms, 32: 1.08 against 0.97 ms).
+  if (can_res && (g->max_m <= 128 || g->n_part >= g->resident_coresident / 3)) return 2;
   // Packed: every community fits shared memory and there are enough of them to occupy the device (measured, DESIGN.md 6:
   // a graph that also needs the tiled kernel for some communities pays a second, poorly filled launch per iteration and
   // is not faster than the tiled kernels alone).
