@@ -564,6 +564,16 @@ def run_sweep(args) -> None:
             e2.record()
             torch.cuda.synchronize()
             _, ph = gbe.gbe_density_timed(Hd, g, n_occ, base.iters, idem_tol, workspace=ws, D_val=D_val)
+            # the paper's own mode: the sequence just logged, given beforehand, no trace reduction between products
+            seq = log.branch
+            gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False, workspace=ws, D_val=D_val, want_log=False)
+            torch.cuda.synchronize()
+            e3, e4 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e3.record()
+            gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False, workspace=ws, D_val=D_val, want_log=False)
+            e4.record()
+            torch.cuda.synchronize()
+            preset_ms = e3.elapsed_time(e4)
             ex = g.export()
             m = (ex["sub_ptr"][1:] - ex["sub_ptr"][:-1]).double()
             rec = {"sweep": args.workload, "tau": tau, "n_part": n_part, "m_min": int(m.min()), "m_mean": float(m.mean()),
@@ -573,7 +583,7 @@ def run_sweep(args) -> None:
                    "sp2_loop_ms": ph["x2_ms"] + ph["x2_last_ms"] + ph["trace_ms"], "gather_ms": ph["gather_ms"],
                    "scatter_ms": ph["scatter_ms"],
                    "sp2_exec_tflops": info["sp2_exec_flops_per_iter"] * max(0, log.iters_done - 1) / max(1e-9, ph["x2_ms"] * 1e-3) * 1e-12,
-                   "x2_tma": int(info["x2_tma"]), "iters_done": int(log.iters_done), "sp2_path": int(info["sp2_path_chosen"]),
+                   "preset_no_trace_ms": preset_ms, "x2_tma": int(info["x2_tma"]), "iters_done": int(log.iters_done), "sp2_path": int(info["sp2_path_chosen"]),
                    "n_small": int(info["n_small"]), "n_bins": int(info["n_bins"]),
                    "sp2_tflops_alg": (info["sp2_flops_per_iter"] * max(0, log.iters_done - 1) + info["sp2_flops_last_iter"])
                                      / (e1.elapsed_time(e2) * 1e-3) * 1e-12,

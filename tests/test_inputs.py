@@ -73,3 +73,32 @@ def test_random_banded_shuffle_is_a_relabelling():
     b = gi.random_banded(40, half_bw=3, n_part=4, seed=2, shuffle=True)
     assert np.allclose(np.sort(np.linalg.eigvalsh(a.H.to_dense())), np.sort(np.linalg.eigvalsh(b.H.to_dense())))
     assert sorted(np.bincount(a.part)) == sorted(np.bincount(b.part)) and not np.array_equal(a.part, b.part)
+
+
+def test_bench_helpers_blob_hash_traffic_record_and_oracle_sample(tmp_path, monkeypatch):
+    """bench.py host logic: the git blob hash that ties profiles/x2_traffic.json to the kernel source it was captured on,
+    the refusal of a stale or foreign record, and the sizing of the oracle sample of the reference arm."""
+    import hashlib
+    import json
+    import os
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path.insert(0, root)
+    import bench
+    f = tmp_path / "k.cu"
+    f.write_bytes(b"hello\n")
+    assert bench.git_blob_sha1(str(f)) == hashlib.sha1(b"blob 6\0hello\n").hexdigest() == "ce013625030ba8dba906f756967f9e9ca394464a"
+    rec = tmp_path / "x2_traffic.json"
+    monkeypatch.setattr(bench, "X2_TRAFFIC_JSON", str(rec))
+    monkeypatch.setattr(bench, "X2_SOURCE", str(f))
+    assert bench.x2_traffic("water4096")[0] is None                      # no record
+    rec.write_text(json.dumps({"workload": "water4096", "dram_bytes_per_launch": 2.0e9,
+                               "gbe_x2_cu_blob": bench.git_blob_sha1(str(f))}))
+    assert bench.x2_traffic("water4096")[0] == 2.0e9
+    assert bench.x2_traffic("water1024")[0] is None                      # another workload
+    f.write_bytes(b"changed\n")
+    assert bench.x2_traffic("water4096")[0] is None                      # the kernel source changed since the capture
+    monkeypatch.setattr(bench, "cpu_cores", lambda: 16)
+    assert bench.oracle_sample_molecules("water4096", 3, 300.0) == 4096   # three passes of the real workload fit
+    assert bench.oracle_sample_molecules("water4096", 25, 300.0) < 4096   # the driver's 20 + 5 do not: a smaller box
+    assert bench.oracle_sample_molecules("water4096", 10 ** 6, 300.0) == 256
