@@ -18,12 +18,8 @@
 // the accumulator of every warp live in shared memory); ncu counters in profiles/r01_spgemm_ncu.md.
 #include "gbe_internal.cuh"
 
-static size_t g_bm_save_max = (size_t)8 << 30;  // gbe_set_build_scratch_limit
-size_t gbe_set_build_scratch_limit(size_t bytes) {
-  const size_t old = g_bm_save_max;
-  g_bm_save_max = bytes;
-  return old;
-}
+static std::atomic<size_t> g_bm_save_max{(size_t)8 << 30};  // gbe_set_build_scratch_limit
+size_t gbe_set_build_scratch_limit(size_t bytes) { return g_bm_save_max.exchange(bytes); }
 
 namespace {
 
