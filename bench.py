@@ -124,7 +124,7 @@ def record_traffic(args) -> None:
 
 
 def measure_fp64_peak(torch) -> dict:
-    """cuBLAS DGEMM in this process, before the timed region (a library call, used for the roofline denominator only):
+    """cuBLAS DGEMM in this process, after the timed regions (a library call, used for the roofline denominator only):
     torch.matmul on float64 8192^3, best of 10 (burst) and back to back for ~4 s (sustained), CUDA events."""
     n = 8192
     a = torch.randn(n, n, dtype=torch.float64, device="cuda")
@@ -156,8 +156,92 @@ def measure_fp64_peak(torch) -> dict:
             "reps_sustained": reps}
 
 
+CLOCK_REASONS = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+
+def _clock_summary(rows, t0: float, t1: float, source: str) -> dict:
+    """rows: (wall time, sm MHz, max sm MHz, power W, set of reason names); the samples inside [t0, t1] summarised."""
+    sm, smax, pw, reasons = [], [], [], set()
+    for ts, a, b, c, r in rows:
+        if t0 <= ts <= t1 + 0.2:
+            sm.append(a); smax.append(b); pw.append(c); reasons |= r
+    return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+            "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons), "source": source}
+
+
+class NvmlSampler:
+    """SM clock, power and throttle reasons through NVML from a thread of this process, every 50 ms.  The default: a
+    separate nvidia-smi process takes a driver lock when it attaches, polls and exits, and each of those showed up as a
+    stall of tens of ms in a timed step; NVML queries from inside the process did not."""
+
+    def __init__(self, gpu_index: int):
+        import pynvml
+        self.nv = pynvml
+        pynvml.nvmlInit()
+        # NVML numbers every device of the box, CUDA those of CUDA_VISIBLE_DEVICES: translate the index when it is set
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+        ids = [x.strip() for x in vis.split(",") if x.strip()]
+        if ids and gpu_index < len(ids):
+            v = ids[gpu_index]
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(int(v)) if v.isdigit() else pynvml.nvmlDeviceGetHandleByUUID(v)
+        else:
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(gpu_index)
+        self.rows, self.run, self.th = [], False, None
+        nv = pynvml
+        self.bits = {"hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown if hasattr(nv, "nvmlClocksEventReasonHwSlowdown") else 0x8,
+                     "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
+        self.smax = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+
+    def _loop(self):
+        nv = self.nv
+        while self.run:
+            try:
+                sm = float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                pw = nv.nvmlDeviceGetPowerUsage(self.h) * 1e-3
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.rows.append((time.time(), sm, self.smax, pw, {k for k, b in self.bits.items() if mask & b}))
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def start(self):
+        self.run = True
+        self.th = threading.Thread(target=self._loop, daemon=True)
+        self.th.start()
+
+    def wait_first(self, timeout: float = 5.0):
+        t = time.time()
+        while not self.rows and time.time() - t < timeout:
+            time.sleep(0.02)
+
+    def stop(self, t0: float, t1: float) -> dict:
+        time.sleep(0.06)
+        self.run = False
+        if self.th is not None:
+            self.th.join(timeout=2)
+        return _clock_summary(self.rows, t0, t1, "nvml")
+
+
+class NoSampler:
+    def __init__(self, why: str = "clock sampling disabled"):
+        self.why = why
+
+    def start(self):
+        pass
+
+    def wait_first(self, timeout: float = 0.0):
+        pass
+
+    def stop(self, t0: float, t1: float) -> dict:
+        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [self.why], "samples": 0, "source": "none"}
+
+
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md, clocks line)."""
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md, clocks line); the fallback when
+    NVML cannot be imported (--clock-sampler nvidia-smi forces it)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -177,11 +261,21 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append((time.time(), line.strip()))
+            f = [x.strip() for x in line.strip().split(",")]
+            try:
+                self.rows.append((time.time(), float(f[1]), float(f[2]), float(f[3]),
+                                  {nm for nm, v in zip(CLOCK_REASONS, f[4:8]) if v.lower().startswith("active")}))
+            except (ValueError, IndexError):
+                continue
+
+    def wait_first(self, timeout: float = 5.0):
+        t = time.time()
+        while self.proc is not None and not self.rows and time.time() - t < timeout:
+            time.sleep(0.02)
 
     def stop(self, t0: float, t1: float) -> dict:
         if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"], "source": "nvidia-smi"}
         time.sleep(0.15)
         self.proc.terminate()
         try:  # nvidia-smi's exit briefly stalls the driver: be sure it is gone before anything else is timed
@@ -189,21 +283,18 @@ class ClockSampler:
         except Exception:
             self.proc.kill()
         time.sleep(0.5)
-        sm, smax, pw, reasons = [], [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ts, line in self.rows:
-            if not (t0 <= ts <= t1 + 0.2):
-                continue
-            f = [x.strip() for x in line.split(",")]
-            try:
-                sm.append(float(f[1])); smax.append(float(f[2])); pw.append(float(f[3]))
-            except (ValueError, IndexError):
-                continue
-            for nm, v in zip(names, f[4:8]):
-                if v.lower().startswith("active"):
-                    reasons.add(nm)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+        return _clock_summary(self.rows, t0, t1, "nvidia-smi")
+
+
+def make_clock_sampler(kind: str, gpu_index: int):
+    if kind == "none":
+        return NoSampler()
+    if kind == "nvml":
+        try:
+            return NvmlSampler(gpu_index)
+        except Exception:
+            pass  # no pynvml / no NVML on this box: the nvidia-smi process
+    return ClockSampler(gpu_index)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -328,7 +419,6 @@ def run_ours(args) -> None:
     import paper_1603_00937_b200 as gbe
     gbe.lib()
 
-    fp64_peak = measure_fp64_peak(torch)  # cuBLAS DGEMM, this process, before anything is timed
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
 
     s = make_system(args.workload, seed=rank)  # replicas: one independent seeded box per rank
@@ -380,13 +470,13 @@ def run_ours(args) -> None:
         step_ms_log.append([round(x, 3) for x in ms])
         return float(np.sum(ms)), int(launches)
 
+    # the sampler runs from before the warm-up: whatever attaching it costs is paid outside the timed region
+    clocks = make_clock_sampler(args.clock_sampler, local)
+    clocks.start()
     for _ in range(max(args.warmup, 3)):
         step_device()
     torch.cuda.synchronize()
-
-    clocks = ClockSampler(local)
-    clocks.start()
-    time.sleep(0.3)
+    clocks.wait_first()
     t_wall0 = time.time()
     total_ms, launches = timed_region(step_device, args.steps)
     t_wall1 = time.time()
@@ -396,6 +486,10 @@ def run_ours(args) -> None:
     for _ in range(max(args.warmup, 3)):
         step_host()
     e2e_ms, _ = timed_region(step_host, args.steps)
+
+    # roofline denominator: cuBLAS DGEMM in this process, AFTER the timed regions (its 4 s of back-to-back GEMMs heat
+    # the part and its 1.5 GB of torch allocations disturb the pool; neither belongs in front of the steps)
+    fp64_peak = measure_fp64_peak(torch)
 
     # per-kernel device times, same process, same inputs (CUDA events around every launch of gbe_density)
     g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
@@ -779,6 +873,8 @@ def main() -> None:
     ap.add_argument("--sp2-path", type=int, default=0, help="sweep: force the SP2 kernels (1 tiled, 2 resident, 3 packed; 0 = the library's choice)")
     ap.add_argument("--waves", action="store_true", help="gbe_density_preset on the whole batch against the same call in a bounded workspace")
     ap.add_argument("--waves-gb", type=float, default=8.0, help="--waves: size of the bounded workspace in GB")
+    ap.add_argument("--clock-sampler", default="nvml", choices=["nvml", "nvidia-smi", "none"],
+                    help="how clocks / throttle reasons are sampled during the timed region (nvml: a thread of this process)")
     ap.add_argument("--record-traffic", default="", help="ncu raw-page CSV of a --set full capture of k_x2: write profiles/x2_traffic.json")
     ap.add_argument("--traffic-source", default="", help="the profiles/ summary that documents the capture")
     args = ap.parse_args()

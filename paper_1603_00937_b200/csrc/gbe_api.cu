@@ -135,7 +135,7 @@ static int build_graph_impl(const gbe_csr_view* H, const gbe_graph_opts* opts, c
   } guard{g};
 
   // step 0: bounds of the H given here; they travel to pinned host words and are looked at after the first
-  // synchronisation of the build (a build has three: accumulator capacity of the product; subgraph sizes + nnz(S); end)
+  // synchronisation of the build (a build has four: accumulator capacity of the product; nnz(S); subgraph sizes; end)
   DevBuf st, bl;
   GBE_TRY(st.alloc(sizeof(gbe_state)));
   GBE_TRY(bl.alloc(2 * 1024 * sizeof(double)));
@@ -149,10 +149,10 @@ static int build_graph_impl(const gbe_csr_view* H, const gbe_graph_opts* opts, c
   // step 1: S_tau - from H and its thresholded powers (A-1), or by Eq.(8) from the previous D and this H
   if (prev)
     GBE_TRY(gbe_build_pattern_eq8(*H, prev->D_row_ptr, prev->D_col, D_prev, g->tau, s, &g->S_row_ptr, &g->S_col, &g->nnz_S,
-                                  &g->S_cap, prev->nnz_D));
+                                  prev->nnz_D));
   else
     GBE_TRY(gbe_build_pattern(*H, st.as<gbe_state>(), g->tau, power, opts->check_symmetry, s, &g->S_row_ptr, &g->S_col,
-                              &g->nnz_S, &g->S_cap));
+                              &g->nnz_S));
   // step 2: subgraphs, layout, pattern of D, work lists (synchronises; checks the bounds)
   GBE_TRY(gbe_build_subgraphs(g, part, s, b));
   g->eps_min = b[0];

@@ -466,10 +466,11 @@ struct Unioner {
   }
 };
 
-// S = P u P^T (P's rows need not be sorted on input; S's are ascending).  P.nnz may be an upper bound; with `bounded` S
-// is sized by 2 P.nnz and nothing comes back to the host (the caller fetches the exact count, S.rp[n], when it next
-// synchronises), else S is sized exactly (one synchronisation)
-int symmetrise(Pattern& P, Unioner& U, DevBuf& cnt, Pattern& S, bool bounded) {
+// S = P u P^T (P's rows need not be sorted on input; S's are ascending).  P.nnz may be an upper bound.  S is sized
+// EXACTLY (one synchronisation): it is the one array of the build that outlives it, and sized by the bound 2 nnz(P) it was
+// a block of tens of MB that cycled through the stream-ordered pool on every build - with the host running ahead of the
+// device (back-to-back builds of an MD loop) the pool then stalled for 0.1 - 0.9 s at a time
+int symmetrise(Pattern& P, Unioner& U, DevBuf& cnt, Pattern& S) {
   const int64_t n = U.n;
   cudaStream_t s = U.s;
   const int rows_grid = (int)((n + 7) / 8);
@@ -484,8 +485,8 @@ int symmetrise(Pattern& P, Unioner& U, DevBuf& cnt, Pattern& S, bool bounded) {
                                              cnt.as<int32_t>(), PT.col.as<int32_t>());
   GBE_LAUNCHED();
   GBE_TRY(U.run(P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr, 0.0, PT.rp.as<int64_t>(), PT.col.as<int32_t>(), nullptr,
-                0, S, bounded ? 2 * P.nnz : -1));
-  return GBE_OK;  // (no synchronisation: the temporaries are released in stream order)
+                0, S));
+  return GBE_OK;
 }
 
 int count_to_rowptr(DevBuf& cnt, int64_t n, DevBuf& rp, int64_t* nnz, cudaStream_t s, int64_t ub) {
@@ -507,7 +508,7 @@ int count_to_rowptr(DevBuf& cnt, int64_t n, DevBuf& rp, int64_t* nnz, cudaStream
 static const size_t UB_BYTES_MAX = (size_t)4 << 30;
 
 int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, int power, int check_sym,
-                      cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S, int64_t* S_cap) {
+                      cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S) {
   const int64_t n = H.n;
   const int W = (int)((n + 31) / 32);
   const int rows_grid = (int)((n + 7) / 8);
@@ -661,13 +662,10 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
     T_val = Tprev.val.as<double>();
     // Tn (now holding the previous T) and Pn are released here, after the sync above
   }
-  // S = P u P^T, sized by 2 nnz(P) while that bound is small: the exact nnz(S) = S_row_ptr[n] is then fetched by the
-  // caller with its next synchronisation (*nnz_S = -1, *S_cap = entries allocated)
+  // S = P u P^T
   Pattern S;
-  const bool bounded = (size_t)P.nnz * 8 <= UB_BYTES_MAX;
-  GBE_TRY(symmetrise(P, U, cnt, S, bounded));
-  *nnz_S = bounded ? -1 : S.nnz;
-  *S_cap = S.nnz;
+  GBE_TRY(symmetrise(P, U, cnt, S));
+  *nnz_S = S.nnz;
   *S_row_ptr = reinterpret_cast<int64_t*>(S.rp.release());
   *S_col = reinterpret_cast<int32_t*>(S.col.release());
   return GBE_OK;
@@ -678,8 +676,7 @@ int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st, double tau, in
 //     M = I u pat(|D_ij| >= tau) u pat(H(t)),   S = pat(M M) ("paths of length two"),  then S u S^T.
 // D is the assembled, non-symmetric P_tau of the previous step on the pattern (D_rp, D_col).
 int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int32_t* D_col, const double* D_val, double tau,
-                          cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S, int64_t* S_cap,
-                          int64_t nnz_D) {
+                          cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S, int64_t nnz_D) {
   const int64_t n = H.n;
   const int W = (int)((n + 31) / 32);
   const int sm_count = gbe_sm_count();  // of the current device
@@ -714,10 +711,8 @@ int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int3
                                                              P.rp.as<int64_t>(), P.col.as<int32_t>(), nullptr, bm_io, nullptr);
   GBE_LAUNCHED();
   Pattern S;
-  const bool bounded = (size_t)P.nnz * 8 <= UB_BYTES_MAX;
-  GBE_TRY(symmetrise(P, U, cnt, S, bounded));
-  *nnz_S = bounded ? -1 : S.nnz;
-  *S_cap = S.nnz;
+  GBE_TRY(symmetrise(P, U, cnt, S));
+  *nnz_S = S.nnz;
   *S_row_ptr = reinterpret_cast<int64_t*>(S.rp.release());
   *S_col = reinterpret_cast<int32_t*>(S.col.release());
   return GBE_OK;

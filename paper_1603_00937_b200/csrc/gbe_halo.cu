@@ -290,23 +290,9 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
   g->h_ncore.resize(n_part);
   GBE_CUDA(cudaMemcpyAsync(g->h_m.data(), g->msize, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaMemcpyAsync(g->h_ncore.data(), g->ncore, (size_t)n_part * 4, cudaMemcpyDeviceToHost, s));
-  int64_t nnz_S_stack = 0;
-  int64_t* const nnz_S_host = pin ? reinterpret_cast<int64_t*>(pin + 4) : &nnz_S_stack;
-  if (g->nnz_S < 0) GBE_CUDA(cudaMemcpyAsync(nnz_S_host, g->S_row_ptr + n, 8, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaStreamSynchronize(s));
   if (*core_flag) return GBE_EINVAL;  // partition id out of range (k_core_count)
   if (bounds && (!(bounds[1] > bounds[0]) || !std::isfinite(bounds[0]) || !std::isfinite(bounds[1]))) return GBE_EDEGENERATE;
-  if (g->nnz_S < 0) {  // S_col was sized by an upper bound (gbe_build_pattern): the exact count is here now - trim
-    g->nnz_S = *nnz_S_host;
-    if (g->S_cap > g->nnz_S + g->nnz_S / 4 + 1024) {
-      int32_t* exact = nullptr;
-      GBE_TRY(gbe_dev_alloc((void**)&exact, std::max<size_t>(16, (size_t)g->nnz_S * 4)));
-      GBE_CUDA(cudaMemcpyAsync(exact, g->S_col, (size_t)g->nnz_S * 4, cudaMemcpyDeviceToDevice, s));
-      gbe_dev_free(g->S_col);  // stream ordered: after the copy
-      g->S_col = exact;
-      g->S_cap = g->nnz_S;
-    }
-  }
   // ---- host: layout, work lists
   std::vector<int64_t> h_sub_ptr(n_part + 1, 0);
   g->h_dense_off.assign(n_part + 1, 0);

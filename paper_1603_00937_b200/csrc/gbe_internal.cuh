@@ -123,7 +123,6 @@ struct gbe_wave {  // a range of communities processed together by gbe_density_p
 // ----------------------------------------------------------------------------------------------
 struct gbe_graph {
   int64_t n = 0, nnz_S = 0, sum_m = 0, nnz_D = 0, dense_elems = 0;
-  int64_t S_cap = 0;  // entries S_col was allocated for (an upper bound until gbe_build_subgraphs trims it)
   int32_t n_part = 0, max_m = 0, max_ncore = 0, tile = 64;
   double eps_min = 0, eps_max = 0, tau = 0, flops_per_iter = 0, exec_flops_per_iter = 0;
   double flops_last_iter = 0, exec_flops_last_iter = 0;  // the core-tiles-only last iteration
@@ -194,14 +193,12 @@ struct gbe_graph {
 int gbe_launch_bounds(const gbe_csr_view& H, double* block_lo, double* block_hi, int max_blocks, gbe_state* st,
                       cudaStream_t s);
 // step 1
-// *nnz_S = -1: S_col was sized by an upper bound (*S_cap entries); the exact count is S_row_ptr[n] on the device and
-// gbe_build_subgraphs fetches it with its first synchronisation (and trims the array)
+// S is sized exactly (*nnz_S entries)
 int gbe_build_pattern(const gbe_csr_view& H, const gbe_state* st_dev, double tau, int power, int check_sym,
-                      cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S, int64_t* S_cap);
+                      cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S);
 // Eq.(8): S for the next MD step from the previous D and the new H
 int gbe_build_pattern_eq8(const gbe_csr_view& H, const int64_t* D_rp, const int32_t* D_col, const double* D_val, double tau,
-                          cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S, int64_t* S_cap,
-                          int64_t nnz_D);
+                          cudaStream_t s, int64_t** S_row_ptr, int32_t** S_col, int64_t* nnz_S, int64_t nnz_D);
 // step 2
 // bounds: pinned host copy of (eps_min, eps_max) of step 0, in flight on `s`: looked at after the first synchronisation
 int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const double* bounds);
