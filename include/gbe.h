@@ -52,7 +52,9 @@ typedef enum {
                            X0 = (eps_max I - H) / 1 carried through the same updates */
   GBE_EMISMATCH = -4,   /* H.n differs from the graph's n */
   GBE_ENOMEM = -5,      /* workspace too small (required size: gbe_graph_info.workspace_bytes) or allocation failed */
-  GBE_ECUDA = -6        /* a CUDA call failed; text via gbe_strerror / gbe_last_cuda_error */
+  GBE_ECUDA = -6,       /* a CUDA call failed; text via gbe_strerror / gbe_last_cuda_error */
+  GBE_ELIMIT = -7       /* the problem is larger than a fixed limit of the entry point (gbe_expectation_static:
+                           n > GBE_STATIC_MAX_N); nothing was launched */
 } gbe_status;
 
 #define GBE_MAX_ITERS 1024
@@ -287,6 +289,25 @@ int gbe_density_fermi(const gbe_csr_view* H, const gbe_graph* g, double mu, doub
  *   A      device CSR of dimension n, ascending columns (need not be symmetric, need not share D's pattern).
  *   out    HOST double; the call synchronises the stream.  The reduction order is fixed: reproducible bit for bit. */
 int gbe_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view* A, void* cuda_stream, double* out);
+
+/* gbe_expectation for callers that cannot allocate (code under CUDA-graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same <A> = Tr[D A], same kernels, same fixed reduction order - bit for bit the value
+ * gbe_expectation returns - but
+ *   - the call allocates NOTHING (no cudaMalloc / cudaMallocAsync / cudaFree, no allocating library routine) and does
+ *     not synchronise: it enqueues two kernels on `cuda_stream` and returns;
+ *   - its scratch (n per-row partial sums) is a static device array of GBE_STATIC_MAX_N doubles (1 MiB) inside the
+ *     library, held by every GPU that loads the library until the process exits.  n > GBE_STATIC_MAX_N: GBE_ELIMIT,
+ *     nothing launched (use gbe_expectation);
+ *   - out_dev is a DEVICE double[1] of the caller, valid once the stream reaches that point.
+ *   g, D_val, A   as for gbe_expectation (device pointers; borrowed for the duration of the enqueued work).
+ * All calls on one device share the scratch array: calls that OVERLAP on the GPU (different streams without an ordering
+ * between them) race on it and return garbage; calls on one stream, or ordered by events, are safe.  Nothing in it needs
+ * clearing between calls (every word read was written by the same call).  The first call on each device looks up the
+ * array's device address (cudaGetSymbolAddress, no allocation); make that first call outside a stream capture.
+ * Errors: GBE_EINVAL (null g / out_dev / A, null D_val with nnz_D > 0), GBE_EMISMATCH (A.n != n), GBE_ELIMIT, GBE_ECUDA. */
+#define GBE_STATIC_MAX_N 131072
+int gbe_expectation_static(const gbe_graph* g, const double* D_val, const gbe_csr_view* A, void* cuda_stream,
+                           double* out_dev);
 
 /* Error of D against a dense reference matrix, e.g. the exact projector (Fig.2: "the error in the calculated
  * density matrix ... as measured by the Frobenius norm (normalized per atom)"; obs. (ii) P:L65: the error is set by tau).

@@ -23,6 +23,8 @@ from .binding import (  # noqa: F401
     gbe_density_preset,
     gbe_density_fermi,
     gbe_expectation,
+    gbe_expectation_static,
+    GBE_STATIC_MAX_N,
     gbe_launch_count,
     gbe_graph_set_sp2_path,
     gbe_graph_set_gather_path,

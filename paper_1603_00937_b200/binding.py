@@ -21,7 +21,7 @@ EXPORTS = [
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
     "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation", "gbe_update_graph", "gbe_density_fermi",
     "gbe_graph_set_sp2_path", "gbe_error_norms", "gbe_graph_set_gather_path", "gbe_set_build_scratch_limit",
-    "gbe_set_packed_max_m",
+    "gbe_set_packed_max_m", "gbe_expectation_static",
 ]
 
 
@@ -102,6 +102,7 @@ def lib() -> C.CDLL:
         l.gbe_graph_set_gather_path.argtypes = [C.c_void_p, C.c_int32]
         l.gbe_set_build_scratch_limit.restype = C.c_size_t
         l.gbe_set_build_scratch_limit.argtypes = [C.c_size_t]
+        l.gbe_expectation_static.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CsrView), C.c_void_p, C.c_void_p]
         l.gbe_set_packed_max_m.restype = C.c_int32
         l.gbe_set_packed_max_m.argtypes = [C.c_int32]
         l.gbe_launch_count.restype = C.c_uint64
@@ -358,6 +359,19 @@ def gbe_expectation(g: Graph, D_val: torch.Tensor, A: DeviceCSR, stream=None) ->
     out = C.c_double(0.0)
     _check(lib().gbe_expectation(g.handle, _ptr(D_val), C.byref(v), _stream(stream), C.byref(out)))
     return float(out.value)
+
+
+GBE_STATIC_MAX_N = 131072  # gbe.h
+
+
+def gbe_expectation_static(g: Graph, D_val: torch.Tensor, A: DeviceCSR, out: torch.Tensor, stream=None) -> torch.Tensor:
+    """<A> = Tr[D A] into the caller's DEVICE double `out` without any allocation or synchronisation (scratch: a static
+    1 MiB device array inside the library, n <= GBE_STATIC_MAX_N; calls that overlap on the GPU race on it)."""
+    assert D_val.dtype == torch.float64 and D_val.is_cuda and D_val.numel() == g.info["nnz_D"]
+    assert out.dtype == torch.float64 and out.is_cuda and out.numel() >= 1 and out.is_contiguous()
+    v = A.view()
+    _check(lib().gbe_expectation_static(g.handle, _ptr(D_val), C.byref(v), _stream(stream), _ptr(out)))
+    return out
 
 
 def gbe_error_norms(g: Graph, D_val: torch.Tensor, D_ref: torch.Tensor, stream=None) -> tuple[float, float, float]:

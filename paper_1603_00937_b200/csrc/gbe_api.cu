@@ -97,6 +97,7 @@ const char* gbe_strerror(int status) {
     case GBE_EMISMATCH: return "H does not match the graph";
     case GBE_ENOMEM: return "workspace too small or allocation failed";
     case GBE_ECUDA: return g_cuda_err[0] ? g_cuda_err : "CUDA error";
+    case GBE_ELIMIT: return "problem larger than the fixed limit of this entry point (n > GBE_STATIC_MAX_N)";
     default: return "unknown status";
   }
 }
@@ -537,6 +538,16 @@ int gbe_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view*
   GBE_CUDA(cudaMemcpyAsync(out, res.p, 8, cudaMemcpyDeviceToHost, s));
   GBE_CUDA(cudaStreamSynchronize(s));
   return GBE_OK;
+}
+
+// no allocation, no synchronisation, no gbe_set_alloc_stream (which may touch the pool's attributes): checks + two launches
+int gbe_expectation_static(const gbe_graph* g, const double* D_val, const gbe_csr_view* A, void* cuda_stream,
+                           double* out_dev) {
+  if (!g || !out_dev || (!D_val && g->nnz_D > 0)) return GBE_EINVAL;
+  GBE_TRY(check_csr(A));
+  if (A->n != g->n) return GBE_EMISMATCH;
+  if (g->n > GBE_STATIC_MAX_N) return GBE_ELIMIT;
+  return gbe_launch_expectation_static(g, D_val, *A, out_dev, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int gbe_error_norms(const gbe_graph* g, const double* D_val, const double* D_ref, int64_t ld_ref, void* cuda_stream,

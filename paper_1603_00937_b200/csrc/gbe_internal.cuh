@@ -243,6 +243,9 @@ int gbe_launch_core_trace(const gbe_graph* g, const double* BD, gbe_state* st, c
 int gbe_launch_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view& A, double* row_sum, double* out,
                            cudaStream_t s);
 
+// the same with the row partials in a static device array of GBE_STATIC_MAX_N doubles: allocates nothing (gbe_observe.cu)
+int gbe_launch_expectation_static(const gbe_graph* g, const double* D_val, const gbe_csr_view& A, double* out_dev,
+                                  cudaStream_t s);
 int gbe_launch_error_norms(const gbe_graph* g, const double* D_val, const double* D_ref, int64_t ld_ref, double* row_out,
                            double* out, cudaStream_t s);
 

@@ -139,3 +139,40 @@ int gbe_launch_error_norms(const gbe_graph* g, const double* D_val, const double
   GBE_LAUNCHED();
   return GBE_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// gbe_expectation_static: <A> = Tr[D A] for callers that may not allocate (gbe.h).  The same two kernels as
+// gbe_launch_expectation; the n per-row partial sums go to a FILE-SCOPE device array instead of a pool allocation.
+//   - GBE_STATIC_MAX_N doubles = 1 MiB of device memory, held by every GPU that loads the library until the process exits;
+//   - in host code the NAME g_expect_scratch is a host-side stand-in of the symbol, not a device address: the address is
+//     looked up once per device, with that device current (cudaGetSymbolAddress), and handed to the kernels;
+//   - nothing in the array has to start at zero: k_expect_rows writes row_sum[k] for every k < n before k_expect_final
+//     reads exactly those n words, so whatever the previous call (or a larger n) left behind is never read;
+//   - every call on a device shares the array: two calls that overlap on the GPU (different streams, no dependency
+//     between them) race on it.
+static __device__ __align__(256) double g_expect_scratch[GBE_STATIC_MAX_N];
+
+namespace {
+int expect_scratch_address(double** out) {
+  static std::atomic<double*> cached[256] = {};  // per device
+  int dev = 0;
+  GBE_CUDA(cudaGetDevice(&dev));
+  const bool slot = dev >= 0 && dev < 256;
+  double* p = slot ? cached[dev].load(std::memory_order_acquire) : nullptr;
+  if (!p) {
+    GBE_CUDA(cudaGetSymbolAddress((void**)&p, g_expect_scratch));
+    if (!p) return GBE_ECUDA;
+    if (slot) cached[dev].store(p, std::memory_order_release);
+  }
+  *out = p;
+  return GBE_OK;
+}
+}  // namespace
+
+int gbe_launch_expectation_static(const gbe_graph* g, const double* D_val, const gbe_csr_view& A, double* out_dev,
+                                  cudaStream_t s) {
+  if (g->n > GBE_STATIC_MAX_N) return GBE_ELIMIT;
+  double* row_sum = nullptr;
+  GBE_TRY(expect_scratch_address(&row_sum));
+  return gbe_launch_expectation(g, D_val, A, row_sum, out_dev, s);
+}
