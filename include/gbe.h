@@ -332,8 +332,8 @@ uint64_t gbe_launch_count(void);
 size_t gbe_set_build_scratch_limit(size_t bytes);
 
 /* Largest core+halo size m_p the packed SP2 kernel takes in graphs built FROM NOW ON (see gbe_graph_set_sp2_path); larger
- * communities of the same graph run through the tiled kernel.  0 <= m <= 160 (160 = what fits one SM's shared memory;
- * default 112 = what fits half of it, so that two bins share an SM).  Process-wide tuning knob; returns the previous value,
+ * communities of the same graph run through the tiled kernel.  0 <= m <= 160 (160 = what fits one SM's shared memory,
+ * and the default: one bin of up to 16 communities per SM).  Process-wide tuning knob; returns the previous value,
  * -1 if m is out of range. */
 int32_t gbe_set_packed_max_m(int32_t m);
 
