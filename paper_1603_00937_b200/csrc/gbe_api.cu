@@ -330,13 +330,26 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
     // Iteration iters - 1 is the last one whether or not the idempotency stop fires before it (then it is a no-op):
     // only the core rows and columns of its result are read again (trace, scatter), so it runs the core tiles only.
     const bool last = it == iters - 1;
+    if (path == 3 && inplace && mode != 2) {
+      // every community packed: one launch per iteration and NO step-5 tail - the bins of launch it + 1 sum the pairs of
+      // launch it themselves (lazy decision, gbe_small.cu); the pairs alternate between two halves of `partials`
+      const int nb = g->n_pk_ctas;
+      GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, 1, [&]() -> int {
+        return gbe_launch_sp2_packed(g, w.st, in, outp, w.partials, (it & 1) * nb, nb, it, last, 2, ((it - 1) & 1) * nb,
+                                     it > 0 ? nb : 0, s);
+      }));
+      if (last)  // t1, t2 of the final X and the last log entry
+        GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials + 2 * (size_t)((it & 1) * nb), nb, s); }));
+      continue;
+    }
     if (path == 3) {
       // small communities: bins in shared memory, one launch per iteration, step 5 taken by the bin that arrives last
       // (gbe_small.cu); the larger communities of the same graph go through the tiled kernel first
       const int n_pairs = g->n_items_last_h + g->n_pk_ctas;
       GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, (g->n_items_h ? 1 : 0) + 1, [&]() -> int {
         GBE_TRY(gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, true, it & 1, s));
-        return gbe_launch_sp2_packed(g, w.st, in, outp, w.partials, g->n_items_last_h, n_pairs, it, last, mode != 2, s);
+        return gbe_launch_sp2_packed(g, w.st, in, outp, w.partials, g->n_items_last_h, n_pairs, it, last, mode != 2 ? 1 : 0,
+                                     0, 0, s);
       }));
       continue;
     }

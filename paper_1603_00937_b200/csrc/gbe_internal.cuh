@@ -224,8 +224,11 @@ int gbe_launch_sp2_resident(const gbe_graph* g, gbe_state* st, double* X0, doubl
 // steps 4 + 5, one iteration per launch, for communities with m <= g->pk_max_m (gbe_small.cu)
 int gbe_packed_max_m();  // process-wide default of the threshold (gbe_set_packed_max_m)
 int gbe_build_packed(gbe_graph* g, cudaStream_t s);
+// fused: 0 no step 5 in the kernel; 1 ticket (last bin decides); 2 lazy (the bins of the NEXT launch sum the lazy_n pairs
+// at partials[lazy_base ...] themselves: pass the previous launch's base and count, 0 for the first launch)
 int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials,
-                          int partial_base, int n_partials, int iter, bool last, bool fused, cudaStream_t s);
+                          int partial_base, int n_partials, int iter, bool last, int fused, int lazy_base, int lazy_n,
+                          cudaStream_t s);
 // step 5
 int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s);
 // step 6

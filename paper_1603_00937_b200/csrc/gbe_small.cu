@@ -34,6 +34,7 @@
 // counter; persistent CTAs with two half-size buffers (the next bin copied in under the products of this one).
 // Bound: FP64 tensor pipe inside a bin; per-bin latencies and launch latency around it.
 #include <algorithm>
+#include <cstdlib>
 #include <numeric>
 #include <queue>
 
@@ -46,6 +47,7 @@ constexpr int PK_THREADS = PK_WARPS * 32;
 constexpr int PK_UCOLS = 4;              // 8-column blocks per work unit
 constexpr int PK_MAX_ROUNDS = 32;        // units per warp (lane j of a warp fetches the code of its j-th unit)
 constexpr unsigned PK_NONE = 0xFFFFu;
+std::atomic<int> g_pk_pdl{1};  // programmatic dependent launch of the packed kernel (GBE_PK_PDL=0 in the environment: off)
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -153,16 +155,25 @@ __device__ __forceinline__ void pk_unit_store(const double (&acc)[PK_UCOLS][2], 
   }
 }
 
-// fused == 1: the last bin to publish its partial reduces all n_partials pairs and takes the decision of step 5
+// Step 5, three ways (`fused`):
+//   0  no decision here (pre-set sequence without traces, or k_trace_branch follows);
+//   1  TICKET: the last bin to publish its partial reduces all n_partials pairs and takes the decision;
+//   2  LAZY: nobody does at the end - EVERY bin of the next launch starts by summing the lazy_n pairs this launch left at
+//      partials[lazy_base ...] (same fixed order in every bin: bitwise the same t1, t2, the same decision), bin 0 also
+//      writes it to the state and the log.  No fence, no ticket, no serial tail; the sums run while the rows land.  The
+//      pairs of consecutive launches alternate between two halves of `partials` (a late bin of launch n + 1 still reads
+//      the pairs of launch n while early bins of n + 1 publish theirs).  lazy_n == 0 (first launch): the decision is in
+//      the state already (k_trace_branch after the gather); after the last launch the host runs k_trace_branch once.
 __global__ void __launch_bounds__(PK_THREADS, 1)
     k_sp2_packed(const gbe_pk_cta* __restrict__ ctas, const uint16_t* __restrict__ ucodes, gbe_state* st,
                  const double* Xin, double* Xout, double* __restrict__ partials,  // Xin == Xout when the loop runs in place
-                 int partial_base, int n_partials, int iter, int last, int fused, int code_stride, int rounds_max) {
+                 int partial_base, int n_partials, int iter, int last, int fused, int code_stride, int rounds_max,
+                 int lazy_base, int lazy_n) {
   extern __shared__ __align__(16) double xs[];  // the X_p of the bin
   __shared__ gbe_pk_cta me;
   __shared__ double red[2 * PK_WARPS];
   __shared__ int is_last;
-  __shared__ __align__(8) unsigned long long load_bar;
+  __shared__ __align__(8) unsigned long long load_bar[GBE_PK_MAX_SLOTS];  // one per community of the bin
 
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5, g = lane >> 2, q = lane & 3;
   // the bin's description (one coalesced read), this warp's unit codes (dealt on the host, longest first, to the least
@@ -170,37 +181,84 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
   // the state: independent loads, all in flight
   if (t < (int)(sizeof(gbe_pk_cta) / 4)) reinterpret_cast<int*>(&me)[t] = reinterpret_cast<const int*>(ctas + blockIdx.x)[t];
   const unsigned my_code = lane < rounds_max ? ucodes[(size_t)blockIdx.x * code_stride + lane * PK_WARPS + wid] : PK_NONE;
-  const int stop = st->stop;
-  const int branch = st->preset ? (int)st->br[iter] : st->branch;
   __syncthreads();
-  if (stop) return;  // idempotency stop already fired (A-7): X is final
   const int n_slots = me.n_slots, n_rounds = me.n_rounds;
+  // ---- everything that does not depend on the previous launch: the mbarrier, the zero rows [m, 8R) of shared memory
+  const uint32_t mbar0 = (uint32_t)__cvta_generic_to_shared(load_bar);
+  if (t < n_slots) {
+    mbar_init(mbar0 + 8u * t, 1);
+    mbar_expect_tx(mbar0 + 8u * t, (uint32_t)(me.slot[t].m * me.slot[t].ld) * 8u);
+  }
+  for (int s = 0; s < n_slots; ++s) {
+    const int m = me.slot[s].m, stride = me.slot[s].ld + 4;
+    for (int i = m * stride + t; i < 8 * me.slot[s].R * stride; i += PK_THREADS) xs[me.slot[s].soff + i] = 0.0;
+  }
+  // Programmatic dependent launch (the launcher sets the stream-serialisation attribute): the bins of iteration n + 1 are
+  // handed to the SMs while the last bins of iteration n still run, do the set-up above, and wait HERE until that grid
+  // has completed and its X_{n+1}, partials and state are visible.  Nothing above reads or writes what a launch produces
+  // (the description and the unit codes belong to the graph).  Without the attribute both instructions are no-ops.
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  int stop = st->stop;
+  int branch = st->preset ? (int)st->br[iter] : st->branch;
+  __syncthreads();   // the mbarriers are initialised
+  if (stop) return;  // idempotency stop already fired (A-7): X is final
 
   // ---- X_n of every community of the bin -> shared memory: one TMA bulk copy per row (row stride ld + 4 doubles in
   //      shared memory: conflict-free 64-bit fragment loads), issued by one thread per row, completion counted in bytes on
   //      one mbarrier - no per-piece instructions.  Rows [m, 8R) are zero: no predicate in the products.
-  const uint32_t mbar = (uint32_t)__cvta_generic_to_shared(&load_bar);
-  if (t == 0) {
-    uint32_t bytes = 0;
-    for (int s = 0; s < n_slots; ++s) bytes += (uint32_t)(me.slot[s].m * me.slot[s].ld) * 8u;
-    mbar_init(mbar, 1);
-    mbar_expect_tx(mbar, bytes);
+  // (the rows of all communities are numbered through and dealt to the threads, warp by warp: row i goes to lane i / 32
+  //  of warp i % 32.  UBLKCP takes its operands from uniform registers, so a warp issues the copies of its lanes one
+  //  after the other: every warp gets a few, none a whole column - that warp would start its products microseconds late)
+  {
+    const int ridx = wid + PK_WARPS * lane;
+    int first = 0;  // number of the first row of slot s
+    for (int s = 0; s < n_slots; ++s) {
+      const int m = me.slot[s].m, ld = me.slot[s].ld, stride = ld + 4;
+      for (int r = ridx - first; r < m; r += PK_THREADS)
+        if (r >= 0)
+          bulk_row_g2s((uint32_t)__cvta_generic_to_shared(xs + me.slot[s].soff + r * stride),
+                       Xin + me.slot[s].dense_off + (size_t)r * ld, (uint32_t)ld * 8u, mbar0 + 8u * s);
+      first = (first + m) % PK_THREADS;
+    }
   }
-  __syncthreads();
   for (int s = 0; s < n_slots; ++s) {
-    const int m = me.slot[s].m, ld = me.slot[s].ld, stride = ld + 4;
-    for (int r = t; r < m; r += PK_THREADS)
-      bulk_row_g2s((uint32_t)__cvta_generic_to_shared(xs + me.slot[s].soff + r * stride),
-                   Xin + me.slot[s].dense_off + (size_t)r * ld, (uint32_t)ld * 8u, mbar);
-    for (int i = m * stride + t; i < 8 * me.slot[s].R * stride; i += PK_THREADS) xs[me.slot[s].soff + i] = 0.0;
-    // pad columns [8R, ld) of the OUTPUT stay zero (no work unit covers them; [m, 8R) come out of the products as zeros)
-    if (ld > 8 * me.slot[s].R) {
+    const int m = me.slot[s].m, ld = me.slot[s].ld;
+    // pad columns [8R, ld) of the OUTPUT stay zero (no work unit covers them; [m, 8R) come out of the products as zeros);
+    // in place they are zero since the gather and nobody writes them
+    if (Xin != Xout && ld > 8 * me.slot[s].R) {
       double* __restrict__ out = Xout + me.slot[s].dense_off + 8 * me.slot[s].R;
       for (int i = t; i < m * 8; i += PK_THREADS) out[(size_t)(i >> 3) * ld + (i & 7)] = 0.0;
     }
   }
-  __syncthreads();  // the zero rows
-  mbar_wait(mbar, 0);
+  if (lazy_n > 0) {
+    // LAZY step 5: t1, t2 of X_iter from the pairs of the previous launch, in the order k_trace_branch uses
+    double a1 = 0.0, a2 = 0.0;
+    const double2* __restrict__ p2 = reinterpret_cast<const double2*>(partials) + lazy_base;
+    for (int i = t; i < lazy_n; i += PK_THREADS) {
+      const double2 v = __ldcg(p2 + i);
+      a1 += v.x;
+      a2 += v.y;
+    }
+    a1 = warp_sum(a1);
+    a2 = warp_sum(a2);
+    if (lane == 0) { red[wid] = a1; red[PK_WARPS + wid] = a2; }
+    __syncthreads();
+    a1 = warp_sum(red[lane]);  // every warp: the same 32 numbers in the same order
+    a2 = warp_sum(red[PK_WARPS + lane]);
+    __syncthreads();           // red is used again below
+    // gbe_trace_decide's rule (A-6, A-7) with k = iter (the state's counter is bin 0's to advance, below)
+    const double idem_tol = st->idem_tol, n_occ = st->n_occ;
+    if (idem_tol >= 0.0 && iter >= 1 && fabs(a1 - a2) <= idem_tol) stop = 1;
+    else if (!st->preset) branch = (fabs(a2 - n_occ) < fabs(2.0 * a1 - a2 - n_occ)) ? 0 : 1;
+    if (blockIdx.x == 0 && t == 0) gbe_trace_decide(st, a1, a2);
+    if (stop) {  // X_iter is final; no copy may be in flight when the CTA retires
+      if (t < n_slots) mbar_wait(mbar0 + 8u * t, 0);
+      return;
+    }
+  }
+  // (no wait here: a unit waits for the rows of ITS community only - the largest community of a bin sits in slot 0, its
+  //  copies are issued first and its units are the first of every warp's list, so the products start while the rest lands)
 
   // ---- Y = X X^T unit by unit (one 8-row block x up to four 8-column blocks on or above the diagonal); the unit's part
   //      of X_{n+1} = Y or 2 X_n - Y goes straight from the accumulators to the other dense buffer, direct + mirrored,
@@ -215,6 +273,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
     const int kmax = (m + 3) & ~3;  // columns >= m are zero
     // the last iteration needs the core rows and (through the mirror) the core columns only (Eq.(6))
     if (code == PK_NONE || (last && bi * 8 >= nc)) continue;
+    mbar_wait(mbar0 + 8u * s, 0);
     const double* x0 = xs + me.slot[s].soff;
     const double* pa = x0 + (size_t)(bi * 8 + g) * stride + q;
     const double* pb = x0 + (size_t)(bj * 8 + g) * stride + q;
@@ -243,6 +302,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
   s1 = warp_sum(s1);
   s2 = warp_sum(s2);
   if (lane == 0) { red[wid] = s1; red[PK_WARPS + wid] = s2; }
+  if (wid == 1 && lane < n_slots) mbar_wait(mbar0 + 8u * lane, 0);  // no copy in flight when the CTA retires
   __syncthreads();
   if (wid == 0) {
     const double a = warp_sum(red[lane]);
@@ -252,14 +312,14 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
       out[0] = a;
       out[1] = b;
       int lastflag = 0;
-      if (fused) {
+      if (fused == 1) {
         __threadfence();  // the pair is visible before the ticket is taken
         lastflag = atomicAdd(&st->ticket, 1u) == gridDim.x - 1;
       }
       is_last = lastflag;
     }
   }
-  if (!fused) return;
+  if (fused != 1) return;
   __syncthreads();
   if (!is_last) return;
 
@@ -451,7 +511,8 @@ int gbe_build_packed(gbe_graph* g, cudaStream_t s) {
 // One SP2 iteration of the packed communities.  partial_base: index of the first bin's pair in `partials` (the pairs of the
 // tiled kernel, if it runs in the same iteration, sit in front); n_partials: all pairs of the iteration.
 int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials,
-                          int partial_base, int n_partials, int iter, bool last, bool fused, cudaStream_t s) {
+                          int partial_base, int n_partials, int iter, bool last, int fused, int lazy_base, int lazy_n,
+                          cudaStream_t s) {
   if (g->n_pk_ctas == 0) return GBE_OK;
   static gbe_device_once configured;
   if (configured.first()) {
@@ -460,11 +521,24 @@ int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, 
     GBE_CUDA(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     GBE_CUDA(cudaFuncSetAttribute(k_sp2_packed, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max - 2048));
     GBE_CUDA(cudaFuncSetAttribute(k_sp2_packed, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    if (const char* e = getenv("GBE_PK_PDL")) g_pk_pdl.store(atoi(e) != 0, std::memory_order_relaxed);
   }
   const gbe_pk_class& a = g->pk[0];
-  k_sp2_packed<<<a.n_ctas, PK_THREADS, a.smem_bytes, s>>>(a.ctas, a.codes, st, Xin, Xout, partials, partial_base,
-                                                         n_partials, iter, last ? 1 : 0, fused ? 1 : 0, a.code_stride,
-                                                         a.rounds_max);
+  // programmatic stream serialisation: the grid may be scheduled before the previous kernel of the stream has finished;
+  // it synchronises with it in the kernel (griddepcontrol.wait) after its set-up
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)a.n_ctas);
+  cfg.blockDim = dim3(PK_THREADS);
+  cfg.dynamicSmemBytes = a.smem_bytes;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = g_pk_pdl.load(std::memory_order_relaxed) ? 1 : 0;
+  GBE_CUDA(cudaLaunchKernelEx(&cfg, k_sp2_packed, (const gbe_pk_cta*)a.ctas, (const uint16_t*)a.codes, st, Xin, Xout,
+                              partials, partial_base, n_partials, iter, last ? 1 : 0, fused, (int)a.code_stride,
+                              (int)a.rounds_max, lazy_base, lazy_n));
   GBE_LAUNCHED();
   return GBE_OK;
 }

@@ -850,9 +850,10 @@ def test_density_is_capturable_in_a_cuda_graph(gbe, sp2_path):
 
 
 def test_packed_kernel_launches_and_reproducibility(gbe):
-    """The packed kernel (gbe_small.cu): ONE launch per SP2 iteration - the bin that publishes its trace partial last takes
-    step 5's decision, whichever bin that is the sums are taken in the same order - so 600 small communities (more than
-    can be co-resident, no grid barrier possible) take 40 launches for the loop instead of 80."""
+    """The packed kernel (gbe_small.cu): ONE launch per SP2 iteration - every bin of launch n + 1 starts by summing the
+    trace pairs launch n left (the same fixed order in every bin, so bitwise the same decision everywhere; one trace
+    kernel after the last launch) - so 600 small communities (more than can be co-resident, no grid barrier possible)
+    take 40 + 1 launches for the loop instead of 80."""
     import torch
     s = gi.chain(4800, 600, seed=5)
     rp, ci = o.build_graph(s.H, s.tau)
@@ -863,7 +864,7 @@ def test_packed_kernel_launches_and_reproducibility(gbe):
     n0 = gbe.gbe_launch_count()
     D0, log0 = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
     torch.cuda.synchronize()
-    assert gbe.gbe_launch_count() - n0 == 2 + 1 + 2 + s.iters + 1  # bounds(2), gather, init + trace of X_0, loop, scatter
+    assert gbe.gbe_launch_count() - n0 == 2 + 1 + 2 + s.iters + 1 + 1  # bounds(2), gather, init + trace of X_0, loop, final trace, scatter
     check_density(D0.cpu().numpy(), log0, r)
     for _ in range(10):
         D1, log1 = gbe.gbe_density(Hd, g, s.n_occ, s.iters)
