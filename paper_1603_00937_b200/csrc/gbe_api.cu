@@ -105,7 +105,7 @@ const char* gbe_strerror(int status) {
 void gbe_free_graph(gbe_graph* g) {
   if (!g) return;
   void* ptrs[] = {g->S_row_ptr, g->S_col,     g->sub_ptr,  g->sub_idx,  g->ncore,    g->msize, g->dense_off, g->D_row_ptr,
-                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->items_h, g->items_last_h, g->pk[0].ctas, g->pk[0].codes, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va, g->tmaps, g->items_w, g->items_last_w};
+                  g->D_col,     g->scat_base, g->scat_pos, g->scat_ofs, g->row_part, g->items, g->items_last, g->items_h, g->items_last_h, g->pk[0].ctas, g->pk[0].codes, g->pk[0].rows, g->gitems, g->row_src, g->row_nc, g->H_rp, g->H_ci, g->H_va, g->tmaps, g->items_w, g->items_last_w};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   delete g;

@@ -92,12 +92,18 @@ struct gbe_pk_slot {  // one community of a bin (40 bytes)
   int64_t dense_off;     // element offset of X_p in a dense buffer
 };
 struct gbe_pk_cta {  // one bin: its communities (its work units sit in the class's code array, [bin][round][warp])
-  int32_t n_slots, n_rounds, smem_doubles, pad1_;  // n_rounds: longest unit list of a warp; shared memory of the bin
+  int32_t n_slots, n_rounds, row0, n_rows;  // n_rounds: longest unit list of a warp; the bin's entries in the row table
   gbe_pk_slot slot[GBE_PK_MAX_SLOTS];
+};
+struct gbe_pk_row {  // one matrix row of a bin = one TMA bulk copy (16 bytes)
+  uint32_t soff;     // byte offset of the row in the bin's shared memory
+  uint32_t bytes;    // ld * 8 | slot << 24
+  int64_t goff;      // element offset of the row in a dense buffer
 };
 struct gbe_pk_class {  // the bins of one launch of the packed kernel (device arrays owned by the graph)
   gbe_pk_cta* ctas = nullptr;
   uint16_t* codes = nullptr;
+  gbe_pk_row* rows = nullptr;  // all bins, slot 0 of a bin first
   int32_t n_ctas = 0, warps = 0, rounds_max = 0, code_stride = 0;
   size_t smem_bytes = 0;
 };

@@ -47,6 +47,8 @@ constexpr int PK_THREADS = PK_WARPS * 32;
 constexpr int PK_UCOLS = 4;              // 8-column blocks per work unit
 constexpr int PK_MAX_ROUNDS = 32;        // units per warp (lane j of a warp fetches the code of its j-th unit)
 constexpr unsigned PK_NONE = 0xFFFFu;
+constexpr int PK_PAD = 4;                // shared-memory row stride = ld + 4 doubles (ld is a multiple of 16): the 16 doubles a
+                                         // half warp loads with LDS.64 (4 rows x 4 columns) fall into distinct banks
 std::atomic<int> g_pk_pdl{1};  // programmatic dependent launch of the packed kernel (GBE_PK_PDL=0 in the environment: off)
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
@@ -165,94 +167,103 @@ __device__ __forceinline__ void pk_unit_store(const double (&acc)[PK_UCOLS][2], 
 //      the pairs of launch n while early bins of n + 1 publish theirs).  lazy_n == 0 (first launch): the decision is in
 //      the state already (k_trace_branch after the gather); after the last launch the host runs k_trace_branch once.
 __global__ void __launch_bounds__(PK_THREADS, 1)
-    k_sp2_packed(const gbe_pk_cta* __restrict__ ctas, const uint16_t* __restrict__ ucodes, gbe_state* st,
+    k_sp2_packed(const gbe_pk_cta* __restrict__ ctas, const uint16_t* __restrict__ ucodes,
+                 const gbe_pk_row* __restrict__ rows, gbe_state* st,
                  const double* Xin, double* Xout, double* __restrict__ partials,  // Xin == Xout when the loop runs in place
                  int partial_base, int n_partials, int iter, int last, int fused, int code_stride, int rounds_max,
                  int lazy_base, int lazy_n) {
   extern __shared__ __align__(16) double xs[];  // the X_p of the bin
   __shared__ gbe_pk_cta me;
-  __shared__ double red[2 * PK_WARPS];
+  __shared__ double red[2 * PK_WARPS], lazy_red[2 * PK_WARPS];
   __shared__ int is_last;
   __shared__ __align__(8) unsigned long long load_bar[GBE_PK_MAX_SLOTS];  // one per community of the bin
 
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5, g = lane >> 2, q = lane & 3;
   // the bin's description (one coalesced read), this warp's unit codes (dealt on the host, longest first, to the least
-  // loaded warp; lane j holds the j-th one; fixed stride per bin, so the address does not wait for the description) and
-  // the state: independent loads, all in flight
+  // loaded warp; lane j holds the j-th one; fixed stride per bin, so the address does not wait for the description):
+  // independent loads, all in flight
   if (t < (int)(sizeof(gbe_pk_cta) / 4)) reinterpret_cast<int*>(&me)[t] = reinterpret_cast<const int*>(ctas + blockIdx.x)[t];
   const unsigned my_code = lane < rounds_max ? ucodes[(size_t)blockIdx.x * code_stride + lane * PK_WARPS + wid] : PK_NONE;
   __syncthreads();
-  const int n_slots = me.n_slots, n_rounds = me.n_rounds;
-  // ---- everything that does not depend on the previous launch: the mbarrier, the zero rows [m, 8R) of shared memory
+  const int n_slots = me.n_slots, n_rounds = me.n_rounds, n_rows = me.n_rows;
+  // ---- everything that does not depend on the previous launch: the mbarriers, the zero rows [m, 8R) of shared memory,
+  //      this thread's entry of the row table (the rows of the bin are dealt warp by warp: entry i goes to lane i / 32 of
+  //      warp i % 32.  UBLKCP takes its operands from uniform registers, so a warp issues the copies of its lanes one
+  //      after the other: every warp gets a few, none a whole column - that warp would start its products late)
   const uint32_t mbar0 = (uint32_t)__cvta_generic_to_shared(load_bar);
+  const uint32_t xs0 = (uint32_t)__cvta_generic_to_shared(xs);
   if (t < n_slots) {
     mbar_init(mbar0 + 8u * t, 1);
     mbar_expect_tx(mbar0 + 8u * t, (uint32_t)(me.slot[t].m * me.slot[t].ld) * 8u);
   }
+  const int ridx = wid + PK_WARPS * lane;
+  gbe_pk_row my_row = {0u, 0u, 0};
+  if (ridx < n_rows) my_row = rows[me.row0 + ridx];
   for (int s = 0; s < n_slots; ++s) {
-    const int m = me.slot[s].m, stride = me.slot[s].ld + 4;
+    const int m = me.slot[s].m, stride = me.slot[s].ld + PK_PAD;
     for (int i = m * stride + t; i < 8 * me.slot[s].R * stride; i += PK_THREADS) xs[me.slot[s].soff + i] = 0.0;
   }
   // Programmatic dependent launch (the launcher sets the stream-serialisation attribute): the bins of iteration n + 1 are
   // handed to the SMs while the last bins of iteration n still run, do the set-up above, and wait HERE until that grid
   // has completed and its X_{n+1}, partials and state are visible.  Nothing above reads or writes what a launch produces
-  // (the description and the unit codes belong to the graph).  Without the attribute both instructions are no-ops.
+  // (the description, the unit codes and the row table belong to the graph).  Without the attribute both instructions
+  // are no-ops.
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
+  // the state and (lazy step 5) this thread's pair(s) of the previous launch: all requested at once, used after the
+  // copies are issued
   int stop = st->stop;
-  int branch = st->preset ? (int)st->br[iter] : st->branch;
-  __syncthreads();   // the mbarriers are initialised
-  if (stop) return;  // idempotency stop already fired (A-7): X is final
-
-  // ---- X_n of every community of the bin -> shared memory: one TMA bulk copy per row (row stride ld + 4 doubles in
-  //      shared memory: conflict-free 64-bit fragment loads), issued by one thread per row, completion counted in bytes on
-  //      one mbarrier - no per-piece instructions.  Rows [m, 8R) are zero: no predicate in the products.
-  // (the rows of all communities are numbered through and dealt to the threads, warp by warp: row i goes to lane i / 32
-  //  of warp i % 32.  UBLKCP takes its operands from uniform registers, so a warp issues the copies of its lanes one
-  //  after the other: every warp gets a few, none a whole column - that warp would start its products microseconds late)
-  {
-    const int ridx = wid + PK_WARPS * lane;
-    int first = 0;  // number of the first row of slot s
-    for (int s = 0; s < n_slots; ++s) {
-      const int m = me.slot[s].m, ld = me.slot[s].ld, stride = ld + 4;
-      for (int r = ridx - first; r < m; r += PK_THREADS)
-        if (r >= 0)
-          bulk_row_g2s((uint32_t)__cvta_generic_to_shared(xs + me.slot[s].soff + r * stride),
-                       Xin + me.slot[s].dense_off + (size_t)r * ld, (uint32_t)ld * 8u, mbar0 + 8u * s);
-      first = (first + m) % PK_THREADS;
-    }
-  }
-  for (int s = 0; s < n_slots; ++s) {
-    const int m = me.slot[s].m, ld = me.slot[s].ld;
-    // pad columns [8R, ld) of the OUTPUT stay zero (no work unit covers them; [m, 8R) come out of the products as zeros);
-    // in place they are zero since the gather and nobody writes them
-    if (Xin != Xout && ld > 8 * me.slot[s].R) {
-      double* __restrict__ out = Xout + me.slot[s].dense_off + 8 * me.slot[s].R;
-      for (int i = t; i < m * 8; i += PK_THREADS) out[(size_t)(i >> 3) * ld + (i & 7)] = 0.0;
-    }
-  }
+  const int preset = st->preset, br_state = st->branch, br_preset = iter < GBE_MAX_ITERS ? (int)st->br[iter] : 0;
+  const double idem_tol = st->idem_tol, n_occ = st->n_occ;
+  double a1 = 0.0, a2 = 0.0;
   if (lazy_n > 0) {
-    // LAZY step 5: t1, t2 of X_iter from the pairs of the previous launch, in the order k_trace_branch uses
-    double a1 = 0.0, a2 = 0.0;
     const double2* __restrict__ p2 = reinterpret_cast<const double2*>(partials) + lazy_base;
     for (int i = t; i < lazy_n; i += PK_THREADS) {
       const double2 v = __ldcg(p2 + i);
       a1 += v.x;
       a2 += v.y;
     }
-    a1 = warp_sum(a1);
-    a2 = warp_sum(a2);
-    if (lane == 0) { red[wid] = a1; red[PK_WARPS + wid] = a2; }
+  }
+  int branch = preset ? br_preset : br_state;
+  __syncthreads();   // the mbarriers are initialised
+  if (stop) return;  // idempotency stop already fired (A-7): X is final
+
+  // ---- X_n of every community of the bin -> shared memory: one TMA bulk copy per row (row stride ld + 4 doubles in
+  //      shared memory: conflict-free 64-bit fragment loads), completion counted in bytes on the community's mbarrier
+  //      - no per-piece instructions.  Rows [m, 8R) are zero: no predicate in the products.
+  if (ridx < n_rows)
+    bulk_row_g2s(xs0 + my_row.soff, Xin + my_row.goff, my_row.bytes & 0xFFFFFFu, mbar0 + 8u * (my_row.bytes >> 24));
+  for (int i = ridx + PK_THREADS; i < n_rows; i += PK_THREADS) {  // bins of more than 1,024 rows
+    const gbe_pk_row e = rows[me.row0 + i];
+    bulk_row_g2s(xs0 + e.soff, Xin + e.goff, e.bytes & 0xFFFFFFu, mbar0 + 8u * (e.bytes >> 24));
+  }
+  if (Xin != Xout) {
+    // pad columns [8R, ld) of the OUTPUT stay zero (no work unit covers them; [m, 8R) come out of the products as zeros);
+    // in place they are zero since the gather and nobody writes them
+    for (int s = 0; s < n_slots; ++s) {
+      const int m = me.slot[s].m, ld = me.slot[s].ld;
+      if (ld > 8 * me.slot[s].R) {
+        double* __restrict__ out = Xout + me.slot[s].dense_off + 8 * me.slot[s].R;
+        for (int i = t; i < m * 8; i += PK_THREADS) out[(size_t)(i >> 3) * ld + (i & 7)] = 0.0;
+      }
+    }
+  }
+  if (lazy_n > 0) {
+    // LAZY step 5: t1, t2 of X_iter from the pairs of the previous launch
+    if (wid * 32 < lazy_n) {  // (a warp without pairs holds zeros)
+      a1 = warp_sum(a1);
+      a2 = warp_sum(a2);
+    }
+    if (lane == 0) { lazy_red[wid] = a1; lazy_red[PK_WARPS + wid] = a2; }
     __syncthreads();
-    a1 = warp_sum(red[lane]);  // every warp: the same 32 numbers in the same order
-    a2 = warp_sum(red[PK_WARPS + lane]);
-    __syncthreads();           // red is used again below
+    a1 = warp_sum(lazy_red[lane]);  // every warp: the same 32 numbers in the same order
+    a2 = warp_sum(lazy_red[PK_WARPS + lane]);
     // gbe_trace_decide's rule (A-6, A-7) with k = iter (the state's counter is bin 0's to advance, below)
-    const double idem_tol = st->idem_tol, n_occ = st->n_occ;
     if (idem_tol >= 0.0 && iter >= 1 && fabs(a1 - a2) <= idem_tol) stop = 1;
-    else if (!st->preset) branch = (fabs(a2 - n_occ) < fabs(2.0 * a1 - a2 - n_occ)) ? 0 : 1;
+    else if (!preset) branch = (fabs(a2 - n_occ) < fabs(2.0 * a1 - a2 - n_occ)) ? 0 : 1;
     if (blockIdx.x == 0 && t == 0) gbe_trace_decide(st, a1, a2);
     if (stop) {  // X_iter is final; no copy may be in flight when the CTA retires
+      __syncthreads();
       if (t < n_slots) mbar_wait(mbar0 + 8u * t, 0);
       return;
     }
@@ -269,7 +280,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
     const unsigned code = __shfl_sync(0xffffffffu, my_code, round);
     const int s = code & 15, bi = (code >> 4) & 31, bj = bi + 4 * ((code >> 9) & 7), nb = 1 + ((code >> 12) & 3);
     const bool tall = (code >> 14) & 1, firstu = bj == bi;
-    const int nc = me.slot[s].nc, m = me.slot[s].m, ld = me.slot[s].ld, stride = ld + 4;
+    const int nc = me.slot[s].nc, m = me.slot[s].m, ld = me.slot[s].ld, stride = ld + PK_PAD;
     const int kmax = (m + 3) & ~3;  // columns >= m are zero
     // the last iteration needs the core rows and (through the mirror) the core columns only (Eq.(6))
     if (code == PK_NONE || (last && bi * 8 >= nc)) continue;
@@ -325,7 +336,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
 
   // ---- step 5, by the bin that arrived last: all partials of this iteration (tiled kernel's and bins') in a fixed order
   __threadfence();
-  double a1 = 0.0, a2 = 0.0;
+  a1 = a2 = 0.0;
   const double2* __restrict__ p2 = reinterpret_cast<const double2*>(partials);
   for (int i = t; i < n_partials; i += PK_THREADS) {
     const double2 v = __ldcg(p2 + i);
@@ -357,7 +368,7 @@ inline int64_t dmma_of(int m, int /*ld*/) {  // DMMA instructions of one X X^T: 
   const int64_t R = (m + 7) / 8;
   return R * (R + 1) / 2 * ((m + 3) / 4);
 }
-inline size_t smem_doubles_of(int m, int ld) { return (size_t)((m + 7) / 8 * 8) * (ld + 4); }  // 8R rows of ld + 4 doubles
+inline size_t smem_doubles_of(int m, int ld) { return (size_t)((m + 7) / 8 * 8) * (ld + PK_PAD); }  // 8R rows of ld + 4 doubles
 
 template <typename T>
 int upload(const std::vector<T>& h, T** d, cudaStream_t s) {
@@ -446,6 +457,7 @@ int gbe_build_packed(gbe_graph* g, cudaStream_t s) {
   std::iota(border.begin(), border.end(), 0);
   std::stable_sort(border.begin(), border.end(), [&](int a, int b) { return bins[a].load > bins[b].load; });
   std::vector<gbe_pk_cta> h_ctas;
+  std::vector<gbe_pk_row> h_rows;
   std::vector<std::vector<uint16_t>> grids;
   size_t smem_need = 0;
   int rounds_max = 0;
@@ -454,12 +466,16 @@ int gbe_build_packed(gbe_graph* g, cudaStream_t s) {
     if (b.ps.empty()) continue;
     gbe_pk_cta c = {};
     c.n_slots = (int32_t)b.ps.size();
+    c.row0 = (int32_t)h_rows.size();
     std::vector<Unit> units;
     size_t soff = 0;
     for (int k = 0; k < (int)b.ps.size(); ++k) {
       const int p = b.ps[k], m = g->h_m[p], ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN, R = (m + 7) / 8;
       c.slot[k] = {p, m, g->h_ncore[p], ld, (int32_t)soff, (int16_t)R, 0, 0, 0, g->h_dense_off[p]};
-      soff += (size_t)(8 * R) * (ld + 4);
+      for (int r = 0; r < m; ++r)
+        h_rows.push_back({(uint32_t)((soff + (size_t)r * (ld + PK_PAD)) * 8), (uint32_t)(ld * 8) | ((uint32_t)k << 24),
+                          g->h_dense_off[p] + (int64_t)r * ld});
+      soff += (size_t)(8 * R) * (ld + PK_PAD);
       // row blocks in pairs (2 x up to 4 blocks per unit: 6 fragment loads per 8 DMMA); an odd last row block alone
       for (int bi = 0; bi < R; bi += 2) {
         const int tall = bi + 1 < R ? 1 : 0;
@@ -469,7 +485,7 @@ int gbe_build_packed(gbe_graph* g, cudaStream_t s) {
         }
       }
     }
-    c.smem_doubles = (int32_t)soff;
+    c.n_rows = (int32_t)h_rows.size() - c.row0;
     smem_need = std::max(smem_need, soff * sizeof(double));
     // the units of the bin onto the 32 warps: longest first, always to the least loaded warp - ties to the warp whose SM
     // sub-partition (warp index mod 4: each has its own FP64 tensor pipe) carries the least; codes stored round-major
@@ -504,6 +520,7 @@ int gbe_build_packed(gbe_graph* g, cudaStream_t s) {
   out.code_stride = rounds_max * PK_WARPS;
   GBE_TRY(upload(h_ctas, &out.ctas, s));
   GBE_TRY(upload(h_codes, &out.codes, s));
+  GBE_TRY(upload(h_rows, &out.rows, s));
   g->n_pk_ctas = out.n_ctas;
   return GBE_OK;
 }
@@ -536,7 +553,8 @@ int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, 
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = g_pk_pdl.load(std::memory_order_relaxed) ? 1 : 0;
-  GBE_CUDA(cudaLaunchKernelEx(&cfg, k_sp2_packed, (const gbe_pk_cta*)a.ctas, (const uint16_t*)a.codes, st, Xin, Xout,
+  GBE_CUDA(cudaLaunchKernelEx(&cfg, k_sp2_packed, (const gbe_pk_cta*)a.ctas, (const uint16_t*)a.codes,
+                              (const gbe_pk_row*)a.rows, st, Xin, Xout,
                               partials, partial_base, n_partials, iter, last ? 1 : 0, fused, (int)a.code_stride,
                               (int)a.rounds_max, lazy_base, lazy_n));
   GBE_LAUNCHED();
