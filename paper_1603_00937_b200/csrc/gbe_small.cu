@@ -10,29 +10,44 @@
 //     on the host: longest processing time first onto exactly k x SM-count bins (a launch is k equally heavy waves),
 //     bounded by shared memory;
 //   - every X_p of the bin is copied to shared memory by TMA: one bulk copy (cp.async.bulk, SASS UBLKCP) per matrix row,
-//     issued by one thread per row, counted in bytes on an mbarrier; row stride ld_p + 4 doubles: conflict-free 64-bit
-//     fragment loads.  The batch is read exactly once per iteration;
+//     described by a per-bin ROW TABLE built with the graph (shared-memory offset, dense offset, bytes, community): a
+//     thread reads its entry before the launch dependency resolves and issues one copy - no per-community loops.  UBLKCP
+//     takes uniform operands, so a warp issues its lanes' copies one by one: the rows are dealt over all 32 warps.  Each
+//     community counts its bytes on an mbarrier of its own, and a work unit waits for ITS community only (the largest
+//     sits in slot 0 and lands first).  Row stride ld_p + 4 doubles: conflict-free 64-bit fragment loads.  The batch is
+//     read exactly once per iteration;
 //   - Y = X X^T on FP64 tensor cores (mma.sync.m8n8k4.f64): a work unit is two 8-row blocks x up to four 8-column blocks
 //     on or above the diagonal (6 fragment loads per 8 DMMA); the host deals the units of the bin, longest first, to the
 //     least loaded warp, ties to the least loaded SM sub-partition (each has its own DMMA pipe).  A unit's part of
 //     X_{n+1} goes straight from the accumulators to the dense buffer (direct + mirrored store; X_n in shared memory
 //     stays intact), with the core-row traces of X_{n+1} (t1 = sum X_ii, t2 = sum_c X_ic^2 = Tr_core X^2 for symmetric
 //     X) taken on the way and summed per bin in a fixed order;
-//   - a bin has ALL of its X_p in shared memory before it stores anything, so when every community of the graph is packed
-//     the iteration runs IN PLACE in one dense buffer;
-//   - step 5 fused: the bin that publishes its partial LAST (one ticket per bin; the fence orders 16 bytes) sums all
-//     partials of the iteration in a fixed order and takes the branch decision exactly as k_trace_branch does - one
-//     launch per SP2 iteration instead of two.  Which CTA is last does not change the order of the sum: results are
-//     reproducible bit for bit.
-// Communities with m_p > 160 of the same graph go through the tiled kernel in the same iteration (launched first; its
-// partials sit in front of the bins' and enter the same sum).
-// Measured on B200 with per-warp %globaltimer stamps: inside a bin the products run at the DMMA issue rate
-// of the sub-partitions that have work; what is left is per bin and serial - description 0.7 us, the copy in 2 - 5 us
-// (the TMA unit retires one row copy per ~17 cycles), trace + ticket 1.2 us - and ~10 us from one launch to the next.
+//   - a unit stores to X_p only after all of X_p is in shared memory (its mbarrier), so when every community of the
+//     graph is packed the iteration runs IN PLACE in one dense buffer;
+//   - programmatic dependent launch: the bins of iteration n + 1 are handed to the SMs while the last bins of iteration
+//     n still run, set themselves up (description, row table entry, mbarriers, zero rows) and wait in the kernel
+//     (griddepcontrol.wait) for iteration n to complete;
+//   - step 5 LAZY (every community packed): a bin ends by storing its trace pair, nothing else.  Every bin of the NEXT
+//     launch starts by summing all pairs of the previous one - the same fixed order in every bin, so bitwise the same
+//     t1, t2 and the same branch everywhere - while its rows land; bin 0 also writes the decision to the state and the
+//     log.  No fence, no ticket, no serial tail after the last bin; one k_trace_branch after the last launch.  (With
+//     larger communities in the same graph the tiled kernel runs first in the iteration and the decision is taken by the
+//     bin that publishes its pair LAST - one ticket per bin; its pairs sit in front of the bins' and enter the same
+//     sum.)  Either way ONE launch per SP2 iteration instead of two, and results reproducible bit for bit.
+// Measured on B200 (profiles/r02_small_m_ncu.md; per-warp %globaltimer stamps in a throw-away build): 1,024 communities of
+// m = 28/69/123 take 1.38 ms per density call (tiled kernels 2.55 ms, first version of this kernel 1.85 ms).  Per bin:
+// ~1.4 us set-up (hidden behind the previous launch for the first wave), rows landed 2.3 - 2.6 us after the dependency
+// resolves (the pair sum runs meanwhile), 10 - 11 us of products and stores, 0.4 us for the pair.  In the product phase
+// the FP64 tensor pipe is busy about 60 % of the time (43 % over the launch): every non-DMMA instruction costs the
+// sub-partition ~1.4 DMMA-pipe cycles, and with K = m ~ 70 a unit is 18 k-steps of 8 DMMA against ~70 instructions of
+// unit decode, update and store per 8 x 8 block.
 // Tried and dropped, none faster: 16 warps and two bins per SM (the two start in phase and share the pipes); copies in
 // column quarters with the first unit started on the first quarter; self-scheduling of the units through a shared-memory
-// counter; persistent CTAs with two half-size buffers (the next bin copied in under the products of this one).
-// Bound: FP64 tensor pipe inside a bin; per-bin latencies and launch latency around it.
+// counter; persistent CTAs with two half-size buffers (the next bin copied in under the products of this one); every
+// warp summing all pairs itself (no CTA barrier, but 32 x the pair traffic: 1.9 ms); 128-bit fragment loads feeding two
+// k-steps (row stride ld + 8, k order 0 2 4 6 | 1 3 5 7, addresses formed in the asm: half the LDS and a third fewer
+// instructions in the main loop, yet 5 - 9 % slower end to end).
+// Bound: FP64 tensor pipe + instruction issue inside a bin; per-bin latencies around it.
 #include <algorithm>
 #include <cstdlib>
 #include <numeric>
