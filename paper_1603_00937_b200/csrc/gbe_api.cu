@@ -2,6 +2,7 @@
 // Every step of the path runs in the kernels of gbe_{bounds,graph,halo,gather,x2,trace,scatter}.cu.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -11,6 +12,8 @@ std::atomic<uint64_t> g_gbe_launches{0};
 // communities up to this size go to the packed kernel (gbe_small.cu); 116: the largest whose X fits half an SM's shared
 // memory, so that two bins share an SM
 static std::atomic<int32_t> g_pk_max_m{GBE_PK_MAX_M};
+// programmatic dependent launch on the tiled SP2 path (GBE_X2_PDL=0 in the environment switches it off: debugging)
+static std::atomic<int> g_x2_pdl{[] { const char* e = getenv("GBE_X2_PDL"); return e ? (atoi(e) != 0 ? 1 : 0) : 1; }()};
 int gbe_packed_max_m() { return g_pk_max_m.load(); }
 
 namespace {
@@ -354,10 +357,14 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
       continue;
     }
     const int n_part_it = g->n_items_last;  // one packed partial per tile with a core row, in every iteration
+    // programmatic dependent launch: behind k_trace_branch the product of iteration it + 1 starts while the decision of
+    // iteration it + 1 is being taken (GBE_PDL_EARLY); without traces an X^2 launch follows an X^2 launch and waits for
+    // it before it reads X (GBE_PDL_TOP)
+    const int pdl = g_x2_pdl.load(std::memory_order_relaxed) ? (mode != 2 ? GBE_PDL_EARLY : GBE_PDL_TOP) : GBE_PDL_NONE;
     GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, g->n_items ? 1 : 0,
-                  [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, false, it & 1, s); }));
+                  [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, false, it & 1, s, pdl); }));
     if (mode != 2)
-      GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, n_part_it, s); }));
+      GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials, n_part_it, s, pdl ? GBE_PDL_TOP : GBE_PDL_NONE); }));
   }
   if (mode == 2) {  // one trace kernel at the end: t1, t2 of the final X for the log (written at index iters)
     const int n_pairs = iters == 0 ? g->n_gitems : (path == 3 ? g->n_items_last_h + g->n_pk_ctas : g->n_items_last);

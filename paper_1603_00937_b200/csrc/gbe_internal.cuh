@@ -193,6 +193,49 @@ struct gbe_graph {
 };
 
 // ----------------------------------------------------------------------------------------------
+// programmatic dependent launch (sm_90+): a kernel launched with the stream-serialisation attribute may become resident
+// once every CTA of the previous kernel of the stream has executed griddepcontrol.launch_dependents (or exited); it must
+// execute griddepcontrol.wait before it touches anything the previous kernel (or, transitively, an earlier one that the
+// previous kernel itself did not wait for) produces.  Without the attribute both instructions are no-ops.
+//   GBE_PDL_TOP    the kernel waits before it reads anything a launch produces (safe behind any kernel)
+//   GBE_PDL_EARLY  X^2 kernel behind k_trace_branch only: k_trace_branch waits for the previous X^2 launch BEFORE it lets
+//                  its dependents go, so X_n is complete when this grid starts; it runs its product first and waits
+//                  (for the branch of this iteration) before its epilogue
+// ----------------------------------------------------------------------------------------------
+enum { GBE_PDL_NONE = 0, GBE_PDL_TOP = 1, GBE_PDL_EARLY = 2 };
+#ifdef __CUDACC__
+__device__ __forceinline__ void gbe_griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void gbe_griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// state words another kernel may be writing while this one runs, or has written since this one started: never cached
+// in L1, never merged with an earlier read by the compiler
+__device__ __forceinline__ int gbe_ld_state(const int32_t* p) {
+  int v;
+  asm volatile("ld.global.cg.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ int gbe_ld_state(const uint8_t* p) {
+  int v;
+  asm volatile("ld.global.cg.u8 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t gbe_launch_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl,
+                                     Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+#endif
+
+// ----------------------------------------------------------------------------------------------
 // kernel launchers (each file holds one step of DESIGN.md section 1)
 // ----------------------------------------------------------------------------------------------
 // step 0
@@ -215,10 +258,12 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
 // iter: index n of the update X_n -> X_{n+1} (selects br[n] when the sequence is preset)
 // hybrid: only the tiles of the communities the packed kernel does not take (items_h / items_last_h)
 // buffer: which dense buffer Xin is (0 or 1: selects the tensor maps)
+// pdl: programmatic dependent launch (GBE_PDL_*): the grid may become resident before the previous kernel of the stream
+// has finished and synchronises with it in the kernel
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                  bool last, bool hybrid, int buffer, cudaStream_t s);
+                  bool last, bool hybrid, int buffer, cudaStream_t s, int pdl = 0);
 int gbe_launch_x2_items(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                        const gbe_tile_item* items, int n_items, int buffer, cudaStream_t s);
+                        const gbe_tile_item* items, int n_items, int buffer, cudaStream_t s, int pdl = 0);
 int gbe_plan_waves(const gbe_graph* g, size_t cap_elems, cudaStream_t s);  // gbe_halo.cu
 int gbe_x2_build_tmaps(gbe_graph* g, cudaStream_t s);                                        // once per graph
 int gbe_x2_prepare(const gbe_graph* g, const double* X0, const double* X1, cudaStream_t s);  // once per density call
@@ -236,7 +281,7 @@ int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, 
                           int partial_base, int n_partials, int iter, bool last, int fused, int lazy_base, int lazy_n,
                           cudaStream_t s);
 // step 5
-int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s);
+int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s, int pdl = 0);
 // step 6
 int gbe_launch_scatter(const gbe_graph* g, const gbe_state* st, const double* X0, const double* X1, double* D_val,
                        cudaStream_t s, int64_t row0 = 0, int64_t n_rows = -1);

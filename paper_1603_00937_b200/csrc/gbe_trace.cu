@@ -17,6 +17,11 @@ constexpr int TB = 1024;
 __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double* __restrict__ partials, int n) {
   __shared__ double s1[32], s2[32];
   const int t = threadIdx.x;
+  // programmatic dependent launch (gbe_internal.cuh): wait for the kernel that wrote the partials FIRST, let the next
+  // kernel of the stream go only then - an X^2 launch behind this kernel may therefore take X_{n+1} as complete when it
+  // starts (GBE_PDL_EARLY) and needs this kernel's result only before its epilogue
+  gbe_griddep_wait();
+  gbe_griddep_launch();
   const int stopped = st->stop;  // read now, tested after the sums: the loads below need not wait for it
   // the kernel is one CTA and latency bound: 8 independent 16-byte loads in flight per thread, summed in a fixed order
   double a1 = 0.0, a2 = 0.0;
@@ -41,8 +46,8 @@ __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double
 }
 }  // namespace
 
-int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s) {
-  k_trace_branch<<<1, TB, 0, s>>>(st, partials, n_partials);
+int gbe_launch_trace_branch(gbe_state* st, const double* partials, int n_partials, cudaStream_t s, int pdl) {
+  GBE_CUDA(gbe_launch_kernel(k_trace_branch, dim3(1), dim3(TB), 0, s, pdl != GBE_PDL_NONE, st, partials, n_partials));
   GBE_LAUNCHED();
   return GBE_OK;
 }

@@ -111,13 +111,19 @@ template <int MINB, int OP>
 __global__ void __launch_bounds__(X2_THREADS, MINB)
     k_x2(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin,
          double* __restrict__ Xout, double* __restrict__ partials, int iter, const double* __restrict__ Xb,
-         double* __restrict__ Dacc, const double* __restrict__ coef) {
+         double* __restrict__ Dacc, const double* __restrict__ coef, int early) {
   extern __shared__ __align__(16) double smem[];  // 2 stages x (A panel, B panel)
   __shared__ double red[8];
 
-  if (OP == 0 && st->stop) return;  // idempotency stop already fired (A-7): X is final
+  // programmatic dependent launch (gbe_internal.cuh): the next kernel of the stream may become resident from here on;
+  // early != 0 (behind k_trace_branch only): X_n is complete, the product runs first and the wait - for the branch of
+  // this iteration - comes before the epilogue.  A stop seen here is final; one not yet seen is seen after the wait.
+  gbe_griddep_launch();
+  if (!early) gbe_griddep_wait();
+  if (OP == 0 && gbe_ld_state(&st->stop)) return;  // idempotency stop already fired (A-7): X is final
   // preset sequence or the on-device choice
-  const int branch = OP == 0 ? (st->preset ? (int)st->br[iter] : st->branch) : 0;
+  int branch = 0;
+  if (OP == 0 && !early) branch = gbe_ld_state(&st->preset) ? gbe_ld_state(&st->br[iter]) : gbe_ld_state(&st->branch);
   const double cn = OP == 1 ? coef[iter] : 0.0;
 
   const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // pidx, ti | tj << 16, p, m
@@ -231,6 +237,11 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
 
   // epilogue: X_{n+1} = Y or 2 X_n - Y, direct + mirrored store, core-row trace partials.
   // Interior tiles (no ragged edge, no core row or column: most of them) take the path without any predicate.
+  if (OP == 0 && early) {  // the branch of this iteration is k_trace_branch's to decide: it is complete once the wait returns
+    gbe_griddep_wait();
+    if (gbe_ld_state(&st->stop)) return;
+    branch = gbe_ld_state(&st->preset) ? gbe_ld_state(&st->br[iter]) : gbe_ld_state(&st->branch);
+  }
   double s1 = 0.0, s2 = 0.0;
   auto epilogue = [&](auto edge_c, auto trace_c, auto full_c) {
     constexpr bool EDGE = decltype(edge_c)::value, TRACE = decltype(trace_c)::value;
@@ -399,13 +410,18 @@ __device__ __forceinline__ void xt_chunk(double (&acc)[2][8][2], const double* _
 template <int MINB>
 __global__ void __launch_bounds__(X2_THREADS, MINB)
     k_x2_tma(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin,
-             double* __restrict__ Xout, double* __restrict__ partials, int iter, const CUtensorMap* __restrict__ maps) {
+             double* __restrict__ Xout, double* __restrict__ partials, int iter, const CUtensorMap* __restrict__ maps,
+             int early) {
   extern __shared__ __align__(1024) double smem_t[];  // 3 stages x (A panel, B panel), every panel 1024-byte aligned
   __shared__ double red[8];
   __shared__ __align__(8) unsigned long long bars[2 * XT_NST];  // full[0..2], empty[0..2]
 
-  if (st->stop) return;
-  const int branch = st->preset ? (int)st->br[iter] : st->branch;
+  // programmatic dependent launch, as in k_x2: early != 0 puts the wait in front of the epilogue
+  gbe_griddep_launch();
+  if (!early) gbe_griddep_wait();
+  if (gbe_ld_state(&st->stop)) return;
+  int branch = 0;
+  if (!early) branch = gbe_ld_state(&st->preset) ? gbe_ld_state(&st->br[iter]) : gbe_ld_state(&st->branch);
 
   const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // pidx, ti | tj << 16, p, m
   const int4 it1 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x + 1];  // nc, ld, dense_off
@@ -520,6 +536,11 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   }
 
   // epilogue: as k_x2 (OP 0)
+  if (early) {  // the branch of this iteration is k_trace_branch's to decide: it is complete once the wait returns
+    gbe_griddep_wait();
+    if (gbe_ld_state(&st->stop)) return;
+    branch = gbe_ld_state(&st->preset) ? gbe_ld_state(&st->br[iter]) : gbe_ld_state(&st->branch);
+  }
   double s1 = 0.0, s2 = 0.0;
   auto epilogue = [&](auto edge_c, auto trace_c, auto full_c) {
     constexpr bool EDGE = decltype(edge_c)::value, TRACE = decltype(trace_c)::value;
@@ -682,7 +703,7 @@ namespace {
 template <int MINB, int OP>
 int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
               const double* Xb, double* Dacc, const double* coef, const gbe_tile_item* items, int n_items,
-              cudaStream_t s) {
+              cudaStream_t s, int pdl) {
   auto kern = k_x2<MINB, OP>;
   const size_t smem = (size_t)2 * X2_STAGE * sizeof(double);
   static gbe_device_once configured;  // one per template instance; function attributes are per device
@@ -690,23 +711,24 @@ int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout
     GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
   }
-  kern<<<n_items, X2_THREADS, smem, s>>>(items, st, Xin, Xout, partials, iter, Xb, Dacc, coef);
+  GBE_CUDA(gbe_launch_kernel(kern, dim3((unsigned)n_items), dim3(X2_THREADS), smem, s, pdl != GBE_PDL_NONE, items, st, Xin,
+                             Xout, partials, iter, Xb, Dacc, coef, pdl == GBE_PDL_EARLY ? 1 : 0));
   GBE_LAUNCHED();
   return GBE_OK;
 }
 }  // namespace
 
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                  bool last, bool hybrid, int buffer, cudaStream_t s) {
+                  bool last, bool hybrid, int buffer, cudaStream_t s, int pdl) {
   // the last SP2 iteration computes the tiles with a core row only: the scatter keeps core columns (Eq.(6));
   // hybrid: the communities with m <= GBE_PK_MAX_M are the packed kernel's (gbe_small.cu), only the others are tiled
   const gbe_tile_item* items = hybrid ? (last ? g->items_last_h : g->items_h) : (last ? g->items_last : g->items);
   const int n_items = hybrid ? (last ? g->n_items_last_h : g->n_items_h) : (last ? g->n_items_last : g->n_items);
-  return gbe_launch_x2_items(g, st, Xin, Xout, partials, iter, items, n_items, buffer, s);
+  return gbe_launch_x2_items(g, st, Xin, Xout, partials, iter, items, n_items, buffer, s, pdl);
 }
 
 int gbe_launch_x2_items(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                        const gbe_tile_item* items, int n_items, int buffer, cudaStream_t s) {
+                        const gbe_tile_item* items, int n_items, int buffer, cudaStream_t s, int pdl) {
   if (n_items == 0) return GBE_OK;
   if (g->tmaps) {  // panels staged by 2-D TMA (k_x2_tma); X_n is in buffer 0 for even iterations, in buffer 1 for odd ones
     const CUtensorMap* maps = reinterpret_cast<const CUtensorMap*>(g->tmaps) + (buffer ? g->n_part : 0);
@@ -717,15 +739,16 @@ int gbe_launch_x2_items(const gbe_graph* g, gbe_state* st, const double* Xin, do
       GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     }
-    kern<<<n_items, X2_THREADS, smem, s>>>(items, st, Xin, Xout, partials, iter, maps);
+    GBE_CUDA(gbe_launch_kernel(kern, dim3((unsigned)n_items), dim3(X2_THREADS), smem, s, pdl != GBE_PDL_NONE, items, st,
+                               Xin, Xout, partials, iter, maps, pdl == GBE_PDL_EARLY ? 1 : 0));
     GBE_LAUNCHED();
     return GBE_OK;
   }
-  return launch_x2<4, 0>(g, st, Xin, Xout, partials, iter, nullptr, nullptr, nullptr, items, n_items, s);
+  return launch_x2<4, 0>(g, st, Xin, Xout, partials, iter, nullptr, nullptr, nullptr, items, n_items, s, pdl);
 }
 
 int gbe_launch_cheb_step(const gbe_graph* g, gbe_state* st, const double* Xt, const double* Tn, double* Tio, double* Dacc,
                          const double* coef, int iter, double* partials, cudaStream_t s) {
   if (g->n_items == 0) return GBE_OK;
-  return launch_x2<4, 1>(g, st, Xt, Tio, partials, iter, Tn, Dacc, coef, g->items, g->n_items, s);
+  return launch_x2<4, 1>(g, st, Xt, Tio, partials, iter, Tn, Dacc, coef, g->items, g->n_items, s, GBE_PDL_NONE);
 }
