@@ -358,9 +358,10 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
     }
     const int n_part_it = g->n_items_last;  // one packed partial per tile with a core row, in every iteration
     // programmatic dependent launch: behind k_trace_branch the product of iteration it + 1 starts while the decision of
-    // iteration it + 1 is being taken (GBE_PDL_EARLY); without traces an X^2 launch follows an X^2 launch and waits for
-    // it before it reads X (GBE_PDL_TOP)
-    const int pdl = g_x2_pdl.load(std::memory_order_relaxed) ? (mode != 2 ? GBE_PDL_EARLY : GBE_PDL_TOP) : GBE_PDL_NONE;
+    // iteration it + 1 is being taken (GBE_PDL_EARLY).  Without traces an X^2 launch follows an X^2 launch and would
+    // have to wait at its top (GBE_PDL_TOP): measured slower than plain stream order on small systems (its CTAs become
+    // resident next to the running ones and only wait), no gain on large ones - not used.
+    const int pdl = g_x2_pdl.load(std::memory_order_relaxed) && mode != 2 ? GBE_PDL_EARLY : GBE_PDL_NONE;
     GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, g->n_items ? 1 : 0,
                   [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, false, it & 1, s, pdl); }));
     if (mode != 2)

@@ -213,6 +213,11 @@ __device__ __forceinline__ int gbe_ld_state(const int32_t* p) {
   asm volatile("ld.global.cg.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
+__device__ __forceinline__ int gbe_ld_acquire(const int32_t* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
 __device__ __forceinline__ int gbe_ld_state(const uint8_t* p) {
   int v;
   asm volatile("ld.global.cg.u8 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -333,7 +338,8 @@ __device__ __forceinline__ void gbe_trace_decide(gbe_state* st, double t1, doubl
     const int b = st->preset ? (int)st->br[k] : ((fabs(t2 - n_occ) < fabs(2.0 * t1 - t2 - n_occ)) ? 0 : 1);
     st->branch = b;
     st->br[k] = (uint8_t)b;
-    st->iter = k + 1;
+    __threadfence();  // iter == k + 1 PUBLISHES the branch of iteration k: a kernel already running (gbe_x2.cu,
+    st->iter = k + 1;  // GBE_PDL_EARLY) reads iter with acquire and, if it finds k + 1, the branch without waiting
   }
 }
 __device__ __forceinline__ double warp_sum(double v) {

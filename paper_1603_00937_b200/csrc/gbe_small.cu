@@ -35,7 +35,7 @@
 //     bin that publishes its pair LAST - one ticket per bin; its pairs sit in front of the bins' and enter the same
 //     sum.)  Either way ONE launch per SP2 iteration instead of two, and results reproducible bit for bit.
 // Measured on B200 (profiles/r02_small_m_ncu.md; per-warp %globaltimer stamps in a throw-away build): 1,024 communities of
-// m = 28/69/123 take 1.38 ms per density call (tiled kernels 2.55 ms, first version of this kernel 1.85 ms).  Per bin:
+// m = 28/69/123 take 1.40 ms per density call (tiled kernels 2.55 ms, first version of this kernel 1.85 ms).  Per bin:
 // ~1.4 us set-up (hidden behind the previous launch for the first wave), rows landed 2.3 - 2.6 us after the dependency
 // resolves (the pair sum runs meanwhile), 10 - 11 us of products and stores, 0.4 us for the pair.  In the product phase
 // the FP64 tensor pipe is busy about 60 % of the time (43 % over the launch): every non-DMMA instruction costs the

@@ -120,10 +120,15 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   // this iteration - comes before the epilogue.  A stop seen here is final; one not yet seen is seen after the wait.
   gbe_griddep_launch();
   if (!early) gbe_griddep_wait();
-  if (OP == 0 && gbe_ld_state(&st->stop)) return;  // idempotency stop already fired (A-7): X is final
-  // preset sequence or the on-device choice
-  int branch = 0;
-  if (OP == 0 && !early) branch = gbe_ld_state(&st->preset) ? gbe_ld_state(&st->br[iter]) : gbe_ld_state(&st->branch);
+  // the state (uncached loads: another kernel may be writing it), requested here and looked at after the tile's own
+  // set-up so that their latency costs nothing.  Preset sequence or the on-device choice; early: if
+  // k_trace_branch has published its decision already - iter advanced to iter + 1 - the branch is known now and the
+  // epilogue does not wait; only the first CTAs of a launch come too early for that.
+  const int stop0 = OP == 0 ? gbe_ld_state(&st->stop) : 0;
+  const int iter_now = OP == 0 && early ? gbe_ld_acquire(&st->iter) : iter + 1;
+  const int br_preset = OP == 0 ? gbe_ld_state(&st->preset) : 0;
+  const int br_given = OP == 0 && iter < GBE_MAX_ITERS ? gbe_ld_state(&st->br[iter]) : 0;
+  const int br_chosen = OP == 0 ? gbe_ld_state(&st->branch) : 0;
   const double cn = OP == 1 ? coef[iter] : 0.0;
 
   const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // pidx, ti | tj << 16, p, m
@@ -220,6 +225,9 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
     }
   };
 
+  if (stop0) return;  // idempotency stop already fired (A-7): X is final
+  const bool decided = OP != 0 || iter_now == iter + 1;
+  int branch = br_preset ? br_given : br_chosen;  // (meaningful once decided)
   issue(0, 0);
   for (int kc = 0; kc < nchunks; kc += 2) {
     cp_async_wait<0>();
@@ -237,7 +245,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
 
   // epilogue: X_{n+1} = Y or 2 X_n - Y, direct + mirrored store, core-row trace partials.
   // Interior tiles (no ragged edge, no core row or column: most of them) take the path without any predicate.
-  if (OP == 0 && early) {  // the branch of this iteration is k_trace_branch's to decide: it is complete once the wait returns
+  if (OP == 0 && !decided) {  // the branch of this iteration is k_trace_branch's to decide: it is complete once the wait returns
     gbe_griddep_wait();
     if (gbe_ld_state(&st->stop)) return;
     branch = gbe_ld_state(&st->preset) ? gbe_ld_state(&st->br[iter]) : gbe_ld_state(&st->branch);
@@ -419,9 +427,11 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   // programmatic dependent launch, as in k_x2: early != 0 puts the wait in front of the epilogue
   gbe_griddep_launch();
   if (!early) gbe_griddep_wait();
-  if (gbe_ld_state(&st->stop)) return;
-  int branch = 0;
-  if (!early) branch = gbe_ld_state(&st->preset) ? gbe_ld_state(&st->br[iter]) : gbe_ld_state(&st->branch);
+  const int stop0 = gbe_ld_state(&st->stop);  // requested here, looked at after the mbarrier set-up (as in k_x2)
+  const int iter_now = early ? gbe_ld_acquire(&st->iter) : iter + 1;
+  const int br_preset = gbe_ld_state(&st->preset);
+  const int br_given = iter < GBE_MAX_ITERS ? gbe_ld_state(&st->br[iter]) : 0;
+  const int br_chosen = gbe_ld_state(&st->branch);
 
   const int4 it0 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x];      // pidx, ti | tj << 16, p, m
   const int4 it1 = reinterpret_cast<const int4*>(items)[2 * (size_t)blockIdx.x + 1];  // nc, ld, dense_off
@@ -449,6 +459,9 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
+  if (stop0) return;  // idempotency stop already fired (A-7): X is final
+  const bool decided = iter_now == iter + 1;
+  int branch = br_preset ? br_given : br_chosen;  // (meaningful once decided)
   const uint32_t stage_bytes = share ? XT_PANEL * 8u : XT_STAGE * 8u;
   auto produce = [&](int s, int kc) {  // thread 0: chunk kc -> stage s
     mbar_expect_tx(bar0 + 8 * s, stage_bytes);
@@ -536,7 +549,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   }
 
   // epilogue: as k_x2 (OP 0)
-  if (early) {  // the branch of this iteration is k_trace_branch's to decide: it is complete once the wait returns
+  if (!decided) {  // the branch of this iteration is k_trace_branch's to decide: it is complete once the wait returns
     gbe_griddep_wait();
     if (gbe_ld_state(&st->stop)) return;
     branch = gbe_ld_state(&st->preset) ? gbe_ld_state(&st->br[iter]) : gbe_ld_state(&st->branch);
