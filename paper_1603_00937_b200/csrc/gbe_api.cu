@@ -357,10 +357,10 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
       continue;
     }
     const int n_part_it = g->n_items_last;  // one packed partial per tile with a core row, in every iteration
-    // programmatic dependent launch: behind k_trace_branch the product of iteration it + 1 starts while the decision of
-    // iteration it + 1 is being taken (GBE_PDL_EARLY).  Without traces an X^2 launch follows an X^2 launch and would
-    // have to wait at its top (GBE_PDL_TOP): measured slower than plain stream order on small systems (its CTAs become
-    // resident next to the running ones and only wait), no gain on large ones - not used.
+    // programmatic dependent launch: k_trace_branch is resident and waiting when the X^2 launch ends, and lets the next
+    // X^2 launch go the moment its decision is visible (GBE_PDL_EARLY: that launch never waits).  Without traces an X^2
+    // launch follows an X^2 launch and would have to wait at its top: measured slower than plain stream order on small
+    // systems (its CTAs become resident next to the running ones and only wait), no gain on large ones - not used.
     const int pdl = g_x2_pdl.load(std::memory_order_relaxed) && mode != 2 ? GBE_PDL_EARLY : GBE_PDL_NONE;
     GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, g->n_items ? 1 : 0,
                   [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, false, it & 1, s, pdl); }));

@@ -197,10 +197,11 @@ struct gbe_graph {
 // once every CTA of the previous kernel of the stream has executed griddepcontrol.launch_dependents (or exited); it must
 // execute griddepcontrol.wait before it touches anything the previous kernel (or, transitively, an earlier one that the
 // previous kernel itself did not wait for) produces.  Without the attribute both instructions are no-ops.
-//   GBE_PDL_TOP    the kernel waits before it reads anything a launch produces (safe behind any kernel)
-//   GBE_PDL_EARLY  X^2 kernel behind k_trace_branch only: k_trace_branch waits for the previous X^2 launch BEFORE it lets
-//                  its dependents go, so X_n is complete when this grid starts; it runs its product first and waits
-//                  (for the branch of this iteration) before its epilogue
+//   GBE_PDL_TOP    the kernel waits at its top, before it reads anything a launch produces (safe behind any kernel):
+//                  k_trace_branch, k_sp2_packed
+//   GBE_PDL_EARLY  X^2 kernel behind k_trace_branch only: it never waits.  k_trace_branch waits for the previous X^2
+//                  launch, decides, fences and only then lets its dependents go, so everything this grid reads is final
+//                  when it starts
 // ----------------------------------------------------------------------------------------------
 enum { GBE_PDL_NONE = 0, GBE_PDL_TOP = 1, GBE_PDL_EARLY = 2 };
 #ifdef __CUDACC__
@@ -211,11 +212,6 @@ __device__ __forceinline__ void gbe_griddep_wait() { asm volatile("griddepcontro
 __device__ __forceinline__ int gbe_ld_state(const int32_t* p) {
   int v;
   asm volatile("ld.global.cg.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ int gbe_ld_acquire(const int32_t* p) {
-  int v;
-  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
 __device__ __forceinline__ int gbe_ld_state(const uint8_t* p) {
@@ -338,8 +334,7 @@ __device__ __forceinline__ void gbe_trace_decide(gbe_state* st, double t1, doubl
     const int b = st->preset ? (int)st->br[k] : ((fabs(t2 - n_occ) < fabs(2.0 * t1 - t2 - n_occ)) ? 0 : 1);
     st->branch = b;
     st->br[k] = (uint8_t)b;
-    __threadfence();  // iter == k + 1 PUBLISHES the branch of iteration k: a kernel already running (gbe_x2.cu,
-    st->iter = k + 1;  // GBE_PDL_EARLY) reads iter with acquire and, if it finds k + 1, the branch without waiting
+    st->iter = k + 1;
   }
 }
 __device__ __forceinline__ double warp_sum(double v) {

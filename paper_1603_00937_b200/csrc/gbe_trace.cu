@@ -17,11 +17,9 @@ constexpr int TB = 1024;
 __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double* __restrict__ partials, int n) {
   __shared__ double s1[32], s2[32];
   const int t = threadIdx.x;
-  // programmatic dependent launch (gbe_internal.cuh): wait for the kernel that wrote the partials FIRST, let the next
-  // kernel of the stream go only then - an X^2 launch behind this kernel may therefore take X_{n+1} as complete when it
-  // starts (GBE_PDL_EARLY) and needs this kernel's result only before its epilogue
+  // programmatic dependent launch (gbe_internal.cuh): this CTA may be resident before the kernel that writes the partials
+  // has finished - wait for it; the next kernel of the stream is let go at the very end, after the decision
   gbe_griddep_wait();
-  gbe_griddep_launch();
   const int stopped = st->stop;  // read now, tested after the sums: the loads below need not wait for it
   // the kernel is one CTA and latency bound: 8 independent 16-byte loads in flight per thread, summed in a fixed order
   double a1 = 0.0, a2 = 0.0;
@@ -42,7 +40,13 @@ __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double
     a1 = warp_sum(s1[t]);
     a2 = warp_sum(s2[t]);
   }
-  if (t == 0 && !stopped) gbe_trace_decide(st, a1, a2);
+  if (t == 0) {
+    if (!stopped) gbe_trace_decide(st, a1, a2);
+    // the X^2 launch behind this kernel (launched with the attribute) never waits: it may start only now, when X_{n+1}
+    // is complete (the wait above) and the decision is visible device-wide
+    __threadfence();
+    gbe_griddep_launch();
+  }
 }
 }  // namespace
 

@@ -111,21 +111,18 @@ template <int MINB, int OP>
 __global__ void __launch_bounds__(X2_THREADS, MINB)
     k_x2(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin,
          double* __restrict__ Xout, double* __restrict__ partials, int iter, const double* __restrict__ Xb,
-         double* __restrict__ Dacc, const double* __restrict__ coef, int early) {
+         double* __restrict__ Dacc, const double* __restrict__ coef) {
   extern __shared__ __align__(16) double smem[];  // 2 stages x (A panel, B panel)
   __shared__ double red[8];
 
-  // programmatic dependent launch (gbe_internal.cuh): the next kernel of the stream may become resident from here on;
-  // early != 0 (behind k_trace_branch only): X_n is complete, the product runs first and the wait - for the branch of
-  // this iteration - comes before the epilogue.  A stop seen here is final; one not yet seen is seen after the wait.
+  // programmatic dependent launch (gbe_internal.cuh): the next kernel of the stream (k_trace_branch, or the packed
+  // kernel) may become resident from here on; it waits for this grid in its own code.  This kernel itself never waits:
+  // launched behind k_trace_branch with the attribute it starts when that kernel lets it go - AFTER it has waited for
+  // the previous X^2 launch, taken the decision and fenced - so X_n, the branch and the stop flag are all final.  The
+  // state is read with uncached loads (a line of it may sit in this SM's L1 from the previous launch), requested here
+  // and looked at after the tile's own set-up so that their latency costs nothing.
   gbe_griddep_launch();
-  if (!early) gbe_griddep_wait();
-  // the state (uncached loads: another kernel may be writing it), requested here and looked at after the tile's own
-  // set-up so that their latency costs nothing.  Preset sequence or the on-device choice; early: if
-  // k_trace_branch has published its decision already - iter advanced to iter + 1 - the branch is known now and the
-  // epilogue does not wait; only the first CTAs of a launch come too early for that.
   const int stop0 = OP == 0 ? gbe_ld_state(&st->stop) : 0;
-  const int iter_now = OP == 0 && early ? gbe_ld_acquire(&st->iter) : iter + 1;
   const int br_preset = OP == 0 ? gbe_ld_state(&st->preset) : 0;
   const int br_given = OP == 0 && iter < GBE_MAX_ITERS ? gbe_ld_state(&st->br[iter]) : 0;
   const int br_chosen = OP == 0 ? gbe_ld_state(&st->branch) : 0;
@@ -226,8 +223,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   };
 
   if (stop0) return;  // idempotency stop already fired (A-7): X is final
-  const bool decided = OP != 0 || iter_now == iter + 1;
-  int branch = br_preset ? br_given : br_chosen;  // (meaningful once decided)
+  const int branch = br_preset ? br_given : br_chosen;  // preset sequence or the on-device choice
   issue(0, 0);
   for (int kc = 0; kc < nchunks; kc += 2) {
     cp_async_wait<0>();
@@ -245,11 +241,6 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
 
   // epilogue: X_{n+1} = Y or 2 X_n - Y, direct + mirrored store, core-row trace partials.
   // Interior tiles (no ragged edge, no core row or column: most of them) take the path without any predicate.
-  if (OP == 0 && !decided) {  // the branch of this iteration is k_trace_branch's to decide: it is complete once the wait returns
-    gbe_griddep_wait();
-    if (gbe_ld_state(&st->stop)) return;
-    branch = gbe_ld_state(&st->preset) ? gbe_ld_state(&st->br[iter]) : gbe_ld_state(&st->branch);
-  }
   double s1 = 0.0, s2 = 0.0;
   auto epilogue = [&](auto edge_c, auto trace_c, auto full_c) {
     constexpr bool EDGE = decltype(edge_c)::value, TRACE = decltype(trace_c)::value;
@@ -418,17 +409,14 @@ __device__ __forceinline__ void xt_chunk(double (&acc)[2][8][2], const double* _
 template <int MINB>
 __global__ void __launch_bounds__(X2_THREADS, MINB)
     k_x2_tma(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin,
-             double* __restrict__ Xout, double* __restrict__ partials, int iter, const CUtensorMap* __restrict__ maps,
-             int early) {
+             double* __restrict__ Xout, double* __restrict__ partials, int iter, const CUtensorMap* __restrict__ maps) {
   extern __shared__ __align__(1024) double smem_t[];  // 3 stages x (A panel, B panel), every panel 1024-byte aligned
   __shared__ double red[8];
   __shared__ __align__(8) unsigned long long bars[2 * XT_NST];  // full[0..2], empty[0..2]
 
-  // programmatic dependent launch, as in k_x2: early != 0 puts the wait in front of the epilogue
+  // programmatic dependent launch and state loads: as in k_x2
   gbe_griddep_launch();
-  if (!early) gbe_griddep_wait();
-  const int stop0 = gbe_ld_state(&st->stop);  // requested here, looked at after the mbarrier set-up (as in k_x2)
-  const int iter_now = early ? gbe_ld_acquire(&st->iter) : iter + 1;
+  const int stop0 = gbe_ld_state(&st->stop);  // requested here, looked at after the mbarrier set-up
   const int br_preset = gbe_ld_state(&st->preset);
   const int br_given = iter < GBE_MAX_ITERS ? gbe_ld_state(&st->br[iter]) : 0;
   const int br_chosen = gbe_ld_state(&st->branch);
@@ -460,8 +448,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   }
   __syncthreads();
   if (stop0) return;  // idempotency stop already fired (A-7): X is final
-  const bool decided = iter_now == iter + 1;
-  int branch = br_preset ? br_given : br_chosen;  // (meaningful once decided)
+  const int branch = br_preset ? br_given : br_chosen;
   const uint32_t stage_bytes = share ? XT_PANEL * 8u : XT_STAGE * 8u;
   auto produce = [&](int s, int kc) {  // thread 0: chunk kc -> stage s
     mbar_expect_tx(bar0 + 8 * s, stage_bytes);
@@ -549,11 +536,6 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   }
 
   // epilogue: as k_x2 (OP 0)
-  if (!decided) {  // the branch of this iteration is k_trace_branch's to decide: it is complete once the wait returns
-    gbe_griddep_wait();
-    if (gbe_ld_state(&st->stop)) return;
-    branch = gbe_ld_state(&st->preset) ? gbe_ld_state(&st->br[iter]) : gbe_ld_state(&st->branch);
-  }
   double s1 = 0.0, s2 = 0.0;
   auto epilogue = [&](auto edge_c, auto trace_c, auto full_c) {
     constexpr bool EDGE = decltype(edge_c)::value, TRACE = decltype(trace_c)::value;
@@ -725,7 +707,7 @@ int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout
     GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
   }
   GBE_CUDA(gbe_launch_kernel(kern, dim3((unsigned)n_items), dim3(X2_THREADS), smem, s, pdl != GBE_PDL_NONE, items, st, Xin,
-                             Xout, partials, iter, Xb, Dacc, coef, pdl == GBE_PDL_EARLY ? 1 : 0));
+                             Xout, partials, iter, Xb, Dacc, coef));
   GBE_LAUNCHED();
   return GBE_OK;
 }
@@ -753,7 +735,7 @@ int gbe_launch_x2_items(const gbe_graph* g, gbe_state* st, const double* Xin, do
       GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     }
     GBE_CUDA(gbe_launch_kernel(kern, dim3((unsigned)n_items), dim3(X2_THREADS), smem, s, pdl != GBE_PDL_NONE, items, st,
-                               Xin, Xout, partials, iter, maps, pdl == GBE_PDL_EARLY ? 1 : 0));
+                               Xin, Xout, partials, iter, maps));
     GBE_LAUNCHED();
     return GBE_OK;
   }
