@@ -163,9 +163,16 @@ class Graph:
 
     def __init__(self, handle: int):
         self._h = C.c_void_p(handle)
-        info = _GraphInfo()
-        _check(lib().gbe_graph_get_info(self._h, C.byref(info)))
-        self.info = {k: getattr(info, k) for k, _ in _GraphInfo._fields_}
+        self._info = None
+
+    @property
+    def info(self) -> dict:
+        """gbe_graph_info as a dict, read on first use (a build + density loop that never looks at it does not pay for it)."""
+        if self._info is None:
+            info = _GraphInfo()
+            _check(lib().gbe_graph_get_info(self.handle, C.byref(info)))
+            self._info = {k: getattr(info, k) for k, _ in _GraphInfo._fields_}
+        return self._info
 
     @property
     def handle(self):
@@ -234,9 +241,7 @@ def gbe_update_graph(prev: Graph, D_prev: torch.Tensor, H: DeviceCSR, tau: float
 def gbe_graph_set_sp2_path(g: "Graph", path: int) -> None:
     """0 auto, 1 tiled kernels, 2 shared-memory-resident kernel, 3 packed kernel for the small communities (include/gbe.h)."""
     _check(lib().gbe_graph_set_sp2_path(g._h, int(path)))
-    info = _GraphInfo()
-    _check(lib().gbe_graph_get_info(g._h, C.byref(info)))
-    g.info = {k: getattr(info, k) for k, _ in _GraphInfo._fields_}
+    g._info = None  # sp2_path_chosen / resident_sp2 change: read again on next use
 
 
 def gbe_graph_set_gather_path(g: "Graph", path: int) -> None:

@@ -140,6 +140,38 @@ __global__ void k_row_meta(int64_t sum_m, const int32_t* __restrict__ row_part, 
   row_src[q] = dense_off[p] + (q - sb) * ld;
   row_nc[q] = ncore[p];
 }
+// The X^2 work lists (gbe_tile_item), written on the device from one small descriptor per community (the host sorts the
+// communities by size and takes two prefix sums; spelling out ~2e4 items on the host cost 0.4 ms per build): block b
+// writes the tiles (ti <= tj) of community desc[b].p, ti outer, tj inner, at items[desc[b].off ...]; those with a core row
+// (ti * tile < ncore: the first Tc tile rows, i.e. the first tiles of the community's run) also at last[desc[b].loff ...],
+// and their position there is the index of their trace partial (pidx; -1 for the others).
+struct gbe_tile_desc { int32_t p, m, nc, ld, off, loff; int64_t dense_off; };
+__global__ void k_tile_items(const gbe_tile_desc* __restrict__ desc, int tile, gbe_tile_item* __restrict__ items,
+                             gbe_tile_item* __restrict__ last) {
+  const gbe_tile_desc d = desc[blockIdx.x];
+  const int T = (d.m + tile - 1) / tile;
+  const int n_t = T * (T + 1) / 2;
+  for (int k = threadIdx.x; k < n_t; k += blockDim.x) {
+    // k = ti * T - ti (ti - 1) / 2 + (tj - ti): the largest ti whose first index is <= k (T <= 2^15: fp32 start, fixed up)
+    int ti = (int)(((float)(2 * T + 1) - sqrtf((float)(2 * T + 1) * (float)(2 * T + 1) - 8.0f * (float)k)) * 0.5f);
+    ti = min(max(ti, 0), T - 1);
+    while (ti > 0 && ti * T - ti * (ti - 1) / 2 > k) --ti;
+    while (ti + 1 < T && (ti + 1) * T - (ti + 1) * ti / 2 <= k) ++ti;
+    const int tj = ti + (k - (ti * T - ti * (ti - 1) / 2));
+    const bool core_row = ti * tile < d.nc;
+    gbe_tile_item it;
+    it.pidx = core_row ? d.loff + k : -1;
+    it.tij = ti | (tj << 16);
+    it.p = d.p;
+    it.m = d.m;
+    it.nc = d.nc;
+    it.ld = d.ld;
+    it.dense_off = d.dense_off;
+    items[d.off + k] = it;
+    if (core_row) last[d.loff + k] = it;
+  }
+}
+
 __global__ void k_row_ncore(int64_t sum_m, const int32_t* __restrict__ row_part, const int32_t* __restrict__ ncore,
                             int32_t* __restrict__ out) {
   const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -317,93 +349,6 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
   GBE_TRY(upload(h_sub_ptr, &g->sub_ptr, s));
   GBE_TRY(upload(g->h_dense_off, &g->dense_off, s));
 
-  // X^2 tile list: communities by decreasing m (longest work first), the tiles of one community adjacent
-  // so that its panels are reused from L2 by the CTAs that run together.
-  {
-    std::vector<int32_t> order(n_part);
-    std::iota(order.begin(), order.end(), 0);
-    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return g->h_m[a] > g->h_m[b]; });
-    g->pk_max_m = gbe_packed_max_m();
-    std::vector<gbe_tile_item> items, last, items_h, last_h;  // _h: the communities the packed kernel does not take
-    const int tile = g->tile;
-    g->exec_flops_per_iter = g->exec_flops_last_iter = g->flops_last_iter = 0;
-    for (int p : order) {
-      const int T = (g->h_m[p] + tile - 1) / tile;
-      const int64_t ld = (g->h_m[p] + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
-      const bool big = g->h_m[p] > g->pk_max_m;
-      for (int ti = 0; ti < T; ++ti)
-        for (int tj = ti; tj < T; ++tj) {
-          // pidx: where the tile's trace partial goes - the tiles with a core row are numbered in list order (which is
-          // their position in the list of the last iteration), the others carry no trace and get -1
-          const bool core_row = ti * tile < g->h_ncore[p];
-          items.push_back({core_row ? (int32_t)last.size() : -1, ti | (tj << 16), p, g->h_m[p], g->h_ncore[p], (int32_t)ld,
-                           g->h_dense_off[p]});
-          if (core_row) last.push_back(items.back());
-          if (big) {
-            items_h.push_back(items.back());
-            items_h.back().pidx = core_row ? (int32_t)last_h.size() : -1;
-            if (core_row) last_h.push_back(items_h.back());
-          }
-        }
-      // executed DMMA work: 8x8 sub-tiles (bi <= bj) with rows < m, columns < ld, each 2*8*8*ld flop
-      const double R = (double)((g->h_m[p] + 7) / 8), C = (double)(ld / 8);
-      g->exec_flops_per_iter += (R * C - R * (R - 1) / 2) * 128.0 * (double)ld;
-      // last iteration: the same count restricted to the row blocks of the tiles with a core row
-      const int Tc = std::min(T, (g->h_ncore[p] + tile - 1) / tile);
-      const double Rc = std::min(R, (double)(Tc * (tile / 8)));
-      g->exec_flops_last_iter += (Rc * C - Rc * (Rc - 1) / 2) * 128.0 * (double)ld;
-      g->flops_last_iter += 2.0 * (double)g->h_m[p] * (double)g->h_m[p] * (double)g->h_ncore[p];
-    }
-    g->n_items_h = (int32_t)items_h.size();
-    g->n_items_last_h = (int32_t)last_h.size();
-    if (!items_h.empty() && items_h.size() < items.size()) {  // only a mixed graph needs the second pair of lists
-      GBE_TRY(upload(items_h, &g->items_h, s));
-      GBE_TRY(upload(last_h, &g->items_last_h, s));
-    }
-    g->n_items = (int32_t)items.size();
-    g->n_items_last = (int32_t)last.size();
-    GBE_TRY(upload(items, &g->items, s));
-    GBE_TRY(upload(last, &g->items_last, s));
-  }
-  {
-    // rows per gather CTA: every CTA first builds the community's index bitmaps over the n vertices (O(n / 32) words), so
-    // large systems amortise that over more rows
-    g->gather_rows = n <= 32768 ? 64 : (n <= 131072 ? 256 : 512);
-    std::vector<int2> gi;
-    for (int p = 0; p < n_part; ++p)
-      for (int r0 = 0; r0 < g->h_m[p]; r0 += g->gather_rows) gi.push_back(make_int2(p, r0));
-    g->n_gitems = (int32_t)gi.size();
-    GBE_TRY(upload(gi, &g->gitems, s));
-  }
-  GBE_TRY(gbe_build_packed(g, s));  // bins of the small communities (gbe_small.cu)
-  GBE_TRY(gbe_x2_build_tmaps(g, s));  // tensor maps of the tiled kernel's panels (gbe_x2.cu); needs dense_off on the device
-  // the resident kernel double-buffers n_part pairs; the packed path writes one pair per bin behind the tiled kernel's
-  g->n_partials = std::max(std::max(std::max(g->n_items, g->n_gitems), 2 * n_part), g->n_items_last_h + g->n_pk_ctas);
-  // wave mode (gbe_plan_waves): the gather of a later wave must not touch the final pairs of an earlier one
-  g->n_partials = std::max(g->n_partials, g->n_items_last + g->n_gitems);
-  GBE_TRY(gbe_resident_capacity(g, &g->resident_fits, &g->resident_coresident, &g->resident_cluster));
-
-  // workspace layout
-  size_t off = align_up(sizeof(gbe_state), 256);
-  g->ws_bounds = off;
-  off += align_up(2 * 1024 * sizeof(double), 256);
-  g->ws_partials = off;
-  off += align_up((size_t)std::max(1, g->n_partials) * 2 * sizeof(double), 256);
-  g->ws_x0 = off;
-  off += align_up((size_t)g->dense_elems * 8, 256);
-  g->ws_x1 = off;
-  off += align_up((size_t)g->dense_elems * 8, 256);
-  g->ws_bytes = off;
-  {  // smallest workspace of gbe_density_preset without traces: two buffers that hold the largest community
-    int64_t big = 0;
-    for (int p = 0; p < n_part; ++p) big = std::max<int64_t>(big, g->h_dense_off[p + 1] - g->h_dense_off[p]);
-    g->ws_bytes_wave_min = g->ws_x0 + 2 * align_up((size_t)big * 8, 256);
-  }
-  g->ws_x2 = off;
-  off += align_up((size_t)g->dense_elems * 8, 256);
-  g->ws_x3 = off;
-  off += align_up((size_t)g->dense_elems * 8, 256);
-  g->ws_bytes_fermi = off;
   // ---- fill sub_idx / row_part
   GBE_TRY(gbe_dev_alloc((void**)&g->sub_idx, std::max<size_t>(16, (size_t)g->sum_m * 4)));
   GBE_TRY(gbe_dev_alloc((void**)&g->row_part, std::max<size_t>(16, (size_t)g->sum_m * 4)));
@@ -444,7 +389,105 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
                                                        g->sub_ptr, g->sub_idx, g->ncore, g->D_row_ptr, g->D_col,
                                                        g->scat_base, flag.as<int32_t>(), nullptr, nullptr);
   GBE_LAUNCHED();
-  GBE_CUDA(cudaMemcpyAsync(&hflag, flag.p, 4, cudaMemcpyDeviceToHost, s));
+  // ---- host: work lists, bins, tensor maps, workspace layout - while the device fills sub_idx and the pattern of D (the
+  //      kernels above need the sizes and offsets only; a timeline of the build showed the device idle for 0.5 ms here
+  //      when the lists were built first).  Their uploads queue up behind k_d_pattern.
+  // X^2 tile list: communities by decreasing m (longest work first), the tiles of one community adjacent
+  // so that its panels are reused from L2 by the CTAs that run together.
+  {
+    std::vector<int32_t> order(n_part);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return g->h_m[a] > g->h_m[b]; });
+    g->pk_max_m = gbe_packed_max_m();
+    // the lists themselves are written on the device (k_tile_items) from one descriptor per community
+    std::vector<gbe_tile_desc> desc, desc_h;  // _h: the communities the packed kernel does not take
+    desc.reserve(n_part);
+    const int tile = g->tile;
+    int64_t n_all = 0, n_last = 0, n_all_h = 0, n_last_h = 0;
+    g->exec_flops_per_iter = g->exec_flops_last_iter = g->flops_last_iter = 0;
+    for (int p : order) {
+      const int m = g->h_m[p], nc = g->h_ncore[p];
+      const int64_t T = (m + tile - 1) / tile;
+      const int64_t ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
+      const int64_t Tc = std::min<int64_t>(T, (nc + tile - 1) / tile);  // tile rows with a core row (ti * tile < ncore)
+      const int64_t n_t = T * (T + 1) / 2, n_c = Tc * T - Tc * (Tc - 1) / 2;
+      if (n_t > 0) {
+        desc.push_back({p, m, nc, (int32_t)ld, (int32_t)n_all, (int32_t)n_last, g->h_dense_off[p]});
+        if (m > g->pk_max_m) desc_h.push_back({p, m, nc, (int32_t)ld, (int32_t)n_all_h, (int32_t)n_last_h, g->h_dense_off[p]});
+      }
+      n_all += n_t;
+      n_last += n_c;
+      if (m > g->pk_max_m) { n_all_h += n_t; n_last_h += n_c; }
+      // executed DMMA work: 8x8 sub-tiles (bi <= bj) with rows < m, columns < ld, each 2*8*8*ld flop
+      const double R = (double)((m + 7) / 8), C = (double)(ld / 8);
+      g->exec_flops_per_iter += (R * C - R * (R - 1) / 2) * 128.0 * (double)ld;
+      // last iteration: the same count restricted to the row blocks of the tiles with a core row
+      const double Rc = std::min(R, (double)(Tc * (tile / 8)));
+      g->exec_flops_last_iter += (Rc * C - Rc * (Rc - 1) / 2) * 128.0 * (double)ld;
+      g->flops_last_iter += 2.0 * (double)m * (double)m * (double)nc;
+    }
+    if (n_all > INT32_MAX) return GBE_EINVAL;  // the work lists are indexed with 32 bits
+    auto make_lists = [&](const std::vector<gbe_tile_desc>& d, int64_t na, int64_t nl, gbe_tile_item** it,
+                          gbe_tile_item** la) -> int {
+      GBE_TRY(gbe_dev_alloc((void**)it, std::max<size_t>(16, (size_t)na * sizeof(gbe_tile_item))));
+      GBE_TRY(gbe_dev_alloc((void**)la, std::max<size_t>(16, (size_t)nl * sizeof(gbe_tile_item))));
+      if (d.empty()) return GBE_OK;
+      DevBuf dd;
+      GBE_TRY(dd.alloc(d.size() * sizeof(gbe_tile_desc)));
+      GBE_CUDA(cudaMemcpyAsync(dd.p, d.data(), d.size() * sizeof(gbe_tile_desc), cudaMemcpyHostToDevice, s));
+      k_tile_items<<<(unsigned)d.size(), 128, 0, s>>>(dd.as<gbe_tile_desc>(), tile, *it, *la);
+      GBE_LAUNCHED();
+      return GBE_OK;  // (dd is released in stream order; the copy of a few KB from pageable memory is staged at once)
+    };
+    g->n_items_h = (int32_t)n_all_h;
+    g->n_items_last_h = (int32_t)n_last_h;
+    if (n_all_h > 0 && n_all_h < n_all)  // only a mixed graph needs the second pair of lists
+      GBE_TRY(make_lists(desc_h, n_all_h, n_last_h, &g->items_h, &g->items_last_h));
+    g->n_items = (int32_t)n_all;
+    g->n_items_last = (int32_t)n_last;
+    GBE_TRY(make_lists(desc, n_all, n_last, &g->items, &g->items_last));
+  }
+  {
+    // rows per gather CTA: every CTA first builds the community's index bitmaps over the n vertices (O(n / 32) words), so
+    // large systems amortise that over more rows
+    g->gather_rows = n <= 32768 ? 64 : (n <= 131072 ? 256 : 512);
+    static thread_local std::vector<int2> gi;
+    gi.clear();
+    for (int p = 0; p < n_part; ++p)
+      for (int r0 = 0; r0 < g->h_m[p]; r0 += g->gather_rows) gi.push_back(make_int2(p, r0));
+    g->n_gitems = (int32_t)gi.size();
+    GBE_TRY(upload(gi, &g->gitems, s));
+  }
+  GBE_TRY(gbe_build_packed(g, s));  // bins of the small communities (gbe_small.cu)
+  GBE_TRY(gbe_x2_build_tmaps(g, s));  // tensor maps of the tiled kernel's panels (gbe_x2.cu); needs dense_off on the device
+  // the resident kernel double-buffers n_part pairs; the packed path writes one pair per bin behind the tiled kernel's
+  g->n_partials = std::max(std::max(std::max(g->n_items, g->n_gitems), 2 * n_part), g->n_items_last_h + g->n_pk_ctas);
+  // wave mode (gbe_plan_waves): the gather of a later wave must not touch the final pairs of an earlier one
+  g->n_partials = std::max(g->n_partials, g->n_items_last + g->n_gitems);
+  GBE_TRY(gbe_resident_capacity(g, &g->resident_fits, &g->resident_coresident, &g->resident_cluster));
+
+  // workspace layout
+  size_t off = align_up(sizeof(gbe_state), 256);
+  g->ws_bounds = off;
+  off += align_up(2 * 1024 * sizeof(double), 256);
+  g->ws_partials = off;
+  off += align_up((size_t)std::max(1, g->n_partials) * 2 * sizeof(double), 256);
+  g->ws_x0 = off;
+  off += align_up((size_t)g->dense_elems * 8, 256);
+  g->ws_x1 = off;
+  off += align_up((size_t)g->dense_elems * 8, 256);
+  g->ws_bytes = off;
+  {  // smallest workspace of gbe_density_preset without traces: two buffers that hold the largest community
+    int64_t big = 0;
+    for (int p = 0; p < n_part; ++p) big = std::max<int64_t>(big, g->h_dense_off[p + 1] - g->h_dense_off[p]);
+    g->ws_bytes_wave_min = g->ws_x0 + 2 * align_up((size_t)big * 8, 256);
+  }
+  g->ws_x2 = off;
+  off += align_up((size_t)g->dense_elems * 8, 256);
+  g->ws_x3 = off;
+  off += align_up((size_t)g->dense_elems * 8, 256);
+  g->ws_bytes_fermi = off;
+  GBE_CUDA(cudaMemcpyAsync(&hflag, flag.p, 4, cudaMemcpyDeviceToHost, s));  // (to pageable memory: blocks the host - kept last)
   GBE_CUDA(cudaStreamSynchronize(s));  // the last synchronisation of a build (the general scatter map below needs one more)
   g->contiguous = hflag ? 0 : 1;
   if (!g->contiguous) {

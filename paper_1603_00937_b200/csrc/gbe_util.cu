@@ -59,8 +59,10 @@ void gbe_dev_free(void* p) {
 }
 
 namespace {
-// One CTA walks the array in tiles of 4,096: every thread takes 4 consecutive elements (a warp reads 512 contiguous
-// bytes), warp scans by shuffle, one scan over the 32 warp sums, a running carry between tiles.
+// One CTA walks the array in tiles of 16,384: every thread takes SCAN_EPT = 16 consecutive elements (four 16-byte loads
+// in flight), warp scans by shuffle, one scan over the 32 warp sums, a running carry between tiles.  (The graph build
+// calls this eight times on n counts; with 4 elements per thread the 24,576-orbital box took six tiles and 20 us a call.)
+constexpr int SCAN_EPT = 16;
 template <typename TI>
 __global__ void __launch_bounds__(1024) k_scan_single_block(const TI* __restrict__ in, int64_t* __restrict__ out,
                                                             int64_t n, int want_max) {
@@ -69,13 +71,27 @@ __global__ void __launch_bounds__(1024) k_scan_single_block(const TI* __restrict
   const int t = threadIdx.x, lane = t & 31, w = t >> 5;
   int64_t carry = 0;
   int64_t vmax = 0;  // want_max: out[n + 1] = max(0, max_i in[i])
-  for (int64_t base = 0; base < n; base += 4096) {
-    const int64_t i0 = base + 4 * t;
-    int64_t v[4];
+  const bool vec_ok = sizeof(TI) == 4 && (reinterpret_cast<uintptr_t>(in) & 15) == 0;
+  const bool vec_out = (reinterpret_cast<uintptr_t>(out) & 15) == 0;
+  for (int64_t base = 0; base < n; base += (int64_t)SCAN_EPT * 1024) {
+    const int64_t i0 = base + (int64_t)SCAN_EPT * t;
+    TI v[SCAN_EPT];
+    if (vec_ok && i0 + SCAN_EPT <= n) {
 #pragma unroll
-    for (int k = 0; k < 4; ++k) v[k] = i0 + k < n ? (int64_t)in[i0 + k] : 0;
-    const int64_t s = (v[0] + v[1]) + (v[2] + v[3]);
-    vmax = max(vmax, max(max(v[0], v[1]), max(v[2], v[3])));
+      for (int k = 0; k < SCAN_EPT / 4; ++k) {
+        const int4 q = reinterpret_cast<const int4*>(in + i0)[k];
+        v[4 * k] = (TI)q.x; v[4 * k + 1] = (TI)q.y; v[4 * k + 2] = (TI)q.z; v[4 * k + 3] = (TI)q.w;
+      }
+    } else {
+#pragma unroll
+      for (int k = 0; k < SCAN_EPT; ++k) v[k] = i0 + k < n ? in[i0 + k] : (TI)0;
+    }
+    int64_t s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_EPT; ++k) {
+      s += (int64_t)v[k];
+      vmax = max(vmax, (int64_t)v[k]);
+    }
     int64_t x = s;  // inclusive scan over the warp
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -97,12 +113,21 @@ __global__ void __launch_bounds__(1024) k_scan_single_block(const TI* __restrict
     }
     __syncthreads();
     int64_t run = carry + wsum[w] + (x - s);
+    if (vec_out && i0 + SCAN_EPT <= n) {
 #pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (i0 + k < n) {
-        out[i0 + k] = run;
-        run += v[k];
+      for (int k = 0; k < SCAN_EPT; k += 2) {  // (i0 is even)
+        const int64_t r1 = run + (int64_t)v[k];
+        *reinterpret_cast<longlong2*>(out + i0 + k) = make_longlong2(run, r1);
+        run = r1 + (int64_t)v[k + 1];
       }
+    } else {
+#pragma unroll
+      for (int k = 0; k < SCAN_EPT; ++k)
+        if (i0 + k < n) {
+          out[i0 + k] = run;
+          run += (int64_t)v[k];
+        }
+    }
     carry += tile_total;
     __syncthreads();  // wsum and tile_total are rewritten by the next tile
   }
