@@ -331,6 +331,13 @@ uint64_t gbe_launch_count(void);
  * Process-wide; returns the previous limit. */
 size_t gbe_set_build_scratch_limit(size_t bytes);
 
+/* Programmatic dependent launch of the SP2 kernels (sm_90+: the next kernel of an iteration becomes resident while the
+ * previous one drains and synchronises with it in the kernel).  It changes when kernels start, never what
+ * they compute: results are bit for bit the same on and off (tests/test_gpu_parity.py).  On by default; GBE_PDL=0 in the
+ * environment at load time, or on = 0 here, switches it off (debugging, profilers that cannot follow programmatic edges).
+ * Process-wide; affects calls made from now on; returns the previous setting (0 / 1). */
+int32_t gbe_set_dependent_launch(int32_t on);
+
 /* Largest core+halo size m_p the packed SP2 kernel takes in graphs built FROM NOW ON (see gbe_graph_set_sp2_path); larger
  * communities of the same graph run through the tiled kernel.  0 <= m <= 160 (160 = what fits one SM's shared memory,
  * and the default: one bin of up to 16 communities per SM).  Process-wide tuning knob; returns the previous value,

@@ -30,6 +30,7 @@ from .binding import (  # noqa: F401
     gbe_graph_set_gather_path,
     gbe_set_build_scratch_limit,
     gbe_set_packed_max_m,
+    gbe_set_dependent_launch,
     gbe_error_norms,
     gbe_graph_export,
     gbe_density,

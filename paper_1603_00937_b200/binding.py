@@ -21,7 +21,7 @@ EXPORTS = [
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
     "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation", "gbe_update_graph", "gbe_density_fermi",
     "gbe_graph_set_sp2_path", "gbe_error_norms", "gbe_graph_set_gather_path", "gbe_set_build_scratch_limit",
-    "gbe_set_packed_max_m", "gbe_expectation_static",
+    "gbe_set_packed_max_m", "gbe_expectation_static", "gbe_set_dependent_launch",
 ]
 
 
@@ -103,6 +103,8 @@ def lib() -> C.CDLL:
         l.gbe_set_build_scratch_limit.restype = C.c_size_t
         l.gbe_set_build_scratch_limit.argtypes = [C.c_size_t]
         l.gbe_expectation_static.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CsrView), C.c_void_p, C.c_void_p]
+        l.gbe_set_dependent_launch.restype = C.c_int32
+        l.gbe_set_dependent_launch.argtypes = [C.c_int32]
         l.gbe_set_packed_max_m.restype = C.c_int32
         l.gbe_set_packed_max_m.argtypes = [C.c_int32]
         l.gbe_launch_count.restype = C.c_uint64
@@ -252,6 +254,11 @@ def gbe_graph_set_gather_path(g: "Graph", path: int) -> None:
 def gbe_set_build_scratch_limit(nbytes: int) -> int:
     """Scratch limit of the graph builds for the candidate bitmaps (include/gbe.h); returns the previous limit."""
     return int(lib().gbe_set_build_scratch_limit(int(nbytes)))
+
+
+def gbe_set_dependent_launch(on: bool) -> bool:
+    """Programmatic dependent launch of the SP2 kernels on / off (process-wide); returns the previous setting."""
+    return bool(lib().gbe_set_dependent_launch(1 if on else 0))
 
 
 def gbe_set_packed_max_m(m: int) -> int:

@@ -12,8 +12,6 @@ std::atomic<uint64_t> g_gbe_launches{0};
 // communities up to this size go to the packed kernel (gbe_small.cu); 116: the largest whose X fits half an SM's shared
 // memory, so that two bins share an SM
 static std::atomic<int32_t> g_pk_max_m{GBE_PK_MAX_M};
-// programmatic dependent launch on the tiled SP2 path (GBE_X2_PDL=0 in the environment switches it off: debugging)
-static std::atomic<int> g_x2_pdl{[] { const char* e = getenv("GBE_X2_PDL"); return e ? (atoi(e) != 0 ? 1 : 0) : 1; }()};
 int gbe_packed_max_m() { return g_pk_max_m.load(); }
 
 namespace {
@@ -361,7 +359,7 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
     // X^2 launch go the moment its decision is visible (GBE_PDL_EARLY: that launch never waits).  Without traces an X^2
     // launch follows an X^2 launch and would have to wait at its top: measured slower than plain stream order on small
     // systems (its CTAs become resident next to the running ones and only wait), no gain on large ones - not used.
-    const int pdl = g_x2_pdl.load(std::memory_order_relaxed) && mode != 2 ? GBE_PDL_EARLY : GBE_PDL_NONE;
+    const int pdl = gbe_pdl_enabled() && mode != 2 ? GBE_PDL_EARLY : GBE_PDL_NONE;
     GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, g->n_items ? 1 : 0,
                   [&] { return gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, false, it & 1, s, pdl); }));
     if (mode != 2)
@@ -584,6 +582,8 @@ int gbe_error_norms(const gbe_graph* g, const double* D_val, const double* D_ref
   GBE_CUDA(cudaStreamSynchronize(s));
   return GBE_OK;
 }
+
+int32_t gbe_set_dependent_launch(int32_t on) { return gbe_pdl_set(on != 0); }
 
 int32_t gbe_set_packed_max_m(int32_t m) {
   if (m < 0 || m > GBE_PK_MAX_M) return -1;

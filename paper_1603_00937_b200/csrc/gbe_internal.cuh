@@ -204,6 +204,8 @@ struct gbe_graph {
 //                  when it starts
 // ----------------------------------------------------------------------------------------------
 enum { GBE_PDL_NONE = 0, GBE_PDL_TOP = 1, GBE_PDL_EARLY = 2 };
+bool gbe_pdl_enabled();   // the process-wide switch (gbe_util.cu; gbe_set_dependent_launch, GBE_PDL=0)
+int gbe_pdl_set(int on);  // returns the previous setting
 #ifdef __CUDACC__
 __device__ __forceinline__ void gbe_griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void gbe_griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }

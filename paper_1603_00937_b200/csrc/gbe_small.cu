@@ -64,7 +64,6 @@ constexpr int PK_MAX_ROUNDS = 32;        // units per warp (lane j of a warp fet
 constexpr unsigned PK_NONE = 0xFFFFu;
 constexpr int PK_PAD = 4;                // shared-memory row stride = ld + 4 doubles (ld is a multiple of 16): the 16 doubles a
                                          // half warp loads with LDS.64 (4 rows x 4 columns) fall into distinct banks
-std::atomic<int> g_pk_pdl{1};  // programmatic dependent launch of the packed kernel (GBE_PK_PDL=0 in the environment: off)
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -553,7 +552,6 @@ int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, 
     GBE_CUDA(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     GBE_CUDA(cudaFuncSetAttribute(k_sp2_packed, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max - 2048));
     GBE_CUDA(cudaFuncSetAttribute(k_sp2_packed, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-    if (const char* e = getenv("GBE_PK_PDL")) g_pk_pdl.store(atoi(e) != 0, std::memory_order_relaxed);
   }
   const gbe_pk_class& a = g->pk[0];
   // programmatic stream serialisation: the grid may be scheduled before the previous kernel of the stream has finished;
@@ -567,7 +565,7 @@ int gbe_launch_sp2_packed(const gbe_graph* g, gbe_state* st, const double* Xin, 
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = g_pk_pdl.load(std::memory_order_relaxed) ? 1 : 0;
+  cfg.numAttrs = gbe_pdl_enabled() ? 1 : 0;
   GBE_CUDA(cudaLaunchKernelEx(&cfg, k_sp2_packed, (const gbe_pk_cta*)a.ctas, (const uint16_t*)a.codes,
                               (const gbe_pk_row*)a.rows, st, Xin, Xout,
                               partials, partial_base, n_partials, iter, last ? 1 : 0, fused, (int)a.code_stride,

@@ -1,4 +1,6 @@
 // Small device utilities: exclusive scans used while sizing CSR outputs (not on the per-iteration path).
+#include <cstdlib>
+
 #include "gbe_internal.cuh"
 
 // ---------------------------------------------------------------------------------------------- allocator
@@ -20,6 +22,12 @@ int gbe_sm_count() {
   if (dev >= 0 && dev < 256) cached[dev].store(n, std::memory_order_relaxed);
   return n;
 }
+// programmatic dependent launch (gbe_internal.cuh), process-wide: on unless GBE_PDL=0 is in the environment when the
+// library is loaded; gbe_set_dependent_launch (gbe.h) changes it
+static std::atomic<int> g_pdl{[] { const char* e = getenv("GBE_PDL"); return e ? (atoi(e) != 0 ? 1 : 0) : 1; }()};
+bool gbe_pdl_enabled() { return g_pdl.load(std::memory_order_relaxed) != 0; }
+int gbe_pdl_set(int on) { return g_pdl.exchange(on ? 1 : 0, std::memory_order_relaxed); }
+
 void gbe_set_alloc_stream(cudaStream_t s) {
   static gbe_device_once pool_ready;  // per device: the release threshold belongs to the device's default pool
   if (pool_ready.first()) {

@@ -60,6 +60,7 @@ def test_sass_uses_fp64_tensor_cores_and_async_copies(libpath):
     assert "LDGSTS" in sass          # cp.async staging of the X panels
     assert "UTMALDG" in sass         # 2-D tensor-map TMA loads of the X^2 panels (cp.async.bulk.tensor)
     assert "UBLKCP" in sass          # TMA bulk copies (cp.async.bulk) of the packed small-m kernel
+    assert "ACQBULK" in sass and "PREEXIT" in sass  # griddepcontrol.wait / .launch_dependents (dependent launch)
     assert "sm_100a" in sass
 
 

@@ -1014,3 +1014,56 @@ def test_errors(gbe):
     with pytest.raises(gbe.GbeError) as e:
         gbe.gbe_density(gbe.DeviceCSR.from_host(gi.chain(32, 4).H), g, 16.0, 10)
     assert e.value.status == -4
+
+
+# ------------------------------------------------------------------------------- programmatic dependent launch
+def test_dependent_launch_changes_when_kernels_start_not_what_they_compute(gbe):
+    """include/gbe.h gbe_set_dependent_launch: the SP2 kernels of an iteration are launched as programmatic dependents of
+    one another (the trace kernel waits for the X^2 launch and releases the next one after its decision; the bins of the
+    packed kernel wait for the previous launch).  Switching that off must not change a single bit - tiled path (both X^2
+    kernels: cp.async and TMA panels), packed path, with an idempotency stop in the middle of the loop, eagerly and
+    replayed from a CUDA graph."""
+    import torch
+    cases = [(gi.config(2), dict(iters=40, idem_tol=-1.0)),              # 6,144 orbitals, TMA panels (mean m >= 360)
+             (gi.config(1), dict(iters=60, idem_tol=1e-9)),              # chain, cp.async panels, stops on the device
+             (gi.chain(4800, 600, seed=5), dict(iters=40, idem_tol=-1.0))]  # 600 small communities: packed kernel
+    prev = gbe.gbe_set_dependent_launch(True)
+    try:
+        for s, kw in cases:
+            Hd = gbe.DeviceCSR.from_host(s.H)
+            part_t = torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
+            g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
+            for path in ((1, 3) if g.info["n_small"] == s.n_part else (1,)):
+                gbe.gbe_graph_set_sp2_path(g, path)
+                out = {}
+                for on in (True, False, True):
+                    assert gbe.gbe_set_dependent_launch(on) in (True, False)
+                    D, log = gbe.gbe_density(Hd, g, s.n_occ, kw["iters"], kw["idem_tol"])
+                    torch.cuda.synchronize()
+                    key = (D.clone(), log.t1.copy(), log.t2.copy(), log.branch.copy(), log.iters_done)
+                    if on in out:
+                        ref = out[on]
+                    else:
+                        out[on] = key
+                        ref = out[True]
+                    assert torch.equal(ref[0], key[0]) and np.array_equal(ref[1], key[1]) and np.array_equal(ref[2], key[2])
+                    assert np.array_equal(ref[3], key[3]) and ref[4] == key[4]
+                # replay from a CUDA graph captured with dependent launches on
+                gbe.gbe_set_dependent_launch(True)
+                ws = g.new_workspace()
+                Dg = torch.empty(g.info["nnz_D"], dtype=torch.float64, device="cuda")
+                st = torch.cuda.Stream()
+                with torch.cuda.stream(st):
+                    gbe.gbe_density(Hd, g, s.n_occ, kw["iters"], kw["idem_tol"], workspace=ws, D_val=Dg, want_log=False, stream=st)
+                    st.synchronize()
+                    cg = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(cg, stream=st):
+                        gbe.gbe_density(Hd, g, s.n_occ, kw["iters"], kw["idem_tol"], workspace=ws, D_val=Dg, want_log=False,
+                                        stream=st)
+                    Dg.zero_()
+                    cg.replay()
+                    st.synchronize()
+                assert torch.equal(Dg, out[True][0])
+            g.free()
+    finally:
+        gbe.gbe_set_dependent_launch(prev)
