@@ -108,7 +108,7 @@ typedef struct {
   double sp2_sym_flops_per_iter; /* sum_p m_p^2 (m_p + 1): the flops of one SP2 iteration the METHOD needs when the symmetry
                                     of X_p is used (only the entries on or above the diagonal of X_p^2 are formed; obs. (x)
                                     P:L65) - the numerator of bench.py's roofline fraction */
-  int64_t n_small;           /* communities with 0 < m_p <= 112 (gbe_set_packed_max_m): the ones the packed kernel takes */
+  int64_t n_small;           /* communities with 0 < m_p <= 160 (gbe_set_packed_max_m): the ones the packed kernel takes */
   int64_t n_bins;            /* CTAs of one packed launch (bins of 1..16 small communities) */
   size_t workspace_bytes_preset_min; /* smallest workspace gbe_density_preset(trace_every_iteration = 0) accepts: it then
                                         works through the communities in waves (see there) */
@@ -162,11 +162,12 @@ int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, 
 
 /* Which kernels run the SP2 loop (steps 4-5) of this graph.  Three implementations compute the same updates:
  *   tiled    (any size)  one X^2 launch + one trace/branch launch per iteration over the batched dense layout in HBM;
- *   packed   (communities with m_p <= 112 [gbe_set_packed_max_m], any number of them; the cost law P:L78 - more partitions, smaller m)
+ *   packed   (communities with m_p <= 160 [gbe_set_packed_max_m], any number of them; the cost law P:L78 - more partitions, smaller m)
  *            one launch per iteration: a CTA copies a bin of 1..16 whole matrices to shared memory, squares them on the
- *            FP64 tensor cores, writes them back; the bin that finishes last reduces the traces and takes the branch
- *            decision, so there is no separate trace/branch launch.  Larger communities of the same graph go through the
- *            tiled kernel in the same iteration;
+ *            FP64 tensor cores, writes them back and leaves one trace pair; the bins of the NEXT launch sum those pairs
+ *            (the same fixed order in every bin) and take the branch decision themselves, so there is no separate
+ *            trace/branch launch between iterations (one after the last).  Larger communities of the same graph go
+ *            through the tiled kernel in the same iteration (the decision is then taken by the bin that finishes last);
  *   resident (max_m <= 160) ONE launch for the whole loop, X_p held in shared memory by one CTA per community; the
  *            global trace (one sequence for all subgraphs) is exchanged through a grid barrier, which needs all
  *            communities co-resident (cooperative launch; one thread-block cluster with the exchange in distributed
