@@ -734,6 +734,50 @@ def run_fermi(args) -> None:
                       "tflops_alg": info["sp2_flops_per_iter"] * (order - 1) / (t * 1e-3) * 1e-12}), flush=True)
 
 
+def run_trace_build(args) -> None:
+    """Timeline of gbe_build_graph (steps 0-2) on the bench workload: every kernel, copy and memset with its start time
+    (CUPTI through torch.profiler - a library used for this report only), so that device IDLE time shows: the span of one
+    build, the time the device is busy in it, and the gaps.  One JSON line; profiles/r02_graph_build.md records it."""
+    import re
+    import torch
+    from torch.profiler import profile, ProfilerActivity
+    from paper_1603_00937_b200 import build as gbe_build
+    gbe_build.build()
+    import paper_1603_00937_b200 as gbe
+    s = make_system(args.workload, seed=0)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    part_t = None if s.meta.get("kind") == "water" else torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
+    for _ in range(3):
+        gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part).free()
+    torch.cuda.synchronize()
+    with profile(activities=[ProfilerActivity.CPU, ProfilerActivity.CUDA]) as prof:
+        for _ in range(3):
+            gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part).free()
+        torch.cuda.synchronize()
+    import tempfile
+    with tempfile.TemporaryDirectory() as td:  # the chrome-trace export is the profiler's stable interface
+        fn = os.path.join(td, "trace.json")
+        prof.export_chrome_trace(fn)
+        with open(fn) as f:
+            tr = json.load(f)["traceEvents"]
+    ev = sorted((e["ts"], e["ts"] + e["dur"], e["name"]) for e in tr if e.get("cat") in ("kernel", "gpu_memcpy", "gpu_memset"))
+    starts = [i for i, e in enumerate(ev) if "k_row_bounds" in e[2]]
+    seg = ev[starts[1]:starts[2]]  # the second of the three profiled builds
+    t0, t1 = seg[0][0], max(e[1] for e in seg)
+    busy = sum(e[1] - e[0] for e in seg)
+    gaps, prev = [], None
+    for a, b, name in seg:
+        m = re.search(r"(k_[a-z0-9_]+(<[^>]*>)?)", name)
+        if prev is not None and a - prev > 8.0:
+            gaps.append({"at_us": round(a - t0, 1), "gap_us": round(a - prev, 1), "before": m.group(1) if m else name[:40]})
+        prev = max(prev or 0, b)
+    top = sorted(({"name": (re.search(r"(k_[a-z0-9_]+(<[^>]*>)?)", n) or re.match(r".{0,40}", n)).group(0), "us": round(b - a, 1)}
+                  for a, b, n in seg), key=lambda d: -d["us"])[:8]
+    print(json.dumps({"trace_build": args.workload, "n": s.n, "n_part": s.n_part, "device_ops": len(seg),
+                      "span_us": round(t1 - t0, 1), "busy_us": round(busy, 1), "idle_us": round(t1 - t0 - busy, 1),
+                      "gaps_over_8us": gaps, "longest": top}), flush=True)
+
+
 def run_waves(args) -> None:
     """SURVEY 8(f) item 1 in a bounded workspace: gbe_density_preset without traces on the whole batch against the same call
     in a workspace of --waves-gb GB (waves of communities: no exchange between the expansions).  One JSON line."""
@@ -872,6 +916,7 @@ def main() -> None:
     ap.add_argument("--sweep-taus", default="", help="comma-separated thresholds of the sweep (default: the five of configs[4])")
     ap.add_argument("--sp2-path", type=int, default=0, help="sweep: force the SP2 kernels (1 tiled, 2 resident, 3 packed; 0 = the library's choice)")
     ap.add_argument("--waves", action="store_true", help="gbe_density_preset on the whole batch against the same call in a bounded workspace")
+    ap.add_argument("--trace-build", action="store_true", help="timeline of one gbe_build_graph: device busy / idle time, gaps")
     ap.add_argument("--waves-gb", type=float, default=8.0, help="--waves: size of the bounded workspace in GB")
     ap.add_argument("--clock-sampler", default="nvml", choices=["nvml", "nvidia-smi", "none"],
                     help="how clocks / throttle reasons are sampled during the timed region (nvml: a thread of this process)")
@@ -886,6 +931,8 @@ def main() -> None:
         run_small(args)
     elif args.waves:
         run_waves(args)
+    elif args.trace_build:
+        run_trace_build(args)
     elif args.fermi:
         run_fermi(args)
     elif args.impl == "reference":
