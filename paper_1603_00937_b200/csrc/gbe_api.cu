@@ -331,7 +331,7 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
     // Iteration iters - 1 is the last one whether or not the idempotency stop fires before it (then it is a no-op):
     // only the core rows and columns of its result are read again (trace, scatter), so it runs the core tiles only.
     const bool last = it == iters - 1;
-    if (path == 3 && inplace && mode != 2) {
+    if (path == 3 && inplace && mode != 2 && 2 * g->n_pk_ctas <= g->n_partials) {  // (always: n_partials >= 2 n_part)
       // every community packed: one launch per iteration and NO step-5 tail - the bins of launch it + 1 sum the pairs of
       // launch it themselves (lazy decision, gbe_small.cu); the pairs alternate between two halves of `partials`
       const int nb = g->n_pk_ctas;
