@@ -167,14 +167,14 @@ int gbe_graph_export(const gbe_graph* g, void* cuda_stream, int64_t* S_row_ptr, 
  *            FP64 tensor cores, writes them back and leaves one trace pair; the bins of the NEXT launch sum those pairs
  *            (the same fixed order in every bin) and take the branch decision themselves, so there is no separate
  *            trace/branch launch between iterations (one after the last).  Larger communities of the same graph go
- *            through the tiled kernel in the same iteration (the decision is then taken by the bin that finishes last);
+ *            through the tiled kernel in the same iteration, launched next to the bins;
  *   resident (max_m <= 160) ONE launch for the whole loop, X_p held in shared memory by one CTA per community; the
  *            global trace (one sequence for all subgraphs) is exchanged through a grid barrier, which needs all
  *            communities co-resident (cooperative launch; one thread-block cluster with the exchange in distributed
  *            shared memory when there are at most 16 communities) - unless the sequence is preset and no trace is logged
  *            (gbe_density_preset with trace_every_iteration = 0), where the CTAs never communicate.
  * path = 0 (default): resident when it applies and all communities fit the device at once; else packed when the graph
- *        has enough small communities to occupy the device; else tiled;
+ *        has enough small communities to occupy the device and at most a few larger ones; else tiled;
  *        1: always tiled;  2: resident whenever it can run (GBE_EINVAL if max_m is too large; calls for which the
  *        communities are not co-resident still take the tiled kernels);  3: packed whenever the graph has a community
  *        small enough (else tiled).

@@ -265,6 +265,10 @@ static int choose_sp2(const gbe_graph* g, int mode) {
   // a graph that also needs the tiled kernel for some communities pays a second, poorly filled launch per iteration and
   // is not faster than the tiled kernels alone).
   if (can_pk && g->n_pk_ctas >= gbe_sm_count() / 2 && g->n_items_h == 0) return 3;
+  // Mixed graph, nearly everything packed: the tiled launch for the few larger communities (at most two tiles per SM)
+  // runs next to the last wave of bins (do_sp2); measured on tau = 1e-3 x 512 communities (504 packed, 8 tiled).  Not
+  // for a pre-set sequence without traces, which has no decision to synchronise on and keeps the serial pair of launches.
+  if (can_pk && mode != 2 && g->n_pk_ctas >= gbe_sm_count() && g->n_items_h > 0 && g->n_items_h <= 2 * gbe_sm_count()) return 3;
   return 1;
 }
 
@@ -343,9 +347,28 @@ static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_t
         GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials + 2 * (size_t)((it & 1) * nb), nb, s); }));
       continue;
     }
+    if (path == 3 && g->n_items_h > 0 && mode != 2 && 2 * (g->n_items_last_h + g->n_pk_ctas) <= g->n_partials) {
+      // MIXED graph, lazy decision over both kinds of pairs.  The packed launch goes first; the tiled launch for the few
+      // larger communities follows as its programmatic dependent: it becomes resident when the last bins have started -
+      // on the SMs the last, partly filled wave of bins leaves free - waits at its top for the branch of the iteration
+      // (published by bin 0: fence + state.iter) and at its end for the packed launch to complete, so that the packed
+      // launch of the next iteration, which waits for the tiled launch only, finds both done.  Pairs: [tiles | bins],
+      // alternating between two halves of `partials`.
+      const int nh = g->n_items_last_h, nb = g->n_pk_ctas, np = nh + nb;
+      const int base = (it & 1) * np, prev = ((it - 1) & 1) * np;
+      const int pdl = gbe_pdl_enabled() ? GBE_PDL_TOP : GBE_PDL_NONE;
+      GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, 2, [&]() -> int {
+        GBE_TRY(gbe_launch_sp2_packed(g, w.st, in, outp, w.partials, base + nh, np, it, last, 2, prev, it > 0 ? np : 0, s));
+        return gbe_launch_x2(g, w.st, in, outp, w.partials + 2 * (size_t)base, it, last, true, it & 1, s, pdl, true);
+      }));
+      if (last)
+        GBE_TRY(timed(tm, PH_TRACE, 1, [&] { return gbe_launch_trace_branch(w.st, w.partials + 2 * (size_t)base, np, s); }));
+      continue;
+    }
     if (path == 3) {
-      // small communities: bins in shared memory, one launch per iteration, step 5 taken by the bin that arrives last
-      // (gbe_small.cu); the larger communities of the same graph go through the tiled kernel first
+      // (pre-set sequence without traces, or no room for two sets of pairs) small communities: bins in shared memory, one
+      // launch per iteration, step 5 taken by the bin that arrives last (gbe_small.cu); the larger communities of the
+      // same graph go through the tiled kernel first
       const int n_pairs = g->n_items_last_h + g->n_pk_ctas;
       GBE_TRY(timed(tm, last ? PH_X2_LAST : PH_X2, (g->n_items_h ? 1 : 0) + 1, [&]() -> int {
         GBE_TRY(gbe_launch_x2(g, w.st, in, outp, w.partials, it, last, true, it & 1, s));

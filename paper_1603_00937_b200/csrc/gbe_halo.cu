@@ -461,7 +461,8 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
   GBE_TRY(gbe_build_packed(g, s));  // bins of the small communities (gbe_small.cu)
   GBE_TRY(gbe_x2_build_tmaps(g, s));  // tensor maps of the tiled kernel's panels (gbe_x2.cu); needs dense_off on the device
   // the resident kernel double-buffers n_part pairs; the packed path writes one pair per bin behind the tiled kernel's
-  g->n_partials = std::max(std::max(std::max(g->n_items, g->n_gitems), 2 * n_part), g->n_items_last_h + g->n_pk_ctas);
+  // (a mixed graph alternates between two sets of tile + bin pairs: the lazy decision, gbe_api.cu)
+  g->n_partials = std::max(std::max(std::max(g->n_items, g->n_gitems), 2 * n_part), 2 * (g->n_items_last_h + g->n_pk_ctas));
   // wave mode (gbe_plan_waves): the gather of a later wave must not touch the final pairs of an earlier one
   g->n_partials = std::max(g->n_partials, g->n_items_last + g->n_gitems);
   GBE_TRY(gbe_resident_capacity(g, &g->resident_fits, &g->resident_coresident, &g->resident_cluster));

@@ -216,6 +216,11 @@ __device__ __forceinline__ int gbe_ld_state(const int32_t* p) {
   asm volatile("ld.global.cg.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
+__device__ __forceinline__ int gbe_ld_acquire(const int32_t* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
 __device__ __forceinline__ int gbe_ld_state(const uint8_t* p) {
   int v;
   asm volatile("ld.global.cg.u8 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -263,10 +268,12 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
 // buffer: which dense buffer Xin is (0 or 1: selects the tensor maps)
 // pdl: programmatic dependent launch (GBE_PDL_*): the grid may become resident before the previous kernel of the stream
 // has finished and synchronises with it in the kernel
+// hyb: the launch runs NEXT TO the packed launch of the same iteration (mixed graphs, gbe_api.cu): its CTAs wait at their
+// top until that launch has published the branch of the iteration, and at their end until it has completed
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                  bool last, bool hybrid, int buffer, cudaStream_t s, int pdl = 0);
+                  bool last, bool hybrid, int buffer, cudaStream_t s, int pdl = 0, bool hyb = false);
 int gbe_launch_x2_items(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                        const gbe_tile_item* items, int n_items, int buffer, cudaStream_t s, int pdl = 0);
+                        const gbe_tile_item* items, int n_items, int buffer, cudaStream_t s, int pdl = 0, bool hyb = false);
 int gbe_plan_waves(const gbe_graph* g, size_t cap_elems, cudaStream_t s);  // gbe_halo.cu
 int gbe_x2_build_tmaps(gbe_graph* g, cudaStream_t s);                                        // once per graph
 int gbe_x2_prepare(const gbe_graph* g, const double* X0, const double* X1, cudaStream_t s);  // once per density call
@@ -336,7 +343,8 @@ __device__ __forceinline__ void gbe_trace_decide(gbe_state* st, double t1, doubl
     const int b = st->preset ? (int)st->br[k] : ((fabs(t2 - n_occ) < fabs(2.0 * t1 - t2 - n_occ)) ? 0 : 1);
     st->branch = b;
     st->br[k] = (uint8_t)b;
-    st->iter = k + 1;
+    __threadfence();   // iter == k + 1 PUBLISHES the branch of iteration k: the tiled kernel of a mixed graph runs next to
+    st->iter = k + 1;  // the packed kernel that decides and reads iter with acquire (gbe_x2.cu, hyb)
   }
 }
 __device__ __forceinline__ double warp_sum(double v) {

@@ -111,7 +111,7 @@ template <int MINB, int OP>
 __global__ void __launch_bounds__(X2_THREADS, MINB)
     k_x2(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin,
          double* __restrict__ Xout, double* __restrict__ partials, int iter, const double* __restrict__ Xb,
-         double* __restrict__ Dacc, const double* __restrict__ coef) {
+         double* __restrict__ Dacc, const double* __restrict__ coef, int hyb) {
   extern __shared__ __align__(16) double smem[];  // 2 stages x (A panel, B panel)
   __shared__ double red[8];
 
@@ -122,6 +122,10 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   // state is read with uncached loads (a line of it may sit in this SM's L1 from the previous launch), requested here
   // and looked at after the tile's own set-up so that their latency costs nothing.
   gbe_griddep_launch();
+  // hyb (mixed graph: this launch runs next to the packed launch of the same iteration, whose first bin takes the
+  // decision): until the branch of THIS iteration is published (iter advanced) or the stop flag is up
+  if (OP == 0 && hyb)
+    while (gbe_ld_acquire(&st->iter) != iter + 1 && !gbe_ld_state(&st->stop)) __nanosleep(200);
   const int stop0 = OP == 0 ? gbe_ld_state(&st->stop) : 0;
   const int br_preset = OP == 0 ? gbe_ld_state(&st->preset) : 0;
   const int br_given = OP == 0 && iter < GBE_MAX_ITERS ? gbe_ld_state(&st->br[iter]) : 0;
@@ -222,7 +226,10 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
     }
   };
 
-  if (stop0) return;  // idempotency stop already fired (A-7): X is final
+  if (stop0) {  // idempotency stop already fired (A-7): X is final
+    if (OP == 0 && hyb) gbe_griddep_wait();
+    return;
+  }
   const int branch = br_preset ? br_given : br_chosen;  // preset sequence or the on-device choice
   issue(0, 0);
   for (int kc = 0; kc < nchunks; kc += 2) {
@@ -323,15 +330,19 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   // only the tiles with a core row carry a trace; their partials are packed (pidx), so that step 5 reads n_tiles_last
   // pairs instead of one per tile
   const int pidx = it0.x;
-  if (OP != 0 || pidx < 0) return;
-  s1 = warp_sum(s1);
-  s2 = warp_sum(s2);
-  if (lane == 0) { red[role] = s1; red[4 + role] = s2; }  // indexed by block position: order independent of the rotation
-  __syncthreads();
-  if (t == 0) {
-    partials[2 * (size_t)pidx] = (red[0] + red[1]) + (red[2] + red[3]);
-    partials[2 * (size_t)pidx + 1] = (red[4] + red[5]) + (red[6] + red[7]);
+  if (OP == 0 && pidx >= 0) {
+    s1 = warp_sum(s1);
+    s2 = warp_sum(s2);
+    if (lane == 0) { red[role] = s1; red[4 + role] = s2; }  // indexed by block position: order independent of the rotation
+    __syncthreads();
+    if (t == 0) {
+      partials[2 * (size_t)pidx] = (red[0] + red[1]) + (red[2] + red[3]);
+      partials[2 * (size_t)pidx + 1] = (red[4] + red[5]) + (red[6] + red[7]);
+    }
   }
+  // hyb: this grid must not count as complete before the packed launch next to it is (the launch behind this one waits
+  // for THIS grid only, and needs both)
+  if (OP == 0 && hyb) gbe_griddep_wait();
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -409,13 +420,16 @@ __device__ __forceinline__ void xt_chunk(double (&acc)[2][8][2], const double* _
 template <int MINB>
 __global__ void __launch_bounds__(X2_THREADS, MINB)
     k_x2_tma(const gbe_tile_item* __restrict__ items, const gbe_state* __restrict__ st, const double* __restrict__ Xin,
-             double* __restrict__ Xout, double* __restrict__ partials, int iter, const CUtensorMap* __restrict__ maps) {
+             double* __restrict__ Xout, double* __restrict__ partials, int iter, const CUtensorMap* __restrict__ maps,
+             int hyb) {
   extern __shared__ __align__(1024) double smem_t[];  // 3 stages x (A panel, B panel), every panel 1024-byte aligned
   __shared__ double red[8];
   __shared__ __align__(8) unsigned long long bars[2 * XT_NST];  // full[0..2], empty[0..2]
 
-  // programmatic dependent launch and state loads: as in k_x2
+  // programmatic dependent launch, hyb and state loads: as in k_x2
   gbe_griddep_launch();
+  if (hyb)
+    while (gbe_ld_acquire(&st->iter) != iter + 1 && !gbe_ld_state(&st->stop)) __nanosleep(200);
   const int stop0 = gbe_ld_state(&st->stop);  // requested here, looked at after the mbarrier set-up
   const int br_preset = gbe_ld_state(&st->preset);
   const int br_given = iter < GBE_MAX_ITERS ? gbe_ld_state(&st->br[iter]) : 0;
@@ -447,7 +461,10 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  if (stop0) return;  // idempotency stop already fired (A-7): X is final
+  if (stop0) {  // idempotency stop already fired (A-7): X is final
+    if (hyb) gbe_griddep_wait();
+    return;
+  }
   const int branch = br_preset ? br_given : br_chosen;
   const uint32_t stage_bytes = share ? XT_PANEL * 8u : XT_STAGE * 8u;
   auto produce = [&](int s, int kc) {  // thread 0: chunk kc -> stage s
@@ -599,15 +616,17 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
     epilogue(std::false_type{}, std::false_type{}, std::false_type{});
   }
   const int pidx = it0.x;
-  if (pidx < 0) return;
-  s1 = warp_sum(s1);
-  s2 = warp_sum(s2);
-  if (lane == 0) { red[role] = s1; red[4 + role] = s2; }
-  __syncthreads();
-  if (t == 0) {
-    partials[2 * (size_t)pidx] = (red[0] + red[1]) + (red[2] + red[3]);
-    partials[2 * (size_t)pidx + 1] = (red[4] + red[5]) + (red[6] + red[7]);
+  if (pidx >= 0) {
+    s1 = warp_sum(s1);
+    s2 = warp_sum(s2);
+    if (lane == 0) { red[role] = s1; red[4 + role] = s2; }
+    __syncthreads();
+    if (t == 0) {
+      partials[2 * (size_t)pidx] = (red[0] + red[1]) + (red[2] + red[3]);
+      partials[2 * (size_t)pidx + 1] = (red[4] + red[5]) + (red[6] + red[7]);
+    }
   }
+  if (hyb) gbe_griddep_wait();
 }
 
 // Tensor maps.  A map describes ONE community's X_p in ONE dense buffer ([m_p rows][ld_p doubles], box 64 x 16, 128-byte
@@ -698,7 +717,7 @@ namespace {
 template <int MINB, int OP>
 int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
               const double* Xb, double* Dacc, const double* coef, const gbe_tile_item* items, int n_items,
-              cudaStream_t s, int pdl) {
+              cudaStream_t s, int pdl, bool hyb) {
   auto kern = k_x2<MINB, OP>;
   const size_t smem = (size_t)2 * X2_STAGE * sizeof(double);
   static gbe_device_once configured;  // one per template instance; function attributes are per device
@@ -707,23 +726,23 @@ int launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout
     GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
   }
   GBE_CUDA(gbe_launch_kernel(kern, dim3((unsigned)n_items), dim3(X2_THREADS), smem, s, pdl != GBE_PDL_NONE, items, st, Xin,
-                             Xout, partials, iter, Xb, Dacc, coef));
+                             Xout, partials, iter, Xb, Dacc, coef, hyb ? 1 : 0));
   GBE_LAUNCHED();
   return GBE_OK;
 }
 }  // namespace
 
 int gbe_launch_x2(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                  bool last, bool hybrid, int buffer, cudaStream_t s, int pdl) {
+                  bool last, bool hybrid, int buffer, cudaStream_t s, int pdl, bool hyb) {
   // the last SP2 iteration computes the tiles with a core row only: the scatter keeps core columns (Eq.(6));
   // hybrid: the communities with m <= GBE_PK_MAX_M are the packed kernel's (gbe_small.cu), only the others are tiled
   const gbe_tile_item* items = hybrid ? (last ? g->items_last_h : g->items_h) : (last ? g->items_last : g->items);
   const int n_items = hybrid ? (last ? g->n_items_last_h : g->n_items_h) : (last ? g->n_items_last : g->n_items);
-  return gbe_launch_x2_items(g, st, Xin, Xout, partials, iter, items, n_items, buffer, s, pdl);
+  return gbe_launch_x2_items(g, st, Xin, Xout, partials, iter, items, n_items, buffer, s, pdl, hyb);
 }
 
 int gbe_launch_x2_items(const gbe_graph* g, gbe_state* st, const double* Xin, double* Xout, double* partials, int iter,
-                        const gbe_tile_item* items, int n_items, int buffer, cudaStream_t s, int pdl) {
+                        const gbe_tile_item* items, int n_items, int buffer, cudaStream_t s, int pdl, bool hyb) {
   if (n_items == 0) return GBE_OK;
   if (g->tmaps) {  // panels staged by 2-D TMA (k_x2_tma); X_n is in buffer 0 for even iterations, in buffer 1 for odd ones
     const CUtensorMap* maps = reinterpret_cast<const CUtensorMap*>(g->tmaps) + (buffer ? g->n_part : 0);
@@ -735,15 +754,15 @@ int gbe_launch_x2_items(const gbe_graph* g, gbe_state* st, const double* Xin, do
       GBE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     }
     GBE_CUDA(gbe_launch_kernel(kern, dim3((unsigned)n_items), dim3(X2_THREADS), smem, s, pdl != GBE_PDL_NONE, items, st,
-                               Xin, Xout, partials, iter, maps));
+                               Xin, Xout, partials, iter, maps, hyb ? 1 : 0));
     GBE_LAUNCHED();
     return GBE_OK;
   }
-  return launch_x2<4, 0>(g, st, Xin, Xout, partials, iter, nullptr, nullptr, nullptr, items, n_items, s, pdl);
+  return launch_x2<4, 0>(g, st, Xin, Xout, partials, iter, nullptr, nullptr, nullptr, items, n_items, s, pdl, hyb);
 }
 
 int gbe_launch_cheb_step(const gbe_graph* g, gbe_state* st, const double* Xt, const double* Tn, double* Tio, double* Dacc,
                          const double* coef, int iter, double* partials, cudaStream_t s) {
   if (g->n_items == 0) return GBE_OK;
-  return launch_x2<4, 1>(g, st, Xt, Tio, partials, iter, Tn, Dacc, coef, g->items, g->n_items, s, GBE_PDL_NONE);
+  return launch_x2<4, 1>(g, st, Xt, Tio, partials, iter, Tn, Dacc, coef, g->items, g->n_items, s, GBE_PDL_NONE, false);
 }

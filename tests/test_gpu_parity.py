@@ -1026,14 +1026,17 @@ def test_dependent_launch_changes_when_kernels_start_not_what_they_compute(gbe):
     import torch
     cases = [(gi.config(2), dict(iters=40, idem_tol=-1.0)),              # 6,144 orbitals, TMA panels (mean m >= 360)
              (gi.config(1), dict(iters=60, idem_tol=1e-9)),              # chain, cp.async panels, stops on the device
-             (gi.chain(4800, 600, seed=5), dict(iters=40, idem_tol=-1.0))]  # 600 small communities: packed kernel
+             (gi.chain(4800, 600, seed=5), dict(iters=40, idem_tol=-1.0)),  # 600 small communities: packed kernel
+             # mixed graph (m ~ 65 - 185): the tiled launch for the larger communities runs NEXT TO the packed launch of
+             # the same iteration and synchronises with it through the published decision; stops on the device
+             (gi.water_box(1024, 128, seed=0, tau=1e-3, iters=30), dict(iters=30, idem_tol=1e-7, paths=(1, 3)))]
     prev = gbe.gbe_set_dependent_launch(True)
     try:
         for s, kw in cases:
             Hd = gbe.DeviceCSR.from_host(s.H)
             part_t = torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
             g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
-            for path in ((1, 3) if g.info["n_small"] == s.n_part else (1,)):
+            for path in kw.get("paths", (1, 3) if g.info["n_small"] == s.n_part else (1,)):
                 gbe.gbe_graph_set_sp2_path(g, path)
                 out = {}
                 for on in (True, False, True):
