@@ -556,7 +556,8 @@ int gbe_density_fermi(const gbe_csr_view* H, const gbe_graph* g, double mu, doub
   for (int n = 1; n < order; ++n) {  // T_{n+1} from T_n (B operand) and T_{n-1} (overwritten), coefficient c_{n+1}
     const double* Tn = (n & 1) ? Tb : Ta;
     double* Tio = (n & 1) ? Ta : Tb;
-    GBE_TRY(gbe_launch_cheb_step(g, w.st, BX, Tn, Tio, BD, w.st->t1, n + 1, w.partials, s));
+    // the LAST term feeds nothing but D, and D is read at its core columns only: core tiles only (as the last SP2 iteration)
+    GBE_TRY(gbe_launch_cheb_step(g, w.st, BX, Tn, Tio, BD, w.st->t1, n + 1, w.partials, s, n == order - 1));
   }
   GBE_TRY(gbe_launch_core_trace(g, BD, w.st, s));
   GBE_TRY(gbe_launch_scatter(g, w.st, BD, BD, D_val, s));

@@ -301,7 +301,7 @@ int gbe_launch_cheb_coef(gbe_state* st, double mu, double beta, int order, cudaS
 int gbe_launch_cheb_init(const gbe_graph* g, const gbe_state* st, double* BX, double* B0, double* B1, double* BD,
                          cudaStream_t s);
 int gbe_launch_cheb_step(const gbe_graph* g, gbe_state* st, const double* Xt, const double* Tn, double* Tio, double* Dacc,
-                         const double* coef, int iter, double* partials, cudaStream_t s);
+                         const double* coef, int iter, double* partials, cudaStream_t s, bool last = false);
 int gbe_launch_core_trace(const gbe_graph* g, const double* BD, gbe_state* st, cudaStream_t s);
 // observables (gbe_observe.cu)
 int gbe_launch_expectation(const gbe_graph* g, const double* D_val, const gbe_csr_view& A, double* row_sum, double* out,

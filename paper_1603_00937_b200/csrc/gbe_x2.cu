@@ -140,6 +140,10 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   double* __restrict__ Y = Xout + doff;
   const double* __restrict__ XB = OP == 1 ? Xb + doff : X;  // rows of the B operand
   double* __restrict__ DA = OP == 1 ? Dacc + doff : nullptr;
+  // OP 1: the sum D is read again only at its core columns (scatter, occupation; Eq.(6)), and with the mirrored
+  // store those all lie in the tiles with a core row - the ones that carry a trace partial (pidx >= 0).  The other tiles
+  // (four fifths on the water box) skip the read-modify-write of D; there D keeps c_0 T_0 + c_1 T_1 and is never read.
+  const bool acc_d = OP == 1 && it0.x >= 0;
   const bool diag = (ti == tj);
   const bool share = diag && OP == 0;  // X X^T on a diagonal tile: the B panel is the A panel
   const int row0 = ti * X2_BT, col0 = tj * X2_BT;
@@ -288,7 +292,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
           if (c + 1 >= m) v1 = 0.0;
         }
         *reinterpret_cast<double2*>(yr + j * 8) = make_double2(v0, v1);
-        if (OP == 1) {  // D += c_{n+1} T_{n+1}
+        if (OP == 1 && acc_d) {  // D += c_{n+1} T_{n+1}
           double2 d = *reinterpret_cast<const double2*>(dr + j * 8);
           d.x = fma(cn, v0, d.x);
           d.y = fma(cn, v1, d.y);
@@ -302,12 +306,12 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
         if (FULL || (mirror & (1u << (i * 8 + j)))) {
           if (!EDGE || c < m) {
             *ym0 = v0;
-            if (OP == 1) *dm0 = fma(cn, v0, *dm0);
+            if (OP == 1 && acc_d) *dm0 = fma(cn, v0, *dm0);
             if (TRACE && c < nc) s2 += v0 * v0;
           }
           if (!EDGE || c + 1 < m) {
             *ym1 = v1;
-            if (OP == 1) *dm1 = fma(cn, v1, *dm1);
+            if (OP == 1 && acc_d) *dm1 = fma(cn, v1, *dm1);
             if (TRACE && c + 1 < nc) s2 += v1 * v1;
           }
         }
@@ -766,7 +770,9 @@ int gbe_launch_x2_items(const gbe_graph* g, gbe_state* st, const double* Xin, do
 }
 
 int gbe_launch_cheb_step(const gbe_graph* g, gbe_state* st, const double* Xt, const double* Tn, double* Tio, double* Dacc,
-                         const double* coef, int iter, double* partials, cudaStream_t s) {
+                         const double* coef, int iter, double* partials, cudaStream_t s, bool last) {
   if (g->n_items == 0) return GBE_OK;
-  return launch_x2<4, 1, false>(g, st, Xt, Tio, partials, iter, Tn, Dacc, coef, g->items, g->n_items, s, GBE_PDL_NONE);
+  // last: T_M feeds D only, and D is read at its core columns only - the tiles with a core row suffice
+  return launch_x2<4, 1, false>(g, st, Xt, Tio, partials, iter, Tn, Dacc, coef, last ? g->items_last : g->items,
+                                last ? g->n_items_last : g->n_items, s, GBE_PDL_NONE);
 }
