@@ -734,6 +734,76 @@ def run_fermi(args) -> None:
                       "tflops_alg": info["sp2_flops_per_iter"] * (order - 1) / (t * 1e-3) * 1e-12}), flush=True)
 
 
+def run_md(args) -> None:
+    """The paper's use of the method, one quantum-MD step at a time, on the bench workload: S(t) from Eq.(8)
+    with D(t - dt) and the moved Hamiltonian H(t) (gbe_update_graph), the density with the SP2 sequence of the previous
+    step (gbe_density_preset, no trace reduction between the products), the band energy Tr[D H] (gbe_expectation).
+    H(t) = the seeded box with every element moved by up to 0.1 % per step, kept symmetric (a stand-in for moving atoms:
+    same pattern, changing values).  Step 0 is an ordinary build + trace-driven density.  One JSON line per step."""
+    import torch
+    from paper_1603_00937_b200 import build as gbe_build
+    gbe_build.build()
+    import paper_1603_00937_b200 as gbe
+    import gbe_inputs as gi
+    # the gapped variant of the water model (oxygens >= 2.4 A apart, 3 electrons per molecule, reading A-15): D decays
+    # exponentially there, as in the paper's systems; on the gapless default box |D_ij| >= tau reaches across the box and
+    # Eq.(8)'s paths of length two make every community the whole system
+    n_mol = WORKLOADS[args.workload][0]
+    s = gi.water_box(n_mol, n_mol // 8, seed=0, min_oo=2.4, occ_per_mol=3.0) if n_mol else make_system(args.workload, seed=0)
+    tau_d = args.md_tau
+    Hs = s.H.to_scipy().tocsr()
+    part_t = None if s.meta.get("kind") == "water" else torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
+
+    def moved(step):
+        m = Hs.copy()
+        m.data = m.data * (1.0 + 1e-3 * np.cos(np.arange(m.nnz) * 0.37 + step))
+        return gbe.DeviceCSR.from_host(gi.CSR.from_scipy((m + m.T) * 0.5))
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    Hd = moved(0)
+    g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
+    D, log = gbe.gbe_density(Hd, g, s.n_occ, s.iters, -1.0)
+    seq = log.branch
+    for step in range(1, args.steps + 1):
+        Hd = moved(step)
+        torch.cuda.synchronize()
+        e = [ev() for _ in range(4)]
+        e[0].record()
+        g1 = gbe.gbe_update_graph(g, D, Hd, tau_d, part_t, s.n_part)
+        e[1].record()
+        info = g1.info
+        if info["workspace_bytes"] > 100e9:
+            print(json.dumps({"md_step": step, "error": "Eq.(8) graph too dense for this tau", "tau_graph": tau_d,
+                              "m_mean": info["sum_m"] / info["n_part"], "m_max": info["max_m"],
+                              "workspace_gb": info["workspace_bytes"] * 1e-9}), flush=True)
+            return
+        ws = g1.new_workspace()
+        D1 = torch.empty(info["nnz_D"], dtype=torch.float64, device="cuda")
+        torch.cuda.synchronize()
+        e[1].record()
+        gbe.gbe_density_preset(Hd, g1, seq, trace_every_iteration=False, workspace=ws, D_val=D1, want_log=False)
+        e[2].record()
+        eband = gbe.gbe_expectation(g1, D1, Hd)
+        e[3].record()
+        torch.cuda.synchronize()
+        # the sequence for the next step: the one a trace-driven run of THIS step chooses (untimed; an MD code would
+        # keep the sequence while the gap estimate holds, P:L90)
+        _, lg = gbe.gbe_density(Hd, g1, s.n_occ, s.iters, -1.0, workspace=ws, D_val=torch.empty_like(D1))
+        same = bool(np.array_equal(lg.branch, seq))
+        seq = lg.branch
+        print(json.dumps({"md_step": step, "workload": args.workload, "n": s.n, "n_part": s.n_part, "tau_graph": tau_d,
+                          "nnz_S": info["nnz_S"], "m_mean": info["sum_m"] / info["n_part"], "m_max": info["max_m"],
+                          "nnz_D": info["nnz_D"], "sp2_path": info["sp2_path_chosen"],
+                          "graph_update_ms": e[0].elapsed_time(e[1]), "density_preset_ms": e[1].elapsed_time(e[2]),
+                          "expectation_ms": e[2].elapsed_time(e[3]),
+                          "step_ms": e[0].elapsed_time(e[1]) + e[1].elapsed_time(e[3]),
+                          "orbitals_per_s": s.n / ((e[0].elapsed_time(e[1]) + e[1].elapsed_time(e[3])) * 1e-3),
+                          "band_energy": eband, "sequence_unchanged": same}), flush=True)
+        g.free()
+        g, D = g1, D1
+    g.free()
+
+
 def run_trace_build(args) -> None:
     """Timeline of gbe_build_graph (steps 0-2) on the bench workload: every kernel, copy and memset with its start time
     (CUPTI through torch.profiler - a library used for this report only), so that device IDLE time shows: the span of one
@@ -916,6 +986,8 @@ def main() -> None:
     ap.add_argument("--sweep-taus", default="", help="comma-separated thresholds of the sweep (default: the five of configs[4])")
     ap.add_argument("--sp2-path", type=int, default=0, help="sweep: force the SP2 kernels (1 tiled, 2 resident, 3 packed; 0 = the library's choice)")
     ap.add_argument("--waves", action="store_true", help="gbe_density_preset on the whole batch against the same call in a bounded workspace")
+    ap.add_argument("--md", action="store_true", help="MD-like loop: Eq.(8) graph update + pre-set SP2 sequence + band energy per step")
+    ap.add_argument("--md-tau", type=float, default=1e-4, help="--md: threshold on D(t - dt) in Eq.(8)")
     ap.add_argument("--trace-build", action="store_true", help="timeline of one gbe_build_graph: device busy / idle time, gaps")
     ap.add_argument("--waves-gb", type=float, default=8.0, help="--waves: size of the bounded workspace in GB")
     ap.add_argument("--clock-sampler", default="nvml", choices=["nvml", "nvidia-smi", "none"],
@@ -933,6 +1005,8 @@ def main() -> None:
         run_waves(args)
     elif args.trace_build:
         run_trace_build(args)
+    elif args.md:
+        run_md(args)
     elif args.fermi:
         run_fermi(args)
     elif args.impl == "reference":
