@@ -734,6 +734,119 @@ def run_fermi(args) -> None:
                       "tflops_alg": info["sp2_flops_per_iter"] * (order - 1) / (t * 1e-3) * 1e-12}), flush=True)
 
 
+def run_timeline(args) -> None:
+    """Timeline INSIDE the two hot kernels from %globaltimer stamps (profiles/r02_small_m_ncu.md, r02_x2_timeline.md).
+    Runs on the instrumented copy of the library (python -m paper_1603_00937_b200.build --stamps -> libgbe_stamps.so; the
+    stamps are compiled out of libgbe.so and add ~10 % to a packed launch), so nothing printed here is a bench value.
+      packed: the 1,024-community point of the sweep (water box, tau = 1e-3): per bin of k_sp2_packed, means over the bins
+              of one launch in the middle of the loop, split by wave;
+      x2:     the bench workload: per CTA of k_x2_tma for two consecutive launches - tile durations, how many CTAs run
+              near the end of a launch (the tail), and the hand-over to the next launch."""
+    import ctypes as C
+    import torch
+    import gbe_inputs as gi
+    from paper_1603_00937_b200 import build as gbe_build
+    import paper_1603_00937_b200.binding as binding
+    binding.LIB_PATH = gbe_build.build(stamps=True)
+    import paper_1603_00937_b200 as gbe
+    l = binding.lib()
+    if args.timeline == "packed":
+        s = gi.water_box(4096, 1024, seed=0, tau=1e-3)
+    else:
+        s = make_system(args.workload, seed=0)
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    part_t = None if s.meta.get("kind") == "water" else torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
+    g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
+    info = g.info
+    ws = g.new_workspace()
+    D = torch.empty(info["nnz_D"], dtype=torch.float64, device="cuda")
+    for _ in range(3):  # the stamps of the last call stay
+        gbe.gbe_density(Hd, g, s.n_occ, 40, -1.0, workspace=ws, D_val=D, want_log=False)
+    torch.cuda.synchronize()
+    us = 1e-3
+    out = {"timeline": args.timeline, "n": s.n, "n_part": s.n_part, "sp2_path": info["sp2_path_chosen"], "unit": "us"}
+    if args.timeline == "packed":
+        if info["sp2_path_chosen"] != 3:
+            raise SystemExit("--timeline packed: the library did not choose the packed kernel for this system")
+        I, B, W = C.c_int(), C.c_int(), C.c_int()
+        l.gbe_stamps_packed_shape(C.byref(I), C.byref(B), C.byref(W))
+        I, B, W = I.value, B.value, W.value
+        buf = np.zeros(I * B * W, dtype=np.uint64)
+        l.gbe_stamps_packed.argtypes = [C.c_void_p, C.c_size_t]
+        rc = l.gbe_stamps_packed(buf.ctypes.data, buf.nbytes)
+        if rc != 0:
+            raise SystemExit(f"gbe_stamps_packed: {rc}")
+        nb = info["n_bins"]
+        st = buf.reshape(I, B, W)[:, :nb, :].astype(np.float64)
+        out["bins"] = nb
+        out["launches"] = []
+        for it in (10, 20, 30):
+            a = st[it]
+            prev_end = st[it - 1][:, 5].max()
+            row = {"iter": it, "launch_to_launch": round((a[:, 5].max() - prev_end) * us, 2),
+                   "first_entry_rel_prev_end": round((a[:, 0].min() - prev_end) * us, 2),
+                   "release_rel_prev_end": [round((a[:, 2].min() - prev_end) * us, 2), round((a[:, 2].max() - prev_end) * us, 2)],
+                   "waves": []}
+            order = np.argsort(a[:, 0])
+            for idx in (order[:148], order[148:]):
+                if len(idx) == 0:
+                    continue
+                e = a[idx]
+                done = e[:, 8:40].max(axis=1)
+                land = (e[:, 40:56] - e[:, 2:3]) * us
+                land[e[:, 40:56] == 0] = np.nan
+                row["waves"].append({
+                    "bins": int(len(idx)),
+                    "setup": round((e[:, 1] - e[:, 0]).mean() * us, 2),
+                    "wait": round((e[:, 2] - e[:, 1]).mean() * us, 2),
+                    "copies_issued": round((e[:, 3] - e[:, 2]).mean() * us, 2),
+                    "step5": round((e[:, 7] - e[:, 3]).mean() * us, 2),
+                    "slot0_landed_after_release": round(float(np.nanmean(land[:, 0])), 2),
+                    "last_slot_landed_after_release": round(float(np.nanmean(np.nanmax(land, axis=1))), 2),
+                    "first_unit_after_step5": round((e[:, 4] - e[:, 7]).mean() * us, 2),
+                    "units": [round((done - e[:, 4]).mean() * us, 2), round((done - e[:, 4]).max() * us, 2)],
+                    "pair_published_after_units": round((e[:, 5] - done).mean() * us, 2),
+                    "bin_total": [round((e[:, 5] - e[:, 0]).mean() * us, 2), round((e[:, 5] - e[:, 0]).max() * us, 2)],
+                })
+            out["launches"].append(row)
+    else:
+        I0, I, B, W = C.c_int(), C.c_int(), C.c_int(), C.c_int()
+        l.gbe_stamps_x2_shape(C.byref(I0), C.byref(I), C.byref(B), C.byref(W))
+        I0, I, B, W = I0.value, I.value, B.value, W.value
+        buf = np.zeros(I * B * W, dtype=np.uint64)
+        l.gbe_stamps_x2.argtypes = [C.c_void_p, C.c_size_t]
+        rc = l.gbe_stamps_x2(buf.ctypes.data, buf.nbytes)
+        if rc != 0:
+            raise SystemExit(f"gbe_stamps_x2: {rc}")
+        nt = info["n_tiles"]
+        if nt > B:
+            raise SystemExit(f"--timeline x2: {nt} tiles, the stamp array holds {B}")
+        st = buf.reshape(I, B, W)[:, :nt, :].astype(np.float64)
+        if not st[:, :, 0].all():
+            raise SystemExit("--timeline x2: k_x2_tma did not run these launches (not the TMA kernel on this system?)")
+        out["tiles"] = nt
+        out["launches"] = []
+        slots = 4 * torch.cuda.get_device_properties(0).multi_processor_count
+        for k in range(I):
+            a = st[k]
+            t0, t_end = a[:, 0].min(), a[:, 2].max()
+            dur, ml, ep = a[:, 2] - a[:, 0], a[:, 1] - a[:, 0], a[:, 2] - a[:, 1]
+            sm = a[:, 3].astype(int)
+            last_end = np.array([a[sm == j, 2].max() for j in np.unique(sm)])
+            out["launches"].append({
+                "iter": I0 + k, "span": round((t_end - t0) * us, 1),
+                "tile_mean": round(dur.mean() * us, 2), "main_loop_mean": round(ml.mean() * us, 2), "epilogue_mean": round(ep.mean() * us, 2),
+                "sum_tile_time_over_slots": round(dur.sum() / slots * us, 1), "slots": slots,
+                "sm_idle_before_end_mean": round((t_end - last_end).mean() * us, 1), "sm_idle_before_end_max": round((t_end - last_end).max() * us, 1),
+                "running_ctas_before_end": {str(b): int(((a[:, 0] <= t_end - b * 1e3) & (a[:, 2] > t_end - b * 1e3)).sum())
+                                            for b in (100, 60, 40, 20, 10, 5)},
+            })
+        if I >= 2:
+            out["handover"] = {"end_to_first_cta_of_next": round((st[1][:, 0].min() - st[0][:, 2].max()) * us, 2),
+                               "end_to_first_epilogue_of_next": round((st[1][:, 1].min() - st[0][:, 2].max()) * us, 1)}
+    print(json.dumps(out), flush=True)
+
+
 def run_md(args) -> None:
     """The paper's use of the method, one quantum-MD step at a time, on the bench workload: S(t) from Eq.(8)
     with D(t - dt) and the moved Hamiltonian H(t) (gbe_update_graph), the density with the SP2 sequence of the previous
@@ -988,6 +1101,8 @@ def main() -> None:
     ap.add_argument("--waves", action="store_true", help="gbe_density_preset on the whole batch against the same call in a bounded workspace")
     ap.add_argument("--md", action="store_true", help="MD-like loop: Eq.(8) graph update + pre-set SP2 sequence + band energy per step")
     ap.add_argument("--md-tau", type=float, default=1e-4, help="--md: threshold on D(t - dt) in Eq.(8)")
+    ap.add_argument("--timeline", default="", choices=["", "packed", "x2"],
+                    help="in-kernel timeline of k_sp2_packed / k_x2_tma from %%globaltimer stamps (instrumented library copy)")
     ap.add_argument("--trace-build", action="store_true", help="timeline of one gbe_build_graph: device busy / idle time, gaps")
     ap.add_argument("--waves-gb", type=float, default=8.0, help="--waves: size of the bounded workspace in GB")
     ap.add_argument("--clock-sampler", default="nvml", choices=["nvml", "nvidia-smi", "none"],
@@ -1005,6 +1120,8 @@ def main() -> None:
         run_waves(args)
     elif args.trace_build:
         run_trace_build(args)
+    elif args.timeline:
+        run_timeline(args)
     elif args.md:
         run_md(args)
     elif args.fermi:

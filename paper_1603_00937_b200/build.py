@@ -1,6 +1,9 @@
 """Builds csrc/*.cu into paper_1603_00937_b200/libgbe.so for sm_100a (in-tree; the .so is git-ignored).
 
     python -m paper_1603_00937_b200.build [--force] [--verbose]
+    python -m paper_1603_00937_b200.build --stamps     the instrumented copy libgbe_stamps.so (-DGBE_STAMPS: %globaltimer
+                                                       stamps in k_sp2_packed and k_x2_tma; read by bench.py --timeline).
+                                                       libgbe.so holds none of it.
 """
 from __future__ import annotations
 
@@ -12,6 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libgbe.so")
+LIB_STAMPS = os.path.join(HERE, "libgbe_stamps.so")
 SOURCES = sorted(glob.glob(os.path.join(HERE, "csrc", "*.cu")))
 HEADERS = sorted(glob.glob(os.path.join(HERE, "csrc", "*.cuh"))) + [os.path.join(ROOT, "include", "gbe.h")]
 
@@ -29,16 +33,18 @@ def _stale(obj: str, src: str) -> bool:
     return any(os.path.getmtime(f) > t for f in [src] + HEADERS + [os.path.abspath(__file__)])
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, stamps: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "nvcc")
-    objdir = os.path.join(HERE, "build")
+    objdir = os.path.join(HERE, "build", "stamps") if stamps else os.path.join(HERE, "build")
+    lib = LIB_STAMPS if stamps else LIB
+    extra = ["-DGBE_STAMPS"] if stamps else []
     os.makedirs(objdir, exist_ok=True)
     objs, procs = [], []
     for src in SOURCES:
         obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
         objs.append(obj)
         if force or _stale(obj, src):
-            cmd = [nvcc, *NVCC_FLAGS, "-I", os.path.join(ROOT, "include"), "-I", os.path.join(HERE, "csrc"), "-c", src, "-o", obj]
+            cmd = [nvcc, *NVCC_FLAGS, *extra, "-I", os.path.join(ROOT, "include"), "-I", os.path.join(HERE, "csrc"), "-c", src, "-o", obj]
             if verbose:
                 print(" ".join(cmd))
             procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
@@ -50,13 +56,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
         failed |= p.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed")
-    if procs or not os.path.exists(LIB) or force:
-        cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "static", "-o", LIB, *objs]
+    if procs or not os.path.exists(lib) or force:
+        cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "static", "-o", lib, *objs]
         if verbose:
             print(" ".join(cmd))
         subprocess.check_call(cmd)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, stamps="--stamps" in sys.argv))

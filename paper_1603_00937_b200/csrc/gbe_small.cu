@@ -55,6 +55,36 @@
 
 #include "gbe_internal.cuh"
 
+// Optional instrumentation (python -m paper_1603_00937_b200.build --stamps -> libgbe_stamps.so; bench.py --timeline packed):
+// %globaltimer stamps per bin at a few points of the kernel.  Compiled out of libgbe.so.
+#ifdef GBE_STAMPS
+constexpr int PK_ST_ITERS = 40, PK_ST_BINS = 1024, PK_ST_W = 64;
+static __device__ unsigned long long g_pk_stamps[(size_t)PK_ST_ITERS * PK_ST_BINS * PK_ST_W];
+__device__ __forceinline__ unsigned long long pk_gtime() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t;
+}
+// slot k of bin blockIdx.x in launch `iter`: 0 CTA start, 1 set-up done, 2 dependency resolved, 3 copies issued,
+// 4 first unit of thread 0 starts, 5 pair published, 7 step 5 done, 8 + w warp w has computed and stored its units,
+// 40 + s the rows of community s have landed
+#define PK_STAMP(k)                                                                                   \
+  do {                                                                                                \
+    if (iter < PK_ST_ITERS && blockIdx.x < PK_ST_BINS)                                                \
+      g_pk_stamps[((size_t)iter * PK_ST_BINS + blockIdx.x) * PK_ST_W + (k)] = pk_gtime();             \
+  } while (0)
+extern "C" int gbe_stamps_packed(unsigned long long* host, size_t bytes) {
+  if (bytes < sizeof(g_pk_stamps)) return -1;
+  return (int)cudaMemcpyFromSymbol(host, g_pk_stamps, sizeof(g_pk_stamps));
+}
+extern "C" int gbe_stamps_packed_shape(int* iters, int* bins, int* width) {
+  *iters = PK_ST_ITERS; *bins = PK_ST_BINS; *width = PK_ST_W;
+  return 0;
+}
+#else
+#define PK_STAMP(k) do { } while (0)
+#endif
+
 namespace {
 
 constexpr int PK_WARPS = 32;             // 1,024 threads, 64 registers each, one CTA per SM
@@ -193,6 +223,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
   __shared__ __align__(8) unsigned long long load_bar[GBE_PK_MAX_SLOTS];  // one per community of the bin
 
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5, g = lane >> 2, q = lane & 3;
+  if (t == 0) PK_STAMP(0);
   // the bin's description (one coalesced read), this warp's unit codes (dealt on the host, longest first, to the least
   // loaded warp; lane j holds the j-th one; fixed stride per bin, so the address does not wait for the description):
   // independent loads, all in flight
@@ -222,8 +253,10 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
   // has completed and its X_{n+1}, partials and state are visible.  Nothing above reads or writes what a launch produces
   // (the description, the unit codes and the row table belong to the graph).  Without the attribute both instructions
   // are no-ops.
+  if (t == 0) PK_STAMP(1);
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (t == 0) PK_STAMP(2);
   // the state and (lazy step 5) this thread's pair(s) of the previous launch: all requested at once, used after the
   // copies are issued
   int stop = st->stop;
@@ -262,6 +295,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
       }
     }
   }
+  if (t == 0) PK_STAMP(3);
   if (lazy_n > 0) {
     // LAZY step 5: t1, t2 of X_iter from the pairs of the previous launch
     if (wid * 32 < lazy_n) {  // (a warp without pairs holds zeros)
@@ -282,6 +316,14 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
       return;
     }
   }
+  if (t == 0) PK_STAMP(7);
+#ifdef GBE_STAMPS
+  if (wid == PK_WARPS - 1)  // (instrumented build only: the last warp watches the communities land before it starts)
+    for (int s = 0; s < n_slots; ++s) {
+      mbar_wait(mbar0 + 8u * s, 0);
+      if (lane == 0) PK_STAMP(40 + s);
+    }
+#endif
   // (no wait here: a unit waits for the rows of ITS community only - the largest community of a bin sits in slot 0, its
   //  copies are issued first and its units are the first of every warp's list, so the products start while the rest lands)
 
@@ -299,6 +341,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
     // the last iteration needs the core rows and (through the mirror) the core columns only (Eq.(6))
     if (code == PK_NONE || (last && bi * 8 >= nc)) continue;
     mbar_wait(mbar0 + 8u * s, 0);
+    if (round == 0 && t == 0) PK_STAMP(4);
     const double* x0 = xs + me.slot[s].soff;
     const double* pa = x0 + (size_t)(bi * 8 + g) * stride + q;
     const double* pb = x0 + (size_t)(bj * 8 + g) * stride + q;
@@ -324,6 +367,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
   }
 
   // ---- core-row traces of X_{n+1}: per warp in the (fixed) order of its unit list, then over the warps: one pair per bin
+  if (lane == 0) PK_STAMP(8 + wid);
   s1 = warp_sum(s1);
   s2 = warp_sum(s2);
   if (lane == 0) { red[wid] = s1; red[PK_WARPS + wid] = s2; }
@@ -342,6 +386,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1)
         lastflag = atomicAdd(&st->ticket, 1u) == gridDim.x - 1;
       }
       is_last = lastflag;
+      PK_STAMP(5);
     }
   }
   if (fused != 1) return;

@@ -37,6 +37,36 @@
 
 #include "gbe_internal.cuh"
 
+// Optional instrumentation (python -m paper_1603_00937_b200.build --stamps -> libgbe_stamps.so; bench.py --timeline x2):
+// %globaltimer per CTA of k_x2_tma at its start, after its main loop and after its epilogue, plus the SM it ran on, for
+// the launches of two consecutive iterations.  Compiled out of libgbe.so.
+#ifdef GBE_STAMPS
+constexpr int X2_ST_IT0 = 10, X2_ST_ITERS = 2, X2_ST_CTAS = 32768, X2_ST_W = 4;
+static __device__ unsigned long long g_x2_stamps[(size_t)X2_ST_ITERS * X2_ST_CTAS * X2_ST_W];
+#define X2_STAMP(k)                                                                                             \
+  do {                                                                                                          \
+    if (threadIdx.x == 0 && iter >= X2_ST_IT0 && iter < X2_ST_IT0 + X2_ST_ITERS && blockIdx.x < X2_ST_CTAS) {   \
+      unsigned long long now_;                                                                                  \
+      unsigned smid_;                                                                                           \
+      asm volatile("mov.u64 %0, %globaltimer;" : "=l"(now_));                                                   \
+      asm volatile("mov.u32 %0, %smid;" : "=r"(smid_));                                                         \
+      unsigned long long* e_ = g_x2_stamps + ((size_t)(iter - X2_ST_IT0) * X2_ST_CTAS + blockIdx.x) * X2_ST_W;  \
+      e_[k] = now_;                                                                                             \
+      e_[3] = smid_;                                                                                            \
+    }                                                                                                           \
+  } while (0)
+extern "C" int gbe_stamps_x2(unsigned long long* host, size_t bytes) {
+  if (bytes < sizeof(g_x2_stamps)) return -1;
+  return (int)cudaMemcpyFromSymbol(host, g_x2_stamps, sizeof(g_x2_stamps));
+}
+extern "C" int gbe_stamps_x2_shape(int* iter0, int* iters, int* ctas, int* width) {
+  *iter0 = X2_ST_IT0; *iters = X2_ST_ITERS; *ctas = X2_ST_CTAS; *width = X2_ST_W;
+  return 0;
+}
+#else
+#define X2_STAMP(k) do { } while (0)
+#endif
+
 namespace {
 
 
@@ -430,6 +460,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   __shared__ double red[8];
   __shared__ __align__(8) unsigned long long bars[2 * XT_NST];  // full[0..2], empty[0..2]
 
+  X2_STAMP(0);
   // programmatic dependent launch, hyb and state loads: as in k_x2
   gbe_griddep_launch();
   if (HYB)
@@ -556,6 +587,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
     }
   }
 
+  X2_STAMP(1);
   // epilogue: as k_x2 (OP 0)
   double s1 = 0.0, s2 = 0.0;
   auto epilogue = [&](auto edge_c, auto trace_c, auto full_c) {
@@ -619,6 +651,7 @@ __global__ void __launch_bounds__(X2_THREADS, MINB)
   } else {
     epilogue(std::false_type{}, std::false_type{}, std::false_type{});
   }
+  X2_STAMP(2);
   const int pidx = it0.x;
   if (!HYB && pidx < 0) return;
   if (pidx >= 0) {

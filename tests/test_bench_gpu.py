@@ -33,3 +33,30 @@ def test_bench_line_keeps_the_contract():
     assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and 0.8 <= r["frac"] <= 1.02
     # traffic comes from the tracked ncu record and is null when gbe_x2.cu changed since it was captured
     assert r["traffic"] is not None and 0.9 <= r["traffic"] / r["algorithmic_bytes_per_launch"] <= 1.1, r.get("traffic_note")
+
+
+@pytest.mark.parametrize("which", ["packed", "x2"])
+def test_timeline_runs_on_the_instrumented_copy(which):
+    """bench.py --timeline (profiles/r02_small_m_ncu.md, r02_x2_timeline.md): builds libgbe_stamps.so (-DGBE_STAMPS), loads
+    it instead of libgbe.so and prints ordered, plausible stamps; libgbe.so itself exports no stamp reader."""
+    import ctypes
+    from paper_1603_00937_b200 import binding
+    assert not hasattr(ctypes.CDLL(binding.LIB_PATH), "gbe_stamps_x2")
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--timeline", which], cwd=ROOT, capture_output=True,
+                       text=True, timeout=900)
+    assert p.returncode == 0, p.stderr[-2000:]
+    l = json.loads([x for x in p.stdout.strip().splitlines() if x.startswith("{")][0])
+    assert l["timeline"] == which and l["unit"] == "us"
+    if which == "packed":
+        assert l["sp2_path"] == 3 and l["bins"] >= 148
+        for launch in l["launches"]:
+            assert 5 < launch["launch_to_launch"] < 200
+            for w in launch["waves"]:
+                assert 0 < w["setup"] < 20 and 0 < w["copies_issued"] < 20 and 0 < w["units"][0] <= w["units"][1] < 100
+                assert 0 < w["slot0_landed_after_release"] <= w["last_slot_landed_after_release"] < 50
+    else:
+        assert l["tiles"] > 10000 and len(l["launches"]) == 2
+        for launch in l["launches"]:
+            assert 500 < launch["span"] < 10000 and 0 < launch["epilogue_mean"] < launch["main_loop_mean"] < launch["tile_mean"]
+            assert 0.8 < launch["sum_tile_time_over_slots"] / launch["span"] <= 1.0
+        assert -50 < l["handover"]["end_to_first_cta_of_next"] < 100
