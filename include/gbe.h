@@ -191,6 +191,14 @@ int gbe_graph_set_sp2_path(gbe_graph* g, int32_t path);
  * The dense blocks of the two are bit-identical; the traces of X_0 are summed in a different order (agree to rounding). */
 int gbe_graph_set_gather_path(gbe_graph* g, int32_t path);
 
+/* Which kernel moves the core columns into D (step 6).  Two variants copy the same runs:
+ *   register  a warp moves 8 runs per iteration through registers (any core sizes, any partition vector);
+ *   bulk      the copy engine moves the runs global -> shared -> global (cp.async.bulk), 32 per warp in flight; needs
+ *             index-range cores of even size and a 16-byte aligned D_val (every run is then a whole number of 16-byte
+ *             pieces on both sides).
+ * path = 0 (default): bulk where its conditions hold, else register; 1: register.  D is bit-identical. */
+int gbe_graph_set_scatter_path(gbe_graph* g, int32_t path);
+
 /* Steps 0 and 3-6: D = P_tau(H) on the pattern fixed by the graph (Eq.(6)).
  *   H         device CSR; values AND pattern may differ from the H the graph was built from (MD use):
  *             H values are looked up at gather time, entries outside a subgraph are simply not gathered.

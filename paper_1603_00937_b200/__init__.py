@@ -28,6 +28,7 @@ from .binding import (  # noqa: F401
     gbe_launch_count,
     gbe_graph_set_sp2_path,
     gbe_graph_set_gather_path,
+    gbe_graph_set_scatter_path,
     gbe_set_build_scratch_limit,
     gbe_set_packed_max_m,
     gbe_set_dependent_launch,

@@ -20,7 +20,7 @@ EXPORTS = [
     "gbe_build_graph", "gbe_graph_get_info", "gbe_graph_export", "gbe_density", "gbe_gather", "gbe_sp2",
     "gbe_scatter", "gbe_read_log", "gbe_density_host", "gbe_free_graph", "gbe_strerror", "gbe_last_cuda_error",
     "gbe_version", "gbe_build_graph_host", "gbe_density_timed", "gbe_launch_count", "gbe_density_preset", "gbe_expectation", "gbe_update_graph", "gbe_density_fermi",
-    "gbe_graph_set_sp2_path", "gbe_error_norms", "gbe_graph_set_gather_path", "gbe_set_build_scratch_limit",
+    "gbe_graph_set_sp2_path", "gbe_error_norms", "gbe_graph_set_gather_path", "gbe_graph_set_scatter_path", "gbe_set_build_scratch_limit",
     "gbe_set_packed_max_m", "gbe_expectation_static", "gbe_set_dependent_launch",
 ]
 
@@ -100,6 +100,7 @@ def lib() -> C.CDLL:
         l.gbe_error_norms.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.POINTER(C.c_double)]
         l.gbe_graph_set_sp2_path.argtypes = [C.c_void_p, C.c_int32]
         l.gbe_graph_set_gather_path.argtypes = [C.c_void_p, C.c_int32]
+        l.gbe_graph_set_scatter_path.argtypes = [C.c_void_p, C.c_int32]
         l.gbe_set_build_scratch_limit.restype = C.c_size_t
         l.gbe_set_build_scratch_limit.argtypes = [C.c_size_t]
         l.gbe_expectation_static.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_CsrView), C.c_void_p, C.c_void_p]
@@ -244,6 +245,11 @@ def gbe_graph_set_sp2_path(g: "Graph", path: int) -> None:
     """0 auto, 1 tiled kernels, 2 shared-memory-resident kernel, 3 packed kernel for the small communities (include/gbe.h)."""
     _check(lib().gbe_graph_set_sp2_path(g._h, int(path)))
     g._info = None  # sp2_path_chosen / resident_sp2 change: read again on next use
+
+
+def gbe_graph_set_scatter_path(g: "Graph", path: int) -> None:
+    """0 auto (bulk copies where the graph allows them), 1 the register variant (include/gbe.h)."""
+    _check(lib().gbe_graph_set_scatter_path(g._h, int(path)))
 
 
 def gbe_graph_set_gather_path(g: "Graph", path: int) -> None:

@@ -285,6 +285,12 @@ int gbe_graph_set_gather_path(gbe_graph* g, int32_t path) {
   return GBE_OK;
 }
 
+int gbe_graph_set_scatter_path(gbe_graph* g, int32_t path) {
+  if (!g || path < 0 || path > 1) return GBE_EINVAL;
+  g->scatter_path = path;
+  return GBE_OK;
+}
+
 static int do_sp2(const gbe_graph* g, double n_occ, int32_t iters, double idem_tol, void* workspace,
                   size_t workspace_bytes, void* cuda_stream, Timer* tm, const uint8_t* preset = nullptr,
                   bool trace_each = true) {

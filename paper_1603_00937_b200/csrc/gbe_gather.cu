@@ -6,9 +6,11 @@
 // ld_p = m_p rounded up to 16 doubles (rows are 128-byte aligned), pad columns zero.
 //
 // One CTA handles `gather_rows` consecutive rows of one community.  The global -> local index translation is a
-// pair of bitmaps (core, halo) over the n vertices with popcount-prefix ranks in shared memory: O(1) per
-// stored entry, no search.  Each warp builds one output row in shared memory (zero fill + scattered entries)
-// and streams it out with 128-bit stores, so every output byte is written exactly once, fully coalesced.
+// pair of bitmaps (core, halo) over the n vertices with popcount-prefix ranks in shared memory, one 16-byte entry
+// {core word, halo word, core rank, nc + halo rank} per 32 vertices: one LDS.128 and no branch per stored entry, no
+// search.  Each warp builds one output row in shared memory (zero fill + scattered entries) and hands it to the
+// copy engine as ONE bulk store (cp.async.bulk shared -> global, UBLKCP), so every output byte is written exactly once,
+// in whole lines, and the warp issues no per-element store; the buffer is reused when the engine has read it.
 // The epilogue accumulates the traces of X_0 and X_0^2 over the core rows (t1, t2 of iteration 0):
 // (X^2)_ii = sum_c X_ic^2 for symmetric X.
 // DIRECT variant (large systems: the bitmaps of ~1e5 vertices plus row buffers of ~2,400 doubles leave one CTA per SM):
@@ -20,6 +22,18 @@
 
 namespace {
 
+// bulk store of one finished row, shared -> global, by the copy engine (sizes and addresses are multiples of 16 bytes);
+// the generic-proxy stores that built the row are fenced before the engine (async proxy) reads them
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void bulk_store_row(double* dst, const double* src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst),
+               "r"((uint32_t)__cvta_generic_to_shared(src_smem)), "r"(bytes)
+               : "memory");
+  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+// until the engine has READ the source of every bulk store this thread issued (the buffer may be written again)
+__device__ __forceinline__ void bulk_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+
 template <bool DIRECT>
 __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_per_cta, const int2* __restrict__ gitems,
                                                 const int64_t* __restrict__ H_rp, const int32_t* __restrict__ H_col,
@@ -29,11 +43,8 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
                                                 const int64_t* __restrict__ dense_off, const gbe_state* __restrict__ st,
                                                 double* __restrict__ X, double* __restrict__ partials) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  uint32_t* coreb = reinterpret_cast<uint32_t*>(smem_raw);
-  uint32_t* halob = coreb + W;
-  uint32_t* corerk = halob + W;
-  uint32_t* halork = corerk + W;
-  int* scratch = reinterpret_cast<int*>(halork + W);                      // 2 * 257 ints
+  uint4* tab = reinterpret_cast<uint4*>(smem_raw);                        // W x {core word, halo word, core rank, nc + halo rank}
+  int* scratch = reinterpret_cast<int*>(tab + W);                         // 2 * 257 ints
   double* red = reinterpret_cast<double*>(scratch + 516);                  // 16 doubles (8-byte aligned: 4W*4 + 2064)
   double* rowbuf = red + 16;                                               // nwarps * ldmax doubles
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5, nw = blockDim.x >> 5;
@@ -55,11 +66,11 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   };
 
   // bitmaps of the community's core and halo vertices
-  for (int w = t; w < 2 * W; w += blockDim.x) coreb[w] = 0u;
+  for (int w = t; w < W; w += blockDim.x) tab[w] = make_uint4(0u, 0u, 0u, 0u);
   __syncthreads();
-  for (int r = t; r < m; r += blockDim.x) {
-    const int v = sub_idx[sb + r];
-    atomicOr(r < nc ? &coreb[v >> 5] : &halob[v >> 5], 1u << (v & 31));
+  for (int l = t; l < m; l += blockDim.x) {
+    const int v = sub_idx[sb + l];
+    atomicOr(l < nc ? &tab[v >> 5].x : &tab[v >> 5].y, 1u << (v & 31));
   }
   __syncthreads();
   // ranks: exclusive popcount prefix per word (both bitmaps at once)
@@ -67,27 +78,29 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
     const int nt = blockDim.x, chunk = (W + nt - 1) / nt;
     const int b = min(W, t * chunk), e = min(W, b + chunk);
     int c0 = 0, c1 = 0;
-    for (int w = b; w < e; ++w) { c0 += __popc(coreb[w]); c1 += __popc(halob[w]); }
+    for (int w = b; w < e; ++w) { c0 += __popc(tab[w].x); c1 += __popc(tab[w].y); }
     scratch[t] = c0;
     scratch[258 + t] = c1;
     __syncthreads();
     for (int which = wid; which < 2; which += nw) {  // one warp each scans the per-thread counts of the core and the halo bitmap
       int* sc = scratch + 258 * which;
       int run = 0;
-      for (int k0 = 0; k0 < nt; k0 += 32) {
-        const int v = k0 + lane < nt ? sc[k0 + lane] : 0;
+      for (int i0 = 0; i0 < nt; i0 += 32) {
+        const int v = i0 + lane < nt ? sc[i0 + lane] : 0;
         int tot;
         const int ex = warp_excl_scan_i(v, lane, &tot);
-        if (k0 + lane < nt) sc[k0 + lane] = run + ex;
+        if (i0 + lane < nt) sc[i0 + lane] = run + ex;
         run += tot;
       }
     }
     __syncthreads();
     c0 = scratch[t];
-    c1 = scratch[258 + t];
+    c1 = nc + scratch[258 + t];
     for (int w = b; w < e; ++w) {
-      corerk[w] = c0; c0 += __popc(coreb[w]);
-      halork[w] = c1; c1 += __popc(halob[w]);
+      const uint4 e4 = tab[w];
+      tab[w] = make_uint4(e4.x, e4.y, (uint32_t)c0, (uint32_t)c1);
+      c0 += __popc(e4.x);
+      c1 += __popc(e4.y);
     }
   }
   __syncthreads();
@@ -95,18 +108,22 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   double* buf = DIRECT ? nullptr : rowbuf + (size_t)wid * ldmax;
   double* Xp = X + dense_off[p];
   double s1 = 0.0, s2 = 0.0;
-  const int rend = min(m, r0 + rows_per_cta);
   // The row loop is latency bound (sub_idx -> H row pointers -> H entries are dependent loads), so it is software
   // pipelined: the vertex of the row after next, the row pointers of the next row and the first 128 entries of the
   // next row are in flight while the current row is scattered into shared memory and streamed out.
-  auto fetch = [&](int64_t base, int64_t end, int (&j)[4], double (&v)[4]) {
+  const int rend = min(m, r0 + rows_per_cta);
+  // (entries base + lane + 32 u of a row of cnt entries; cnt <= 0: nothing)
+  auto fetch = [&](int64_t base, int cnt, int (&j)[4], double (&v)[4]) {
+    const int32_t* __restrict__ pc = H_col + base + lane;
+    const double* __restrict__ pv = H_val + base + lane;
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-      const int64_t e = base + lane + 32 * u;
-      j[u] = e < end ? H_col[e] : -1;
-      v[u] = e < end ? H_val[e] : 0.0;
+      const bool ok = lane + 32 * u < cnt;
+      j[u] = ok ? pc[32 * u] : -1;
+      v[u] = ok ? pv[32 * u] : 0.0;
     }
   };
+  const uint32_t nlim = (uint32_t)(n < (int64_t)INT32_MAX ? n : (int64_t)INT32_MAX);  // column indices are int32
   double* out = nullptr;     // DIRECT: the output row being built
   double q = 0.0, dg = 0.0;  // DIRECT: this lane's sum of squares of the row, and the stored diagonal if it placed it
   bool dseen = false;
@@ -114,17 +131,13 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const int col = j[u];
-      if (col < 0 || (int64_t)col >= n) continue;
-      const uint32_t bit = 1u << (col & 31), wj = col >> 5;
-      int c = -1;
-      const uint32_t cw = coreb[wj];
-      if (cw & bit) {
-        c = corerk[wj] + __popc(cw & (bit - 1u));
-      } else {
-        const uint32_t hw = halob[wj];
-        if (hw & bit) c = nc + halork[wj] + __popc(hw & (bit - 1u));
-      }
-      if (c >= 0) {
+      const bool inr = (uint32_t)col < nlim;  // (an empty slot holds -1)
+      const uint4 e4 = tab[inr ? col >> 5 : 0];
+      const uint32_t bit = 1u << (col & 31);
+      const bool isc = (e4.x & bit) != 0u;  // core and halo are disjoint
+      const uint32_t wsel = isc ? e4.x : e4.y;
+      const int c = (int)(isc ? e4.z : e4.w) + __popc(wsel & (bit - 1u));
+      if (inr && (wsel & bit) != 0u) {
         const double x = div_delta((col == k ? eps_max : 0.0) - v[u]);
         if (DIRECT) {
           out[c] = x;
@@ -139,22 +152,27 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   int r = r0 + wid;
   int k0 = r < rend ? sub_idx[sb + r] : 0;
   int k1 = r + nw < rend ? sub_idx[sb + r + nw] : 0;
-  int64_t a0 = 0, b0 = 0, a1 = 0, b1 = 0;
+  int64_t a0 = 0, a1 = 0;  // first entry and length of the current and of the next row of H
+  int n0 = 0, n1 = 0;
   int cj[4], nj[4];
   double cv[4], nv[4];
   if (r < rend) {
     a0 = H_rp[k0];
-    b0 = H_rp[k0 + 1];
-    fetch(a0, b0, cj, cv);
+    n0 = (int)(H_rp[k0 + 1] - a0);
+    fetch(a0, n0, cj, cv);
   }
   for (; r < rend; r += nw) {
     const bool has1 = r + nw < rend;
     const int k2 = r + 2 * nw < rend ? sub_idx[sb + r + 2 * nw] : 0;
     if (has1) {
       a1 = H_rp[k1];
-      b1 = H_rp[k1 + 1];
+      n1 = (int)(H_rp[k1 + 1] - a1);
     }
     double* const zrow = DIRECT ? Xp + (size_t)r * ld : buf;
+    if (!DIRECT) {  // the engine has read the previous row out of the buffer
+      if (lane == 0) bulk_store_wait_read();
+      __syncwarp();
+    }
     for (int c = lane * 2; c < ld; c += 64) *reinterpret_cast<double2*>(zrow + c) = make_double2(0.0, 0.0);
     __syncwarp();  // orders the zero fill before the entries other lanes store into the same row
     if (DIRECT) {
@@ -165,14 +183,14 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
       if (lane == 0) buf[r] = div_delta(eps_max - 0.0);  // a stored diagonal overwrites this below
       __syncwarp();
     }
-    for (int64_t base = a0; base < b0; base += 128) {
-      if (base + 128 < b0) fetch(base + 128, b0, nj, nv);        // rest of a long row
-      else if (has1) fetch(a1, b1, nj, nv);                      // first entries of the next row
+    for (int off = 0; off < n0; off += 128) {
+      if (off + 128 < n0) fetch(a0 + off + 128, n0 - off - 128, nj, nv);  // rest of a long row
+      else if (has1) fetch(a1, n1, nj, nv);                               // first entries of the next row
       place(k0, cj, cv);
 #pragma unroll
       for (int u = 0; u < 4; ++u) { cj[u] = nj[u]; cv[u] = nv[u]; }
     }
-    if (a0 >= b0 && has1) fetch(a1, b1, cj, cv);                 // empty row: nothing was prefetched above
+    if (n0 <= 0 && has1) fetch(a1, n1, cj, cv);                  // empty row: nothing was prefetched above
     if (DIRECT) {
       if (!__any_sync(0xffffffffu, dseen) && lane == 0) {  // H_kk is not stored: it is zero (A-12)
         dg = div_delta(eps_max - 0.0);
@@ -187,20 +205,22 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
     } else {
       __syncwarp();
       double* orow = Xp + (size_t)r * ld;
-      double qq = 0.0;
-      for (int c = lane * 2; c < ld; c += 64) {
-        const double2 v = *reinterpret_cast<const double2*>(buf + c);
-        *reinterpret_cast<double2*>(orow + c) = v;
-        qq += v.x * v.x + v.y * v.y;
-      }
-      if (r < nc) {  // warp-uniform
+      if (r < nc) {  // warp-uniform: a core row, whose diagonal and squares enter t1 and t2 of iteration 0
+        double qq = 0.0;
+        for (int c = lane * 2; c < ld; c += 64) {
+          const double2 v = *reinterpret_cast<const double2*>(buf + c);
+          qq += v.x * v.x + v.y * v.y;
+        }
         s2 += qq;
         if (lane == 0) s1 += buf[r];
       }
+      fence_proxy_async_smem();
       __syncwarp();
+      if (lane == 0) bulk_store_row(orow, buf, (uint32_t)ld * 8u);
     }
-    k0 = k1; k1 = k2; a0 = a1; b0 = b1;
+    k0 = k1; k1 = k2; a0 = a1; n0 = n1;
   }
+  if (!DIRECT && lane == 0) bulk_store_wait_read();  // the buffers live as long as the CTA
   s1 = warp_sum(s1);
   s2 = warp_sum(s2);
   if (lane == 0) { red[wid] = s1; red[8 + wid] = s2; }

@@ -330,6 +330,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
   g->h_dense_off.assign(n_part + 1, 0);
   g->max_m = 0;
   g->max_ncore = 0;
+  g->ncore_all_even = 1;
   g->nnz_D = 0;
   g->flops_per_iter = 0;
   g->sym_flops_per_iter = 0;
@@ -340,6 +341,7 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
     g->h_dense_off[p + 1] = g->h_dense_off[p] + m * ld;
     g->max_m = std::max<int32_t>(g->max_m, (int32_t)m);
     g->max_ncore = std::max<int32_t>(g->max_ncore, g->h_ncore[p]);
+    if (g->h_ncore[p] & 1) g->ncore_all_even = 0;
     g->nnz_D += m * g->h_ncore[p];
     g->flops_per_iter += 2.0 * (double)m * (double)m * (double)m;
     g->sym_flops_per_iter += (double)m * (double)m * (double)(m + 1);  // m (m + 1) / 2 entries of 2 m flop each

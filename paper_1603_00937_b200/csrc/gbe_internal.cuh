@@ -134,6 +134,8 @@ struct gbe_graph {
   double flops_last_iter = 0, exec_flops_last_iter = 0;  // the core-tiles-only last iteration
   double sym_flops_per_iter = 0;  // sum m^2 (m + 1): upper triangle incl. diagonal of X_p^2
   int32_t power = 2, contiguous = 1;
+  int32_t ncore_all_even = 0;  // every core size is even (the scatter's bulk variant moves 16-byte pieces)
+  int32_t scatter_path = 0;    // 0 = the library's choice, 1 = register variant (gbe_graph_set_scatter_path)
   // device arrays (owned)
   int64_t* S_row_ptr = nullptr;  // n+1
   int32_t* S_col = nullptr;      // nnz_S

@@ -29,10 +29,11 @@ def gbe():
     return pkg
 
 
-def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None, sp2_path=0, gather_path=0):
+def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None, sp2_path=0, gather_path=0, scatter_path=0):
     """sp2_path: 0 = the library's choice, 1 = tiled kernels, 2 = shared-memory-resident kernel, 3 = packed kernel for
     the communities with m <= 160 + tiled kernel for the others (include/gbe.h);
-    gather_path: 0 = the library's choice, 1 = staged through shared memory, 2 = direct to global memory."""
+    gather_path: 0 = the library's choice, 1 = staged through shared memory, 2 = direct to global memory;
+    scatter_path: 0 = the library's choice (bulk copies where the graph allows), 1 = the register variant."""
     import torch
     Hd = gbe.DeviceCSR.from_host(s.H if H is None else H)
     part_t = None if part is None else torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
@@ -44,6 +45,8 @@ def run_gpu(gbe, s, iters=None, idem_tol=-1.0, power=2, part="given", H=None, sp
             assert g.info["sp2_path_chosen"] == (3 if g.info["n_small"] > 0 else 1)
     if gather_path:
         gbe.gbe_graph_set_gather_path(g, gather_path)
+    if scatter_path:
+        gbe.gbe_graph_set_scatter_path(g, scatter_path)
     D, log = gbe.gbe_density(Hd, g, s.n_occ, s.iters if iters is None else iters, idem_tol)
     torch.cuda.synchronize()
     ex = {k: v.cpu().numpy() for k, v in g.export().items()}
@@ -350,6 +353,27 @@ def test_gather_paths_pack_identical_blocks(gbe, which):
     graph, r = run_oracle(s)
     check_structure(ex, graph, r, g.info)
     check_density(Dg, log, r)
+
+
+@pytest.mark.parametrize("which", ["chain", "water", "water_ragged", "odd_cores", "shuffled", "wide_cores"])
+def test_scatter_paths_write_identical_d(gbe, which):
+    """The bulk-copy and the register scatter kernel (include/gbe.h, gbe_graph_set_scatter_path) move the same runs: D
+    agrees bit for bit after a full expansion and with iters = 0 (D = the core columns of X0: every entry distinct, so a
+    run put in the wrong place or cut short cannot hide).  chain / water: even index-range cores - the bulk kernel runs;
+    water_ragged: 5 communities - a ragged last group of runs; odd_cores (cores of 33) / shuffled:
+    the bulk kernel's conditions fail and the default must fall back; wide_cores: cores of 192 (slots of 1.5 KB)."""
+    s = {"chain": lambda: gi.config(1),
+         "water": lambda: gi.water_box(256, 32, seed=3, tau=1e-5, iters=12),
+         "water_ragged": lambda: gi.water_box(40, 5, seed=4, tau=1e-4, iters=8),
+         "odd_cores": lambda: gi.random_banded(297, half_bw=6, n_part=9, seed=5, tau=1e-4, iters=10),
+         "shuffled": lambda: gi.random_banded(300, half_bw=6, n_part=9, seed=5, tau=1e-4, iters=10, shuffle=True),
+         "wide_cores": lambda: gi.water_box(128, 4, seed=6, tau=1e-4, iters=6)}[which]()
+    for iters in (0, None):
+        g0, _, D0, _ = run_gpu(gbe, s, iters=iters, scatter_path=0)
+        _, _, D1, _ = run_gpu(gbe, s, iters=iters, scatter_path=1)
+        assert D0.size == g0.info["nnz_D"] and np.array_equal(D0, D1)
+    graph, r = run_oracle(s)
+    assert np.abs(D0 - r.D_val).max() <= 1e-10
 
 
 @pytest.mark.parametrize("sp2_path", [1, 2, 3])
