@@ -355,19 +355,21 @@ def test_gather_paths_pack_identical_blocks(gbe, which):
     check_density(Dg, log, r)
 
 
-@pytest.mark.parametrize("which", ["chain", "water", "water_ragged", "odd_cores", "shuffled", "wide_cores"])
+@pytest.mark.parametrize("which", ["chain", "water", "water_ragged", "odd_cores", "shuffled", "wide_cores", "tiny_cores"])
 def test_scatter_paths_write_identical_d(gbe, which):
     """The bulk-copy and the register scatter kernel (include/gbe.h, gbe_graph_set_scatter_path) move the same runs: D
     agrees bit for bit after a full expansion and with iters = 0 (D = the core columns of X0: every entry distinct, so a
     run put in the wrong place or cut short cannot hide).  chain / water: even index-range cores - the bulk kernel runs;
     water_ragged: 5 communities - a ragged last group of runs; odd_cores (cores of 33) / shuffled:
-    the bulk kernel's conditions fail and the default must fall back; wide_cores: cores of 192 (slots of 1.5 KB)."""
+    the bulk kernel's conditions fail and the default must fall back; wide_cores: cores of 192 (slots of 1.5 KB);
+    tiny_cores: cores of 2 (16-byte runs)."""
     s = {"chain": lambda: gi.config(1),
          "water": lambda: gi.water_box(256, 32, seed=3, tau=1e-5, iters=12),
          "water_ragged": lambda: gi.water_box(40, 5, seed=4, tau=1e-4, iters=8),
          "odd_cores": lambda: gi.random_banded(297, half_bw=6, n_part=9, seed=5, tau=1e-4, iters=10),
          "shuffled": lambda: gi.random_banded(300, half_bw=6, n_part=9, seed=5, tau=1e-4, iters=10, shuffle=True),
-         "wide_cores": lambda: gi.water_box(128, 4, seed=6, tau=1e-4, iters=6)}[which]()
+         "wide_cores": lambda: gi.water_box(128, 4, seed=6, tau=1e-4, iters=6),
+         "tiny_cores": lambda: gi.random_banded(64, half_bw=3, n_part=32, seed=7, tau=1e-4, iters=10)}[which]()
     for iters in (0, None):
         g0, _, D0, _ = run_gpu(gbe, s, iters=iters, scatter_path=0)
         _, _, D1, _ = run_gpu(gbe, s, iters=iters, scatter_path=1)
