@@ -109,15 +109,18 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   double* Xp = X + dense_off[p];
   double s1 = 0.0, s2 = 0.0;
   // The row loop is latency bound (sub_idx -> H row pointers -> H entries are dependent loads), so it is software
-  // pipelined: the vertex of the row after next, the row pointers of the next row and the first 128 entries of the
-  // next row are in flight while the current row is scattered into shared memory and streamed out.
+  // pipelined: the vertex of the row after next and the row pointers of the next row are in flight while the current
+  // row is scattered into shared memory; the first 256 entries of the next row (GS slots of 32 per lane: a whole row for
+  // all but the longest) are requested into the SAME registers as soon as the current row's have been placed, and land
+  // while this row is handed to the copy engine and the buffer turns over.
   const int rend = min(m, r0 + rows_per_cta);
   // (entries base + lane + 32 u of a row of cnt entries; cnt <= 0: nothing)
-  auto fetch = [&](int64_t base, int cnt, int (&j)[4], double (&v)[4]) {
+  constexpr int GS = 8;
+  auto fetch = [&](int64_t base, int cnt, int (&j)[GS], double (&v)[GS]) {
     const int32_t* __restrict__ pc = H_col + base + lane;
     const double* __restrict__ pv = H_val + base + lane;
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < GS; ++u) {
       const bool ok = lane + 32 * u < cnt;
       j[u] = ok ? pc[32 * u] : -1;
       v[u] = ok ? pv[32 * u] : 0.0;
@@ -127,9 +130,9 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   double* out = nullptr;     // DIRECT: the output row being built
   double q = 0.0, dg = 0.0;  // DIRECT: this lane's sum of squares of the row, and the stored diagonal if it placed it
   bool dseen = false;
-  auto place = [&](int k, const int (&j)[4], const double (&v)[4]) {
+  auto place = [&](int k, const int (&j)[GS], const double (&v)[GS]) {
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < GS; ++u) {
       const int col = j[u];
       const bool inr = (uint32_t)col < nlim;  // (an empty slot holds -1)
       const uint4 e4 = tab[inr ? col >> 5 : 0];
@@ -154,8 +157,8 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   int k1 = r + nw < rend ? sub_idx[sb + r + nw] : 0;
   int64_t a0 = 0, a1 = 0;  // first entry and length of the current and of the next row of H
   int n0 = 0, n1 = 0;
-  int cj[4], nj[4];
-  double cv[4], nv[4];
+  int cj[GS];
+  double cv[GS];
   if (r < rend) {
     a0 = H_rp[k0];
     n0 = (int)(H_rp[k0 + 1] - a0);
@@ -183,14 +186,11 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
       if (lane == 0) buf[r] = div_delta(eps_max - 0.0);  // a stored diagonal overwrites this below
       __syncwarp();
     }
-    for (int off = 0; off < n0; off += 128) {
-      if (off + 128 < n0) fetch(a0 + off + 128, n0 - off - 128, nj, nv);  // rest of a long row
-      else if (has1) fetch(a1, n1, nj, nv);                               // first entries of the next row
+    for (int off = 0; off < n0; off += 32 * GS) {
       place(k0, cj, cv);
-#pragma unroll
-      for (int u = 0; u < 4; ++u) { cj[u] = nj[u]; cv[u] = nv[u]; }
+      if (off + 32 * GS < n0) fetch(a0 + off + 32 * GS, n0 - off - 32 * GS, cj, cv);  // rest of a very long row
     }
-    if (n0 <= 0 && has1) fetch(a1, n1, cj, cv);                  // empty row: nothing was prefetched above
+    if (has1) fetch(a1, n1, cj, cv);  // the next row's entries: in flight until the buffer has turned over
     if (DIRECT) {
       if (!__any_sync(0xffffffffu, dseen) && lane == 0) {  // H_kk is not stored: it is zero (A-12)
         dg = div_delta(eps_max - 0.0);
