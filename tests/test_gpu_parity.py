@@ -378,25 +378,28 @@ def test_scatter_paths_write_identical_d(gbe, which):
     assert np.abs(D0 - r.D_val).max() <= 1e-10
 
 
-@pytest.mark.parametrize("which", ["chain", "water_ragged", "odd_cores", "shuffled", "tiny_cores", "peptide"])
+@pytest.mark.parametrize("which", ["chain", "water_ragged", "odd_cores", "shuffled", "tiny_cores", "peptide", "water_tma"])
 @pytest.mark.parametrize("d_offset", [0, 1])
 def test_nothing_is_written_outside_workspace_and_d(gbe, which, d_offset):
     """Guard bands around the caller's buffers (the bulk row stores of the gather and the bulk run copies of the scatter
     address whole rows and runs; ragged tails and the last community are where an overrun would show): the workspace and
     D_val are slices of larger buffers filled with a sentinel, which must be intact after gbe_density, and D must equal
     the result in buffers of their own.  d_offset = 1: D_val is only 8-byte aligned - the bulk scatter does not apply and
-    the library must fall back by itself."""
+    the library must fall back by itself.  water_tma: long K loops - the tiled kernel runs its TMA variant."""
     import torch
     s = {"chain": lambda: gi.config(1),
          "water_ragged": lambda: gi.water_box(40, 5, seed=4, tau=1e-4, iters=8),
          "odd_cores": lambda: gi.random_banded(297, half_bw=6, n_part=9, seed=5, tau=1e-4, iters=10),
          "shuffled": lambda: gi.random_banded(300, half_bw=6, n_part=9, seed=5, tau=1e-4, iters=10, shuffle=True),
          "tiny_cores": lambda: gi.random_banded(64, half_bw=3, n_part=32, seed=7, tau=1e-4, iters=10),
-         "peptide": lambda: gi.peptide_water(40, box=20.0, seed=2)}[which]()
+         "peptide": lambda: gi.peptide_water(40, box=20.0, seed=2),
+         "water_tma": lambda: gi.water_box(384, 3, seed=8, tau=1e-5, iters=6)}[which]()
     Hd = gbe.DeviceCSR.from_host(s.H)
     part_t = torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
     g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
     info = g.info
+    if which == "water_tma":  # three communities of m ~ 2,260 (ragged last tile): the X^2 kernel with panels by 2-D TMA
+        assert info["x2_tma"] == 1 and info["max_m"] % 64 != 0
     D_ref, _ = gbe.gbe_density(Hd, g, s.n_occ, s.iters, -1.0)
     pad_ws, pad_d, sentinel = 1 << 16, 1024, 1.2345e300
     ws_big = torch.full((info["workspace_bytes"] + 2 * pad_ws,), 0xA5, dtype=torch.uint8, device="cuda")
