@@ -593,6 +593,40 @@ def test_preset_sequence_in_a_bounded_workspace(gbe, which):
     assert e.value.status == -5
 
 
+@pytest.mark.parametrize("which", ["water_ragged", "shuffled", "peptide"])
+def test_guard_bands_waves_and_fermi(gbe, which):
+    """The same guard bands (test_nothing_is_written_outside_workspace_and_d) around the SMALLEST workspace the pre-set
+    sequence accepts (waves of communities: dense offsets are shifted per wave) and around the Fermi expansion's
+    workspace (four dense batches)."""
+    import torch
+    s = {"water_ragged": lambda: gi.water_box(40, 5, seed=4, tau=1e-4, iters=8),
+         "shuffled": lambda: gi.random_banded(300, half_bw=6, n_part=9, seed=5, tau=1e-4, iters=10, shuffle=True),
+         "peptide": lambda: gi.peptide_water(40, box=20.0, seed=2)}[which]()
+    Hd = gbe.DeviceCSR.from_host(s.H)
+    part_t = torch.from_numpy(np.asarray(s.part, dtype=np.int32)).cuda()
+    g = gbe.gbe_build_graph(Hd, s.tau, part_t, s.n_part)
+    gbe.gbe_graph_set_sp2_path(g, 1)
+    info = g.info
+    pad_ws, pad_d, sentinel = 1 << 16, 1024, 1.2345e300
+    d_big = torch.full((info["nnz_D"] + 2 * pad_d,), sentinel, dtype=torch.float64, device="cuda")
+    D = d_big[pad_d:pad_d + info["nnz_D"]]
+    seq = np.array([1, 0, 0, 1, 0, 1, 1, 0], dtype=np.uint8)
+    D_ref, _ = gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False)
+    F_ref, _ = gbe.gbe_density_fermi(Hd, g, 0.0, 1.5, 21)
+    for nbytes, run, ref in (
+            (info["workspace_bytes_preset_min"],
+             lambda ws: gbe.gbe_density_preset(Hd, g, seq, trace_every_iteration=False, workspace=ws, D_val=D, want_log=False), D_ref),
+            (info["workspace_bytes_fermi"],
+             lambda ws: gbe.gbe_density_fermi(Hd, g, 0.0, 1.5, 21, workspace=ws, D_val=D, want_n_elec=False), F_ref)):
+        ws_big = torch.full((nbytes + 2 * pad_ws,), 0xA5, dtype=torch.uint8, device="cuda")
+        D.fill_(sentinel)
+        run(ws_big[pad_ws:pad_ws + nbytes])
+        torch.cuda.synchronize()
+        assert bool((ws_big[:pad_ws] == 0xA5).all()) and bool((ws_big[pad_ws + nbytes:] == 0xA5).all())
+        assert bool((d_big[:pad_d] == sentinel).all()) and bool((d_big[pad_d + info["nnz_D"]:] == sentinel).all())
+        assert torch.equal(D, ref)
+
+
 # ------------------------------------------------------------------------------- Eq.(8): graph of the next MD step
 @pytest.mark.parametrize("which", ["chain", "water"])
 def test_update_graph_eq8_md_step(gbe, which):
