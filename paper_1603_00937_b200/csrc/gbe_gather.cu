@@ -66,9 +66,15 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   };
 
   // bitmaps of the community's core and halo vertices
+  // (this thread's first two vertices are requested before the table is cleared: their latency hides behind it)
+  const int l0 = t, l1 = t + (int)blockDim.x;
+  const int v0 = l0 < m ? sub_idx[sb + l0] : 0;
+  const int v1 = l1 < m ? sub_idx[sb + l1] : 0;
   for (int w = t; w < W; w += blockDim.x) tab[w] = make_uint4(0u, 0u, 0u, 0u);
   __syncthreads();
-  for (int l = t; l < m; l += blockDim.x) {
+  if (l0 < m) atomicOr(l0 < nc ? &tab[v0 >> 5].x : &tab[v0 >> 5].y, 1u << (v0 & 31));
+  if (l1 < m) atomicOr(l1 < nc ? &tab[v1 >> 5].x : &tab[v1 >> 5].y, 1u << (v1 & 31));
+  for (int l = t + 2 * (int)blockDim.x; l < m; l += blockDim.x) {
     const int v = sub_idx[sb + l];
     atomicOr(l < nc ? &tab[v >> 5].x : &tab[v >> 5].y, 1u << (v & 31));
   }
