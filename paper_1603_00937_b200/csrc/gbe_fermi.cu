@@ -36,12 +36,11 @@ __global__ void __launch_bounds__(256) k_cheb_coef(gbe_state* st, double mu, dou
 
 // From the gathered X0 (in BX): BX <- Ht = I - 2 X0; B0 <- T_0 = I; B1 <- T_1 = Ht; BD <- c_0 I + c_1 Ht.
 // One CTA per gather work item (community, 64 rows); pad columns stay zero in all four buffers.
-__global__ void __launch_bounds__(256) k_cheb_init(int rows_per_cta, const int2* __restrict__ gitems,
+__global__ void __launch_bounds__(256) k_cheb_init(int rows_per_cta, const gbe_gitem* __restrict__ gitems,
                                                    const int64_t* __restrict__ sub_ptr, const int64_t* __restrict__ dense_off,
                                                    const gbe_state* __restrict__ st, double* __restrict__ BX,
                                                    double* __restrict__ B0, double* __restrict__ B1, double* __restrict__ BD) {
-  const int2 it = gitems[blockIdx.x];
-  const int p = it.x, r0 = it.y;
+  const int p = gitems[blockIdx.x].p, r0 = gitems[blockIdx.x].r0;
   const int m = (int)(sub_ptr[p + 1] - sub_ptr[p]);
   const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
   const int64_t off = dense_off[p];

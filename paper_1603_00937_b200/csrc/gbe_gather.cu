@@ -35,12 +35,10 @@ __device__ __forceinline__ void bulk_store_row(double* dst, const double* src_sm
 __device__ __forceinline__ void bulk_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
 template <bool DIRECT>
-__global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_per_cta, const int2* __restrict__ gitems,
+__global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_per_cta, const gbe_gitem* __restrict__ gitems,
                                                 const int64_t* __restrict__ H_rp, const int32_t* __restrict__ H_col,
                                                 const double* __restrict__ H_val, int64_t n,
-                                                const int64_t* __restrict__ sub_ptr, const int32_t* __restrict__ sub_idx,
-                                                const int32_t* __restrict__ ncore_arr,
-                                                const int64_t* __restrict__ dense_off, const gbe_state* __restrict__ st,
+                                                const int32_t* __restrict__ sub_idx, const gbe_state* __restrict__ st,
                                                 double* __restrict__ X, double* __restrict__ partials) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   uint4* tab = reinterpret_cast<uint4*>(smem_raw);                        // W x {core word, halo word, core rank, nc + halo rank}
@@ -48,11 +46,11 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   double* red = reinterpret_cast<double*>(scratch + 516);                  // 16 doubles (8-byte aligned: 4W*4 + 2064)
   double* rowbuf = red + 16;                                               // nwarps * ldmax doubles
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5, nw = blockDim.x >> 5;
-  const int2 it = gitems[blockIdx.x];
-  const int p = it.x, r0 = it.y;
-  const int64_t sb = sub_ptr[p];
-  const int m = (int)(sub_ptr[p + 1] - sb);
-  const int nc = ncore_arr[p];
+  // the work item carries the community's sizes and offsets: two 16-byte loads, then sub_idx - no chain through p
+  const int4 ia = reinterpret_cast<const int4*>(gitems)[2 * (size_t)blockIdx.x];            // p, r0, m, nc
+  const longlong2 ib = reinterpret_cast<const longlong2*>(gitems)[2 * (size_t)blockIdx.x + 1];  // sb, dense_off
+  const int r0 = ia.y, m = ia.z, nc = ia.w;
+  const int64_t sb = ib.x;
   const int ld = (m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
   // degenerate bounds (eps_max == eps_min, A-12: H is a multiple of I): the status travels with gbe_read_log; the values are
   // kept finite with delta = 1 (X0 = 0) so that a call without a log still writes a defined D
@@ -112,7 +110,7 @@ __global__ void __launch_bounds__(256, 3) k_gather(int W, int ldmax, int rows_pe
   __syncthreads();
 
   double* buf = DIRECT ? nullptr : rowbuf + (size_t)wid * ldmax;
-  double* Xp = X + dense_off[p];
+  double* Xp = X + ib.y;
   double s1 = 0.0, s2 = 0.0;
   // The row loop is latency bound (sub_idx -> H row pointers -> H entries are dependent loads), so it is software
   // pipelined: the vertex of the row after next and the row pointers of the next row are in flight while the current
@@ -247,7 +245,7 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
                       cudaStream_t s, int item0, int n_it) {
   if (n_it < 0) { item0 = 0; n_it = g->n_gitems; }
   if (n_it == 0) return GBE_OK;
-  const int2* const gitems = g->gitems + item0;
+  const gbe_gitem* const gitems = g->gitems + item0;
   partials += 2 * (size_t)item0;
   const int W = (int)((g->n + 31) / 32);
   const int ldmax = (g->max_m + GBE_LD_ALIGN - 1) / GBE_LD_ALIGN * GBE_LD_ALIGN;
@@ -263,14 +261,14 @@ int gbe_launch_gather(const gbe_csr_view& H, const gbe_graph* g, const gbe_state
     GBE_CUDA(cudaFuncSetAttribute(k_gather<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fixed));
     GBE_CUDA(cudaFuncSetAttribute(k_gather<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     k_gather<true><<<n_it, 256, fixed, s>>>(W, ldmax, g->gather_rows, gitems, H.row_ptr, H.col_idx, H.val, g->n,
-                                                   g->sub_ptr, g->sub_idx, g->ncore, g->dense_off, st, X, partials);
+                                                   g->sub_idx, st, X, partials);
   } else {
     const int nw = (int)std::min<size_t>(8, (budget - fixed) / ((size_t)ldmax * 8));
     const size_t smem = fixed + (size_t)nw * ldmax * 8;
     GBE_CUDA(cudaFuncSetAttribute(k_gather<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     GBE_CUDA(cudaFuncSetAttribute(k_gather<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     k_gather<false><<<n_it, nw * 32, smem, s>>>(W, ldmax, g->gather_rows, gitems, H.row_ptr, H.col_idx, H.val,
-                                                       g->n, g->sub_ptr, g->sub_idx, g->ncore, g->dense_off, st, X, partials);
+                                                       g->n, g->sub_idx, st, X, partials);
   }
   GBE_LAUNCHED();
   return GBE_OK;

@@ -453,10 +453,11 @@ int gbe_build_subgraphs(gbe_graph* g, const int32_t* part, cudaStream_t s, const
     // rows per gather CTA: every CTA first builds the community's index bitmaps over the n vertices (O(n / 32) words), so
     // large systems amortise that over more rows
     g->gather_rows = n <= 32768 ? 64 : (n <= 131072 ? 256 : 512);
-    static thread_local std::vector<int2> gi;
+    static thread_local std::vector<gbe_gitem> gi;
     gi.clear();
     for (int p = 0; p < n_part; ++p)
-      for (int r0 = 0; r0 < g->h_m[p]; r0 += g->gather_rows) gi.push_back(make_int2(p, r0));
+      for (int r0 = 0; r0 < g->h_m[p]; r0 += g->gather_rows)
+        gi.push_back(gbe_gitem{p, r0, g->h_m[p], g->h_ncore[p], h_sub_ptr[p], g->h_dense_off[p]});
     g->n_gitems = (int32_t)gi.size();
     GBE_TRY(upload(gi, &g->gitems, s));
   }

@@ -127,6 +127,13 @@ struct gbe_wave {  // a range of communities processed together by gbe_density_p
 // ----------------------------------------------------------------------------------------------
 // the graph handle
 // ----------------------------------------------------------------------------------------------
+// One work item of the gather (and of the Chebyshev initialisation): rows r0 .. r0 + gather_rows - 1 of community p.  It
+// carries what the CTA needs about the community, so that one 32-byte load replaces a chain of dependent ones.
+struct __align__(16) gbe_gitem {
+  int32_t p, r0, m, nc;     // community, first row, size, core size
+  int64_t sb, dense_off;    // offset of the community in sub_idx, and of its block in the dense batch
+};
+
 struct gbe_graph {
   int64_t n = 0, nnz_S = 0, sum_m = 0, nnz_D = 0, dense_elems = 0;
   int32_t n_part = 0, max_m = 0, max_ncore = 0, tile = 64;
@@ -171,7 +178,7 @@ struct gbe_graph {
   // the mirrored store, every core row and core column of X_p - all that the trace and the scatter read (Eq.(6))
   gbe_tile_item* items_last = nullptr;
   int32_t n_items_last = 0;
-  int2* gitems = nullptr;  // gather work items (p, first row)
+  gbe_gitem* gitems = nullptr;  // gather work items (community, first row, and the community's sizes and offsets)
   int32_t n_gitems = 0, gather_rows = 0;
   // device copy of the H uploaded by gbe_build_graph_host (owned; null for graphs built from device pointers)
   int64_t H_n = 0, H_nnz = 0;
