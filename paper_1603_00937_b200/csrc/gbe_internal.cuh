@@ -340,6 +340,39 @@ int gbe_exclusive_scan_i32_to_i64_max(const int32_t* in, int64_t* out, int64_t n
 // Step 5's decision (A-6, A-7), taken by ONE thread from the global traces t1, t2 of X_k, k = st->iter: the log entry,
 // the idempotency stop, the branch of iteration k (preset or chosen).  Shared by k_trace_branch and by the kernels that
 // reduce the traces themselves.
+// what gbe_trace_decide reads from the state; none of it is written by an X^2 launch, so k_trace_branch loads it BEFORE it
+// waits for the launch that writes the partials
+struct gbe_decide_in {
+  double n_occ, idem_tol;
+  int k, iters, preset, brk;
+};
+__device__ __forceinline__ gbe_decide_in gbe_trace_decide_load(const gbe_state* st) {
+  // (loads that bypass L1: the CTA may have become resident, under a programmatic dependent launch, on an SM whose L1
+  //  still holds a line of the state from an earlier launch)
+  gbe_decide_in d;
+  d.n_occ = __ldcg(&st->n_occ);
+  d.idem_tol = __ldcg(&st->idem_tol);
+  d.k = __ldcg(&st->iter);  // the partials describe X_k
+  d.iters = __ldcg(&st->iters);
+  d.preset = __ldcg(&st->preset);
+  d.brk = d.k < GBE_MAX_ITERS ? (int)__ldcg(&st->br[d.k]) : 0;
+  return d;
+}
+__device__ __forceinline__ void gbe_trace_decide(gbe_state* st, double t1, double t2, const gbe_decide_in& d) {
+  const int k = d.k;
+  st->t1[k] = t1;
+  st->t2[k] = t2;
+  st->iters_done = k;
+  if (k >= d.iters || (d.idem_tol >= 0.0 && k >= 1 && fabs(t1 - t2) <= d.idem_tol)) {
+    st->stop = 1;
+  } else {
+    const int b = d.preset ? d.brk : ((fabs(t2 - d.n_occ) < fabs(2.0 * t1 - t2 - d.n_occ)) ? 0 : 1);
+    st->branch = b;
+    st->br[k] = (uint8_t)b;
+    __threadfence();
+    st->iter = k + 1;
+  }
+}
 __device__ __forceinline__ void gbe_trace_decide(gbe_state* st, double t1, double t2) {
   const double n_occ = st->n_occ;
   const int k = st->iter;  // the partials describe X_k

@@ -19,8 +19,15 @@ __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double
   const int t = threadIdx.x;
   // programmatic dependent launch (gbe_internal.cuh): this CTA may be resident before the kernel that writes the partials
   // has finished - wait for it; the next kernel of the stream is let go at the very end, after the decision
+  // the state this kernel decides from is written by kernels of its own kind only (and before the first X^2 launch):
+  // thread 0 requests it before the wait, so that the decision costs no load after the sums
+  gbe_decide_in din = {};
+  int stopped = 0;
+  if (t == 0) {
+    din = gbe_trace_decide_load(st);
+    stopped = __ldcg(&st->stop);
+  }
   gbe_griddep_wait();
-  const int stopped = st->stop;  // read now, tested after the sums: the loads below need not wait for it
   // the kernel is one CTA and latency bound: 8 independent 16-byte loads in flight per thread, summed in a fixed order
   double a1 = 0.0, a2 = 0.0;
   const double2* __restrict__ p2 = reinterpret_cast<const double2*>(partials);
@@ -41,7 +48,7 @@ __global__ void __launch_bounds__(TB) k_trace_branch(gbe_state* st, const double
     a2 = warp_sum(s2[t]);
   }
   if (t == 0) {
-    if (!stopped) gbe_trace_decide(st, a1, a2);
+    if (!stopped) gbe_trace_decide(st, a1, a2, din);
     // the X^2 launch behind this kernel (launched with the attribute) never waits: it may start only now, when X_{n+1}
     // is complete (the wait above) and the decision is visible device-wide
     __threadfence();
